@@ -1,0 +1,160 @@
+/*
+ * bloch.h -- C ABI of libbloch_b200: the spin-parallel Bloch-equation solve of KomaMRI (arxiv 2301.02702)
+ * as hand-written CUDA for sm_100a.
+ *
+ * The calls follow the paper's problem statement (Fig 3 :188): scanner parameters +
+ * phantom + sequence (+ simulation parameters) in; raw complex signal per ADC sample, and optionally the
+ * final magnetisation, out.  No torch types, no C++ types, no exceptions across this boundary.
+ *
+ * Conventions
+ *   - SI units: position [m], gradient [T/m], B1 [T], off-resonance [rad/s], time [s], gamma [rad/s/T].
+ *   - Every function returns 0 (BLOCH_OK) or a negative bloch_status; bloch_last_error() gives thread-local
+ *     detail text.  Nothing is printed, nothing aborts.
+ *   - "h_" pointers are HOST memory, "d_" pointers are DEVICE memory of the current CUDA device.
+ *   - The library never allocates device memory: tables, workspace and all spin / signal buffers are
+ *     caller-owned (in this repo: torch tensors).  Host arrays passed to bloch_plan_create are borrowed
+ *     for the duration of that call only.
+ *   - `stream` arguments are a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - Complex values are interleaved (re, im) fp32 pairs.
+ */
+#ifndef BLOCH_B200_H
+#define BLOCH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BLOCH_OK = 0,
+    BLOCH_EINVAL = -1,         /* NULL pointer, negative size, non-finite value, bad enum */
+    BLOCH_ENONMONOTONIC = -2,  /* gradient vertex / RF sample / ADC times not ascending, or RF samples overlap */
+    BLOCH_EADC_IN_RF = -3,     /* an ADC time lies strictly inside an RF-active run (reading G7) */
+    BLOCH_EWORKSPACE = -4,     /* workspace / table buffer too small or misaligned (256 B) */
+    BLOCH_ECUDA = -5,          /* a CUDA runtime call failed; text in bloch_last_error() */
+    BLOCH_EARCH = -6,          /* current device is not compute capability 10.x */
+    BLOCH_ENOTUPLOADED = -7,   /* bloch_simulate before bloch_plan_upload */
+    BLOCH_ENOMEM = -8          /* host allocation failed */
+} bloch_status;
+
+enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
+enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1 };
+
+/* Scanner.  Only gamma enters the arithmetic (Eq 1-2, :105-114); B0, G_max, S_max are
+ * carried for completeness and are not validated against.  gamma <= 0 selects 2*pi*42.58e6 (:322). */
+typedef struct {
+    double gamma;
+    double B0;
+    double G_max;
+    double S_max;
+} bloch_scanner;
+
+/* Sequence: G(t) piecewise linear through per-axis vertices (G = 0 outside the vertex range,
+ * :180), complex B1(t) piecewise constant on [rf_t, rf_t + rf_dt) (:182), ADC sample times.  All times in
+ * [0, t_end], each array strictly ascending; RF samples may abut but not overlap. */
+typedef struct {
+    const double *g_t[3];
+    const double *g_v[3];
+    int64_t g_n[3];
+    const double *rf_t;
+    const double *rf_dt;
+    const double *rf_re;
+    const double *rf_im;
+    int64_t rf_n;
+    const double *adc_t;
+    int64_t adc_n;
+    double t_end;
+} bloch_sequence;
+
+/* simParams.  dt_rf_max: RF sample pieces longer than this are cut into equal sub-steps
+ * (the paper's dt_rf, :182).  dt_max: spacing of extra points in RF-free intervals; only needed with
+ * motion (:180), accepted and ignored (<= 0 or inf).  max_block_points: precession blocks hold at most
+ * this many evaluated points (the paper's Nblocks memory bound, :171); <= 0 selects the default. */
+typedef struct {
+    double dt_max;
+    double dt_rf_max;
+    int64_t max_block_points;
+    int32_t phase_mode;   /* BLOCH_PHASE_* */
+    int32_t output_mode;  /* BLOCH_OUT_*   */
+} bloch_sim_params;
+
+typedef struct {
+    int64_t n_intervals;     /* intervals of the merged, refined time grid (what a step-by-step solver runs) */
+    int64_t n_rf_steps;      /* RF-active intervals */
+    int64_t n_adc;           /* ADC samples */
+    int64_t n_blocks;        /* excitation + precession blocks */
+    int64_t n_rf_blocks;
+    int64_t n_eval_points;   /* precession evaluations per spin: ADC samples + block ends */
+    int64_t n_launches;      /* kernels one bloch_simulate enqueues for this plan (SUM_ALL, final state on) */
+    int64_t table_bytes;     /* size of the device table buffer bloch_plan_upload needs */
+    int64_t max_block_adc;   /* largest number of ADC samples in one precession block */
+    int32_t phase_mode;      /* resolved: BLOCH_PHASE_FP32 or BLOCH_PHASE_FP64 */
+    int32_t output_mode;
+} bloch_plan_info;
+
+typedef struct bloch_plan bloch_plan;
+
+int bloch_version(void);
+const char *bloch_strerror(int code);
+const char *bloch_last_error(void);
+
+/* Host only: merge the time grid, interpolate G, classify intervals into excitation
+ * / precession blocks (:132, :171), precompute per precession block the spin-independent cumulative
+ * gradient moment k(t) by the trapezoidal rule on the vertices (Eq 12-13, :173-180) and per RF step the
+ * rotation-vector table.  *out is owned by the library until bloch_plan_destroy. */
+int bloch_plan_create(const bloch_scanner *scanner, const bloch_sequence *seq,
+                      const bloch_sim_params *params, bloch_plan **out);
+int bloch_plan_destroy(bloch_plan *plan);
+int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out);
+
+/* Bytes of caller-allocated device workspace bloch_simulate needs for n_spins (256-B aligned buffer). */
+int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out);
+
+/* Copy the plan's tables into d_tables (>= table_bytes, 256-B aligned, caller keeps it alive until the
+ * plan is destroyed or re-uploaded).  Asynchronous on `stream`; the host staging copy is owned by the plan. */
+int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stream);
+
+/* Run the whole sequence for n_spins spins (device pointers, fp32 SoA arrays of n_spins each).
+ *   d_Mxy (2*n_spins floats, interleaved) / d_Mz: if init_equilibrium == 0 they hold the initial state
+ *       (both required); if non-NULL they receive the final magnetisation.  With init_equilibrium != 0
+ *       the state starts at Mxy = 0, Mz = M0 (reading G8).
+ *   d_signal: SUM_ALL: n_adc complex, S[j] = sum over spins of Mxy at ADC sample j;
+ *             PER_SPIN: n_spins x n_adc complex, row-major [spin][adc].
+ *   Asynchronous on `stream`: no hidden synchronisation, no allocation, no host copies.  The result is
+ *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 (not checked). */
+int bloch_simulate(const bloch_plan *plan, int64_t n_spins,
+                   const float *d_x, const float *d_y, const float *d_z, const float *d_M0,
+                   const float *d_T1, const float *d_T2, const float *d_dw,
+                   float *d_Mxy, float *d_Mz, int init_equilibrium,
+                   float *d_signal, void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Same computation with HOST buffers (pageable or pinned): copies the seven phantom arrays (and the initial
+ * state, if any) to the device, runs bloch_simulate, copies the signal (and final state, if requested)
+ * back and synchronises `stream` before returning.  d_scratch is caller-allocated device memory of at
+ * least bloch_simulate_host_scratch_bytes(); the tables must have been uploaded. */
+int bloch_simulate_host_scratch_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out);
+int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins,
+                        const float *h_x, const float *h_y, const float *h_z, const float *h_M0,
+                        const float *h_T1, const float *h_T2, const float *h_dw,
+                        float *h_Mxy, float *h_Mz, int init_equilibrium,
+                        float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
+
+/* Timing taps for the benchmark: after a bloch_simulate on `stream` has been synchronised by the caller,
+ * returns the device time (ms, CUDA events recorded on `stream`) spent in the RF kernels, in the
+ * free-precession signal kernels (+ their reductions) and in total, and the number of kernels launched.
+ * Enabled with bloch_plan_set_profiling(plan, 1); off by default (no events are recorded). */
+int bloch_plan_set_profiling(bloch_plan *plan, int enable);
+int bloch_plan_last_timing(const bloch_plan *plan, float *ms_rf, float *ms_precession, float *ms_total,
+                           int64_t *n_launches);
+
+/* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
+ * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA, 2 = DFMA.  Runs `iters` dependent-chain iterations with 8
+ * independent chains per thread on all SMs at full occupancy and returns operations per second. */
+int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLOCH_B200_H */

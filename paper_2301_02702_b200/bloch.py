@@ -1,0 +1,288 @@
+"""Thin ctypes binding of libbloch_b200.so (include/bloch.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels / host planner.  PyTorch is used for
+device memory and streams only.  There is NO CPU fallback: importing this module without the built
+extension raises, and nothing here imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libbloch_b200.so")
+
+PHASE_AUTO, PHASE_FP32, PHASE_FP64 = 0, 1, 2
+OUT_SUM_ALL, OUT_PER_SPIN = 0, 1
+_PHASE = {"auto": PHASE_AUTO, "fp32": PHASE_FP32, "fp64": PHASE_FP64}
+_OUT = {"sum": OUT_SUM_ALL, "per_spin": OUT_PER_SPIN}
+
+_dp = C.POINTER(C.c_double)
+_fp = C.c_void_p  # float* (host or device) passed as an address
+
+
+class bloch_scanner(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("B0", C.c_double), ("G_max", C.c_double), ("S_max", C.c_double)]
+
+
+class bloch_sequence(C.Structure):
+    _fields_ = [("g_t", _dp * 3), ("g_v", _dp * 3), ("g_n", C.c_int64 * 3),
+                ("rf_t", _dp), ("rf_dt", _dp), ("rf_re", _dp), ("rf_im", _dp), ("rf_n", C.c_int64),
+                ("adc_t", _dp), ("adc_n", C.c_int64), ("t_end", C.c_double)]
+
+
+class bloch_sim_params(C.Structure):
+    _fields_ = [("dt_max", C.c_double), ("dt_rf_max", C.c_double), ("max_block_points", C.c_int64),
+                ("phase_mode", C.c_int32), ("output_mode", C.c_int32)]
+
+
+class bloch_plan_info(C.Structure):
+    _fields_ = [("n_intervals", C.c_int64), ("n_rf_steps", C.c_int64), ("n_adc", C.c_int64),
+                ("n_blocks", C.c_int64), ("n_rf_blocks", C.c_int64), ("n_eval_points", C.c_int64),
+                ("n_launches", C.c_int64), ("table_bytes", C.c_int64), ("max_block_adc", C.c_int64),
+                ("phase_mode", C.c_int32), ("output_mode", C.c_int32)]
+
+
+EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",
+           "bloch_plan_get_info", "bloch_plan_workspace_bytes", "bloch_plan_upload", "bloch_simulate",
+           "bloch_simulate_host_scratch_bytes", "bloch_simulate_host", "bloch_plan_set_profiling",
+           "bloch_plan_last_timing", "bloch_microbench"]
+
+
+def _load():
+    if not os.path.exists(_SO):
+        raise ImportError(f"{_SO} is missing: build it with `python -m paper_2301_02702_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(_SO)
+    vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
+    lib.bloch_version.restype = C.c_int
+    lib.bloch_strerror.restype = C.c_char_p
+    lib.bloch_strerror.argtypes = [C.c_int]
+    lib.bloch_last_error.restype = C.c_char_p
+    lib.bloch_plan_create.argtypes = [C.POINTER(bloch_scanner), C.POINTER(bloch_sequence),
+                                      C.POINTER(bloch_sim_params), C.POINTER(vp)]
+    lib.bloch_plan_destroy.argtypes = [vp]
+    lib.bloch_plan_get_info.argtypes = [vp, C.POINTER(bloch_plan_info)]
+    lib.bloch_plan_workspace_bytes.argtypes = [vp, i64, C.POINTER(sz)]
+    lib.bloch_plan_upload.argtypes = [vp, vp, sz, vp]
+    sim_args = [vp, i64] + [_fp] * 7 + [_fp, _fp, C.c_int, _fp, vp, sz, vp]
+    lib.bloch_simulate.argtypes = sim_args
+    lib.bloch_simulate_host_scratch_bytes.argtypes = [vp, i64, C.POINTER(sz)]
+    lib.bloch_simulate_host.argtypes = sim_args
+    lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
+    lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float),
+                                           C.POINTER(C.c_float), C.POINTER(i64)]
+    lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
+    for name in EXPORTS:
+        if name not in ("bloch_strerror", "bloch_last_error"):
+            getattr(lib, name).restype = C.c_int
+    return lib
+
+
+_lib = _load()
+
+
+class BlochError(RuntimeError):
+    def __init__(self, code: int):
+        self.code = code
+        detail = _lib.bloch_last_error().decode()
+        super().__init__(f"{_lib.bloch_strerror(code).decode()} ({code}): {detail}")
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise BlochError(rc)
+
+
+# ---- same-name wrappers (marshalling only) ------------------------------------------------------
+def bloch_version() -> int:
+    return _lib.bloch_version()
+
+
+def bloch_strerror(code: int) -> str:
+    return _lib.bloch_strerror(code).decode()
+
+
+def bloch_last_error() -> str:
+    return _lib.bloch_last_error().decode()
+
+
+def _darr(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
+                      max_block_points: int = 0, phase_mode="auto", output_mode="sum") -> int:
+    """seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
+    Returns the opaque plan handle (an integer address)."""
+    keep = []
+    cs = bloch_sequence()
+    for a in range(3):
+        t, tp = _darr(seq.g_t[a]); v, vp_ = _darr(seq.g_v[a])
+        if t.shape != v.shape:
+            raise ValueError("g_t / g_v length mismatch")
+        keep += [t, v]
+        cs.g_t[a], cs.g_v[a], cs.g_n[a] = tp, vp_, t.shape[0]
+    rt, cs.rf_t = _darr(seq.rf_t); rd, cs.rf_dt = _darr(seq.rf_dt)
+    rr, cs.rf_re = _darr(seq.rf_re); ri, cs.rf_im = _darr(seq.rf_im)
+    if not (rt.shape == rd.shape == rr.shape == ri.shape):
+        raise ValueError("RF array length mismatch")
+    ad, cs.adc_t = _darr(seq.adc_t)
+    keep += [rt, rd, rr, ri, ad]
+    cs.rf_n, cs.adc_n, cs.t_end = rt.shape[0], ad.shape[0], float(seq.t_end)
+    if dt_rf_max is None:
+        dt_rf_max = float(getattr(seq, "dt_rf_max", 0.0))
+    sc = bloch_scanner(float(gamma), 0.0, 0.0, 0.0)
+    pm = _PHASE[phase_mode] if isinstance(phase_mode, str) else int(phase_mode)
+    om = _OUT[output_mode] if isinstance(output_mode, str) else int(output_mode)
+    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om)
+    h = C.c_void_p()
+    _check(_lib.bloch_plan_create(C.byref(sc), C.byref(cs), C.byref(sp), C.byref(h)))
+    return h.value
+
+
+def bloch_plan_destroy(plan: int):
+    _check(_lib.bloch_plan_destroy(plan))
+
+
+def bloch_plan_get_info(plan: int) -> dict:
+    inf = bloch_plan_info()
+    _check(_lib.bloch_plan_get_info(plan, C.byref(inf)))
+    return {k: int(getattr(inf, k)) for k, _ in bloch_plan_info._fields_}
+
+
+def bloch_plan_workspace_bytes(plan: int, n_spins: int) -> int:
+    out = C.c_size_t()
+    _check(_lib.bloch_plan_workspace_bytes(plan, n_spins, C.byref(out)))
+    return int(out.value)
+
+
+def bloch_plan_upload(plan: int, d_tables_ptr: int, nbytes: int, stream: int = 0):
+    _check(_lib.bloch_plan_upload(plan, d_tables_ptr, nbytes, stream))
+
+
+def bloch_simulate(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, Mxy, Mz, init_equilibrium: bool,
+                   signal, workspace, workspace_bytes: int, stream: int = 0):
+    """All array arguments are raw DEVICE addresses (ints) or None."""
+    _check(_lib.bloch_simulate(plan, n_spins, x, y, z, M0, T1, T2, dw, Mxy, Mz, int(bool(init_equilibrium)),
+                               signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_host_scratch_bytes(plan: int, n_spins: int) -> int:
+    out = C.c_size_t()
+    _check(_lib.bloch_simulate_host_scratch_bytes(plan, n_spins, C.byref(out)))
+    return int(out.value)
+
+
+def bloch_simulate_host(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, Mxy, Mz, init_equilibrium: bool,
+                        signal, scratch, scratch_bytes: int, stream: int = 0):
+    """Phantom / state / signal arguments are raw HOST addresses (ints) or None; scratch is a device address."""
+    _check(_lib.bloch_simulate_host(plan, n_spins, x, y, z, M0, T1, T2, dw, Mxy, Mz,
+                                    int(bool(init_equilibrium)), signal, scratch, scratch_bytes, stream))
+
+
+def bloch_plan_set_profiling(plan: int, enable: bool):
+    _check(_lib.bloch_plan_set_profiling(plan, int(bool(enable))))
+
+
+def bloch_plan_last_timing(plan: int) -> dict:
+    a, b, c, n = C.c_float(), C.c_float(), C.c_float(), C.c_int64()
+    _check(_lib.bloch_plan_last_timing(plan, C.byref(a), C.byref(b), C.byref(c), C.byref(n)))
+    return {"ms_rf": a.value, "ms_precession": b.value, "ms_total": c.value, "launches": int(n.value)}
+
+
+def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:
+    out = C.c_double()
+    _check(_lib.bloch_microbench(kind, iters, C.byref(out), stream))
+    return float(out.value)
+
+
+# ---- convenience object: owns the handle and the torch buffers ------------------------------------
+class Plan:
+    """Owns a bloch_plan handle plus the caller-side device buffers (torch tensors)."""
+
+    def __init__(self, seq, **kw):
+        self.handle = bloch_plan_create(seq, **kw)
+        self.info = bloch_plan_get_info(self.handle)
+        self._tables = None
+        self._ws = None
+        self._scratch = None
+
+    def close(self):
+        if getattr(self, "handle", None):
+            bloch_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @staticmethod
+    def _stream():
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+
+    def upload(self):
+        import torch
+        self._tables = torch.empty(max(self.info["table_bytes"], 256), dtype=torch.uint8, device="cuda")
+        bloch_plan_upload(self.handle, self._tables.data_ptr(), self._tables.numel(), self._stream())
+        return self
+
+    def _workspace(self, n):
+        import torch
+        need = max(bloch_plan_workspace_bytes(self.handle, n), 256)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        return self._ws
+
+    def simulate(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None):
+        """Device path: torch float32 CUDA tensors in, complex64 signal tensor out (asynchronous)."""
+        import torch
+        if self._tables is None:
+            self.upload()
+        n = int(x.numel())
+        for t in (x, y, z, M0, T1, T2, dw):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
+        n_adc = self.info["n_adc"]
+        shape = (n, n_adc) if self.info["output_mode"] == OUT_PER_SPIN else (n_adc,)
+        if signal is None:
+            signal = torch.empty(shape, dtype=torch.complex64, device="cuda")
+        ws = self._workspace(n)
+        bloch_simulate(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(), T1.data_ptr(),
+                       T2.data_ptr(), dw.data_ptr(),
+                       None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
+                       init_equilibrium, signal.data_ptr() if signal.numel() else None,
+                       ws.data_ptr(), ws.numel(), self._stream())
+        return signal
+
+    def simulate_host(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None):
+        """End-to-end path: numpy float32 HOST arrays in, numpy complex64 signal out (synchronous)."""
+        import torch
+        if self._tables is None:
+            self.upload()
+        arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (x, y, z, M0, T1, T2, dw)]
+        n = int(arrs[0].shape[0])
+        n_adc = self.info["n_adc"]
+        shape = (n, n_adc) if self.info["output_mode"] == OUT_PER_SPIN else (n_adc,)
+        if signal is None:
+            signal = np.empty(shape, dtype=np.complex64)
+        need = max(bloch_simulate_host_scratch_bytes(self.handle, n), 256)
+        if self._scratch is None or self._scratch.numel() < need:
+            self._scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
+        bloch_simulate_host(self.handle, n, *[a.ctypes.data for a in arrs],
+                            None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
+                            init_equilibrium, signal.ctypes.data if signal.size else None,
+                            self._scratch.data_ptr(), self._scratch.numel(), self._stream())
+        return signal
+
+
+def phantom_to_device(ph):
+    """Phantom (fp64 numpy, fp32-exact values) -> tuple of 7 float32 CUDA tensors."""
+    import torch
+    return tuple(torch.from_numpy(np.ascontiguousarray(getattr(ph, k), dtype=np.float32)).cuda()
+                 for k in ("x", "y", "z", "M0", "T1", "T2", "dw"))

@@ -1,0 +1,457 @@
+// api.cu -- C-ABI entry points of libbloch_b200 (include/bloch.h) and the per-block launch logic.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "internal.h"
+#include "kernels.cuh"
+
+namespace bloch {
+const char *last_error_cstr();
+
+namespace {
+
+int cuda_fail(cudaError_t e, const char *what) {
+    return fail(BLOCH_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define BLOCH_CUDA(call)                                         \
+    do {                                                         \
+        cudaError_t e_ = (call);                                 \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);      \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int env_int(const char *name, int dflt) {
+    const char *v = std::getenv(name);
+    return (v && *v) ? std::atoi(v) : dflt;
+}
+
+int check_arch() {
+    int dev = 0;
+    BLOCH_CUDA(cudaGetDevice(&dev));
+    int major = 0;
+    BLOCH_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(BLOCH_EARCH, "device is not compute capability 10.x (built for sm_100a only)");
+    return BLOCH_OK;
+}
+
+// Signal-kernel launch shape for a block with n_pts evaluated points.
+struct SigShape {
+    int P;
+    int ptiles;
+    int chunks;
+    int spins_per_chunk;
+};
+
+SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
+    SigShape s;
+    const int forceP = env_int("BLOCH_SIGNAL_P", 0);
+    s.P = forceP ? forceP : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1));
+    if (s.P != 1 && s.P != 2 && s.P != 4) s.P = 1;
+    s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
+    const int per_sm = env_int("BLOCH_SIGNAL_CTAS_PER_SM", 2);
+    const int64_t target = (int64_t)sm_count * per_sm;
+    int64_t chunks = (target + s.ptiles - 1) / s.ptiles;
+    const int64_t max_chunks = (n_spins + 31) / 32;
+    if (chunks > max_chunks) chunks = max_chunks;
+    if (chunks < 1) chunks = 1;
+    if (chunks > 65535) chunks = 65535;
+    s.spins_per_chunk = (int)((n_spins + chunks - 1) / chunks);
+    s.chunks = (int)((n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
+    return s;
+}
+
+int max_chunks_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+    // upper bound over the plan's blocks; partial buffer is sized with it
+    int64_t worst = 1;
+    for (const Block &b : plan->blocks) {
+        if (b.type != kBlockPrecession || b.adc_count == 0) continue;
+        const SigShape s = sig_shape(b.adc_count, n_spins, sm_count);
+        worst = std::max<int64_t>(worst, (int64_t)s.chunks * b.adc_count);
+    }
+    return (int)std::min<int64_t>(worst, INT32_MAX);
+}
+
+struct Workspace {
+    float4 *A, *C, *S;
+    float2 *partial;
+    size_t bytes;
+};
+
+int sm_count_cached() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    }
+    return sms;
+}
+
+// Layout of the caller's workspace.  sm_count = 148 is used for sizing when no device is present so that
+// bloch_plan_workspace_bytes is a pure host function.
+Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_count) {
+    Workspace w{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        void *p = base ? (void *)((unsigned char *)base + off) : nullptr;
+        off = align_up(off + bytes, kAlign);
+        return p;
+    };
+    w.A = (float4 *)take(size_t(n_spins) * sizeof(float4));
+    w.C = (float4 *)take(size_t(n_spins) * sizeof(float4));
+    w.S = (float4 *)take(size_t(n_spins) * sizeof(float4));
+    size_t pbytes = kAlign;
+    if (plan->info.output_mode == BLOCH_OUT_SUM_ALL)
+        pbytes = size_t(max_chunks_for(plan, n_spins, sm_count)) * sizeof(float2);
+    w.partial = (float2 *)take(pbytes);
+    w.bytes = off;
+    return w;
+}
+
+struct Taps {
+    const bloch_plan *plan;
+    cudaStream_t stream;
+    size_t used = 0;
+    int mark(int kind) {
+        if (!plan->profiling) return BLOCH_OK;
+        if (used == plan->events.size()) {
+            cudaEvent_t e;
+            BLOCH_CUDA(cudaEventCreate(&e));
+            plan->events.push_back((void *)e);
+        }
+        BLOCH_CUDA(cudaEventRecord((cudaEvent_t)plan->events[used], stream));
+        if (plan->event_kind.size() <= used) plan->event_kind.resize(used + 1);
+        plan->event_kind[used] = kind;
+        ++used;
+        return BLOCH_OK;
+    }
+};
+
+}  // namespace
+}  // namespace bloch
+
+using namespace bloch;
+
+extern "C" {
+
+int bloch_version(void) { return 100; }
+
+const char *bloch_strerror(int code) {
+    switch (code) {
+        case BLOCH_OK: return "ok";
+        case BLOCH_EINVAL: return "invalid argument";
+        case BLOCH_ENONMONOTONIC: return "times not ascending or RF samples overlap";
+        case BLOCH_EADC_IN_RF: return "ADC sample inside an RF-active run";
+        case BLOCH_EWORKSPACE: return "workspace or table buffer too small or misaligned";
+        case BLOCH_ECUDA: return "CUDA runtime error";
+        case BLOCH_EARCH: return "device is not sm_100";
+        case BLOCH_ENOTUPLOADED: return "tables not uploaded";
+        case BLOCH_ENOMEM: return "host allocation failed";
+        default: return "unknown error";
+    }
+}
+
+const char *bloch_last_error(void) { return bloch::last_error_cstr(); }
+
+int bloch_plan_create(const bloch_scanner *scanner, const bloch_sequence *seq, const bloch_sim_params *params,
+                      bloch_plan **out) {
+    if (!out) return fail(BLOCH_EINVAL, "out is NULL");
+    *out = nullptr;
+    bloch_plan *p = new (std::nothrow) bloch_plan();
+    if (!p) return fail(BLOCH_ENOMEM, "plan allocation failed");
+    int rc;
+    try {
+        rc = build_plan(scanner, seq, params, p);
+    } catch (const std::bad_alloc &) {
+        rc = fail(BLOCH_ENOMEM, "host allocation failed while planning");
+    } catch (...) {
+        rc = fail(BLOCH_EINVAL, "unexpected exception while planning");
+    }
+    if (rc != BLOCH_OK) {
+        delete p;
+        return rc;
+    }
+    *out = p;
+    return BLOCH_OK;
+}
+
+int bloch_plan_destroy(bloch_plan *plan) {
+    if (!plan) return BLOCH_OK;
+    for (void *e : plan->events) cudaEventDestroy((cudaEvent_t)e);
+    delete plan;
+    return BLOCH_OK;
+}
+
+int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out) {
+    if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
+    *out = plan->info;
+    return BLOCH_OK;
+}
+
+int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out) {
+    if (!plan || !out || n_spins < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative n_spins");
+    if (n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins exceeds 2^31-1");
+    // sized for the larger of the real SM count and 148 so the answer is usable without a device
+    int sms = 148;
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > sms) sms = v;
+    } else {
+        (void)cudaGetLastError();
+    }
+    *out = carve(plan, n_spins, nullptr, sms).bytes;
+    return BLOCH_OK;
+}
+
+int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stream) {
+    if (!plan || !d_tables) return fail(BLOCH_EINVAL, "NULL argument");
+    if (bytes < plan->tables.size() || (reinterpret_cast<uintptr_t>(d_tables) % kAlign) != 0)
+        return fail(BLOCH_EWORKSPACE, "table buffer too small or not 256-B aligned");
+    BLOCH_CUDA(cudaMemcpyAsync(d_tables, plan->tables.data(), plan->tables.size(), cudaMemcpyHostToDevice,
+                               (cudaStream_t)stream));
+    plan->d_tables = (const unsigned char *)d_tables;
+    return BLOCH_OK;
+}
+
+int bloch_plan_set_profiling(bloch_plan *plan, int enable) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    plan->profiling = enable != 0;
+    return BLOCH_OK;
+}
+
+int bloch_plan_last_timing(const bloch_plan *plan, float *ms_rf, float *ms_prec, float *ms_total,
+                           int64_t *n_launches) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    Timing t{};
+    t.launches = plan->last.launches;
+    const size_t n = plan->event_kind.size();
+    for (size_t k = 0; k + 1 < n; ++k) {
+        float ms = 0.f;
+        BLOCH_CUDA(cudaEventElapsedTime(&ms, (cudaEvent_t)plan->events[k], (cudaEvent_t)plan->events[k + 1]));
+        if (plan->event_kind[k] == 1) t.ms_rf += ms;
+        else if (plan->event_kind[k] == 2) t.ms_prec += ms;
+        t.ms_total += ms;
+    }
+    if (ms_rf) *ms_rf = t.ms_rf;
+    if (ms_prec) *ms_prec = t.ms_prec;
+    if (ms_total) *ms_total = t.ms_total;
+    if (n_launches) *n_launches = t.launches;
+    return BLOCH_OK;
+}
+
+int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                   const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                   const float *d_dw, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                   void *d_workspace, size_t workspace_bytes, void *stream_) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    if (n_spins < 0 || n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins out of range");
+    if (!plan->d_tables) return fail(BLOCH_ENOTUPLOADED, "call bloch_plan_upload first");
+    if (n_spins > 0 && (!d_x || !d_y || !d_z || !d_M0 || !d_T1 || !d_T2 || !d_dw))
+        return fail(BLOCH_EINVAL, "NULL phantom array");
+    if (!init_equilibrium && (!d_Mxy || !d_Mz)) return fail(BLOCH_EINVAL, "initial state requested but d_Mxy/d_Mz NULL");
+    if ((d_Mxy == nullptr) != (d_Mz == nullptr)) return fail(BLOCH_EINVAL, "d_Mxy and d_Mz must both be given or both NULL");
+    if (plan->info.n_adc > 0 && !d_signal) return fail(BLOCH_EINVAL, "d_signal is NULL");
+    int rc = check_arch();
+    if (rc != BLOCH_OK) return rc;
+    const int sms = sm_count_cached();
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const bool per_spin = plan->info.output_mode == BLOCH_OUT_PER_SPIN;
+    const bool ph64 = plan->info.phase_mode == BLOCH_PHASE_FP64;
+
+    if (n_spins == 0) {  // degenerate: the sum over no spins is zero
+        if (!per_spin && plan->info.n_adc > 0)
+            BLOCH_CUDA(cudaMemsetAsync(d_signal, 0, size_t(plan->info.n_adc) * sizeof(float2), stream));
+        return BLOCH_OK;
+    }
+    if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) != 0)
+        return fail(BLOCH_EWORKSPACE, "workspace NULL or not 256-B aligned");
+    const Workspace w = carve(plan, n_spins, d_workspace, sms);
+    if (workspace_bytes < w.bytes) return fail(BLOCH_EWORKSPACE, "workspace too small; see bloch_plan_workspace_bytes");
+
+    const int n = (int)n_spins;
+    Taps taps{plan, stream};
+    int64_t launches = 0;
+    rc = taps.mark(0);
+    if (rc) return rc;
+    pack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw,
+                                                     (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
+                                                     w.A, w.C, w.S);
+    ++launches;
+
+    bool pending = false;
+    PropRec prop{0, 0, 0, 0};
+    const int rf_grid = (n + kRfThreads - 1) / kRfThreads;
+    for (const Block &b : plan->blocks) {
+        if (b.type == kBlockRF) {
+            if ((rc = taps.mark(1))) return rc;
+            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>((const float4 *)(plan->d_tables + b.table_off),
+                                                           (int)b.count, prop, pending ? 1 : 0, w.A, w.C, w.S, n);
+            ++launches;
+            pending = false;
+            continue;
+        }
+        if (pending) {  // two precession blocks in a row: apply the first one's end transform now
+            if ((rc = taps.mark(2))) return rc;
+            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            ++launches;
+            pending = false;
+        }
+        if (b.adc_count > 0) {
+            if ((rc = taps.mark(2))) return rc;
+            const void *recs = plan->d_tables + b.table_off;
+            const int n_pts = (int)b.adc_count;
+            if (per_spin) {
+                const long long total = (long long)n * n_pts;
+                const unsigned grid = (unsigned)((total + 255) / 256);
+                if (ph64)
+                    perspin_kernel<true><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, n,
+                                                                   (long long)plan->info.n_adc, (long long)b.adc_first,
+                                                                   (float2 *)d_signal);
+                else
+                    perspin_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, n,
+                                                                    (long long)plan->info.n_adc, (long long)b.adc_first,
+                                                                    (float2 *)d_signal);
+                ++launches;
+            } else {
+                const SigShape s = sig_shape(n_pts, n, sms);
+                const dim3 grid(s.ptiles, s.chunks);
+#define BLOCH_LAUNCH_SIG(PP)                                                                                   \
+    do {                                                                                                       \
+        if (ph64)                                                                                              \
+            signal_kernel_f64<PP><<<grid, kSigThreads, 0, stream>>>((const double4 *)recs, n_pts, w.A, w.C,    \
+                                                                    w.S, n, s.spins_per_chunk, w.partial);     \
+        else                                                                                                   \
+            signal_kernel_f32<PP><<<grid, kSigThreads, 0, stream>>>((const float4 *)recs, n_pts, w.A, w.S, n,  \
+                                                                    s.spins_per_chunk, w.partial);             \
+    } while (0)
+                if (s.P == 4) BLOCH_LAUNCH_SIG(4);
+                else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
+                else BLOCH_LAUNCH_SIG(1);
+#undef BLOCH_LAUNCH_SIG
+                reduce_kernel<<<(n_pts + 31) / 32, dim3(32, 8), 0, stream>>>(w.partial, s.chunks, n_pts,
+                                                                            (float2 *)d_signal + b.adc_first);
+                launches += 2;
+            }
+        }
+        prop.kx = b.kend[0];
+        prop.ky = b.kend[1];
+        prop.kz = b.kend[2];
+        prop.tau = b.tau_end;
+        pending = true;
+    }
+    if (d_Mxy) {
+        if ((rc = taps.mark(0))) return rc;
+        if (pending) {
+            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            ++launches;
+        }
+        unpack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, w.S, (float2 *)d_Mxy, d_Mz);
+        ++launches;
+    }
+    if ((rc = taps.mark(0))) return rc;
+    if (plan->profiling) plan->event_kind.resize(taps.used);
+    plan->last.launches = launches;
+    BLOCH_CUDA(cudaGetLastError());
+    return BLOCH_OK;
+}
+
+int bloch_simulate_host_scratch_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out) {
+    if (!plan || !out || n_spins < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative n_spins");
+    size_t ws = 0;
+    int rc = bloch_plan_workspace_bytes(plan, n_spins, &ws);
+    if (rc) return rc;
+    const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
+    const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
+                           ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
+                           : size_t(plan->info.n_adc) * sizeof(float2);
+    *out = 10 * arr + align_up(sig, kAlign) + ws + kAlign;
+    return BLOCH_OK;
+}
+
+int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                        const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                        const float *h_dw, float *h_Mxy, float *h_Mz, int init_equilibrium, float *h_signal,
+                        void *d_scratch, size_t scratch_bytes, void *stream_) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    size_t need = 0;
+    int rc = bloch_simulate_host_scratch_bytes(plan, n_spins, &need);
+    if (rc) return rc;
+    if (!d_scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(d_scratch) % kAlign) != 0)
+        return fail(BLOCH_EWORKSPACE, "scratch NULL, too small or not 256-B aligned");
+    if (n_spins > 0 && (!h_x || !h_y || !h_z || !h_M0 || !h_T1 || !h_T2 || !h_dw))
+        return fail(BLOCH_EINVAL, "NULL phantom array");
+    if (!init_equilibrium && (!h_Mxy || !h_Mz)) return fail(BLOCH_EINVAL, "initial state requested but h_Mxy/h_Mz NULL");
+    if ((h_Mxy == nullptr) != (h_Mz == nullptr)) return fail(BLOCH_EINVAL, "h_Mxy and h_Mz must both be given or both NULL");
+    if (plan->info.n_adc > 0 && !h_signal) return fail(BLOCH_EINVAL, "h_signal is NULL");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
+    unsigned char *base = (unsigned char *)d_scratch;
+    float *d[7];
+    const float *h[7] = {h_x, h_y, h_z, h_M0, h_T1, h_T2, h_dw};
+    for (int k = 0; k < 7; ++k) {
+        d[k] = (float *)(base + k * arr);
+        if (n_spins > 0)
+            BLOCH_CUDA(cudaMemcpyAsync(d[k], h[k], size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+    }
+    float *d_Mxy = h_Mxy ? (float *)(base + 7 * arr) : nullptr;
+    float *d_Mz = h_Mz ? (float *)(base + 9 * arr) : nullptr;
+    if (!init_equilibrium && n_spins > 0) {
+        BLOCH_CUDA(cudaMemcpyAsync(d_Mxy, h_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyHostToDevice, stream));
+        BLOCH_CUDA(cudaMemcpyAsync(d_Mz, h_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+    }
+    const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
+                           ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
+                           : size_t(plan->info.n_adc) * sizeof(float2);
+    float *d_sig = (float *)(base + 10 * arr);
+    unsigned char *d_ws = base + 10 * arr + align_up(sig, kAlign);
+    const size_t ws_bytes = scratch_bytes - (size_t)(d_ws - base);
+    rc = bloch_simulate(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d_Mxy, d_Mz, init_equilibrium,
+                        d_sig, d_ws, ws_bytes, stream_);
+    if (rc) return rc;
+    if (sig > 0) BLOCH_CUDA(cudaMemcpyAsync(h_signal, d_sig, sig, cudaMemcpyDeviceToHost, stream));
+    if (h_Mxy && n_spins > 0) {
+        BLOCH_CUDA(cudaMemcpyAsync(h_Mxy, d_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyDeviceToHost, stream));
+        BLOCH_CUDA(cudaMemcpyAsync(h_Mz, d_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyDeviceToHost, stream));
+    }
+    BLOCH_CUDA(cudaStreamSynchronize(stream));
+    return BLOCH_OK;
+}
+
+int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {
+    if (!ops_per_s || iters <= 0 || kind < 0 || kind > 2) return fail(BLOCH_EINVAL, "bad microbench argument");
+    int rc = check_arch();
+    if (rc) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int sms = sm_count_cached();
+    const int grid = sms * 8, threads = 256;
+    float *d_out = nullptr;
+    BLOCH_CUDA(cudaMalloc(&d_out, sizeof(float)));  // diagnostic entry point only; not on the hot path
+    cudaEvent_t e0, e1;
+    BLOCH_CUDA(cudaEventCreate(&e0));
+    BLOCH_CUDA(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        BLOCH_CUDA(cudaEventRecord(e0, stream));
+        if (kind == 0) mb_mufu<<<grid, threads, 0, stream>>>(iters, d_out);
+        else if (kind == 1) mb_ffma<<<grid, threads, 0, stream>>>(iters, d_out);
+        else mb_dfma<<<grid, threads, 0, stream>>>(iters, d_out);
+        BLOCH_CUDA(cudaEventRecord(e1, stream));
+        BLOCH_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        BLOCH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_out);
+    const double per_thread = kind == 0 ? 24.0 * iters : 32.0 * iters;
+    *ops_per_s = per_thread * (double)grid * threads / (best * 1e-3);
+    return BLOCH_OK;
+}
+
+}  // extern "C"

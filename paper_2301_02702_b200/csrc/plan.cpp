@@ -1,0 +1,314 @@
+// plan.cpp -- host side of the hot path, fp64:
+//   a1 sequence discretiser: merged time grid from gradient vertices, RF sample edges and ADC times,
+//      refined so that no RF-active interval exceeds dt_rf_max ("sequence-aware time
+//      stepping")
+//   a2 block splitter / regime classification
+//   a3 k(t) table per precession block: cumulative trapezoid of G on the vertices (Eq 12-13, :173-180),
+//      stored only at the points that are evaluated (ADC samples) + one end record per block
+//   a4 rotation-vector table per RF step (Eq 8 with piecewise-constant B1, :146-148, :182)
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+
+#include "internal.h"
+
+namespace bloch {
+
+static thread_local std::string g_err;
+void set_error(const std::string &msg) { g_err = msg; }
+int fail(int code, const std::string &msg) {
+    g_err = msg;
+    return code;
+}
+const char *last_error_cstr() { return g_err.c_str(); }
+
+namespace {
+
+bool ascending(const double *a, int64_t n, bool strict) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (!std::isfinite(a[i])) return false;
+        if (i > 0 && (strict ? !(a[i] > a[i - 1]) : !(a[i] >= a[i - 1]))) return false;
+    }
+    return true;
+}
+
+// Piecewise-linear gradient of one axis sampled on the (ascending) grid by a forward sweep.
+void sample_axis(const double *gt, const double *gv, int64_t gn, const std::vector<double> &t,
+                 std::vector<double> &out, int axis) {
+    const size_t np = t.size();
+    int64_t seg = 0;
+    for (size_t n = 0; n < np; ++n) {
+        double v = 0.0;
+        const double tn = t[n];
+        if (gn == 1) {
+            v = (std::fabs(tn - gt[0]) <= kTimeTol) ? gv[0] : 0.0;
+        } else if (gn >= 2 && tn >= gt[0] - kTimeTol && tn <= gt[gn - 1] + kTimeTol) {
+            while (seg + 2 < gn && gt[seg + 1] <= tn) ++seg;
+            const double t0 = gt[seg], t1 = gt[seg + 1];
+            double w = (t1 > t0) ? (tn - t0) / (t1 - t0) : 1.0;
+            w = std::min(1.0, std::max(0.0, w));
+            v = gv[seg] + w * (gv[seg + 1] - gv[seg]);
+        }
+        out[3 * n + axis] = v;
+    }
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bloch_sim_params *params,
+               bloch_plan *plan) {
+    // ------------------------------------------------------------------ validation
+    if (!seq || !params || !plan) return fail(BLOCH_EINVAL, "NULL argument");
+    const double gamma = (scanner && scanner->gamma > 0.0) ? scanner->gamma : 2.0 * M_PI * 42.58e6;
+    if (!std::isfinite(gamma)) return fail(BLOCH_EINVAL, "gamma not finite");
+    if (!(seq->t_end > 0.0) || !std::isfinite(seq->t_end)) return fail(BLOCH_EINVAL, "t_end must be > 0");
+    if (params->phase_mode < BLOCH_PHASE_AUTO || params->phase_mode > BLOCH_PHASE_FP64)
+        return fail(BLOCH_EINVAL, "bad phase_mode");
+    if (params->output_mode != BLOCH_OUT_SUM_ALL && params->output_mode != BLOCH_OUT_PER_SPIN)
+        return fail(BLOCH_EINVAL, "bad output_mode");
+    for (int a = 0; a < 3; ++a) {
+        if (seq->g_n[a] < 0 || (seq->g_n[a] > 0 && (!seq->g_t[a] || !seq->g_v[a])))
+            return fail(BLOCH_EINVAL, "gradient arrays NULL or negative count");
+        if (!ascending(seq->g_t[a], seq->g_n[a], true))
+            return fail(BLOCH_ENONMONOTONIC, "gradient vertex times must be strictly ascending and finite");
+        for (int64_t i = 0; i < seq->g_n[a]; ++i) {
+            if (!std::isfinite(seq->g_v[a][i])) return fail(BLOCH_EINVAL, "gradient value not finite");
+            if (seq->g_t[a][i] < -kTimeTol || seq->g_t[a][i] > seq->t_end + kTimeTol)
+                return fail(BLOCH_EINVAL, "gradient vertex outside [0, t_end]");
+        }
+    }
+    if (seq->rf_n < 0 || (seq->rf_n > 0 && (!seq->rf_t || !seq->rf_dt || !seq->rf_re || !seq->rf_im)))
+        return fail(BLOCH_EINVAL, "RF arrays NULL or negative count");
+    for (int64_t i = 0; i < seq->rf_n; ++i) {
+        if (!std::isfinite(seq->rf_t[i]) || !(seq->rf_dt[i] > 0.0) || !std::isfinite(seq->rf_dt[i]) ||
+            !std::isfinite(seq->rf_re[i]) || !std::isfinite(seq->rf_im[i]))
+            return fail(BLOCH_EINVAL, "RF sample not finite or rf_dt <= 0");
+        if (seq->rf_t[i] < -kTimeTol || seq->rf_t[i] + seq->rf_dt[i] > seq->t_end + kTimeTol)
+            return fail(BLOCH_EINVAL, "RF sample outside [0, t_end]");
+        if (i > 0 && seq->rf_t[i] < seq->rf_t[i - 1] + seq->rf_dt[i - 1] - kTimeTol)
+            return fail(BLOCH_ENONMONOTONIC, "RF samples overlap or are not ascending");
+    }
+    if (seq->adc_n < 0 || (seq->adc_n > 0 && !seq->adc_t)) return fail(BLOCH_EINVAL, "ADC array NULL");
+    for (int64_t i = 0; i < seq->adc_n; ++i) {
+        if (!std::isfinite(seq->adc_t[i]) || seq->adc_t[i] < -kTimeTol || seq->adc_t[i] > seq->t_end + kTimeTol)
+            return fail(BLOCH_EINVAL, "ADC time outside [0, t_end]");
+        if (i > 0 && !(seq->adc_t[i] > seq->adc_t[i - 1] + kTimeTol))
+            return fail(BLOCH_ENONMONOTONIC, "ADC times must be strictly ascending");
+    }
+    const double dt_rf = (params->dt_rf_max > 0.0 && std::isfinite(params->dt_rf_max))
+                             ? params->dt_rf_max : std::numeric_limits<double>::infinity();
+
+    // ------------------------------------------------------------------ a1: merged grid
+    std::vector<double> pts;
+    pts.reserve(size_t(2 + seq->g_n[0] + seq->g_n[1] + seq->g_n[2] + 2 * seq->rf_n + seq->adc_n));
+    pts.push_back(0.0);
+    pts.push_back(seq->t_end);
+    for (int a = 0; a < 3; ++a) pts.insert(pts.end(), seq->g_t[a], seq->g_t[a] + seq->g_n[a]);
+    for (int64_t i = 0; i < seq->rf_n; ++i) {
+        pts.push_back(seq->rf_t[i]);
+        pts.push_back(seq->rf_t[i] + seq->rf_dt[i]);
+    }
+    pts.insert(pts.end(), seq->adc_t, seq->adc_t + seq->adc_n);
+    std::sort(pts.begin(), pts.end());
+    std::vector<double> coarse;
+    coarse.reserve(pts.size());
+    for (double t : pts) {
+        t = std::min(std::max(t, 0.0), seq->t_end);
+        if (coarse.empty() || t - coarse.back() > kTimeTol) coarse.push_back(t);
+    }
+    // RF coverage of the coarse intervals (sweep), then refinement of RF-active ones
+    std::vector<double> t;          // refined points
+    std::vector<int64_t> rf_of;     // per refined interval: RF sample index or -1
+    t.reserve(coarse.size());
+    rf_of.reserve(coarse.size());
+    t.push_back(coarse[0]);
+    {
+        int64_t j = 0;
+        for (size_t i = 0; i + 1 < coarse.size(); ++i) {
+            const double a = coarse[i], b = coarse[i + 1], mid = 0.5 * (a + b);
+            while (j < seq->rf_n && seq->rf_t[j] + seq->rf_dt[j] <= mid) ++j;
+            const bool covered = (j < seq->rf_n && seq->rf_t[j] <= mid);
+            int64_t parts = 1;
+            if (covered && std::isfinite(dt_rf)) parts = std::max<int64_t>(1, (int64_t)std::ceil((b - a) / dt_rf - 1e-9));
+            for (int64_t p = 1; p <= parts; ++p) {
+                t.push_back(p == parts ? b : a + (b - a) * (double(p) / double(parts)));
+                rf_of.push_back(covered ? j : -1);
+            }
+        }
+    }
+    const int64_t N = (int64_t)rf_of.size();
+    std::vector<double> G(3 * t.size(), 0.0);
+    for (int a = 0; a < 3; ++a) sample_axis(seq->g_t[a], seq->g_v[a], seq->g_n[a], t, G, a);
+    // ADC index per point (both ascending)
+    std::vector<int64_t> adc_at(t.size(), -1);
+    {
+        size_t n = 0;
+        for (int64_t i = 0; i < seq->adc_n; ++i) {
+            while (n + 1 < t.size() && t[n] < seq->adc_t[i] - kTimeTol) ++n;
+            if (std::fabs(t[n] - seq->adc_t[i]) > 2 * kTimeTol) return fail(BLOCH_EINVAL, "internal: ADC time not on the grid");
+            if (adc_at[n] != -1) return fail(BLOCH_ENONMONOTONIC, "two ADC samples closer than 1e-12 s");
+            adc_at[n] = i;
+        }
+    }
+
+    // ------------------------------------------------------------------ a2: blocks
+    const int64_t max_pts = params->max_block_points > 0 ? params->max_block_points : kDefaultMaxBlockPoints;
+    std::vector<Block> blocks;
+    {
+        int64_t n = 0;
+        while (n < N) {
+            Block b;
+            b.type = rf_of[n] >= 0 ? kBlockRF : kBlockPrecession;
+            b.first = n;
+            int64_t pts_in = 0;
+            while (n < N && (rf_of[n] >= 0) == (b.type == kBlockRF)) {
+                if (b.type == kBlockPrecession && adc_at[n + 1] >= 0) {
+                    if (pts_in + 1 > max_pts) break;
+                    ++pts_in;
+                }
+                ++n;
+            }
+            if (n == b.first) ++n;  // max_pts == 0 guard: always advance
+            b.count = n - b.first;
+            blocks.push_back(b);
+        }
+    }
+    // ADC assignment (reading G7): strictly inside an RF run -> error; on an RF/precession boundary ->
+    // served by the precession block (tau = 0 or tau = T); on a precession/precession cut -> the earlier.
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        Block &b = blocks[bi];
+        if (b.type == kBlockRF) {
+            for (int64_t n = b.first + 1; n < b.first + b.count; ++n)
+                if (adc_at[n] >= 0) return fail(BLOCH_EADC_IN_RF, "ADC sample strictly inside an RF-active run");
+            if (bi == 0 && adc_at[0] >= 0)
+                return fail(BLOCH_EADC_IN_RF, "ADC sample at t = 0 with RF starting at t = 0");
+            if (bi + 1 == blocks.size() && adc_at[N] >= 0)
+                return fail(BLOCH_EADC_IN_RF, "ADC sample at t_end with RF ending at t_end");
+            continue;
+        }
+        const bool serve_start = (bi == 0) || (blocks[bi - 1].type == kBlockRF);
+        const int64_t p0 = serve_start ? b.first : b.first + 1;
+        b.adc_first = -1;
+        b.adc_count = 0;
+        for (int64_t n = p0; n <= b.first + b.count; ++n) {
+            if (adc_at[n] < 0) continue;
+            if (b.adc_first < 0) b.adc_first = adc_at[n];
+            ++b.adc_count;
+        }
+        if (b.adc_first < 0) b.adc_first = 0;
+    }
+
+    // ------------------------------------------------------------------ a3 + phase-mode resolution
+    const double gbar = gamma / (2.0 * M_PI);
+    double worst_turns = 0.0;
+    std::vector<double> krec;  // 4 doubles per evaluated point, all precession blocks in order
+    std::vector<int64_t> krec_first(blocks.size(), 0);
+    int64_t n_rf_steps = 0, n_rf_blocks = 0, n_eval = 0, max_block_adc = 0;
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        Block &b = blocks[bi];
+        if (b.type == kBlockRF) {
+            n_rf_steps += b.count;
+            ++n_rf_blocks;
+            continue;
+        }
+        krec_first[bi] = (int64_t)krec.size() / 4;
+        const bool serve_start = (bi == 0) || (blocks[bi - 1].type == kBlockRF);
+        double K[3] = {0, 0, 0};
+        const double tb = t[b.first];
+        if (serve_start && adc_at[b.first] >= 0) krec.insert(krec.end(), {0.0, 0.0, 0.0, 0.0});
+        for (int64_t n = b.first; n < b.first + b.count; ++n) {
+            const double dt = t[n + 1] - t[n];
+            for (int a = 0; a < 3; ++a) K[a] += 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]) * dt;  // Eq 12-13
+            const double tau = t[n + 1] - tb;
+            const double kn = gbar * std::sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]);
+            worst_turns = std::max(worst_turns, kn * 0.25 + 1000.0 * tau);
+            if (adc_at[n + 1] >= 0) krec.insert(krec.end(), {-gbar * K[0], -gbar * K[1], -gbar * K[2], tau});
+        }
+        for (int a = 0; a < 3; ++a) b.kend[a] = -gbar * K[a];
+        b.tau_end = t[b.first + b.count] - tb;
+        n_eval += b.adc_count + 1;
+        max_block_adc = std::max(max_block_adc, b.adc_count);
+        if ((int64_t)krec.size() / 4 - krec_first[bi] != b.adc_count)
+            return fail(BLOCH_EINVAL, "internal: ADC bookkeeping mismatch");
+    }
+    // AUTO: fp32 phase (in turns, block-relative) keeps ~2^-24 * turns of resolution; above 256 turns
+    // (bound: |k| * 0.25 m + 1 kHz * tau) switch to fp64 phase accumulation (north_star item 4).
+    int phase = params->phase_mode;
+    if (phase == BLOCH_PHASE_AUTO) phase = worst_turns > 256.0 ? BLOCH_PHASE_FP64 : BLOCH_PHASE_FP32;
+
+    // ------------------------------------------------------------------ tables: layout + fill
+    size_t off = 0;
+    const size_t rec_bytes = phase == BLOCH_PHASE_FP64 ? 32 : 16;
+    for (Block &b : blocks) {
+        b.table_off = (int64_t)off;
+        const size_t bytes = b.type == kBlockRF ? size_t(b.count) * kRfStepFloats * sizeof(float)
+                                                : size_t(b.adc_count) * rec_bytes;
+        off = align_up(off + bytes, kAlign);
+    }
+    if (off == 0) off = kAlign;
+    plan->tables.assign(off, 0);
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        const Block &b = blocks[bi];
+        unsigned char *dst = plan->tables.data() + b.table_off;
+        if (b.type == kBlockRF) {
+            float *r = reinterpret_cast<float *>(dst);
+            for (int64_t n = b.first; n < b.first + b.count; ++n, r += kRfStepFloats) {
+                const double dt = t[n + 1] - t[n];
+                const int64_t j = rf_of[n];
+                // rotation vector w = gamma * B * dt (Eq 8); gradient part is per-metre, mean of the two
+                // vertex values (reading G5)
+                r[0] = (float)(gamma * dt * seq->rf_re[j]);
+                r[1] = (float)(gamma * dt * seq->rf_im[j]);
+                for (int a = 0; a < 3; ++a)
+                    r[2 + a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]));
+                r[5] = (float)dt;
+                r[6] = 0.f;
+                r[7] = 0.f;
+            }
+        } else {
+            const double *src = krec.data() + 4 * krec_first[bi];
+            if (phase == BLOCH_PHASE_FP64) {
+                std::memcpy(dst, src, size_t(b.adc_count) * 32);
+            } else {
+                float *r = reinterpret_cast<float *>(dst);
+                for (int64_t i = 0; i < 4 * b.adc_count; ++i) r[i] = (float)src[i];
+            }
+        }
+    }
+
+    // ------------------------------------------------------------------ launch count (SUM_ALL, final state)
+    int64_t launches = 2;  // pack + unpack
+    {
+        bool pending = false;
+        for (const Block &b : blocks) {
+            if (b.type == kBlockRF) { ++launches; pending = false; continue; }
+            if (pending) ++launches;
+            if (b.adc_count > 0) launches += (params->output_mode == BLOCH_OUT_SUM_ALL) ? 2 : 1;
+            pending = true;
+        }
+        if (pending) ++launches;
+    }
+
+    plan->gamma = gamma;
+    plan->params = *params;
+    plan->blocks = std::move(blocks);
+    plan->d_tables = nullptr;
+    bloch_plan_info &inf = plan->info;
+    inf.n_intervals = N;
+    inf.n_rf_steps = n_rf_steps;
+    inf.n_adc = seq->adc_n;
+    inf.n_blocks = (int64_t)plan->blocks.size();
+    inf.n_rf_blocks = n_rf_blocks;
+    inf.n_eval_points = n_eval;
+    inf.n_launches = launches;
+    inf.table_bytes = (int64_t)plan->tables.size();
+    inf.max_block_adc = max_block_adc;
+    inf.phase_mode = phase;
+    inf.output_mode = params->output_mode;
+    return BLOCH_OK;
+}
+
+}  // namespace bloch

@@ -351,7 +351,8 @@ def _spiral(axes, t0: float, n_samp: int, dwell: float, k_max: float, turns: flo
 # --------------------------------------------------------------------------------------------------
 # config 4: 1M-spin slab, 16-interleave spiral
 # --------------------------------------------------------------------------------------------------
-def config4(n_spins: int = 1_000_000, n_shots: int = 16, n_samp: int = 4096, n_rf: int = 2000) -> Workload:
+def config4(n_spins: int = 1_000_000, n_shots: int = 16, n_samp: int = 4096, n_rf: int = 2000,
+            turns: float = 8.0) -> Workload:
     rng = np.random.default_rng(SEED0 + 4)
     x = rng.uniform(-0.11, 0.11, n_spins)
     y = rng.uniform(-0.11, 0.11, n_spins)
@@ -368,7 +369,7 @@ def config4(n_spins: int = 1_000_000, n_shots: int = 16, n_samp: int = 4096, n_r
         t0 = j * TR + 200e-6
         rf_parts.append(_sinc_rf(t0, dur, n_rf, math.radians(30.0)))
         t_reph = _slice_select(axes[2], t0, dur, 4.0, thk)
-        adc, _ = _spiral(axes, t_reph + 10e-6, n_samp, dwell, k_max, 8.0, 2 * math.pi * j / n_shots)
+        adc, _ = _spiral(axes, t_reph + 10e-6, n_samp, dwell, k_max, turns, 2 * math.pi * j / n_shots)
         adc_parts.append(adc)
     seq = _finish(axes, rf_parts, adc_parts, n_shots * TR, dur / n_rf, {"config": 4})
     return Workload("config4_1M_spiral", ph, seq)
@@ -377,7 +378,7 @@ def config4(n_spins: int = 1_000_000, n_shots: int = 16, n_samp: int = 4096, n_r
 # --------------------------------------------------------------------------------------------------
 # config 5 / 5b: MRF FISP
 # --------------------------------------------------------------------------------------------------
-def _mrf_sequence(n_tr: int, n_samp: int, n_rf: int, one_adc_per_tr: bool, rng) -> Sequence:
+def _mrf_sequence(n_tr: int, n_samp: int, n_rf: int, one_adc_per_tr: bool, rng, turns: float = 6.0) -> Sequence:
     k = np.arange(n_tr)
     fa = np.clip(37.5 + 32.5 * np.sin(2 * math.pi * k / 250.0) + 2.0 * rng.standard_normal(n_tr), 5.0, 70.0)
     TRs = rng.uniform(10e-3, 15e-3, n_tr)
@@ -390,7 +391,7 @@ def _mrf_sequence(n_tr: int, n_samp: int, n_rf: int, one_adc_per_tr: bool, rng) 
     for i in range(n_tr):
         t0 = t_tr + 100e-6
         rf_parts.append(_sinc_rf(t0, dur, n_rf, math.radians(float(fa[i]))))
-        adc, t_sp = _spiral(axes, t0 + dur + 500e-6, n_samp, dwell, 128.0, 6.0, golden * i)
+        adc, t_sp = _spiral(axes, t0 + dur + 500e-6, n_samp, dwell, 128.0, turns, golden * i)
         adc_parts.append(adc[:1] if one_adc_per_tr else adc)
         a, r, f = _area_trap(320.0)              # x-axis spoiler, 320 1/m
         axes[0].trap(t_sp + 10e-6, a, r, f)
@@ -399,7 +400,8 @@ def _mrf_sequence(n_tr: int, n_samp: int, n_rf: int, one_adc_per_tr: bool, rng) 
                    {"config": 5, "fa_deg": fa, "TR": TRs})
 
 
-def config5(n_grid: int = 256, n_tr: int = 1000, n_samp: int = 1024, n_rf: int = 1000) -> Workload:
+def config5(n_grid: int = 256, n_tr: int = 1000, n_samp: int = 1024, n_rf: int = 1000,
+            turns: float = 6.0) -> Workload:
     rng = np.random.default_rng(SEED0 + 5)
     fov = 0.2
     g = _grid(n_grid, fov)
@@ -408,18 +410,19 @@ def config5(n_grid: int = 256, n_tr: int = 1000, n_samp: int = 1024, n_rf: int =
     T1 = rng.uniform(0.1, 4.0, n)
     T2 = rng.uniform(0.01, 0.6, n)
     ph = _phantom(X.ravel(), Y.ravel(), np.zeros(n), np.ones(n), T1, T2, np.zeros(n))
-    seq = _mrf_sequence(n_tr, n_samp, n_rf, False, rng)
+    seq = _mrf_sequence(n_tr, n_samp, n_rf, False, rng, turns)
     return Workload("config5_mrf_fisp", ph, seq)
 
 
-def config5b(n_entries: int = 100_000, n_tr: int = 1000, n_samp: int = 1024, n_rf: int = 1000) -> Workload:
+def config5b(n_entries: int = 100_000, n_tr: int = 1000, n_samp: int = 1024, n_rf: int = 1000,
+             turns: float = 6.0) -> Workload:
     """Dictionary mode: the phantom draws come from their own stream; the schedule is config 5's
     (same seed, same draw order for the sequence part)."""
     rng5 = np.random.default_rng(SEED0 + 5)
     n5 = 256 * 256
     rng5.uniform(0.1, 4.0, n5)
     rng5.uniform(0.01, 0.6, n5)                  # skip config 5's phantom draws -> same schedule
-    seq = _mrf_sequence(n_tr, n_samp, n_rf, True, rng5)
+    seq = _mrf_sequence(n_tr, n_samp, n_rf, True, rng5, turns)
     rng = np.random.default_rng(SEED0 + 6)
     T1 = rng.uniform(0.1, 4.0, n_entries)
     T2 = rng.uniform(0.01, 0.6, n_entries)
@@ -437,7 +440,8 @@ def make(name: str, **kw) -> Workload:
 
 def small(name: str) -> Workload:
     """Reduced-size variants (same structure) that the CPU oracle finishes in seconds; used by the
-    parity tests.  Sizes still span several kernel tiles and leave ragged tails."""
+    parity tests.  Sizes still span several kernel tiles and leave ragged tails.  Spiral turn counts are
+    scaled with the shortened readouts so that the gradient amplitudes stay those of the full configs."""
     name = str(name)
     if name == "1":
         return config1()
@@ -446,9 +450,9 @@ def small(name: str) -> Workload:
     if name == "3":
         return config3(n_grid=48, n_epi=32, n_rf=250)
     if name == "4":
-        return config4(n_spins=5003, n_shots=3, n_samp=700, n_rf=300)
+        return config4(n_spins=5003, n_shots=3, n_samp=700, n_rf=300, turns=8.0 * 700 / 4096)
     if name == "5":
-        return config5(n_grid=40, n_tr=12, n_samp=300, n_rf=200)
+        return config5(n_grid=40, n_tr=12, n_samp=300, n_rf=200, turns=6.0 * 300 / 1024)
     if name == "5b":
-        return config5b(n_entries=777, n_tr=40, n_samp=512, n_rf=200)
+        return config5b(n_entries=777, n_tr=40, n_samp=512, n_rf=200, turns=3.0)
     raise KeyError(name)

@@ -1,0 +1,123 @@
+"""Host logic of the C-ABI library (no GPU): symbols, planner counts, error paths."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2301_02702_b200 import build as bl
+from paper_2301_02702_b200 import workloads as W
+from seqtools import seq
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    bl.build()
+    from paper_2301_02702_b200 import bloch
+    return bloch
+
+
+def test_library_exports_every_declared_symbol(B):
+    hdr = open(os.path.join(ROOT, "include", "bloch.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(bloch_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(B.EXPORTS)
+    lib = ctypes.CDLL(os.path.join(ROOT, "paper_2301_02702_b200", "libbloch_b200.so"))
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert B.bloch_version() >= 100
+    assert B.bloch_strerror(-3)
+
+
+@pytest.mark.parametrize("name", ["1", "2", "3", "4", "5", "5b"])
+def test_plan_counts_match_oracle_grid(B, oracle_mod, name):
+    w = W.small(name)
+    h = B.bloch_plan_create(w.seq, phase_mode=w.phase_mode, output_mode=w.output_mode)
+    try:
+        info = B.bloch_plan_get_info(h)
+        t, G, rf, adc = oracle_mod.grid(w.seq)
+        assert info["n_intervals"] == len(t) - 1
+        assert info["n_rf_steps"] == int(rf.sum())
+        assert info["n_adc"] == len(w.seq.adc_t)
+        assert info["n_eval_points"] == info["n_adc"] + (info["n_blocks"] - info["n_rf_blocks"])
+        assert info["table_bytes"] % 256 == 0
+        assert B.bloch_plan_workspace_bytes(h, w.phantom.n) >= 48 * w.phantom.n
+        assert info["phase_mode"] == (B.PHASE_FP64 if w.phase_mode == "fp64" else B.PHASE_FP32)
+    finally:
+        B.bloch_plan_destroy(h)
+
+
+def test_plan_error_paths(B):
+    ok = dict(g={0: ([1e-3, 2e-3], [0.0, 0.0])}, rf=([0.0], [1e-4], [1e-6], [0.0]), adc=[5e-4], t_end=3e-3)
+    h = B.bloch_plan_create(seq(**ok))
+    B.bloch_plan_destroy(h)
+    bad = dict(ok); bad["g"] = {0: ([2e-3, 1e-3], [0.0, 0.0])}
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(seq(**bad))
+    assert e.value.code == -2
+    bad = dict(ok); bad["adc"] = [5e-5]                 # strictly inside the RF run
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(seq(**bad, dt_rf_max=1e-5))
+    assert e.value.code == -3
+    bad = dict(ok); bad["rf"] = ([0.0, 5e-5], [1e-4, 1e-4], [1e-6, 1e-6], [0.0, 0.0])   # overlap
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(seq(**bad))
+    assert e.value.code == -2
+    bad = dict(ok); bad["t_end"] = -1.0
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(seq(**bad))
+    assert e.value.code == -1
+    bad = dict(ok); bad["adc"] = [4e-3]                 # beyond t_end
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(seq(**bad))
+    assert e.value.code == -1
+    with pytest.raises(B.BlochError) as e:              # simulate before upload
+        h = B.bloch_plan_create(seq(**ok))
+        try:
+            B.bloch_simulate(h, 4, 1, 1, 1, 1, 1, 1, 1, None, None, True, 1, 256, 1 << 20)
+        finally:
+            B.bloch_plan_destroy(h)
+    assert e.value.code == -7
+
+
+def test_adc_on_rf_boundary_is_served_by_precession_block(B):
+    s = seq(rf=([1e-3], [1e-4], [1e-6], [0.0]), adc=[1e-3, 1.1e-3, 2e-3], t_end=3e-3, dt_rf_max=1e-5)
+    h = B.bloch_plan_create(s)
+    info = B.bloch_plan_get_info(h)
+    B.bloch_plan_destroy(h)
+    assert info["n_blocks"] == 3 and info["n_rf_blocks"] == 1 and info["n_rf_steps"] == 10
+    assert info["n_adc"] == 3 and info["max_block_adc"] == 2
+
+
+def test_max_block_points_splits_precession_blocks(B):
+    adc = np.linspace(1e-3, 9e-3, 100)
+    s = seq(adc=adc, t_end=10e-3)
+    h = B.bloch_plan_create(s, max_block_points=16)
+    info = B.bloch_plan_get_info(h)
+    B.bloch_plan_destroy(h)
+    assert info["n_blocks"] == 7 and info["max_block_adc"] == 16
+
+
+def test_rf_increment_form_equals_eq9():
+    """The RF kernel applies Eq 9 as M+ = M + a (w x M) + b (w x (w x M)) (kernels.cuh).  Check that
+    identity against Eq 6-9 written out with complex spinors, in fp64 numpy."""
+    rng = np.random.default_rng(0)
+    for _ in range(200):
+        w = rng.normal(0, 1.0, 3) * rng.choice([1e-4, 1e-2, 1.0])
+        M = rng.normal(0, 1, 3)
+        t = np.linalg.norm(w)
+        phi = -t                                       # Eq 8 with w = gamma B dt
+        nxy, nz = (w[0] + 1j * w[1]) / t, w[2] / t
+        al = math.cos(phi / 2) - 1j * nz * math.sin(phi / 2)
+        be = -1j * nxy * math.sin(phi / 2)
+        mxy = M[0] + 1j * M[1]
+        mxy2 = 2 * np.conj(al) * be * M[2] + np.conj(al) ** 2 * mxy - be ** 2 * np.conj(mxy)
+        mz2 = (abs(al) ** 2 - abs(be) ** 2) * M[2] - 2 * (al * be * np.conj(mxy)).real
+        a, b = -math.sin(t) / t, (1 - math.cos(t)) / t ** 2
+        u = np.cross(w, M)
+        got = M + a * u + b * np.cross(w, u)
+        np.testing.assert_allclose(got, [mxy2.real, mxy2.imag, mz2], rtol=0, atol=1e-14)
