@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path (plan tables resident; pack, every RF and
+free-precession block, the two-pass signal reduction, final state) over one synthetic workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  metric = Bloch spin*steps/s: N_spins x N_intervals of the discretised
+sequence (what the step-by-step solver of the paper executes, SURVEY.md 8(d) "Counting") / device time.
+See DESIGN.md "Measurement" for the roofline arithmetic.  The reference arm (--impl reference) times the
+fp64 CPU oracle, as it stands, on the host cores; it is the only place besides cpu_baseline that touches
+oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bloch_spin_steps_per_s"
+UNIT = "spin*steps/s"
+SM_COUNT = 148
+# pipe peaks derived from unit counts x max SM clock: MUFU 16 lanes/SM/clk,
+# FP32 128 lanes/SM/clk
+MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)
+FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML every 100 ms while running (timed region only)."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def make_workload(name: str, rank: int):
+    """Rank r simulates shard r of an (N x n_spins)-spin phantom on the SAME sequence: the phantom comes from
+    the same generator with the seed moved by the rank (weak scaling: per-GPU work is fixed)."""
+    from paper_2301_02702_b200 import workloads as W
+    w = W.make(name)
+    if rank:
+        base = W.SEED0
+        try:
+            W.SEED0 = base + 1000 * rank
+            w = W.Workload(w.name, W.make(name).phantom, w.seq, w.phase_mode, w.output_mode)
+        finally:
+            W.SEED0 = base
+    return w
+
+
+def oracle_sample(w, budget_spin_steps: float, n_intervals: int):
+    """A bounded sample of the workload for the CPU oracle: every m-th spin, the full sequence."""
+    n = w.phantom.n
+    take = int(max(1, min(n, budget_spin_steps // max(1, n_intervals))))
+    idx = np.linspace(0, n - 1, take).astype(np.int64)
+    return w.phantom.subset(idx), take
+
+
+def time_oracle(w, n_intervals: int, budget_spin_steps: float):
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    ph, take = oracle_sample(w, budget_spin_steps, n_intervals)
+    t0 = time.perf_counter()
+    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": take * n_intervals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{take} of {w.phantom.n} spins (evenly spaced), full sequence ({n_intervals} intervals), "
+                      f"fp64, OpenMP over spins, {dt:.2f} s"}, dt, take
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the fp64 CPU oracle, as it stands, on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    import oracle
+    w = make_workload(args.workload, 0)
+    t, _, _, _ = oracle.grid(w.seq)
+    n_int = len(t) - 1
+    cores = os.cpu_count() or 1
+    # size a step at ~3 s of CPU work from a short probe
+    probe, dtp, take_p = time_oracle(w, n_int, 2e7)
+    per_step = max(2e7, probe["value"] * 3.0)
+    times = []
+    take = 0
+    for i in range(args.warmup + args.steps):
+        res, dt, take = time_oracle(w, n_int, per_step)
+        if i >= args.warmup:
+            times.append(dt)
+    total = float(np.sum(times))
+    value = take * n_int * len(times) / total
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": w.name, "n_spins": w.phantom.n, "n_intervals": n_int,
+                      "sample_spins_per_step": take},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": f"{take} of {w.phantom.n} spins per step, full sequence, fp64"},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2301_02702_b200 import build as bl
+    if rank == 0:
+        bl.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2301_02702_b200 import bloch
+    from paper_2301_02702_b200.dist import reduce_signal
+
+    w = make_workload(args.workload, rank)
+    per_spin = w.output_mode == "per_spin"
+    t_plan0 = time.perf_counter()
+    plan = bloch.Plan(w.seq, phase_mode=w.phase_mode, output_mode=w.output_mode)
+    plan.upload()
+    torch.cuda.synchronize()
+    plan_s = time.perf_counter() - t_plan0
+    info = plan.info
+    n = w.phantom.n
+    n_int = info["n_intervals"]
+    spin_steps = float(n) * float(n_int)
+    dev = bloch.phantom_to_device(w.phantom)
+    Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda")
+    Mz = torch.zeros(n, dtype=torch.float32, device="cuda")
+    shape = (n, info["n_adc"]) if per_spin else (info["n_adc"],)
+    sig = torch.empty(shape, dtype=torch.complex64, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig)
+        if not per_spin:
+            reduce_signal(sig)
+
+    bloch.bloch_plan_set_profiling(plan.handle, True)
+    for _ in range(args.warmup):
+        flush.zero_()
+        step()
+    barrier()
+
+    # ---- device-resident timing: K steps, L2 flushed (untimed) before each, CUDA events around each step
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kinds_ms = {k: 0.0 for k in bloch.KINDS}
+    kinds_n = {k: 0 for k in bloch.KINDS}
+    clocks = ClockSampler(local_rank)
+    with clocks:
+        barrier()
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            step()
+            b.record()
+            b.synchronize()
+            tm = bloch.bloch_plan_last_timing(plan.handle)
+            for k in bloch.KINDS:
+                kinds_ms[k] += tm["ms"][k]
+                kinds_n[k] += tm["launches"][k]
+        barrier()
+    ms_local = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = spin_steps * world * args.steps / (ms_total * 1e-3)
+    bloch.bloch_plan_set_profiling(plan.handle, False)
+
+    # ---- end to end through the host-buffer C-ABI entry: pinned host inputs, H2D + D2H inside the timed region
+    ph = w.phantom
+    pinned = [torch.from_numpy(np.ascontiguousarray(getattr(ph, k), dtype=np.float32)).pin_memory()
+              for k in ("x", "y", "z", "M0", "T1", "T2", "dw")]
+    h_sig = torch.empty(shape, dtype=torch.complex64).pin_memory()
+    h_arrs = [p.numpy() for p in pinned]
+    h_sig_np = h_sig.numpy()
+    e2e_steps = max(1, min(args.steps, 5))
+    plan.simulate_host(*h_arrs, signal=h_sig_np)           # warm-up (allocates the scratch)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.simulate_host(*h_arrs, signal=h_sig_np)       # synchronous: returns after the D2H copy
+        if not per_spin and world > 1:
+            reduce_signal(torch.from_numpy(h_sig_np).cuda())
+    barrier()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = spin_steps * world * e2e_steps / float(e2e_s.item())
+    h2d = sum(int(a.nbytes) for a in h_arrs)
+    d2h = int(h_sig_np.nbytes)
+
+    if rank != 0:
+        return
+    peaks = load_peaks()
+    sm_max = float(clocks.max_mhz or peaks.get("sm_max_mhz") or 1965.0)
+    mufu_peak = SM_COUNT * 16 * sm_max * 1e6          # MUFU ops/s
+    fp32_peak = SM_COUNT * 128 * sm_max * 1e6         # FP32 instr/s
+    n_eval_sig = float(n) * float(info["n_adc"])      # evaluations in the signal kernels per step
+    rf_steps = float(n) * float(info["n_rf_steps"])
+    kern = {}
+    if kinds_n["signal"]:
+        dur = kinds_ms["signal"] * 1e-3 / args.steps
+        ach = MUFU_PER_EVAL * n_eval_sig / dur
+        kern["signal"] = {"bound": "alu", "pipe": "mufu", "achieved": ach / 1e12, "peak": mufu_peak / 1e12,
+                          "unit": "Tmufu-op/s", "frac": ach / mufu_peak, "traffic": None,
+                          "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
+                          "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
+                          "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}
+    if kinds_n["rf"]:
+        dur = kinds_ms["rf"] * 1e-3 / args.steps
+        ach = FP32_PER_RF_STEP * rf_steps / dur
+        kern["rf"] = {"bound": "alu", "pipe": "fp32", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
+                      "unit": "Tfp32-instr/s", "frac": ach / fp32_peak, "traffic": None,
+                      "launches_per_step": kinds_n["rf"] // args.steps, "ms_per_step": dur * 1e3,
+                      "avg_launch_ms": kinds_ms["rf"] / kinds_n["rf"],
+                      "algorithmic_ops_per_launch": FP32_PER_RF_STEP * rf_steps * args.steps / kinds_n["rf"]}
+    dominant = max(kern, key=lambda k: kern[k]["ms_per_step"]) if kern else None
+    roofline = dict(kern[dominant], kernel=dominant,
+                    peak_source=f"derived: {SM_COUNT} SMs x lanes/SM/clk x {sm_max:.0f} MHz (DESIGN.md Roofline)") \
+        if dominant else None
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32" if info["phase_mode"] == 1 else "f32+f64phase",
+           "data": "synthetic",
+           "config": {"workload": w.name, "n_spins_per_gpu": n, "n_intervals": n_int,
+                      "n_rf_steps": info["n_rf_steps"], "n_adc": info["n_adc"], "n_blocks": info["n_blocks"],
+                      "output_mode": w.output_mode, "spin_steps_per_step": spin_steps * world,
+                      "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
+                      "plan_create_upload_s": plan_s},
+           "sim_wall_time_s": ms_total / args.steps * 1e-3,
+           "clocks": clocks.summary(),
+           "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "steps": e2e_steps, "api": "bloch_simulate_host (pinned host buffers)"},
+           "gpu_launches": int(sum(kinds_n.values())),
+           "roofline": roofline,
+           "kernels": kern,
+           "ms_by_kind_per_step": {k: v / args.steps for k, v in kinds_ms.items()}}
+    if args.microbench:
+        out["pipe_microbench"] = {"mufu_ops_per_s": bloch.bloch_microbench(0), "ffma_per_s": bloch.bloch_microbench(1),
+                                  "dfma_per_s": bloch.bloch_microbench(2)}
+    if not args.no_cpu_baseline:
+        cb, _, _ = time_oracle(w, n_int, args.cpu_budget)
+        out["cpu_baseline"] = cb
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 4 (default, 1M-spin spiral), 5, 5b")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")
+    ap.add_argument("--microbench", action="store_true", help="also run the MUFU/FFMA/DFMA pipe micro-benchmarks")
+    args = ap.parse_args()
+    from paper_2301_02702_b200.dist import env_world
+    rank, local_rank, world = env_world()
+    if args.cpu_budget <= 0:
+        args.cpu_budget = 2e8 * max(1, (os.cpu_count() or 1))   # ~10-30 s at ~10-20 ns per spin*step per core
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    run_ours(args, rank, local_rank, world)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -141,13 +141,19 @@ int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins,
                         float *h_Mxy, float *h_Mz, int init_equilibrium,
                         float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
 
-/* Timing taps for the benchmark: after a bloch_simulate on `stream` has been synchronised by the caller,
- * returns the device time (ms, CUDA events recorded on `stream`) spent in the RF kernels, in the
- * free-precession signal kernels (+ their reductions) and in total, and the number of kernels launched.
- * Enabled with bloch_plan_set_profiling(plan, 1); off by default (no events are recorded). */
+/* Timing taps for the benchmark.  With bloch_plan_set_profiling(plan, 1) bloch_simulate records one CUDA
+ * event on `stream` before every kernel it launches (and one after the last); off by default.  After the
+ * caller has synchronised `stream`, bloch_plan_last_timing fills, per kernel kind, the summed device time
+ * [ms] and the number of launches of the last bloch_simulate: arrays of BLOCH_N_KINDS entries indexed by
+ * BLOCH_KIND_*.  A kernel's time is the interval to the next event on the stream, so it includes the
+ * launch gap that follows it. */
+enum { BLOCH_KIND_OTHER = 0,   /* pack / unpack / block-end propagation only */
+       BLOCH_KIND_RF = 1,      /* excitation kernel */
+       BLOCH_KIND_SIGNAL = 2,  /* free-precession signal kernel (a6) */
+       BLOCH_KIND_REDUCE = 3,  /* second pass of the signal reduction (a7) */
+       BLOCH_N_KINDS = 4 };
 int bloch_plan_set_profiling(bloch_plan *plan, int enable);
-int bloch_plan_last_timing(const bloch_plan *plan, float *ms_rf, float *ms_precession, float *ms_total,
-                           int64_t *n_launches);
+int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *launches_by_kind);
 
 /* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
  * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA, 2 = DFMA.  Runs `iters` dependent-chain iterations with 8

@@ -72,8 +72,7 @@ def _load():
     lib.bloch_simulate_host_scratch_bytes.argtypes = [vp, i64, C.POINTER(sz)]
     lib.bloch_simulate_host.argtypes = sim_args
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
-    lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float),
-                                           C.POINTER(C.c_float), C.POINTER(i64)]
+    lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
     for name in EXPORTS:
         if name not in ("bloch_strerror", "bloch_last_error"):
@@ -188,10 +187,15 @@ def bloch_plan_set_profiling(plan: int, enable: bool):
     _check(_lib.bloch_plan_set_profiling(plan, int(bool(enable))))
 
 
+KINDS = ("other", "rf", "signal", "reduce")   # BLOCH_KIND_*
+
+
 def bloch_plan_last_timing(plan: int) -> dict:
-    a, b, c, n = C.c_float(), C.c_float(), C.c_float(), C.c_int64()
-    _check(_lib.bloch_plan_last_timing(plan, C.byref(a), C.byref(b), C.byref(c), C.byref(n)))
-    return {"ms_rf": a.value, "ms_precession": b.value, "ms_total": c.value, "launches": int(n.value)}
+    ms = (C.c_float * len(KINDS))()
+    cnt = (C.c_int64 * len(KINDS))()
+    _check(_lib.bloch_plan_last_timing(plan, ms, cnt))
+    return {"ms": {k: float(ms[i]) for i, k in enumerate(KINDS)},
+            "launches": {k: int(cnt[i]) for i, k in enumerate(KINDS)}}
 
 
 def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:

@@ -1,4 +1,5 @@
 // api.cu -- C-ABI entry points of libbloch_b200 (include/bloch.h) and the per-block launch logic.
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -59,8 +60,8 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
     if (chunks > max_chunks) chunks = max_chunks;
     if (chunks < 1) chunks = 1;
     if (chunks > 65535) chunks = 65535;
-    s.spins_per_chunk = (int)((n_spins + chunks - 1) / chunks);
-    s.chunks = (int)((n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
+    s.spins_per_chunk = (int)std::max<int64_t>(1, (n_spins + chunks - 1) / chunks);
+    s.chunks = (int)std::max<int64_t>(1, (n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
     return s;
 }
 
@@ -224,23 +225,20 @@ int bloch_plan_set_profiling(bloch_plan *plan, int enable) {
     return BLOCH_OK;
 }
 
-int bloch_plan_last_timing(const bloch_plan *plan, float *ms_rf, float *ms_prec, float *ms_total,
-                           int64_t *n_launches) {
-    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
-    Timing t{};
-    t.launches = plan->last.launches;
+int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *launches_by_kind) {
+    if (!plan || !ms_by_kind || !launches_by_kind) return fail(BLOCH_EINVAL, "NULL argument");
+    for (int k = 0; k < BLOCH_N_KINDS; ++k) {
+        ms_by_kind[k] = 0.f;
+        launches_by_kind[k] = 0;
+    }
     const size_t n = plan->event_kind.size();
     for (size_t k = 0; k + 1 < n; ++k) {
         float ms = 0.f;
         BLOCH_CUDA(cudaEventElapsedTime(&ms, (cudaEvent_t)plan->events[k], (cudaEvent_t)plan->events[k + 1]));
-        if (plan->event_kind[k] == 1) t.ms_rf += ms;
-        else if (plan->event_kind[k] == 2) t.ms_prec += ms;
-        t.ms_total += ms;
+        const int kind = plan->event_kind[k];
+        ms_by_kind[kind] += ms;
+        launches_by_kind[kind] += 1;
     }
-    if (ms_rf) *ms_rf = t.ms_rf;
-    if (ms_prec) *ms_prec = t.ms_prec;
-    if (ms_total) *ms_total = t.ms_total;
-    if (n_launches) *n_launches = t.launches;
     return BLOCH_OK;
 }
 
@@ -276,8 +274,7 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     const int n = (int)n_spins;
     Taps taps{plan, stream};
     int64_t launches = 0;
-    rc = taps.mark(0);
-    if (rc) return rc;
+    if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
     pack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw,
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S);
@@ -288,7 +285,7 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     const int rf_grid = (n + kRfThreads - 1) / kRfThreads;
     for (const Block &b : plan->blocks) {
         if (b.type == kBlockRF) {
-            if ((rc = taps.mark(1))) return rc;
+            if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
             rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>((const float4 *)(plan->d_tables + b.table_off),
                                                            (int)b.count, prop, pending ? 1 : 0, w.A, w.C, w.S, n);
             ++launches;
@@ -296,13 +293,13 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
             continue;
         }
         if (pending) {  // two precession blocks in a row: apply the first one's end transform now
-            if ((rc = taps.mark(2))) return rc;
+            if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
             rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
             ++launches;
             pending = false;
         }
         if (b.adc_count > 0) {
-            if ((rc = taps.mark(2))) return rc;
+            if ((rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
             const void *recs = plan->d_tables + b.table_off;
             const int n_pts = (int)b.adc_count;
             if (per_spin) {
@@ -333,6 +330,7 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
                 else BLOCH_LAUNCH_SIG(1);
 #undef BLOCH_LAUNCH_SIG
+                if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
                 reduce_kernel<<<(n_pts + 31) / 32, dim3(32, 8), 0, stream>>>(w.partial, s.chunks, n_pts,
                                                                             (float2 *)d_signal + b.adc_first);
                 launches += 2;
@@ -345,15 +343,16 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
         pending = true;
     }
     if (d_Mxy) {
-        if ((rc = taps.mark(0))) return rc;
         if (pending) {
+            if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
             rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
             ++launches;
         }
+        if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
         unpack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, w.S, (float2 *)d_Mxy, d_Mz);
         ++launches;
     }
-    if ((rc = taps.mark(0))) return rc;
+    if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;  // closing event
     if (plan->profiling) plan->event_kind.resize(taps.used);
     plan->last.launches = launches;
     BLOCH_CUDA(cudaGetLastError());
