@@ -86,7 +86,9 @@ static void grid_free(ref_grid *g) {
 /*
  * Time grid: sorted unique union of 0, t_end, gradient vertices, RF sample edges and ADC times, refined so
  * that no RF-covered interval exceeds dt_rf_max (an RF piece of length L is cut into ceil(L/dt_rf_max)
- * equal sub-steps, reading G18).  Returns 0 or a negative error.
+ * equal sub-steps, reading G18; L is taken with the time tolerance of reading G13, i.e. a piece is longer
+ * than dt_rf_max only if it exceeds it by more than 1e-12 s, so that the rounding of t_{n+1} - t_n late in a
+ * long sequence -- ulp(10 s) = 1.8e-15 s -- never splits a nominal dt_rf_max step).  Returns 0 or a negative error.
  */
 static int grid_build(ref_grid *g,
                       const double *const gt[3], const double *const gv[3], const int64_t gn[3],
@@ -118,7 +120,7 @@ static int grid_build(ref_grid *g,
         double a = raw[i], b = raw[i + 1];
         int64_t parts = 1;
         if (rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0 && dt_rf_max > 0.0)
-            parts = (int64_t)ceil((b - a) / dt_rf_max - 1e-9);
+            parts = (int64_t)ceil(((b - a) - REF_TOL_T) / dt_rf_max);
         if (parts < 1) parts = 1;
         total += parts;
     }
@@ -136,7 +138,7 @@ static int grid_build(ref_grid *g,
         double a = raw[i], b = raw[i + 1];
         int64_t parts = 1;
         if (rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0 && dt_rf_max > 0.0)
-            parts = (int64_t)ceil((b - a) / dt_rf_max - 1e-9);
+            parts = (int64_t)ceil(((b - a) - REF_TOL_T) / dt_rf_max);
         if (parts < 1) parts = 1;
         for (int64_t p = 1; p < parts; ++p) g->t[k++] = a + (b - a) * ((double)p / (double)parts);
         g->t[k++] = b;

@@ -8,6 +8,7 @@
 
 #include "internal.h"
 #include "kernels.cuh"
+#include "rf.cuh"
 
 namespace bloch {
 const char *last_error_cstr();
@@ -282,19 +283,22 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
 
     bool pending = false;
     PropRec prop{0, 0, 0, 0};
-    const int rf_grid = (n + kRfThreads - 1) / kRfThreads;
+    // RF launch shape: one spin per thread; small CTAs when spins are few so the warps spread over all
+    // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
+    const int rf_threads = env_int("BLOCH_RF_THREADS", (n + 31) / 32 >= sms * 32 ? 128 : 32);
+    const int rf_grid = (n + rf_threads - 1) / rf_threads;
     for (const Block &b : plan->blocks) {
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
-            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>((const float4 *)(plan->d_tables + b.table_off),
-                                                           (int)b.count, prop, pending ? 1 : 0, w.A, w.C, w.S, n);
+            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(plan->d_tables + b.table_off, (int)b.n_tiles, prop,
+                                                           pending ? 1 : 0, w.A, w.C, w.S, n);
             ++launches;
             pending = false;
             continue;
         }
         if (pending) {  // two precession blocks in a row: apply the first one's end transform now
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
             ++launches;
             pending = false;
         }
@@ -345,7 +349,7 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     if (d_Mxy) {
         if (pending) {
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, kRfThreads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
             ++launches;
         }
         if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;

@@ -14,7 +14,30 @@ constexpr int kBlockRF = 1;
 constexpr double kTimeTol = 1e-12;       // reading G13
 constexpr int64_t kDefaultMaxBlockPoints = int64_t(1) << 22;
 constexpr size_t kAlign = 256;
-constexpr int kRfStepFloats = 8;         // (wx, wy, gx, gy, gz, dt, 0, 0) per RF step
+
+// RF block table (a4), read by rf_kernel through 1-D bulk copies (TMA) tile by tile:
+//   [directory: n_tiles x {int32 byte offset from the block's table start, int32 bytes}, padded to 16 B]
+//   [tile 0][tile 1]...      tile = RfTileHdr (64 B) + n_steps records, 16-B aligned
+// A tile never mixes two step lengths dt (the planner cuts tiles where dt changes), so the relaxation
+// factors of Eq 11 are per-tile constants of a spin.  Records:
+//   compact (kRfFlagUniformG: gamma*dt*G identical for all steps of the tile, e.g. a slice-select plateau)
+//       16 B  (wx, wy, wx^2 + wy^2, 0)          wx + i wy = gamma * dt * B1 (Eq 8)
+//   general
+//       32 B  (wx, wy, wx^2 + wy^2, 0) (gx, gy, gz, 0)      g = gamma * dt * mean G of the step (reading G5)
+constexpr int kRfTileSteps = 128;
+constexpr int kRfHdrBytes = 64;
+constexpr int kRfTileBytesMax = kRfHdrBytes + kRfTileSteps * 32;
+constexpr int kRfFlagUniformG = 1;
+struct RfTileHdr {
+    float wxy2_max, gx_max, gy_max, gz_max;  // max over the tile's steps of wx^2+wy^2, |gx|, |gy|, |gz|
+    float dt;                                // step length [s], the same for every step of the tile
+    int32_t n_steps;
+    int32_t flags;
+    float pad0;
+    float gx, gy, gz, pad1;                  // the tile's gradient part when kRfFlagUniformG
+    float pad2[4];
+};
+static_assert(sizeof(RfTileHdr) == kRfHdrBytes, "RfTileHdr must be 64 B");
 
 // One block of the time axis: a maximal run of RF-active intervals (excitation regime) or
 // a run of RF-free intervals (precession regime), :132.
@@ -25,6 +48,7 @@ struct Block {
     int64_t adc_first = 0;    // precession: first ADC sample served, in ADC order
     int64_t adc_count = 0;    //             number of ADC samples served (= evaluated points of the signal kernel)
     int64_t table_off = 0;    // byte offset of this block's records in the table buffer
+    int64_t n_tiles = 0;      // RF: tiles in the block's table (see RfTileHdr)
     // precession block end record: k' = -gamma_bar * K(T) [turns/m] and tau = T [s] (Eq 12-13)
     double kend[3] = {0, 0, 0};
     double tau_end = 0;

@@ -76,101 +76,6 @@ __device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, con
 }
 
 // ------------------------------------------------------------------------------------------------
-// a8: RF (excitation) kernel.  One thread = one spin, state in registers for the whole block.
-//
-// Per step the Cayley-Klein rotation of Eq 6-9 is applied in its increment form.  With the rotation vector
-// w = gamma * (B1x, B1y, Bz) * dt (so phi = -|w| in Eq 8), alpha = cos(|w|/2) + i (wz/|w|) sin(|w|/2),
-// beta = i ((wx + i wy)/|w|) sin(|w|/2), and Eq 9 expanded in real components is identically
-//     M+ = M + a (w x M) + b (w x (w x M)),     a = -sin|w| / |w|,     b = (1 - cos|w|) / |w|^2
-// (tests/test_host_math.py checks the identity against Eq 9 numerically).  a and b
-// are even polynomials in |w|: no sqrt, no division, no 0/0 at |B| = 0 (reading G10), and the increment
-// never forms 1 - cos by cancellation (SURVEY.md hard parts H1/H2).  Relaxation (Eq 11) is applied after
-// the rotation in the same increment form with D = -expm1(-dt/T); the state is accumulated with Kahan
-// compensation so 1e6 tiny increments stay at fp32 round-off of the state, not of the sum.
-// ------------------------------------------------------------------------------------------------
-constexpr int kRfThreads = 64;
-constexpr int kRfTileSteps = 256;
-
-__device__ __forceinline__ void kahan_add(float &m, float &c, float d) {
-    const float yv = d - c;
-    const float t = m + yv;
-    c = (t - m) - yv;
-    m = t;
-}
-
-__global__ void __launch_bounds__(kRfThreads)
-rf_kernel(const float4 *__restrict__ steps, int n_steps, PropRec prop, int has_prop,
-          const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
-    __shared__ float4 tile[2 * kRfTileSteps];
-    const int i = blockIdx.x * kRfThreads + threadIdx.x;
-    const bool active = i < n;
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f),
-           s = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (active) {
-        a = A[i];
-        c = Cc[i];
-        s = S[i];
-    }
-    float mx = s.x, my = s.y, mz = s.z;
-    if (has_prop) propagate(prop, a, c, mx, my, mz);
-    float cx = 0.f, cy = 0.f, cz = 0.f;
-    float dt_prev = -1.f, D1 = 0.f, D2 = 0.f, E1 = 1.f, E2 = 1.f;
-    const float x = a.x, y = a.y, z = a.z, dw = c.w, m0 = c.z;
-
-    for (int base = 0; base < n_steps; base += kRfTileSteps) {
-        const int cnt = min(kRfTileSteps, n_steps - base);
-        __syncthreads();
-        for (int k = threadIdx.x; k < 2 * cnt; k += kRfThreads) tile[k] = steps[2 * base + k];
-        __syncthreads();
-#pragma unroll 2
-        for (int k = 0; k < cnt; ++k) {
-            const float4 u = tile[2 * k];      // (wx, wy, gx, gy)
-            const float4 v = tile[2 * k + 1];  // (gz, dt, -, -)
-            if (v.y != dt_prev) {              // warp-uniform: dt comes from the table
-                dt_prev = v.y;
-                D1 = -expm1f(-v.y * c.x);
-                D2 = -expm1f(-v.y * c.y);
-                E1 = 1.0f - D1;
-                E2 = 1.0f - D2;
-            }
-            const float wx = u.x, wy = u.y;
-            const float wz = fmaf(u.z, x, fmaf(u.w, y, fmaf(v.x, z, v.y * dw)));  // gamma Bz dt, Eq 2
-            const float q = fmaf(wx, wx, fmaf(wy, wy, wz * wz));                  // |w|^2
-            float ca, cb;
-            if (q <= 0.25f) {
-                // a = -sin(t)/t, b = (1-cos t)/t^2, t^2 = q <= 0.25: truncation < 2e-9
-                ca = -fmaf(q, fmaf(q, fmaf(q, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
-                cb = fmaf(q, fmaf(q, fmaf(q, -1.0f / 40320.0f, 1.0f / 720.0f), -1.0f / 24.0f), 0.5f);
-            } else {
-                const float t = sqrtf(q);
-                float sh, ch;
-                sincosf(0.5f * t, &sh, &ch);
-                ca = -2.0f * sh * ch / t;        // -sin t / t
-                cb = 2.0f * sh * sh / q;         // (1 - cos t) / t^2
-            }
-            // u1 = w x M, u2 = w x u1
-            const float ux = fmaf(wy, mz, -wz * my);
-            const float uy = fmaf(wz, mx, -wx * mz);
-            const float uz = fmaf(wx, my, -wy * mx);
-            const float vx = fmaf(wy, uz, -wz * uy);
-            const float vy = fmaf(wz, ux, -wx * uz);
-            const float vz = fmaf(wx, uy, -wy * ux);
-            const float dx = fmaf(ca, ux, cb * vx);   // rotation increment, Eq 9
-            const float dy = fmaf(ca, uy, cb * vy);
-            const float dz = fmaf(ca, uz, cb * vz);
-            // relaxation after rotation, Eq 11: M'' = E (M + d) (+ M0 D1) -> increment E d - D M (+ D1 M0)
-            const float tx = fmaf(E2, dx, -D2 * mx);
-            const float ty = fmaf(E2, dy, -D2 * my);
-            const float tz = fmaf(E1, dz, D1 * (m0 - mz));
-            kahan_add(mx, cx, tx);
-            kahan_add(my, cy, ty);
-            kahan_add(mz, cz, tz);
-        }
-    }
-    if (active) S[i] = make_float4(mx, my, mz, s.w);
-}
-
-// ------------------------------------------------------------------------------------------------
 // a6 + a7: free-precession signal kernel (SUM_ALL).
 //
 // Grid = (point tiles, spin chunks).  A thread OWNS P evaluated points (k', tau in registers) and walks the

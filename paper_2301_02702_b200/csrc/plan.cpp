@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstring>
 #include <limits>
+#include <utility>
 
 #include "internal.h"
 
@@ -132,7 +133,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             while (j < seq->rf_n && seq->rf_t[j] + seq->rf_dt[j] <= mid) ++j;
             const bool covered = (j < seq->rf_n && seq->rf_t[j] <= mid);
             int64_t parts = 1;
-            if (covered && std::isfinite(dt_rf)) parts = std::max<int64_t>(1, (int64_t)std::ceil((b - a) / dt_rf - 1e-9));
+            // a piece is longer than dt_rf_max only beyond the time tolerance (readings G13 + G18)
+            if (covered && std::isfinite(dt_rf)) parts = std::max<int64_t>(1, (int64_t)std::ceil(((b - a) - kTimeTol) / dt_rf));
             for (int64_t p = 1; p <= parts; ++p) {
                 t.push_back(p == parts ? b : a + (b - a) * (double(p) / double(parts)));
                 rf_of.push_back(covered ? j : -1);
@@ -239,13 +241,77 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     int phase = params->phase_mode;
     if (phase == BLOCH_PHASE_AUTO) phase = worst_turns > 256.0 ? BLOCH_PHASE_FP64 : BLOCH_PHASE_FP32;
 
+    // ------------------------------------------------------------------ a4: RF tile images
+    std::vector<std::vector<unsigned char>> rf_img(blocks.size());
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        Block &b = blocks[bi];
+        if (b.type != kBlockRF) continue;
+        // per step, in fp32 as the kernel sees them: rotation vector w = gamma * B * dt (Eq 8); the gradient
+        // part is per metre, mean of the two vertex values (reading G5)
+        struct StepF { float wx, wy, g[3], dt; };
+        std::vector<StepF> st((size_t)b.count);
+        for (int64_t n = b.first; n < b.first + b.count; ++n) {
+            const double dt = t[n + 1] - t[n];
+            const int64_t j = rf_of[n];
+            StepF &s = st[(size_t)(n - b.first)];
+            s.wx = (float)(gamma * dt * seq->rf_re[j]);
+            s.wy = (float)(gamma * dt * seq->rf_im[j]);
+            for (int a = 0; a < 3; ++a) s.g[a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]));
+            s.dt = (float)dt;
+        }
+        // cut into tiles: at most kRfTileSteps steps, one dt per tile
+        std::vector<std::pair<size_t, size_t>> tiles;  // (first, count)
+        for (size_t k = 0; k < st.size();) {
+            size_t c = 1;
+            while (k + c < st.size() && c < (size_t)kRfTileSteps && st[k + c].dt == st[k].dt) ++c;
+            tiles.emplace_back(k, c);
+            k += c;
+        }
+        b.n_tiles = (int64_t)tiles.size();
+        const size_t dir_bytes = align_up(tiles.size() * 8, 16);
+        std::vector<unsigned char> &img = rf_img[bi];
+        img.assign(dir_bytes, 0);
+        for (size_t ti = 0; ti < tiles.size(); ++ti) {
+            const size_t k0 = tiles[ti].first, c = tiles[ti].second;
+            RfTileHdr h;
+            std::memset(&h, 0, sizeof(h));
+            bool uniform = true;
+            for (size_t k = k0; k < k0 + c; ++k) {
+                const StepF &s = st[k];
+                h.wxy2_max = std::max(h.wxy2_max, s.wx * s.wx + s.wy * s.wy);
+                h.gx_max = std::max(h.gx_max, std::fabs(s.g[0]));
+                h.gy_max = std::max(h.gy_max, std::fabs(s.g[1]));
+                h.gz_max = std::max(h.gz_max, std::fabs(s.g[2]));
+                uniform = uniform && s.g[0] == st[k0].g[0] && s.g[1] == st[k0].g[1] && s.g[2] == st[k0].g[2];
+            }
+            h.dt = st[k0].dt;
+            h.n_steps = (int32_t)c;
+            h.flags = uniform ? kRfFlagUniformG : 0;
+            h.gx = st[k0].g[0]; h.gy = st[k0].g[1]; h.gz = st[k0].g[2];
+            const size_t rec = uniform ? 16 : 32;
+            const size_t off0 = img.size();
+            img.resize(off0 + kRfHdrBytes + c * rec, 0);
+            std::memcpy(img.data() + off0, &h, sizeof(h));
+            float *r = reinterpret_cast<float *>(img.data() + off0 + kRfHdrBytes);
+            for (size_t k = k0; k < k0 + c; ++k, r += rec / 4) {
+                const StepF &s = st[k];
+                r[0] = s.wx; r[1] = s.wy; r[2] = s.wx * s.wx + s.wy * s.wy; r[3] = 0.f;
+                if (!uniform) { r[4] = s.g[0]; r[5] = s.g[1]; r[6] = s.g[2]; r[7] = 0.f; }
+            }
+            int32_t *dir = reinterpret_cast<int32_t *>(img.data());
+            dir[2 * ti] = (int32_t)off0;
+            dir[2 * ti + 1] = (int32_t)(img.size() - off0);
+        }
+        if (img.size() > (size_t)INT32_MAX) return fail(BLOCH_EINVAL, "RF block table exceeds 2 GiB");
+    }
+
     // ------------------------------------------------------------------ tables: layout + fill
     size_t off = 0;
     const size_t rec_bytes = phase == BLOCH_PHASE_FP64 ? 32 : 16;
-    for (Block &b : blocks) {
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        Block &b = blocks[bi];
         b.table_off = (int64_t)off;
-        const size_t bytes = b.type == kBlockRF ? size_t(b.count) * kRfStepFloats * sizeof(float)
-                                                : size_t(b.adc_count) * rec_bytes;
+        const size_t bytes = b.type == kBlockRF ? rf_img[bi].size() : size_t(b.adc_count) * rec_bytes;
         off = align_up(off + bytes, kAlign);
     }
     if (off == 0) off = kAlign;
@@ -254,20 +320,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         const Block &b = blocks[bi];
         unsigned char *dst = plan->tables.data() + b.table_off;
         if (b.type == kBlockRF) {
-            float *r = reinterpret_cast<float *>(dst);
-            for (int64_t n = b.first; n < b.first + b.count; ++n, r += kRfStepFloats) {
-                const double dt = t[n + 1] - t[n];
-                const int64_t j = rf_of[n];
-                // rotation vector w = gamma * B * dt (Eq 8); gradient part is per-metre, mean of the two
-                // vertex values (reading G5)
-                r[0] = (float)(gamma * dt * seq->rf_re[j]);
-                r[1] = (float)(gamma * dt * seq->rf_im[j]);
-                for (int a = 0; a < 3; ++a)
-                    r[2 + a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]));
-                r[5] = (float)dt;
-                r[6] = 0.f;
-                r[7] = 0.f;
-            }
+            std::memcpy(dst, rf_img[bi].data(), rf_img[bi].size());
         } else {
             const double *src = krec.data() + 4 * krec_first[bi];
             if (phase == BLOCH_PHASE_FP64) {

@@ -1,0 +1,220 @@
+// rf.cuh -- a8: RF (excitation) kernel for sm_100a.  One thread = one spin; the magnetisation stays in
+// registers for the whole excitation block; the block's step table is streamed through shared memory tile
+// by tile with 1-D bulk copies (TMA) into a two-stage mbarrier ring and broadcast to all threads.
+//
+// Per step the Cayley-Klein rotation of Eq 6-9 is applied in its increment form.  With
+// the rotation vector w = gamma * (B1x, B1y, Bz) * dt (so phi = -|w| in Eq 8),
+//     alpha = cos(|w|/2) + i (wz/|w|) sin(|w|/2),   beta = i ((wx + i wy)/|w|) sin(|w|/2),
+// Eq 9 expanded in real components is identically
+//     M+ = M + a (w x M) + b (w x (w x M)),     a = -sin|w| / |w|,     b = (1 - cos|w|) / |w|^2
+// (tests/test_host_plan.py checks the identity against Eq 9 numerically).  a and b are even series in
+// q = |w|^2: no sqrt, no division, no 0/0 at |B| = 0 (reading G10), and 1 - cos is never formed by
+// cancellation (SURVEY.md hard parts H1/H2).  Relaxation (Eq 11, :160-163) follows the rotation in the same
+// increment form with D = -expm1(-dt/T):   M++ = M + [E d - D M (+ D1 M0 z)],  d the rotation increment.
+//
+// The work per step is chosen per tile and per warp from a bound on q (tile header maxima x the spin's own
+// |x|, |y|, |z|, |dw|), so the hot loops are branch-free:
+//   tier 0  q <= 2^-8 : series through q^2 (truncation < 1.2e-11), state carried as hi + lo with the
+//                       increments summed in lo and folded into hi every 8 steps (error-free Fast2Sum)
+//   tier 1  q <= 1/4  : series through q^3 (truncation < 1.1e-8), Kahan-compensated state
+//   tier 2  otherwise : sqrt + sincos per step where needed, Kahan-compensated state
+// Tiles whose gradient part is the same for every step (compact records) hoist wz out of the step loop.
+#pragma once
+#include "internal.h"
+#include "tma.cuh"
+
+namespace bloch {
+
+struct RfSpin {
+    float x, y, z, dw, r1, r2, m0;
+};
+struct RfRelax {
+    float E1, E2, D1, D2, D1m0;
+};
+
+template <int TIER>
+__device__ __forceinline__ void rf_series(float q, float &ca, float &cb) {
+    if (TIER == 0) {
+        ca = fmaf(q, fmaf(q, -1.0f / 120.0f, 1.0f / 6.0f), -1.0f);
+        cb = fmaf(q, fmaf(q, 1.0f / 720.0f, -1.0f / 24.0f), 0.5f);
+    } else if (TIER == 1) {
+        ca = fmaf(q, fmaf(q, fmaf(q, 1.0f / 5040.0f, -1.0f / 120.0f), 1.0f / 6.0f), -1.0f);
+        cb = fmaf(q, fmaf(q, fmaf(q, -1.0f / 40320.0f, 1.0f / 720.0f), -1.0f / 24.0f), 0.5f);
+    } else {
+        if (q <= 0.25f) {
+            ca = fmaf(q, fmaf(q, fmaf(q, 1.0f / 5040.0f, -1.0f / 120.0f), 1.0f / 6.0f), -1.0f);
+            cb = fmaf(q, fmaf(q, fmaf(q, -1.0f / 40320.0f, 1.0f / 720.0f), -1.0f / 24.0f), 0.5f);
+        } else {
+            const float t = sqrtf(q);
+            float sh, ch;
+            sincosf(0.5f * t, &sh, &ch);
+            ca = -2.0f * sh * ch / t;  // -sin t / t
+            cb = 2.0f * sh * sh / q;   // (1 - cos t) / t^2
+        }
+    }
+}
+
+// increment of one step (rotation Eq 9, then relaxation Eq 11) for the state (mx, my, mz)
+template <int TIER>
+__device__ __forceinline__ void rf_increment(float wx, float wy, float wz, float q, float mx, float my, float mz,
+                                             const RfRelax &r, float &tx, float &ty, float &tz) {
+    float ca, cb;
+    rf_series<TIER>(q, ca, cb);
+    const float ux = fmaf(wy, mz, -wz * my);  // u = w x M
+    const float uy = fmaf(wz, mx, -wx * mz);
+    const float uz = fmaf(wx, my, -wy * mx);
+    const float vx = fmaf(wy, uz, -wz * uy);  // v = w x u
+    const float vy = fmaf(wz, ux, -wx * uz);
+    const float vz = fmaf(wx, uy, -wy * ux);
+    const float dx = fmaf(ca, ux, cb * vx);
+    const float dy = fmaf(ca, uy, cb * vy);
+    const float dz = fmaf(ca, uz, cb * vz);
+    tx = fmaf(r.E2, dx, -r.D2 * mx);
+    ty = fmaf(r.E2, dy, -r.D2 * my);
+    tz = fmaf(r.E1, dz, fmaf(-r.D1, mz, r.D1m0));
+}
+
+__device__ __forceinline__ void kahan_add(float &m, float &c, float d) {
+    const float yv = d - c;
+    const float t = m + yv;
+    c = (t - m) - yv;
+    m = t;
+}
+
+// hi <- fl(hi + lo), lo <- the rounding error of that sum (Fast2Sum; |lo| << |hi| here, and where it is not
+// the residual is below an ulp of lo)
+__device__ __forceinline__ void fold(float &hi, float &lo) {
+    const float s = hi + lo;
+    lo -= (s - hi);
+    hi = s;
+}
+
+// One tile of steps.  State in and out as (h, l) with h + l the magnetisation.
+template <int TIER, bool UG>
+__device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileHdr &hd, const RfSpin &sp,
+                                        const RfRelax &rx, float &hx, float &hy, float &hz, float &lx, float &ly,
+                                        float &lz) {
+    const float4 *rec = reinterpret_cast<const float4 *>(tile + kRfHdrBytes);
+    const int n = hd.n_steps;
+    const float dtdw = hd.dt * sp.dw;
+    // Eq 2: gamma Bz dt = g . x + dw dt
+    const float wz_u = fmaf(hd.gx, sp.x, fmaf(hd.gy, sp.y, fmaf(hd.gz, sp.z, dtdw)));
+    const float wz2_u = wz_u * wz_u;
+#define BLOCH_RF_LOAD(k)                                                              \
+    float wx, wy, wz, q;                                                              \
+    if (UG) {                                                                         \
+        const float4 a = rec[k];                                                      \
+        wx = a.x; wy = a.y; wz = wz_u; q = a.z + wz2_u;                               \
+    } else {                                                                          \
+        const float4 a = rec[2 * (k)], g = rec[2 * (k) + 1];                          \
+        wx = a.x; wy = a.y;                                                           \
+        wz = fmaf(g.x, sp.x, fmaf(g.y, sp.y, fmaf(g.z, sp.z, dtdw)));                 \
+        q = fmaf(wz, wz, a.z);                                                        \
+    }
+    if (TIER == 0) {
+        int k = 0;
+        for (; k + 8 <= n; k += 8) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                BLOCH_RF_LOAD(k + j)
+                float tx, ty, tz;
+                rf_increment<0>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, tx, ty, tz);
+                lx += tx; ly += ty; lz += tz;
+            }
+            fold(hx, lx); fold(hy, ly); fold(hz, lz);
+        }
+        for (; k < n; ++k) {
+            BLOCH_RF_LOAD(k)
+            float tx, ty, tz;
+            rf_increment<0>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, tx, ty, tz);
+            lx += tx; ly += ty; lz += tz;
+        }
+        fold(hx, lx); fold(hy, ly); fold(hz, lz);
+    } else {
+        float cx = -lx, cy = -ly, cz = -lz;  // Kahan carries the negated low part
+#pragma unroll 4
+        for (int k = 0; k < n; ++k) {
+            BLOCH_RF_LOAD(k)
+            float tx, ty, tz;
+            rf_increment<TIER>(wx, wy, wz, q, hx, hy, hz, rx, tx, ty, tz);
+            kahan_add(hx, cx, tx);
+            kahan_add(hy, cy, ty);
+            kahan_add(hz, cz, tz);
+        }
+        lx = -cx; ly = -cy; lz = -cz;
+    }
+#undef BLOCH_RF_LOAD
+}
+
+constexpr int kRfMaxThreads = 128;
+
+__global__ void __launch_bounds__(kRfMaxThreads)
+rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int has_prop,
+          const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
+    __shared__ __align__(128) unsigned char buf[2][kRfTileBytesMax];
+    __shared__ __align__(8) uint64_t bar[2];
+    const int tid = threadIdx.x;
+    const int2 *dir = reinterpret_cast<const int2 *>(tbl);
+    if (tid == 0 && n_tiles > 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init_fence();
+        for (int b = 0; b < 2 && b < n_tiles; ++b) {
+            const int2 d = dir[b];
+            mbar_expect_tx(&bar[b], (uint32_t)d.y);
+            bulk_g2s(buf[b], tbl + d.x, (uint32_t)d.y, &bar[b]);
+        }
+    }
+    const int i = blockIdx.x * blockDim.x + tid;
+    const bool active = i < n;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f),
+           s = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (active) {
+        a = A[i];
+        c = Cc[i];
+        s = S[i];
+    }
+    float hx = s.x, hy = s.y, hz = s.z;
+    if (has_prop) propagate(prop, a, c, hx, hy, hz);
+    float lx = 0.f, ly = 0.f, lz = 0.f;
+    const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z};
+    const float ax = fabsf(sp.x), ay = fabsf(sp.y), az = fabsf(sp.z), adw = fabsf(sp.dw);
+    __syncthreads();  // barrier initialisation visible to every waiter
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int b = t & 1;
+        mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
+        const unsigned char *tile = buf[b];
+        const RfTileHdr hd = *reinterpret_cast<const RfTileHdr *>(tile);
+        RfRelax rx;
+        rx.D1 = -expm1f(-hd.dt * sp.r1);
+        rx.D2 = -expm1f(-hd.dt * sp.r2);
+        rx.E1 = 1.0f - rx.D1;
+        rx.E2 = 1.0f - rx.D2;
+        rx.D1m0 = rx.D1 * sp.m0;
+        // bound on q = |w|^2 over the tile for this spin -> tier, decided per warp
+        const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
+        const float qb = fmaf(wzb, wzb, hd.wxy2_max);
+        const bool ug = (hd.flags & kRfFlagUniformG) != 0;
+        const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
+        if (tier == 0) {
+            if (ug) rf_tile<0, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+            else rf_tile<0, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        } else if (tier == 1) {
+            if (ug) rf_tile<1, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+            else rf_tile<1, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        } else {
+            if (ug) rf_tile<2, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+            else rf_tile<2, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        }
+        __syncthreads();  // every thread is done reading buf[b]
+        if (tid == 0 && t + 2 < n_tiles) {
+            const int2 d = dir[t + 2];
+            mbar_expect_tx(&bar[b], (uint32_t)d.y);
+            bulk_g2s(buf[b], tbl + d.x, (uint32_t)d.y, &bar[b]);
+        }
+    }
+    if (active) S[i] = make_float4(hx + lx, hy + ly, hz + lz, s.w);
+}
+
+}  // namespace bloch
