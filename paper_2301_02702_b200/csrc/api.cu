@@ -9,6 +9,7 @@
 #include "internal.h"
 #include "kernels.cuh"
 #include "rf.cuh"
+#include "signal.cuh"
 
 namespace bloch {
 const char *last_error_cstr();
@@ -54,7 +55,7 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
     s.P = forceP ? forceP : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1));
     if (s.P != 1 && s.P != 2 && s.P != 4) s.P = 1;
     s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
-    const int per_sm = env_int("BLOCH_SIGNAL_CTAS_PER_SM", 2);
+    const int per_sm = env_int("BLOCH_SIGNAL_CTAS_PER_SM", 4);
     const int64_t target = (int64_t)sm_count * per_sm;
     int64_t chunks = (target + s.ptiles - 1) / s.ptiles;
     const int64_t max_chunks = (n_spins + 31) / 32;
@@ -79,6 +80,7 @@ int max_chunks_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 
 struct Workspace {
     float4 *A, *C, *S;
+    double4 *Ad;  // fp64-phase plans only
     float2 *partial;
     size_t bytes;
 };
@@ -106,6 +108,7 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.A = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.C = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.S = (float4 *)take(size_t(n_spins) * sizeof(float4));
+    w.Ad = plan->info.phase_mode == BLOCH_PHASE_FP64 ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL)
         pbytes = size_t(max_chunks_for(plan, n_spins, sm_count)) * sizeof(float2);
@@ -278,7 +281,7 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
     pack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw,
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
-                                                     w.A, w.C, w.S);
+                                                     w.A, w.C, w.S, w.Ad);
     ++launches;
 
     bool pending = false;
@@ -324,11 +327,11 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
 #define BLOCH_LAUNCH_SIG(PP)                                                                                   \
     do {                                                                                                       \
         if (ph64)                                                                                              \
-            signal_kernel_f64<PP><<<grid, kSigThreads, 0, stream>>>((const double4 *)recs, n_pts, w.A, w.C,    \
-                                                                    w.S, n, s.spins_per_chunk, w.partial);     \
+            signal_kernel<PP, true><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.Ad, w.S, n,               \
+                                                                      s.spins_per_chunk, w.partial);           \
         else                                                                                                   \
-            signal_kernel_f32<PP><<<grid, kSigThreads, 0, stream>>>((const float4 *)recs, n_pts, w.A, w.S, n,  \
-                                                                    s.spins_per_chunk, w.partial);             \
+            signal_kernel<PP, false><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.A, w.S, n,               \
+                                                                       s.spins_per_chunk, w.partial);          \
     } while (0)
                 if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);

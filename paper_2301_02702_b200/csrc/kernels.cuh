@@ -1,12 +1,14 @@
 // kernels.cuh -- device code of the hot path for sm_100a.
 //
-// Internal spin layout (built once per bloch_simulate by pack_kernel, 48 B per spin):
-//   A[i] = (x, y, z, f')        f' = -dw / (2 pi)  [turns/s]     constant
+// Internal spin layout (built once per bloch_simulate by pack_kernel, 48 B per spin; +32 B with fp64 phase):
+//   A[i] = (x, y, z, f')        f' = -dw  [rad/s]                  constant
+//   Ad[i] = (x, y, z, f') as doubles, f' = -dw / (2 pi) [turns/s]  constant, fp64-phase plans only
 //   C[i] = (1/T1, 1/T2, M0, dw)                                   constant
 //   S[i] = (Mxy.re, Mxy.im, Mz, e2)   e2 = -(1/T2) log2(e)        state (e2 rides along for the signal kernel)
 //
 // Phase convention (reading G3): Mxy(t) = Mxy(0) exp(-t/T2) exp(-i (2 pi gamma_bar K.x + dw t)); the tables
-// hold k' = -gamma_bar K [turns/m] so that the phase in turns is theta = k'.x + f' tau.
+// hold k' = -gamma K [rad/m] (fp32 phase) or -gamma_bar K [turns/m] (fp64 phase, block-end records), so that
+// the phase is theta = k'.x + f' tau.
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -17,6 +19,12 @@ constexpr float kInv2Pi = 0.15915494309189535f;
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kLog2e = 1.4426950408889634f;
 
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // ------------------------------------------------------------------------------------------------
 // a5: spin state init / pack, and a9: unpack
 // ------------------------------------------------------------------------------------------------
@@ -25,11 +33,12 @@ __global__ void pack_kernel(int n, const float *__restrict__ x, const float *__r
                             const float *__restrict__ T1, const float *__restrict__ T2,
                             const float *__restrict__ dw, const float2 *__restrict__ Mxy,
                             const float *__restrict__ Mz, int init_eq, float4 *__restrict__ A,
-                            float4 *__restrict__ Cc, float4 *__restrict__ S) {
+                            float4 *__restrict__ Cc, float4 *__restrict__ S, double4 *__restrict__ Ad) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float r1 = 1.0f / T1[i], r2 = 1.0f / T2[i], m0 = M0[i], w = dw[i];
-    A[i] = make_float4(x[i], y[i], z[i], -w * kInv2Pi);
+    A[i] = make_float4(x[i], y[i], z[i], -w);
+    if (Ad) Ad[i] = make_double4((double)x[i], (double)y[i], (double)z[i], -(double)w * 0.15915494309189535);
     Cc[i] = make_float4(r1, r2, m0, w);
     float4 s;
     if (init_eq) {
@@ -75,172 +84,6 @@ __device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, con
     mz = c.z + (mz - c.z) * e1;  // Eq 11
 }
 
-// ------------------------------------------------------------------------------------------------
-// a6 + a7: free-precession signal kernel (SUM_ALL).
-//
-// Grid = (point tiles, spin chunks).  A thread OWNS P evaluated points (k', tau in registers) and walks the
-// spins of its chunk, which are staged through shared memory and broadcast to all threads (every lane
-// reads the same address: conflict-free LDS.128).  The sum over spins is therefore thread-local: no
-// shuffles, no atomics.  Each CTA writes its partial sums P[chunk][point]; reduce_kernel adds the chunks
-// in index order (deterministic two-pass reduction, "add them later").
-// Per evaluation: 4 FMA phase, 3 ops range reduction to [-1/2, 1/2] turns, MUFU sin + cos, MUFU ex2,
-// 2 mul + 4 FMA complex multiply-accumulate.
-// ------------------------------------------------------------------------------------------------
-constexpr int kSigThreads = 256;
-
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-template <int P>
-__global__ void __launch_bounds__(kSigThreads)
-signal_kernel_f32(const float4 *__restrict__ recs, int n_pts, const float4 *__restrict__ A,
-                  const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
-                  float2 *__restrict__ partial) {
-    __shared__ float4 shA[kSigThreads];
-    __shared__ float4 shB[kSigThreads];
-    const int tid = threadIdx.x;
-    const int p0 = blockIdx.x * (kSigThreads * P) + tid;
-    float kx[P], ky[P], kz[P], tau[P], ar[P], ai[P];
-#pragma unroll
-    for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
-        const float4 r = p < n_pts ? recs[p] : make_float4(0.f, 0.f, 0.f, 0.f);
-        kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
-        ar[j] = 0.f; ai[j] = 0.f;
-    }
-    const int s0 = blockIdx.y * spins_per_chunk;
-    const int s1 = min(n_spins, s0 + spins_per_chunk);
-    for (int base = s0; base < s1; base += kSigThreads) {
-        __syncthreads();
-        {
-            const int idx = base + tid;
-            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-            if (idx < s1) {
-                a = A[idx];
-                const float4 st = S[idx];
-                b = make_float4(st.w, st.x, st.y, 0.f);
-            }
-            shA[tid] = a;
-            shB[tid] = b;
-        }
-        __syncthreads();
-        const int cnt = min(kSigThreads, s1 - base);
-#pragma unroll 2
-        for (int s = 0; s < cnt; ++s) {
-            const float4 a = shA[s];
-            const float4 b = shB[s];
-#pragma unroll
-            for (int j = 0; j < P; ++j) {
-                float th = fmaf(kx[j], a.x, fmaf(ky[j], a.y, fmaf(kz[j], a.z, tau[j] * a.w)));
-                th -= (th + 12582912.0f) - 12582912.0f;          // th - rint(th): [-1/2, 1/2] turns
-                const float ang = th * kTwoPi;
-                const float sn = __sinf(ang), cs = __cosf(ang);  // MUFU.SIN / MUFU.COS
-                const float e = ex2_approx(tau[j] * b.x);        // MUFU.EX2: exp(-tau/T2)
-                const float er = b.y * e, ei = b.z * e;
-                ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
-                ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
-            }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
-        if (p < n_pts) partial[(size_t)blockIdx.y * n_pts + p] = make_float2(ar[j], ai[j]);
-    }
-}
-
-// fp64 phase accumulation (north_star item 4): k', tau, x, f' in double; the fractional turn goes to
-// fp32 for MUFU sin/cos.  4 DFMA + 3 DADD + 1 F2F per evaluation on top of the fp32 work.
-template <int P>
-__global__ void __launch_bounds__(kSigThreads)
-signal_kernel_f64(const double4 *__restrict__ recs, int n_pts, const float4 *__restrict__ A,
-                  const float4 *__restrict__ Cc, const float4 *__restrict__ S, int n_spins,
-                  int spins_per_chunk, float2 *__restrict__ partial) {
-    __shared__ double4 shA[kSigThreads];
-    __shared__ float4 shB[kSigThreads];
-    const int tid = threadIdx.x;
-    const int p0 = blockIdx.x * (kSigThreads * P) + tid;
-    double kx[P], ky[P], kz[P], tau[P];
-    float tf[P], ar[P], ai[P];
-#pragma unroll
-    for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
-        const double4 r = p < n_pts ? recs[p] : make_double4(0., 0., 0., 0.);
-        kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
-        tf[j] = (float)r.w;
-        ar[j] = 0.f; ai[j] = 0.f;
-    }
-    const int s0 = blockIdx.y * spins_per_chunk;
-    const int s1 = min(n_spins, s0 + spins_per_chunk);
-    for (int base = s0; base < s1; base += kSigThreads) {
-        __syncthreads();
-        {
-            const int idx = base + tid;
-            double4 a = make_double4(0., 0., 0., 0.);
-            float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (idx < s1) {
-                const float4 af = A[idx];
-                const float4 st = S[idx];
-                a = make_double4((double)af.x, (double)af.y, (double)af.z,
-                                 -(double)Cc[idx].w * 0.15915494309189535);
-                b = make_float4(st.w, st.x, st.y, 0.f);
-            }
-            shA[tid] = a;
-            shB[tid] = b;
-        }
-        __syncthreads();
-        const int cnt = min(kSigThreads, s1 - base);
-        for (int s = 0; s < cnt; ++s) {
-            const double4 a = shA[s];
-            const float4 b = shB[s];
-#pragma unroll
-            for (int j = 0; j < P; ++j) {
-                double th = fma(kx[j], a.x, fma(ky[j], a.y, fma(kz[j], a.z, tau[j] * a.w)));
-                th -= (th + 6755399441055744.0) - 6755399441055744.0;   // th - rint(th)
-                const float ang = (float)th * kTwoPi;
-                const float sn = __sinf(ang), cs = __cosf(ang);
-                const float e = ex2_approx(tf[j] * b.x);
-                const float er = b.y * e, ei = b.z * e;
-                ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
-                ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
-            }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
-        if (p < n_pts) partial[(size_t)blockIdx.y * n_pts + p] = make_float2(ar[j], ai[j]);
-    }
-}
-
-// Second pass of a7: fixed-order sum over the spin chunks.  blockDim = (32, 8): x = point, y = chunk lane.
-__global__ void __launch_bounds__(256)
-reduce_kernel(const float2 *__restrict__ partial, int n_chunks, int n_pts, float2 *__restrict__ out) {
-    __shared__ float2 sh[8][33];
-    const int p = blockIdx.x * 32 + threadIdx.x;
-    float re = 0.f, im = 0.f;
-    if (p < n_pts) {
-        for (int c = threadIdx.y; c < n_chunks; c += 8) {
-            const float2 v = partial[(size_t)c * n_pts + p];
-            re += v.x;
-            im += v.y;
-        }
-    }
-    sh[threadIdx.y][threadIdx.x] = make_float2(re, im);
-    __syncthreads();
-    if (threadIdx.y == 0 && p < n_pts) {
-#pragma unroll
-        for (int k = 1; k < 8; ++k) {
-            re += sh[k][threadIdx.x].x;
-            im += sh[k][threadIdx.x].y;
-        }
-        out[p] = make_float2(re, im);
-    }
-}
-
 // PER_SPIN output (dictionary mode): one thread per (spin, point); accurate functions because nothing
 // averages the per-evaluation error; phase in fp64 turns.  recs are float4 or double4 by PH64.
 template <bool PH64>
@@ -256,8 +99,9 @@ perspin_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restri
         const double4 r = reinterpret_cast<const double4 *>(recs_)[p];
         kx = r.x; ky = r.y; kz = r.z; tau = r.w;
     } else {
-        const float4 r = reinterpret_cast<const float4 *>(recs_)[p];
-        kx = r.x; ky = r.y; kz = r.z; tau = r.w;
+        const float4 r = reinterpret_cast<const float4 *>(recs_)[p];  // fp32-phase tables hold k' in rad/m
+        kx = (double)r.x * 0.15915494309189535; ky = (double)r.y * 0.15915494309189535;
+        kz = (double)r.z * 0.15915494309189535; tau = r.w;
     }
     const float4 a = A[sp], c = Cc[sp], s = S[sp];
     double th = kx * (double)a.x + ky * (double)a.y + kz * (double)a.z - (double)c.w * 0.15915494309189535 * tau;

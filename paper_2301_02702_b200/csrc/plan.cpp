@@ -326,8 +326,10 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             if (phase == BLOCH_PHASE_FP64) {
                 std::memcpy(dst, src, size_t(b.adc_count) * 32);
             } else {
+                // fp32 phase: k' in rad/m (the signal kernel's phase is in radians), tau in s
                 float *r = reinterpret_cast<float *>(dst);
-                for (int64_t i = 0; i < 4 * b.adc_count; ++i) r[i] = (float)src[i];
+                for (int64_t i = 0; i < 4 * b.adc_count; ++i)
+                    r[i] = (float)((i & 3) == 3 ? src[i] : 2.0 * M_PI * src[i]);
             }
         }
     }

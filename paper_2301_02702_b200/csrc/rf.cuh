@@ -21,6 +21,7 @@
 // Tiles whose gradient part is the same for every step (compact records) hoist wz out of the step loop.
 #pragma once
 #include "internal.h"
+#include "kernels.cuh"
 #include "tma.cuh"
 
 namespace bloch {

@@ -1,0 +1,147 @@
+// signal.cuh -- a6 + a7: free-precession signal kernels (SUM_ALL) for sm_100a.
+//
+// Free precession is evaluated in closed form from the block start (Eq 10-11, are diagonal
+// in (Mxy, Mz) and commute, so the step-by-step product collapses exactly; :132 "exact solution"):
+//     c_in = Mxy_i(0) * exp(-tau_n / T2_i) * exp(i theta_in),    theta_in = k'_n . x_i + f'_i tau_n
+// with k' = -gamma K(t) the cumulative gradient moment of the block (Eq 12-13, :173-180) and f' = -dw.
+//
+// Grid = (point tiles, spin chunks).  A thread OWNS P evaluated points (k', tau in registers) and walks the
+// spins of its chunk.  Spin tiles (x, y, z, f') and (Mxy, e2) are staged global -> shared by 1-D bulk copies
+// (TMA) into a two-stage mbarrier ring by one elected thread and then broadcast to all threads (every lane
+// reads the same address: conflict-free LDS.128).  The sum over spins is therefore thread-local: no
+// shuffles, no atomics.  Each CTA writes its partial sums P[chunk][point]; reduce_kernel adds the chunks in
+// index order (deterministic two-pass reduction, :194 "add them later").
+//
+// fp32 phase: tables and f' in radians; per evaluation 4 FMA (phase), 1 FMUL (MUFU pre-scale to turns),
+// MUFU sin + cos, 1 FMUL + MUFU ex2 (T2 decay), 2 FMUL + 4 FMA (complex multiply-accumulate) = 15 issue
+// slots, 3 of them on the 16-lane MUFU pipe -- the bound.  No explicit range reduction: MUFU.SIN/COS take
+// their argument in turns and wrap it themselves; the planner keeps |theta| below 256 turns in this mode,
+// where the fp32 rounding of theta (~1e-4 rad) is already the error floor.
+// fp64 phase (north_star item 4): k', tau, x, f' in double, theta in turns by 4 DFMA; adding 1.5 * 2^20
+// leaves frac(theta) as a 32-bit fixed-point number in the low word of the double, which is turned into a
+// float in [0, 1) with two integer ops and one FADD -- no F2F (it would be a fourth op on the MUFU pipe).
+#pragma once
+#include <type_traits>
+
+#include "internal.h"
+#include "kernels.cuh"
+#include "tma.cuh"
+
+namespace bloch {
+
+constexpr int kSigThreads = 256;
+constexpr int kSigTile = 256;  // spins per staged tile
+
+template <int P, bool PH64>
+__global__ void __launch_bounds__(kSigThreads)
+signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
+              const float4 *__restrict__ S, int n_spins, int spins_per_chunk, float2 *__restrict__ partial) {
+    using RecT = typename std::conditional<PH64, double4, float4>::type;   // (k'x, k'y, k'z, tau)
+    using PosT = typename std::conditional<PH64, double4, float4>::type;   // (x, y, z, f')
+    using real = typename std::conditional<PH64, double, float>::type;
+    __shared__ __align__(128) PosT shA[2][kSigTile];
+    __shared__ __align__(128) float4 shS[2][kSigTile];
+    __shared__ __align__(8) uint64_t bar[2];
+    const RecT *recs = reinterpret_cast<const RecT *>(recs_);
+    const PosT *A = reinterpret_cast<const PosT *>(A_);
+    const int tid = threadIdx.x;
+    const int s0 = blockIdx.y * spins_per_chunk;
+    const int s1 = min(n_spins, s0 + spins_per_chunk);
+    const int n_tiles = (s1 - s0 + kSigTile - 1) / kSigTile;
+    auto issue = [&](int t) {
+        const int b = t & 1;
+        const int base = s0 + t * kSigTile;
+        const uint32_t cnt = (uint32_t)min(kSigTile, s1 - base);
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + sizeof(float4)));
+        bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
+        bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
+    };
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init_fence();
+        if (n_tiles > 0) issue(0);
+        if (n_tiles > 1) issue(1);
+    }
+    const int p0 = blockIdx.x * (kSigThreads * P) + tid;
+    real kx[P], ky[P], kz[P], tau[P];
+    float tf[P], ar[P], ai[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        const int p = p0 + j * kSigThreads;
+        RecT r;
+        r.x = 0; r.y = 0; r.z = 0; r.w = 0;
+        if (p < n_pts) r = recs[p];
+        kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
+        tf[j] = (float)r.w;
+        ar[j] = 0.f; ai[j] = 0.f;
+    }
+    __syncthreads();  // barrier initialisation visible to every waiter
+    for (int t = 0; t < n_tiles; ++t) {
+        const int b = t & 1;
+        mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
+        const int cnt = min(kSigTile, s1 - (s0 + t * kSigTile));
+#pragma unroll 2
+        for (int s = 0; s < cnt; ++s) {
+            const PosT a = shA[b][s];
+            const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                float sn, cs;
+                if (PH64) {
+                    double th = fma((double)kx[j], (double)a.x, fma((double)ky[j], (double)a.y,
+                                    fma((double)kz[j], (double)a.z, (double)tau[j] * (double)a.w)));  // turns
+                    th += 1572864.0;  // 1.5 * 2^20: ulp = 2^-32, low word = frac(theta) in 0.32 fixed point
+                    const unsigned lo = (unsigned)__double2loint(th);
+                    const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;  // [0, 1) turns
+                    const float ang = fr * 6.283185307179586f;
+                    sn = __sinf(ang);
+                    cs = __cosf(ang);
+                } else {
+                    const float th = fmaf((float)kx[j], (float)a.x, fmaf((float)ky[j], (float)a.y,
+                                          fmaf((float)kz[j], (float)a.z, (float)tau[j] * (float)a.w)));  // radians
+                    sn = __sinf(th);  // FMUL by 1/(2 pi) + MUFU.SIN
+                    cs = __cosf(th);
+                }
+                const float e = ex2_approx(tf[j] * st.w);  // MUFU.EX2: exp(-tau/T2)
+                const float er = st.x * e, ei = st.y * e;
+                ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
+                ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
+            }
+        }
+        __syncthreads();  // every thread is done with stage b
+        if (tid == 0 && t + 2 < n_tiles) issue(t + 2);
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        const int p = p0 + j * kSigThreads;
+        if (p < n_pts) partial[(size_t)blockIdx.y * n_pts + p] = make_float2(ar[j], ai[j]);
+    }
+}
+
+// Second pass of a7: fixed-order sum over the spin chunks.  blockDim = (32, 8): x = point, y = chunk lane.
+__global__ void __launch_bounds__(256)
+reduce_kernel(const float2 *__restrict__ partial, int n_chunks, int n_pts, float2 *__restrict__ out) {
+    __shared__ float2 sh[8][33];
+    const int p = blockIdx.x * 32 + threadIdx.x;
+    float re = 0.f, im = 0.f;
+    if (p < n_pts) {
+        for (int c = threadIdx.y; c < n_chunks; c += 8) {
+            const float2 v = partial[(size_t)c * n_pts + p];
+            re += v.x;
+            im += v.y;
+        }
+    }
+    sh[threadIdx.y][threadIdx.x] = make_float2(re, im);
+    __syncthreads();
+    if (threadIdx.y == 0 && p < n_pts) {
+#pragma unroll
+        for (int k = 1; k < 8; ++k) {
+            re += sh[k][threadIdx.x].x;
+            im += sh[k][threadIdx.x].y;
+        }
+        out[p] = make_float2(re, im);
+    }
+}
+
+}  // namespace bloch
