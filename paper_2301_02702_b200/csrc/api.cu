@@ -80,7 +80,8 @@ int max_chunks_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 
 struct Workspace {
     float4 *A, *C, *S;
-    double4 *Ad;  // fp64-phase plans only
+    double4 *Ad;     // fp64-phase plans only
+    unsigned *scal;  // device scalars: [0] = max 1/T2 (float bits)
     float2 *partial;
     size_t bytes;
 };
@@ -109,6 +110,7 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.C = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.S = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.Ad = plan->info.phase_mode == BLOCH_PHASE_FP64 ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
+    w.scal = (unsigned *)take(kAlign);
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL)
         pbytes = size_t(max_chunks_for(plan, n_spins, sm_count)) * sizeof(float2);
@@ -279,9 +281,10 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     Taps taps{plan, stream};
     int64_t launches = 0;
     if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
+    BLOCH_CUDA(cudaMemsetAsync(w.scal, 0, kAlign, stream));
     pack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw,
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
-                                                     w.A, w.C, w.S, w.Ad);
+                                                     w.A, w.C, w.S, w.Ad, w.scal);
     ++launches;
 
     bool pending = false;
@@ -328,10 +331,10 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     do {                                                                                                       \
         if (ph64)                                                                                              \
             signal_kernel<PP, true><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.Ad, w.S, n,               \
-                                                                      s.spins_per_chunk, w.partial);           \
+                                                                      s.spins_per_chunk, (const float *)w.scal, w.partial);           \
         else                                                                                                   \
             signal_kernel<PP, false><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.A, w.S, n,               \
-                                                                       s.spins_per_chunk, w.partial);          \
+                                                                       s.spins_per_chunk, (const float *)w.scal, w.partial);          \
     } while (0)
                 if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);

@@ -33,8 +33,15 @@ __global__ void pack_kernel(int n, const float *__restrict__ x, const float *__r
                             const float *__restrict__ T1, const float *__restrict__ T2,
                             const float *__restrict__ dw, const float2 *__restrict__ Mxy,
                             const float *__restrict__ Mz, int init_eq, float4 *__restrict__ A,
-                            float4 *__restrict__ Cc, float4 *__restrict__ S, double4 *__restrict__ Ad) {
+                            float4 *__restrict__ Cc, float4 *__restrict__ S, double4 *__restrict__ Ad,
+                            unsigned *__restrict__ scal) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    // scal[0] = max 1/T2 over the spins.  The bit pattern of a non-negative float orders like the unsigned
+    // integer and an integer max is order-independent, so this stays reproducible.
+    float r2w = i < n ? 1.0f / T2[i] : 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r2w = fmaxf(r2w, __shfl_xor_sync(0xffffffffu, r2w, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(scal, __float_as_uint(fmaxf(r2w, 0.f)));
     if (i >= n) return;
     const float r1 = 1.0f / T1[i], r2 = 1.0f / T2[i], m0 = M0[i], w = dw[i];
     A[i] = make_float4(x[i], y[i], z[i], -w);

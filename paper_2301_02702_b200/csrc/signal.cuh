@@ -35,7 +35,8 @@ constexpr int kSigTile = 256;  // spins per staged tile
 template <int P, bool PH64>
 __global__ void __launch_bounds__(kSigThreads)
 signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
-              const float4 *__restrict__ S, int n_spins, int spins_per_chunk, float2 *__restrict__ partial) {
+              const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
+              const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial) {
     using RecT = typename std::conditional<PH64, double4, float4>::type;   // (k'x, k'y, k'z, tau)
     using PosT = typename std::conditional<PH64, double4, float4>::type;   // (x, y, z, f')
     using real = typename std::conditional<PH64, double, float>::type;
@@ -63,20 +64,29 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         if (n_tiles > 0) issue(0);
         if (n_tiles > 1) issue(1);
     }
-    const int p0 = blockIdx.x * (kSigThreads * P) + tid;
+    // the thread's P points are ADJACENT ADC samples, so tau_j - tau_0 is a few dwell times
+    const int p0 = (blockIdx.x * kSigThreads + tid) * P;
     real kx[P], ky[P], kz[P], tau[P];
-    float tf[P], ar[P], ai[P];
+    float tf[P], cj[P], ar[P], ai[P];
+    float cmax = 0.f;
 #pragma unroll
     for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
+        const int p = p0 + j;
         RecT r;
-        r.x = 0; r.y = 0; r.z = 0; r.w = 0;
+        r.x = 0; r.y = 0; r.z = 0; r.w = j ? tau[0] : (real)0;
         if (p < n_pts) r = recs[p];
         kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
         tf[j] = (float)r.w;
+        cj[j] = (float)(r.w - tau[0]) * 0.6931471805599453f;  // (tau_j - tau_0) ln 2; times e2 = -(tau_j - tau_0)/T2
+        cmax = fmaxf(cmax, fabsf(cj[j]));
         ar[j] = 0.f; ai[j] = 0.f;
     }
+    // exp(-tau_j/T2) for j > 0 from the j = 0 value by a cubic series in (tau_j - tau_0)/T2 when that ratio is
+    // <= 0.02 for every spin (truncation < 7e-9); decided per warp, otherwise every point takes its own MUFU.EX2
+    const bool series = P > 1 && __all_sync(0xffffffffu, cmax * (scal[0] * kLog2e) <= 0.02f);
     __syncthreads();  // barrier initialisation visible to every waiter
+    auto run = [&](auto series_tag) {
+    constexpr bool SERIES = decltype(series_tag)::value;
     for (int t = 0; t < n_tiles; ++t) {
         const int b = t & 1;
         mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
@@ -85,6 +95,7 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         for (int s = 0; s < cnt; ++s) {
             const PosT a = shA[b][s];
             const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            float er0 = 0.f, ei0 = 0.f;
 #pragma unroll
             for (int j = 0; j < P; ++j) {
                 float sn, cs;
@@ -103,8 +114,18 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
                     sn = __sinf(th);  // FMUL by 1/(2 pi) + MUFU.SIN
                     cs = __cosf(th);
                 }
-                const float e = ex2_approx(tf[j] * st.w);  // MUFU.EX2: exp(-tau/T2)
-                const float er = st.x * e, ei = st.y * e;
+                float er, ei;
+                if (j == 0 || !SERIES) {
+                    const float e = ex2_approx(tf[j] * st.w);  // MUFU.EX2: exp(-tau/T2)
+                    er = st.x * e;
+                    ei = st.y * e;
+                    if (j == 0) { er0 = er; ei0 = ei; }
+                } else {
+                    const float y = cj[j] * st.w;  // -(tau_j - tau_0)/T2
+                    const float pe = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+                    er = er0 * pe;
+                    ei = ei0 * pe;
+                }
                 ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
                 ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
             }
@@ -112,9 +133,12 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         __syncthreads();  // every thread is done with stage b
         if (tid == 0 && t + 2 < n_tiles) issue(t + 2);
     }
+    };
+    if (series) run(std::true_type{});
+    else run(std::false_type{});
 #pragma unroll
     for (int j = 0; j < P; ++j) {
-        const int p = p0 + j * kSigThreads;
+        const int p = p0 + j;
         if (p < n_pts) partial[(size_t)blockIdx.y * n_pts + p] = make_float2(ar[j], ai[j]);
     }
 }
