@@ -32,6 +32,9 @@ SM_COUNT = 148
 # FP32 128 lanes/SM/clk
 MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)
 FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full captures
+NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v2_signal_kernel_cfg4_ncu.txt"),
+               ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v2_rf_kernel_cfg4_ncu.txt")}
 
 
 def load_peaks():
@@ -270,7 +273,12 @@ def run_ours(args, rank, local_rank, world):
         dur = kinds_ms["signal"] * 1e-3 / args.steps
         ach = MUFU_PER_EVAL * n_eval_sig / dur
         kern["signal"] = {"bound": "alu", "pipe": "mufu", "achieved": ach / 1e12, "peak": mufu_peak / 1e12,
-                          "unit": "Tmufu-op/s", "frac": ach / mufu_peak, "traffic": None,
+                          "unit": "Tmufu-op/s", "frac": ach / mufu_peak,
+                          "traffic": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[0],
+                          "traffic_source": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[1],
+                          "note": "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample), SURVEY.md 8(d); "
+                                  "the kernel issues 2 + 1/P (P = 4 adjacent samples share one ex2), so frac can "
+                                  "reach 3 / 2.25 = 1.33 at a saturated MUFU pipe",
                           "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
                           "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
                           "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}
@@ -278,7 +286,11 @@ def run_ours(args, rank, local_rank, world):
         dur = kinds_ms["rf"] * 1e-3 / args.steps
         ach = FP32_PER_RF_STEP * rf_steps / dur
         kern["rf"] = {"bound": "alu", "pipe": "fp32", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
-                      "unit": "Tfp32-instr/s", "frac": ach / fp32_peak, "traffic": None,
+                      "unit": "Tfp32-instr/s", "frac": ach / fp32_peak,
+                      "traffic": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[0],
+                      "traffic_source": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[1],
+                      "note": "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly), "
+                              "SURVEY.md 8(d); the tier-0 loop issues 38.6 per step on plateau-gradient tiles",
                       "launches_per_step": kinds_n["rf"] // args.steps, "ms_per_step": dur * 1e3,
                       "avg_launch_ms": kinds_ms["rf"] / kinds_n["rf"],
                       "algorithmic_ops_per_launch": FP32_PER_RF_STEP * rf_steps * args.steps / kinds_n["rf"]}
@@ -326,7 +338,7 @@ def main():
     from paper_2301_02702_b200.dist import env_world
     rank, local_rank, world = env_world()
     if args.cpu_budget <= 0:
-        args.cpu_budget = 2e8 * max(1, (os.cpu_count() or 1))   # ~10-30 s at ~10-20 ns per spin*step per core
+        args.cpu_budget = 1e8 * max(1, (os.cpu_count() or 1))   # ~15-20 s at ~6e6 spin*steps/s per core
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
