@@ -205,32 +205,40 @@ def run_ours(args, rank, local_rank, world):
         if not per_spin:
             reduce_signal(sig)
 
-    bloch.bloch_plan_set_profiling(plan.handle, True)
     for _ in range(args.warmup):
         flush.zero_()
         step()
     barrier()
 
-    # ---- device-resident timing: K steps, L2 flushed (untimed) before each, CUDA events around each step
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    # ---- device-resident timing: K steps, L2 flushed (untimed) before each, CUDA events around each step.
+    # Pass 1 (no per-kernel events) gives `value`; pass 2 repeats the same K steps with the library's per-kernel
+    # CUDA events on the launching stream (they cost ~4 % on the 9000-launch MRF config) for the roofline.
     kinds_ms = {k: 0.0 for k in bloch.KINDS}
     kinds_n = {k: 0 for k in bloch.KINDS}
     clocks = ClockSampler(local_rank)
+    ms_pass = {}
     with clocks:
-        barrier()
-        for a, b in ev:
-            flush.zero_()
-            a.record()
-            step()
-            b.record()
-            b.synchronize()
-            tm = bloch.bloch_plan_last_timing(plan.handle)
-            for k in bloch.KINDS:
-                kinds_ms[k] += tm["ms"][k]
-                kinds_n[k] += tm["launches"][k]
-        barrier()
-    ms_local = sum(a.elapsed_time(b) for a, b in ev)
-    t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
+        for taps in (False, True):
+            if taps and args.no_taps:
+                continue
+            bloch.bloch_plan_set_profiling(plan.handle, taps)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                  for _ in range(args.steps)]
+            barrier()
+            for a, b in ev:
+                flush.zero_()
+                a.record()
+                step()
+                b.record()
+                b.synchronize()
+                if taps:
+                    tm = bloch.bloch_plan_last_timing(plan.handle)
+                    for k in bloch.KINDS:
+                        kinds_ms[k] += tm["ms"][k]
+                        kinds_n[k] += tm["launches"][k]
+            barrier()
+            ms_pass[taps] = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([ms_pass[False]], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
@@ -311,7 +319,8 @@ def run_ours(args, rank, local_rank, world):
            "clocks": clocks.summary(),
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "steps": e2e_steps, "api": "bloch_simulate_host (pinned host buffers)"},
-           "gpu_launches": int(sum(kinds_n.values())),
+           "gpu_launches": bloch.bloch_plan_last_launches(plan.handle) * args.steps,
+           "ms_per_step_with_kernel_events": (ms_pass.get(True, 0.0) / args.steps) or None,
            "roofline": roofline,
            "kernels": kern,
            "ms_by_kind_per_step": {k: v / args.steps for k, v in kinds_ms.items()}}
@@ -332,6 +341,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 4 (default, 1M-spin spiral), 5, 5b")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")
     ap.add_argument("--microbench", action="store_true", help="also run the MUFU/FFMA/DFMA pipe micro-benchmarks")
     args = ap.parse_args()

@@ -154,6 +154,9 @@ enum { BLOCH_KIND_OTHER = 0,   /* pack / unpack / block-end propagation only */
        BLOCH_N_KINDS = 4 };
 int bloch_plan_set_profiling(bloch_plan *plan, int enable);
 int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *launches_by_kind);
+/* Number of kernels the last bloch_simulate on this plan enqueued (it depends on n_spins through the batching
+ * of the second-pass reduction; bloch_plan_info.n_launches is the upper bound with one second pass per block). */
+int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
 
 /* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
  * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA, 2 = DFMA.  Runs `iters` dependent-chain iterations with 8

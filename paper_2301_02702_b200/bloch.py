@@ -48,7 +48,7 @@ class bloch_plan_info(C.Structure):
 EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",
            "bloch_plan_get_info", "bloch_plan_workspace_bytes", "bloch_plan_upload", "bloch_simulate",
            "bloch_simulate_host_scratch_bytes", "bloch_simulate_host", "bloch_plan_set_profiling",
-           "bloch_plan_last_timing", "bloch_microbench"]
+           "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_microbench"]
 
 
 def _load():
@@ -73,6 +73,7 @@ def _load():
     lib.bloch_simulate_host.argtypes = sim_args
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
+    lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
     lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
     for name in EXPORTS:
         if name not in ("bloch_strerror", "bloch_last_error"):
@@ -196,6 +197,12 @@ def bloch_plan_last_timing(plan: int) -> dict:
     _check(_lib.bloch_plan_last_timing(plan, ms, cnt))
     return {"ms": {k: float(ms[i]) for i, k in enumerate(KINDS)},
             "launches": {k: int(cnt[i]) for i, k in enumerate(KINDS)}}
+
+
+def bloch_plan_last_launches(plan: int) -> int:
+    out = C.c_int64()
+    _check(_lib.bloch_plan_last_launches(plan, C.byref(out)))
+    return int(out.value)
 
 
 def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:

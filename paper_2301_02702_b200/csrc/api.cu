@@ -67,15 +67,21 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
     return s;
 }
 
-int max_chunks_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
-    // upper bound over the plan's blocks; partial buffer is sized with it
-    int64_t worst = 1;
+// Partial-sum buffer (a7): consecutive ADC-bearing precession blocks with the same launch shape share one
+// buffer P[chunk][points of the batch] and ONE second-pass launch, up to kPartialCapBytes; at least the
+// largest single block always fits.
+constexpr size_t kPartialCapBytes = size_t(512) << 20;
+
+size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+    size_t worst = 1, total = 0;
     for (const Block &b : plan->blocks) {
         if (b.type != kBlockPrecession || b.adc_count == 0) continue;
         const SigShape s = sig_shape(b.adc_count, n_spins, sm_count);
-        worst = std::max<int64_t>(worst, (int64_t)s.chunks * b.adc_count);
+        const size_t e = size_t(s.chunks) * size_t(b.adc_count);
+        worst = std::max(worst, e);
+        total += e;
     }
-    return (int)std::min<int64_t>(worst, INT32_MAX);
+    return std::max(worst, std::min(total, kPartialCapBytes / sizeof(float2)));
 }
 
 struct Workspace {
@@ -83,6 +89,7 @@ struct Workspace {
     double4 *Ad;     // fp64-phase plans only
     unsigned *scal;  // device scalars: [0] = max 1/T2 (float bits)
     float2 *partial;
+    size_t partial_elems;
     size_t bytes;
 };
 
@@ -100,6 +107,7 @@ int sm_count_cached() {
 // bloch_plan_workspace_bytes is a pure host function.
 Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_count) {
     Workspace w{};
+    w.partial_elems = 0;
     size_t off = 0;
     auto take = [&](size_t bytes) {
         void *p = base ? (void *)((unsigned char *)base + off) : nullptr;
@@ -112,8 +120,10 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.Ad = plan->info.phase_mode == BLOCH_PHASE_FP64 ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
     w.scal = (unsigned *)take(kAlign);
     size_t pbytes = kAlign;
-    if (plan->info.output_mode == BLOCH_OUT_SUM_ALL)
-        pbytes = size_t(max_chunks_for(plan, n_spins, sm_count)) * sizeof(float2);
+    if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
+        w.partial_elems = partial_elems_for(plan, n_spins, sm_count);
+        pbytes = w.partial_elems * sizeof(float2);
+    }
     w.partial = (float2 *)take(pbytes);
     w.bytes = off;
     return w;
@@ -248,6 +258,12 @@ int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *l
     return BLOCH_OK;
 }
 
+int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out) {
+    if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
+    *out = plan->last.launches;
+    return BLOCH_OK;
+}
+
 int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
                    const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
                    const float *d_dw, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
@@ -293,7 +309,11 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
     const int rf_threads = env_int("BLOCH_RF_THREADS", (n + 31) / 32 >= sms * 32 ? 128 : 32);
     const int rf_grid = (n + rf_threads - 1) / rf_threads;
-    for (const Block &b : plan->blocks) {
+    bool batch_open = false;
+    SigShape batch_shape{};
+    int64_t batch_adc_first = 0, batch_pts = 0, batch_done = 0;
+    for (size_t bi = 0; bi < plan->blocks.size(); ++bi) {
+        const Block &b = plan->blocks[bi];
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
             rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(plan->d_tables + b.table_off, (int)b.n_tiles, prop,
@@ -326,24 +346,46 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                 ++launches;
             } else {
                 const SigShape s = sig_shape(n_pts, n, sms);
+                if (!batch_open) {  // look ahead: how many of the following blocks share this batch
+                    batch_shape = s;
+                    batch_adc_first = b.adc_first;
+                    batch_pts = 0;
+                    batch_done = 0;
+                    const int64_t cap_pts = std::max<int64_t>(n_pts, (int64_t)(w.partial_elems / (size_t)s.chunks));
+                    for (size_t bj = bi; bj < plan->blocks.size(); ++bj) {
+                        const Block &c = plan->blocks[bj];
+                        if (c.type != kBlockPrecession || c.adc_count == 0) continue;
+                        const SigShape sc = sig_shape(c.adc_count, n, sms);
+                        if (sc.P != s.P || sc.chunks != s.chunks || sc.spins_per_chunk != s.spins_per_chunk) break;
+                        if (batch_pts + c.adc_count > cap_pts || batch_pts + c.adc_count > INT32_MAX) break;
+                        batch_pts += c.adc_count;
+                    }
+                    batch_open = true;
+                }
                 const dim3 grid(s.ptiles, s.chunks);
+                const int row = (int)batch_pts, poff = (int)batch_done;
 #define BLOCH_LAUNCH_SIG(PP)                                                                                   \
     do {                                                                                                       \
         if (ph64)                                                                                              \
             signal_kernel<PP, true><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.Ad, w.S, n,               \
-                                                                      s.spins_per_chunk, (const float *)w.scal, w.partial);           \
+                s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);                               \
         else                                                                                                   \
             signal_kernel<PP, false><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.A, w.S, n,               \
-                                                                       s.spins_per_chunk, (const float *)w.scal, w.partial);          \
+                s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);                               \
     } while (0)
                 if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
                 else BLOCH_LAUNCH_SIG(1);
 #undef BLOCH_LAUNCH_SIG
-                if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
-                reduce_kernel<<<(n_pts + 31) / 32, dim3(32, 8), 0, stream>>>(w.partial, s.chunks, n_pts,
-                                                                            (float2 *)d_signal + b.adc_first);
-                launches += 2;
+                ++launches;
+                batch_done += n_pts;
+                if (batch_done == batch_pts) {  // batch complete: second pass over all its points
+                    if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
+                    reduce_kernel<<<(unsigned)((batch_pts + 31) / 32), dim3(32, 8), 0, stream>>>(
+                        w.partial, batch_shape.chunks, (int)batch_pts, (float2 *)d_signal + batch_adc_first);
+                    ++launches;
+                    batch_open = false;
+                }
             }
         }
         prop.kx = b.kend[0];

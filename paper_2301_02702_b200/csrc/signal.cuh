@@ -36,7 +36,8 @@ template <int P, bool PH64>
 __global__ void __launch_bounds__(kSigThreads)
 signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
               const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
-              const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial) {
+              const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial,
+              int row_stride /* points of the whole batch */, int p_off /* this block's first point in the batch */) {
     using RecT = typename std::conditional<PH64, double4, float4>::type;   // (k'x, k'y, k'z, tau)
     using PosT = typename std::conditional<PH64, double4, float4>::type;   // (x, y, z, f')
     using real = typename std::conditional<PH64, double, float>::type;
@@ -139,7 +140,7 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
 #pragma unroll
     for (int j = 0; j < P; ++j) {
         const int p = p0 + j;
-        if (p < n_pts) partial[(size_t)blockIdx.y * n_pts + p] = make_float2(ar[j], ai[j]);
+        if (p < n_pts) partial[(size_t)blockIdx.y * row_stride + p_off + p] = make_float2(ar[j], ai[j]);
     }
 }
 
