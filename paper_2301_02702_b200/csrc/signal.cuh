@@ -5,16 +5,20 @@
 //     c_in = Mxy_i(0) * exp(-tau_n / T2_i) * exp(i theta_in),    theta_in = k'_n . x_i + f'_i tau_n
 // with k' = -gamma K(t) the cumulative gradient moment of the block (Eq 12-13, :173-180) and f' = -dw.
 //
-// Grid = (point tiles, spin chunks).  A thread OWNS P evaluated points (k', tau in registers) and walks the
-// spins of its chunk.  Spin tiles (x, y, z, f') and (Mxy, e2) are staged global -> shared by 1-D bulk copies
+// Grid = (point tiles, spin chunks).  A thread OWNS P adjacent evaluated points (k', tau in registers) and
+// walks the spins of its chunk.  Spin tiles (x, y, z, f') and (Mxy, e2) are staged global -> shared by 1-D bulk copies
 // (TMA) into a two-stage mbarrier ring by one elected thread and then broadcast to all threads (every lane
 // reads the same address: conflict-free LDS.128).  The sum over spins is therefore thread-local: no
 // shuffles, no atomics.  Each CTA writes its partial sums P[chunk][point]; reduce_kernel adds the chunks in
 // index order (deterministic two-pass reduction, :194 "add them later").
 //
 // fp32 phase: tables and f' in radians; per evaluation 4 FMA (phase), 1 FMUL (MUFU pre-scale to turns),
-// MUFU sin + cos, 1 FMUL + MUFU ex2 (T2 decay), 2 FMUL + 4 FMA (complex multiply-accumulate) = 15 issue
-// slots, 3 of them on the 16-lane MUFU pipe -- the bound.  No explicit range reduction: MUFU.SIN/COS take
+// MUFU sin + cos, 1 FMUL + MUFU ex2 (T2 decay), 2 FMUL + 4 FMA (complex multiply-accumulate) = 16 issue
+// slots, 3 of them on the 16-lane MUFU pipe -- the bound.  Because a thread's P points are adjacent samples,
+// exp(-tau_j/T2) for j > 0 is the j = 0 value times a cubic series in (tau_j - tau_0)/T2 on the FMA pipe
+// whenever that ratio is <= 0.02 for every spin (bound from max 1/T2, found by pack_kernel): 2 + 1/P MUFU
+// operations and 17.9 instructions per evaluation.  Consecutive blocks of one batch write their partials
+// side by side (row_stride, p_off) so that one second-pass launch serves the whole batch.  No explicit range reduction: MUFU.SIN/COS take
 // their argument in turns and wrap it themselves; the planner keeps |theta| below 256 turns in this mode,
 // where the fp32 rounding of theta (~1e-4 rad) is already the error floor.
 // fp64 phase (north_star item 4): k', tau, x, f' in double, theta in turns by 4 DFMA; adding 1.5 * 2^20

@@ -1,0 +1,133 @@
+"""GPU-vs-oracle parity on inputs chosen to drive every code path of the kernels (pytest -m gpu):
+RF tiers 0/1/2, compact and general step tiles, tiles cut where the step length changes, the signal kernel's
+series / per-sample exponential, P = 1, 2, 4 launch shapes with ragged tails, and batched second passes.
+Same acceptance as test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_2301_02702_b200 import workloads as W
+from seqtools import seq
+
+pytestmark = pytest.mark.gpu
+
+TOL_MAX = 1e-4
+TOL_NRMSE = 1e-5
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2301_02702_b200 import build as bl
+    bl.build()
+    from paper_2301_02702_b200 import bloch
+    return bloch
+
+
+def errors(got, ref):
+    got = np.asarray(got, dtype=np.complex128)
+    ref = np.asarray(ref, dtype=np.complex128)
+    scale = max(np.abs(ref).max(), 1e-300)
+    d = np.abs(got - ref)
+    return d.max() / scale, np.sqrt(np.mean(d ** 2)) / scale
+
+
+def check(B, oracle_mod, ph, s, what, output_mode="sum", **plan_kw):
+    import torch
+    plan = B.Plan(s, output_mode=output_mode, **plan_kw)
+    dev = B.phantom_to_device(ph)
+    Mxy = torch.zeros(ph.n, 2, dtype=torch.float32, device="cuda")
+    Mz = torch.zeros(ph.n, dtype=torch.float32, device="cuda")
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz)
+    torch.cuda.synchronize()
+    launches = B.bloch_plan_last_launches(plan.handle)
+    plan.close()
+    ref, rxy, rz = oracle_mod.simulate(ph, s, output_mode=output_mode, return_state=True)
+    m = Mxy.cpu().numpy()
+    got_state = np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)])
+    ref_state = np.concatenate([rxy, rz.astype(np.complex128)])
+    for name, g, r in (("signal", sig.cpu().numpy(), ref), ("state", got_state, ref_state)):
+        if r.size == 0:
+            continue
+        emax, nrmse = errors(g, r)
+        print(f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}")
+        assert emax <= TOL_MAX and nrmse <= TOL_NRMSE, f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}"
+    return launches
+
+
+def rand_phantom(n, seed, zmax=0.01, dwmax=300.0, t2=(0.03, 0.3)):
+    rng = np.random.default_rng(seed)
+    return W._phantom(rng.uniform(-.1, .1, n), rng.uniform(-.1, .1, n), rng.uniform(-zmax, zmax, n),
+                      rng.uniform(.5, 1, n), rng.uniform(.3, 2, n), rng.uniform(*t2, n), rng.uniform(-dwmax, dwmax, n))
+
+
+def sinc_rf(t0, dur, n, flip):
+    dt = dur / n
+    tm = (np.arange(n) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - dur / 2) / dur)
+    b1 = env * flip / (W.GAMMA * dt * env.sum())
+    return t0 + np.arange(n) * dt, np.full(n, dt), b1, np.zeros(n)
+
+
+@pytest.mark.parametrize("dt_rf,zmax,tier", [(1e-6, 0.002, 0), (1e-6, 0.08, 1), (4e-6, 0.08, 2)])
+def test_rf_tiers_on_a_slice_select_plateau(B, oracle_mod, dt_rf, zmax, tier):
+    """|w|^2 per step is set by gamma*G*z*dt: 10 mT/m, z up to 2 mm / 8 cm, dt 1 / 4 us -> tiers 0 / 1 / 2."""
+    n_rf = int(round(1e-3 / dt_rf))
+    rf = sinc_rf(2e-4, 1e-3, n_rf, np.deg2rad(40))
+    g = {2: ([1e-4, 2e-4, 1.2e-3, 1.3e-3, 1.8e-3, 1.9e-3], [0, 10e-3, 10e-3, 0, -8e-3, 0]),
+         0: ([1.4e-3, 1.5e-3, 2.5e-3, 2.6e-3], [0, 5e-3, 5e-3, 0])}
+    adc = 1.5e-3 + (np.arange(300) + 0.5) * 3e-6
+    s = seq(g=g, rf=rf, adc=adc, t_end=3e-3, dt_rf_max=dt_rf)
+    ph = rand_phantom(777, 100 + tier, zmax=zmax)
+    wz = W.GAMMA * 10e-3 * zmax * dt_rf
+    assert (wz * wz <= 2 ** -8) == (tier == 0) and (wz * wz > 0.25) == (tier == 2)
+    check(B, oracle_mod, ph, s, f"RF tier {tier}")
+
+
+def test_rf_on_gradient_ramps_and_changing_step_length(B, oracle_mod):
+    """General (32-B) step records: the gradient changes from step to step; RF samples of three different
+    lengths force tile cuts where dt changes; 300 steps of one dt span more than one 128-step tile."""
+    dts = np.concatenate([np.full(300, 1e-6), np.full(40, 5e-6), np.full(7, 2e-6), np.full(150, 1e-6)])
+    t0 = 1e-4 + np.concatenate([[0.0], np.cumsum(dts)[:-1]])
+    rng = np.random.default_rng(5)
+    b1 = rng.uniform(-4e-6, 4e-6, dts.size)
+    b1i = rng.uniform(-4e-6, 4e-6, dts.size)
+    t_rf_end = t0[-1] + dts[-1]
+    g = {0: ([0.0, 3e-4, 5e-4, 9e-4], [0, 12e-3, -6e-3, 0]),
+         1: ([5e-5, 4e-4, 1.5e-3], [0, 8e-3, 0]),
+         2: ([0.0, 2e-4, 6e-4, 1.2e-3], [3e-3, 3e-3, -9e-3, 0])}
+    adc = t_rf_end + 1e-5 + np.arange(77) * 7e-6
+    s = seq(g=g, rf=(t0, dts, b1, b1i), adc=adc, t_end=2.5e-3, dt_rf_max=1.0)
+    check(B, oracle_mod, rand_phantom(333, 6), s, "RF on ramps, mixed dt")
+
+
+@pytest.mark.parametrize("n_adc", [1, 5, 300, 700, 1023, 2049])
+def test_signal_launch_shapes_and_ragged_tails(B, oracle_mod, n_adc):
+    """n_adc selects P = 1 (< 512 points), 2 (< 1024) or 4 and leaves ragged point tiles; 1111 spins leave a
+    ragged spin tile."""
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 3) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    g = {0: ([2e-4, 3e-4, 9e-3], [0, 4e-3, 4e-3]), 1: ([2e-4, 3e-4, 9e-3], [0, -2e-3, 1e-3])}
+    adc = 3.5e-4 + (np.arange(n_adc) + 0.5) * 4e-6
+    s = seq(g=g, rf=rf, adc=adc, t_end=1e-2, dt_rf_max=1.0)
+    check(B, oracle_mod, rand_phantom(1111, 7), s, f"signal n_adc={n_adc}")
+
+
+def test_signal_series_fallback_when_adjacent_samples_are_far_apart(B, oracle_mod):
+    """Bursts of 5 samples separated by 1.5 ms with T2 down to 5 ms: (tau_j - tau_0)/T2 reaches 0.3 inside a
+    thread's 4 adjacent points, so those warps must take one MUFU.EX2 per sample; others keep the series."""
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    bursts = 2e-4 + np.arange(300)[:, None] * 1.5e-3 + np.arange(5)[None, :] * 5e-6
+    adc = np.sort(bursts.ravel())
+    g = {0: ([1.5e-4, 2e-4, adc[-1] + 1e-4], [0, 1e-3, 1e-3])}
+    s = seq(g=g, rf=rf, adc=adc, t_end=adc[-1] + 2e-4, dt_rf_max=1.0)
+    check(B, oracle_mod, rand_phantom(600, 8, t2=(0.005, 0.05)), s, "series fallback")
+
+
+def test_batched_second_pass_over_many_blocks(B, oracle_mod):
+    """20 TRs with one readout each: the precession blocks share partial-sum batches; forcing tiny blocks
+    (max_block_points) multiplies the number of blocks per batch."""
+    w = W.small("5")
+    a = check(B, oracle_mod, w.phantom, w.seq, "batched reduce")
+    b = check(B, oracle_mod, w.phantom, w.seq, "batched reduce, cut blocks", max_block_points=50)
+    assert b > a
