@@ -348,7 +348,7 @@ def main():
     from paper_2301_02702_b200.dist import env_world
     rank, local_rank, world = env_world()
     if args.cpu_budget <= 0:
-        args.cpu_budget = 1e8 * max(1, (os.cpu_count() or 1))   # ~15-20 s at ~6e6 spin*steps/s per core
+        args.cpu_budget = 5e8 * max(1, (os.cpu_count() or 1))   # ~12 s at ~4e7 spin*steps/s per core (B200 host)
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
