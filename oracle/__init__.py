@@ -39,8 +39,12 @@ def _load():
         _lib.bloch_ref_simulate.restype = C.c_int
         _lib.bloch_ref_simulate.argtypes = ([C.c_double] + seq_args + [i64] + [dp] * 7 +
                                             [dp, dp, C.c_int, dp, C.c_int, C.c_int, C.c_int])
+        _lib.bloch_ref_simulate_motion.restype = C.c_int
+        _lib.bloch_ref_simulate_motion.argtypes = (_lib.bloch_ref_simulate.argtypes + [C.c_double, dp, dp, dp])
         _lib.bloch_ref_grid.restype = i64
         _lib.bloch_ref_grid.argtypes = seq_args + [dp, dp, C.POINTER(C.c_uint8), C.POINTER(i64)]
+        _lib.bloch_ref_grid_motion.restype = i64
+        _lib.bloch_ref_grid_motion.argtypes = _lib.bloch_ref_grid.argtypes + [C.c_double]
     return _lib
 
 
@@ -64,11 +68,14 @@ def _seq_args(seq, keep):
 
 
 def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state: bool = False,
-             n_threads: int | None = None, gamma: float = GAMMA, force_excitation: bool = False):
+             n_threads: int | None = None, gamma: float = GAMMA, force_excitation: bool = False,
+             velocity=None, dt_max: float = 0.0):
     """Step-by-step fp64 Bloch integration (SURVEY.md 8(c) listing).
 
     phantom: object with fp64 arrays x, y, z, M0, T1, T2, dw.   seq: object with g_t, g_v (3 arrays each),
     rf_t, rf_dt, rf_re, rf_im, adc_t, t_end, dt_rf_max.
+    velocity: optional (vx, vy, vz) fp64 arrays [m/s]: every spin moves as x(t) = x + v t (PAPER.md:96, :236);
+    dt_max then refines every interval to at most dt_max (:180).
     Returns complex128 signal [n_adc] ("sum") or [n_spins, n_adc] ("per_spin"); with return_state also
     (Mxy complex128 [n_spins], Mz float64 [n_spins]).
     """
@@ -94,10 +101,19 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     if n_threads is None:
         n_threads = os.cpu_count() or 1
     dp = C.POINTER(C.c_double)
-    rc = lib.bloch_ref_simulate(C.c_double(gamma), *sargs, C.c_int64(n), *pa,
-                                mxy.ctypes.data_as(dp), mz.ctypes.data_as(dp), C.c_int(use_state),
-                                sig.ctypes.data_as(dp), C.c_int(mode), C.c_int(int(n_threads)),
-                                C.c_int(1 if force_excitation else 0))
+    common = [C.c_double(gamma), *sargs, C.c_int64(n), *pa, mxy.ctypes.data_as(dp), mz.ctypes.data_as(dp),
+              C.c_int(use_state), sig.ctypes.data_as(dp), C.c_int(mode), C.c_int(int(n_threads)),
+              C.c_int(1 if force_excitation else 0)]
+    if velocity is None and not dt_max:
+        rc = lib.bloch_ref_simulate(*common)
+    else:
+        va = [None, None, None]
+        if velocity is not None:
+            for k in range(3):
+                a, pk = _d(np.broadcast_to(np.asarray(velocity[k], dtype=np.float64), (n,)))
+                keep.append(a)
+                va[k] = pk
+        rc = lib.bloch_ref_simulate_motion(*common, C.c_double(float(dt_max)), *va)
     if rc != 0:
         raise ValueError(f"bloch_ref_simulate failed with code {rc}")
     if return_state:
@@ -105,18 +121,20 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     return sig
 
 
-def grid(seq):
+def grid(seq, dt_max: float = 0.0):
     """The oracle's own discretisation: (t[n+1], G[n+1,3], rf[n] uint8, adc[n+1] int64)."""
     lib = _load()
     keep = []
     sargs, _ = _seq_args(seq, keep)
     null_d = C.POINTER(C.c_double)()
-    n = lib.bloch_ref_grid(*sargs, null_d, null_d, C.POINTER(C.c_uint8)(), C.POINTER(C.c_int64)())
+    n = lib.bloch_ref_grid_motion(*sargs, null_d, null_d, C.POINTER(C.c_uint8)(), C.POINTER(C.c_int64)(),
+                                  C.c_double(float(dt_max)))
     if n < 0:
         raise ValueError(f"bloch_ref_grid failed with code {n}")
     t = np.zeros(n + 1); G = np.zeros((n + 1, 3)); rf = np.zeros(max(n, 1), dtype=np.uint8)
     adc = np.zeros(n + 1, dtype=np.int64)
     dp = C.POINTER(C.c_double)
-    lib.bloch_ref_grid(*sargs, t.ctypes.data_as(dp), G.ctypes.data_as(dp),
-                       rf.ctypes.data_as(C.POINTER(C.c_uint8)), adc.ctypes.data_as(C.POINTER(C.c_int64)))
+    lib.bloch_ref_grid_motion(*sargs, t.ctypes.data_as(dp), G.ctypes.data_as(dp),
+                              rf.ctypes.data_as(C.POINTER(C.c_uint8)), adc.ctypes.data_as(C.POINTER(C.c_int64)),
+                              C.c_double(float(dt_max)))
     return t, G, rf[:n], adc

@@ -17,6 +17,11 @@
  *   - per-thread signal buffers added at the end
  * Readings of silent / garbled passages (G1..G18) are those of SURVEY.md 8(c), restated in DESIGN.md.
  *
+ * Motion: bloch_ref_simulate_motion moves every spin as x(t) = x + v t
+ * and takes the trapezoid of Eq (12)-(13) on Bz(t_n) = G(t_n) . x(t_n); dt_max adds the intermediate points.  Pins M1-M5:
+ * tests/test_oracle_motion_pins.py (closed-form phase under constant G, bipolar velocity encoding, O(dt^2)
+ * convergence on a ramp, regime consistency).
+ *
  * Pins (tests/test_oracle_pins.py): closed forms P1-P10 of SURVEY.md 8(c); no value printed by the paper
  * exists for this path, so "against the paper's own numbers" the parity is unpinned (stated in DESIGN.md).
  *
@@ -83,6 +88,17 @@ static void grid_free(ref_grid *g) {
     memset(g, 0, sizeof(*g));
 }
 
+/* Number of equal sub-steps of the interval [a, b]: RF-covered intervals are limited to dt_rf_max (:182),
+ * and, with motion, every interval to dt_max (the paper's "intermediate points in the case of motion", :180). */
+static int64_t ref_parts(double a, double b, int covered, double dt_rf_max, double dt_max) {
+    double lim = 0.0;
+    if (covered && dt_rf_max > 0.0) lim = dt_rf_max;
+    if (dt_max > 0.0 && isfinite(dt_max) && (lim == 0.0 || dt_max < lim)) lim = dt_max;
+    if (lim <= 0.0) return 1;
+    int64_t parts = (int64_t)ceil(((b - a) - REF_TOL_T) / lim);
+    return parts < 1 ? 1 : parts;
+}
+
 /*
  * Time grid: sorted unique union of 0, t_end, gradient vertices, RF sample edges and ADC times, refined so
  * that no RF-covered interval exceeds dt_rf_max (an RF piece of length L is cut into ceil(L/dt_rf_max)
@@ -93,7 +109,8 @@ static void grid_free(ref_grid *g) {
 static int grid_build(ref_grid *g,
                       const double *const gt[3], const double *const gv[3], const int64_t gn[3],
                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
-                      int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max) {
+                      int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
+                      double dt_max) {
     memset(g, 0, sizeof(*g));
     if (!(t_end > 0.0)) return -1;
     int64_t cap = 2 + gn[0] + gn[1] + gn[2] + 2 * rf_n + adc_n;
@@ -118,10 +135,7 @@ static int grid_build(ref_grid *g,
     int64_t total = 1;
     for (int64_t i = 0; i + 1 < u; ++i) {
         double a = raw[i], b = raw[i + 1];
-        int64_t parts = 1;
-        if (rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0 && dt_rf_max > 0.0)
-            parts = (int64_t)ceil(((b - a) - REF_TOL_T) / dt_rf_max);
-        if (parts < 1) parts = 1;
+        int64_t parts = ref_parts(a, b, rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0, dt_rf_max, dt_max);
         total += parts;
     }
     g->n = total - 1;
@@ -136,10 +150,7 @@ static int grid_build(ref_grid *g,
     g->t[k++] = raw[0];
     for (int64_t i = 0; i + 1 < u; ++i) {
         double a = raw[i], b = raw[i + 1];
-        int64_t parts = 1;
-        if (rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0 && dt_rf_max > 0.0)
-            parts = (int64_t)ceil(((b - a) - REF_TOL_T) / dt_rf_max);
-        if (parts < 1) parts = 1;
+        int64_t parts = ref_parts(a, b, rf_n > 0 && rf_cover(rf_t, rf_dt, rf_n, 0.5 * (a + b)) >= 0, dt_rf_max, dt_max);
         for (int64_t p = 1; p < parts; ++p) g->t[k++] = a + (b - a) * ((double)p / (double)parts);
         g->t[k++] = b;
     }
@@ -169,7 +180,7 @@ static int grid_build(ref_grid *g,
 
 /* One spin, all intervals, exactly as the listing of SURVEY.md 8(c). */
 static void integrate_spin(const ref_grid *g, double gamma, double x, double y, double z, double M0,
-                           double T1, double T2, double dw, double complex *pMxy, double *pMz,
+                           double T1, double T2, double dw, const double *vel, double complex *pMxy, double *pMz,
                            double complex *S, int accumulate, int force_excitation) {
     double complex Mxy = *pMxy;
     double Mz = *pMz;
@@ -181,6 +192,16 @@ static void integrate_spin(const ref_grid *g, double gamma, double x, double y, 
         double Gy = 0.5 * (g->G[3 * n + 1] + g->G[3 * n + 4]);
         double Gz = 0.5 * (g->G[3 * n + 2] + g->G[3 * n + 5]);
         double Bz = Gx * x + Gy * y + Gz * z + dw / gamma;                 /* Eq (2) */
+        if (vel) {
+            /* motion x(t) = x + v t: the trapezoid of Eq (12)-(13) is taken on the
+             * effective field itself, Bz(t_n) = G(t_n) . x(t_n), at the two ends of the interval (:180, :336) */
+            double t0 = g->t[n], t1 = g->t[n + 1];
+            double b0 = g->G[3 * n + 0] * (x + vel[0] * t0) + g->G[3 * n + 1] * (y + vel[1] * t0)
+                        + g->G[3 * n + 2] * (z + vel[2] * t0);
+            double b1 = g->G[3 * n + 3] * (x + vel[0] * t1) + g->G[3 * n + 4] * (y + vel[1] * t1)
+                        + g->G[3 * n + 5] * (z + vel[2] * t1);
+            Bz = 0.5 * (b0 + b1) + dw / gamma;
+        }
         if (g->rf[n] || force_excitation) {
             /* excitation regime, Eq (5)-(9) */
             double complex B1 = g->b1re[n] + I * g->b1im[n];
@@ -228,7 +249,7 @@ static void integrate_spin(const ref_grid *g, double gamma, double x, double y, 
  *   flags        bit 0: force every interval through the excitation branch (invariant I5 only)
  *   returns 0, or <0 on invalid input.
  */
-int bloch_ref_simulate(double gamma,
+int bloch_ref_simulate_motion(double gamma,
                        const double *gx_t, const double *gx_v, int64_t gx_n,
                        const double *gy_t, const double *gy_v, int64_t gy_n,
                        const double *gz_t, const double *gz_v, int64_t gz_n,
@@ -237,13 +258,15 @@ int bloch_ref_simulate(double gamma,
                        int64_t n_spins, const double *x, const double *y, const double *z,
                        const double *M0, const double *T1, const double *T2, const double *dw,
                        double *Mxy, double *Mz, int use_state,
-                       double *signal, int output_mode, int n_threads, int flags) {
+                       double *signal, int output_mode, int n_threads, int flags,
+                       double dt_max, const double *vx, const double *vy, const double *vz) {
     const double *const gt[3] = {gx_t, gy_t, gz_t};
     const double *const gv[3] = {gx_v, gy_v, gz_v};
     const int64_t gn[3] = {gx_n, gy_n, gz_n};
     ref_grid g;
-    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max);
+    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max);
     if (rc) return rc;
+    const int moving = vx && vy && vz;
     int nth = n_threads > 0 ? n_threads : 1;
 #ifndef _OPENMP
     nth = 1;
@@ -256,7 +279,10 @@ int bloch_ref_simulate(double gamma,
             double mz = M0[i];
             if (use_state && Mxy && Mz) { mxy = Mxy[2 * i] + I * Mxy[2 * i + 1]; mz = Mz[i]; }
             double complex *S = (double complex *)(signal + 2 * i * adc_n);
-            integrate_spin(&g, gamma, x[i], y[i], z[i], M0[i], T1[i], T2[i], dw[i], &mxy, &mz, S, 0, force);
+            double vel[3] = {0.0, 0.0, 0.0};
+            if (moving) { vel[0] = vx[i]; vel[1] = vy[i]; vel[2] = vz[i]; }
+            integrate_spin(&g, gamma, x[i], y[i], z[i], M0[i], T1[i], T2[i], dw[i], moving ? vel : NULL, &mxy, &mz,
+                           S, 0, force);
             if (Mxy && Mz) { Mxy[2 * i] = creal(mxy); Mxy[2 * i + 1] = cimag(mxy); Mz[i] = mz; }
         }
     } else {
@@ -276,7 +302,10 @@ int bloch_ref_simulate(double gamma,
                 double complex mxy = 0.0;
                 double mz = M0[i];
                 if (use_state && Mxy && Mz) { mxy = Mxy[2 * i] + I * Mxy[2 * i + 1]; mz = Mz[i]; }
-                integrate_spin(&g, gamma, x[i], y[i], z[i], M0[i], T1[i], T2[i], dw[i], &mxy, &mz, S, 1, force);
+                double vel[3] = {0.0, 0.0, 0.0};
+                if (moving) { vel[0] = vx[i]; vel[1] = vy[i]; vel[2] = vz[i]; }
+                integrate_spin(&g, gamma, x[i], y[i], z[i], M0[i], T1[i], T2[i], dw[i], moving ? vel : NULL, &mxy,
+                               &mz, S, 1, force);
                 if (Mxy && Mz) { Mxy[2 * i] = creal(mxy); Mxy[2 * i + 1] = cimag(mxy); Mz[i] = mz; }
             }
         }
@@ -292,22 +321,38 @@ int bloch_ref_simulate(double gamma,
     return 0;
 }
 
+/* The static-phantom entry: no motion, no dt_max refinement. */
+int bloch_ref_simulate(double gamma,
+                       const double *gx_t, const double *gx_v, int64_t gx_n,
+                       const double *gy_t, const double *gy_v, int64_t gy_n,
+                       const double *gz_t, const double *gz_v, int64_t gz_n,
+                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
+                       int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
+                       int64_t n_spins, const double *x, const double *y, const double *z,
+                       const double *M0, const double *T1, const double *T2, const double *dw,
+                       double *Mxy, double *Mz, int use_state,
+                       double *signal, int output_mode, int n_threads, int flags) {
+    return bloch_ref_simulate_motion(gamma, gx_t, gx_v, gx_n, gy_t, gy_v, gy_n, gz_t, gz_v, gz_n, rf_t, rf_dt, rf_re,
+                                     rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, n_spins, x, y, z, M0, T1, T2, dw,
+                                     Mxy, Mz, use_state, signal, output_mode, n_threads, flags, 0.0, NULL, NULL, NULL);
+}
+
 /*
  * bloch_ref_grid: expose the oracle's own discretisation for tests (refinement invariance, trapezoid areas).
  * Call with t_out == NULL to get the number of intervals; otherwise fills t_out[n+1], G_out[3(n+1)],
  * rf_out[n], adc_out[n+1] (caller-allocated).  Returns n (>= 0) or <0 on error.
  */
-int64_t bloch_ref_grid(const double *gx_t, const double *gx_v, int64_t gx_n,
+int64_t bloch_ref_grid_motion(const double *gx_t, const double *gx_v, int64_t gx_n,
                        const double *gy_t, const double *gy_v, int64_t gy_n,
                        const double *gz_t, const double *gz_v, int64_t gz_n,
                        const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
                        int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
-                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out) {
+                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out, double dt_max) {
     const double *const gt[3] = {gx_t, gy_t, gz_t};
     const double *const gv[3] = {gx_v, gy_v, gz_v};
     const int64_t gn[3] = {gx_n, gy_n, gz_n};
     ref_grid g;
-    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max);
+    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max);
     if (rc) return rc;
     int64_t n = g.n;
     if (t_out) {
@@ -318,4 +363,14 @@ int64_t bloch_ref_grid(const double *gx_t, const double *gx_v, int64_t gx_n,
     }
     grid_free(&g);
     return n;
+}
+
+int64_t bloch_ref_grid(const double *gx_t, const double *gx_v, int64_t gx_n,
+                       const double *gy_t, const double *gy_v, int64_t gy_n,
+                       const double *gz_t, const double *gz_v, int64_t gz_n,
+                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
+                       int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
+                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out) {
+    return bloch_ref_grid_motion(gx_t, gx_v, gx_n, gy_t, gy_v, gy_n, gz_t, gz_v, gz_n, rf_t, rf_dt, rf_re, rf_im, rf_n,
+                                 adc_t, adc_n, t_end, dt_rf_max, t_out, G_out, rf_out, adc_out, 0.0);
 }

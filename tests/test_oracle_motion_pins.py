@@ -1,0 +1,101 @@
+"""Pins for the oracle's motion extension (PAPER.md:96 motion field u(x,t), :180
+intermediate points "in the case of motion", :236 experiment (d) u_y = v_y t): x(t) = x + v t per spin.
+None of these call the CUDA path."""
+import numpy as np
+import pytest
+
+from seqtools import phantom, seq
+
+GAMMA = 2.0 * np.pi * 42.58e6
+
+
+def run(oracle_mod, ph, s, v, state=None, **kw):
+    if state is None:
+        state = (np.ones(ph.x.shape[0], dtype=np.complex128), np.zeros(ph.x.shape[0]))
+    return oracle_mod.simulate(ph, s, state=state, velocity=v, output_mode="per_spin", **kw)
+
+
+def test_m1_constant_gradient_constant_velocity_closed_form(oracle_mod):
+    """G constant, x(t) = x0 + v t: G.x(t) is linear in t, so the trapezoid on ANY grid is exact and
+    Mxy(t) = exp(-i gamma G (x0 t + v t^2 / 2)) exp(-i dw t) exp(-t/T2)."""
+    G, T = 7e-3, 4e-3
+    x0 = np.array([0.01, -0.03, 0.05])
+    v = np.array([0.1, -0.25, 0.0])
+    dw = np.array([30.0, 0.0, -80.0])
+    adc = np.array([0.3e-3, 1.1e-3, 2.7e-3, 4e-3])
+    s = seq(g={1: ([0.0, T], [G, G])}, adc=adc, t_end=T)
+    ph = phantom(y=x0, T2=[0.05, 0.1, 1e30], dw=dw)
+    sig = run(oracle_mod, ph, s, (np.zeros(3), v, np.zeros(3)))
+    for i in range(3):
+        exact = np.exp(-1j * (GAMMA * G * (x0[i] * adc + v[i] * adc ** 2 / 2) + dw[i] * adc)) * np.exp(-adc / ph.T2[i])
+        np.testing.assert_allclose(sig[i], exact, rtol=0, atol=2e-11)
+    # refining the grid changes nothing here (exactness), and zero velocity equals the static entry
+    sig2 = run(oracle_mod, ph, s, (np.zeros(3), v, np.zeros(3)), dt_max=1e-5)
+    np.testing.assert_allclose(sig2, sig, rtol=0, atol=2e-11)
+    stat = oracle_mod.simulate(ph, s, state=(np.ones(3, dtype=np.complex128), np.zeros(3)), output_mode="per_spin")
+    zero = run(oracle_mod, ph, s, (np.zeros(3), np.zeros(3), np.zeros(3)))
+    np.testing.assert_allclose(zero, stat, rtol=0, atol=1e-14)
+
+
+def test_m2_bipolar_pair_encodes_velocity_not_position(oracle_mod):
+    """Rectangular bipolar lobes (+G for d, -G for d): zeroth moment 0, first moment -G d^2, so the phase after
+    the pair is +gamma v G d^2 whatever x0 is (velocity encoding).  The lobes are given with 1 ns edges; the
+    trapezoid on the edge intervals carries an O(edge) error, far below the tolerance used."""
+    G, d, e = 10e-3, 1e-3, 1e-9
+    t0 = 0.5e-3
+    tv = [t0, t0 + e, t0 + d, t0 + d + e, t0 + 2 * d, t0 + 2 * d + e]
+    gv = [0.0, G, G, -G, -G, 0.0]
+    adc = [t0 + 2 * d + 1e-4]
+    s = seq(g={0: (tv, gv)}, adc=adc, t_end=3e-3)
+    x0 = np.array([-0.04, 0.0, 0.07, 0.07])
+    v = np.array([0.1, 0.1, 0.1, -0.3])
+    sig = run(oracle_mod, phantom(x=x0), s, (v, np.zeros(4), np.zeros(4)))[:, 0]
+    expected = np.exp(1j * GAMMA * v * G * d * d)
+    np.testing.assert_allclose(sig, expected, rtol=0, atol=5e-5)
+    assert abs(sig[0] - sig[2]) < 1e-4            # same v, different x0
+    static = run(oracle_mod, phantom(x=x0), s, (np.zeros(4), np.zeros(4), np.zeros(4)))[:, 0]
+    np.testing.assert_allclose(static, np.ones(4), rtol=0, atol=5e-5)
+
+
+def test_m3_a_ramp_converges_with_dt_max_at_second_order(oracle_mod):
+    """On a ramp G(t).x(t) is quadratic in t, so the trapezoid needs the intermediate points of :180; halving
+    dt_max must shrink the error about 4x towards the analytic moment.  A single sawtooth ramp is used: on a
+    symmetric trapezoid lobe the errors of the up and down ramps cancel exactly."""
+    G, R, e, t0 = 12e-3, 1e-3, 1e-9, 2e-4
+    s = seq(g={2: ([t0, t0 + R, t0 + R + e], [0.0, G, 0.0])}, adc=[t0 + R + 1e-4], t_end=2e-3)
+    v = 0.2
+    m1 = G * (R * R / 3 + t0 * R / 2)              # int G(t) t dt over the ramp, x0 = 0
+    exact = np.exp(-1j * GAMMA * v * m1)
+    errs = []
+    for dt in (4e-5, 2e-5, 1e-5):
+        sig = run(oracle_mod, phantom(z=[0.0]), s, (np.zeros(1), np.zeros(1), np.array([v])), dt_max=dt)[0, 0]
+        errs.append(abs(sig - exact))
+    assert errs[0] > 1e-5, "coarse grid should show the trapezoid error"
+    assert 3.7 < errs[0] / errs[1] < 4.3 and 3.7 < errs[1] / errs[2] < 4.3, errs
+
+
+def test_m4_both_regimes_see_the_same_moving_field(oracle_mod):
+    """Invariant I5 with motion: RF-free intervals pushed through the excitation branch give the precession
+    branch's answer, so both branches use the same Bz for a moving spin."""
+    rng = np.random.default_rng(3)
+    n = 6
+    ph = phantom(x=rng.uniform(-.1, .1, n), y=rng.uniform(-.1, .1, n), z=rng.uniform(-.1, .1, n),
+                 T1=rng.uniform(.3, 2, n), T2=rng.uniform(.03, .3, n), dw=rng.uniform(-200, 200, n))
+    v = tuple(rng.uniform(-.3, .3, n) for _ in range(3))
+    g = {0: ([0, 1e-3, 2e-3], [0, 8e-3, -3e-3]), 1: ([2e-4, 1.5e-3], [5e-3, 0]), 2: ([0, 2e-3], [-4e-3, 6e-3])}
+    s = seq(g=g, adc=np.linspace(1e-4, 2e-3, 9), t_end=2e-3)
+    st = (rng.normal(size=n) + 1j * rng.normal(size=n), rng.normal(size=n))
+    a = oracle_mod.simulate(ph, s, state=st, velocity=v, dt_max=2e-5, output_mode="per_spin")
+    b = oracle_mod.simulate(ph, s, state=st, velocity=v, dt_max=2e-5, output_mode="per_spin", force_excitation=True)
+    np.testing.assert_allclose(a, b, rtol=0, atol=1e-12)
+
+
+def test_m5_dt_max_refines_every_interval(oracle_mod):
+    s = seq(g={0: ([0.0, 1e-3], [0.0, 5e-3])}, rf=([2e-4], [1e-4], [1e-6], [0.0]), adc=[5e-4], t_end=1e-3,
+            dt_rf_max=2e-5)
+    t0, *_ = oracle_mod.grid(s)
+    t1, _, rf1, _ = oracle_mod.grid(s, dt_max=5e-5)
+    assert len(t1) > len(t0) and np.diff(t1).max() <= 5e-5 + 1e-12
+    assert np.all(np.diff(t1)[rf1.astype(bool)] <= 2e-5 + 1e-12)
+    t2, *_ = oracle_mod.grid(s, dt_max=1e-5)       # dt_max below dt_rf_max also limits RF steps
+    assert np.diff(t2).max() <= 1e-5 + 1e-12
