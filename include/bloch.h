@@ -41,6 +41,7 @@ typedef enum {
 
 enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
 enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1 };
+enum { BLOCH_MOTION_NONE = 0, BLOCH_MOTION_LINEAR = 1 };
 
 /* Scanner.  Only gamma enters the arithmetic (Eq 1-2, :105-114); B0, G_max, S_max are
  * carried for completeness and are not validated against.  gamma <= 0 selects 2*pi*42.58e6 (:322). */
@@ -69,8 +70,11 @@ typedef struct {
 } bloch_sequence;
 
 /* simParams.  dt_rf_max: RF sample pieces longer than this are cut into equal sub-steps
- * (the paper's dt_rf, :182).  dt_max: spacing of extra points in RF-free intervals; only needed with
- * motion (:180), accepted and ignored (<= 0 or inf).  max_block_points: precession blocks hold at most
+ * (the paper's dt_rf, :182).  dt_max: with motion_mode != NONE every interval longer than this is cut into
+ * equal sub-steps (the paper's "intermediate points in the case of motion", :180); ignored without motion
+ * or when <= 0 / inf.  motion_mode: BLOCH_MOTION_LINEAR builds the first-moment tables that let every spin
+ * move as x(t) = x + v t (PAPER.md:96 motion field, :236 experiment (d)); velocities are given to
+ * bloch_simulate_motion.  max_block_points: precession blocks hold at most
  * this many evaluated points (the paper's Nblocks memory bound, :171); <= 0 selects the default. */
 typedef struct {
     double dt_max;
@@ -78,6 +82,8 @@ typedef struct {
     int64_t max_block_points;
     int32_t phase_mode;   /* BLOCH_PHASE_* */
     int32_t output_mode;  /* BLOCH_OUT_*   */
+    int32_t motion_mode;  /* BLOCH_MOTION_* */
+    int32_t reserved;     /* 0 */
 } bloch_sim_params;
 
 typedef struct {
@@ -92,6 +98,8 @@ typedef struct {
     int64_t max_block_adc;   /* largest number of ADC samples in one precession block */
     int32_t phase_mode;      /* resolved: BLOCH_PHASE_FP32 or BLOCH_PHASE_FP64 */
     int32_t output_mode;
+    int32_t motion_mode;
+    int32_t reserved;
 } bloch_plan_info;
 
 typedef struct bloch_plan bloch_plan;
@@ -130,6 +138,19 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins,
                    float *d_Mxy, float *d_Mz, int init_equilibrium,
                    float *d_signal, void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* bloch_simulate for a moving phantom: spin i is at x_i + v_i t at sequence time t.
+ * d_vx, d_vy, d_vz: fp32 device arrays [m/s] of n_spins each; the plan must have been created with
+ * motion_mode = BLOCH_MOTION_LINEAR (else BLOCH_EINVAL).  All three NULL = bloch_simulate.  The effective
+ * field is sampled at the ends of every interval of the dt_max-refined grid and integrated by the trapezoidal
+ * rule exactly as the paper prescribes (:180, :336); because x(t) is linear in t this needs only one more
+ * spin-independent table, the first moment sum of (G_n t_n + G_{n+1} t_{n+1}) dt_n / 2. */
+int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins,
+                          const float *d_x, const float *d_y, const float *d_z, const float *d_M0,
+                          const float *d_T1, const float *d_T2, const float *d_dw,
+                          const float *d_vx, const float *d_vy, const float *d_vz,
+                          float *d_Mxy, float *d_Mz, int init_equilibrium,
+                          float *d_signal, void *d_workspace, size_t workspace_bytes, void *stream);
+
 /* Same computation with HOST buffers (pageable or pinned): copies the seven phantom arrays (and the initial
  * state, if any) to the device, runs bloch_simulate, copies the signal (and final state, if requested)
  * back and synchronises `stream` before returning.  d_scratch is caller-allocated device memory of at
@@ -140,6 +161,15 @@ int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins,
                         const float *h_T1, const float *h_T2, const float *h_dw,
                         float *h_Mxy, float *h_Mz, int init_equilibrium,
                         float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
+
+/* Host-buffer variant of bloch_simulate_motion (h_vx, h_vy, h_vz host arrays, all three NULL = no motion);
+ * scratch as bloch_simulate_host_scratch_bytes. */
+int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins,
+                               const float *h_x, const float *h_y, const float *h_z, const float *h_M0,
+                               const float *h_T1, const float *h_T2, const float *h_dw,
+                               const float *h_vx, const float *h_vy, const float *h_vz,
+                               float *h_Mxy, float *h_Mz, int init_equilibrium,
+                               float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
 
 /* Timing taps for the benchmark.  With bloch_plan_set_profiling(plan, 1) bloch_simulate records one CUDA
  * event on `stream` before every kernel it launches (and one after the last); off by default.  After the

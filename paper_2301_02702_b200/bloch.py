@@ -18,6 +18,8 @@ PHASE_AUTO, PHASE_FP32, PHASE_FP64 = 0, 1, 2
 OUT_SUM_ALL, OUT_PER_SPIN = 0, 1
 _PHASE = {"auto": PHASE_AUTO, "fp32": PHASE_FP32, "fp64": PHASE_FP64}
 _OUT = {"sum": OUT_SUM_ALL, "per_spin": OUT_PER_SPIN}
+MOTION_NONE, MOTION_LINEAR = 0, 1
+_MOTION = {"none": MOTION_NONE, "linear": MOTION_LINEAR}
 
 _dp = C.POINTER(C.c_double)
 _fp = C.c_void_p  # float* (host or device) passed as an address
@@ -35,19 +37,22 @@ class bloch_sequence(C.Structure):
 
 class bloch_sim_params(C.Structure):
     _fields_ = [("dt_max", C.c_double), ("dt_rf_max", C.c_double), ("max_block_points", C.c_int64),
-                ("phase_mode", C.c_int32), ("output_mode", C.c_int32)]
+                ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 class bloch_plan_info(C.Structure):
     _fields_ = [("n_intervals", C.c_int64), ("n_rf_steps", C.c_int64), ("n_adc", C.c_int64),
                 ("n_blocks", C.c_int64), ("n_rf_blocks", C.c_int64), ("n_eval_points", C.c_int64),
                 ("n_launches", C.c_int64), ("table_bytes", C.c_int64), ("max_block_adc", C.c_int64),
-                ("phase_mode", C.c_int32), ("output_mode", C.c_int32)]
+                ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",
            "bloch_plan_get_info", "bloch_plan_workspace_bytes", "bloch_plan_upload", "bloch_simulate",
-           "bloch_simulate_host_scratch_bytes", "bloch_simulate_host", "bloch_plan_set_profiling",
+           "bloch_simulate_motion", "bloch_simulate_host_scratch_bytes", "bloch_simulate_host",
+           "bloch_simulate_host_motion", "bloch_plan_set_profiling",
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_microbench"]
 
 
@@ -71,6 +76,9 @@ def _load():
     lib.bloch_simulate.argtypes = sim_args
     lib.bloch_simulate_host_scratch_bytes.argtypes = [vp, i64, C.POINTER(sz)]
     lib.bloch_simulate_host.argtypes = sim_args
+    mo_args = [vp, i64] + [_fp] * 10 + [_fp, _fp, C.c_int, _fp, vp, sz, vp]
+    lib.bloch_simulate_motion.argtypes = mo_args
+    lib.bloch_simulate_host_motion.argtypes = mo_args
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
@@ -115,7 +123,7 @@ def _darr(a):
 
 
 def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
-                      max_block_points: int = 0, phase_mode="auto", output_mode="sum") -> int:
+                      max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none") -> int:
     """seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
     Returns the opaque plan handle (an integer address)."""
     keep = []
@@ -138,7 +146,8 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     sc = bloch_scanner(float(gamma), 0.0, 0.0, 0.0)
     pm = _PHASE[phase_mode] if isinstance(phase_mode, str) else int(phase_mode)
     om = _OUT[output_mode] if isinstance(output_mode, str) else int(output_mode)
-    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om)
+    mm = _MOTION[motion] if isinstance(motion, str) else int(motion)
+    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, 0)
     h = C.c_void_p()
     _check(_lib.bloch_plan_create(C.byref(sc), C.byref(cs), C.byref(sp), C.byref(h)))
     return h.value
@@ -169,6 +178,20 @@ def bloch_simulate(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, Mxy, Mz, in
     """All array arguments are raw DEVICE addresses (ints) or None."""
     _check(_lib.bloch_simulate(plan, n_spins, x, y, z, M0, T1, T2, dw, Mxy, Mz, int(bool(init_equilibrium)),
                                signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
+                          init_equilibrium: bool, signal, workspace, workspace_bytes: int, stream: int = 0):
+    """bloch_simulate with per-spin velocities (raw DEVICE addresses or None for all three)."""
+    _check(_lib.bloch_simulate_motion(plan, n_spins, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
+                                      int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_host_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
+                               init_equilibrium: bool, signal, scratch, scratch_bytes: int, stream: int = 0):
+    """bloch_simulate_host with per-spin velocities (raw HOST addresses or None for all three)."""
+    _check(_lib.bloch_simulate_host_motion(plan, n_spins, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
+                                           int(bool(init_equilibrium)), signal, scratch, scratch_bytes, stream))
 
 
 def bloch_simulate_host_scratch_bytes(plan: int, n_spins: int) -> int:
@@ -251,8 +274,10 @@ class Plan:
             self._ws = torch.empty(need, dtype=torch.uint8, device="cuda")
         return self._ws
 
-    def simulate(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None):
-        """Device path: torch float32 CUDA tensors in, complex64 signal tensor out (asynchronous)."""
+    def simulate(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None,
+                 velocity=None):
+        """Device path: torch float32 CUDA tensors in, complex64 signal tensor out (asynchronous).
+        velocity: optional (vx, vy, vz) float32 CUDA tensors (plan created with motion="linear")."""
         import torch
         if self._tables is None:
             self.upload()
@@ -264,14 +289,20 @@ class Plan:
         if signal is None:
             signal = torch.empty(shape, dtype=torch.complex64, device="cuda")
         ws = self._workspace(n)
-        bloch_simulate(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(), T1.data_ptr(),
-                       T2.data_ptr(), dw.data_ptr(),
-                       None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
-                       init_equilibrium, signal.data_ptr() if signal.numel() else None,
-                       ws.data_ptr(), ws.numel(), self._stream())
+        vp = [None, None, None]
+        if velocity is not None:
+            for t in velocity:
+                assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
+            vp = [t.data_ptr() for t in velocity]
+        bloch_simulate_motion(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(), T1.data_ptr(),
+                              T2.data_ptr(), dw.data_ptr(), *vp,
+                              None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
+                              init_equilibrium, signal.data_ptr() if signal.numel() else None,
+                              ws.data_ptr(), ws.numel(), self._stream())
         return signal
 
-    def simulate_host(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None):
+    def simulate_host(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None,
+                      velocity=None):
         """End-to-end path: numpy float32 HOST arrays in, numpy complex64 signal out (synchronous)."""
         import torch
         if self._tables is None:
@@ -285,10 +316,14 @@ class Plan:
         need = max(bloch_simulate_host_scratch_bytes(self.handle, n), 256)
         if self._scratch is None or self._scratch.numel() < need:
             self._scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
-        bloch_simulate_host(self.handle, n, *[a.ctypes.data for a in arrs],
-                            None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
-                            init_equilibrium, signal.ctypes.data if signal.size else None,
-                            self._scratch.data_ptr(), self._scratch.numel(), self._stream())
+        vel = [None, None, None]
+        if velocity is not None:
+            vel = [np.ascontiguousarray(a, dtype=np.float32) for a in velocity]
+        bloch_simulate_host_motion(self.handle, n, *[a.ctypes.data for a in arrs],
+                                   *[None if a is None else a.ctypes.data for a in vel],
+                                   None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
+                                   init_equilibrium, signal.ctypes.data if signal.size else None,
+                                   self._scratch.data_ptr(), self._scratch.numel(), self._stream())
         return signal
 
 

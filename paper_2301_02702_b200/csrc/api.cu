@@ -87,6 +87,8 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
 struct Workspace {
     float4 *A, *C, *S;
     double4 *Ad;     // fp64-phase plans only
+    float4 *V;       // motion plans only: (vx, vy, vz, 0)
+    double4 *Vd;     // motion + fp64 phase
     unsigned *scal;  // device scalars: [0] = max 1/T2 (float bits)
     float2 *partial;
     size_t partial_elems;
@@ -118,6 +120,9 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.C = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.S = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.Ad = plan->info.phase_mode == BLOCH_PHASE_FP64 ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
+    const bool mo = plan->info.motion_mode == BLOCH_MOTION_LINEAR;
+    w.V = mo ? (float4 *)take(size_t(n_spins) * sizeof(float4)) : nullptr;
+    w.Vd = (mo && plan->info.phase_mode == BLOCH_PHASE_FP64) ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
     w.scal = (unsigned *)take(kAlign);
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
@@ -268,7 +273,21 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                    const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
                    const float *d_dw, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
                    void *d_workspace, size_t workspace_bytes, void *stream_) {
+    return bloch_simulate_motion(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, nullptr, nullptr, nullptr, d_Mxy,
+                                 d_Mz, init_equilibrium, d_signal, d_workspace, workspace_bytes, stream_);
+}
+
+int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                          const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                          const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz,
+                          float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                          void *d_workspace, size_t workspace_bytes, void *stream_) {
     if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    const bool has_v = d_vx || d_vy || d_vz;
+    if (has_v && !(d_vx && d_vy && d_vz)) return fail(BLOCH_EINVAL, "give all of d_vx, d_vy, d_vz or none");
+    if (has_v && plan->info.motion_mode != BLOCH_MOTION_LINEAR)
+        return fail(BLOCH_EINVAL, "velocities given but the plan was not created with BLOCH_MOTION_LINEAR");
+    const bool mo = plan->info.motion_mode == BLOCH_MOTION_LINEAR;
     if (n_spins < 0 || n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins out of range");
     if (!plan->d_tables) return fail(BLOCH_ENOTUPLOADED, "call bloch_plan_upload first");
     if (n_spins > 0 && (!d_x || !d_y || !d_z || !d_M0 || !d_T1 || !d_T2 || !d_dw))
@@ -300,11 +319,11 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
     BLOCH_CUDA(cudaMemsetAsync(w.scal, 0, kAlign, stream));
     pack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw,
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
-                                                     w.A, w.C, w.S, w.Ad, w.scal);
+                                                     w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
 
     bool pending = false;
-    PropRec prop{0, 0, 0, 0};
+    PropRec prop{0, 0, 0, 0, 0, 0, 0};
     // RF launch shape: one spin per thread; small CTAs when spins are few so the warps spread over all
     // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
     const int rf_threads = env_int("BLOCH_RF_THREADS", (n + 31) / 32 >= sms * 32 ? 128 : 32);
@@ -317,14 +336,14 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
             rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(plan->d_tables + b.table_off, (int)b.n_tiles, prop,
-                                                           pending ? 1 : 0, w.A, w.C, w.S, n);
+                                                           pending ? 1 : 0, w.A, w.C, w.S, w.V, n);
             ++launches;
             pending = false;
             continue;
         }
         if (pending) {  // two precession blocks in a row: apply the first one's end transform now
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, w.V, n);
             ++launches;
             pending = false;
         }
@@ -336,11 +355,11 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                 const long long total = (long long)n * n_pts;
                 const unsigned grid = (unsigned)((total + 255) / 256);
                 if (ph64)
-                    perspin_kernel<true><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, n,
+                    perspin_kernel<true><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n,
                                                                    (long long)plan->info.n_adc, (long long)b.adc_first,
                                                                    (float2 *)d_signal);
                 else
-                    perspin_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, n,
+                    perspin_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n,
                                                                     (long long)plan->info.n_adc, (long long)b.adc_first,
                                                                     (float2 *)d_signal);
                 ++launches;
@@ -364,19 +383,21 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                 }
                 const dim3 grid(s.ptiles, s.chunks);
                 const int row = (int)batch_pts, poff = (int)batch_done;
+#define BLOCH_LAUNCH_SIG3(PP, H, M, AP, VP)                                                                    \
+    signal_kernel<PP, H, M><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, VP, w.S, n, s.spins_per_chunk,  \
+                                                              (const float *)w.scal, w.partial, row, poff)
 #define BLOCH_LAUNCH_SIG(PP)                                                                                   \
     do {                                                                                                       \
-        if (ph64)                                                                                              \
-            signal_kernel<PP, true><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.Ad, w.S, n,               \
-                s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);                               \
-        else                                                                                                   \
-            signal_kernel<PP, false><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, w.A, w.S, n,               \
-                s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);                               \
+        if (ph64 && mo) BLOCH_LAUNCH_SIG3(PP, true, true, w.Ad, w.Vd);                                         \
+        else if (ph64) BLOCH_LAUNCH_SIG3(PP, true, false, w.Ad, nullptr);                                      \
+        else if (mo) BLOCH_LAUNCH_SIG3(PP, false, true, w.A, w.V);                                             \
+        else BLOCH_LAUNCH_SIG3(PP, false, false, w.A, nullptr);                                                \
     } while (0)
                 if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
                 else BLOCH_LAUNCH_SIG(1);
 #undef BLOCH_LAUNCH_SIG
+#undef BLOCH_LAUNCH_SIG3
                 ++launches;
                 batch_done += n_pts;
                 if (batch_done == batch_pts) {  // batch complete: second pass over all its points
@@ -392,12 +413,15 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
         prop.ky = b.kend[1];
         prop.kz = b.kend[2];
         prop.tau = b.tau_end;
+        prop.mx = b.mend[0];
+        prop.my = b.mend[1];
+        prop.mz = b.mend[2];
         pending = true;
     }
     if (d_Mxy) {
         if (pending) {
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, n);
+            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, w.V, n);
             ++launches;
         }
         if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
@@ -420,7 +444,7 @@ int bloch_simulate_host_scratch_bytes(const bloch_plan *plan, int64_t n_spins, s
     const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
                            ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
                            : size_t(plan->info.n_adc) * sizeof(float2);
-    *out = 10 * arr + align_up(sig, kAlign) + ws + kAlign;
+    *out = 13 * arr + align_up(sig, kAlign) + ws + kAlign;
     return BLOCH_OK;
 }
 
@@ -428,7 +452,18 @@ int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins, const float *h_
                         const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
                         const float *h_dw, float *h_Mxy, float *h_Mz, int init_equilibrium, float *h_signal,
                         void *d_scratch, size_t scratch_bytes, void *stream_) {
+    return bloch_simulate_host_motion(plan, n_spins, h_x, h_y, h_z, h_M0, h_T1, h_T2, h_dw, nullptr, nullptr, nullptr,
+                                      h_Mxy, h_Mz, init_equilibrium, h_signal, d_scratch, scratch_bytes, stream_);
+}
+
+int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                               const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                               const float *h_dw, const float *h_vx, const float *h_vy, const float *h_vz,
+                               float *h_Mxy, float *h_Mz, int init_equilibrium, float *h_signal,
+                               void *d_scratch, size_t scratch_bytes, void *stream_) {
     if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    const bool has_v = h_vx || h_vy || h_vz;
+    if (has_v && !(h_vx && h_vy && h_vz)) return fail(BLOCH_EINVAL, "give all of h_vx, h_vy, h_vz or none");
     size_t need = 0;
     int rc = bloch_simulate_host_scratch_bytes(plan, n_spins, &need);
     if (rc) return rc;
@@ -458,11 +493,20 @@ int bloch_simulate_host(const bloch_plan *plan, int64_t n_spins, const float *h_
     const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
                            ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
                            : size_t(plan->info.n_adc) * sizeof(float2);
-    float *d_sig = (float *)(base + 10 * arr);
-    unsigned char *d_ws = base + 10 * arr + align_up(sig, kAlign);
+    float *d_v[3] = {nullptr, nullptr, nullptr};
+    if (has_v) {
+        const float *hv[3] = {h_vx, h_vy, h_vz};
+        for (int k = 0; k < 3; ++k) {
+            d_v[k] = (float *)(base + (10 + k) * arr);
+            if (n_spins > 0)
+                BLOCH_CUDA(cudaMemcpyAsync(d_v[k], hv[k], size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+        }
+    }
+    float *d_sig = (float *)(base + 13 * arr);
+    unsigned char *d_ws = base + 13 * arr + align_up(sig, kAlign);
     const size_t ws_bytes = scratch_bytes - (size_t)(d_ws - base);
-    rc = bloch_simulate(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d_Mxy, d_Mz, init_equilibrium,
-                        d_sig, d_ws, ws_bytes, stream_);
+    rc = bloch_simulate_motion(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d_v[0], d_v[1], d_v[2], d_Mxy,
+                               d_Mz, init_equilibrium, d_sig, d_ws, ws_bytes, stream_);
     if (rc) return rc;
     if (sig > 0) BLOCH_CUDA(cudaMemcpyAsync(h_signal, d_sig, sig, cudaMemcpyDeviceToHost, stream));
     if (h_Mxy && n_spins > 0) {

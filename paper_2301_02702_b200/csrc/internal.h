@@ -26,8 +26,12 @@ constexpr size_t kAlign = 256;
 //       32 B  (wx, wy, wx^2 + wy^2, 0) (gx, gy, gz, 0)      g = gamma * dt * mean G of the step (reading G5)
 constexpr int kRfTileSteps = 128;
 constexpr int kRfHdrBytes = 64;
-constexpr int kRfTileBytesMax = kRfHdrBytes + kRfTileSteps * 32;
+//   motion (kRfFlagMotion, never compact)
+//       48 B  general record + (hx, hy, hz, 0)     h = gamma * dt * (G_n t_n + G_{n+1} t_{n+1}) / 2, so that
+//                                                  gamma Bz dt = g . x + h . v + dw dt for x(t) = x + v t
+constexpr int kRfTileBytesMax = kRfHdrBytes + kRfTileSteps * 48;
 constexpr int kRfFlagUniformG = 1;
+constexpr int kRfFlagMotion = 2;
 struct RfTileHdr {
     float wxy2_max, gx_max, gy_max, gz_max;  // max over the tile's steps of wx^2+wy^2, |gx|, |gy|, |gz|
     float dt;                                // step length [s], the same for every step of the tile
@@ -35,7 +39,7 @@ struct RfTileHdr {
     int32_t flags;
     float pad0;
     float gx, gy, gz, pad1;                  // the tile's gradient part when kRfFlagUniformG
-    float pad2[4];
+    float hx_max, hy_max, hz_max, pad2;      // max |hx|, |hy|, |hz| (kRfFlagMotion)
 };
 static_assert(sizeof(RfTileHdr) == kRfHdrBytes, "RfTileHdr must be 64 B");
 
@@ -52,6 +56,7 @@ struct Block {
     // precession block end record: k' = -gamma_bar * K(T) [turns/m] and tau = T [s] (Eq 12-13)
     double kend[3] = {0, 0, 0};
     double tau_end = 0;
+    double mend[3] = {0, 0, 0};  // motion: first moment mu' = -gamma_bar * sum (G_n t_n + G_{n+1} t_{n+1}) dt / 2 [turns s/m]
 };
 
 struct Timing {

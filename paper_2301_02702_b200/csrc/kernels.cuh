@@ -2,6 +2,7 @@
 //
 // Internal spin layout (built once per bloch_simulate by pack_kernel, 48 B per spin; +32 B with fp64 phase):
 //   A[i] = (x, y, z, f')        f' = -dw  [rad/s]                  constant
+//   V[i]  = (vx, vy, vz, 0)     velocity [m/s], motion plans only (Vd[i]: the same as doubles, fp64 phase)
 //   Ad[i] = (x, y, z, f') as doubles, f' = -dw / (2 pi) [turns/s]  constant, fp64-phase plans only
 //   C[i] = (1/T1, 1/T2, M0, dw)                                   constant
 //   S[i] = (Mxy.re, Mxy.im, Mz, e2)   e2 = -(1/T2) log2(e)        state (e2 rides along for the signal kernel)
@@ -34,7 +35,9 @@ __global__ void pack_kernel(int n, const float *__restrict__ x, const float *__r
                             const float *__restrict__ dw, const float2 *__restrict__ Mxy,
                             const float *__restrict__ Mz, int init_eq, float4 *__restrict__ A,
                             float4 *__restrict__ Cc, float4 *__restrict__ S, double4 *__restrict__ Ad,
-                            unsigned *__restrict__ scal) {
+                            unsigned *__restrict__ scal, const float *__restrict__ vx,
+                            const float *__restrict__ vy, const float *__restrict__ vz, float4 *__restrict__ V,
+                            double4 *__restrict__ Vd) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     // scal[0] = max 1/T2 over the spins.  The bit pattern of a non-negative float orders like the unsigned
     // integer and an integer max is order-independent, so this stays reproducible.
@@ -46,6 +49,11 @@ __global__ void pack_kernel(int n, const float *__restrict__ x, const float *__r
     const float r1 = 1.0f / T1[i], r2 = 1.0f / T2[i], m0 = M0[i], w = dw[i];
     A[i] = make_float4(x[i], y[i], z[i], -w);
     if (Ad) Ad[i] = make_double4((double)x[i], (double)y[i], (double)z[i], -(double)w * 0.15915494309189535);
+    if (V) {  // motion plan: zero velocity when the caller gave none
+        const float a = vx ? vx[i] : 0.f, b = vy ? vy[i] : 0.f, c = vz ? vz[i] : 0.f;
+        V[i] = make_float4(a, b, c, 0.f);
+        if (Vd) Vd[i] = make_double4((double)a, (double)b, (double)c, 0.0);
+    }
     Cc[i] = make_float4(r1, r2, m0, w);
     float4 s;
     if (init_eq) {
@@ -74,12 +82,14 @@ __global__ void unpack_kernel(int n, const float4 *__restrict__ S, float2 *__res
 // ------------------------------------------------------------------------------------------------
 struct PropRec {
     double kx, ky, kz, tau;  // k' = -gamma_bar K(T) [turns/m], tau = T [s]
+    double mx, my, mz;       // motion: first moment mu'(T) [turns s/m]
 };
 
-__device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, const float4 &c, float &mx,
-                                          float &my, float &mz) {
+__device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, const float4 &c, const float4 &v,
+                                          float &mx, float &my, float &mz) {
     double th = p.kx * (double)a.x + p.ky * (double)a.y + p.kz * (double)a.z -
                 (double)c.w * 0.15915494309189535 * p.tau;
+    th += p.mx * (double)v.x + p.my * (double)v.y + p.mz * (double)v.z;  // x(t) = x + v t
     th -= rint(th);
     float sn, cs;
     sincospif(2.0f * (float)th, &sn, &cs);
@@ -96,22 +106,36 @@ __device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, con
 template <bool PH64>
 __global__ void __launch_bounds__(256)
 perspin_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restrict__ A,
-               const float4 *__restrict__ Cc, const float4 *__restrict__ S, int n_spins,
-               long long n_adc_total, long long adc_first, float2 *__restrict__ out) {
+               const float4 *__restrict__ Cc, const float4 *__restrict__ S, const float4 *__restrict__ V,
+               int n_spins, long long n_adc_total, long long adc_first, float2 *__restrict__ out) {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)n_spins * n_pts) return;
     const int sp = (int)(gid / n_pts), p = (int)(gid % n_pts);
-    double kx, ky, kz, tau;
+    double kx, ky, kz, tau, ux = 0., uy = 0., uz = 0.;
+    const int rs = V ? 2 : 1;  // motion plans: (k', tau) is followed by (mu', 0)
     if (PH64) {
-        const double4 r = reinterpret_cast<const double4 *>(recs_)[p];
+        const double4 r = reinterpret_cast<const double4 *>(recs_)[rs * p];
         kx = r.x; ky = r.y; kz = r.z; tau = r.w;
+        if (V) {
+            const double4 m = reinterpret_cast<const double4 *>(recs_)[rs * p + 1];
+            ux = m.x; uy = m.y; uz = m.z;
+        }
     } else {
-        const float4 r = reinterpret_cast<const float4 *>(recs_)[p];  // fp32-phase tables hold k' in rad/m
+        const float4 r = reinterpret_cast<const float4 *>(recs_)[rs * p];  // fp32-phase tables hold k' in rad/m
         kx = (double)r.x * 0.15915494309189535; ky = (double)r.y * 0.15915494309189535;
         kz = (double)r.z * 0.15915494309189535; tau = r.w;
+        if (V) {
+            const float4 m = reinterpret_cast<const float4 *>(recs_)[rs * p + 1];
+            ux = (double)m.x * 0.15915494309189535; uy = (double)m.y * 0.15915494309189535;
+            uz = (double)m.z * 0.15915494309189535;
+        }
     }
     const float4 a = A[sp], c = Cc[sp], s = S[sp];
     double th = kx * (double)a.x + ky * (double)a.y + kz * (double)a.z - (double)c.w * 0.15915494309189535 * tau;
+    if (V) {
+        const float4 v = V[sp];
+        th += ux * (double)v.x + uy * (double)v.y + uz * (double)v.z;
+    }
     th -= rint(th);
     float sn, cs;
     sincospif(2.0f * (float)th, &sn, &cs);

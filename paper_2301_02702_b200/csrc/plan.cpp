@@ -70,6 +70,11 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         return fail(BLOCH_EINVAL, "bad phase_mode");
     if (params->output_mode != BLOCH_OUT_SUM_ALL && params->output_mode != BLOCH_OUT_PER_SPIN)
         return fail(BLOCH_EINVAL, "bad output_mode");
+    if (params->motion_mode != BLOCH_MOTION_NONE && params->motion_mode != BLOCH_MOTION_LINEAR)
+        return fail(BLOCH_EINVAL, "bad motion_mode");
+    const bool motion = params->motion_mode == BLOCH_MOTION_LINEAR;
+    const double dt_mo = (motion && params->dt_max > 0.0 && std::isfinite(params->dt_max))
+                             ? params->dt_max : std::numeric_limits<double>::infinity();
     for (int a = 0; a < 3; ++a) {
         if (seq->g_n[a] < 0 || (seq->g_n[a] > 0 && (!seq->g_t[a] || !seq->g_v[a])))
             return fail(BLOCH_EINVAL, "gradient arrays NULL or negative count");
@@ -133,8 +138,10 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             while (j < seq->rf_n && seq->rf_t[j] + seq->rf_dt[j] <= mid) ++j;
             const bool covered = (j < seq->rf_n && seq->rf_t[j] <= mid);
             int64_t parts = 1;
-            // a piece is longer than dt_rf_max only beyond the time tolerance (readings G13 + G18)
-            if (covered && std::isfinite(dt_rf)) parts = std::max<int64_t>(1, (int64_t)std::ceil(((b - a) - kTimeTol) / dt_rf));
+            // a piece is longer than its limit only beyond the time tolerance (readings G13 + G18); with motion
+            // every interval is also limited to dt_max
+            const double lim = std::min(covered ? dt_rf : std::numeric_limits<double>::infinity(), dt_mo);
+            if (std::isfinite(lim)) parts = std::max<int64_t>(1, (int64_t)std::ceil(((b - a) - kTimeTol) / lim));
             for (int64_t p = 1; p <= parts; ++p) {
                 t.push_back(p == parts ? b : a + (b - a) * (double(p) / double(parts)));
                 rf_of.push_back(covered ? j : -1);
@@ -207,6 +214,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     const double gbar = gamma / (2.0 * M_PI);
     double worst_turns = 0.0;
     std::vector<double> krec;  // 4 doubles per evaluated point, all precession blocks in order
+    std::vector<double> mrec;  // motion: (mu'x, mu'y, mu'z, 0) per evaluated point, same order
     std::vector<int64_t> krec_first(blocks.size(), 0);
     int64_t n_rf_steps = 0, n_rf_blocks = 0, n_eval = 0, max_block_adc = 0;
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
@@ -218,18 +226,28 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         }
         krec_first[bi] = (int64_t)krec.size() / 4;
         const bool serve_start = (bi == 0) || (blocks[bi - 1].type == kBlockRF);
-        double K[3] = {0, 0, 0};
+        double K[3] = {0, 0, 0}, Mo[3] = {0, 0, 0};
         const double tb = t[b.first];
-        if (serve_start && adc_at[b.first] >= 0) krec.insert(krec.end(), {0.0, 0.0, 0.0, 0.0});
+        if (serve_start && adc_at[b.first] >= 0) {
+            krec.insert(krec.end(), {0.0, 0.0, 0.0, 0.0});
+            if (motion) mrec.insert(mrec.end(), {0.0, 0.0, 0.0, 0.0});
+        }
         for (int64_t n = b.first; n < b.first + b.count; ++n) {
             const double dt = t[n + 1] - t[n];
             for (int a = 0; a < 3; ++a) K[a] += 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]) * dt;  // Eq 12-13
+            // motion: the same trapezoid on G(t) t, so that sum of Bz(t_n) = G_n . (x + v t_n) splits into K . x + Mo . v
+            for (int a = 0; a < 3; ++a) Mo[a] += 0.5 * (G[3 * n + a] * t[n] + G[3 * (n + 1) + a] * t[n + 1]) * dt;
             const double tau = t[n + 1] - tb;
             const double kn = gbar * std::sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]);
-            worst_turns = std::max(worst_turns, kn * 0.25 + 1000.0 * tau);
-            if (adc_at[n + 1] >= 0) krec.insert(krec.end(), {-gbar * K[0], -gbar * K[1], -gbar * K[2], tau});
+            const double mn = gbar * std::sqrt(Mo[0] * Mo[0] + Mo[1] * Mo[1] + Mo[2] * Mo[2]);
+            worst_turns = std::max(worst_turns, kn * 0.25 + 1000.0 * tau + (motion ? mn * 1.0 : 0.0));  // |v| <= 1 m/s
+            if (adc_at[n + 1] >= 0) {
+                krec.insert(krec.end(), {-gbar * K[0], -gbar * K[1], -gbar * K[2], tau});
+                if (motion) mrec.insert(mrec.end(), {-gbar * Mo[0], -gbar * Mo[1], -gbar * Mo[2], 0.0});
+            }
         }
         for (int a = 0; a < 3; ++a) b.kend[a] = -gbar * K[a];
+        for (int a = 0; a < 3; ++a) b.mend[a] = -gbar * Mo[a];
         b.tau_end = t[b.first + b.count] - tb;
         n_eval += b.adc_count + 1;
         max_block_adc = std::max(max_block_adc, b.adc_count);
@@ -248,7 +266,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         if (b.type != kBlockRF) continue;
         // per step, in fp32 as the kernel sees them: rotation vector w = gamma * B * dt (Eq 8); the gradient
         // part is per metre, mean of the two vertex values (reading G5)
-        struct StepF { float wx, wy, g[3], dt; };
+        struct StepF { float wx, wy, g[3], dt, h[3]; };
         std::vector<StepF> st((size_t)b.count);
         for (int64_t n = b.first; n < b.first + b.count; ++n) {
             const double dt = t[n + 1] - t[n];
@@ -257,6 +275,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             s.wx = (float)(gamma * dt * seq->rf_re[j]);
             s.wy = (float)(gamma * dt * seq->rf_im[j]);
             for (int a = 0; a < 3; ++a) s.g[a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]));
+            for (int a = 0; a < 3; ++a)
+                s.h[a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] * t[n] + G[3 * (n + 1) + a] * t[n + 1]));
             s.dt = (float)dt;
         }
         // cut into tiles: at most kRfTileSteps steps, one dt per tile
@@ -283,12 +303,18 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                 h.gy_max = std::max(h.gy_max, std::fabs(s.g[1]));
                 h.gz_max = std::max(h.gz_max, std::fabs(s.g[2]));
                 uniform = uniform && s.g[0] == st[k0].g[0] && s.g[1] == st[k0].g[1] && s.g[2] == st[k0].g[2];
+                if (motion) {
+                    h.hx_max = std::max(h.hx_max, std::fabs(s.h[0]));
+                    h.hy_max = std::max(h.hy_max, std::fabs(s.h[1]));
+                    h.hz_max = std::max(h.hz_max, std::fabs(s.h[2]));
+                }
             }
+            if (motion) uniform = false;  // h = g t changes with every step
             h.dt = st[k0].dt;
             h.n_steps = (int32_t)c;
-            h.flags = uniform ? kRfFlagUniformG : 0;
+            h.flags = (uniform ? kRfFlagUniformG : 0) | (motion ? kRfFlagMotion : 0);
             h.gx = st[k0].g[0]; h.gy = st[k0].g[1]; h.gz = st[k0].g[2];
-            const size_t rec = uniform ? 16 : 32;
+            const size_t rec = motion ? 48 : (uniform ? 16 : 32);
             const size_t off0 = img.size();
             img.resize(off0 + kRfHdrBytes + c * rec, 0);
             std::memcpy(img.data() + off0, &h, sizeof(h));
@@ -297,6 +323,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                 const StepF &s = st[k];
                 r[0] = s.wx; r[1] = s.wy; r[2] = s.wx * s.wx + s.wy * s.wy; r[3] = 0.f;
                 if (!uniform) { r[4] = s.g[0]; r[5] = s.g[1]; r[6] = s.g[2]; r[7] = 0.f; }
+                if (motion) { r[8] = s.h[0]; r[9] = s.h[1]; r[10] = s.h[2]; r[11] = 0.f; }
             }
             int32_t *dir = reinterpret_cast<int32_t *>(img.data());
             dir[2 * ti] = (int32_t)off0;
@@ -307,7 +334,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
 
     // ------------------------------------------------------------------ tables: layout + fill
     size_t off = 0;
-    const size_t rec_bytes = phase == BLOCH_PHASE_FP64 ? 32 : 16;
+    // precession records: (k', tau) per ADC sample, followed by (mu', 0) with motion
+    const size_t rec_bytes = (phase == BLOCH_PHASE_FP64 ? 32 : 16) * (motion ? 2 : 1);
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
         Block &b = blocks[bi];
         b.table_off = (int64_t)off;
@@ -323,13 +351,21 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             std::memcpy(dst, rf_img[bi].data(), rf_img[bi].size());
         } else {
             const double *src = krec.data() + 4 * krec_first[bi];
+            const double *msrc = motion ? mrec.data() + 4 * krec_first[bi] : nullptr;
+            const int stride = motion ? 8 : 4;  // scalars per point
             if (phase == BLOCH_PHASE_FP64) {
-                std::memcpy(dst, src, size_t(b.adc_count) * 32);
+                double *r = reinterpret_cast<double *>(dst);
+                for (int64_t i = 0; i < b.adc_count; ++i) {
+                    for (int c = 0; c < 4; ++c) r[stride * i + c] = src[4 * i + c];
+                    if (motion) for (int c = 0; c < 4; ++c) r[stride * i + 4 + c] = msrc[4 * i + c];
+                }
             } else {
-                // fp32 phase: k' in rad/m (the signal kernel's phase is in radians), tau in s
+                // fp32 phase: k', mu' in rad (the signal kernel's phase is in radians), tau in s
                 float *r = reinterpret_cast<float *>(dst);
-                for (int64_t i = 0; i < 4 * b.adc_count; ++i)
-                    r[i] = (float)((i & 3) == 3 ? src[i] : 2.0 * M_PI * src[i]);
+                for (int64_t i = 0; i < b.adc_count; ++i) {
+                    for (int c = 0; c < 4; ++c) r[stride * i + c] = (float)(c == 3 ? src[4 * i + c] : 2.0 * M_PI * src[4 * i + c]);
+                    if (motion) for (int c = 0; c < 4; ++c) r[stride * i + 4 + c] = (float)(2.0 * M_PI * msrc[4 * i + c]);
+                }
             }
         }
     }
@@ -363,6 +399,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     inf.max_block_adc = max_block_adc;
     inf.phase_mode = phase;
     inf.output_mode = params->output_mode;
+    inf.motion_mode = params->motion_mode;
+    inf.reserved = 0;
     return BLOCH_OK;
 }
 

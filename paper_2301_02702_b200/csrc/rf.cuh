@@ -28,6 +28,7 @@ namespace bloch {
 
 struct RfSpin {
     float x, y, z, dw, r1, r2, m0;
+    float vx, vy, vz;  // motion plans (x(t) = x + v t); zero otherwise
 };
 struct RfRelax {
     float E1, E2, D1, D2, D1m0;
@@ -91,7 +92,8 @@ __device__ __forceinline__ void fold(float &hi, float &lo) {
 }
 
 // One tile of steps.  State in and out as (h, l) with h + l the magnetisation.
-template <int TIER, bool UG>
+// MODE 0: compact records (uniform gradient part), 1: general records, 2: general + motion records.
+template <int TIER, int MODE>
 __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileHdr &hd, const RfSpin &sp,
                                         const RfRelax &rx, float &hx, float &hy, float &hz, float &lx, float &ly,
                                         float &lz) {
@@ -103,13 +105,19 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
     const float wz2_u = wz_u * wz_u;
 #define BLOCH_RF_LOAD(k)                                                              \
     float wx, wy, wz, q;                                                              \
-    if (UG) {                                                                         \
+    if (MODE == 0) {                                                                  \
         const float4 a = rec[k];                                                      \
         wx = a.x; wy = a.y; wz = wz_u; q = a.z + wz2_u;                               \
-    } else {                                                                          \
+    } else if (MODE == 1) {                                                           \
         const float4 a = rec[2 * (k)], g = rec[2 * (k) + 1];                          \
         wx = a.x; wy = a.y;                                                           \
         wz = fmaf(g.x, sp.x, fmaf(g.y, sp.y, fmaf(g.z, sp.z, dtdw)));                 \
+        q = fmaf(wz, wz, a.z);                                                        \
+    } else {                                                                          \
+        const float4 a = rec[3 * (k)], g = rec[3 * (k) + 1], h = rec[3 * (k) + 2];    \
+        wx = a.x; wy = a.y;                                                           \
+        wz = fmaf(g.x, sp.x, fmaf(g.y, sp.y, fmaf(g.z, sp.z, dtdw)));                 \
+        wz = fmaf(h.x, sp.vx, fmaf(h.y, sp.vy, fmaf(h.z, sp.vz, wz)));                \
         q = fmaf(wz, wz, a.z);                                                        \
     }
     if (TIER == 0) {
@@ -151,7 +159,8 @@ constexpr int kRfMaxThreads = 128;
 
 __global__ void __launch_bounds__(kRfMaxThreads)
 rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int has_prop,
-          const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
+          const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S,
+          const float4 *__restrict__ V /* motion plans, else NULL */, int n) {
     __shared__ __align__(128) unsigned char buf[2][kRfTileBytesMax];
     __shared__ __align__(8) uint64_t bar[2];
     const int tid = threadIdx.x;
@@ -170,16 +179,19 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
     const bool active = i < n;
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f),
            s = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
     if (active) {
         a = A[i];
         c = Cc[i];
         s = S[i];
+        if (V) v = V[i];
     }
     float hx = s.x, hy = s.y, hz = s.z;
-    if (has_prop) propagate(prop, a, c, hx, hy, hz);
+    if (has_prop) propagate(prop, a, c, v, hx, hy, hz);
     float lx = 0.f, ly = 0.f, lz = 0.f;
-    const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z};
+    const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z, v.x, v.y, v.z};
     const float ax = fabsf(sp.x), ay = fabsf(sp.y), az = fabsf(sp.z), adw = fabsf(sp.dw);
+    const float avx = fabsf(v.x), avy = fabsf(v.y), avz = fabsf(v.z);
     __syncthreads();  // barrier initialisation visible to every waiter
 
     for (int t = 0; t < n_tiles; ++t) {
@@ -194,20 +206,23 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         rx.E2 = 1.0f - rx.D2;
         rx.D1m0 = rx.D1 * sp.m0;
         // bound on q = |w|^2 over the tile for this spin -> tier, decided per warp
-        const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
+        float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
+        wzb = fmaf(hd.hx_max, avx, fmaf(hd.hy_max, avy, fmaf(hd.hz_max, avz, wzb)));
         const float qb = fmaf(wzb, wzb, hd.wxy2_max);
-        const bool ug = (hd.flags & kRfFlagUniformG) != 0;
+        const int mode = (hd.flags & kRfFlagMotion) ? 2 : ((hd.flags & kRfFlagUniformG) ? 0 : 1);
         const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
-        if (tier == 0) {
-            if (ug) rf_tile<0, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-            else rf_tile<0, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-        } else if (tier == 1) {
-            if (ug) rf_tile<1, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-            else rf_tile<1, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-        } else {
-            if (ug) rf_tile<2, true>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-            else rf_tile<2, false>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);
-        }
+#define BLOCH_RF_TILE(T, M) rf_tile<T, M>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz)
+#define BLOCH_RF_MODES(T)                       \
+    do {                                        \
+        if (mode == 0) BLOCH_RF_TILE(T, 0);     \
+        else if (mode == 1) BLOCH_RF_TILE(T, 1);\
+        else BLOCH_RF_TILE(T, 2);               \
+    } while (0)
+        if (tier == 0) BLOCH_RF_MODES(0);
+        else if (tier == 1) BLOCH_RF_MODES(1);
+        else BLOCH_RF_MODES(2);
+#undef BLOCH_RF_MODES
+#undef BLOCH_RF_TILE
         __syncthreads();  // every thread is done reading buf[b]
         if (tid == 0 && t + 2 < n_tiles) {
             const int2 d = dir[t + 2];

@@ -36,9 +36,11 @@ namespace bloch {
 constexpr int kSigThreads = 256;
 constexpr int kSigTile = 256;  // spins per staged tile
 
-template <int P, bool PH64>
+// MO (motion plans): every record (k', tau) is followed by (mu', 0), the spins' velocities are a third staged
+// tile, and the phase gains mu' . v (x(t) = x + v t).
+template <int P, bool PH64, bool MO>
 __global__ void __launch_bounds__(kSigThreads)
-signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
+signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_, const void *__restrict__ V_,
               const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
               const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial,
               int row_stride /* points of the whole batch */, int p_off /* this block's first point in the batch */) {
@@ -47,9 +49,12 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
     using real = typename std::conditional<PH64, double, float>::type;
     __shared__ __align__(128) PosT shA[2][kSigTile];
     __shared__ __align__(128) float4 shS[2][kSigTile];
+    __shared__ __align__(128) PosT shV[MO ? 2 : 1][MO ? kSigTile : 1];
     __shared__ __align__(8) uint64_t bar[2];
     const RecT *recs = reinterpret_cast<const RecT *>(recs_);
     const PosT *A = reinterpret_cast<const PosT *>(A_);
+    const PosT *V = reinterpret_cast<const PosT *>(V_);
+    constexpr int RS = MO ? 2 : 1;
     const int tid = threadIdx.x;
     const int s0 = blockIdx.y * spins_per_chunk;
     const int s1 = min(n_spins, s0 + spins_per_chunk);
@@ -58,9 +63,10 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         const int b = t & 1;
         const int base = s0 + t * kSigTile;
         const uint32_t cnt = (uint32_t)min(kSigTile, s1 - base);
-        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + sizeof(float4)));
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)((MO ? 2 : 1) * sizeof(PosT) + sizeof(float4)));
         bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
         bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
+        if (MO) bulk_g2s(shV[b], V + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
     };
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -71,7 +77,7 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
     }
     // the thread's P points are ADJACENT ADC samples, so tau_j - tau_0 is a few dwell times
     const int p0 = (blockIdx.x * kSigThreads + tid) * P;
-    real kx[P], ky[P], kz[P], tau[P];
+    real kx[P], ky[P], kz[P], tau[P], ux[MO ? P : 1], uy[MO ? P : 1], uz[MO ? P : 1];
     float tf[P], cj[P], ar[P], ai[P];
     float cmax = 0.f;
 #pragma unroll
@@ -79,8 +85,14 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         const int p = p0 + j;
         RecT r;
         r.x = 0; r.y = 0; r.z = 0; r.w = j ? tau[0] : (real)0;
-        if (p < n_pts) r = recs[p];
+        if (p < n_pts) r = recs[RS * p];
         kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
+        if (MO) {
+            RecT m;
+            m.x = 0; m.y = 0; m.z = 0; m.w = 0;
+            if (p < n_pts) m = recs[RS * p + 1];
+            ux[j] = m.x; uy[j] = m.y; uz[j] = m.z;
+        }
         tf[j] = (float)r.w;
         cj[j] = (float)(r.w - tau[0]) * 0.6931471805599453f;  // (tau_j - tau_0) ln 2; times e2 = -(tau_j - tau_0)/T2
         cmax = fmaxf(cmax, fabsf(cj[j]));
@@ -100,6 +112,9 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         for (int s = 0; s < cnt; ++s) {
             const PosT a = shA[b][s];
             const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            PosT vv;
+            vv.x = 0; vv.y = 0; vv.z = 0; vv.w = 0;
+            if (MO) vv = shV[b][s];
             float er0 = 0.f, ei0 = 0.f;
 #pragma unroll
             for (int j = 0; j < P; ++j) {
@@ -107,6 +122,8 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
                 if (PH64) {
                     double th = fma((double)kx[j], (double)a.x, fma((double)ky[j], (double)a.y,
                                     fma((double)kz[j], (double)a.z, (double)tau[j] * (double)a.w)));  // turns
+                    if (MO) th = fma((double)ux[j], (double)vv.x, fma((double)uy[j], (double)vv.y,
+                                     fma((double)uz[j], (double)vv.z, th)));
                     th += 1572864.0;  // 1.5 * 2^20: ulp = 2^-32, low word = frac(theta) in 0.32 fixed point
                     const unsigned lo = (unsigned)__double2loint(th);
                     const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;  // [0, 1) turns
@@ -114,8 +131,10 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
                     sn = __sinf(ang);
                     cs = __cosf(ang);
                 } else {
-                    const float th = fmaf((float)kx[j], (float)a.x, fmaf((float)ky[j], (float)a.y,
-                                          fmaf((float)kz[j], (float)a.z, (float)tau[j] * (float)a.w)));  // radians
+                    float th = fmaf((float)kx[j], (float)a.x, fmaf((float)ky[j], (float)a.y,
+                                    fmaf((float)kz[j], (float)a.z, (float)tau[j] * (float)a.w)));  // radians
+                    if (MO) th = fmaf((float)ux[j], (float)vv.x, fmaf((float)uy[j], (float)vv.y,
+                                      fmaf((float)uz[j], (float)vv.z, th)));
                     sn = __sinf(th);  // FMUL by 1/(2 pi) + MUFU.SIN
                     cs = __cosf(th);
                 }

@@ -1,0 +1,132 @@
+"""GPU-vs-oracle parity with moving spins, x(t) = x + v t.
+Same acceptance as the static path: max <= 1e-4, NRMSE <= 1e-5 of the oracle maximum."""
+import numpy as np
+import pytest
+
+from paper_2301_02702_b200 import workloads as W
+from seqtools import seq
+
+pytestmark = pytest.mark.gpu
+
+TOL_MAX = 1e-4
+TOL_NRMSE = 1e-5
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2301_02702_b200 import build as bl
+    bl.build()
+    from paper_2301_02702_b200 import bloch
+    return bloch
+
+
+def errors(got, ref):
+    got = np.asarray(got, dtype=np.complex128)
+    ref = np.asarray(ref, dtype=np.complex128)
+    scale = np.abs(ref).max()
+    d = np.abs(got - ref)
+    return d.max() / scale, np.sqrt(np.mean(d ** 2)) / scale
+
+
+def f32(a):
+    return np.asarray(a, dtype=np.float32).astype(np.float64)
+
+
+def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mode="auto", host=False):
+    import torch
+    v = tuple(f32(a) for a in v)
+    plan = B.Plan(s, output_mode=output_mode, phase_mode=phase_mode, motion="linear", dt_max=dt_max)
+    assert plan.info["motion_mode"] == 1
+    t, *_ = oracle_mod.grid(s, dt_max=dt_max)
+    assert plan.info["n_intervals"] == len(t) - 1, "planner and oracle refine the grid differently"
+    if host:
+        Mxy = np.zeros((ph.n, 2), dtype=np.float32)
+        Mz = np.zeros(ph.n, dtype=np.float32)
+        sig = plan.simulate_host(ph.x, ph.y, ph.z, ph.M0, ph.T1, ph.T2, ph.dw, Mxy=Mxy, Mz=Mz, velocity=v)
+        m, z = Mxy, Mz
+    else:
+        dev = B.phantom_to_device(ph)
+        vel = tuple(torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in v)
+        Mxy = torch.zeros(ph.n, 2, dtype=torch.float32, device="cuda")
+        Mz = torch.zeros(ph.n, dtype=torch.float32, device="cuda")
+        sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, velocity=vel)
+        torch.cuda.synchronize()
+        sig, m, z = sig.cpu().numpy(), Mxy.cpu().numpy(), Mz.cpu().numpy()
+    plan.close()
+    ref, rxy, rz = oracle_mod.simulate(ph, s, velocity=v, dt_max=dt_max, output_mode=output_mode, return_state=True)
+    got_state = np.concatenate([m[:, 0] + 1j * m[:, 1], z.astype(np.complex128)])
+    ref_state = np.concatenate([rxy, rz.astype(np.complex128)])
+    for name, g, r in (("signal", sig, ref), ("state", got_state, ref_state)):
+        emax, nrmse = errors(g, r)
+        print(f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}")
+        assert emax <= TOL_MAX and nrmse <= TOL_NRMSE, f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}"
+    return sig, ref
+
+
+def moving_phantom(n, seed):
+    rng = np.random.default_rng(seed)
+    ph = W._phantom(rng.uniform(-.1, .1, n), rng.uniform(-.1, .1, n), rng.uniform(-.005, .005, n),
+                    rng.uniform(.5, 1, n), rng.uniform(.3, 2, n), rng.uniform(.03, .3, n), rng.uniform(-100, 100, n))
+    v = (rng.uniform(-.2, .2, n), rng.uniform(-.2, .2, n), rng.uniform(-.05, .05, n))
+    return ph, v
+
+
+@pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
+def test_epi_with_in_plane_motion_like_experiment_d(B, oracle_mod, phase_mode):
+    """Config-1-like EPI (hard 90 + 32x32 readout) with every spin moving: the paper's experiment (d) has
+    u_y = v_y t with v_y = 0.1 m/s (:236)."""
+    w = W.small("1")
+    n = w.phantom.n
+    v = (np.zeros(n), np.full(n, 0.1), np.zeros(n))
+    sig, ref = run_both(B, oracle_mod, w.phantom, w.seq, v, 2e-5, f"EPI v_y=0.1 {phase_mode}", phase_mode=phase_mode)
+    static = oracle_mod.simulate(w.phantom, w.seq)
+    assert errors(ref, static)[0] > 1e-2, "the motion must change the signal for the test to mean anything"
+
+
+def test_slice_selective_rf_on_moving_spins_and_ramps(B, oracle_mod):
+    """Through-plane motion during a slice-selective sinc (RF tiles with motion records), a bipolar pair on a
+    second axis, readout on a third; random velocities; 1 us RF steps, dt_max = 10 us elsewhere."""
+    n_rf = 400
+    dt = 1e-6
+    tm = (np.arange(n_rf) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - n_rf * dt / 2) / (n_rf * dt))
+    b1 = env * np.deg2rad(60) / (W.GAMMA * dt * env.sum())
+    rf = (2e-4 + np.arange(n_rf) * dt, np.full(n_rf, dt), b1, np.zeros(n_rf))
+    g = {2: ([1e-4, 2e-4, 6e-4, 7e-4, 9e-4, 1e-3], [0, 15e-3, 15e-3, 0, -12e-3, 0]),
+         1: ([1.0e-3, 1.1e-3, 1.5e-3, 1.6e-3, 1.7e-3, 2.1e-3, 2.2e-3], [0, 20e-3, 20e-3, 0, -20e-3, -20e-3, 0]),
+         0: ([2.2e-3, 2.3e-3, 3.6e-3, 3.7e-3], [0, 6e-3, 6e-3, 0])}
+    adc = 2.3e-3 + (np.arange(321) + 0.5) * 4e-6
+    s = seq(g=g, rf=rf, adc=adc, t_end=4e-3, dt_rf_max=dt)
+    ph, v = moving_phantom(1500, 21)
+    run_both(B, oracle_mod, ph, s, v, 1e-5, "slice-select + bipolar, moving")
+    run_both(B, oracle_mod, ph, s, v, 1e-5, "same through the host entry", host=True)
+
+
+def test_per_spin_output_with_motion(B, oracle_mod):
+    g = {0: ([0.0, 1e-4, 2e-3], [0, 8e-3, 8e-3])}
+    rf = (np.array([0.0]), np.array([5e-5]), np.array([(np.pi / 2) / (W.GAMMA * 5e-5)]), np.array([0.0]))
+    adc = 2e-4 + np.arange(40) * 2e-5
+    s = seq(g=g, rf=rf, adc=adc, t_end=2e-3, dt_rf_max=1.0)
+    ph, v = moving_phantom(37, 22)
+    run_both(B, oracle_mod, ph, s, v, 5e-5, "per-spin with motion", output_mode="per_spin")
+
+
+def test_zero_velocity_equals_the_static_plan_and_velocities_need_a_motion_plan(B, oracle_mod):
+    import torch
+    w = W.small("4")
+    n = w.phantom.n
+    zero = (np.zeros(n), np.zeros(n), np.zeros(n))
+    sig, _ = run_both(B, oracle_mod, w.phantom, w.seq, zero, 0.0, "zero velocity")
+    plan = B.Plan(w.seq)
+    dev = B.phantom_to_device(w.phantom)
+    stat = plan.simulate(*dev)
+    torch.cuda.synchronize()
+    assert errors(sig, stat.cpu().numpy())[0] < 5e-6
+    vel = tuple(torch.zeros(n, dtype=torch.float32, device="cuda") for _ in range(3))
+    with pytest.raises(B.BlochError) as e:
+        plan.simulate(*dev, velocity=vel)
+    assert e.value.code == -1
+    plan.close()

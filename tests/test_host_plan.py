@@ -121,3 +121,23 @@ def test_rf_increment_form_equals_eq9():
         u = np.cross(w, M)
         got = M + a * u + b * np.cross(w, u)
         np.testing.assert_allclose(got, [mxy2.real, mxy2.imag, mz2], rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("name,dt_max", [("1", 2e-5), ("2", 1e-4), ("4", 5e-6)])
+def test_motion_plan_refines_like_the_oracle(B, oracle_mod, name, dt_max):
+    """With motion every interval is limited to dt_max; the planner's grid must be the oracle's."""
+    w = W.small(name)
+    h0 = B.bloch_plan_create(w.seq)
+    h1 = B.bloch_plan_create(w.seq, motion="linear", dt_max=dt_max)
+    try:
+        i0, i1 = B.bloch_plan_get_info(h0), B.bloch_plan_get_info(h1)
+        t, _, rf, _ = oracle_mod.grid(w.seq, dt_max=dt_max)
+        assert i1["n_intervals"] == len(t) - 1 and i1["n_rf_steps"] == int(rf.sum())
+        assert i1["n_intervals"] > i0["n_intervals"] and i1["motion_mode"] == 1 and i0["motion_mode"] == 0
+        assert i1["table_bytes"] > i0["table_bytes"]      # first-moment records
+        assert i1["n_adc"] == i0["n_adc"] and i1["n_blocks"] == i0["n_blocks"]
+    finally:
+        B.bloch_plan_destroy(h0)
+        B.bloch_plan_destroy(h1)
+    with pytest.raises(B.BlochError):
+        B.bloch_plan_create(w.seq, motion=7)
