@@ -103,7 +103,8 @@ def make_workload(name: str, rank: int):
         base = W.SEED0
         try:
             W.SEED0 = base + 1000 * rank
-            w = W.Workload(w.name, W.make(name).phantom, w.seq, w.phase_mode, w.output_mode)
+            import dataclasses
+            w = dataclasses.replace(w, phantom=W.make(name).phantom)
         finally:
             W.SEED0 = base
     return w
@@ -114,16 +115,17 @@ def oracle_sample(w, budget_spin_steps: float, n_intervals: int):
     n = w.phantom.n
     take = int(max(1, min(n, budget_spin_steps // max(1, n_intervals))))
     idx = np.linspace(0, n - 1, take).astype(np.int64)
-    return w.phantom.subset(idx), take
+    vel = None if w.velocity is None else tuple(np.ascontiguousarray(a[idx]) for a in w.velocity)
+    return w.phantom.subset(idx), take, vel
 
 
 def time_oracle(w, n_intervals: int, budget_spin_steps: float):
     import oracle
     oracle.build()
     cores = os.cpu_count() or 1
-    ph, take = oracle_sample(w, budget_spin_steps, n_intervals)
+    ph, take, vel = oracle_sample(w, budget_spin_steps, n_intervals)
     t0 = time.perf_counter()
-    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores)
+    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max)
     dt = time.perf_counter() - t0
     return {"value": take * n_intervals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{take} of {w.phantom.n} spins (evenly spaced), full sequence ({n_intervals} intervals), "
@@ -136,7 +138,7 @@ def run_reference(args, rank, world):
         return
     import oracle
     w = make_workload(args.workload, 0)
-    t, _, _, _ = oracle.grid(w.seq)
+    t, _, _, _ = oracle.grid(w.seq, dt_max=w.dt_max if w.velocity is not None else 0.0)
     n_int = len(t) - 1
     cores = os.cpu_count() or 1
     # size a step at ~3 s of CPU work from a short probe
@@ -180,7 +182,7 @@ def run_ours(args, rank, local_rank, world):
     w = make_workload(args.workload, rank)
     per_spin = w.output_mode == "per_spin"
     t_plan0 = time.perf_counter()
-    plan = bloch.Plan(w.seq, phase_mode=w.phase_mode, output_mode=w.output_mode)
+    plan = bloch.Plan(w.seq, **w.plan_kw)
     plan.upload()
     torch.cuda.synchronize()
     plan_s = time.perf_counter() - t_plan0
@@ -189,6 +191,8 @@ def run_ours(args, rank, local_rank, world):
     n_int = info["n_intervals"]
     spin_steps = float(n) * float(n_int)
     dev = bloch.phantom_to_device(w.phantom)
+    vel = None if w.velocity is None else tuple(
+        torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
     Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda")
     Mz = torch.zeros(n, dtype=torch.float32, device="cuda")
     shape = (n, info["n_adc"]) if per_spin else (info["n_adc"],)
@@ -201,7 +205,7 @@ def run_ours(args, rank, local_rank, world):
         torch.cuda.synchronize()
 
     def step():
-        plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig)
+        plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig, velocity=vel)
         if not per_spin:
             reduce_signal(sig)
 
@@ -253,11 +257,15 @@ def run_ours(args, rank, local_rank, world):
     h_arrs = [p.numpy() for p in pinned]
     h_sig_np = h_sig.numpy()
     e2e_steps = max(1, min(args.steps, 5))
-    plan.simulate_host(*h_arrs, signal=h_sig_np)           # warm-up (allocates the scratch)
+    h_vel = None
+    if w.velocity is not None:
+        pinned_v = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory() for a in w.velocity]
+        h_vel = [p.numpy() for p in pinned_v]
+    plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel)   # warm-up (allocates the scratch)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        plan.simulate_host(*h_arrs, signal=h_sig_np)       # synchronous: returns after the D2H copy
+        plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel)   # synchronous: returns after the D2H copy
         if not per_spin and world > 1:
             reduce_signal(torch.from_numpy(h_sig_np).cuda())
     barrier()
@@ -265,7 +273,7 @@ def run_ours(args, rank, local_rank, world):
     if world > 1:
         dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
     e2e_value = spin_steps * world * e2e_steps / float(e2e_s.item())
-    h2d = sum(int(a.nbytes) for a in h_arrs)
+    h2d = sum(int(a.nbytes) for a in h_arrs) + (sum(int(a.nbytes) for a in h_vel) if h_vel else 0)
     d2h = int(h_sig_np.nbytes)
 
     if rank != 0:
@@ -312,7 +320,7 @@ def run_ours(args, rank, local_rank, world):
            "data": "synthetic",
            "config": {"workload": w.name, "n_spins_per_gpu": n, "n_intervals": n_int,
                       "n_rf_steps": info["n_rf_steps"], "n_adc": info["n_adc"], "n_blocks": info["n_blocks"],
-                      "output_mode": w.output_mode, "spin_steps_per_step": spin_steps * world,
+                      "output_mode": w.output_mode, "motion": w.velocity is not None, "spin_steps_per_step": spin_steps * world,
                       "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
                       "plan_create_upload_s": plan_s},
            "sim_wall_time_s": ms_total / args.steps * 1e-3,
@@ -339,7 +347,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 4 (default, 1M-spin spiral), 5, 5b")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 5, 5b")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")

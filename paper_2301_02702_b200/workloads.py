@@ -69,6 +69,15 @@ class Workload:
     seq: Sequence
     phase_mode: str = "auto"      # "auto" | "fp32" | "fp64"
     output_mode: str = "sum"      # "sum" | "per_spin"
+    velocity: tuple | None = None  # (vx, vy, vz) fp32-exact arrays [m/s]: x(t) = x + v t
+    dt_max: float = 0.0            # spacing of the intermediate points needed with motion
+
+    @property
+    def plan_kw(self) -> dict:
+        kw = dict(phase_mode=self.phase_mode, output_mode=self.output_mode)
+        if self.velocity is not None:
+            kw.update(motion="linear", dt_max=self.dt_max)
+        return kw
 
 
 def _f32(a):
@@ -431,7 +440,18 @@ def config5b(n_entries: int = 100_000, n_tr: int = 1000, n_samp: int = 1024, n_r
     return Workload("config5b_mrf_dictionary", ph, seq, output_mode="per_spin")
 
 
-CONFIGS = {"1": config1, "2": config2, "3": config3, "4": config4, "5": config5, "5b": config5b}
+def config3m(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, vy: float = 0.1, dt_max: float = 1e-5) -> Workload:
+    """Config 3 without off-resonance but with motion, the paper's experiment (d):
+    u_y(x, t) = v_y t with v_y = 0.1 m/s for every spin; intermediate points every dt_max."""
+    w = config3(n_grid, n_epi, n_rf)
+    ph = w.phantom
+    n = ph.n
+    ph = Phantom(ph.x, ph.y, ph.z, ph.M0, ph.T1, ph.T2, np.zeros(n))
+    vel = (np.zeros(n), _f32(np.full(n, vy)), np.zeros(n))
+    return Workload("config3m_brain_epi128_motion", ph, w.seq, phase_mode="fp64", velocity=vel, dt_max=dt_max)
+
+
+CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b}
 
 
 def make(name: str, **kw) -> Workload:
@@ -449,6 +469,8 @@ def small(name: str) -> Workload:
         return config2(n_grid=24, n_pe=6, n_ro=64, n_rf=200)
     if name == "3":
         return config3(n_grid=48, n_epi=32, n_rf=250)
+    if name == "3m":
+        return config3m(n_grid=24, n_epi=16, n_rf=100)
     if name == "4":
         return config4(n_spins=5003, n_shots=3, n_samp=700, n_rf=300, turns=8.0 * 700 / 4096)
     if name == "5":

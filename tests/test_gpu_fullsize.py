@@ -123,3 +123,21 @@ def test_dictionary_full_size_sampled_rows(B, oracle_mod):
     for k in range(len(idx)):
         emax, _ = errors(rows[k], ref[k])
         assert emax <= TOL_MAX, f"entry {idx[k]}: max {emax:.3e}"
+
+
+def test_full_config3_with_motion_experiment_d(B, oracle_mod):
+    """Config 3m: the brain-like EPI with u_y = v_y t, v_y = 0.1 m/s, whole oracle."""
+    import torch
+    w = W.make("3m")
+    plan = B.Plan(w.seq, **w.plan_kw)
+    dev = B.phantom_to_device(w.phantom)
+    vel = tuple(torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
+    Mxy = torch.zeros(w.phantom.n, 2, dtype=torch.float32, device="cuda")
+    Mz = torch.zeros(w.phantom.n, dtype=torch.float32, device="cuda")
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, velocity=vel)
+    torch.cuda.synchronize()
+    plan.close()
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, velocity=w.velocity, dt_max=w.dt_max, return_state=True)
+    m = Mxy.cpu().numpy()
+    assert_parity(sig.cpu().numpy(), ref, "config 3m full-size signal")
+    assert_parity(state_vec(m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy()), state_vec(rxy, rz), "config 3m full-size final state")
