@@ -69,7 +69,7 @@ def _seq_args(seq, keep):
 
 def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state: bool = False,
              n_threads: int | None = None, gamma: float = GAMMA, force_excitation: bool = False,
-             velocity=None, dt_max: float = 0.0):
+             velocity=None, dt_max: float = 0.0, group_size: int = 0):
     """Step-by-step fp64 Bloch integration (SURVEY.md 8(c) listing).
 
     phantom: object with fp64 arrays x, y, z, M0, T1, T2, dw.   seq: object with g_t, g_v (3 arrays each),
@@ -79,6 +79,19 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     Returns complex128 signal [n_adc] ("sum") or [n_spins, n_adc] ("per_spin"); with return_state also
     (Mxy complex128 [n_spins], Mz float64 [n_spins]).
     """
+    if output_mode == "grouped":
+        # SURVEY.md 8(f) f2: S[g][j] = sum of Mxy over the spins of group g (consecutive blocks of group_size
+        # spins: an isochromat ensemble per voxel / dictionary entry, PAPER.md:167, :220) -- by definition the
+        # per-spin signals added up group by group.
+        n_all = int(np.asarray(phantom.x).shape[0])
+        if group_size <= 0 or n_all % group_size:
+            raise ValueError("group_size must be positive and divide the number of spins")
+        res = simulate(phantom, seq, output_mode="per_spin", state=state, return_state=return_state,
+                       n_threads=n_threads, gamma=gamma, force_excitation=force_excitation, velocity=velocity,
+                       dt_max=dt_max)
+        per = res[0] if return_state else res
+        grouped = per.reshape(n_all // group_size, group_size, per.shape[1]).sum(axis=1)
+        return (grouped,) + tuple(res[1:]) if return_state else grouped
     lib = _load()
     keep = []
     sargs, n_adc = _seq_args(seq, keep)

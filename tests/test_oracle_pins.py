@@ -385,3 +385,34 @@ def test_grid_contents_and_rf_refinement(oracle_mod):
     assert rf.tolist() == [1] * 5 + [0] * 6
     np.testing.assert_allclose(G[:, 0], np.interp(want_t, [1e-3, 2e-3, 3e-3], [0, 1e-3, 0]), atol=1e-18)
     assert adc.tolist() == [-1] * 7 + [0, -1, 1, -1, -1]
+
+
+# ---------------------------------------------------------------------------------------------- f2
+def test_grouped_output_is_a_fisp_ensemble_dictionary(oracle_mod):
+    """three (T1, T2) entries, each an ensemble of 128 isochromats whose spoiler phase covers
+    2 pi per TR; the grouped signal of entry g, divided by the group size, must be ITS closed-form FISP FID
+    steady state (P7 formula) -- which pins the group indexing and ordering, not only the sum.  Degenerate
+    group sizes reduce to the other two modes."""
+    alpha, TR, n_iso, n_tr = math.radians(30.0), 6e-3, 128, 300
+    T1s, T2s = np.array([0.1, 0.25, 0.08]), np.array([0.04, 0.02, 0.06])
+    tp = 1e-9
+    rf_t = np.arange(n_tr) * TR
+    s = seq(rf=(rf_t, np.full(n_tr, tp), np.full(n_tr, alpha / (GAMMA * tp)), np.zeros(n_tr)),
+            adc=[rf_t[-1] + tp], t_end=rf_t[-1] + TR, dt_rf_max=tp)
+    dws = np.tile(2 * math.pi * np.arange(n_iso) / (n_iso * TR), 3)
+    ph = phantom(M0=1.0, T1=np.repeat(T1s, n_iso), T2=np.repeat(T2s, n_iso), dw=dws)
+    grouped = oracle_mod.simulate(ph, s, output_mode="grouped", group_size=n_iso)
+    assert grouped.shape == (3, 1)
+    ca = math.cos(alpha)
+    for g in range(3):
+        E1, E2 = math.exp(-TR / T1s[g]), math.exp(-TR / T2s[g])
+        r = math.sqrt((1 - E2 ** 2) / ((1 - E1 * ca) ** 2 - E2 ** 2 * (E1 - ca) ** 2))
+        fid = math.tan(alpha / 2) * (1 - (E1 - ca) * r)
+        assert abs(abs(grouped[g, 0]) / n_iso - fid) < 1e-6, g
+    per = oracle_mod.simulate(ph, s, output_mode="per_spin")
+    np.testing.assert_allclose(oracle_mod.simulate(ph, s, output_mode="grouped", group_size=1), per, rtol=0, atol=0)
+    total = oracle_mod.simulate(ph, s)
+    np.testing.assert_allclose(oracle_mod.simulate(ph, s, output_mode="grouped", group_size=3 * n_iso)[0], total,
+                               rtol=0, atol=1e-10)
+    with pytest.raises(ValueError):
+        oracle_mod.simulate(ph, s, output_mode="grouped", group_size=5)
