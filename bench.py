@@ -114,7 +114,13 @@ def oracle_sample(w, budget_spin_steps: float, n_intervals: int):
     """A bounded sample of the workload for the CPU oracle: every m-th spin, the full sequence."""
     n = w.phantom.n
     take = int(max(1, min(n, budget_spin_steps // max(1, n_intervals))))
-    idx = np.linspace(0, n - 1, take).astype(np.int64)
+    if w.group_size > 1:   # whole groups
+        g = max(1, take // w.group_size)
+        first = np.linspace(0, n // w.group_size - 1, g).astype(np.int64) * w.group_size
+        idx = (first[:, None] + np.arange(w.group_size)[None, :]).ravel()
+        take = int(idx.size)
+    else:
+        idx = np.linspace(0, n - 1, take).astype(np.int64)
     vel = None if w.velocity is None else tuple(np.ascontiguousarray(a[idx]) for a in w.velocity)
     return w.phantom.subset(idx), take, vel
 
@@ -125,7 +131,8 @@ def time_oracle(w, n_intervals: int, budget_spin_steps: float):
     cores = os.cpu_count() or 1
     ph, take, vel = oracle_sample(w, budget_spin_steps, n_intervals)
     t0 = time.perf_counter()
-    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max)
+    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max,
+                    group_size=w.group_size)
     dt = time.perf_counter() - t0
     return {"value": take * n_intervals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{take} of {w.phantom.n} spins (evenly spaced), full sequence ({n_intervals} intervals), "
@@ -180,7 +187,7 @@ def run_ours(args, rank, local_rank, world):
     from paper_2301_02702_b200.dist import reduce_signal
 
     w = make_workload(args.workload, rank)
-    per_spin = w.output_mode == "per_spin"
+    per_spin = w.output_mode in ("per_spin", "grouped")   # no cross-rank sum: outputs stay sharded
     t_plan0 = time.perf_counter()
     plan = bloch.Plan(w.seq, **w.plan_kw)
     plan.upload()
@@ -195,7 +202,7 @@ def run_ours(args, rank, local_rank, world):
         torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
     Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda")
     Mz = torch.zeros(n, dtype=torch.float32, device="cuda")
-    shape = (n, info["n_adc"]) if per_spin else (info["n_adc"],)
+    shape = plan._signal_shape(n)
     sig = torch.empty(shape, dtype=torch.complex64, device="cuda")
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -347,7 +354,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 5, 5b")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 5, 5b, 5c (ensemble dictionary)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")

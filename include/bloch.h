@@ -40,7 +40,7 @@ typedef enum {
 } bloch_status;
 
 enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
-enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1 };
+enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1, BLOCH_OUT_GROUPED = 2 };
 enum { BLOCH_MOTION_NONE = 0, BLOCH_MOTION_LINEAR = 1 };
 
 /* Scanner.  Only gamma enters the arithmetic (Eq 1-2, :105-114); B0, G_max, S_max are
@@ -83,7 +83,7 @@ typedef struct {
     int32_t phase_mode;   /* BLOCH_PHASE_* */
     int32_t output_mode;  /* BLOCH_OUT_*   */
     int32_t motion_mode;  /* BLOCH_MOTION_* */
-    int32_t reserved;     /* 0 */
+    int32_t group_size;   /* BLOCH_OUT_GROUPED: spins per group (>= 1; n_spins must be a multiple); else ignored */
 } bloch_sim_params;
 
 typedef struct {
@@ -99,7 +99,7 @@ typedef struct {
     int32_t phase_mode;      /* resolved: BLOCH_PHASE_FP32 or BLOCH_PHASE_FP64 */
     int32_t output_mode;
     int32_t motion_mode;
-    int32_t reserved;
+    int32_t group_size;
 } bloch_plan_info;
 
 typedef struct bloch_plan bloch_plan;
@@ -129,7 +129,10 @@ int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stre
  *       (both required); if non-NULL they receive the final magnetisation.  With init_equilibrium != 0
  *       the state starts at Mxy = 0, Mz = M0 (reading G8).
  *   d_signal: SUM_ALL: n_adc complex, S[j] = sum over spins of Mxy at ADC sample j;
- *             PER_SPIN: n_spins x n_adc complex, row-major [spin][adc].
+ *             PER_SPIN: n_spins x n_adc complex, row-major [spin][adc];
+ *             GROUPED: (n_spins / group_size) x n_adc complex, row-major [group][adc],
+ *             S[g][j] = sum of Mxy over the group_size consecutive spins of group g -- an isochromat ensemble
+ *             per voxel or per dictionary entry.
  *   Asynchronous on `stream`: no hidden synchronisation, no allocation, no host copies.  The result is
  *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 (not checked). */
 int bloch_simulate(const bloch_plan *plan, int64_t n_spins,

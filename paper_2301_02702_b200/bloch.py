@@ -15,9 +15,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libbloch_b200.so")
 
 PHASE_AUTO, PHASE_FP32, PHASE_FP64 = 0, 1, 2
-OUT_SUM_ALL, OUT_PER_SPIN = 0, 1
+OUT_SUM_ALL, OUT_PER_SPIN, OUT_GROUPED = 0, 1, 2
 _PHASE = {"auto": PHASE_AUTO, "fp32": PHASE_FP32, "fp64": PHASE_FP64}
-_OUT = {"sum": OUT_SUM_ALL, "per_spin": OUT_PER_SPIN}
+_OUT = {"sum": OUT_SUM_ALL, "per_spin": OUT_PER_SPIN, "grouped": OUT_GROUPED}
 MOTION_NONE, MOTION_LINEAR = 0, 1
 _MOTION = {"none": MOTION_NONE, "linear": MOTION_LINEAR}
 
@@ -38,7 +38,7 @@ class bloch_sequence(C.Structure):
 class bloch_sim_params(C.Structure):
     _fields_ = [("dt_max", C.c_double), ("dt_rf_max", C.c_double), ("max_block_points", C.c_int64),
                 ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("group_size", C.c_int32)]
 
 
 class bloch_plan_info(C.Structure):
@@ -46,7 +46,7 @@ class bloch_plan_info(C.Structure):
                 ("n_blocks", C.c_int64), ("n_rf_blocks", C.c_int64), ("n_eval_points", C.c_int64),
                 ("n_launches", C.c_int64), ("table_bytes", C.c_int64), ("max_block_adc", C.c_int64),
                 ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("group_size", C.c_int32)]
 
 
 EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",
@@ -123,7 +123,8 @@ def _darr(a):
 
 
 def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
-                      max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none") -> int:
+                      max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
+                      group_size: int = 0) -> int:
     """seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
     Returns the opaque plan handle (an integer address)."""
     keep = []
@@ -147,7 +148,7 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     pm = _PHASE[phase_mode] if isinstance(phase_mode, str) else int(phase_mode)
     om = _OUT[output_mode] if isinstance(output_mode, str) else int(output_mode)
     mm = _MOTION[motion] if isinstance(motion, str) else int(motion)
-    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, 0)
+    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, int(group_size))
     h = C.c_void_p()
     _check(_lib.bloch_plan_create(C.byref(sc), C.byref(cs), C.byref(sp), C.byref(h)))
     return h.value
@@ -256,6 +257,14 @@ class Plan:
         except Exception:
             pass
 
+    def _signal_shape(self, n):
+        n_adc, mode = self.info["n_adc"], self.info["output_mode"]
+        if mode == OUT_PER_SPIN:
+            return (n, n_adc)
+        if mode == OUT_GROUPED:
+            return (n // max(1, self.info["group_size"]), n_adc)
+        return (n_adc,)
+
     @staticmethod
     def _stream():
         import torch
@@ -285,7 +294,7 @@ class Plan:
         for t in (x, y, z, M0, T1, T2, dw):
             assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
         n_adc = self.info["n_adc"]
-        shape = (n, n_adc) if self.info["output_mode"] == OUT_PER_SPIN else (n_adc,)
+        shape = self._signal_shape(n)
         if signal is None:
             signal = torch.empty(shape, dtype=torch.complex64, device="cuda")
         ws = self._workspace(n)
@@ -310,7 +319,7 @@ class Plan:
         arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (x, y, z, M0, T1, T2, dw)]
         n = int(arrs[0].shape[0])
         n_adc = self.info["n_adc"]
-        shape = (n, n_adc) if self.info["output_mode"] == OUT_PER_SPIN else (n_adc,)
+        shape = self._signal_shape(n)
         if signal is None:
             signal = np.empty(shape, dtype=np.complex64)
         need = max(bloch_simulate_host_scratch_bytes(self.handle, n), 256)

@@ -84,6 +84,13 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
     return std::max(worst, std::min(total, kPartialCapBytes / sizeof(float2)));
 }
 
+// rows of the signal buffer: 1 (SUM_ALL), n_spins (PER_SPIN), n_spins / group_size (GROUPED)
+size_t signal_rows(const bloch_plan *plan, int64_t n_spins) {
+    if (plan->info.output_mode == BLOCH_OUT_PER_SPIN) return size_t(n_spins);
+    if (plan->info.output_mode == BLOCH_OUT_GROUPED) return size_t(n_spins) / size_t(std::max(1, plan->info.group_size));
+    return 1;
+}
+
 struct Workspace {
     float4 *A, *C, *S;
     double4 *Ad;     // fp64-phase plans only
@@ -299,7 +306,10 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
     if (rc != BLOCH_OK) return rc;
     const int sms = sm_count_cached();
     cudaStream_t stream = (cudaStream_t)stream_;
-    const bool per_spin = plan->info.output_mode == BLOCH_OUT_PER_SPIN;
+    const bool grouped = plan->info.output_mode == BLOCH_OUT_GROUPED;
+    const bool per_spin = plan->info.output_mode == BLOCH_OUT_PER_SPIN || grouped;  // no cross-CTA reduction
+    if (grouped && n_spins % plan->info.group_size != 0)
+        return fail(BLOCH_EINVAL, "n_spins is not a multiple of the plan's group_size");
     const bool ph64 = plan->info.phase_mode == BLOCH_PHASE_FP64;
 
     if (n_spins == 0) {  // degenerate: the sum over no spins is zero
@@ -351,7 +361,19 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
             if ((rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
             const void *recs = plan->d_tables + b.table_off;
             const int n_pts = (int)b.adc_count;
-            if (per_spin) {
+            if (grouped) {
+                const int gs = plan->info.group_size, n_groups = n / gs;
+                const unsigned grid = (unsigned)(((long long)n_groups * 32 + 255) / 256);
+                if (ph64)
+                    grouped_kernel<true><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n_groups, gs,
+                                                                   (long long)plan->info.n_adc, (long long)b.adc_first,
+                                                                   (float2 *)d_signal);
+                else
+                    grouped_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n_groups, gs,
+                                                                    (long long)plan->info.n_adc, (long long)b.adc_first,
+                                                                    (float2 *)d_signal);
+                ++launches;
+            } else if (per_spin) {
                 const long long total = (long long)n * n_pts;
                 const unsigned grid = (unsigned)((total + 255) / 256);
                 if (ph64)
@@ -441,9 +463,7 @@ int bloch_simulate_host_scratch_bytes(const bloch_plan *plan, int64_t n_spins, s
     int rc = bloch_plan_workspace_bytes(plan, n_spins, &ws);
     if (rc) return rc;
     const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
-    const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
-                           ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
-                           : size_t(plan->info.n_adc) * sizeof(float2);
+    const size_t sig = signal_rows(plan, n_spins) * size_t(plan->info.n_adc) * sizeof(float2);
     *out = 13 * arr + align_up(sig, kAlign) + ws + kAlign;
     return BLOCH_OK;
 }
@@ -490,9 +510,7 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins, const fl
         BLOCH_CUDA(cudaMemcpyAsync(d_Mxy, h_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyHostToDevice, stream));
         BLOCH_CUDA(cudaMemcpyAsync(d_Mz, h_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
     }
-    const size_t sig = plan->info.output_mode == BLOCH_OUT_PER_SPIN
-                           ? size_t(n_spins) * size_t(plan->info.n_adc) * sizeof(float2)
-                           : size_t(plan->info.n_adc) * sizeof(float2);
+    const size_t sig = signal_rows(plan, n_spins) * size_t(plan->info.n_adc) * sizeof(float2);
     float *d_v[3] = {nullptr, nullptr, nullptr};
     if (has_v) {
         const float *hv[3] = {h_vx, h_vy, h_vz};

@@ -144,6 +144,64 @@ perspin_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restri
     out[(size_t)sp * n_adc_total + adc_first + p] = make_float2(er * cs - ei * sn, er * sn + ei * cs);
 }
 
+// GROUPED output: one warp per group of `gs` consecutive spins (an isochromat ensemble);
+// the lanes take the group's spins, evaluate the block's points one after the other with the accurate
+// functions of perspin_kernel, and add up with a fixed butterfly (bitwise reproducible); lane 0 writes
+// out[group][adc].
+template <bool PH64>
+__global__ void __launch_bounds__(256)
+grouped_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restrict__ A,
+               const float4 *__restrict__ Cc, const float4 *__restrict__ S, const float4 *__restrict__ V,
+               int n_groups, int gs, long long n_adc_total, long long adc_first, float2 *__restrict__ out) {
+    const int warp = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (warp >= n_groups) return;
+    const int rs = V ? 2 : 1;
+    const long long s0 = (long long)warp * gs;
+    for (int p = 0; p < n_pts; ++p) {
+        double kx, ky, kz, tau, ux = 0., uy = 0., uz = 0.;
+        if (PH64) {
+            const double4 r = reinterpret_cast<const double4 *>(recs_)[rs * p];
+            kx = r.x; ky = r.y; kz = r.z; tau = r.w;
+            if (V) {
+                const double4 m = reinterpret_cast<const double4 *>(recs_)[rs * p + 1];
+                ux = m.x; uy = m.y; uz = m.z;
+            }
+        } else {
+            const float4 r = reinterpret_cast<const float4 *>(recs_)[rs * p];
+            kx = (double)r.x * 0.15915494309189535; ky = (double)r.y * 0.15915494309189535;
+            kz = (double)r.z * 0.15915494309189535; tau = r.w;
+            if (V) {
+                const float4 m = reinterpret_cast<const float4 *>(recs_)[rs * p + 1];
+                ux = (double)m.x * 0.15915494309189535; uy = (double)m.y * 0.15915494309189535;
+                uz = (double)m.z * 0.15915494309189535;
+            }
+        }
+        float re = 0.f, im = 0.f;
+        for (int k = lane; k < gs; k += 32) {
+            const float4 a = A[s0 + k], c = Cc[s0 + k], s = S[s0 + k];
+            double th = kx * (double)a.x + ky * (double)a.y + kz * (double)a.z -
+                        (double)c.w * 0.15915494309189535 * tau;
+            if (V) {
+                const float4 v = V[s0 + k];
+                th += ux * (double)v.x + uy * (double)v.y + uz * (double)v.z;
+            }
+            th -= rint(th);
+            float sn, cs;
+            sincospif(2.0f * (float)th, &sn, &cs);
+            const float e = expf(-(float)tau * c.y);
+            const float er = s.x * e, ei = s.y * e;
+            re += er * cs - ei * sn;
+            im += er * sn + ei * cs;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            re += __shfl_xor_sync(0xffffffffu, re, o);
+            im += __shfl_xor_sync(0xffffffffu, im, o);
+        }
+        if (lane == 0) out[(size_t)warp * n_adc_total + adc_first + p] = make_float2(re, im);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // pipe micro-benchmarks (roofline denominators)
 // ------------------------------------------------------------------------------------------------

@@ -68,8 +68,11 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     if (!(seq->t_end > 0.0) || !std::isfinite(seq->t_end)) return fail(BLOCH_EINVAL, "t_end must be > 0");
     if (params->phase_mode < BLOCH_PHASE_AUTO || params->phase_mode > BLOCH_PHASE_FP64)
         return fail(BLOCH_EINVAL, "bad phase_mode");
-    if (params->output_mode != BLOCH_OUT_SUM_ALL && params->output_mode != BLOCH_OUT_PER_SPIN)
+    if (params->output_mode != BLOCH_OUT_SUM_ALL && params->output_mode != BLOCH_OUT_PER_SPIN &&
+        params->output_mode != BLOCH_OUT_GROUPED)
         return fail(BLOCH_EINVAL, "bad output_mode");
+    if (params->output_mode == BLOCH_OUT_GROUPED && params->group_size < 1)
+        return fail(BLOCH_EINVAL, "group_size must be >= 1 with BLOCH_OUT_GROUPED");
     if (params->motion_mode != BLOCH_MOTION_NONE && params->motion_mode != BLOCH_MOTION_LINEAR)
         return fail(BLOCH_EINVAL, "bad motion_mode");
     const bool motion = params->motion_mode == BLOCH_MOTION_LINEAR;
@@ -400,7 +403,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     inf.phase_mode = phase;
     inf.output_mode = params->output_mode;
     inf.motion_mode = params->motion_mode;
-    inf.reserved = 0;
+    inf.group_size = params->output_mode == BLOCH_OUT_GROUPED ? params->group_size : 0;
     return BLOCH_OK;
 }
 

@@ -71,12 +71,15 @@ class Workload:
     output_mode: str = "sum"      # "sum" | "per_spin"
     velocity: tuple | None = None  # (vx, vy, vz) fp32-exact arrays [m/s]: x(t) = x + v t
     dt_max: float = 0.0            # spacing of the intermediate points needed with motion
+    group_size: int = 0            # output_mode "grouped": spins per group
 
     @property
     def plan_kw(self) -> dict:
         kw = dict(phase_mode=self.phase_mode, output_mode=self.output_mode)
         if self.velocity is not None:
             kw.update(motion="linear", dt_max=self.dt_max)
+        if self.output_mode == "grouped":
+            kw.update(group_size=self.group_size)
         return kw
 
 
@@ -440,6 +443,23 @@ def config5b(n_entries: int = 100_000, n_tr: int = 1000, n_samp: int = 1024, n_r
     return Workload("config5b_mrf_dictionary", ph, seq, output_mode="per_spin")
 
 
+def config5c(n_entries: int = 10_000, n_iso: int = 64, n_tr: int = 1000, n_samp: int = 1024, n_rf: int = 1000,
+             turns: float = 6.0) -> Workload:
+    """Ensemble dictionary: config 5b's schedule, but every (T1, T2) entry is n_iso
+    isochromats spread evenly over one period of the x spoiler (320 1/m -> 3.125 mm), so that an entry's
+    GROUPED signal is a proper FISP ensemble (PAPER.md:167 "use more spins", :368).  Output
+    [entry][TR] complex."""
+    w = config5b(n_entries, n_tr, n_samp, n_rf, turns)
+    period = 1.0 / 320.0
+    xk = ((np.arange(n_iso) + 0.5) / n_iso - 0.5) * period
+    T1 = np.repeat(w.phantom.T1, n_iso)
+    T2 = np.repeat(w.phantom.T2, n_iso)
+    n = n_entries * n_iso
+    z = np.zeros(n)
+    ph = _phantom(np.tile(xk, n_entries), z, z, np.full(n, 1.0 / n_iso), T1, T2, z)
+    return Workload("config5c_mrf_ensemble_dictionary", ph, w.seq, output_mode="grouped", group_size=n_iso)
+
+
 def config3m(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, vy: float = 0.1, dt_max: float = 1e-5) -> Workload:
     """Config 3 without off-resonance but with motion, the paper's experiment (d):
     u_y(x, t) = v_y t with v_y = 0.1 m/s for every spin; intermediate points every dt_max."""
@@ -451,7 +471,8 @@ def config3m(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, vy: float = 
     return Workload("config3m_brain_epi128_motion", ph, w.seq, phase_mode="fp64", velocity=vel, dt_max=dt_max)
 
 
-CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b}
+CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b,
+           "5c": config5c}
 
 
 def make(name: str, **kw) -> Workload:
@@ -477,4 +498,6 @@ def small(name: str) -> Workload:
         return config5(n_grid=40, n_tr=12, n_samp=300, n_rf=200, turns=6.0 * 300 / 1024)
     if name == "5b":
         return config5b(n_entries=777, n_tr=40, n_samp=512, n_rf=200, turns=3.0)
+    if name == "5c":
+        return config5c(n_entries=41, n_iso=24, n_tr=40, n_samp=512, n_rf=200, turns=3.0)
     raise KeyError(name)
