@@ -338,6 +338,11 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
     // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
     const int rf_threads = env_int("BLOCH_RF_THREADS", (n + 31) / 32 >= sms * 32 ? 128 : 32);
     const int rf_grid = (n + rf_threads - 1) / rf_threads;
+    auto launch_rf = [&](const unsigned char *tbl, int n_tiles, int has_prop) -> int {
+        if (mo) rf_kernel<true><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, w.V, n);
+        else rf_kernel<false><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, nullptr, n);
+        return BLOCH_OK;
+    };
     bool batch_open = false;
     SigShape batch_shape{};
     int64_t batch_adc_first = 0, batch_pts = 0, batch_done = 0;
@@ -345,15 +350,14 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
         const Block &b = plan->blocks[bi];
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
-            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(plan->d_tables + b.table_off, (int)b.n_tiles, prop,
-                                                           pending ? 1 : 0, w.A, w.C, w.S, w.V, n);
+            if ((rc = launch_rf(plan->d_tables + b.table_off, (int)b.n_tiles, pending ? 1 : 0))) return rc;
             ++launches;
             pending = false;
             continue;
         }
         if (pending) {  // two precession blocks in a row: apply the first one's end transform now
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, w.V, n);
+            if ((rc = launch_rf(nullptr, 0, 1))) return rc;
             ++launches;
             pending = false;
         }
@@ -443,7 +447,7 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
     if (d_Mxy) {
         if (pending) {
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
-            rf_kernel<<<rf_grid, rf_threads, 0, stream>>>(nullptr, 0, prop, 1, w.A, w.C, w.S, w.V, n);
+            if ((rc = launch_rf(nullptr, 0, 1))) return rc;
             ++launches;
         }
         if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;

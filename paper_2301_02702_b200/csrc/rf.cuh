@@ -157,11 +157,14 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
 
 constexpr int kRfMaxThreads = 128;
 
+// MO: motion plans (48-B step records, velocities); the static instantiation keeps its registers and shared
+// memory (48 registers, 8.3 KB) so that 10 CTAs of 128 threads fit an SM.
+template <bool MO>
 __global__ void __launch_bounds__(kRfMaxThreads)
 rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int has_prop,
           const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S,
           const float4 *__restrict__ V /* motion plans, else NULL */, int n) {
-    __shared__ __align__(128) unsigned char buf[2][kRfTileBytesMax];
+    __shared__ __align__(128) unsigned char buf[2][kRfHdrBytes + kRfTileSteps * (MO ? 48 : 32)];
     __shared__ __align__(8) uint64_t bar[2];
     const int tid = threadIdx.x;
     const int2 *dir = reinterpret_cast<const int2 *>(tbl);
@@ -184,7 +187,7 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         a = A[i];
         c = Cc[i];
         s = S[i];
-        if (V) v = V[i];
+        if (MO) v = V[i];
     }
     float hx = s.x, hy = s.y, hz = s.z;
     if (has_prop) propagate(prop, a, c, v, hx, hy, hz);
@@ -207,16 +210,16 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         rx.D1m0 = rx.D1 * sp.m0;
         // bound on q = |w|^2 over the tile for this spin -> tier, decided per warp
         float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
-        wzb = fmaf(hd.hx_max, avx, fmaf(hd.hy_max, avy, fmaf(hd.hz_max, avz, wzb)));
+        if (MO) wzb = fmaf(hd.hx_max, avx, fmaf(hd.hy_max, avy, fmaf(hd.hz_max, avz, wzb)));
         const float qb = fmaf(wzb, wzb, hd.wxy2_max);
-        const int mode = (hd.flags & kRfFlagMotion) ? 2 : ((hd.flags & kRfFlagUniformG) ? 0 : 1);
+        const int mode = MO ? 2 : ((hd.flags & kRfFlagUniformG) ? 0 : 1);  // motion plans hold motion tiles only
         const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
 #define BLOCH_RF_TILE(T, M) rf_tile<T, M>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz)
 #define BLOCH_RF_MODES(T)                       \
     do {                                        \
-        if (mode == 0) BLOCH_RF_TILE(T, 0);     \
-        else if (mode == 1) BLOCH_RF_TILE(T, 1);\
-        else BLOCH_RF_TILE(T, 2);               \
+        if (MO) BLOCH_RF_TILE(T, 2);            \
+        else if (mode == 0) BLOCH_RF_TILE(T, 0);\
+        else BLOCH_RF_TILE(T, 1);               \
     } while (0)
         if (tier == 0) BLOCH_RF_MODES(0);
         else if (tier == 1) BLOCH_RF_MODES(1);
