@@ -32,6 +32,7 @@ SM_COUNT = 148
 # FP32 128 lanes/SM/clk
 MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)
 FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
+FP32_PER_EVAL = 15         # FP32-pipe instructions per (spin, evaluated point)
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full captures
 NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v2_signal_kernel_cfg4_ncu.txt"),
                ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v2_rf_kernel_cfg4_ncu.txt")}
@@ -189,7 +190,7 @@ def run_ours(args, rank, local_rank, world):
     w = make_workload(args.workload, rank)
     per_spin = w.output_mode in ("per_spin", "grouped")   # no cross-rank sum: outputs stay sharded
     t_plan0 = time.perf_counter()
-    plan = bloch.Plan(w.seq, **w.plan_kw)
+    plan = bloch.Plan(w.seq, path=args.path, **w.plan_kw)
     plan.upload()
     torch.cuda.synchronize()
     plan_s = time.perf_counter() - t_plan0
@@ -317,6 +318,25 @@ def run_ours(args, rank, local_rank, world):
                       "launches_per_step": kinds_n["rf"] // args.steps, "ms_per_step": dur * 1e3,
                       "avg_launch_ms": kinds_ms["rf"] / kinds_n["rf"],
                       "algorithmic_ops_per_launch": FP32_PER_RF_STEP * rf_steps * args.steps / kinds_n["rf"]}
+    if kinds_n["fused"]:
+        # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
+        # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)
+        dur = kinds_ms["fused"] * 1e-3 / args.steps
+        fp32_ops = FP32_PER_RF_STEP * rf_steps + FP32_PER_EVAL * n_eval_sig
+        mufu_ops = MUFU_PER_EVAL * n_eval_sig
+        t_fp32, t_mufu = fp32_ops / fp32_peak, mufu_ops / mufu_peak
+        pipe, ops, peak = ("fp32", fp32_ops, fp32_peak) if t_fp32 >= t_mufu else ("mufu", mufu_ops, mufu_peak)
+        ach = ops / dur
+        kern["fused"] = {"bound": "alu", "pipe": pipe, "achieved": ach / 1e12, "peak": peak / 1e12,
+                         "unit": "Tfp32-instr/s" if pipe == "fp32" else "Tmufu-op/s", "frac": ach / peak,
+                         "traffic": NCU_TRAFFIC.get((w.name, "fused"), (None, None))[0],
+                         "traffic_source": NCU_TRAFFIC.get((w.name, "fused"), (None, None))[1],
+                         "note": "seq_kernel (a5-a8 in one launch): algorithmic count = 46 FP32 instructions per spin*step "
+                                 "+ 15 FP32 instructions per (spin, ADC sample), SURVEY.md 8(d); the MUFU count "
+                                 f"(3 per evaluation) would take {t_mufu * 1e3:.1f} ms, the FP32 count {t_fp32 * 1e3:.1f} ms",
+                         "launches_per_step": kinds_n["fused"] // args.steps, "ms_per_step": dur * 1e3,
+                         "avg_launch_ms": kinds_ms["fused"] / kinds_n["fused"],
+                         "algorithmic_ops_per_launch": ops * args.steps / kinds_n["fused"]}
     dominant = max(kern, key=lambda k: kern[k]["ms_per_step"]) if kern else None
     roofline = dict(kern[dominant], kernel=dominant,
                     peak_source=f"derived: {SM_COUNT} SMs x lanes/SM/clk x {sm_max:.0f} MHz (DESIGN.md Roofline)") \
@@ -327,7 +347,8 @@ def run_ours(args, rank, local_rank, world):
            "data": "synthetic",
            "config": {"workload": w.name, "n_spins_per_gpu": n, "n_intervals": n_int,
                       "n_rf_steps": info["n_rf_steps"], "n_adc": info["n_adc"], "n_blocks": info["n_blocks"],
-                      "output_mode": w.output_mode, "motion": w.velocity is not None, "spin_steps_per_step": spin_steps * world,
+                      "output_mode": w.output_mode, "motion": w.velocity is not None,
+                      "path": "fused" if bloch.bloch_plan_uses_fused(plan.handle, n) else "per_block", "spin_steps_per_step": spin_steps * world,
                       "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
                       "plan_create_upload_s": plan_s},
            "sim_wall_time_s": ms_total / args.steps * 1e-3,
@@ -355,6 +376,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 5, 5b, 5c (ensemble dictionary)")
+    ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
+                    help="execution path (bloch_plan_set_path); auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")

@@ -184,12 +184,27 @@ enum { BLOCH_KIND_OTHER = 0,   /* pack / unpack / block-end propagation only */
        BLOCH_KIND_RF = 1,      /* excitation kernel */
        BLOCH_KIND_SIGNAL = 2,  /* free-precession signal kernel (a6) */
        BLOCH_KIND_REDUCE = 3,  /* second pass of the signal reduction (a7) */
-       BLOCH_N_KINDS = 4 };
+       BLOCH_KIND_FUSED = 4,   /* whole-sequence kernel (a5-a8 in one launch, BLOCH_PATH_FUSED) */
+       BLOCH_N_KINDS = 5 };
 int bloch_plan_set_profiling(bloch_plan *plan, int enable);
 int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *launches_by_kind);
 /* Number of kernels the last bloch_simulate on this plan enqueued (it depends on n_spins through the batching
  * of the second-pass reduction; bloch_plan_info.n_launches is the upper bound with one second pass per block). */
 int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
+
+/* Execution path of bloch_simulate for this plan.
+ *   BLOCH_PATH_PER_BLOCK: one excitation launch per RF block and one signal launch per precession block.
+ *   BLOCH_PATH_FUSED: ONE persistent whole-sequence launch (a CTA per SM owns a chunk of spins for the whole
+ *       sequence; warp-specialised excitation / readout, see csrc/seq.cuh) plus the second-pass reduction.
+ *       Available for SUM_ALL output, fp32 phase, no motion and at most 29 x 32 spins per SM; bloch_simulate
+ *       returns BLOCH_EINVAL when it is forced and not available.
+ *   BLOCH_PATH_AUTO (default): FUSED when available and the sequence is excitation-heavy, else PER_BLOCK.
+ * Both paths compute the same thing; the final magnetisation is bitwise identical, the signal differs only in
+ * the order of the fixed-order sums.  Set before bloch_plan_workspace_bytes: the workspace size depends on it. */
+enum { BLOCH_PATH_AUTO = 0, BLOCH_PATH_PER_BLOCK = 1, BLOCH_PATH_FUSED = 2 };
+int bloch_plan_set_path(bloch_plan *plan, int path);
+/* *out = 1 if bloch_simulate would take the fused path for n_spins on the current device, else 0. */
+int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out);
 
 /* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
  * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA, 2 = DFMA.  Runs `iters` dependent-chain iterations with 8

@@ -53,7 +53,8 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_plan_get_info", "bloch_plan_workspace_bytes", "bloch_plan_upload", "bloch_simulate",
            "bloch_simulate_motion", "bloch_simulate_host_scratch_bytes", "bloch_simulate_host",
            "bloch_simulate_host_motion", "bloch_plan_set_profiling",
-           "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_microbench"]
+           "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
+           "bloch_microbench"]
 
 
 def _load():
@@ -82,6 +83,8 @@ def _load():
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
+    lib.bloch_plan_set_path.argtypes = [vp, C.c_int]
+    lib.bloch_plan_uses_fused.argtypes = [vp, i64, C.POINTER(C.c_int)]
     lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
     for name in EXPORTS:
         if name not in ("bloch_strerror", "bloch_last_error"):
@@ -212,7 +215,18 @@ def bloch_plan_set_profiling(plan: int, enable: bool):
     _check(_lib.bloch_plan_set_profiling(plan, int(bool(enable))))
 
 
-KINDS = ("other", "rf", "signal", "reduce")   # BLOCH_KIND_*
+KINDS = ("other", "rf", "signal", "reduce", "fused")   # BLOCH_KIND_*
+PATHS = {"auto": 0, "per_block": 1, "fused": 2}       # BLOCH_PATH_*
+
+
+def bloch_plan_set_path(plan: int, path):
+    _check(_lib.bloch_plan_set_path(plan, PATHS[path] if isinstance(path, str) else int(path)))
+
+
+def bloch_plan_uses_fused(plan: int, n_spins: int) -> bool:
+    out = C.c_int()
+    _check(_lib.bloch_plan_uses_fused(plan, n_spins, C.byref(out)))
+    return bool(out.value)
 
 
 def bloch_plan_last_timing(plan: int) -> dict:
@@ -239,8 +253,9 @@ def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:
 class Plan:
     """Owns a bloch_plan handle plus the caller-side device buffers (torch tensors)."""
 
-    def __init__(self, seq, **kw):
+    def __init__(self, seq, path="auto", **kw):
         self.handle = bloch_plan_create(seq, **kw)
+        bloch_plan_set_path(self.handle, path)
         self.info = bloch_plan_get_info(self.handle)
         self._tables = None
         self._ws = None

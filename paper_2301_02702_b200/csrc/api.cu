@@ -9,6 +9,7 @@
 #include "internal.h"
 #include "kernels.cuh"
 #include "rf.cuh"
+#include "seq.cuh"
 #include "signal.cuh"
 
 namespace bloch {
@@ -84,6 +85,40 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
     return std::max(worst, std::min(total, kPartialCapBytes / sizeof(float2)));
 }
 
+// Launch shape of the whole-sequence kernel (seq.cuh): one CTA per chunk of spins, chunk = spins per SM rounded
+// up to whole warps; ok = the plan and n_spins qualify, use = bloch_simulate takes it (plan->path, heuristic).
+struct SeqShape {
+    bool ok, use;
+    int n_ctas, chunk, rf_warps, sig_warps, threads, min_items;
+    size_t smem, partial_elems;
+};
+constexpr size_t kSeqPartialCapBytes = size_t(8) << 30;
+
+SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+    SeqShape q{};
+    const bloch_plan_info &inf = plan->info;
+    if (inf.output_mode != BLOCH_OUT_SUM_ALL || inf.motion_mode != BLOCH_MOTION_NONE ||
+        inf.phase_mode != BLOCH_PHASE_FP32 || n_spins <= 0 || plan->path == BLOCH_PATH_PER_BLOCK)
+        return q;
+    const int64_t per_sm = (n_spins + sm_count - 1) / sm_count;
+    q.chunk = (int)std::max<int64_t>(32, (per_sm + 31) / 32 * 32);
+    q.rf_warps = q.chunk / 32;
+    // 10 signal warps: measured optimum on config 5 (14 RF warps per SM; 4: 168 ms, 8: 133, 10: 129.5, 16: 141)
+    const int want = std::min(std::max(env_int("BLOCH_SEQ_SIGNAL_WARPS", 10), 1), 30);
+    q.sig_warps = std::min(want, kSeqMaxThreads / 32 - 1 - q.rf_warps);
+    if (q.sig_warps < std::min(want, 2)) return q;  // no room beside the RF warps: more than 29 x 32 spins per SM
+    q.threads = 32 * (1 + q.rf_warps + q.sig_warps);
+    q.min_items = std::max(1, q.sig_warps * env_int("BLOCH_SEQ_ITEMS_PER_WARP_X4", 4) / 4);
+    q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
+    q.smem = seq_smem_bytes(q.chunk);
+    q.partial_elems = size_t(q.n_ctas) * size_t(std::max<int64_t>(inf.n_adc, 1));
+    if (q.partial_elems * sizeof(float2) > kSeqPartialCapBytes || inf.max_block_adc > INT32_MAX) return q;
+    q.ok = true;
+    // AUTO: the fused kernel pays when the excitation dominates (its readout runs on sig_warps warps per SM only)
+    q.use = plan->path == BLOCH_PATH_FUSED || 2 * inf.n_rf_steps >= inf.n_adc;
+    return q;
+}
+
 // rows of the signal buffer: 1 (SUM_ALL), n_spins (PER_SPIN), n_spins / group_size (GROUPED)
 size_t signal_rows(const bloch_plan *plan, int64_t n_spins) {
     if (plan->info.output_mode == BLOCH_OUT_PER_SPIN) return size_t(n_spins);
@@ -133,7 +168,8 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.scal = (unsigned *)take(kAlign);
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
-        w.partial_elems = partial_elems_for(plan, n_spins, sm_count);
+        const SeqShape q = seq_shape(plan, n_spins, sm_count);
+        w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
@@ -270,6 +306,21 @@ int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *l
     return BLOCH_OK;
 }
 
+int bloch_plan_set_path(bloch_plan *plan, int path) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    if (path != BLOCH_PATH_AUTO && path != BLOCH_PATH_PER_BLOCK && path != BLOCH_PATH_FUSED)
+        return fail(BLOCH_EINVAL, "path is not a BLOCH_PATH_* value");
+    plan->path = path;
+    return BLOCH_OK;
+}
+
+int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out) {
+    if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
+    const SeqShape q = seq_shape(plan, n_spins, sm_count_cached());
+    *out = (q.ok && q.use) ? 1 : 0;
+    return BLOCH_OK;
+}
+
 int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out) {
     if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
     *out = plan->last.launches;
@@ -331,6 +382,41 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
+
+    const SeqShape sq = seq_shape(plan, n_spins, sms);
+    if (plan->path == BLOCH_PATH_FUSED && !sq.ok)
+        return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output, fp32 phase, no motion and <= 29 x 32 spins per SM");
+    if (sq.ok && sq.use) {
+        // ONE persistent launch for the whole sequence + the second pass over all ADC samples
+        static bool attr_set = false;  // per process; the attribute is sticky for the function
+        if (!attr_set) {
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)seq_smem_bytes(kSeqMaxThreads)));
+            attr_set = true;
+        }
+        if ((rc = taps.mark(BLOCH_KIND_FUSED))) return rc;
+        seq_kernel<<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
+            plan->d_tables, reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off), (int)plan->blocks.size(),
+            w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items, (const float *)w.scal, w.partial, (long long)plan->info.n_adc,
+            d_Mxy ? 1 : 0);
+        ++launches;
+        if (plan->info.n_adc > 0) {
+            if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
+            reduce_kernel<<<(unsigned)((plan->info.n_adc + 31) / 32), dim3(32, 8), 0, stream>>>(
+                w.partial, sq.n_ctas, (int)plan->info.n_adc, (float2 *)d_signal);
+            ++launches;
+        }
+        if (d_Mxy) {
+            if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
+            unpack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, w.S, (float2 *)d_Mxy, d_Mz);
+            ++launches;
+        }
+        if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;  // closing event
+        if (plan->profiling) plan->event_kind.resize(taps.used);
+        plan->last.launches = launches;
+        BLOCH_CUDA(cudaGetLastError());
+        return BLOCH_OK;
+    }
 
     bool pending = false;
     PropRec prop{0, 0, 0, 0, 0, 0, 0};

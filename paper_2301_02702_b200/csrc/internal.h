@@ -59,6 +59,19 @@ struct Block {
     double mend[3] = {0, 0, 0};  // motion: first moment mu' = -gamma_bar * sum (G_n t_n + G_{n+1} t_{n+1}) dt / 2 [turns s/m]
 };
 
+// Whole-sequence program for the fused kernel (seq.cuh): one 64-B descriptor per block, in block order, appended
+// to the table buffer at bloch_plan::prog_off.
+struct SeqOp {
+    int32_t type;       // kBlockRF / kBlockPrecession
+    int32_t n;          // RF: tiles of the block's table; precession: ADC samples served (evaluated points)
+    int64_t table_off;  // byte offset of the block's records in the table buffer
+    int64_t adc_first;  // precession: first ADC sample served, in ADC order
+    int64_t pad;
+    double kend[3];     // precession block end record: k' = -gamma_bar K(T) [turns/m]   (offset 32: read as double4)
+    double tau_end;     //                              T [s]
+};
+static_assert(sizeof(SeqOp) == 64, "SeqOp must be 64 B");
+
 struct Timing {
     float ms_rf = 0, ms_prec = 0, ms_total = 0;
     int64_t launches = 0;
@@ -73,6 +86,8 @@ struct bloch_plan {
     std::vector<bloch::Block> blocks;
     std::vector<unsigned char> tables;   // host staging copy of the device tables
     const unsigned char *d_tables = nullptr;
+    int64_t prog_off = 0;                // byte offset of the SeqOp program in the table buffer
+    int path = 0;                        // BLOCH_PATH_*
     // profiling taps
     bool profiling = false;
     mutable std::vector<void *> events;  // cudaEvent_t pool

@@ -87,18 +87,19 @@ struct PropRec {
 
 __device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, const float4 &c, const float4 &v,
                                           float &mx, float &my, float &mz) {
-    double th = p.kx * (double)a.x + p.ky * (double)a.y + p.kz * (double)a.z -
-                (double)c.w * 0.15915494309189535 * p.tau;
-    th += p.mx * (double)v.x + p.my * (double)v.y + p.mz * (double)v.z;  // x(t) = x + v t
+    // every contraction is written out (__fma_rn / __fmaf_rn / __fmul_rn), so rf_kernel and seq_kernel round alike
+    double th = __fma_rn(p.kx, (double)a.x, __fma_rn(p.ky, (double)a.y, __fma_rn(p.kz, (double)a.z,
+                         -__dmul_rn(__dmul_rn((double)c.w, 0.15915494309189535), p.tau))));
+    th = __fma_rn(p.mx, (double)v.x, __fma_rn(p.my, (double)v.y, __fma_rn(p.mz, (double)v.z, th)));  // x(t) = x + v t
     th -= rint(th);
     float sn, cs;
     sincospif(2.0f * (float)th, &sn, &cs);
     const float tau = (float)p.tau;
-    const float e2 = expf(-tau * c.y), e1 = expf(-tau * c.x);
-    const float ax = mx * e2, ay = my * e2;
-    mx = ax * cs - ay * sn;
-    my = ax * sn + ay * cs;
-    mz = c.z + (mz - c.z) * e1;  // Eq 11
+    const float e2 = expf(-__fmul_rn(tau, c.y)), e1 = expf(-__fmul_rn(tau, c.x));
+    const float ax = __fmul_rn(mx, e2), ay = __fmul_rn(my, e2);
+    mx = __fmaf_rn(ax, cs, -__fmul_rn(ay, sn));
+    my = __fmaf_rn(ax, sn, __fmul_rn(ay, cs));
+    mz = __fmaf_rn(__fsub_rn(mz, c.z), e1, c.z);  // Eq 11
 }
 
 // PER_SPIN output (dictionary mode): one thread per (spin, point); accurate functions because nothing

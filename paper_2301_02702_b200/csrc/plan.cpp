@@ -345,8 +345,24 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         const size_t bytes = b.type == kBlockRF ? rf_img[bi].size() : size_t(b.adc_count) * rec_bytes;
         off = align_up(off + bytes, kAlign);
     }
+    // whole-sequence program for the fused kernel: one SeqOp per block
+    const size_t prog_off = off;
+    off = align_up(off + blocks.size() * sizeof(SeqOp), kAlign);
     if (off == 0) off = kAlign;
     plan->tables.assign(off, 0);
+    plan->prog_off = (int64_t)prog_off;
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        const Block &b = blocks[bi];
+        SeqOp op;
+        std::memset(&op, 0, sizeof(op));
+        op.type = b.type;
+        op.n = (int32_t)(b.type == kBlockRF ? b.n_tiles : b.adc_count);
+        op.table_off = b.table_off;
+        op.adc_first = b.adc_first;
+        for (int a = 0; a < 3; ++a) op.kend[a] = b.kend[a];
+        op.tau_end = b.tau_end;
+        std::memcpy(plan->tables.data() + prog_off + bi * sizeof(SeqOp), &op, sizeof(op));
+    }
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
         const Block &b = blocks[bi];
         unsigned char *dst = plan->tables.data() + b.table_off;

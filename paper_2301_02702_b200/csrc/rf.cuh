@@ -102,12 +102,12 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
     const float dtdw = hd.dt * sp.dw;
     // Eq 2: gamma Bz dt = g . x + dw dt
     const float wz_u = fmaf(hd.gx, sp.x, fmaf(hd.gy, sp.y, fmaf(hd.gz, sp.z, dtdw)));
-    const float wz2_u = wz_u * wz_u;
+    const float wz2_u = __fmul_rn(wz_u, wz_u);  // __fmul_rn / __fadd_rn: no contraction, rf_kernel and seq_kernel round alike
 #define BLOCH_RF_LOAD(k)                                                              \
     float wx, wy, wz, q;                                                              \
     if (MODE == 0) {                                                                  \
         const float4 a = rec[k];                                                      \
-        wx = a.x; wy = a.y; wz = wz_u; q = a.z + wz2_u;                               \
+        wx = a.x; wy = a.y; wz = wz_u; q = __fadd_rn(a.z, wz2_u);                              \
     } else if (MODE == 1) {                                                           \
         const float4 a = rec[2 * (k)], g = rec[2 * (k) + 1];                          \
         wx = a.x; wy = a.y;                                                           \

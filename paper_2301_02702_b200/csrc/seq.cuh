@@ -1,0 +1,275 @@
+// seq.cuh -- whole-sequence kernel (a5-a8 in ONE launch) for plans with few spins and many blocks (MRF, GRE).
+//
+// With 65,536 spins an excitation launch holds 3.5 warps per SM sub-partition and is bound by the latency of
+// its own dependent chain, and the signal launch that follows leaves the FMA pipe half idle; launched one
+// after the other neither fills the machine (profiles/r01_v2_cfg5.md).  Spins are independent,
+// so here ONE persistent CTA per SM owns a fixed chunk of spins for the whole sequence and its warps are
+// specialised:
+//   warp 0              producer: streams the RF step tiles of ALL excitation blocks, in sequence order, through a
+//                       4-stage shared-memory ring with 1-D bulk copies (TMA) -- across block boundaries, so the
+//                       first tile of the next pulse is already resident when the RF warps get there
+//   warps 1 .. R        RF warps: one spin per thread, magnetisation in registers for the WHOLE SEQUENCE (a8:
+//                       rf_tile of rf.cuh; block-end free precession by propagate()); at the start of every
+//                       precession block that serves ADC samples they publish (Mxy, e2) to a double-buffered
+//                       shared array and carry straight on with the next pulse
+//   warps R+1 .. R+G    signal warps: for every published state evaluate the block's ADC samples (a6: a thread
+//                       owns P adjacent samples and walks the chunk's spins in shared memory, arithmetic as
+//                       signal_kernel) and write the CTA's partial sums P[cta][adc] (a7; reduce_kernel adds
+//                       the CTAs in index order -- still no float atomics, still bitwise reproducible).  The
+//                       block's samples are cut into items of 32 x P samples which the warps take from a
+//                       shared counter, so a sub-partition that holds fewer RF warps serves more items; a
+//                       sample's sum is one thread's walk over the chunk in spin order whichever warp takes it
+// so the FMA-bound excitation of pulse k+1 and the MUFU-bound readout of block k share the SM's issue slots.
+// The roles meet only at mbarriers (tile full/empty, state full/empty); there is no CTA-wide barrier after set-up.
+// The published states go through a ring of kSeqStateBufs buffers: the signal warps may lag that many blocks.
+// The state is rounded to one float per component at the end of every RF block exactly as rf_kernel stores it,
+// so the final magnetisation is bitwise equal to the per-block path.
+#pragma once
+#include <type_traits>
+
+#include "internal.h"
+#include "kernels.cuh"
+#include "rf.cuh"
+#include "tma.cuh"
+
+namespace bloch {
+
+constexpr int kSeqStages = 4;
+constexpr int kSeqTileStride = 4224;  // >= kRfHdrBytes + kRfTileSteps * 32 (static plans), multiple of 128
+constexpr int kSeqMaxThreads = 1024;
+constexpr int kSeqStateBufs = 4;
+constexpr int kSeqBarBytes = 256;
+static_assert(kSeqTileStride >= kRfHdrBytes + kRfTileSteps * 32 && kSeqTileStride % 128 == 0, "tile stride");
+
+// dynamic shared memory: [ring: kSeqStages x kSeqTileStride][barriers + item counters: 256 B][shA: chunk float4]
+// [shS: kSeqStateBufs x chunk float4]
+__host__ __device__ inline size_t seq_smem_bytes(int chunk) {
+    return size_t(kSeqStages) * kSeqTileStride + kSeqBarBytes + size_t(1 + kSeqStateBufs) * chunk * sizeof(float4);
+}
+static_assert((2 * kSeqStages + 2 * kSeqStateBufs) * 8 + kSeqStateBufs * 4 <= kSeqBarBytes, "barrier area");
+
+// One item (32 x P adjacent ADC samples starting at `base`) of a precession block for the chunk's spins.
+template <int P>
+__device__ __forceinline__ void seq_signal_item(const float4 *__restrict__ recs, int n_pts, int base, const float4 *shA,
+                                                const float4 *shS, int cnt, int lane, float r2max_log2e,
+                                                float2 *__restrict__ out) {
+    const int p0 = base + lane * P;
+    float kx[P], ky[P], kz[P], tau[P], cj[P], ar[P], ai[P];
+    float cmax = 0.f;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        const int p = p0 + j;
+        float4 r = make_float4(0.f, 0.f, 0.f, j ? tau[0] : 0.f);
+        if (p < n_pts) r = recs[p];
+        kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
+        cj[j] = (r.w - tau[0]) * 0.6931471805599453f;
+        cmax = fmaxf(cmax, fabsf(cj[j]));
+        ar[j] = 0.f; ai[j] = 0.f;
+    }
+    // exp(-tau_j/T2), j > 0, from the j = 0 value by a cubic series when (tau_j - tau_0)/T2 <= 0.02 for every spin
+    const bool series = P > 1 && __all_sync(0xffffffffu, cmax * r2max_log2e <= 0.02f);
+    auto run = [&](auto series_tag) {
+        constexpr bool SERIES = decltype(series_tag)::value;
+#pragma unroll 2
+        for (int s = 0; s < cnt; ++s) {
+            const float4 a = shA[s];
+            const float4 st = shS[s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            float er0 = 0.f, ei0 = 0.f;
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                const float th = fmaf(kx[j], a.x, fmaf(ky[j], a.y, fmaf(kz[j], a.z, tau[j] * a.w)));  // radians
+                const float sn = __sinf(th), cs = __cosf(th);
+                float er, ei;
+                if (j == 0 || !SERIES) {
+                    const float e = ex2_approx(tau[j] * st.w);
+                    er = st.x * e;
+                    ei = st.y * e;
+                    if (j == 0) { er0 = er; ei0 = ei; }
+                } else {
+                    const float y = cj[j] * st.w;
+                    const float pe = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+                    er = er0 * pe;
+                    ei = ei0 * pe;
+                }
+                ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
+                ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
+            }
+        }
+    };
+    if (series) run(std::true_type{});
+    else run(std::false_type{});
+#pragma unroll
+    for (int j = 0; j < P; ++j)
+        if (p0 + j < n_pts) out[p0 + j] = make_float2(ar[j], ai[j]);
+}
+
+// A signal warp's share of one block: items taken from the block's shared counter until none is left.
+template <int P>
+__device__ __forceinline__ void seq_signal_block(const float4 *__restrict__ recs, int n_pts, const float4 *shA,
+                                                 const float4 *shS, int cnt, int lane, int *item_ctr,
+                                                 float r2max_log2e, float2 *__restrict__ out) {
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = atomicAdd(item_ctr, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        const int base = item * (32 * P);
+        if (base >= n_pts) break;
+        seq_signal_item<P>(recs, n_pts, base, shA, shS, cnt, lane, r2max_log2e, out);
+    }
+}
+
+__global__ void __launch_bounds__(kSeqMaxThreads, 1)
+seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ ops, int n_ops,
+           const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n, int chunk,
+           int rf_warps, int min_items, const float *__restrict__ scal, float2 *__restrict__ partial,
+           long long n_adc, int final_state) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char *ring = smem;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kSeqStages * kSeqTileStride);
+    uint64_t *tile_full = bars, *tile_empty = bars + kSeqStages, *st_full = bars + 2 * kSeqStages,
+             *st_empty = bars + 2 * kSeqStages + kSeqStateBufs;
+    int *item_ctr = reinterpret_cast<int *>(bars + 2 * kSeqStages + 2 * kSeqStateBufs);  // [kSeqStateBufs]
+    float4 *shA = reinterpret_cast<float4 *>(smem + kSeqStages * kSeqTileStride + kSeqBarBytes);
+    float4 *shS = shA + chunk;  // [kSeqStateBufs][chunk]
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const int n_rf_thr = rf_warps * 32;
+    const int nsig = (int)blockDim.x - 32 - n_rf_thr;
+    const int s0 = blockIdx.x * chunk;
+    const int cnt = min(chunk, n - s0);
+    if (tid == 0) {
+        for (int k = 0; k < kSeqStages; ++k) {
+            mbar_init(&tile_full[k], 1);
+            mbar_init(&tile_empty[k], n_rf_thr);
+        }
+        for (int k = 0; k < kSeqStateBufs; ++k) {
+            mbar_init(&st_full[k], n_rf_thr);
+            mbar_init(&st_empty[k], nsig);
+            item_ctr[k] = 0;
+        }
+        mbar_init_fence();
+    }
+    __syncthreads();  // the only CTA-wide barrier: from here on the roles meet at mbarriers
+
+    if (warp == 0) {
+        // ---------------------------------------------------------------- producer
+        if (tid != 0) return;
+        int g = 0;
+        for (int oi = 0; oi < n_ops; ++oi) {
+            const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
+            if (tn.x != kBlockRF) continue;
+            const unsigned char *tbl = tables + ops[oi].table_off;
+            const int2 *dir = reinterpret_cast<const int2 *>(tbl);
+            for (int t = 0; t < tn.y; ++t, ++g) {
+                const int st = g % kSeqStages, use = g / kSeqStages;
+                if (use > 0) mbar_wait(&tile_empty[st], (uint32_t)((use - 1) & 1));
+                const int2 d = dir[t];
+                mbar_expect_tx(&tile_full[st], (uint32_t)d.y);
+                bulk_g2s(ring + st * kSeqTileStride, tbl + d.x, (uint32_t)d.y, &tile_full[st]);
+            }
+        }
+        return;
+    }
+
+    if (warp <= rf_warps) {
+        // ---------------------------------------------------------------- RF warps: one spin per thread
+        const int r = tid - 32;
+        const bool active = r < cnt;
+        const int i = s0 + r;
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f),
+               s = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (active) {
+            a = A[i];
+            c = Cc[i];
+            s = S[i];
+            shA[r] = a;
+        }
+        float hx = s.x, hy = s.y, hz = s.z, lx = 0.f, ly = 0.f, lz = 0.f;
+        const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z, 0.f, 0.f, 0.f};
+        const float ax = fabsf(sp.x), ay = fabsf(sp.y), az = fabsf(sp.z), adw = fabsf(sp.dw);
+        bool pending = false;
+        PropRec prop{0, 0, 0, 0, 0, 0, 0};
+        int g = 0, pub = 0;
+        for (int oi = 0; oi < n_ops; ++oi) {
+            const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
+            if (pending) {  // end transform of the precession block before this one (Eq 10-11 in closed form)
+                propagate(prop, a, c, v, hx, hy, hz);
+                pending = false;
+            }
+            if (tn.x == kBlockRF) {
+                for (int t = 0; t < tn.y; ++t, ++g) {
+                    const int st = g % kSeqStages;
+                    mbar_wait(&tile_full[st], (uint32_t)((g / kSeqStages) & 1));
+                    const unsigned char *tile = ring + st * kSeqTileStride;
+                    const RfTileHdr hd = *reinterpret_cast<const RfTileHdr *>(tile);
+                    RfRelax rx;
+                    rx.D1 = -expm1f(-hd.dt * sp.r1);
+                    rx.D2 = -expm1f(-hd.dt * sp.r2);
+                    rx.E1 = 1.0f - rx.D1;
+                    rx.E2 = 1.0f - rx.D2;
+                    rx.D1m0 = rx.D1 * sp.m0;
+                    const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
+                    const float qb = fmaf(wzb, wzb, hd.wxy2_max);
+                    const bool uni = (hd.flags & kRfFlagUniformG) != 0;
+                    const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0
+                                     : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
+#define BLOCH_SEQ_TILE(T)                                                          \
+    do {                                                                           \
+        if (uni) rf_tile<T, 0>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);          \
+        else rf_tile<T, 1>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);              \
+    } while (0)
+                    if (tier == 0) BLOCH_SEQ_TILE(0);
+                    else if (tier == 1) BLOCH_SEQ_TILE(1);
+                    else BLOCH_SEQ_TILE(2);
+#undef BLOCH_SEQ_TILE
+                    mbar_arrive(&tile_empty[st]);  // this thread is done reading the stage
+                }
+                // round the state to one float per component, as rf_kernel stores it between launches
+                hx += lx; hy += ly; hz += lz;
+                lx = 0.f; ly = 0.f; lz = 0.f;
+            } else {
+                if (tn.y > 0) {  // publish the block-start state for the signal warps
+                    const int b = pub % kSeqStateBufs, use = pub / kSeqStateBufs;
+                    if (use > 0) mbar_wait(&st_empty[b], (uint32_t)((use - 1) & 1));
+                    if (active) shS[b * chunk + r] = make_float4(hx, hy, hz, s.w);
+                    if (r == 0) item_ctr[b] = 0;  // every signal warp is past its last atomicAdd of the previous use
+                    mbar_arrive(&st_full[b]);
+                    ++pub;
+                }
+                const double4 k4 = *reinterpret_cast<const double4 *>(&ops[oi].kend[0]);
+                prop.kx = k4.x; prop.ky = k4.y; prop.kz = k4.z; prop.tau = k4.w;
+                pending = true;
+            }
+        }
+        if (final_state) {
+            if (pending) propagate(prop, a, c, v, hx, hy, hz);
+            if (active) S[i] = make_float4(hx, hy, hz, s.w);
+        }
+        return;
+    }
+
+    // -------------------------------------------------------------------- signal warps
+    {
+        const int lane = tid & 31;
+        const float r2max_log2e = scal[0] * kLog2e;
+        float2 *row = partial + (size_t)blockIdx.x * (size_t)n_adc;
+        int pub = 0;
+        for (int oi = 0; oi < n_ops; ++oi) {
+            const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
+            if (tn.x != kBlockPrecession || tn.y == 0) continue;
+            const float4 *recs = reinterpret_cast<const float4 *>(tables + ops[oi].table_off);
+            float2 *out = row + ops[oi].adc_first;
+            const int b = pub % kSeqStateBufs;
+            mbar_wait(&st_full[b], (uint32_t)((pub / kSeqStateBufs) & 1));
+            const float4 *stS = shS + b * chunk;
+            // item size: the largest P that still leaves min_items items (about one per signal warp)
+            if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            else if (tn.y >= 64 * min_items) seq_signal_block<2>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            else seq_signal_block<1>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            mbar_arrive(&st_empty[b]);
+            ++pub;
+        }
+    }
+}
+
+}  // namespace bloch

@@ -34,25 +34,33 @@ def errors(got, ref):
 
 
 def check(B, oracle_mod, ph, s, what, output_mode="sum", **plan_kw):
+    """Both execution paths (one launch per block; the whole-sequence kernel where the plan qualifies) against
+    the oracle.  Returns the launch count of the per-block path."""
     import torch
-    plan = B.Plan(s, output_mode=output_mode, **plan_kw)
-    dev = B.phantom_to_device(ph)
-    Mxy = torch.zeros(ph.n, 2, dtype=torch.float32, device="cuda")
-    Mz = torch.zeros(ph.n, dtype=torch.float32, device="cuda")
-    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz)
-    torch.cuda.synchronize()
-    launches = B.bloch_plan_last_launches(plan.handle)
-    plan.close()
     ref, rxy, rz = oracle_mod.simulate(ph, s, output_mode=output_mode, return_state=True)
-    m = Mxy.cpu().numpy()
-    got_state = np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)])
     ref_state = np.concatenate([rxy, rz.astype(np.complex128)])
-    for name, g, r in (("signal", sig.cpu().numpy(), ref), ("state", got_state, ref_state)):
-        if r.size == 0:
+    dev = B.phantom_to_device(ph)
+    launches = None
+    for path in ("per_block", "fused"):
+        plan = B.Plan(s, path=path, output_mode=output_mode, **plan_kw)
+        if path == "fused" and not B.bloch_plan_uses_fused(plan.handle, ph.n):
+            plan.close()
             continue
-        emax, nrmse = errors(g, r)
-        print(f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}")
-        assert emax <= TOL_MAX and nrmse <= TOL_NRMSE, f"{what} {name}: max {emax:.3e} nrmse {nrmse:.3e}"
+        Mxy = torch.zeros(ph.n, 2, dtype=torch.float32, device="cuda")
+        Mz = torch.zeros(ph.n, dtype=torch.float32, device="cuda")
+        sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz)
+        torch.cuda.synchronize()
+        if path == "per_block":
+            launches = B.bloch_plan_last_launches(plan.handle)
+        plan.close()
+        m = Mxy.cpu().numpy()
+        got_state = np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)])
+        for name, g, r in (("signal", sig.cpu().numpy(), ref), ("state", got_state, ref_state)):
+            if r.size == 0:
+                continue
+            emax, nrmse = errors(g, r)
+            print(f"{what} [{path}] {name}: max {emax:.3e} nrmse {nrmse:.3e}")
+            assert emax <= TOL_MAX and nrmse <= TOL_NRMSE, f"{what} [{path}] {name}: max {emax:.3e} nrmse {nrmse:.3e}"
     return launches
 
 
