@@ -23,14 +23,28 @@ def shard_bounds(n_spins: int, rank: int, world_size: int):
     return lo, lo + base + (1 if rank < rem else 0)
 
 
-def reduce_signal(signal, group=None):
+def reduce_signal(signal, group=None, deterministic=False):
     """In-place sum over ranks of a complex64 signal tensor [n_adc] (SUM_ALL output).  NCCL all-reduce on
     GPU tensors, gloo on CPU tensors; complex is reduced through its real view.  A no-op when
-    torch.distributed is not initialised (single GPU)."""
+    torch.distributed is not initialised (single GPU).
+
+    deterministic=True: all-gather the per-rank signals and add them in rank order on every rank, so the result
+    does not depend on the collective's algorithm (ring / tree / in-switch reduction) -- the multi-GPU
+    continuation of the fixed-order two-pass reduction inside one GPU; costs world_size x the
+    bytes of the all-reduce, still <= 8 MB x world_size once per simulation."""
     import torch
     import torch.distributed as dist
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
         return signal
     view = torch.view_as_real(signal) if signal.is_complex() else signal
-    dist.all_reduce(view, op=dist.ReduceOp.SUM, group=group)
+    if not deterministic:
+        dist.all_reduce(view, op=dist.ReduceOp.SUM, group=group)
+        return signal
+    world = dist.get_world_size(group)
+    parts = [torch.empty_like(view) for _ in range(world)]
+    dist.all_gather(parts, view.contiguous(), group=group)
+    acc = parts[0].clone()
+    for r in range(1, world):     # fixed order: ((s0 + s1) + s2) + ...
+        acc += parts[r]
+    view.copy_(acc)
     return signal

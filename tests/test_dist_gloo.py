@@ -55,6 +55,11 @@ def _worker(rank, world, port, out_dir):
         sig = torch.from_numpy(part.astype(np.complex64))
         reduce_signal(sig)                      # the path's one collective
         np.save(os.path.join(out_dir, f"sig{rank}.npy"), sig.numpy())
+        # the rank-ordered variant: same sum, and bitwise what adding the shards in rank order gives
+        det = torch.from_numpy(part.astype(np.complex64))
+        reduce_signal(det, deterministic=True)
+        np.save(os.path.join(out_dir, f"det{rank}.npy"), det.numpy())
+        np.save(os.path.join(out_dir, f"part{rank}.npy"), part.astype(np.complex64))
         # a second, real-valued tensor goes through the same call
         t = torch.full((4,), float(rank + 1))
         reduce_signal(t)
@@ -73,6 +78,9 @@ def test_two_rank_shards_sum_to_the_full_signal(tmp_path, oracle_mod):
     assert np.array_equal(a, b), "all-reduce must leave the same signal on every rank"
     scale = np.abs(full).max()
     assert np.abs(a - full).max() / scale < 1e-6   # complex64 rounding of the two partial sums
+    d0, d1 = np.load(tmp_path / "det0.npy"), np.load(tmp_path / "det1.npy")
+    want = np.load(tmp_path / "part0.npy") + np.load(tmp_path / "part1.npy")   # rank order, complex64 adds
+    assert np.array_equal(d0, d1) and np.array_equal(d0.view(np.float32), want.view(np.float32))
 
 
 def test_reduce_signal_is_a_noop_without_a_process_group():

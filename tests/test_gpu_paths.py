@@ -139,3 +139,31 @@ def test_batched_second_pass_over_many_blocks(B, oracle_mod):
     a = check(B, oracle_mod, w.phantom, w.seq, "batched reduce")
     b = check(B, oracle_mod, w.phantom, w.seq, "batched reduce, cut blocks", max_block_points=50)
     assert b > a
+
+
+def test_adiabatic_inversion_recovery_long_soft_pulse(B, oracle_mod):
+    """The paper's stated weak spot: a long soft pulse with a frequency sweep.  10.24 ms hyperbolic-
+    secant inversion (10,240 steps of phase-modulated complex B1 = 80 step tiles) under a slice gradient, spins spread
+    over +-1.5 kHz of off-resonance so that some lie inside, some on the edge of and some outside the inverted band,
+    then inversion recovery, a hard 90 and a gradient-echo readout."""
+    mu, beta, T, n = 5.0, 800.0, 10.24e-3, 10240
+    dt = T / n
+    tm = (np.arange(n) + 0.5) * dt - T / 2
+    amp = 4500.0 / W.GAMMA / np.cosh(beta * tm)
+    phi = mu * np.log(1.0 / np.cosh(beta * tm))
+    t90 = 40e-3
+    b90 = (np.pi / 2) / (W.GAMMA * 1e-4)
+    rf = (np.concatenate([1e-4 + np.arange(n) * dt, t90 + np.arange(10) * 1e-5]),
+          np.concatenate([np.full(n, dt), np.full(10, 1e-5)]),
+          np.concatenate([amp * np.cos(phi), np.full(10, b90)]),
+          np.concatenate([amp * np.sin(phi), np.zeros(10)]))
+    g = {2: ([0.0, 1e-4, 1e-4 + T, 2e-4 + T], [0, 2e-3, 2e-3, 0]),
+         0: ([t90 + 2e-4, t90 + 3e-4, t90 + 8e-4, t90 + 9e-4, t90 + 2.0e-3, t90 + 2.1e-3], [0, -6e-3, -6e-3, 6e-3, 6e-3, 0])}
+    adc = t90 + 9.5e-4 + (np.arange(256) + 0.5) * 4e-6
+    s = seq(g=g, rf=rf, adc=adc, t_end=t90 + 3e-3, dt_rf_max=1.0)
+    ph = rand_phantom(3000, 21, zmax=0.01, dwmax=2 * np.pi * 1500.0, t2=(0.03, 0.3))
+    check(B, oracle_mod, ph, s, "adiabatic inversion recovery")
+    _, _, rz = oracle_mod.simulate(ph, seq(g={2: g[2]}, rf=tuple(a[:n] for a in rf), t_end=2e-4 + T, dt_rf_max=1.0),
+                                   return_state=True)
+    frac = rz / ph.M0
+    assert (frac < -0.8).sum() > 300 and (frac > 0.8).sum() > 300, "the phantom must straddle the inverted band"

@@ -416,3 +416,37 @@ def test_grouped_output_is_a_fisp_ensemble_dictionary(oracle_mod):
                                rtol=0, atol=1e-10)
     with pytest.raises(ValueError):
         oracle_mod.simulate(ph, s, output_mode="grouped", group_size=5)
+
+
+# ---------------------------------------------------------------------------------------------- P11
+def hs_pulse(T, n, w1max, mu, beta, t0=0.0):
+    """Hyperbolic-secant pulse B1(t) = (w1max / gamma) sech(beta t)^(1 + i mu), piecewise constant at step midpoints."""
+    dt = T / n
+    tm = (np.arange(n) + 0.5) * dt - T / 2
+    amp = w1max / GAMMA / np.cosh(beta * tm)
+    phi = mu * np.log(1.0 / np.cosh(beta * tm))
+    return t0 + np.arange(n) * dt, np.full(n, dt), amp * np.cos(phi), amp * np.sin(phi)
+
+
+@pytest.mark.parametrize("w1max", [3000.0, 4500.0])
+def test_p11_adiabatic_hyperbolic_secant_inversion_profile(oracle_mod, w1max):
+    """A long soft pulse with a frequency sweep -- the paper's own weak spot ("long soft RF pulses
+    (like adiabatic pulses)") -- has a closed form without relaxation: for B1 = w1max sech(beta t)^(1+i mu) over the
+    whole time axis the Bloch equations solve in hypergeometric functions and
+        Mz/M0 = tanh(a+b) tanh(a-b) + cos(pi sqrt((w1max/beta)^2 - mu^2)) sech(a+b) sech(a-b),
+        a = pi Omega / (2 beta), b = pi mu / 2                       (Silver, Joseph & Hoult, Phys Rev A 31, 1985).
+    15,000 steps of complex, phase-modulated B1 composed by Eq 6-9 must land on it for every off-resonance Omega,
+    inside, on the edge of and outside the inverted band |Omega| < mu beta; the pulse is cut at beta T/2 = 12 where
+    sech = 1.2e-5.  Both amplitudes (below and above w1max = mu beta, where the square root turns imaginary)."""
+    mu, beta, T, n = 5.0, 800.0, 30e-3, 15000
+    Om = np.linspace(-8000.0, 8000.0, 81)
+    ph = phantom(dw=Om)                                            # T1 = T2 = inf
+    s = seq(rf=hs_pulse(T, n, w1max, mu, beta), t_end=T, dt_rf_max=T / n)
+    _, mxy, mz = oracle_mod.simulate(ph, s, return_state=True)
+    a, b = math.pi * Om / (2 * beta), math.pi * mu / 2
+    root = np.sqrt(complex((w1max / beta) ** 2 - mu ** 2))
+    want = np.tanh(a + b) * np.tanh(a - b) + np.cos(math.pi * root).real / (np.cosh(a + b) * np.cosh(a - b))
+    np.testing.assert_allclose(mz, want, rtol=0, atol=1e-4)
+    np.testing.assert_allclose(np.abs(mxy) ** 2 + mz ** 2, 1.0, rtol=0, atol=1e-9)   # a rotation: |M| kept
+    inside, outside = np.abs(Om) < 0.4 * mu * beta, np.abs(Om) > 1.5 * mu * beta
+    assert mz[inside].max() < -0.98 and mz[outside].min() > 0.999                      # what "inversion band" means
