@@ -363,7 +363,8 @@ def run_ours(args, rank, local_rank, world):
            "ms_by_kind_per_step": {k: v / args.steps for k, v in kinds_ms.items()}}
     if args.microbench:
         out["pipe_microbench"] = {"mufu_ops_per_s": bloch.bloch_microbench(0), "ffma_per_s": bloch.bloch_microbench(1),
-                                  "dfma_per_s": bloch.bloch_microbench(2)}
+                                  "dfma_per_s": bloch.bloch_microbench(2),
+                                  "ffma_3_distinct_regs_per_s": bloch.bloch_microbench(3)}
     if not args.no_cpu_baseline:
         cb, _, _ = time_oracle(w, n_int, args.cpu_budget)
         out["cpu_baseline"] = cb

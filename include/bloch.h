@@ -207,7 +207,8 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
 int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out);
 
 /* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
- * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA, 2 = DFMA.  Runs `iters` dependent-chain iterations with 8
+ * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA (two operands reused), 2 = DFMA, 3 = FFMA with three different changing
+ * register operands (register-file operand bandwidth, the bound of the RF step's cross products).  Runs `iters` dependent-chain iterations with 8
  * independent chains per thread on all SMs at full occupancy and returns operations per second. */
 int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream);
 

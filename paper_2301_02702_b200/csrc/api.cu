@@ -626,7 +626,7 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins, const fl
 }
 
 int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {
-    if (!ops_per_s || iters <= 0 || kind < 0 || kind > 2) return fail(BLOCH_EINVAL, "bad microbench argument");
+    if (!ops_per_s || iters <= 0 || kind < 0 || kind > 3) return fail(BLOCH_EINVAL, "bad microbench argument");
     int rc = check_arch();
     if (rc) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -642,7 +642,8 @@ int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {
         BLOCH_CUDA(cudaEventRecord(e0, stream));
         if (kind == 0) mb_mufu<<<grid, threads, 0, stream>>>(iters, d_out);
         else if (kind == 1) mb_ffma<<<grid, threads, 0, stream>>>(iters, d_out);
-        else mb_dfma<<<grid, threads, 0, stream>>>(iters, d_out);
+        else if (kind == 2) mb_dfma<<<grid, threads, 0, stream>>>(iters, d_out);
+        else mb_ffma3<<<grid, threads, 0, stream>>>(iters, d_out);
         BLOCH_CUDA(cudaEventRecord(e1, stream));
         BLOCH_CUDA(cudaEventSynchronize(e1));
         float ms = 0.f;

@@ -239,6 +239,25 @@ __global__ void __launch_bounds__(256) mb_ffma(int iters, float *out) {
     for (int k = 0; k < 8; ++k) s += v[k];
     if (s == 123.456f) out[0] = s;
 }
+// FFMA whose three source operands are three different, changing registers (no operand reuse, no immediate):
+// the form most FFMAs of the RF step have (cross products).  The register file delivers about two 32-bit operands
+// per lane per clock, so this runs at ~2/3 of the mb_ffma rate.
+__global__ void __launch_bounds__(256) mb_ffma3(int iters, float *out) {
+    float v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = 0.5f + 0.001f * (threadIdx.x + k);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(v[k]) : "f"(v[(k + 3) & 7]), "f"(v[(k + 5) & 7]));
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += v[k];
+    if (s == 123.456f) out[0] = s;
+}
 __global__ void __launch_bounds__(256) mb_dfma(int iters, float *out) {
     double v[8];
     const double a = 1.0 + 1e-12 * threadIdx.x, b = 1e-15 * blockIdx.x;
