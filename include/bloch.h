@@ -198,7 +198,8 @@ int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
  *       sequence; warp-specialised excitation / readout, see csrc/seq.cuh) plus the second-pass reduction.
  *       Available for SUM_ALL output, fp32 phase, no motion and at most 29 x 32 spins per SM; bloch_simulate
  *       returns BLOCH_EINVAL when it is forced and not available.
- *   BLOCH_PATH_AUTO (default): FUSED when available and the sequence is excitation-heavy, else PER_BLOCK.
+ *   BLOCH_PATH_AUTO (default): FUSED when available, 4 N_rf >= N_adc and at most 21 x 32 spins per SM (the full set
+ *       of signal warps fits beside the RF warps), else PER_BLOCK.
  * Both paths compute the same thing; the final magnetisation is bitwise identical, the signal differs only in
  * the order of the fixed-order sums.  Set before bloch_plan_workspace_bytes: the workspace size depends on it. */
 enum { BLOCH_PATH_AUTO = 0, BLOCH_PATH_PER_BLOCK = 1, BLOCH_PATH_FUSED = 2 };

@@ -114,8 +114,11 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     q.partial_elems = size_t(q.n_ctas) * size_t(std::max<int64_t>(inf.n_adc, 1));
     if (q.partial_elems * sizeof(float2) > kSeqPartialCapBytes || inf.max_block_adc > INT32_MAX) return q;
     q.ok = true;
-    // AUTO: the fused kernel pays when the excitation dominates (its readout runs on sig_warps warps per SM only)
-    q.use = plan->path == BLOCH_PATH_FUSED || 2 * inf.n_rf_steps >= inf.n_adc;
+    // AUTO: the fused kernel pays when the excitation is a fair share of the work and the full set of signal warps
+    // fits beside the RF warps (its readout runs on sig_warps warps per SM only).  Measured, fused / per-block ms:
+    // N_rf/N_adc = 0.98: 13.1 / 15.5 at 65,536 spins, 42.1 / 29.4 at 131,044 (3 signal warps left);
+    // 0.49: 5.97 / 6.17 at 65,536, 22.2 / 11.3 at 131,072;  0.06: 1.05 / 0.84 at 65,522.
+    q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && q.sig_warps >= want);
     return q;
 }
 

@@ -50,6 +50,9 @@ def test_auto_picks_fused_only_where_it_qualifies(B):
     assert not uses(phase_mode="fp32", output_mode="per_spin")
     assert not uses(n_spins=1_000_000, phase_mode="fp32")          # more than 29 warps of spins per SM
     assert not uses(n_spins=1_000_000, phase_mode="fp32", path="fused")
+    # 131,072 spins = 28 RF warps per SM leave 3 signal warps: allowed when forced, not what AUTO picks
+    assert not uses(n_spins=131_072, phase_mode="fp32")
+    assert uses(n_spins=131_072, phase_mode="fp32", path="fused")
     # readout-heavy sequence (config 1: 50 RF steps, 1024 ADC samples): AUTO stays per-block, FUSED can be forced
     w1 = W.small("1")
     p = B.Plan(w1.seq, phase_mode="fp32")
