@@ -36,7 +36,8 @@ typedef enum {
     BLOCH_ECUDA = -5,          /* a CUDA runtime call failed; text in bloch_last_error() */
     BLOCH_EARCH = -6,          /* current device is not compute capability 10.x */
     BLOCH_ENOTUPLOADED = -7,   /* bloch_simulate before bloch_plan_upload */
-    BLOCH_ENOMEM = -8          /* host allocation failed */
+    BLOCH_ENOMEM = -8,         /* host allocation failed */
+    BLOCH_EHWLIMIT = -9        /* a gradient vertex exceeds scanner G_max, or a segment exceeds S_max (when given) */
 } bloch_status;
 
 enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
@@ -44,7 +45,9 @@ enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1, BLOCH_OUT_GROUPED = 2 };
 enum { BLOCH_MOTION_NONE = 0, BLOCH_MOTION_LINEAR = 1 };
 
 /* Scanner.  Only gamma enters the arithmetic (Eq 1-2, :105-114); B0, G_max, S_max are
- * carried for completeness and are not validated against.  gamma <= 0 selects 2*pi*42.58e6 (:322). */
+ * limits: when G_max [T/m] or S_max [T/m/s] is > 0, bloch_plan_create checks every gradient vertex and every
+ * segment between vertices against it, per axis, and returns BLOCH_EHWLIMIT; 0 = not checked.  B0 is carried
+ * only.  gamma <= 0 selects 2*pi*42.58e6 (:322). */
 typedef struct {
     double gamma;
     double B0;

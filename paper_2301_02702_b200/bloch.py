@@ -127,8 +127,9 @@ def _darr(a):
 
 def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
                       max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
-                      group_size: int = 0) -> int:
-    """seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
+                      group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0) -> int:
+    """G_max [T/m], S_max [T/m/s]: scanner limits the gradient waveforms are checked against when > 0.
+    seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
     Returns the opaque plan handle (an integer address)."""
     keep = []
     cs = bloch_sequence()
@@ -147,7 +148,7 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     cs.rf_n, cs.adc_n, cs.t_end = rt.shape[0], ad.shape[0], float(seq.t_end)
     if dt_rf_max is None:
         dt_rf_max = float(getattr(seq, "dt_rf_max", 0.0))
-    sc = bloch_scanner(float(gamma), 0.0, 0.0, 0.0)
+    sc = bloch_scanner(float(gamma), float(B0), float(G_max), float(S_max))
     pm = _PHASE[phase_mode] if isinstance(phase_mode, str) else int(phase_mode)
     om = _OUT[output_mode] if isinstance(output_mode, str) else int(output_mode)
     mm = _MOTION[motion] if isinstance(motion, str) else int(motion)

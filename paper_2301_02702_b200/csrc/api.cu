@@ -219,6 +219,7 @@ const char *bloch_strerror(int code) {
         case BLOCH_EARCH: return "device is not sm_100";
         case BLOCH_ENOTUPLOADED: return "tables not uploaded";
         case BLOCH_ENOMEM: return "host allocation failed";
+        case BLOCH_EHWLIMIT: return "gradient waveform exceeds the scanner's G_max or S_max";
         default: return "unknown error";
     }
 }

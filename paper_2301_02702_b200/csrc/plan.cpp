@@ -107,6 +107,19 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         if (i > 0 && !(seq->adc_t[i] > seq->adc_t[i - 1] + kTimeTol))
             return fail(BLOCH_ENONMONOTONIC, "ADC times must be strictly ascending");
     }
+    // hardware limits: checked when given (> 0), never part of the arithmetic.  Per axis, between
+    // consecutive vertices; a waveform that starts or ends on a non-zero vertex is not charged for that edge.
+    if (scanner && (scanner->G_max > 0.0 || scanner->S_max > 0.0)) {
+        for (int a = 0; a < 3; ++a)
+            for (int64_t i = 0; i < seq->g_n[a]; ++i) {
+                if (scanner->G_max > 0.0 && std::fabs(seq->g_v[a][i]) > scanner->G_max * (1.0 + 1e-9))
+                    return fail(BLOCH_EHWLIMIT, "gradient amplitude exceeds scanner G_max");
+                if (scanner->S_max > 0.0 && i > 0 &&
+                    std::fabs(seq->g_v[a][i] - seq->g_v[a][i - 1]) >
+                        scanner->S_max * (seq->g_t[a][i] - seq->g_t[a][i - 1]) * (1.0 + 1e-9))
+                    return fail(BLOCH_EHWLIMIT, "gradient slew rate exceeds scanner S_max");
+            }
+    }
     const double dt_rf = (params->dt_rf_max > 0.0 && std::isfinite(params->dt_rf_max))
                              ? params->dt_rf_max : std::numeric_limits<double>::infinity();
 

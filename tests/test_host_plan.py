@@ -141,3 +141,21 @@ def test_motion_plan_refines_like_the_oracle(B, oracle_mod, name, dt_max):
         B.bloch_plan_destroy(h1)
     with pytest.raises(B.BlochError):
         B.bloch_plan_create(w.seq, motion=7)
+
+
+def test_scanner_limits_are_checked_when_given(B):
+    """the scanner carries B0, G_max, S_max; they bound the waveforms, not the arithmetic."""
+    # trapezoid: 30 mT/m reached in 200 us (150 T/m/s), then a 10 us edge of 3000 T/m/s
+    s = seq(g={1: ([1e-3, 1.2e-3, 2e-3, 2.01e-3], [0.0, 30e-3, 30e-3, 0.0])}, adc=[1.5e-3], t_end=3e-3)
+    for kw in ({}, dict(G_max=60e-3, S_max=5000.0), dict(G_max=30e-3), dict(S_max=3000.0)):
+        h = B.bloch_plan_create(s, **kw)       # within limits (equality allowed) or limits not given
+        B.bloch_plan_destroy(h)
+    for kw in (dict(G_max=29e-3), dict(S_max=200.0), dict(G_max=60e-3, S_max=2999.0)):
+        with pytest.raises(B.BlochError) as e:
+            B.bloch_plan_create(s, **kw)
+        assert e.value.code == -9, kw
+    # the generators' own sequences respect the limits they were built for (SURVEY 8(d): 60 mT/m, 200 T/m/s ramps)
+    from paper_2301_02702_b200 import workloads as W
+    for name in ("1", "2", "3"):
+        h = B.bloch_plan_create(W.small(name).seq, G_max=60e-3)
+        B.bloch_plan_destroy(h)
