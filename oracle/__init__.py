@@ -69,7 +69,7 @@ def _seq_args(seq, keep):
 
 def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state: bool = False,
              n_threads: int | None = None, gamma: float = GAMMA, force_excitation: bool = False,
-             velocity=None, dt_max: float = 0.0, group_size: int = 0):
+             velocity=None, dt_max: float = 0.0, group_size: int = 0, coils=None):
     """Step-by-step fp64 Bloch integration (SURVEY.md 8(c) listing).
 
     phantom: object with fp64 arrays x, y, z, M0, T1, T2, dw.   seq: object with g_t, g_v (3 arrays each),
@@ -78,7 +78,25 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     dt_max then refines every interval to at most dt_max (:180).
     Returns complex128 signal [n_adc] ("sum") or [n_spins, n_adc] ("per_spin"); with return_state also
     (Mxy complex128 [n_spins], Mz float64 [n_spins]).
+    coils: optional complex [n_coils, n_spins] receive sensitivities at the spins (output_mode "sum" only):
+    the signal becomes [n_coils, n_adc] (SURVEY.md 8(f) f2 "per-coil weights"; reading C1).
     """
+    if coils is not None:
+        # Reading C1 (the paper has no coils yet, :372 "straightforward to implement"): the standard receive
+        # model S_c(t_j) = sum_i C_c(x_i) Mxy_i(t_j), C_c complex, no conjugation -- by definition the per-spin
+        # signals weighted and added per coil.
+        if output_mode != "sum":
+            raise ValueError("coils need output_mode='sum'")
+        Wc = np.asarray(coils, dtype=np.complex128)
+        n_all = int(np.asarray(phantom.x).shape[0])
+        if Wc.ndim != 2 or Wc.shape[1] != n_all:
+            raise ValueError("coils must be [n_coils, n_spins]")
+        res = simulate(phantom, seq, output_mode="per_spin", state=state, return_state=return_state,
+                       n_threads=n_threads, gamma=gamma, force_excitation=force_excitation, velocity=velocity,
+                       dt_max=dt_max)
+        per = res[0] if return_state else res
+        out = Wc @ per
+        return (out,) + tuple(res[1:]) if return_state else out
     if output_mode == "grouped":
         # SURVEY.md 8(f) f2: S[g][j] = sum of Mxy over the spins of group g (consecutive blocks of group_size
         # spins: an isochromat ensemble per voxel / dictionary entry, PAPER.md:167, :220) -- by definition the
