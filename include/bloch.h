@@ -195,6 +195,21 @@ int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *l
  * of the second-pass reduction; bloch_plan_info.n_launches is the upper bound with one second pass per block). */
 int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
 
+/* Multi-coil receive (SURVEY.md 8(f) f2 "per-coil weights"; PAPER.md:95 "coil sensitivity", :372; reading C1 of
+ * DESIGN.md): S_c(t_n) = sum_i C_c(x_i) Mxy_i(t_n) for n_coils receive coils.
+ *   d_coil    DEVICE, float2 [n_coils][n_spins] row-major: complex sensitivity of coil c at spin i (re, im); borrowed
+ *   d_signal  DEVICE, float2 [n_coils][n_adc] row-major, written
+ *   workspace as bloch_simulate, sized by bloch_plan_workspace_bytes_coils(plan, n_spins, n_coils)
+ * Everything else as bloch_simulate (same integration, same final magnetisation).  The plan must be BLOCH_OUT_SUM_ALL
+ * without motion (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  The coil-independent part of every evaluation (phase,
+ * sin / cos / exp) is computed once per 4 coils.  Asynchronous on `stream`; never allocates. */
+int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out);
+int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                         const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                         const float *d_dw, int n_coils, const float *d_coil, float *d_Mxy, float *d_Mz,
+                         int init_equilibrium, float *d_signal, void *d_workspace, size_t workspace_bytes,
+                         void *stream);
+
 /* Execution path of bloch_simulate for this plan.
  *   BLOCH_PATH_PER_BLOCK: one excitation launch per RF block and one signal launch per precession block.
  *   BLOCH_PATH_FUSED: ONE persistent whole-sequence launch (a CTA per SM owns a chunk of spins for the whole

@@ -54,6 +54,7 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_simulate_motion", "bloch_simulate_host_scratch_bytes", "bloch_simulate_host",
            "bloch_simulate_host_motion", "bloch_plan_set_profiling",
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
+           "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils",
            "bloch_microbench"]
 
 
@@ -80,6 +81,8 @@ def _load():
     mo_args = [vp, i64] + [_fp] * 10 + [_fp, _fp, C.c_int, _fp, vp, sz, vp]
     lib.bloch_simulate_motion.argtypes = mo_args
     lib.bloch_simulate_host_motion.argtypes = mo_args
+    lib.bloch_plan_workspace_bytes_coils.argtypes = [vp, i64, C.c_int, C.POINTER(sz)]
+    lib.bloch_simulate_coils.argtypes = [vp, i64] + [_fp] * 7 + [C.c_int, _fp, _fp, _fp, C.c_int, _fp, vp, sz, vp]
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
@@ -192,6 +195,20 @@ def bloch_simulate_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, 
                                       int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
 
 
+def bloch_plan_workspace_bytes_coils(plan: int, n_spins: int, n_coils: int) -> int:
+    out = C.c_size_t()
+    _check(_lib.bloch_plan_workspace_bytes_coils(plan, n_spins, n_coils, C.byref(out)))
+    return int(out.value)
+
+
+def bloch_simulate_coils(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, n_coils: int, coil, Mxy, Mz,
+                         init_equilibrium: bool, signal, workspace, workspace_bytes: int, stream: int = 0):
+    """bloch_simulate with n_coils receive coils: coil = DEVICE address of float2 [n_coils][n_spins], signal =
+    DEVICE address of float2 [n_coils][n_adc]."""
+    _check(_lib.bloch_simulate_coils(plan, n_spins, x, y, z, M0, T1, T2, dw, n_coils, coil, Mxy, Mz,
+                                     int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
+
+
 def bloch_simulate_host_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
                                init_equilibrium: bool, signal, scratch, scratch_bytes: int, stream: int = 0):
     """bloch_simulate_host with per-spin velocities (raw HOST addresses or None for all three)."""
@@ -292,17 +309,19 @@ class Plan:
         bloch_plan_upload(self.handle, self._tables.data_ptr(), self._tables.numel(), self._stream())
         return self
 
-    def _workspace(self, n):
+    def _workspace(self, n, n_coils=0):
         import torch
-        need = max(bloch_plan_workspace_bytes(self.handle, n), 256)
+        need = max(bloch_plan_workspace_bytes_coils(self.handle, n, n_coils), 256)
         if self._ws is None or self._ws.numel() < need:
             self._ws = torch.empty(need, dtype=torch.uint8, device="cuda")
         return self._ws
 
     def simulate(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None,
-                 velocity=None):
+                 velocity=None, coils=None):
         """Device path: torch float32 CUDA tensors in, complex64 signal tensor out (asynchronous).
-        velocity: optional (vx, vy, vz) float32 CUDA tensors (plan created with motion="linear")."""
+        velocity: optional (vx, vy, vz) float32 CUDA tensors (plan created with motion="linear").
+        coils: optional complex64 CUDA tensor [n_coils, n_spins] of receive sensitivities; the signal is then
+        [n_coils, n_adc] (bloch_simulate_coils)."""
         import torch
         if self._tables is None:
             self.upload()
@@ -311,6 +330,19 @@ class Plan:
             assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
         n_adc = self.info["n_adc"]
         shape = self._signal_shape(n)
+        if coils is not None:
+            assert coils.is_cuda and coils.dtype == torch.complex64 and coils.is_contiguous() and \
+                coils.dim() == 2 and coils.shape[1] == n and velocity is None
+            n_coils = int(coils.shape[0])
+            if signal is None:
+                signal = torch.empty((n_coils, n_adc), dtype=torch.complex64, device="cuda")
+            ws = self._workspace(n, n_coils)
+            bloch_simulate_coils(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(),
+                                 T1.data_ptr(), T2.data_ptr(), dw.data_ptr(), n_coils, coils.data_ptr(),
+                                 None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
+                                 init_equilibrium, signal.data_ptr() if signal.numel() else None,
+                                 ws.data_ptr(), ws.numel(), self._stream())
+            return signal
         if signal is None:
             signal = torch.empty(shape, dtype=torch.complex64, device="cuda")
         ws = self._workspace(n)

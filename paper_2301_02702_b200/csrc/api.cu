@@ -8,6 +8,7 @@
 
 #include "internal.h"
 #include "kernels.cuh"
+#include "coils.cuh"
 #include "rf.cuh"
 #include "seq.cuh"
 #include "signal.cuh"
@@ -122,6 +123,29 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     return q;
 }
 
+// Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
+SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
+    SigShape s;
+    s.P = n_pts >= 2 * kSigThreads ? 2 : 1;
+    s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
+    int64_t chunks = ((int64_t)sm_count * 4 + s.ptiles - 1) / s.ptiles;
+    chunks = std::min<int64_t>(std::max<int64_t>(chunks, 1), std::min<int64_t>((n_spins + 31) / 32, 65535));
+    chunks = std::max<int64_t>(chunks, 1);
+    s.spins_per_chunk = (int)std::max<int64_t>(1, (n_spins + chunks - 1) / chunks);
+    s.chunks = (int)std::max<int64_t>(1, (n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
+    return s;
+}
+
+size_t coil_partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+    size_t worst = 1;
+    for (const Block &b : plan->blocks) {
+        if (b.type != kBlockPrecession || b.adc_count == 0) continue;
+        const SigShape s = coil_shape(b.adc_count, n_spins, sm_count);
+        worst = std::max(worst, size_t(kCoilsPerPass) * size_t(s.chunks) * size_t(b.adc_count));
+    }
+    return worst;
+}
+
 // rows of the signal buffer: 1 (SUM_ALL), n_spins (PER_SPIN), n_spins / group_size (GROUPED)
 size_t signal_rows(const bloch_plan *plan, int64_t n_spins) {
     if (plan->info.output_mode == BLOCH_OUT_PER_SPIN) return size_t(n_spins);
@@ -137,6 +161,7 @@ struct Workspace {
     unsigned *scal;  // device scalars: [0] = max 1/T2 (float bits)
     float2 *partial;
     size_t partial_elems;
+    float2 *W;       // multi-coil receive only: weights repacked as [pass][spin][4]
     size_t bytes;
 };
 
@@ -152,7 +177,7 @@ int sm_count_cached() {
 
 // Layout of the caller's workspace.  sm_count = 148 is used for sizing when no device is present so that
 // bloch_plan_workspace_bytes is a pure host function.
-Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_count) {
+Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_count, int n_coils = 0) {
     Workspace w{};
     w.partial_elems = 0;
     size_t off = 0;
@@ -172,10 +197,13 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
         const SeqShape q = seq_shape(plan, n_spins, sm_count);
-        w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
+        if (n_coils > 0) w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count);
+        else w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
+    const size_t n_pass = size_t((n_coils + kCoilsPerPass - 1) / kCoilsPerPass);
+    w.W = n_coils > 0 ? (float2 *)take(n_pass * size_t(n_spins) * kCoilsPerPass * sizeof(float2)) : nullptr;
     w.bytes = off;
     return w;
 }
@@ -262,7 +290,11 @@ int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out) {
 }
 
 int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out) {
-    if (!plan || !out || n_spins < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative n_spins");
+    return bloch_plan_workspace_bytes_coils(plan, n_spins, 0, out);
+}
+
+int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out) {
+    if (!plan || !out || n_spins < 0 || n_coils < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative size");
     if (n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins exceeds 2^31-1");
     // sized for the larger of the real SM count and 148 so the answer is usable without a device
     int sms = 148;
@@ -273,7 +305,7 @@ int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *
     } else {
         (void)cudaGetLastError();
     }
-    *out = carve(plan, n_spins, nullptr, sms).bytes;
+    *out = carve(plan, n_spins, nullptr, sms, n_coils).bytes;
     return BLOCH_OK;
 }
 
@@ -339,11 +371,48 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins, const float *d_x, co
                                  d_Mz, init_equilibrium, d_signal, d_workspace, workspace_bytes, stream_);
 }
 
+namespace bloch {
+namespace {
+int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                  const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                  const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz,
+                  int n_coils, const float *d_coil,
+                  float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                  void *d_workspace, size_t workspace_bytes, void *stream_);
+}
+}  // namespace bloch
+
 int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
                           const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
                           const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz,
                           float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
                           void *d_workspace, size_t workspace_bytes, void *stream_) {
+    return bloch::simulate_impl(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, d_vx, d_vy, d_vz, 0, nullptr,
+                                d_Mxy, d_Mz, init_equilibrium, d_signal, d_workspace, workspace_bytes, stream_);
+}
+
+int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                         const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                         const float *d_dw, int n_coils, const float *d_coil, float *d_Mxy, float *d_Mz,
+                         int init_equilibrium, float *d_signal, void *d_workspace, size_t workspace_bytes,
+                         void *stream_) {
+    if (!plan) return bloch::fail(BLOCH_EINVAL, "NULL plan");
+    if (n_coils < 1 || n_coils > 4096) return bloch::fail(BLOCH_EINVAL, "n_coils must be in [1, 4096]");
+    if (n_spins > 0 && !d_coil) return bloch::fail(BLOCH_EINVAL, "d_coil is NULL");
+    if (plan->info.output_mode != BLOCH_OUT_SUM_ALL || plan->info.motion_mode != BLOCH_MOTION_NONE)
+        return bloch::fail(BLOCH_EINVAL, "multi-coil receive needs a BLOCH_OUT_SUM_ALL plan without motion");
+    return bloch::simulate_impl(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, nullptr, nullptr, nullptr, n_coils,
+                                d_coil, d_Mxy, d_Mz, init_equilibrium, d_signal, d_workspace, workspace_bytes, stream_);
+}
+
+namespace bloch {
+namespace {
+int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                  const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                  const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz,
+                  int n_coils, const float *d_coil,
+                  float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                  void *d_workspace, size_t workspace_bytes, void *stream_) {
     if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
     const bool has_v = d_vx || d_vy || d_vz;
     if (has_v && !(d_vx && d_vy && d_vz)) return fail(BLOCH_EINVAL, "give all of d_vx, d_vy, d_vz or none");
@@ -369,13 +438,14 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
 
     if (n_spins == 0) {  // degenerate: the sum over no spins is zero
         if (!per_spin && plan->info.n_adc > 0)
-            BLOCH_CUDA(cudaMemsetAsync(d_signal, 0, size_t(plan->info.n_adc) * sizeof(float2), stream));
+            BLOCH_CUDA(cudaMemsetAsync(d_signal, 0, size_t(std::max(n_coils, 1)) * size_t(plan->info.n_adc) * sizeof(float2),
+                                       stream));
         return BLOCH_OK;
     }
     if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) != 0)
         return fail(BLOCH_EWORKSPACE, "workspace NULL or not 256-B aligned");
-    const Workspace w = carve(plan, n_spins, d_workspace, sms);
-    if (workspace_bytes < w.bytes) return fail(BLOCH_EWORKSPACE, "workspace too small; see bloch_plan_workspace_bytes");
+    const Workspace w = carve(plan, n_spins, d_workspace, sms, n_coils);
+    if (workspace_bytes < w.bytes) return fail(BLOCH_EWORKSPACE, "workspace too small; see bloch_plan_workspace_bytes[_coils]");
 
     const int n = (int)n_spins;
     Taps taps{plan, stream};
@@ -386,8 +456,14 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
+    const int n_pass = (n_coils + kCoilsPerPass - 1) / kCoilsPerPass;
+    if (n_coils > 0) {
+        pack_coils_kernel<<<dim3((n + 255) / 256, n_pass), 256, 0, stream>>>(n, n_coils, (const float2 *)d_coil, w.W);
+        ++launches;
+    }
 
-    const SeqShape sq = seq_shape(plan, n_spins, sms);
+    SeqShape sq = seq_shape(plan, n_spins, sms);
+    if (n_coils > 0) sq.use = false;  // multi-coil receive runs on the per-block path
     if (plan->path == BLOCH_PATH_FUSED && !sq.ok)
         return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output, fp32 phase, no motion and <= 29 x 32 spins per SM");
     if (sq.ok && sq.use) {
@@ -479,6 +555,26 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
                                                                     (long long)plan->info.n_adc, (long long)b.adc_first,
                                                                     (float2 *)d_signal);
                 ++launches;
+            } else if (n_coils > 0) {
+                const SigShape s = coil_shape(n_pts, n, sms);
+                const dim3 grid(s.ptiles, s.chunks);
+                for (int pass = 0; pass < n_pass; ++pass) {
+                    const float4 *Wp = reinterpret_cast<const float4 *>(w.W + (size_t)pass * n * kCoilsPerPass);
+                    const int in_pass = std::min(kCoilsPerPass, n_coils - pass * kCoilsPerPass);
+                    if (pass > 0 && (rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
+#define BLOCH_LAUNCH_COIL(PP, H, AP)                                                                           \
+    signal_coils_kernel<PP, H><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk, \
+                                                                 (const float *)w.scal, w.partial)
+                    if (s.P == 2) { if (ph64) BLOCH_LAUNCH_COIL(2, true, w.Ad); else BLOCH_LAUNCH_COIL(2, false, w.A); }
+                    else { if (ph64) BLOCH_LAUNCH_COIL(1, true, w.Ad); else BLOCH_LAUNCH_COIL(1, false, w.A); }
+#undef BLOCH_LAUNCH_COIL
+                    if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
+                    reduce_coils_kernel<<<dim3((unsigned)((n_pts + 31) / 32), in_pass), dim3(32, 8), 0, stream>>>(
+                        w.partial, s.chunks, n_pts,
+                        (float2 *)d_signal + (size_t)pass * kCoilsPerPass * (size_t)plan->info.n_adc + b.adc_first,
+                        (long long)plan->info.n_adc);
+                    launches += 2;
+                }
             } else {
                 const SigShape s = sig_shape(n_pts, n, sms);
                 if (!batch_open) {  // look ahead: how many of the following blocks share this batch
@@ -550,6 +646,8 @@ int bloch_simulate_motion(const bloch_plan *plan, int64_t n_spins, const float *
     BLOCH_CUDA(cudaGetLastError());
     return BLOCH_OK;
 }
+}  // namespace
+}  // namespace bloch
 
 int bloch_simulate_host_scratch_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out) {
     if (!plan || !out || n_spins < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative n_spins");

@@ -1,0 +1,111 @@
+"""Multi-coil receive on the GPU (bloch_simulate_coils; SURVEY.md 8(f) f2 "per-coil weights", reading C1) against the
+oracle (pytest -m gpu).  Same acceptance as test_gpu_parity.py, per coil and normalised by the largest coil signal."""
+import numpy as np
+import pytest
+
+from paper_2301_02702_b200 import workloads as W
+from test_gpu_parity import B, assert_parity, errors  # noqa: F401  (B is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def coil_maps(ph, n_coils, seed=0):
+    """Smooth synthetic sensitivities: coils on a ring of radius 0.15 m, magnitude ~ 1/(d^2 + r0^2), phase = angle
+    towards the coil (a Biot-Savart-like stand-in; values only need to be smooth, complex and different per coil)."""
+    rng = np.random.default_rng(seed)
+    ang = 2 * np.pi * (np.arange(n_coils) + rng.uniform(0, 1)) / n_coils
+    cx, cy = 0.15 * np.cos(ang), 0.15 * np.sin(ang)
+    dx, dy = ph.x[None, :] - cx[:, None], ph.y[None, :] - cy[:, None]
+    mag = 0.01 / (dx * dx + dy * dy + 0.01)
+    w = mag * np.exp(1j * np.arctan2(dy, dx))
+    return w.astype(np.complex64)
+
+
+def run_coils(B, w, coils, want_state=False, **kw):
+    import torch
+    plan = B.Plan(w.seq, phase_mode=kw.pop("phase_mode", w.phase_mode), output_mode="sum", **kw)
+    dev = B.phantom_to_device(w.phantom)
+    n = w.phantom.n
+    Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda") if want_state else None
+    Mz = torch.zeros(n, dtype=torch.float32, device="cuda") if want_state else None
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, coils=torch.from_numpy(np.ascontiguousarray(coils)).cuda())
+    torch.cuda.synchronize()
+    out = sig.cpu().numpy()
+    launches = B.bloch_plan_last_launches(plan.handle)
+    plan.close()
+    if want_state:
+        m = Mxy.cpu().numpy()
+        return out, m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy(), launches
+    return out
+
+
+@pytest.mark.parametrize("name,n_coils,phase", [("1", 1, "fp32"), ("1", 4, "fp32"), ("2", 3, "fp32"), ("3", 8, "fp64"),
+                                               ("4", 5, "fp32"), ("5", 2, "fp32")])
+def test_small_configs_with_coils_match_oracle(B, oracle_mod, name, n_coils, phase):
+    w = W.small(name)
+    coils = coil_maps(w.phantom, n_coils, seed=n_coils)
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
+    got, gxy, gz, _ = run_coils(B, w, coils, want_state=True, phase_mode=phase)
+    assert got.shape == ref.shape == (n_coils, w.seq.adc_t.size)
+    assert_parity(got, ref, f"config {name}, {n_coils} coils")
+    for c in range(n_coils):   # every coil on its own scale as well
+        emax, nrmse = errors(got[c], ref[c])
+        assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
+    assert_parity(np.concatenate([gxy, gz.astype(np.complex128)]), np.concatenate([rxy, rz.astype(np.complex128)]),
+                  "final state with coils")
+
+
+def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
+    """One coil with weight 1 everywhere returns the plain signal; 9 coils (three passes of 4, the last with one
+    coil) give the same rows as the same coils simulated in separate calls, bitwise."""
+    from test_gpu_parity import run_gpu
+    w = W.small("4")
+    n = w.phantom.n
+    plain = run_gpu(B, w, path="per_block")
+    one = run_coils(B, w, np.ones((1, n), dtype=np.complex64))
+    emax, _ = errors(one[0], plain)
+    assert emax < 2e-6, f"uniform coil vs plain: {emax:.3e}"
+    coils = coil_maps(w.phantom, 9, seed=4)
+    all9 = run_coils(B, w, coils)
+    again = run_coils(B, w, coils)
+    assert np.array_equal(all9.view(np.float32), again.view(np.float32)), "run-to-run not bitwise identical"
+    first4 = run_coils(B, w, coils[:4])
+    last1 = run_coils(B, w, coils[8:9])
+    assert np.array_equal(all9[:4].view(np.float32), first4.view(np.float32))
+    assert np.array_equal(all9[8:9].view(np.float32), last1.view(np.float32))
+
+
+def test_coil_argument_errors_and_edge_cases(B):
+    import torch
+    w = W.small("1")
+    n = w.phantom.n
+    dev = B.phantom_to_device(w.phantom)
+    coils = torch.ones(2, n, dtype=torch.complex64, device="cuda")
+    for kw in (dict(output_mode="per_spin"), dict(motion="linear", dt_max=1e-4)):
+        plan = B.Plan(w.seq, **kw)
+        ws = torch.empty(1 << 24, dtype=torch.uint8, device="cuda")
+        sig = torch.empty(2, plan.info["n_adc"], dtype=torch.complex64, device="cuda")
+        plan.upload()
+        with pytest.raises(B.BlochError) as e:
+            B.bloch_simulate_coils(plan.handle, n, *[t.data_ptr() for t in dev], 2, coils.data_ptr(), None, None, True,
+                                   sig.data_ptr(), ws.data_ptr(), ws.numel())
+        assert e.value.code == -1
+        plan.close()
+    plan = B.Plan(w.seq).upload()
+    ws = torch.empty(1 << 24, dtype=torch.uint8, device="cuda")
+    sig = torch.empty(2, plan.info["n_adc"], dtype=torch.complex64, device="cuda")
+    with pytest.raises(B.BlochError):      # n_coils = 0
+        B.bloch_simulate_coils(plan.handle, n, *[t.data_ptr() for t in dev], 0, coils.data_ptr(), None, None, True,
+                               sig.data_ptr(), ws.data_ptr(), ws.numel())
+    with pytest.raises(B.BlochError) as e:  # workspace sized without the coils
+        small = B.bloch_plan_workspace_bytes(plan.handle, n)
+        assert B.bloch_plan_workspace_bytes_coils(plan.handle, n, 2) > small
+        B.bloch_simulate_coils(plan.handle, n, *[t.data_ptr() for t in dev], 2, coils.data_ptr(), None, None, True,
+                               sig.data_ptr(), ws.data_ptr(), small)
+    assert e.value.code == -4
+    # zero spins: every coil's empty sum
+    z = torch.zeros(0, dtype=torch.float32, device="cuda")
+    out = plan.simulate(z, z, z, z, z, z, z, coils=torch.zeros(3, 0, dtype=torch.complex64, device="cuda"))
+    torch.cuda.synchronize()
+    assert out.shape == (3, plan.info["n_adc"]) and float(out.abs().max()) == 0.0
+    plan.close()
