@@ -124,17 +124,18 @@ def oracle_sample(w, budget_spin_steps: float, n_intervals: int):
     else:
         idx = np.linspace(0, n - 1, take).astype(np.int64)
     vel = None if w.velocity is None else tuple(np.ascontiguousarray(a[idx]) for a in w.velocity)
-    return w.phantom.subset(idx), take, vel
+    coils = None if w.coils is None else np.ascontiguousarray(w.coils[:, idx]).astype(np.complex128)
+    return w.phantom.subset(idx), take, vel, coils
 
 
 def time_oracle(w, n_intervals: int, budget_spin_steps: float):
     import oracle
     oracle.build()
     cores = os.cpu_count() or 1
-    ph, take, vel = oracle_sample(w, budget_spin_steps, n_intervals)
+    ph, take, vel, coils = oracle_sample(w, budget_spin_steps, n_intervals)
     t0 = time.perf_counter()
     oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max,
-                    group_size=w.group_size)
+                    group_size=w.group_size, coils=coils)
     dt = time.perf_counter() - t0
     return {"value": take * n_intervals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{take} of {w.phantom.n} spins (evenly spaced), full sequence ({n_intervals} intervals), "
@@ -204,7 +205,8 @@ def run_ours(args, rank, local_rank, world):
         torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
     Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda")
     Mz = torch.zeros(n, dtype=torch.float32, device="cuda")
-    shape = plan._signal_shape(n)
+    coils = None if w.coils is None else torch.from_numpy(np.ascontiguousarray(w.coils)).cuda()
+    shape = plan._signal_shape(n) if coils is None else (int(coils.shape[0]), info["n_adc"])
     sig = torch.empty(shape, dtype=torch.complex64, device="cuda")
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -214,7 +216,7 @@ def run_ours(args, rank, local_rank, world):
         torch.cuda.synchronize()
 
     def step():
-        plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig, velocity=vel)
+        plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig, velocity=vel, coils=coils)
         if not per_spin:
             reduce_signal(sig)
 
@@ -270,11 +272,24 @@ def run_ours(args, rank, local_rank, world):
     if w.velocity is not None:
         pinned_v = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory() for a in w.velocity]
         h_vel = [p.numpy() for p in pinned_v]
-    plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel)   # warm-up (allocates the scratch)
+    h_coils = None if w.coils is None else torch.from_numpy(np.ascontiguousarray(w.coils)).pin_memory()
+
+    def e2e_step():
+        if h_coils is None:
+            plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel)   # synchronous: returns after the D2H copy
+            return
+        # multi-coil receive has no host-buffer entry: the same copies around the device entry
+        d = [p.cuda(non_blocking=True) for p in pinned]
+        dc = h_coils.cuda(non_blocking=True)
+        out = plan.simulate(*d, coils=dc)
+        h_sig.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()   # warm-up (allocates the scratch)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel)   # synchronous: returns after the D2H copy
+        e2e_step()
         if not per_spin and world > 1:
             reduce_signal(torch.from_numpy(h_sig_np).cuda())
     barrier()
@@ -282,7 +297,8 @@ def run_ours(args, rank, local_rank, world):
     if world > 1:
         dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
     e2e_value = spin_steps * world * e2e_steps / float(e2e_s.item())
-    h2d = sum(int(a.nbytes) for a in h_arrs) + (sum(int(a.nbytes) for a in h_vel) if h_vel else 0)
+    h2d = sum(int(a.nbytes) for a in h_arrs) + (sum(int(a.nbytes) for a in h_vel) if h_vel else 0) + \
+        (int(h_coils.numel()) * 8 if h_coils is not None else 0)
     d2h = int(h_sig_np.nbytes)
 
     if rank != 0:
@@ -292,6 +308,8 @@ def run_ours(args, rank, local_rank, world):
     mufu_peak = SM_COUNT * 16 * sm_max * 1e6          # MUFU ops/s
     fp32_peak = SM_COUNT * 128 * sm_max * 1e6         # FP32 instr/s
     n_eval_sig = float(n) * float(info["n_adc"])      # evaluations in the signal kernels per step
+    n_coils = 0 if coils is None else int(coils.shape[0])
+    n_pass = max(1, (n_coils + 3) // 4)               # the coil kernel evaluates sin / cos / ex2 once per 4 coils
     rf_steps = float(n) * float(info["n_rf_steps"])
     kern = {}
     if kinds_n["signal"]:
@@ -301,12 +319,25 @@ def run_ours(args, rank, local_rank, world):
                           "unit": "Tmufu-op/s", "frac": ach / mufu_peak,
                           "traffic": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[0],
                           "traffic_source": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[1],
+                          "coils": n_coils,
                           "note": "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample), SURVEY.md 8(d); "
                                   "the kernel issues 2 + 1/P (P = 4 adjacent samples share one ex2), so frac can "
                                   "reach 3 / 2.25 = 1.33 at a saturated MUFU pipe",
                           "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
                           "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
                           "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}
+    if kinds_n["signal"] and n_coils > 0:
+        # multi-coil receive: sin / cos / ex2 are coil-independent (3 MUFU per evaluation whatever the number of
+        # coils); every coil adds one complex multiply-accumulate = 4 FP32 instructions per evaluation
+        dur = kinds_ms["signal"] * 1e-3 / args.steps
+        fp32_ops = (FP32_PER_EVAL + 4 * n_coils) * n_eval_sig
+        if fp32_ops / fp32_peak > MUFU_PER_EVAL * n_eval_sig / mufu_peak:
+            kern["signal"].update({"pipe": "fp32", "achieved": fp32_ops / dur / 1e12, "peak": fp32_peak / 1e12,
+                                   "unit": "Tfp32-instr/s", "frac": fp32_ops / dur / fp32_peak,
+                                   "algorithmic_ops_per_launch": fp32_ops * args.steps / kinds_n["signal"],
+                                   "note": f"signal_coils_kernel, {n_coils} coils: algorithmic count = 15 + 4 x n_coils FP32 "
+                                           "instructions per (spin, ADC sample) (SURVEY.md 8(d) + one complex MAC per coil); "
+                                           "the 3 MUFU per evaluation are shared by all coils and are the smaller term"})
     if kinds_n["rf"]:
         dur = kinds_ms["rf"] * 1e-3 / args.steps
         ach = FP32_PER_RF_STEP * rf_steps / dur
@@ -348,14 +379,15 @@ def run_ours(args, rank, local_rank, world):
            "data": "synthetic",
            "config": {"workload": w.name, "n_spins_per_gpu": n, "n_intervals": n_int,
                       "n_rf_steps": info["n_rf_steps"], "n_adc": info["n_adc"], "n_blocks": info["n_blocks"],
-                      "output_mode": w.output_mode, "motion": w.velocity is not None,
+                      "output_mode": w.output_mode, "motion": w.velocity is not None, "coils": n_coils,
                       "path": "fused" if bloch.bloch_plan_uses_fused(plan.handle, n) else "per_block", "spin_steps_per_step": spin_steps * world,
                       "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
                       "plan_create_upload_s": plan_s},
            "sim_wall_time_s": ms_total / args.steps * 1e-3,
            "clocks": clocks.summary(),
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                   "steps": e2e_steps, "api": "bloch_simulate_host (pinned host buffers)"},
+                   "steps": e2e_steps, "api": "bloch_simulate_host (pinned host buffers)" if h_coils is None else
+                          "Plan.simulate(coils=) with pinned-host H2D / D2H copies around it"},
            "gpu_launches": bloch.bloch_plan_last_launches(plan.handle) * args.steps,
            "ms_per_step_with_kernel_events": (ms_pass.get(True, 0.0) / args.steps) or None,
            "roofline": roofline,
@@ -377,7 +409,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 5, 5b, 5c (ensemble dictionary)")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 5, 5b, 5c (ensemble dictionary)")
     ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
                     help="execution path (bloch_plan_set_path); auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")

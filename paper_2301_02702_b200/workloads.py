@@ -16,6 +16,8 @@ from __future__ import annotations
 import math
 from dataclasses import dataclass, field
 
+import dataclasses
+
 import numpy as np
 
 GAMMA = 2.0 * math.pi * 42.58e6  # rad/s/T   (PAPER.md:322 -> 0.267538 rad/us/mT)
@@ -72,6 +74,7 @@ class Workload:
     velocity: tuple | None = None  # (vx, vy, vz) fp32-exact arrays [m/s]: x(t) = x + v t
     dt_max: float = 0.0            # spacing of the intermediate points needed with motion
     group_size: int = 0            # output_mode "grouped": spins per group
+    coils: np.ndarray | None = None  # complex64 [n_coils, n_spins] receive sensitivities (reading C1)
 
     @property
     def plan_kw(self) -> dict:
@@ -471,8 +474,26 @@ def config3m(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, vy: float = 
     return Workload("config3m_brain_epi128_motion", ph, w.seq, phase_mode="fp64", velocity=vel, dt_max=dt_max)
 
 
+def coil_maps(ph: Phantom, n_coils: int, radius: float = 0.15, seed: int = 0) -> np.ndarray:
+    """Smooth synthetic receive sensitivities, complex64 [n_coils, n_spins]: coils on a ring of `radius` around the
+    z axis, magnitude r0^2 / (d^2 + r0^2) with d the in-plane distance to the coil and r0 = 0.1 m, phase = the angle
+    from the coil to the spin (a Biot-Savart-like stand-in for measured maps, which are not in this container)."""
+    rng = np.random.default_rng(SEED0 + 40 + seed)
+    ang = 2 * np.pi * (np.arange(n_coils) + rng.uniform(0, 1)) / n_coils
+    cx, cy = radius * np.cos(ang), radius * np.sin(ang)
+    dx, dy = ph.x[None, :] - cx[:, None], ph.y[None, :] - cy[:, None]
+    w = 0.01 / (dx * dx + dy * dy + 0.01) * np.exp(1j * np.arctan2(dy, dx))
+    return w.astype(np.complex64)
+
+
+def config4c(n_coils: int = 8, **kw) -> Workload:
+    """Config 4 received by 8 coils (SURVEY.md 8(f) f2 "per-coil weights"): output 8 x 65,536 complex."""
+    w = config4(**kw)
+    return dataclasses.replace(w, name=f"config4c_1M_spiral_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
+
+
 CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b,
-           "5c": config5c}
+           "5c": config5c, "4c": config4c}
 
 
 def make(name: str, **kw) -> Workload:

@@ -10,15 +10,7 @@ pytestmark = pytest.mark.gpu
 
 
 def coil_maps(ph, n_coils, seed=0):
-    """Smooth synthetic sensitivities: coils on a ring of radius 0.15 m, magnitude ~ 1/(d^2 + r0^2), phase = angle
-    towards the coil (a Biot-Savart-like stand-in; values only need to be smooth, complex and different per coil)."""
-    rng = np.random.default_rng(seed)
-    ang = 2 * np.pi * (np.arange(n_coils) + rng.uniform(0, 1)) / n_coils
-    cx, cy = 0.15 * np.cos(ang), 0.15 * np.sin(ang)
-    dx, dy = ph.x[None, :] - cx[:, None], ph.y[None, :] - cy[:, None]
-    mag = 0.01 / (dx * dx + dy * dy + 0.01)
-    w = mag * np.exp(1j * np.arctan2(dy, dx))
-    return w.astype(np.complex64)
+    return W.coil_maps(ph, n_coils, seed=seed)
 
 
 def run_coils(B, w, coils, want_state=False, **kw):
