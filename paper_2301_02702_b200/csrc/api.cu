@@ -124,11 +124,12 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 }
 
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
-SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
+SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp) {
     SigShape s;
     s.P = n_pts >= 2 * kSigThreads ? 2 : 1;
     s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
-    int64_t chunks = ((int64_t)sm_count * 4 + s.ptiles - 1) / s.ptiles;
+    const int per_sm = ncp == 8 ? 2 : 4;  // resident CTAs per SM (96 / 64 registers)
+    int64_t chunks = ((int64_t)sm_count * per_sm + s.ptiles - 1) / s.ptiles;
     chunks = std::min<int64_t>(std::max<int64_t>(chunks, 1), std::min<int64_t>((n_spins + 31) / 32, 65535));
     chunks = std::max<int64_t>(chunks, 1);
     s.spins_per_chunk = (int)std::max<int64_t>(1, (n_spins + chunks - 1) / chunks);
@@ -136,12 +137,12 @@ SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
     return s;
 }
 
-size_t coil_partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+size_t coil_partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count, int ncp) {
     size_t worst = 1;
     for (const Block &b : plan->blocks) {
         if (b.type != kBlockPrecession || b.adc_count == 0) continue;
-        const SigShape s = coil_shape(b.adc_count, n_spins, sm_count);
-        worst = std::max(worst, size_t(kCoilsPerPass) * size_t(s.chunks) * size_t(b.adc_count));
+        const SigShape s = coil_shape(b.adc_count, n_spins, sm_count, ncp);
+        worst = std::max(worst, size_t(ncp) * size_t(s.chunks) * size_t(b.adc_count));
     }
     return worst;
 }
@@ -197,13 +198,14 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
         const SeqShape q = seq_shape(plan, n_spins, sm_count);
-        if (n_coils > 0) w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count);
+        if (n_coils > 0) w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, coils_per_pass(n_coils));
         else w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
-    const size_t n_pass = size_t((n_coils + kCoilsPerPass - 1) / kCoilsPerPass);
-    w.W = n_coils > 0 ? (float2 *)take(n_pass * size_t(n_spins) * kCoilsPerPass * sizeof(float2)) : nullptr;
+    const int ncp = coils_per_pass(n_coils);
+    const size_t n_pass = size_t((n_coils + ncp - 1) / ncp);
+    w.W = n_coils > 0 ? (float2 *)take(n_pass * size_t(n_spins) * ncp * sizeof(float2)) : nullptr;
     w.bytes = off;
     return w;
 }
@@ -456,9 +458,10 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
-    const int n_pass = (n_coils + kCoilsPerPass - 1) / kCoilsPerPass;
+    const int ncp = coils_per_pass(n_coils);
+    const int n_pass = (n_coils + ncp - 1) / ncp;
     if (n_coils > 0) {
-        pack_coils_kernel<<<dim3((n + 255) / 256, n_pass), 256, 0, stream>>>(n, n_coils, (const float2 *)d_coil, w.W);
+        pack_coils_kernel<<<dim3((n + 255) / 256, n_pass), 256, 0, stream>>>(n, n_coils, ncp, (const float2 *)d_coil, w.W);
         ++launches;
     }
 
@@ -556,22 +559,28 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                                     (float2 *)d_signal);
                 ++launches;
             } else if (n_coils > 0) {
-                const SigShape s = coil_shape(n_pts, n, sms);
+                const SigShape s = coil_shape(n_pts, n, sms, ncp);
                 const dim3 grid(s.ptiles, s.chunks);
                 for (int pass = 0; pass < n_pass; ++pass) {
-                    const float4 *Wp = reinterpret_cast<const float4 *>(w.W + (size_t)pass * n * kCoilsPerPass);
-                    const int in_pass = std::min(kCoilsPerPass, n_coils - pass * kCoilsPerPass);
+                    const float4 *Wp = reinterpret_cast<const float4 *>(w.W + (size_t)pass * n * ncp);
+                    const int in_pass = std::min(ncp, n_coils - pass * ncp);
                     if (pass > 0 && (rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
-#define BLOCH_LAUNCH_COIL(PP, H, AP)                                                                           \
-    signal_coils_kernel<PP, H><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk, \
-                                                                 (const float *)w.scal, w.partial)
-                    if (s.P == 2) { if (ph64) BLOCH_LAUNCH_COIL(2, true, w.Ad); else BLOCH_LAUNCH_COIL(2, false, w.A); }
-                    else { if (ph64) BLOCH_LAUNCH_COIL(1, true, w.Ad); else BLOCH_LAUNCH_COIL(1, false, w.A); }
+#define BLOCH_LAUNCH_COIL(PP, NCC, H, AP)                                                                           \
+    signal_coils_kernel<PP, NCC, H><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk, \
+                                                                      (const float *)w.scal, w.partial)
+#define BLOCH_LAUNCH_COIL2(PP, NCC)                                \
+    do {                                                           \
+        if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, w.Ad);          \
+        else BLOCH_LAUNCH_COIL(PP, NCC, false, w.A);               \
+    } while (0)
+                    if (ncp == 8) { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 8); else BLOCH_LAUNCH_COIL2(1, 8); }
+                    else { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 4); else BLOCH_LAUNCH_COIL2(1, 4); }
+#undef BLOCH_LAUNCH_COIL2
 #undef BLOCH_LAUNCH_COIL
                     if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
                     reduce_coils_kernel<<<dim3((unsigned)((n_pts + 31) / 32), in_pass), dim3(32, 8), 0, stream>>>(
                         w.partial, s.chunks, n_pts,
-                        (float2 *)d_signal + (size_t)pass * kCoilsPerPass * (size_t)plan->info.n_adc + b.adc_first,
+                        (float2 *)d_signal + (size_t)pass * ncp * (size_t)plan->info.n_adc + b.adc_first,
                         (long long)plan->info.n_adc);
                     launches += 2;
                 }

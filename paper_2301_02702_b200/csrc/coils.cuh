@@ -3,11 +3,12 @@
 //
 // The expensive part of an evaluation -- the phase, MUFU sin / cos / ex2, the decay -- does not depend on the
 // coil, so one kernel evaluates c_in = Mxy_i(0) exp(-tau_n/T2_i) exp(i theta_in) ONCE (arithmetic of
-// signal_kernel, signal.cuh) and accumulates it into kCoilsPerPass = 4 coil sums with 4 FMA per coil: an extra
-// coil costs 4 FMA-pipe instructions per evaluation instead of a second pass of 18.  More than 4 coils take
-// ceil(n_coils / 4) passes over the block.  The weights are repacked once per simulation into one 32-B record
-// (4 x float2) per spin per pass so that a spin tile's weights arrive by ONE bulk copy (TMA) next to its position
-// and state tiles; unused slots of the last pass hold zeros.  Partials P[coil][chunk][point], second pass in
+// signal_kernel, signal.cuh) and accumulates it into NC coil sums with 4 FMA per coil: an extra coil costs 4
+// FMA-pipe instructions per evaluation instead of a second pass of 18.  NC = 4 coils per pass for up to 4 coils,
+// 8 beyond (the shared part is then amortised over twice the coils; 96 registers, 2 CTAs per SM); more coils take
+// ceil(n_coils / NC) passes over the block.  The weights are repacked once per simulation into one record of NC
+// float2 per spin per pass so that a spin tile's weights arrive by ONE bulk copy (TMA) next to its position and
+// state tiles; unused slots of the last pass hold zeros.  Partials P[coil][chunk][point], second pass in
 // chunk order (no float atomics, bitwise reproducible), as a7.
 #pragma once
 #include <type_traits>
@@ -19,52 +20,53 @@
 
 namespace bloch {
 
-constexpr int kCoilsPerPass = 4;
+constexpr int kCoilsPerPassMax = 8;
+__host__ __device__ inline int coils_per_pass(int n_coils) { return n_coils > 4 ? 8 : 4; }
 
-// caller layout coil[c][i] (float2) -> W[pass][i][k] (float2), k = c - 4 pass
+// caller layout coil[c][i] (float2) -> W[pass][i][k] (float2), k = c - ncp pass
 __global__ void __launch_bounds__(256)
-pack_coils_kernel(int n, int n_coils, const float2 *__restrict__ coil, float2 *__restrict__ W) {
+pack_coils_kernel(int n, int n_coils, int ncp, const float2 *__restrict__ coil, float2 *__restrict__ W) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int pass = blockIdx.y;
     if (i >= n) return;
-    float2 w[kCoilsPerPass];
-#pragma unroll
-    for (int k = 0; k < kCoilsPerPass; ++k) {
-        const int c = pass * kCoilsPerPass + k;
-        w[k] = c < n_coils ? coil[(size_t)c * n + i] : make_float2(0.f, 0.f);
+    float4 *dst = reinterpret_cast<float4 *>(W + ((size_t)pass * n + i) * ncp);
+    for (int k = 0; k < ncp; k += 2) {
+        const int c = pass * ncp + k;
+        const float2 a = c < n_coils ? coil[(size_t)c * n + i] : make_float2(0.f, 0.f);
+        const float2 b = c + 1 < n_coils ? coil[(size_t)(c + 1) * n + i] : make_float2(0.f, 0.f);
+        dst[k / 2] = make_float4(a.x, a.y, b.x, b.y);
     }
-    float4 *dst = reinterpret_cast<float4 *>(W + ((size_t)pass * n + i) * kCoilsPerPass);
-    dst[0] = make_float4(w[0].x, w[0].y, w[1].x, w[1].y);
-    dst[1] = make_float4(w[2].x, w[2].y, w[3].x, w[3].y);
 }
 
-template <int P, bool PH64>
-__global__ void __launch_bounds__(kSigThreads)
+template <int P, int NC, bool PH64>
+__global__ void __launch_bounds__(kSigThreads, NC == 8 ? 2 : 4)
 signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
-                    const float4 *__restrict__ S, const float4 *__restrict__ W /* this pass: 2 float4 per spin */,
+                    const float4 *__restrict__ S, const float4 *__restrict__ W /* this pass: NC / 2 float4 per spin */,
                     int n_spins, int spins_per_chunk, const float *__restrict__ scal,
-                    float2 *__restrict__ partial /* [4][chunks][n_pts] */) {
+                    float2 *__restrict__ partial /* [NC][chunks][n_pts] */) {
     using RecT = typename std::conditional<PH64, double4, float4>::type;
     using PosT = typename std::conditional<PH64, double4, float4>::type;
     using real = typename std::conditional<PH64, double, float>::type;
-    __shared__ __align__(128) PosT shA[2][kSigTile];
-    __shared__ __align__(128) float4 shS[2][kSigTile];
-    __shared__ __align__(128) float4 shW[2][2 * kSigTile];
+    constexpr int TILE = NC == 8 ? 128 : kSigTile;  // spins per staged tile (static shared memory stays < 48 KB)
+    __shared__ __align__(128) PosT shA[2][TILE];
+    __shared__ __align__(128) float4 shS[2][TILE];
+    constexpr int WQ = NC / 2;  // float4 per spin
+    __shared__ __align__(128) float4 shW[2][WQ * TILE];
     __shared__ __align__(8) uint64_t bar[2];
     const RecT *recs = reinterpret_cast<const RecT *>(recs_);
     const PosT *A = reinterpret_cast<const PosT *>(A_);
     const int tid = threadIdx.x;
     const int s0 = blockIdx.y * spins_per_chunk;
     const int s1 = min(n_spins, s0 + spins_per_chunk);
-    const int n_tiles = (s1 - s0 + kSigTile - 1) / kSigTile;
+    const int n_tiles = (s1 - s0 + TILE - 1) / TILE;
     auto issue = [&](int t) {
         const int b = t & 1;
-        const int base = s0 + t * kSigTile;
-        const uint32_t cnt = (uint32_t)min(kSigTile, s1 - base);
-        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + 3 * sizeof(float4)));
+        const int base = s0 + t * TILE;
+        const uint32_t cnt = (uint32_t)min(TILE, s1 - base);
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + (1 + WQ) * sizeof(float4)));
         bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
         bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
-        bulk_g2s(shW[b], W + 2 * (size_t)base, cnt * (uint32_t)(2 * sizeof(float4)), &bar[b]);
+        bulk_g2s(shW[b], W + WQ * (size_t)base, cnt * (uint32_t)(WQ * sizeof(float4)), &bar[b]);
     };
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -75,7 +77,7 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
     }
     const int p0 = (blockIdx.x * kSigThreads + tid) * P;
     real kx[P], ky[P], kz[P], tau[P];
-    float tf[P], cj[P], ar[kCoilsPerPass][P], ai[kCoilsPerPass][P];
+    float tf[P], cj[P], ar[NC][P], ai[NC][P];
     float cmax = 0.f;
 #pragma unroll
     for (int j = 0; j < P; ++j) {
@@ -88,21 +90,24 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         cj[j] = (float)(r.w - tau[0]) * 0.6931471805599453f;
         cmax = fmaxf(cmax, fabsf(cj[j]));
 #pragma unroll
-        for (int k = 0; k < kCoilsPerPass; ++k) { ar[k][j] = 0.f; ai[k][j] = 0.f; }
+        for (int k = 0; k < NC; ++k) { ar[k][j] = 0.f; ai[k][j] = 0.f; }
     }
     const bool series = P > 1 && __all_sync(0xffffffffu, cmax * (scal[0] * kLog2e) <= 0.02f);
     __syncthreads();  // barrier initialisation visible to every waiter
     for (int t = 0; t < n_tiles; ++t) {
         const int b = t & 1;
         mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
-        const int cnt = min(kSigTile, s1 - (s0 + t * kSigTile));
+        const int cnt = min(TILE, s1 - (s0 + t * TILE));
 #pragma unroll 2
         for (int s = 0; s < cnt; ++s) {
             const PosT a = shA[b][s];
             const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
-            const float4 w01 = shW[b][2 * s], w23 = shW[b][2 * s + 1];
-            const float wr[kCoilsPerPass] = {w01.x, w01.z, w23.x, w23.z};
-            const float wi[kCoilsPerPass] = {w01.y, w01.w, w23.y, w23.w};
+            float wr[NC], wi[NC];
+#pragma unroll
+            for (int q = 0; q < WQ; ++q) {
+                const float4 w2 = shW[b][WQ * s + q];
+                wr[2 * q] = w2.x; wi[2 * q] = w2.y; wr[2 * q + 1] = w2.z; wi[2 * q + 1] = w2.w;
+            }
             float er0 = 0.f, ei0 = 0.f;
 #pragma unroll
             for (int j = 0; j < P; ++j) {
@@ -137,7 +142,7 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
                 const float cr = fmaf(er, cs, -ei * sn);  // c_in, once for all coils
                 const float ci = fmaf(er, sn, ei * cs);
 #pragma unroll
-                for (int k = 0; k < kCoilsPerPass; ++k) {
+                for (int k = 0; k < NC; ++k) {
                     ar[k][j] = fmaf(wr[k], cr, fmaf(-wi[k], ci, ar[k][j]));
                     ai[k][j] = fmaf(wr[k], ci, fmaf(wi[k], cr, ai[k][j]));
                 }
@@ -152,7 +157,7 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         const int p = p0 + j;
         if (p < n_pts) {
 #pragma unroll
-            for (int k = 0; k < kCoilsPerPass; ++k)
+            for (int k = 0; k < NC; ++k)
                 partial[k * coil_stride + (size_t)blockIdx.y * n_pts + p] = make_float2(ar[k][j], ai[k][j]);
         }
     }

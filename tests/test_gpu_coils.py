@@ -48,8 +48,9 @@ def test_small_configs_with_coils_match_oracle(B, oracle_mod, name, n_coils, pha
 
 
 def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
-    """One coil with weight 1 everywhere returns the plain signal; 9 coils (three passes of 4, the last with one
-    coil) give the same rows as the same coils simulated in separate calls, bitwise."""
+    """One coil with weight 1 everywhere returns the plain signal; 9 coils (two passes of 8, the last with one coil)
+    give the same rows as the same coils simulated in separate calls: bitwise when the pass width is the same
+    (coils 0-7 alone), to rounding when it is not (4 coils per pass for up to 4 coils: other tile sizes)."""
     from test_gpu_parity import run_gpu
     w = W.small("4")
     n = w.phantom.n
@@ -61,10 +62,12 @@ def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
     all9 = run_coils(B, w, coils)
     again = run_coils(B, w, coils)
     assert np.array_equal(all9.view(np.float32), again.view(np.float32)), "run-to-run not bitwise identical"
+    first8 = run_coils(B, w, coils[:8])
+    assert np.array_equal(all9[:8].view(np.float32), first8.view(np.float32))
+    scale = np.abs(all9).max()
     first4 = run_coils(B, w, coils[:4])
     last1 = run_coils(B, w, coils[8:9])
-    assert np.array_equal(all9[:4].view(np.float32), first4.view(np.float32))
-    assert np.array_equal(all9[8:9].view(np.float32), last1.view(np.float32))
+    assert np.abs(all9[:4] - first4).max() / scale < 2e-6 and np.abs(all9[8:9] - last1).max() / scale < 2e-6
 
 
 def test_coil_argument_errors_and_edge_cases(B):
