@@ -214,7 +214,8 @@ int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d
  *   BLOCH_PATH_PER_BLOCK: one excitation launch per RF block and one signal launch per precession block.
  *   BLOCH_PATH_FUSED: ONE persistent whole-sequence launch (a CTA per SM owns a chunk of spins for the whole
  *       sequence; warp-specialised excitation / readout, see csrc/seq.cuh) plus the second-pass reduction.
- *       Available for SUM_ALL output, fp32 phase, no motion and at most 29 x 32 spins per SM; bloch_simulate
+ *       Available for SUM_ALL output (and for PER_SPIN plans whose blocks hold at most 16 ADC samples: dictionary
+ *       mode), fp32 phase, no motion and at most 29 x 32 spins per SM; bloch_simulate
  *       returns BLOCH_EINVAL when it is forced and not available.
  *   BLOCH_PATH_AUTO (default): FUSED when available, 4 N_rf >= N_adc and at most 21 x 32 spins per SM (the full set
  *       of signal warps fits beside the RF warps), else PER_BLOCK.

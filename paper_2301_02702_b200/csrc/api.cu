@@ -98,16 +98,21 @@ constexpr size_t kSeqPartialCapBytes = size_t(8) << 30;
 SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     SeqShape q{};
     const bloch_plan_info &inf = plan->info;
-    if (inf.output_mode != BLOCH_OUT_SUM_ALL || inf.motion_mode != BLOCH_MOTION_NONE ||
-        inf.phase_mode != BLOCH_PHASE_FP32 || n_spins <= 0 || plan->path == BLOCH_PATH_PER_BLOCK)
+    // PER_SPIN plans qualify when every block holds only a few samples (dictionary mode: the RF thread that owns
+    // the spin evaluates them itself, no signal warps)
+    const bool ps = inf.output_mode == BLOCH_OUT_PER_SPIN;
+    if ((inf.output_mode != BLOCH_OUT_SUM_ALL && !(ps && inf.max_block_adc <= 16)) ||
+        inf.motion_mode != BLOCH_MOTION_NONE || inf.phase_mode != BLOCH_PHASE_FP32 || n_spins <= 0 ||
+        plan->path == BLOCH_PATH_PER_BLOCK)
         return q;
     const int64_t per_sm = (n_spins + sm_count - 1) / sm_count;
     q.chunk = (int)std::max<int64_t>(32, (per_sm + 31) / 32 * 32);
     q.rf_warps = q.chunk / 32;
     // 10 signal warps: measured optimum on config 5 (14 RF warps per SM; 4: 168 ms, 8: 133, 10: 129.5, 16: 141)
     const int want = std::min(std::max(env_int("BLOCH_SEQ_SIGNAL_WARPS", 10), 1), 30);
-    q.sig_warps = std::min(want, kSeqMaxThreads / 32 - 1 - q.rf_warps);
-    if (q.sig_warps < std::min(want, 2)) return q;  // no room beside the RF warps: more than 29 x 32 spins per SM
+    q.sig_warps = ps ? 0 : std::min(want, kSeqMaxThreads / 32 - 1 - q.rf_warps);
+    if (ps ? q.rf_warps > kSeqMaxThreads / 32 - 1 : q.sig_warps < std::min(want, 2))
+        return q;  // no room beside the RF warps: more than 29 x 32 spins per SM (31 x 32 for PER_SPIN)
     q.threads = 32 * (1 + q.rf_warps + q.sig_warps);
     q.min_items = std::max(1, q.sig_warps * env_int("BLOCH_SEQ_ITEMS_PER_WARP_X4", 4) / 4);
     q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
@@ -119,7 +124,7 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     // fits beside the RF warps (its readout runs on sig_warps warps per SM only).  Measured, fused / per-block ms:
     // N_rf/N_adc = 0.98: 13.1 / 15.5 at 65,536 spins, 42.1 / 29.4 at 131,044 (3 signal warps left);
     // 0.49: 5.97 / 6.17 at 65,536, 22.2 / 11.3 at 131,072;  0.06: 1.05 / 0.84 at 65,522.
-    q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && q.sig_warps >= want);
+    q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || q.sig_warps >= want));
     return q;
 }
 
@@ -468,22 +473,29 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     SeqShape sq = seq_shape(plan, n_spins, sms);
     if (n_coils > 0) sq.use = false;  // multi-coil receive runs on the per-block path
     if (plan->path == BLOCH_PATH_FUSED && !sq.ok)
-        return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output, fp32 phase, no motion and <= 29 x 32 spins per SM");
+        return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output (or PER_SPIN with <= 16 samples per block), fp32 phase, no motion and <= 29 x 32 spins per SM");
     if (sq.ok && sq.use) {
         // ONE persistent launch for the whole sequence + the second pass over all ADC samples
         static bool attr_set = false;  // per process; the attribute is sticky for the function
         if (!attr_set) {
-            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)seq_smem_bytes(kSeqMaxThreads)));
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)seq_smem_bytes(kSeqMaxThreads)));
             attr_set = true;
         }
         if ((rc = taps.mark(BLOCH_KIND_FUSED))) return rc;
-        seq_kernel<<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
-            plan->d_tables, reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off), (int)plan->blocks.size(),
-            w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items, (const float *)w.scal, w.partial, (long long)plan->info.n_adc,
-            d_Mxy ? 1 : 0);
+        const SeqOp *prog = reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off);
+        if (per_spin)
+            seq_kernel<true><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
+                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items,
+                (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, (float2 *)d_signal);
+        else
+            seq_kernel<false><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
+                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items,
+                (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, nullptr);
         ++launches;
-        if (plan->info.n_adc > 0) {
+        if (plan->info.n_adc > 0 && !per_spin) {
             if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
             reduce_kernel<<<(unsigned)((plan->info.n_adc + 31) / 32), dim3(32, 8), 0, stream>>>(
                 w.partial, sq.n_ctas, (int)plan->info.n_adc, (float2 *)d_signal);

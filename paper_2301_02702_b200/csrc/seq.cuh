@@ -118,11 +118,13 @@ __device__ __forceinline__ void seq_signal_block(const float4 *__restrict__ recs
     }
 }
 
+// PS: PER_SPIN plans (a separate instantiation so that the SUM_ALL kernel keeps its 64 registers without spills)
+template <bool PS>
 __global__ void __launch_bounds__(kSeqMaxThreads, 1)
 seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ ops, int n_ops,
            const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n, int chunk,
            int rf_warps, int min_items, const float *__restrict__ scal, float2 *__restrict__ partial,
-           long long n_adc, int final_state) {
+           long long n_adc, int final_state, float2 *__restrict__ out_ps /* PER_SPIN plans: out[spin][adc], else NULL */) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *ring = smem;
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kSeqStages * kSeqTileStride);
@@ -143,7 +145,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
         }
         for (int k = 0; k < kSeqStateBufs; ++k) {
             mbar_init(&st_full[k], n_rf_thr);
-            mbar_init(&st_empty[k], nsig);
+            mbar_init(&st_empty[k], max(nsig, 1));
             item_ctr[k] = 0;
         }
         mbar_init_fence();
@@ -228,7 +230,23 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                 hx += lx; hy += ly; hz += lz;
                 lx = 0.f; ly = 0.f; lz = 0.f;
             } else {
-                if (tn.y > 0) {  // publish the block-start state for the signal warps
+                if (PS && tn.y > 0) {
+                    // PER_SPIN output (dictionary mode; blocks of a few samples): the spin's own thread evaluates
+                    // them with the accurate functions and fp64 phase of perspin_kernel -- no signal warps
+                    const float4 *recs = reinterpret_cast<const float4 *>(tables + ops[oi].table_off);
+                    float2 *row = out_ps + (size_t)i * (size_t)n_adc + ops[oi].adc_first;
+                    for (int p = 0; p < tn.y; ++p) {
+                        const float4 rc = recs[p];  // k' in rad/m, tau
+                        double th = ((double)rc.x * (double)a.x + (double)rc.y * (double)a.y + (double)rc.z * (double)a.z) *
+                                        0.15915494309189535 - (double)c.w * 0.15915494309189535 * (double)rc.w;
+                        th -= rint(th);
+                        float sn, cs;
+                        sincospif(2.0f * (float)th, &sn, &cs);
+                        const float e = expf(-rc.w * c.y);
+                        const float er = hx * e, ei = hy * e;
+                        if (active) row[p] = make_float2(er * cs - ei * sn, er * sn + ei * cs);
+                    }
+                } else if (tn.y > 0) {  // publish the block-start state for the signal warps
                     const int b = pub % kSeqStateBufs, use = pub / kSeqStateBufs;
                     if (use > 0) mbar_wait(&st_empty[b], (uint32_t)((use - 1) & 1));
                     if (active) shS[b * chunk + r] = make_float4(hx, hy, hz, s.w);

@@ -162,3 +162,30 @@ def test_fused_mixed_tiles_and_tiers(B, oracle_mod):
     assert np.array_equal(out["fused"][1], out["per_block"][1]) and np.array_equal(out["fused"][2], out["per_block"][2])
     assert_parity(np.concatenate([out["fused"][1], out["fused"][2].astype(np.complex128)]),
                   np.concatenate([rxy, rz.astype(np.complex128)]), "mixed tiles: state")
+
+
+def test_fused_per_spin_dictionary_mode(B, oracle_mod):
+    """PER_SPIN plans with a few samples per block (an MRF dictionary: one sample per TR) run as ONE launch: the
+    thread that owns the spin evaluates its samples itself.  Against the oracle and the per-block path."""
+    w = W.small("5b")
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, output_mode="per_spin", return_state=True)
+    out = {}
+    for path in ("per_block", "fused"):
+        out[path] = run_gpu(B, w, want_state=True, path=path, phase_mode="fp32")
+    sig, mxy, mz = out["fused"]
+    assert sig.shape == ref.shape == (w.phantom.n, w.seq.adc_t.size)
+    assert_parity(sig, ref, "dictionary, whole-sequence kernel")
+    assert_parity(np.concatenate([mxy, mz.astype(np.complex128)]), np.concatenate([rxy, rz.astype(np.complex128)]),
+                  "dictionary final state")
+    assert np.array_equal(mxy, out["per_block"][1]) and np.array_equal(mz, out["per_block"][2])
+    emax, _ = errors(sig, out["per_block"][0])
+    assert emax < 2e-6
+    plan = B.Plan(w.seq, phase_mode="fp32", output_mode="per_spin")
+    assert B.bloch_plan_uses_fused(plan.handle, w.phantom.n)          # AUTO takes it
+    assert B.bloch_plan_uses_fused(plan.handle, 100_000)              # 22 RF warps per SM
+    assert not B.bloch_plan_uses_fused(plan.handle, 640_000)
+    plan.close()
+    w5 = W.small("5")                                                 # 300 samples per block: not this way
+    plan = B.Plan(w5.seq, phase_mode="fp32", output_mode="per_spin", path="fused")
+    assert not B.bloch_plan_uses_fused(plan.handle, w5.phantom.n)
+    plan.close()
