@@ -189,3 +189,20 @@ def test_fused_per_spin_dictionary_mode(B, oracle_mod):
     plan = B.Plan(w5.seq, phase_mode="fp32", output_mode="per_spin", path="fused")
     assert not B.bloch_plan_uses_fused(plan.handle, w5.phantom.n)
     plan.close()
+
+
+def test_fused_is_race_free_over_many_runs(B, monkeypatch):
+    """The roles of the whole-sequence kernel meet only at mbarriers; a missing edge would show up as run-to-run
+    differences.  25 runs each with 2, 5 and 10 signal warps (different interleavings of the roles), all bitwise equal
+    per configuration, signal and final state."""
+    w = W.small("5")
+    for nw in ("2", "5", "10"):
+        monkeypatch.setenv("BLOCH_SEQ_SIGNAL_WARPS", nw)
+        first = None
+        for _ in range(25):
+            sig, mxy, mz = run_gpu(B, w, want_state=True, path="fused", phase_mode="fp32")
+            cur = (sig.view(np.float32).copy(), mxy.view(np.float32).copy(), mz.copy())
+            if first is None:
+                first = cur
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(first, cur)), f"{nw} signal warps: runs differ"
