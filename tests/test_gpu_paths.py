@@ -167,3 +167,28 @@ def test_adiabatic_inversion_recovery_long_soft_pulse(B, oracle_mod):
                                    return_state=True)
     frac = rz / ph.M0
     assert (frac < -0.8).sum() > 300 and (frac > 0.8).sum() > 300, "the phantom must straddle the inverted band"
+
+
+def test_off_centre_slices_by_rf_phase_ramps(B, oracle_mod):
+    """Two slice-selective pulses with frequency offsets of +3 kHz and -2 kHz (phase ramps on the complex B1: the step
+    records change in both components from step to step), each followed by a readout; spins across 4 cm of z."""
+    T, n, Gz = 2e-3, 2000, 8e-3
+    dt = T / n
+    tm = (np.arange(n) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - T / 2) / T)
+    b1 = env * (np.pi / 4) / (W.GAMMA * dt * env.sum())
+    parts, g2, adc = [], [[], []], []
+    gx = [[], []]
+    for k, df in enumerate((3000.0, -2000.0)):
+        t0 = 1e-4 + k * 6e-3
+        ph = -2 * np.pi * df * tm
+        parts.append((t0 + np.arange(n) * dt, np.full(n, dt), b1 * np.cos(ph), b1 * np.sin(ph)))
+        g2[0] += [t0 - 1e-4, t0, t0 + T, t0 + T + 1e-4, t0 + T + 6e-4, t0 + T + 7e-4]
+        g2[1] += [0.0, Gz, Gz, -Gz, -Gz, 0.0]           # slice select, then a rephaser lobe
+        gx[0] += [t0 + T + 8e-4, t0 + T + 9e-4, t0 + T + 2.9e-3, t0 + T + 3e-3]
+        gx[1] += [0.0, 5e-3, 5e-3, 0.0]
+        adc.append(t0 + T + 1e-3 + (np.arange(150) + 0.5) * 1e-5)
+    rf = tuple(np.concatenate([p[i] for p in parts]) for i in range(4))
+    s = seq(g={2: (g2[0], g2[1]), 0: (gx[0], gx[1])}, rf=rf, adc=np.concatenate(adc), t_end=13e-3, dt_rf_max=1.0)
+    ph = rand_phantom(4000, 31, zmax=0.02, dwmax=100.0)
+    check(B, oracle_mod, ph, s, "off-centre slices")

@@ -450,3 +450,32 @@ def test_p11_adiabatic_hyperbolic_secant_inversion_profile(oracle_mod, w1max):
     np.testing.assert_allclose(np.abs(mxy) ** 2 + mz ** 2, 1.0, rtol=0, atol=1e-9)   # a rotation: |M| kept
     inside, outside = np.abs(Om) < 0.4 * mu * beta, np.abs(Om) > 1.5 * mu * beta
     assert mz[inside].max() < -0.98 and mz[outside].min() > 0.999                      # what "inversion band" means
+
+
+# ---------------------------------------------------------------------------------------------- P12
+def test_p12_frequency_offset_pulse_excites_the_shifted_slice(oracle_mod):
+    """Reading G12 (B1 is complex; an RF frequency offset is a phase ramp on it) together with reading G3 (free
+    precession is Mxy e^{-i dw t}): a pulse B1(t) e^{-i 2 pi df t} under a slice gradient Gz is, in the frame rotating
+    at df, the same pulse on resonance for the spin at z0 = df / (gamma_bar Gz).  So the excited profile is the
+    on-centre profile moved to z0 -- same Mz, same |Mxy| -- and NOT to -z0 (which is what a sign slip between the
+    B1 phase convention and the precession direction would give).  PAPER.md:99-101 off-centre slices."""
+    T, n, Gz, df = 2e-3, 4000, 8e-3, 3000.0     # 0.5 us steps: the piecewise-constant phase ramp costs (2 pi df dt)^2 / 24 = 4e-6
+    dt = T / n
+    tm = (np.arange(n) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - T / 2) / T) * (0.54 + 0.46 * np.cos(2 * math.pi * (tm - T / 2) / T))
+    b1 = env * (math.pi / 3) / (GAMMA * dt * env.sum())
+    z0 = df / (GAMMA / (2 * math.pi) * Gz)                     # 8.8 mm
+    z = np.linspace(-0.02, 0.02, 161)
+    g = {2: ([0.0, T], [Gz, Gz])}
+    on = seq(g=g, rf=(np.arange(n) * dt, np.full(n, dt), b1, np.zeros(n)), t_end=T, dt_rf_max=dt)
+    ph = -2 * math.pi * df * tm
+    off = seq(g=g, rf=(np.arange(n) * dt, np.full(n, dt), b1 * np.cos(ph), b1 * np.sin(ph)), t_end=T, dt_rf_max=dt)
+    _, mxy_on, mz_on = oracle_mod.simulate(phantom(z=z - z0), on, return_state=True)     # profile at z' = z - z0
+    _, mxy_off, mz_off = oracle_mod.simulate(phantom(z=z), off, return_state=True)
+    np.testing.assert_allclose(mz_off, mz_on, rtol=0, atol=2e-5)
+    np.testing.assert_allclose(np.abs(mxy_off), np.abs(mxy_on), rtol=0, atol=2e-5)
+    # in the frame rotating at df the transverse magnetisation is the on-centre one: Mxy_off = Mxy_on e^{-i 2 pi df T}
+    np.testing.assert_allclose(mxy_off, mxy_on * np.exp(-2j * math.pi * df * T), rtol=0, atol=2e-5)
+    # and the slice really sits at +z0: the profile's centre of mass
+    com = (z * np.abs(mxy_off)).sum() / np.abs(mxy_off).sum()
+    assert abs(com - z0) < 2e-4 and np.abs(mxy_off)[np.argmin(np.abs(z + z0))] < 0.02
