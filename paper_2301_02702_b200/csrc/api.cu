@@ -51,11 +51,14 @@ struct SigShape {
     int spins_per_chunk;
 };
 
-SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
+// max_P: 8, or 4 for fp64-phase motion plans (P = 8 would need 172 registers there: config 3m 2.09 -> 2.47 ms)
+SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count, int max_P) {
     SigShape s;
     const int forceP = env_int("BLOCH_SIGNAL_P", 0);
-    s.P = forceP ? forceP : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1));
-    if (s.P != 1 && s.P != 2 && s.P != 4) s.P = 1;
+    // 8 adjacent samples per thread when the block is long enough (config 4: 42.5 -> 35.6 ms together with the
+    // geometric decay; ~100 registers, 2 CTAs per SM), else 4 / 2 / 1
+    s.P = forceP ? forceP : (n_pts >= 8 * kSigThreads && max_P >= 8 ? 8 : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1)));
+    if (s.P != 1 && s.P != 2 && s.P != 4 && s.P != 8) s.P = 1;
     s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
     const int per_sm = env_int("BLOCH_SIGNAL_CTAS_PER_SM", 4);
     const int64_t target = (int64_t)sm_count * per_sm;
@@ -69,6 +72,10 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count) {
     return s;
 }
 
+int sig_max_P(const bloch_plan *plan) {
+    return (plan->info.phase_mode == BLOCH_PHASE_FP64 && plan->info.motion_mode == BLOCH_MOTION_LINEAR) ? 4 : 8;
+}
+
 // Partial-sum buffer (a7): consecutive ADC-bearing precession blocks with the same launch shape share one
 // buffer P[chunk][points of the batch] and ONE second-pass launch, up to kPartialCapBytes; at least the
 // largest single block always fits.
@@ -78,7 +85,7 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
     size_t worst = 1, total = 0;
     for (const Block &b : plan->blocks) {
         if (b.type != kBlockPrecession || b.adc_count == 0) continue;
-        const SigShape s = sig_shape(b.adc_count, n_spins, sm_count);
+        const SigShape s = sig_shape(b.adc_count, n_spins, sm_count, sig_max_P(plan));
         const size_t e = size_t(s.chunks) * size_t(b.adc_count);
         worst = std::max(worst, e);
         total += e;
@@ -597,7 +604,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     launches += 2;
                 }
             } else {
-                const SigShape s = sig_shape(n_pts, n, sms);
+                const SigShape s = sig_shape(n_pts, n, sms, sig_max_P(plan));
                 if (!batch_open) {  // look ahead: how many of the following blocks share this batch
                     batch_shape = s;
                     batch_adc_first = b.adc_first;
@@ -607,7 +614,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     for (size_t bj = bi; bj < plan->blocks.size(); ++bj) {
                         const Block &c = plan->blocks[bj];
                         if (c.type != kBlockPrecession || c.adc_count == 0) continue;
-                        const SigShape sc = sig_shape(c.adc_count, n, sms);
+                        const SigShape sc = sig_shape(c.adc_count, n, sms, sig_max_P(plan));
                         if (sc.P != s.P || sc.chunks != s.chunks || sc.spins_per_chunk != s.spins_per_chunk) break;
                         if (batch_pts + c.adc_count > cap_pts || batch_pts + c.adc_count > INT32_MAX) break;
                         batch_pts += c.adc_count;
@@ -626,7 +633,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else if (mo) BLOCH_LAUNCH_SIG3(PP, false, true, w.A, w.V);                                             \
         else BLOCH_LAUNCH_SIG3(PP, false, false, w.A, nullptr);                                                \
     } while (0)
-                if (s.P == 4) BLOCH_LAUNCH_SIG(4);
+                if (s.P == 8) BLOCH_LAUNCH_SIG(8);
+                else if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
                 else BLOCH_LAUNCH_SIG(1);
 #undef BLOCH_LAUNCH_SIG

@@ -68,13 +68,23 @@ __device__ __forceinline__ void seq_signal_item(const float4 *__restrict__ recs,
     }
     // exp(-tau_j/T2), j > 0, from the j = 0 value by a cubic series when (tau_j - tau_0)/T2 <= 0.02 for every spin
     const bool series = P > 1 && __all_sync(0xffffffffu, cmax * r2max_log2e <= 0.02f);
-    auto run = [&](auto series_tag) {
-        constexpr bool SERIES = decltype(series_tag)::value;
+    // equally spaced samples: decay of sample j = decay of sample j-1 times q = exp(-dwell/T2) (signal.cuh)
+    float dev = 0.f;
+#pragma unroll
+    for (int j = 2; j < P; ++j) dev = fmaxf(dev, fabsf(cj[j] - (float)j * cj[1]));
+    const bool geom = P > 2 && series && __all_sync(0xffffffffu, dev * r2max_log2e <= 1e-6f);
+    auto run = [&](auto mode_tag) {
+        constexpr int MODE = decltype(mode_tag)::value;  // 0: MUFU.EX2 per sample, 1: series per sample, 2: geometric
+        constexpr bool SERIES = MODE != 0;
 #pragma unroll 2
         for (int s = 0; s < cnt; ++s) {
             const float4 a = shA[s];
             const float4 st = shS[s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
-            float er0 = 0.f, ei0 = 0.f;
+            float er0 = 0.f, ei0 = 0.f, qd = 1.f;
+            if (MODE == 2) {
+                const float y = cj[1] * st.w;  // -dwell/T2
+                qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+            }
 #pragma unroll
             for (int j = 0; j < P; ++j) {
                 const float th = fmaf(kx[j], a.x, fmaf(ky[j], a.y, fmaf(kz[j], a.z, tau[j] * a.w)));  // radians
@@ -85,6 +95,11 @@ __device__ __forceinline__ void seq_signal_item(const float4 *__restrict__ recs,
                     er = st.x * e;
                     ei = st.y * e;
                     if (j == 0) { er0 = er; ei0 = ei; }
+                } else if (MODE == 2) {
+                    er0 *= qd;
+                    ei0 *= qd;
+                    er = er0;
+                    ei = ei0;
                 } else {
                     const float y = cj[j] * st.w;
                     const float pe = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
@@ -96,8 +111,9 @@ __device__ __forceinline__ void seq_signal_item(const float4 *__restrict__ recs,
             }
         }
     };
-    if (series) run(std::true_type{});
-    else run(std::false_type{});
+    if (geom) run(std::integral_constant<int, 2>{});
+    else if (series) run(std::integral_constant<int, 1>{});
+    else run(std::integral_constant<int, 0>{});
 #pragma unroll
     for (int j = 0; j < P; ++j)
         if (p0 + j < n_pts) out[p0 + j] = make_float2(ar[j], ai[j]);

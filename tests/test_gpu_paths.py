@@ -110,9 +110,9 @@ def test_rf_on_gradient_ramps_and_changing_step_length(B, oracle_mod):
     check(B, oracle_mod, rand_phantom(333, 6), s, "RF on ramps, mixed dt")
 
 
-@pytest.mark.parametrize("n_adc", [1, 5, 300, 700, 1023, 2049])
+@pytest.mark.parametrize("n_adc", [1, 5, 300, 700, 1023, 2049, 2300])
 def test_signal_launch_shapes_and_ragged_tails(B, oracle_mod, n_adc):
-    """n_adc selects P = 1 (< 512 points), 2 (< 1024) or 4 and leaves ragged point tiles; 1111 spins leave a
+    """n_adc selects P = 1 (< 512 points), 2 (< 1024), 4 (< 2048) or 8 and leaves ragged point tiles; 1111 spins leave a
     ragged spin tile."""
     rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 3) / (W.GAMMA * 1e-4)]), np.array([0.0]))
     g = {0: ([2e-4, 3e-4, 9e-3], [0, 4e-3, 4e-3]), 1: ([2e-4, 3e-4, 9e-3], [0, -2e-3, 1e-3])}
@@ -192,3 +192,16 @@ def test_off_centre_slices_by_rf_phase_ramps(B, oracle_mod):
     s = seq(g={2: (g2[0], g2[1]), 0: (gx[0], gx[1])}, rf=rf, adc=np.concatenate(adc), t_end=13e-3, dt_rf_max=1.0)
     ph = rand_phantom(4000, 31, zmax=0.02, dwmax=100.0)
     check(B, oracle_mod, ph, s, "off-centre slices")
+
+
+@pytest.mark.parametrize("jitter", [0.0, 2e-9, 3e-7])
+def test_signal_decay_modes_equal_spacing_and_jitter(B, oracle_mod, jitter):
+    """Equally spaced samples take the geometric decay (sample j = sample j-1 times exp(-dwell/T2)); samples jittered
+    by a few ns still do (below the 1e-6 bound on |deviation|/T2 with T2 >= 5 ms), by 0.3 us fall back to the
+    per-sample series.  4100 samples = P = 8 per thread with a ragged tail; short T2 makes the decay matter."""
+    rng = np.random.default_rng(12)
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    adc = 3e-4 + (np.arange(4100) + 0.5) * 2e-6 + rng.uniform(-jitter, jitter, 4100)
+    g = {0: ([2e-4, 3e-4, 9e-3], [0, 4e-3, 4e-3]), 1: ([2e-4, 3e-4, 9e-3], [0, -2e-3, 1e-3])}
+    s = seq(g=g, rf=rf, adc=np.sort(adc), t_end=1e-2, dt_rf_max=1.0)
+    check(B, oracle_mod, rand_phantom(900, 13, t2=(0.005, 0.05)), s, f"decay modes, jitter {jitter}")
