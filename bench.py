@@ -34,8 +34,8 @@ MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)          
 FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
 FP32_PER_EVAL = 15         # FP32-pipe instructions per (spin, evaluated point)
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full captures
-NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v2_signal_kernel_cfg4_ncu.txt"),
-               ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v2_rf_kernel_cfg4_ncu.txt"),
+NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v3_signal_kernel_cfg4_ncu.txt"),
+               ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v3_rf_kernel_cfg4_ncu.txt"),
                ("config5_mrf_fisp", "fused"): (1224.6e6, "profiles/r01_v3_seq_kernel_cfg5_ncu.txt")}
 
 
@@ -321,8 +321,8 @@ def run_ours(args, rank, local_rank, world):
                           "traffic_source": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[1],
                           "coils": n_coils,
                           "note": "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample), SURVEY.md 8(d); "
-                                  "the kernel issues 2 + 1/P (P = 4 adjacent samples share one ex2), so frac can "
-                                  "reach 3 / 2.25 = 1.33 at a saturated MUFU pipe",
+                                  "the kernel issues 2 + 1/P (P = 8 adjacent samples share one ex2; 4 in shorter blocks), so frac "
+                                  "can reach 3 / 2.125 = 1.41 at a saturated MUFU pipe",
                           "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
                           "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
                           "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}
