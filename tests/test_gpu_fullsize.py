@@ -141,3 +141,37 @@ def test_full_config3_with_motion_experiment_d(B, oracle_mod):
     m = Mxy.cpu().numpy()
     assert_parity(sig.cpu().numpy(), ref, "config 3m full-size signal")
     assert_parity(state_vec(m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy()), state_vec(rxy, rz), "config 3m full-size final state")
+
+
+def test_full_config4_with_8_coils_by_subset_and_superposition(B, oracle_mod):
+    """Workload 4c (config 4 received by 8 coils) at full size: an evenly spaced subset against the
+    oracle (every coil on its own scale), and superposition S_c(full) = S_c(subset) + S_c(complement) per coil, which
+    ties the full-size launch (one pass of 8 coils, P = 2, 296 CTAs) to it."""
+    import torch
+    w = W.make("4c")
+    n = w.phantom.n
+    plan = B.Plan(w.seq, phase_mode=w.phase_mode, output_mode="sum")
+
+    def run(idx):
+        ph = w.phantom if idx is None else w.phantom.subset(idx)
+        c = w.coils if idx is None else np.ascontiguousarray(w.coils[:, idx])
+        sig = plan.simulate(*B.phantom_to_device(ph), coils=torch.from_numpy(c).cuda())
+        torch.cuda.synchronize()
+        return sig.cpu().numpy()
+
+    full = run(None)
+    assert full.shape == (8, 65536)
+    assert np.array_equal(full.view(np.float32), run(None).view(np.float32)), "not bitwise reproducible"
+    sub = np.linspace(0, n - 1, 192).astype(np.int64)
+    s_sub = run(sub)
+    ref = oracle_mod.simulate(w.phantom.subset(sub), w.seq, coils=w.coils[:, sub].astype(np.complex128))
+    assert_parity(s_sub, ref, "config 4c subset, all coils")
+    for c in range(8):
+        assert_parity(s_sub[c], ref[c], f"config 4c subset, coil {c}")
+    mask = np.ones(n, dtype=bool)
+    mask[sub] = False
+    s_rest = run(np.flatnonzero(mask))
+    plan.close()
+    for c in range(8):
+        emax, nrmse = errors(s_sub[c].astype(np.complex128) + s_rest[c], full[c])
+        assert emax < 5e-6 and nrmse < 1e-6, f"coil {c} superposition: max {emax:.3e} nrmse {nrmse:.3e}"
