@@ -210,6 +210,17 @@ int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d
                          int init_equilibrium, float *d_signal, void *d_workspace, size_t workspace_bytes,
                          void *stream);
 
+/* Host-buffer variant of bloch_simulate_coils: phantom, coil weights (float2 [n_coils][n_spins]), state and signal
+ * (float2 [n_coils][n_adc]) are HOST arrays (pinned memory makes the copies asynchronous); H2D and D2H copies are
+ * made on `stream` inside the call, which synchronises the stream before returning.  d_scratch: DEVICE, 256-B
+ * aligned, at least bloch_simulate_host_coils_scratch_bytes(). */
+int bloch_simulate_host_coils_scratch_bytes(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out);
+int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                              const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                              const float *h_dw, int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz,
+                              int init_equilibrium, float *h_signal, void *d_scratch, size_t scratch_bytes,
+                              void *stream);
+
 /* Execution path of bloch_simulate for this plan.
  *   BLOCH_PATH_PER_BLOCK: one excitation launch per RF block and one signal launch per precession block.
  *   BLOCH_PATH_FUSED: ONE persistent whole-sequence launch (a CTA per SM owns a chunk of spins for the whole

@@ -54,7 +54,8 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_simulate_motion", "bloch_simulate_host_scratch_bytes", "bloch_simulate_host",
            "bloch_simulate_host_motion", "bloch_plan_set_profiling",
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
-           "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils",
+           "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils", "bloch_simulate_host_coils_scratch_bytes",
+           "bloch_simulate_host_coils",
            "bloch_microbench"]
 
 
@@ -83,6 +84,8 @@ def _load():
     lib.bloch_simulate_host_motion.argtypes = mo_args
     lib.bloch_plan_workspace_bytes_coils.argtypes = [vp, i64, C.c_int, C.POINTER(sz)]
     lib.bloch_simulate_coils.argtypes = [vp, i64] + [_fp] * 7 + [C.c_int, _fp, _fp, _fp, C.c_int, _fp, vp, sz, vp]
+    lib.bloch_simulate_host_coils_scratch_bytes.argtypes = [vp, i64, C.c_int, C.POINTER(sz)]
+    lib.bloch_simulate_host_coils.argtypes = lib.bloch_simulate_coils.argtypes
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
@@ -207,6 +210,19 @@ def bloch_simulate_coils(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, n_coi
     DEVICE address of float2 [n_coils][n_adc]."""
     _check(_lib.bloch_simulate_coils(plan, n_spins, x, y, z, M0, T1, T2, dw, n_coils, coil, Mxy, Mz,
                                      int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_host_coils_scratch_bytes(plan: int, n_spins: int, n_coils: int) -> int:
+    out = C.c_size_t()
+    _check(_lib.bloch_simulate_host_coils_scratch_bytes(plan, n_spins, n_coils, C.byref(out)))
+    return int(out.value)
+
+
+def bloch_simulate_host_coils(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, n_coils: int, coil, Mxy, Mz,
+                              init_equilibrium: bool, signal, scratch, scratch_bytes: int, stream: int = 0):
+    """bloch_simulate_coils with HOST phantom / coil / state / signal addresses; scratch is a device address."""
+    _check(_lib.bloch_simulate_host_coils(plan, n_spins, x, y, z, M0, T1, T2, dw, n_coils, coil, Mxy, Mz,
+                                          int(bool(init_equilibrium)), signal, scratch, scratch_bytes, stream))
 
 
 def bloch_simulate_host_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
@@ -359,7 +375,7 @@ class Plan:
         return signal
 
     def simulate_host(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None,
-                      velocity=None):
+                      velocity=None, coils=None):
         """End-to-end path: numpy float32 HOST arrays in, numpy complex64 signal out (synchronous)."""
         import torch
         if self._tables is None:
@@ -370,6 +386,20 @@ class Plan:
         shape = self._signal_shape(n)
         if signal is None:
             signal = np.empty(shape, dtype=np.complex64)
+        if coils is not None:
+            cw = np.ascontiguousarray(coils, dtype=np.complex64)
+            assert cw.ndim == 2 and cw.shape[1] == n and velocity is None
+            n_coils = int(cw.shape[0])
+            if signal is None or signal.shape != (n_coils, n_adc):
+                signal = np.empty((n_coils, n_adc), dtype=np.complex64)
+            need = max(bloch_simulate_host_coils_scratch_bytes(self.handle, n, n_coils), 256)
+            if self._scratch is None or self._scratch.numel() < need:
+                self._scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
+            bloch_simulate_host_coils(self.handle, n, *[a.ctypes.data for a in arrs], n_coils, cw.ctypes.data,
+                                      None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
+                                      init_equilibrium, signal.ctypes.data if signal.size else None,
+                                      self._scratch.data_ptr(), self._scratch.numel(), self._stream())
+            return signal
         need = max(bloch_simulate_host_scratch_bytes(self.handle, n), 256)
         if self._scratch is None or self._scratch.numel() < need:
             self._scratch = torch.empty(need, dtype=torch.uint8, device="cuda")

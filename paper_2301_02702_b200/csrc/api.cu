@@ -756,6 +756,71 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins, const fl
     return BLOCH_OK;
 }
 
+int bloch_simulate_host_coils_scratch_bytes(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out) {
+    if (!plan || !out || n_spins < 0 || n_coils < 1) return fail(BLOCH_EINVAL, "NULL plan/out, negative n_spins or n_coils < 1");
+    size_t ws = 0;
+    int rc = bloch_plan_workspace_bytes_coils(plan, n_spins, n_coils, &ws);
+    if (rc) return rc;
+    const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
+    const size_t coil = align_up(size_t(n_coils) * size_t(n_spins) * sizeof(float2), kAlign);
+    const size_t sig = align_up(size_t(n_coils) * size_t(plan->info.n_adc) * sizeof(float2), kAlign);
+    *out = 10 * arr + coil + sig + ws + kAlign;
+    return BLOCH_OK;
+}
+
+int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                              const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                              const float *h_dw, int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz,
+                              int init_equilibrium, float *h_signal, void *d_scratch, size_t scratch_bytes,
+                              void *stream_) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    size_t need = 0;
+    int rc = bloch_simulate_host_coils_scratch_bytes(plan, n_spins, n_coils, &need);
+    if (rc) return rc;
+    if (!d_scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(d_scratch) % kAlign) != 0)
+        return fail(BLOCH_EWORKSPACE, "scratch NULL, too small or not 256-B aligned");
+    if (n_spins > 0 && (!h_x || !h_y || !h_z || !h_M0 || !h_T1 || !h_T2 || !h_dw || !h_coil))
+        return fail(BLOCH_EINVAL, "NULL phantom or coil array");
+    if (!init_equilibrium && (!h_Mxy || !h_Mz)) return fail(BLOCH_EINVAL, "initial state requested but h_Mxy/h_Mz NULL");
+    if ((h_Mxy == nullptr) != (h_Mz == nullptr)) return fail(BLOCH_EINVAL, "h_Mxy and h_Mz must both be given or both NULL");
+    if (plan->info.n_adc > 0 && !h_signal) return fail(BLOCH_EINVAL, "h_signal is NULL");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
+    const size_t coil = align_up(size_t(n_coils) * size_t(n_spins) * sizeof(float2), kAlign);
+    const size_t sig = size_t(n_coils) * size_t(plan->info.n_adc) * sizeof(float2);
+    unsigned char *base = (unsigned char *)d_scratch;
+    float *d[7];
+    const float *h[7] = {h_x, h_y, h_z, h_M0, h_T1, h_T2, h_dw};
+    for (int k = 0; k < 7; ++k) {
+        d[k] = (float *)(base + k * arr);
+        if (n_spins > 0)
+            BLOCH_CUDA(cudaMemcpyAsync(d[k], h[k], size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+    }
+    float *d_Mxy = h_Mxy ? (float *)(base + 7 * arr) : nullptr;
+    float *d_Mz = h_Mz ? (float *)(base + 9 * arr) : nullptr;
+    if (!init_equilibrium && n_spins > 0) {
+        BLOCH_CUDA(cudaMemcpyAsync(d_Mxy, h_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyHostToDevice, stream));
+        BLOCH_CUDA(cudaMemcpyAsync(d_Mz, h_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+    }
+    float *d_coil = (float *)(base + 10 * arr);
+    if (n_spins > 0)
+        BLOCH_CUDA(cudaMemcpyAsync(d_coil, h_coil, size_t(n_coils) * size_t(n_spins) * sizeof(float2),
+                                   cudaMemcpyHostToDevice, stream));
+    float *d_sig = (float *)(base + 10 * arr + coil);
+    unsigned char *d_ws = base + 10 * arr + coil + align_up(sig, kAlign);
+    const size_t ws_bytes = scratch_bytes - (size_t)(d_ws - base);
+    rc = bloch_simulate_coils(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], n_coils, d_coil, d_Mxy, d_Mz,
+                              init_equilibrium, d_sig, d_ws, ws_bytes, stream_);
+    if (rc) return rc;
+    if (sig > 0) BLOCH_CUDA(cudaMemcpyAsync(h_signal, d_sig, sig, cudaMemcpyDeviceToHost, stream));
+    if (h_Mxy && n_spins > 0) {
+        BLOCH_CUDA(cudaMemcpyAsync(h_Mxy, d_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyDeviceToHost, stream));
+        BLOCH_CUDA(cudaMemcpyAsync(h_Mz, d_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyDeviceToHost, stream));
+    }
+    BLOCH_CUDA(cudaStreamSynchronize(stream));
+    return BLOCH_OK;
+}
+
 int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {
     if (!ops_per_s || iters <= 0 || kind < 0 || kind > 3) return fail(BLOCH_EINVAL, "bad microbench argument");
     int rc = check_arch();

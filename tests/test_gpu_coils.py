@@ -104,3 +104,17 @@ def test_coil_argument_errors_and_edge_cases(B):
     torch.cuda.synchronize()
     assert out.shape == (3, plan.info["n_adc"]) and float(out.abs().max()) == 0.0
     plan.close()
+
+
+def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
+    w = W.small("4")
+    coils = coil_maps(w.phantom, 6, seed=2)
+    dev_sig = run_coils(B, w, coils)
+    plan = B.Plan(w.seq)
+    ph = w.phantom
+    mxy = np.zeros((ph.n, 2), dtype=np.float32); mz = np.zeros(ph.n, dtype=np.float32)
+    h = plan.simulate_host(ph.x, ph.y, ph.z, ph.M0, ph.T1, ph.T2, ph.dw, Mxy=mxy, Mz=mz, coils=coils)
+    plan.close()
+    assert h.shape == (6, w.seq.adc_t.size)
+    assert np.array_equal(h.view(np.float32), dev_sig.view(np.float32)), "host-buffer coil entry differs from device entry"
+    assert np.abs(mz).max() > 0.1
