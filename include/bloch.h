@@ -137,7 +137,9 @@ int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stre
  *             S[g][j] = sum of Mxy over the group_size consecutive spins of group g -- an isochromat ensemble
  *             per voxel or per dictionary entry.
  *   Asynchronous on `stream`: no hidden synchronisation, no allocation, no host copies.  The result is
- *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 (not checked). */
+ *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 (not checked). 
+ * The call only enqueues work on `stream` (kernels and memsets; CUDA events too when profiling is on): it may be
+ * captured into a CUDA graph by the caller and replayed. */
 int bloch_simulate(const bloch_plan *plan, int64_t n_spins,
                    const float *d_x, const float *d_y, const float *d_z, const float *d_M0,
                    const float *d_T1, const float *d_T2, const float *d_dw,
