@@ -339,7 +339,9 @@ def run_ours(args, rank, local_rank, world):
                       "traffic": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[0],
                       "traffic_source": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[1],
                       "note": "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly), "
-                              "SURVEY.md 8(d); the tier-0 loop issues 38.6 per step on plateau-gradient tiles",
+                              "SURVEY.md 8(d); the tier-0 loop issues 38.5 per step on plateau-gradient tiles and reads 87 register "
+                              "operands, so its hardware floor is the register file's 2 operands per lane per clock "
+                              "(43.5 clocks per warp step; profiles/r01_pipe_microbench.md)",
                       "launches_per_step": kinds_n["rf"] // args.steps, "ms_per_step": dur * 1e3,
                       "avg_launch_ms": kinds_ms["rf"] / kinds_n["rf"],
                       "algorithmic_ops_per_launch": FP32_PER_RF_STEP * rf_steps * args.steps / kinds_n["rf"]}
