@@ -49,6 +49,7 @@ struct SigShape {
     int ptiles;
     int chunks;
     int spins_per_chunk;
+    int threads;  // CTA size: kSigThreads, or fewer for blocks of fewer samples (every thread owns a sample)
 };
 
 // max_P: 8, or 4 for fp64-phase motion plans (P = 8 would need 172 registers there: config 3m 2.09 -> 2.47 ms)
@@ -59,8 +60,13 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count, int max_P) {
     // geometric decay; ~100 registers, 2 CTAs per SM), else 4 / 2 / 1
     s.P = forceP ? forceP : (n_pts >= 8 * kSigThreads && max_P >= 8 ? 8 : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1)));
     if (s.P != 1 && s.P != 2 && s.P != 4 && s.P != 8) s.P = 1;
-    s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
-    const int per_sm = env_int("BLOCH_SIGNAL_CTAS_PER_SM", 4);
+    // a readout of fewer than 256 samples (Cartesian lines) gets CTAs of just enough warps and more of them per SM,
+    // so that the spins are split over all lanes instead of leaving 256 - n_pts threads of every CTA idle
+    s.threads = kSigThreads;
+    if (s.P == 1 && n_pts < kSigThreads && !env_int("BLOCH_SIGNAL_FIXED_CTA", 0))
+        s.threads = (int)std::max<int64_t>(32, (n_pts + 31) / 32 * 32);
+    s.ptiles = (int)((n_pts + (int64_t)s.threads * s.P - 1) / ((int64_t)s.threads * s.P));
+    const int per_sm = std::min(env_int("BLOCH_SIGNAL_CTAS_PER_SM", 4) * (kSigThreads / s.threads), 12);
     const int64_t target = (int64_t)sm_count * per_sm;
     int64_t chunks = (target + s.ptiles - 1) / s.ptiles;
     const int64_t max_chunks = (n_spins + 31) / 32;
@@ -615,7 +621,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                         const Block &c = plan->blocks[bj];
                         if (c.type != kBlockPrecession || c.adc_count == 0) continue;
                         const SigShape sc = sig_shape(c.adc_count, n, sms, sig_max_P(plan));
-                        if (sc.P != s.P || sc.chunks != s.chunks || sc.spins_per_chunk != s.spins_per_chunk) break;
+                        if (sc.P != s.P || sc.chunks != s.chunks || sc.spins_per_chunk != s.spins_per_chunk ||
+                            sc.threads != s.threads) break;
                         if (batch_pts + c.adc_count > cap_pts || batch_pts + c.adc_count > INT32_MAX) break;
                         batch_pts += c.adc_count;
                     }
@@ -624,7 +631,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                 const dim3 grid(s.ptiles, s.chunks);
                 const int row = (int)batch_pts, poff = (int)batch_done;
 #define BLOCH_LAUNCH_SIG3(PP, H, M, AP, VP)                                                                    \
-    signal_kernel<PP, H, M><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, VP, w.S, n, s.spins_per_chunk,  \
+    signal_kernel<PP, H, M><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, VP, w.S, n, s.spins_per_chunk,    \
                                                               (const float *)w.scal, w.partial, row, poff)
 #define BLOCH_LAUNCH_SIG(PP)                                                                                   \
     do {                                                                                                       \

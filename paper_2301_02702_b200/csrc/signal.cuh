@@ -76,7 +76,7 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         if (n_tiles > 1) issue(1);
     }
     // the thread's P points are ADJACENT ADC samples, so tau_j - tau_0 is a few dwell times
-    const int p0 = (blockIdx.x * kSigThreads + tid) * P;
+    const int p0 = (blockIdx.x * (int)blockDim.x + tid) * P;  // blockDim.x < kSigThreads for blocks of few samples
     real kx[P], ky[P], kz[P], tau[P], ux[MO ? P : 1], uy[MO ? P : 1], uz[MO ? P : 1];
     float tf[P], cj[P], ar[P], ai[P];
     float cmax = 0.f;

@@ -110,9 +110,10 @@ def test_rf_on_gradient_ramps_and_changing_step_length(B, oracle_mod):
     check(B, oracle_mod, rand_phantom(333, 6), s, "RF on ramps, mixed dt")
 
 
-@pytest.mark.parametrize("n_adc", [1, 5, 300, 700, 1023, 2049, 2300])
+@pytest.mark.parametrize("n_adc", [1, 5, 40, 100, 200, 300, 700, 1023, 2049, 2300])
 def test_signal_launch_shapes_and_ragged_tails(B, oracle_mod, n_adc):
-    """n_adc selects P = 1 (< 512 points), 2 (< 1024), 4 (< 2048) or 8 and leaves ragged point tiles; 1111 spins leave a
+    """n_adc selects the CTA size (32 ... 256 threads below 256 points), P = 1 (< 512 points), 2 (< 1024), 4 (< 2048) or 8
+    and leaves ragged point tiles; 1111 spins leave a
     ragged spin tile."""
     rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 3) / (W.GAMMA * 1e-4)]), np.array([0.0]))
     g = {0: ([2e-4, 3e-4, 9e-3], [0, 4e-3, 4e-3]), 1: ([2e-4, 3e-4, 9e-3], [0, -2e-3, 1e-3])}
