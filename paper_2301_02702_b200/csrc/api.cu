@@ -145,8 +145,9 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp) {
     SigShape s;
     s.P = n_pts >= 2 * kSigThreads ? 2 : 1;
-    s.ptiles = (int)((n_pts + (int64_t)kSigThreads * s.P - 1) / ((int64_t)kSigThreads * s.P));
-    const int per_sm = ncp == 8 ? 2 : 4;  // resident CTAs per SM (96 / 64 registers)
+    s.threads = n_pts < kSigThreads ? (int)std::max<int64_t>(32, (n_pts + 31) / 32 * 32) : kSigThreads;  // as sig_shape
+    s.ptiles = (int)((n_pts + (int64_t)s.threads * s.P - 1) / ((int64_t)s.threads * s.P));
+    const int per_sm = std::min((ncp == 8 ? 2 : 4) * (kSigThreads / s.threads), 12);  // resident CTAs per SM (96 / 64 registers)
     int64_t chunks = ((int64_t)sm_count * per_sm + s.ptiles - 1) / s.ptiles;
     chunks = std::min<int64_t>(std::max<int64_t>(chunks, 1), std::min<int64_t>((n_spins + 31) / 32, 65535));
     chunks = std::max<int64_t>(chunks, 1);
@@ -591,7 +592,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     const int in_pass = std::min(ncp, n_coils - pass * ncp);
                     if (pass > 0 && (rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
 #define BLOCH_LAUNCH_COIL(PP, NCC, H, AP)                                                                           \
-    signal_coils_kernel<PP, NCC, H><<<grid, kSigThreads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk, \
+    signal_coils_kernel<PP, NCC, H><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk,   \
                                                                       (const float *)w.scal, w.partial)
 #define BLOCH_LAUNCH_COIL2(PP, NCC)                                \
     do {                                                           \

@@ -75,7 +75,7 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         if (n_tiles > 0) issue(0);
         if (n_tiles > 1) issue(1);
     }
-    const int p0 = (blockIdx.x * kSigThreads + tid) * P;
+    const int p0 = (blockIdx.x * (int)blockDim.x + tid) * P;  // blockDim.x < kSigThreads for blocks of few samples
     real kx[P], ky[P], kz[P], tau[P];
     float tf[P], cj[P], ar[NC][P], ai[NC][P];
     float cmax = 0.f;
