@@ -117,3 +117,54 @@ def test_random_sequences(B, oracle_mod, seed):
               f"max {emax:.3e} nrmse {nrmse:.3e}")
         assert g.shape == r.shape
         assert emax <= TOL_MAX and nrmse <= TOL_NRMSE
+
+
+@pytest.mark.parametrize("seed", range(12, 24))
+def test_random_sequences_whole_sequence_kernel_and_coils(B, oracle_mod, seed):
+    """The same random sequences on the paths added later: the whole-sequence kernel (forced where the planner's
+    phase choice is fp32, SUM_ALL; odd seeds from a supplied state) and multi-coil receive with 1-9 random smooth coil maps (per-block path, both
+    phase modes)."""
+    import torch
+    s, ph, state, vel, rng = random_case(seed)
+    n = ph.n
+    use_state = seed % 2 == 1
+    dev = B.phantom_to_device(ph)
+
+    def fresh_state():
+        if use_state:
+            return (torch.view_as_real(torch.from_numpy(state[0].astype(np.complex64)).cuda()).contiguous(),
+                    torch.from_numpy(state[1].astype(np.float32)).cuda())
+        return (torch.zeros(n, 2, dtype=torch.float32, device="cuda"), torch.zeros(n, dtype=torch.float32, device="cuda"))
+
+    def compare(what, g, r):
+        g = np.asarray(g, dtype=np.complex128)
+        scale = max(np.abs(r).max(), 1e-30)
+        d = np.abs(g - r)
+        emax, nrmse = d.max() / scale, np.sqrt(np.mean(d ** 2)) / scale
+        print(f"seed {seed} n={n} {what}: max {emax:.3e} nrmse {nrmse:.3e}")
+        assert g.shape == r.shape and emax <= TOL_MAX and nrmse <= TOL_NRMSE, what
+
+    # (1) whole-sequence kernel
+    ref, rxy, rz = oracle_mod.simulate(ph, s, state=state if use_state else None, return_state=True)
+    ref_state = np.concatenate([rxy, rz.astype(np.complex128)])
+    plan = B.Plan(s, path="fused")   # phase AUTO: 9 of the 12 sequences resolve to fp32, which the kernel needs
+    if plan.info["phase_mode"] == B.PHASE_FP32 and B.bloch_plan_uses_fused(plan.handle, n):
+        Mxy, Mz = fresh_state()
+        sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=not use_state)
+        torch.cuda.synchronize()
+        m = Mxy.cpu().numpy()
+        compare("fused signal", sig.cpu().numpy(), ref)
+        compare("fused state", np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)]), ref_state)
+    plan.close()
+    # (2) multi-coil receive
+    n_coils = int(rng.integers(1, 10))
+    cw = (rng.uniform(.2, 1, (n_coils, 1)) * np.exp(1j * (rng.uniform(-20, 20, (n_coils, 1)) * ph.x[None, :] +
+                                                        rng.uniform(-20, 20, (n_coils, 1)) * ph.y[None, :])) /
+          (1.0 + 30.0 * (ph.x[None, :] - rng.uniform(-.1, .1, (n_coils, 1))) ** 2)).astype(np.complex64)
+    refc = oracle_mod.simulate(ph, s, state=state if use_state else None, coils=cw.astype(np.complex128))
+    plan = B.Plan(s, phase_mode=["fp32", "fp64"][seed % 2])
+    Mxy, Mz = fresh_state()
+    sigc = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=not use_state, coils=torch.from_numpy(cw).cuda())
+    torch.cuda.synchronize()
+    plan.close()
+    compare(f"{n_coils} coils", sigc.cpu().numpy(), refc)
