@@ -126,15 +126,34 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     // ------------------------------------------------------------------ a1: merged grid
     std::vector<double> pts;
     pts.reserve(size_t(2 + seq->g_n[0] + seq->g_n[1] + seq->g_n[2] + 2 * seq->rf_n + seq->adc_n));
+    // every source is ascending on its own (validated above), so the union is a merge of sorted runs, not a sort
+    // (config 5: 5.1e6 points; std::sort took half of the planning time)
     pts.push_back(0.0);
     pts.push_back(seq->t_end);
-    for (int a = 0; a < 3; ++a) pts.insert(pts.end(), seq->g_t[a], seq->g_t[a] + seq->g_n[a]);
-    for (int64_t i = 0; i < seq->rf_n; ++i) {
-        pts.push_back(seq->rf_t[i]);
-        pts.push_back(seq->rf_t[i] + seq->rf_dt[i]);
+    auto merge_run = [&pts](size_t run_first) {
+        std::inplace_merge(pts.begin(), pts.begin() + (std::ptrdiff_t)run_first, pts.end());
+    };
+    for (int a = 0; a < 3; ++a) {
+        const size_t first = pts.size();
+        pts.insert(pts.end(), seq->g_t[a], seq->g_t[a] + seq->g_n[a]);
+        merge_run(first);
     }
-    pts.insert(pts.end(), seq->adc_t, seq->adc_t + seq->adc_n);
-    std::sort(pts.begin(), pts.end());
+    {
+        const size_t first = pts.size();
+        for (int64_t i = 0; i < seq->rf_n; ++i) {
+            pts.push_back(seq->rf_t[i]);
+            pts.push_back(seq->rf_t[i] + seq->rf_dt[i]);
+        }
+        // rf_t[i] + rf_dt[i] may exceed rf_t[i + 1] by rounding when samples abut: insertion pass over the run
+        for (size_t k = first + 1; k < pts.size(); ++k)
+            for (size_t m = k; m > first && pts[m] < pts[m - 1]; --m) std::swap(pts[m], pts[m - 1]);
+        merge_run(first);
+    }
+    {
+        const size_t first = pts.size();
+        pts.insert(pts.end(), seq->adc_t, seq->adc_t + seq->adc_n);
+        merge_run(first);
+    }
     std::vector<double> coarse;
     coarse.reserve(pts.size());
     for (double t : pts) {
