@@ -230,8 +230,8 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
  *       Available for SUM_ALL output (and for PER_SPIN plans whose blocks hold at most 16 ADC samples: dictionary
  *       mode), fp32 phase, no motion and at most 29 x 32 spins per SM; bloch_simulate
  *       returns BLOCH_EINVAL when it is forced and not available.
- *   BLOCH_PATH_AUTO (default): FUSED when available, 4 N_rf >= N_adc and at most 21 x 32 spins per SM (the full set
- *       of signal warps fits beside the RF warps), else PER_BLOCK.
+ *   BLOCH_PATH_AUTO (default): FUSED when available, 4 N_rf >= N_adc and the signal warps of the balanced layout fit
+ *       beside the RF warps (up to about 20 x 32 spins per SM), else PER_BLOCK.
  * Both paths compute the same thing; the final magnetisation is bitwise identical, the signal differs only in
  * the order of the fixed-order sums.  Set before bloch_plan_workspace_bytes: the workspace size depends on it. */
 enum { BLOCH_PATH_AUTO = 0, BLOCH_PATH_PER_BLOCK = 1, BLOCH_PATH_FUSED = 2 };

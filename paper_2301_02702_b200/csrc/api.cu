@@ -104,6 +104,7 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
 struct SeqShape {
     bool ok, use;
     int n_ctas, chunk, rf_warps, sig_warps, threads, min_items;
+    SeqRoles roles;
     size_t smem, partial_elems;
 };
 constexpr size_t kSeqPartialCapBytes = size_t(8) << 30;
@@ -121,12 +122,58 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     const int64_t per_sm = (n_spins + sm_count - 1) / sm_count;
     q.chunk = (int)std::max<int64_t>(32, (per_sm + 31) / 32 * 32);
     q.rf_warps = q.chunk / 32;
-    // 10 signal warps: measured optimum on config 5 (14 RF warps per SM; 4: 168 ms, 8: 133, 10: 129.5, 16: 141)
-    const int want = std::min(std::max(env_int("BLOCH_SEQ_SIGNAL_WARPS", 10), 1), 30);
-    q.sig_warps = ps ? 0 : std::min(want, kSeqMaxThreads / 32 - 1 - q.rf_warps);
-    if (ps ? q.rf_warps > kSeqMaxThreads / 32 - 1 : q.sig_warps < std::min(want, 2))
+    // Roles per warp.  A warp runs on SM sub-partition (warp id mod 4); the RF warps are spread as evenly as they go
+    // (the producer's sub-partition 0 takes an extra one last) and every sub-partition gets sig_base signal warps plus
+    // sig_extra for every RF warp it holds fewer than the fullest one, so that all four carry about the same load.
+    // Measured on config 5 (14 RF warps: 3,4,4,3): signal warps 3,1,1,3 124.1 ms; 3,2,2,3 125.9; 2,1,1,2 128.4;
+    // 1,1,1,1 144.8; 2,2,2,2 133.6; 5,1,1,5 127.0.  Default: two extra per missing RF warp, and a base that brings the
+    // total to about 0.6 signal warps per RF warp.
+    int rf_per[4], sig_per[4], cnt_per[4];
+    for (int k = 0; k < 4; ++k) rf_per[k] = q.rf_warps / 4;
+    { const int order[4] = {1, 2, 3, 0}; for (int e = 0; e < q.rf_warps % 4; ++e) ++rf_per[order[e]]; }
+    const int rf_max = *std::max_element(rf_per, rf_per + 4);
+    const int sig_extra = std::min(std::max(env_int("BLOCH_SEQ_SIG_EXTRA", 2), 0), 7);
+    int deficit = 0;
+    for (int k = 0; k < 4; ++k) deficit += rf_max - rf_per[k];
+    const int target = std::max(4, (6 * q.rf_warps + 5) / 10);
+    const int auto_base = std::max(1, (target - sig_extra * deficit + 2) / 4);
+    const int sig_base = std::min(std::max(env_int("BLOCH_SEQ_SIG_BASE", auto_base), 0), 7);
+    auto total_warps = [&](int base, int extra) {
+        int top = 0;
+        for (int k = 0; k < 4; ++k) {
+            sig_per[k] = ps ? 0 : base + extra * (rf_max - rf_per[k]);
+            cnt_per[k] = rf_per[k] + sig_per[k] + (k == 0 ? 1 : 0);
+            if (cnt_per[k] > 0) top = std::max(top, (cnt_per[k] - 1) * 4 + k + 1);
+        }
+        return top;
+    };
+    int base = sig_base, extra = sig_extra;
+    while (total_warps(base, extra) > kSeqMaxThreads / 32 && (extra > 0 || base > 0)) {
+        if (base > 2) --base;          // give up base warps down to two per sub-partition first,
+        else if (extra > 0) --extra;   // then the balancing extras,
+        else --base;                   // then the rest
+    }
+    const int n_warps = total_warps(base, extra);
+    // AUTO wants the whole set of signal warps, or at least two per sub-partition next to the balancing extras
+    // (20 RF warps: 18.1 ms with 2 per sub-partition against 19.2 per-block and 21.4 with 1)
+    const bool full_layout = (base == sig_base || base >= 2) && extra == sig_extra;
+    q.sig_warps = sig_per[0] + sig_per[1] + sig_per[2] + sig_per[3];
+    if (n_warps > kSeqMaxThreads / 32 || (!ps && q.sig_warps < 1))
         return q;  // no room beside the RF warps: more than 29 x 32 spins per SM (31 x 32 for PER_SPIN)
-    q.threads = 32 * (1 + q.rf_warps + q.sig_warps);
+    {
+        int rf_next = 0;
+        for (int w = 0; w < kSeqMaxThreads / 32; ++w) q.roles.role[w] = (signed char)kRoleIdle;
+        for (int k = 0; k < 4; ++k) {
+            int slot = k;
+            if (k == 0) { q.roles.role[slot] = (signed char)kRoleProducer; slot += 4; }
+            for (int r = 0; r < rf_per[k]; ++r, slot += 4) q.roles.role[slot] = (signed char)0;  // index set below
+            for (int g = 0; g < sig_per[k]; ++g, slot += 4) q.roles.role[slot] = (signed char)kRoleSignal;
+        }
+        for (int w = 0; w < n_warps; ++w)
+            if (q.roles.role[w] == 0) q.roles.role[w] = (signed char)rf_next++;
+        q.roles.n_sig_warps = q.sig_warps;
+    }
+    q.threads = 32 * n_warps;
     q.min_items = std::max(1, q.sig_warps * env_int("BLOCH_SEQ_ITEMS_PER_WARP_X4", 0) / 4);  // 0: always the largest P (config 5: 127.6 ms against 131.1 with one item per warp)
     q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
     q.smem = seq_smem_bytes(q.chunk);
@@ -137,7 +184,7 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     // fits beside the RF warps (its readout runs on sig_warps warps per SM only).  Measured, fused / per-block ms:
     // N_rf/N_adc = 0.98: 13.1 / 15.5 at 65,536 spins, 42.1 / 29.4 at 131,044 (3 signal warps left);
     // 0.49: 5.97 / 6.17 at 65,536, 22.2 / 11.3 at 131,072;  0.06: 1.05 / 0.84 at 65,522.
-    q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || q.sig_warps >= want));
+    q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || full_layout));
     return q;
 }
 
@@ -502,11 +549,11 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         const SeqOp *prog = reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off);
         if (per_spin)
             seq_kernel<true><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
-                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items,
+                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.roles, sq.min_items,
                 (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, (float2 *)d_signal);
         else
             seq_kernel<false><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
-                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.min_items,
+                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.roles, sq.min_items,
                 (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, nullptr);
         ++launches;
         if (plan->info.n_adc > 0 && !per_spin) {

@@ -39,6 +39,15 @@ constexpr int kSeqTileStride = 4224;  // >= kRfHdrBytes + kRfTileSteps * 32 (sta
 constexpr int kSeqMaxThreads = 1024;
 constexpr int kSeqStateBufs = 4;
 constexpr int kSeqBarBytes = 256;
+
+// Role of each warp of the CTA, chosen on the host (api.cu seq_shape) so that every SM sub-partition (warp id mod 4)
+// carries about the same load: >= 0: RF warp with that index (spins 32 i .. 32 i + 31 of the chunk), -1: producer,
+// -2: signal warp, -3: idle (exits at once).
+struct SeqRoles {
+    signed char role[kSeqMaxThreads / 32];
+    int n_sig_warps;
+};
+constexpr int kRoleProducer = -1, kRoleSignal = -2, kRoleIdle = -3;
 static_assert(kSeqTileStride >= kRfHdrBytes + kRfTileSteps * 32 && kSeqTileStride % 128 == 0, "tile stride");
 
 // dynamic shared memory: [ring: kSeqStages x kSeqTileStride][barriers + item counters: 256 B][shA: chunk float4]
@@ -139,7 +148,7 @@ template <bool PS>
 __global__ void __launch_bounds__(kSeqMaxThreads, 1)
 seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ ops, int n_ops,
            const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n, int chunk,
-           int rf_warps, int min_items, const float *__restrict__ scal, float2 *__restrict__ partial,
+           int rf_warps, SeqRoles roles, int min_items, const float *__restrict__ scal, float2 *__restrict__ partial,
            long long n_adc, int final_state, float2 *__restrict__ out_ps /* PER_SPIN plans: out[spin][adc], else NULL */) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *ring = smem;
@@ -151,7 +160,8 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
     float4 *shS = shA + chunk;  // [kSeqStateBufs][chunk]
     const int tid = threadIdx.x, warp = tid >> 5;
     const int n_rf_thr = rf_warps * 32;
-    const int nsig = (int)blockDim.x - 32 - n_rf_thr;
+    const int nsig = roles.n_sig_warps * 32;
+    const int my_role = roles.role[warp];
     const int s0 = blockIdx.x * chunk;
     const int cnt = min(chunk, n - s0);
     if (tid == 0) {
@@ -167,10 +177,11 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
         mbar_init_fence();
     }
     __syncthreads();  // the only CTA-wide barrier: from here on the roles meet at mbarriers
+    if (my_role == kRoleIdle) return;
 
-    if (warp == 0) {
+    if (my_role == kRoleProducer) {
         // ---------------------------------------------------------------- producer
-        if (tid != 0) return;
+        if ((tid & 31) != 0) return;
         int g = 0;
         for (int oi = 0; oi < n_ops; ++oi) {
             const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
@@ -188,9 +199,9 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
         return;
     }
 
-    if (warp <= rf_warps) {
+    if (my_role >= 0) {
         // ---------------------------------------------------------------- RF warps: one spin per thread
-        const int r = tid - 32;
+        const int r = my_role * 32 + (tid & 31);
         const bool active = r < cnt;
         const int i = s0 + r;
         float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f),

@@ -50,9 +50,9 @@ def test_auto_picks_fused_only_where_it_qualifies(B):
     assert not uses(phase_mode="fp32", output_mode="per_spin")
     assert not uses(n_spins=1_000_000, phase_mode="fp32")          # more than 29 warps of spins per SM
     assert not uses(n_spins=1_000_000, phase_mode="fp32", path="fused")
-    # 131,072 spins = 28 RF warps per SM leave 3 signal warps: allowed when forced, not what AUTO picks
-    assert not uses(n_spins=131_072, phase_mode="fp32")
-    assert uses(n_spins=131_072, phase_mode="fp32", path="fused")
+    # 120,000 spins = 26 RF warps per SM leave room for 4 signal warps only: allowed when forced, not what AUTO picks
+    assert not uses(n_spins=120_000, phase_mode="fp32")
+    assert uses(n_spins=120_000, phase_mode="fp32", path="fused")
     # readout-heavy sequence (config 1: 50 RF steps, 1024 ADC samples): AUTO stays per-block, FUSED can be forced
     w1 = W.small("1")
     p = B.Plan(w1.seq, phase_mode="fp32")
@@ -100,11 +100,12 @@ def test_fused_is_bitwise_reproducible_and_independent_of_the_signal_warp_count(
     assert np.array_equal(a.view(np.float32), b.view(np.float32)), "run-to-run not bitwise identical"
     # the partial of a CTA is one thread's sum over the chunk's spins in index order whatever the number of signal
     # warps (only which thread owns which sample changes; the P = 1/2/4 choice moves with it, hence a tolerance)
-    for nw in ("1", "3", "16"):
-        monkeypatch.setenv("BLOCH_SEQ_SIGNAL_WARPS", nw)
+    for base, extra in (("1", "0"), ("0", "1"), ("3", "2"), ("5", "0")):
+        monkeypatch.setenv("BLOCH_SEQ_SIG_BASE", base)
+        monkeypatch.setenv("BLOCH_SEQ_SIG_EXTRA", extra)
         c = run_gpu(B, w, path="fused", phase_mode="fp32")
         emax, _ = errors(c, a)
-        assert emax < 2e-6, f"{nw} signal warps: {emax:.3e}"
+        assert emax < 2e-6, f"signal warps base {base} extra {extra}: {emax:.3e}"
 
 
 def test_fused_supplied_state_precession_first_and_no_adc(B, oracle_mod):
@@ -193,11 +194,11 @@ def test_fused_per_spin_dictionary_mode(B, oracle_mod):
 
 def test_fused_is_race_free_over_many_runs(B, monkeypatch):
     """The roles of the whole-sequence kernel meet only at mbarriers; a missing edge would show up as run-to-run
-    differences.  25 runs each with 2, 5 and 10 signal warps (different interleavings of the roles), all bitwise equal
+    differences.  25 runs each with 1, 2 and 3 signal warps per sub-partition (plus the balancing extras) (different interleavings of the roles), all bitwise equal
     per configuration, signal and final state."""
     w = W.small("5")
-    for nw in ("2", "5", "10"):
-        monkeypatch.setenv("BLOCH_SEQ_SIGNAL_WARPS", nw)
+    for nw in ("1", "2", "3"):
+        monkeypatch.setenv("BLOCH_SEQ_SIG_BASE", nw)
         first = None
         for _ in range(25):
             sig, mxy, mz = run_gpu(B, w, want_state=True, path="fused", phase_mode="fp32")
