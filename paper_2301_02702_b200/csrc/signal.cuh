@@ -38,8 +38,10 @@ constexpr int kSigTile = 256;  // spins per staged tile
 
 // MO (motion plans): every record (k', tau) is followed by (mu', 0), the spins' velocities are a third staged
 // tile, and the phase gains mu' . v (x(t) = x + v t).
+// fp32 phase, static plans: held to 64 registers (P <= 4: 4 CTAs per SM) or 85 (P = 8: 3 CTAs per SM); ptxas otherwise
+// drifts to 72 / 100 registers and loses a resident CTA
 template <int P, bool PH64, bool MO>
-__global__ void __launch_bounds__(kSigThreads)
+__global__ void __launch_bounds__(kSigThreads, (PH64 || MO) ? 1 : (P == 8 ? 3 : 4))
 signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_, const void *__restrict__ V_,
               const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
               const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial,
