@@ -9,6 +9,7 @@
 #include "internal.h"
 #include "kernels.cuh"
 #include "coils.cuh"
+#include "coils_tc.cuh"
 #include "rf.cuh"
 #include "seq.cuh"
 #include "signal.cuh"
@@ -189,7 +190,25 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 }
 
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
-SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp) {
+// tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 256 threads, 2 CTAs per SM, chunks of whole 16-spin stages
+bool coil_use_tc(const bloch_plan *plan, int n_coils) {
+    return coils_per_pass(n_coils) == 8 && plan->info.phase_mode == BLOCH_PHASE_FP32 && env_int("BLOCH_COIL_TC", 0) != 0;  // opt-in: correct, not yet faster than the FFMA kernel
+}
+
+SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp, bool tc) {
+    if (tc) {
+        SigShape s;
+        s.P = 1;
+        s.threads = 256;
+        s.ptiles = (int)((n_pts + kTcM - 1) / kTcM);
+        int64_t chunks = std::max<int64_t>(1, ((int64_t)sm_count * 2) / s.ptiles);  // one wave of 2 CTAs per SM
+        chunks = std::min<int64_t>(chunks, std::max<int64_t>(1, (n_spins + 255) / 256));
+        chunks = std::min<int64_t>(chunks, 65535);
+        const int64_t per = (n_spins + chunks - 1) / chunks;
+        s.spins_per_chunk = (int)std::max<int64_t>(kTcStageSpins, (per + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins);
+        s.chunks = (int)std::max<int64_t>(1, (n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
+        return s;
+    }
     SigShape s;
     s.P = n_pts >= 2 * kSigThreads ? 2 : 1;
     s.threads = n_pts < kSigThreads ? (int)std::max<int64_t>(32, (n_pts + 31) / 32 * 32) : kSigThreads;  // as sig_shape
@@ -203,11 +222,11 @@ SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp) {
     return s;
 }
 
-size_t coil_partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count, int ncp) {
+size_t coil_partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count, int ncp, bool tc) {
     size_t worst = 1;
     for (const Block &b : plan->blocks) {
         if (b.type != kBlockPrecession || b.adc_count == 0) continue;
-        const SigShape s = coil_shape(b.adc_count, n_spins, sm_count, ncp);
+        const SigShape s = coil_shape(b.adc_count, n_spins, sm_count, ncp, tc);
         worst = std::max(worst, size_t(ncp) * size_t(s.chunks) * size_t(b.adc_count));
     }
     return worst;
@@ -264,14 +283,19 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
         const SeqShape q = seq_shape(plan, n_spins, sm_count);
-        if (n_coils > 0) w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, coils_per_pass(n_coils));
+        if (n_coils > 0)
+            w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, coils_per_pass(n_coils), coil_use_tc(plan, n_coils));
         else w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
     const int ncp = coils_per_pass(n_coils);
     const size_t n_pass = size_t((n_coils + ncp - 1) / ncp);
-    w.W = n_coils > 0 ? (float2 *)take(n_pass * size_t(n_spins) * ncp * sizeof(float2)) : nullptr;
+    // the tcgen05 kernel takes its weights as ready-made B tiles: 2048 B per 8 spins (spins padded to whole stages)
+    const size_t n_pad = (size_t(n_spins) + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
+    const size_t w_bytes = (n_coils > 0 && coil_use_tc(plan, n_coils)) ? n_pass * (n_pad / 8) * kTcBGroup
+                                                                       : n_pass * size_t(n_spins) * ncp * sizeof(float2);
+    w.W = n_coils > 0 ? (float2 *)take(w_bytes) : nullptr;
     w.bytes = off;
     return w;
 }
@@ -526,7 +550,18 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     ++launches;
     const int ncp = coils_per_pass(n_coils);
     const int n_pass = (n_coils + ncp - 1) / ncp;
-    if (n_coils > 0) {
+    const bool tc = n_coils > 0 && coil_use_tc(plan, n_coils);
+    const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
+    if (tc) {
+        static bool tc_attr = false;
+        if (!tc_attr) {
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+            tc_attr = true;
+        }
+        pack_coils_tc_kernel<<<dim3((n_pad + 255) / 256, n_pass), 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil,
+                                                                                    (unsigned char *)w.W);
+        ++launches;
+    } else if (n_coils > 0) {
         pack_coils_kernel<<<dim3((n + 255) / 256, n_pass), 256, 0, stream>>>(n, n_coils, ncp, (const float2 *)d_coil, w.W);
         ++launches;
     }
@@ -632,7 +667,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                                     (float2 *)d_signal);
                 ++launches;
             } else if (n_coils > 0) {
-                const SigShape s = coil_shape(n_pts, n, sms, ncp);
+                const SigShape s = coil_shape(n_pts, n, sms, ncp, tc);
                 const dim3 grid(s.ptiles, s.chunks);
                 for (int pass = 0; pass < n_pass; ++pass) {
                     const float4 *Wp = reinterpret_cast<const float4 *>(w.W + (size_t)pass * n * ncp);
@@ -646,7 +681,12 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, w.Ad);          \
         else BLOCH_LAUNCH_COIL(PP, NCC, false, w.A);               \
     } while (0)
-                    if (ncp == 8) { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 8); else BLOCH_LAUNCH_COIL2(1, 8); }
+                    if (tc)
+                        signal_coils_tc_kernel<<<grid, kTcThreads, kTcSmemBytes, stream>>>(
+                            (const float4 *)recs, n_pts, w.A, w.S,
+                            (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * kTcBGroup, n, s.spins_per_chunk,
+                            (const float *)w.scal, w.partial);
+                    else if (ncp == 8) { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 8); else BLOCH_LAUNCH_COIL2(1, 8); }
                     else { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 4); else BLOCH_LAUNCH_COIL2(1, 4); }
 #undef BLOCH_LAUNCH_COIL2
 #undef BLOCH_LAUNCH_COIL

@@ -118,3 +118,23 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
     assert h.shape == (6, w.seq.adc_t.size)
     assert np.array_equal(h.view(np.float32), dev_sig.view(np.float32)), "host-buffer coil entry differs from device entry"
     assert np.abs(mz).max() > 0.1
+
+
+@pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11)])
+def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, monkeypatch, name, n_coils):
+    """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with BLOCH_COIL_TC=1): contributions generated on the fly
+    as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
+    tiles (n_adc not a multiple of 128), ragged 16-spin stages and two passes of 8 coils are all in these cases."""
+    monkeypatch.setenv("BLOCH_COIL_TC", "1")
+    w = W.small(name)
+    coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
+    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32")
+    assert_parity(got, ref, f"tensor-core coil kernel, config {name}, {n_coils} coils")
+    for c in range(n_coils):
+        emax, nrmse = errors(got[c], ref[c])
+        assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
+    monkeypatch.setenv("BLOCH_COIL_TC", "0")
+    ffma = run_coils(B, w, coils, phase_mode="fp32")
+    emax, _ = errors(got, ffma)
+    assert emax < 2e-5, f"tensor-core vs FFMA kernel: {emax:.3e}"   # TMEM accumulation is coarser than FFMA sums
