@@ -404,7 +404,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 5, 5b, 5c (ensemble dictionary)")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary)")
     ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
                     help="execution path (bloch_plan_set_path); auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -192,7 +192,12 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
 // tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 256 threads, 2 CTAs per SM, chunks of whole 16-spin stages
 bool coil_use_tc(const bloch_plan *plan, int n_coils) {
-    return coils_per_pass(n_coils) == 8 && plan->info.phase_mode == BLOCH_PHASE_FP32 && env_int("BLOCH_COIL_TC", 0) != 0;  // opt-in: correct, not yet faster than the FFMA kernel
+    // BLOCH_COIL_TC: 0 = never, 1 = whenever it applies (more than 4 coils, fp32 phase), unset = when it pays: more
+    // than 8 coils (16 coils per pass cost what 8 cost: config 4 with 32 coils 260 ms against 486 ms for the FFMA
+    // kernel; with 8 coils 129.5 against 121.4)
+    const int mode = env_int("BLOCH_COIL_TC", -1);
+    if (mode == 0 || n_coils <= 4 || plan->info.phase_mode != BLOCH_PHASE_FP32) return false;
+    return mode == 1 || n_coils > 8;
 }
 
 SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp, bool tc) {
@@ -283,17 +288,20 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
         const SeqShape q = seq_shape(plan, n_spins, sm_count);
-        if (n_coils > 0)
-            w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, coils_per_pass(n_coils), coil_use_tc(plan, n_coils));
+        if (n_coils > 0) {
+            const bool tc_ = coil_use_tc(plan, n_coils);
+            w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, tc_ ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils), tc_);
+        }
         else w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
-    const int ncp = coils_per_pass(n_coils);
+    const bool tc_ws = n_coils > 0 && coil_use_tc(plan, n_coils);
+    const int ncp = tc_ws ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const size_t n_pass = size_t((n_coils + ncp - 1) / ncp);
     // the tcgen05 kernel takes its weights as ready-made B tiles: 2048 B per 8 spins (spins padded to whole stages)
     const size_t n_pad = (size_t(n_spins) + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
-    const size_t w_bytes = (n_coils > 0 && coil_use_tc(plan, n_coils)) ? n_pass * (n_pad / 8) * kTcBGroup
+    const size_t w_bytes = tc_ws ? n_pass * (n_pad / 8) * tc_bgroup(ncp)
                                                                        : n_pass * size_t(n_spins) * ncp * sizeof(float2);
     w.W = n_coils > 0 ? (float2 *)take(w_bytes) : nullptr;
     w.bytes = off;
@@ -548,18 +556,20 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
-    const int ncp = coils_per_pass(n_coils);
-    const int n_pass = (n_coils + ncp - 1) / ncp;
     const bool tc = n_coils > 0 && coil_use_tc(plan, n_coils);
+    const int ncp = tc ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
+    const int n_pass = (n_coils + ncp - 1) / ncp;
     const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
     if (tc) {
         static bool tc_attr = false;
         if (!tc_attr) {
-            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(8)));
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(16)));
             tc_attr = true;
         }
-        pack_coils_tc_kernel<<<dim3((n_pad + 255) / 256, n_pass), 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil,
-                                                                                    (unsigned char *)w.W);
+        const dim3 pg((n_pad + 255) / 256, n_pass);
+        if (ncp == 16) pack_coils_tc_kernel<16><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
+        else pack_coils_tc_kernel<8><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
         ++launches;
     } else if (n_coils > 0) {
         pack_coils_kernel<<<dim3((n + 255) / 256, n_pass), 256, 0, stream>>>(n, n_coils, ncp, (const float2 *)d_coil, w.W);
@@ -681,11 +691,15 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, w.Ad);          \
         else BLOCH_LAUNCH_COIL(PP, NCC, false, w.A);               \
     } while (0)
-                    if (tc)
-                        signal_coils_tc_kernel<<<grid, kTcThreads, kTcSmemBytes, stream>>>(
-                            (const float4 *)recs, n_pts, w.A, w.S,
-                            (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * kTcBGroup, n, s.spins_per_chunk,
-                            (const float *)w.scal, w.partial);
+                    if (tc) {
+                        const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
+                        if (ncp == 16)
+                            signal_coils_tc_kernel<16><<<grid, kTcThreads, tc_smem(16), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, (const float *)w.scal, w.partial);
+                        else
+                            signal_coils_tc_kernel<8><<<grid, kTcThreads, tc_smem(8), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, (const float *)w.scal, w.partial);
+                    }
                     else if (ncp == 8) { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 8); else BLOCH_LAUNCH_COIL2(1, 8); }
                     else { if (s.P == 2) BLOCH_LAUNCH_COIL2(2, 4); else BLOCH_LAUNCH_COIL2(1, 4); }
 #undef BLOCH_LAUNCH_COIL2

@@ -30,11 +30,13 @@ constexpr int kTcStageSpins = 16;     // spins per stage
 constexpr int kTcGroups = kTcStageSpins / 8;
 constexpr int kTcSlots = 4;           // TMA ring: spin records + B tiles
 constexpr int kTcATile = kTcM * 32;   // one A tile: 128 rows x 8 TF32 = 4096 B
-constexpr int kTcBTile = 16 * 32;     // one B tile: 16 rows x 8 TF32 = 512 B
-constexpr int kTcBGroup = 4 * kTcBTile;  // per 8-spin group: cr-part hi, cr-part lo, ci-part hi, ci-part lo
-constexpr int kTcSlotBytes = kTcStageSpins * 32 + kTcGroups * kTcBGroup;  // spin records (A, S) + B tiles = 4608
+// NC = coils per pass (8 or 16): N = 2 NC columns (re | im)
+__host__ __device__ constexpr int tc_btile(int nc) { return 2 * nc * 32; }     // one B tile: 2 NC rows x 8 TF32
+__host__ __device__ constexpr int tc_bgroup(int nc) { return 4 * tc_btile(nc); }  // per 8-spin group: cr hi, cr lo, ci hi, ci lo
+__host__ __device__ constexpr int tc_slot(int nc) { return kTcStageSpins * 32 + kTcGroups * tc_bgroup(nc); }  // spin records + B tiles
 constexpr int kTcAStage = kTcGroups * 4 * kTcATile;                       // 32 KB
-constexpr size_t kTcSmemBytes = 2 * (size_t)kTcAStage + kTcSlots * (size_t)kTcSlotBytes + 256;
+__host__ __device__ constexpr size_t tc_smem(int nc) { return 2 * (size_t)kTcAStage + kTcSlots * (size_t)tc_slot(nc) + 256; }
+__host__ __device__ inline int tc_coils_per_pass(int n_coils) { return n_coils > 8 ? 16 : 8; }
 
 __device__ __forceinline__ uint32_t tc_tf32(float x) {
     uint32_t r;
@@ -43,22 +45,24 @@ __device__ __forceinline__ uint32_t tc_tf32(float x) {
 }
 
 // Weights -> B tiles.  Bt[pass][group][part][512 B], group = spin / 8 over the spins padded to a multiple of 16.
+template <int NC>
 __global__ void __launch_bounds__(256)
 pack_coils_tc_kernel(int n, int n_pad, int n_coils, const float2 *__restrict__ coil, unsigned char *__restrict__ Bt) {
+    constexpr int kTcBTile = tc_btile(NC), kTcBGroup = tc_bgroup(NC);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;  // spin (padded range)
     const int pass = blockIdx.y;
     if (i >= n_pad) return;
     unsigned char *grp = Bt + ((size_t)pass * (n_pad / 8) + (size_t)(i / 8)) * kTcBGroup;
     const int k = i & 7;
-    for (int c = 0; c < 8; ++c) {
-        const int cc = pass * 8 + c;
+    for (int c = 0; c < NC; ++c) {
+        const int cc = pass * NC + c;
         float2 w = make_float2(0.f, 0.f);
         if (i < n && cc < n_coils) w = coil[(size_t)cc * n + i];
         // column n of the stacked B: cr-part [Wr | Wi], ci-part [-Wi | Wr]
-        const float vals[2][2] = {{w.x, w.y}, {-w.y, w.x}};  // [part cr/ci][n < 8 / n >= 8]
+        const float vals[2][2] = {{w.x, w.y}, {-w.y, w.x}};  // [part cr/ci][n < NC / n >= NC]
         for (int part = 0; part < 2; ++part)
             for (int hi8 = 0; hi8 < 2; ++hi8) {
-                const int nn = c + 8 * hi8;
+                const int nn = c + NC * hi8;
                 const float x = vals[part][hi8];
                 const uint32_t h = tc_tf32(x);
                 const uint32_t l = tc_tf32(x - __uint_as_float(h));
@@ -74,25 +78,31 @@ __device__ __forceinline__ uint64_t tc_desc(uint32_t smem_addr) {
     return (uint64_t)((smem_addr >> 4) & 0x3fffu) | ((uint64_t)(128u >> 4) << 16) | ((uint64_t)(256u >> 4) << 32) |
            ((uint64_t)1 << 46);
 }
-// instruction descriptor: D = F32, A = B = TF32, both K-major, N = 16, M = 128
-constexpr uint32_t kTcIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
+// instruction descriptor: D = F32, A = B = TF32, both K-major, N columns, M = 128
+__host__ __device__ constexpr uint32_t tc_idesc(int n) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+}
 
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t accumulate) {
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
-        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(kTcIdesc), "r"(accumulate) : "memory");
+        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 
 constexpr int kTcThreads = 288;  // 8 generator warps + 1 control warp (TMA + MMA issue by its lane 0)
 
+template <int NC>
 __global__ void __launch_bounds__(kTcThreads, 2)
 signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *__restrict__ A,
                        const float4 *__restrict__ S, const unsigned char *__restrict__ Bt /* this pass */,
                        int n_spins, int spins_per_chunk /* multiple of 16 */, const float *__restrict__ scal,
-                       float2 *__restrict__ partial /* [8][chunks][n_pts] */) {
+                       float2 *__restrict__ partial /* [NC][chunks][n_pts] */) {
+    constexpr int kTcBTile = tc_btile(NC), kTcBGroup = tc_bgroup(NC), kTcSlotBytes = tc_slot(NC);
+    constexpr uint32_t kIdesc = tc_idesc(2 * NC);
+    constexpr int kCols = 2 * NC < 32 ? 32 : 2 * NC;  // TMEM columns (power of two >= 32)
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *a_tiles = smem;                                  // [2][groups][4 parts][4096]
     unsigned char *slots = smem + 2 * kTcAStage;                    // [kTcSlots][spin A (256 B) | spin S (256 B) | B tiles]
@@ -124,7 +134,7 @@ signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 
     }
     if (warp == 0) {  // TMEM: 32 columns (128 lanes x 16 FP32 columns used)
         __syncwarp();
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kCols) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -147,12 +157,12 @@ signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 
                 for (int gq = 0; gq < kTcGroups; ++gq) {
                     const uint32_t ag = a0 + gq * (4 * kTcATile), bg = b0 + gq * kTcBGroup;
                     const uint32_t first = (st == 0 && gq == 0) ? 0u : 1u;
-                    tc_mma(tmem, tc_desc(ag + 0 * kTcATile), tc_desc(bg + 0 * kTcBTile), first);  // cr hi x B hi
-                    tc_mma(tmem, tc_desc(ag + 1 * kTcATile), tc_desc(bg + 0 * kTcBTile), 1u);     // cr lo x B hi
-                    tc_mma(tmem, tc_desc(ag + 0 * kTcATile), tc_desc(bg + 1 * kTcBTile), 1u);     // cr hi x B lo
-                    tc_mma(tmem, tc_desc(ag + 2 * kTcATile), tc_desc(bg + 2 * kTcBTile), 1u);     // ci hi x B' hi
-                    tc_mma(tmem, tc_desc(ag + 3 * kTcATile), tc_desc(bg + 2 * kTcBTile), 1u);     // ci lo x B' hi
-                    tc_mma(tmem, tc_desc(ag + 2 * kTcATile), tc_desc(bg + 3 * kTcBTile), 1u);     // ci hi x B' lo
+                    tc_mma(tmem, tc_desc(ag + 0 * kTcATile), tc_desc(bg + 0 * kTcBTile), kIdesc, first);  // cr hi x B hi
+                    tc_mma(tmem, tc_desc(ag + 1 * kTcATile), tc_desc(bg + 0 * kTcBTile), kIdesc, 1u);     // cr lo x B hi
+                    tc_mma(tmem, tc_desc(ag + 0 * kTcATile), tc_desc(bg + 1 * kTcBTile), kIdesc, 1u);     // cr hi x B lo
+                    tc_mma(tmem, tc_desc(ag + 2 * kTcATile), tc_desc(bg + 2 * kTcBTile), kIdesc, 1u);     // ci hi x B' hi
+                    tc_mma(tmem, tc_desc(ag + 3 * kTcATile), tc_desc(bg + 2 * kTcBTile), kIdesc, 1u);     // ci lo x B' hi
+                    tc_mma(tmem, tc_desc(ag + 2 * kTcATile), tc_desc(bg + 3 * kTcBTile), kIdesc, 1u);     // ci hi x B' lo
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mma_done[ab])) : "memory");
                 // refill the ring: slot (st + 3) % 4 held stage st - 1, whose MMAs must be complete
@@ -241,33 +251,36 @@ signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 
         }
         // all MMAs complete -> epilogue (warps 0-3: TMEM lanes 32 w .. 32 w + 31 = sample rows)
         if (warp < 4) {
-            uint32_t v[16];
+            uint32_t v[2 * NC];
 #pragma unroll
-            for (int c = 0; c < 16; ++c) v[c] = 0u;
+            for (int c = 0; c < 2 * NC; ++c) v[c] = 0u;
             if (n_stages > 0) {
                 const int last = n_stages - 1;
                 mbar_wait(&mma_done[last & 1], (uint32_t)((last >> 1) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t taddr = tmem + ((uint32_t)(32 * warp) << 16);
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                             : "r"(taddr));
+#pragma unroll
+                for (int c0 = 0; c0 < 2 * NC; c0 += 16)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                                 : "=r"(v[c0 + 0]), "=r"(v[c0 + 1]), "=r"(v[c0 + 2]), "=r"(v[c0 + 3]), "=r"(v[c0 + 4]), "=r"(v[c0 + 5]),
+                                   "=r"(v[c0 + 6]), "=r"(v[c0 + 7]), "=r"(v[c0 + 8]), "=r"(v[c0 + 9]), "=r"(v[c0 + 10]), "=r"(v[c0 + 11]),
+                                   "=r"(v[c0 + 12]), "=r"(v[c0 + 13]), "=r"(v[c0 + 14]), "=r"(v[c0 + 15])
+                                 : "r"(taddr + (uint32_t)c0));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             }
             const int pp = blockIdx.x * kTcM + 32 * warp + (tid & 31);
             if (pp < n_pts) {
                 const size_t coil_stride = (size_t)gridDim.y * (size_t)n_pts;
 #pragma unroll
-                for (int c = 0; c < 8; ++c)
+                for (int c = 0; c < NC; ++c)
                     partial[(size_t)c * coil_stride + (size_t)blockIdx.y * n_pts + pp] =
-                        make_float2(__uint_as_float(v[c]), __uint_as_float(v[8 + c]));
+                        make_float2(__uint_as_float(v[c]), __uint_as_float(v[NC + c]));
             }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 32;" ::"r"(tmem) : "memory");
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kCols) : "memory");
 }
 
 }  // namespace bloch

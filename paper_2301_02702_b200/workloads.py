@@ -493,7 +493,8 @@ def config4c(n_coils: int = 8, **kw) -> Workload:
 
 
 CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b,
-           "5c": config5c, "4c": config4c}
+           "5c": config5c, "4c": config4c,
+           "4c32": lambda **kw: config4c(n_coils=32, **kw)}
 
 
 def make(name: str, **kw) -> Workload:

@@ -47,11 +47,12 @@ def test_small_configs_with_coils_match_oracle(B, oracle_mod, name, n_coils, pha
                   "final state with coils")
 
 
-def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
+def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B, monkeypatch):
     """One coil with weight 1 everywhere returns the plain signal; 9 coils (two passes of 8, the last with one coil)
     give the same rows as the same coils simulated in separate calls: bitwise when the pass width is the same
     (coils 0-7 alone), to rounding when it is not (4 coils per pass for up to 4 coils: other tile sizes)."""
     from test_gpu_parity import run_gpu
+    monkeypatch.setenv("BLOCH_COIL_TC", "0")   # the FFMA kernel (9 coils would take the tensor-core kernel otherwise)
     w = W.small("4")
     n = w.phantom.n
     plain = run_gpu(B, w, path="per_block")
@@ -120,11 +121,11 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
     assert np.abs(mz).max() > 0.1
 
 
-@pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11)])
+@pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20)])
 def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, monkeypatch, name, n_coils):
     """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with BLOCH_COIL_TC=1): contributions generated on the fly
     as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
-    tiles (n_adc not a multiple of 128), ragged 16-spin stages and two passes of 8 coils are all in these cases."""
+    tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8 and 16 coils per pass and two passes are all in these cases."""
     monkeypatch.setenv("BLOCH_COIL_TC", "1")
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
