@@ -134,8 +134,17 @@ def time_oracle(w, n_intervals: int, budget_spin_steps: float):
     cores = os.cpu_count() or 1
     ph, take, vel, coils = oracle_sample(w, budget_spin_steps, n_intervals)
     t0 = time.perf_counter()
-    oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max,
-                    group_size=w.group_size, coils=coils)
+    if coils is None:
+        oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max,
+                        group_size=w.group_size)
+    else:
+        # the oracle's coil path holds the per-spin signals [spins, n_adc] in memory: feed it batches of spins
+        # (spins are independent, the coil signals add) so that the batch stays below ~1 GB
+        n_adc = int(np.asarray(w.seq.adc_t).size)
+        step = max(1, int(1e9 // (16 * max(1, n_adc))))
+        for lo in range(0, ph.n, step):
+            idx = np.arange(lo, min(ph.n, lo + step))
+            oracle.simulate(ph.subset(idx), w.seq, n_threads=cores, coils=coils[:, idx])
     dt = time.perf_counter() - t0
     return {"value": take * n_intervals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{take} of {w.phantom.n} spins (evenly spaced), full sequence ({n_intervals} intervals), "
