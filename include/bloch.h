@@ -205,7 +205,7 @@ int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
  * Everything else as bloch_simulate (same integration, same final magnetisation).  The plan must be BLOCH_OUT_SUM_ALL
  * without motion (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  The coil-independent part of every evaluation (phase,
  * sin / cos / exp) is computed once per 4 or 8 coils; with more than 8 coils (fp32 phase) the sum over spins runs on the
- * tensor cores (tcgen05, 3xTF32, 16 coils per pass).  Asynchronous on `stream`; never allocates. */
+ * tensor cores (tcgen05, 3xTF32, 16 or 32 coils per pass).  Asynchronous on `stream`; never allocates. */
 int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out);
 int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
                          const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,

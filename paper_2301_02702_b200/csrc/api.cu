@@ -565,10 +565,12 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if (!tc_attr) {
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(8)));
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(16)));
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(32)));
             tc_attr = true;
         }
         const dim3 pg((n_pad + 255) / 256, n_pass);
-        if (ncp == 16) pack_coils_tc_kernel<16><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
+        if (ncp == 32) pack_coils_tc_kernel<32><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
+        else if (ncp == 16) pack_coils_tc_kernel<16><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
         else pack_coils_tc_kernel<8><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
         ++launches;
     } else if (n_coils > 0) {
@@ -693,7 +695,10 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     } while (0)
                     if (tc) {
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
-                        if (ncp == 16)
+                        if (ncp == 32)
+                            signal_coils_tc_kernel<32><<<grid, kTcThreads, tc_smem(32), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, (const float *)w.scal, w.partial);
+                        else if (ncp == 16)
                             signal_coils_tc_kernel<16><<<grid, kTcThreads, tc_smem(16), stream>>>(
                                 (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, (const float *)w.scal, w.partial);
                         else

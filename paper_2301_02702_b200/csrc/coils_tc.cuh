@@ -30,13 +30,15 @@ constexpr int kTcStageSpins = 16;     // spins per stage
 constexpr int kTcGroups = kTcStageSpins / 8;
 constexpr int kTcSlots = 4;           // TMA ring: spin records + B tiles
 constexpr int kTcATile = kTcM * 32;   // one A tile: 128 rows x 8 TF32 = 4096 B
-// NC = coils per pass (8 or 16): N = 2 NC columns (re | im)
+// NC = coils per pass (8, 16 or 32): N = 2 NC columns (re | im)
 __host__ __device__ constexpr int tc_btile(int nc) { return 2 * nc * 32; }     // one B tile: 2 NC rows x 8 TF32
 __host__ __device__ constexpr int tc_bgroup(int nc) { return 4 * tc_btile(nc); }  // per 8-spin group: cr hi, cr lo, ci hi, ci lo
 __host__ __device__ constexpr int tc_slot(int nc) { return kTcStageSpins * 32 + kTcGroups * tc_bgroup(nc); }  // spin records + B tiles
 constexpr int kTcAStage = kTcGroups * 4 * kTcATile;                       // 32 KB
 __host__ __device__ constexpr size_t tc_smem(int nc) { return 2 * (size_t)kTcAStage + kTcSlots * (size_t)tc_slot(nc) + 256; }
-__host__ __device__ inline int tc_coils_per_pass(int n_coils) { return n_coils > 8 ? 16 : 8; }
+// the MMA count per stage does not depend on N, so more coils per pass are nearly free; 32 per pass need 132 KB of
+// shared memory (one CTA per SM, which the tensor-pipe-bound kernel does not mind)
+__host__ __device__ inline int tc_coils_per_pass(int n_coils) { return n_coils > 16 ? 32 : (n_coils > 8 ? 16 : 8); }
 
 __device__ __forceinline__ uint32_t tc_tf32(float x) {
     uint32_t r;
@@ -95,7 +97,7 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_
 constexpr int kTcThreads = 288;  // 8 generator warps + 1 control warp (TMA + MMA issue by its lane 0)
 
 template <int NC>
-__global__ void __launch_bounds__(kTcThreads, 2)
+__global__ void __launch_bounds__(kTcThreads, NC == 32 ? 1 : 2)
 signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *__restrict__ A,
                        const float4 *__restrict__ S, const unsigned char *__restrict__ Bt /* this pass */,
                        int n_spins, int spins_per_chunk /* multiple of 16 */, const float *__restrict__ scal,

@@ -121,11 +121,11 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
     assert np.abs(mz).max() > 0.1
 
 
-@pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20)])
+@pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20), ("4", 37)])
 def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, monkeypatch, name, n_coils):
     """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with BLOCH_COIL_TC=1): contributions generated on the fly
     as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
-    tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8 and 16 coils per pass and two passes are all in these cases."""
+    tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8, 16 and 32 coils per pass and two passes (37 coils) are all in these cases."""
     monkeypatch.setenv("BLOCH_COIL_TC", "1")
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
