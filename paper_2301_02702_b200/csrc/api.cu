@@ -737,9 +737,10 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                 }
                 const dim3 grid(s.ptiles, s.chunks);
                 const int row = (int)batch_pts, poff = (int)batch_done;
+                const int allow_lin = env_int("BLOCH_SIGNAL_LIN", 1);
 #define BLOCH_LAUNCH_SIG3(PP, H, M, AP, VP)                                                                    \
     signal_kernel<PP, H, M><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, VP, w.S, n, s.spins_per_chunk,    \
-                                                              (const float *)w.scal, w.partial, row, poff)
+                                                              (const float *)w.scal, w.partial, row, poff, allow_lin)
 #define BLOCH_LAUNCH_SIG(PP)                                                                                   \
     do {                                                                                                       \
         if (ph64 && mo) BLOCH_LAUNCH_SIG3(PP, true, true, w.Ad, w.Vd);                                         \

@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(kSigThreads, (PH64 || MO) ? 1 : (P == 8 ? 3 : 
 signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_, const void *__restrict__ V_,
               const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
               const float *__restrict__ scal /* [0] = max 1/T2, from pack_kernel */, float2 *__restrict__ partial,
-              int row_stride /* points of the whole batch */, int p_off /* this block's first point in the batch */) {
+              int row_stride /* points of the whole batch */, int p_off /* this block's first point in the batch */,
+              int allow_lin /* 0: never take the rotation recurrence (BLOCH_SIGNAL_LIN=0, diagnostics) */) {
     using RecT = typename std::conditional<PH64, double4, float4>::type;   // (k'x, k'y, k'z, tau)
     using PosT = typename std::conditional<PH64, double4, float4>::type;   // (x, y, z, f')
     using real = typename std::conditional<PH64, double, float>::type;
@@ -111,9 +112,59 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
 #pragma unroll
     for (int j = 2; j < P; ++j) dev = fmaxf(dev, fabsf(cj[j] - (float)j * cj[1]));
     const bool geom = P > 2 && series && __all_sync(0xffffffffu, dev * (scal[0] * kLog2e) <= 1e-6f);
+    // ... and when k' itself advances by the same step from sample to sample (a Cartesian / EPI readout on its
+    // plateau), the whole factor exp(-tau_j/T2) exp(i theta_j) of sample j is that of sample j-1 times
+    // zeta = q exp(i delta), delta = dk' . x + f' dwell: one sincos for theta_0 and one for delta per spin, then one
+    // complex multiply per sample on the FMA pipe -- (5 MUFU + ~74 issue slots) / P instead of 2 + 1/P MUFU per
+    // evaluation.  dk' is the slope through the thread's first and last sample; the mode is taken when every
+    // sample in between lies on that line to within the rounding of the table itself (1.25e-7 relative to the larger
+    // end in fp32, i.e. 1-2 ulp; 1e-13 in fp64), so the phase it reconstructs differs from the tabulated one by no more
+    // than the table's own rounding.  Not for motion plans (the first-moment term is quadratic in time).
+    real dkx = 0, dky = 0, dkz = 0, dta = 0;
+    bool lin = false;
+    if (!MO && P > 2 && allow_lin) {
+        constexpr real inv = (real)1 / (real)(P - 1);
+        constexpr real rel = PH64 ? (real)1e-13 : (real)1.25e-7;
+        dkx = (kx[P - 1] - kx[0]) * inv;
+        dky = (ky[P - 1] - ky[0]) * inv;
+        dkz = (kz[P - 1] - kz[0]) * inv;
+        dta = (tau[P - 1] - tau[0]) * inv;
+        // fp64 tables (turns / m): the ADC times themselves are equally spaced only to the rounding of t (7e-18 s in
+        // 4e-6 s: 2e-12 of a step), so allow 1e-8 turns / m absolute -- below 1e-8 turns of phase for |x| < 1 m, an
+        // order under the 2^-23-turn granularity of the reduced phase
+        constexpr real fl = PH64 ? (real)1e-8 : (real)0;
+        const real tx = rel * fmax(fabs(kx[0]), fabs(kx[P - 1])) + fl, ty = rel * fmax(fabs(ky[0]), fabs(ky[P - 1])) + fl;
+        const real tz = rel * fmax(fabs(kz[0]), fabs(kz[P - 1])) + fl, tt = rel * fmax(fabs(tau[0]), fabs(tau[P - 1]));
+        bool ok = true;
+#pragma unroll
+        for (int j = 1; j < P - 1; ++j) {
+            ok = ok && fabs(kx[j] - (kx[0] + (real)j * dkx)) <= tx && fabs(ky[j] - (ky[0] + (real)j * dky)) <= ty &&
+                 fabs(kz[j] - (kz[0] + (real)j * dkz)) <= tz && fabs(tau[j] - (tau[0] + (real)j * dta)) <= tt;
+        }
+        lin = geom && __all_sync(0xffffffffu, ok);
+    }
     __syncthreads();  // barrier initialisation visible to every waiter
+    // sin and cos of the phase k . x + w tau (fp32: radians; fp64: turns, reduced as described in the header)
+    auto phase_sincos = [&](real qx, real qy, real qz, real qt, const PosT &a, float &sn, float &cs) {
+        if (PH64) {
+            double th = fma((double)qx, (double)a.x, fma((double)qy, (double)a.y,
+                            fma((double)qz, (double)a.z, (double)qt * (double)a.w)));  // turns
+            th += 1572864.0;  // 1.5 * 2^20: ulp = 2^-32, low word = frac(theta) in 0.32 fixed point
+            const unsigned lo = (unsigned)__double2loint(th);
+            const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;  // [0, 1) turns
+            const float ang = fr * 6.283185307179586f;
+            sn = __sinf(ang);
+            cs = __cosf(ang);
+        } else {
+            const float th = fmaf((float)qx, (float)a.x, fmaf((float)qy, (float)a.y,
+                                  fmaf((float)qz, (float)a.z, (float)qt * (float)a.w)));  // radians
+            sn = __sinf(th);
+            cs = __cosf(th);
+        }
+    };
     auto run = [&](auto mode_tag) {
-    constexpr int MODE = decltype(mode_tag)::value;  // 0: one MUFU.EX2 per sample, 1: series per sample, 2: geometric
+    // 0: one MUFU.EX2 per sample, 1: series per sample, 2: geometric decay, 3: geometric decay and rotation
+    constexpr int MODE = decltype(mode_tag)::value;
     constexpr bool SERIES = MODE != 0;
     for (int t = 0; t < n_tiles; ++t) {
         const int b = t & 1;
@@ -127,9 +178,41 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
             vv.x = 0; vv.y = 0; vv.z = 0; vv.w = 0;
             if (MO) vv = shV[b][s];
             float er0 = 0.f, ei0 = 0.f, qd = 1.f;
-            if (MODE == 2) {
+            if (MODE >= 2) {
                 const float y = cj[1] * st.w;  // -dwell/T2
                 qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+            }
+            if (MODE == 3) {
+                float sn, cs, sd, cd;
+                phase_sincos(kx[0], ky[0], kz[0], tau[0], a, sn, cs);
+                phase_sincos(dkx, dky, dkz, dta, a, sd, cd);
+                const float e = ex2_approx(tf[0] * st.w);  // MUFU.EX2: exp(-tau_0/T2)
+                const float zr = qd * cd, zi = qd * sd;    // zeta
+                const float er = st.x * e, ei = st.y * e;
+                // w_j = w_0 zeta^j through zeta^2, zeta^4: dependency depth log2(P) instead of P - 1
+                float wr[P], wi[P];
+                wr[0] = fmaf(er, cs, -ei * sn);
+                wi[0] = fmaf(er, sn, ei * cs);
+                float pr = zr, pi = zi;  // zeta^(2^m)
+#pragma unroll
+                for (int h = 1; h < P; h *= 2) {
+#pragma unroll
+                    for (int j = 0; j < h; ++j) {
+                        wr[h + j] = fmaf(wr[j], pr, -wi[j] * pi);
+                        wi[h + j] = fmaf(wr[j], pi, wi[j] * pr);
+                    }
+                    if (2 * h < P) {
+                        const float t2 = fmaf(pr, pr, -pi * pi);
+                        pi = 2.0f * pr * pi;
+                        pr = t2;
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    ar[j] += wr[j];
+                    ai[j] += wi[j];
+                }
+                continue;
             }
 #pragma unroll
             for (int j = 0; j < P; ++j) {
@@ -178,7 +261,8 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
         if (tid == 0 && t + 2 < n_tiles) issue(t + 2);
     }
     };
-    if (geom) run(std::integral_constant<int, 2>{});
+    if (lin) run(std::integral_constant<int, 3>{});
+    else if (geom) run(std::integral_constant<int, 2>{});
     else if (series) run(std::integral_constant<int, 1>{});
     else run(std::integral_constant<int, 0>{});
 #pragma unroll

@@ -206,3 +206,37 @@ def test_signal_decay_modes_equal_spacing_and_jitter(B, oracle_mod, jitter):
     g = {0: ([2e-4, 3e-4, 9e-3], [0, 4e-3, 4e-3]), 1: ([2e-4, 3e-4, 9e-3], [0, -2e-3, 1e-3])}
     s = seq(g=g, rf=rf, adc=np.sort(adc), t_end=1e-2, dt_rf_max=1.0)
     check(B, oracle_mod, rand_phantom(900, 13, t2=(0.005, 0.05)), s, f"decay modes, jitter {jitter}")
+
+
+@pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
+def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode, monkeypatch):
+    """EPI-like train sampled THROUGH the ramps: the warps whose 8 (or 4) adjacent samples sit on a plateau take the
+    rotation recurrence (k' advances by a constant step), those that touch a ramp or a blip must not.  Both against the
+    oracle, and against the same kernel with the recurrence switched off (BLOCH_SIGNAL_LIN=0)."""
+    import torch
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    n_lines, flat, ramp, G = 12, 1.2e-3, 1.0e-4, 9e-3
+    t, v, ty, vy = [2e-4], [0.0], [2e-4], [0.0]
+    for ln in range(n_lines):
+        sgn = 1.0 if ln % 2 == 0 else -1.0
+        t0 = t[-1]
+        t += [t0 + ramp, t0 + ramp + flat, t0 + 2 * ramp + flat]
+        v += [sgn * G, sgn * G, 0.0]
+        ty += [t0 + 2 * ramp + flat - 5e-5, t0 + 2 * ramp + flat - 2.5e-5, t0 + 2 * ramp + flat]
+        vy += [0.0, 2e-3, 0.0]
+    t_end = t[-1] + 1e-4
+    adc = 2.1e-4 + (np.arange(int((t[-1] - 2.2e-4) / 4e-6)) + 0.5) * 4e-6   # ~4200 samples: P = 8, ragged tail
+    s = seq(g={0: (t, v), 1: (ty, vy)}, rf=rf, adc=adc, t_end=t_end, dt_rf_max=1.0)
+    ph = rand_phantom(1500, 21)
+    check(B, oracle_mod, ph, s, f"recurrence {phase_mode}", phase_mode=phase_mode)
+    dev = B.phantom_to_device(ph)
+    out = {}
+    for lin in ("1", "0"):
+        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
+        plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+        out[lin] = plan.simulate(*dev).cpu().numpy()
+        torch.cuda.synchronize()
+        plan.close()
+    emax, nrmse = errors(out["1"], out["0"])
+    print(f"recurrence on/off {phase_mode}: max {emax:.3e} nrmse {nrmse:.3e}")
+    assert 0 < emax <= 2e-5 and nrmse <= 5e-6      # different arithmetic (not bitwise), same answer
