@@ -324,7 +324,8 @@ def run_ours(args, rank, local_rank, world):
                           "coils": n_coils,
                           "note": "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample), SURVEY.md 8(d); "
                                   "the kernel issues 2 + 1/P (P = 8 adjacent samples share one ex2; 4 in shorter blocks), so frac "
-                                  "can reach 3 / 2.125 = 1.41 at a saturated MUFU pipe",
+                                  "can reach 3 / 2.125 = 1.41 at a saturated MUFU pipe; on Cartesian readouts (k' advances by a constant step) the "
+                                  "rotation recurrence issues 5 MUFU per P samples and the loop is issue-bound instead, so frac exceeds that",
                           "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
                           "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
                           "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}

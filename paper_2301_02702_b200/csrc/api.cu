@@ -748,7 +748,35 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else if (mo) BLOCH_LAUNCH_SIG3(PP, false, true, w.A, w.V);                                             \
         else BLOCH_LAUNCH_SIG3(PP, false, false, w.A, nullptr);                                                \
     } while (0)
-                if (s.P == 8) BLOCH_LAUNCH_SIG(8);
+                if (b.lin_pts > 0 && allow_lin && !mo) {
+                    // Cartesian readout (planner: constant k' step inside every aligned group of kLinP samples): the
+                    // recurrence kernel on the first lin_pts samples, the n % kLinP tail through signal_kernel<1>;
+                    // both with this block's chunking, so the partial rows and the second pass are unchanged
+                    const int n_groups = (int)(b.lin_pts / kLinP);
+                    const dim3 lgrid((unsigned)((n_groups + kSigThreads - 1) / kSigThreads), s.chunks);
+                    if (ph64)
+                        signal_lin_kernel<true><<<lgrid, kSigThreads, 0, stream>>>(
+                            recs, n_groups, w.Ad, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);
+                    else
+                        signal_lin_kernel<false><<<lgrid, kSigThreads, 0, stream>>>(
+                            recs, n_groups, w.A, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);
+                    const int n_tail = n_pts - (int)b.lin_pts;
+                    if (n_tail > 0) {
+                        const void *trecs = (const unsigned char *)recs + (size_t)b.lin_pts * (ph64 ? 32 : 16);
+                        const dim3 tgrid(1, s.chunks);
+                        const int toff = poff + (int)b.lin_pts;
+                        if (ph64)
+                            signal_kernel<1, true, false><<<tgrid, 32, 0, stream>>>(
+                                trecs, n_tail, w.Ad, nullptr, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial,
+                                row, toff, 0);
+                        else
+                            signal_kernel<1, false, false><<<tgrid, 32, 0, stream>>>(
+                                trecs, n_tail, w.A, nullptr, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial,
+                                row, toff, 0);
+                        ++launches;
+                    }
+                }
+                else if (s.P == 8) BLOCH_LAUNCH_SIG(8);
                 else if (s.P == 4) BLOCH_LAUNCH_SIG(4);
                 else if (s.P == 2) BLOCH_LAUNCH_SIG(2);
                 else BLOCH_LAUNCH_SIG(1);

@@ -52,6 +52,7 @@ struct Block {
     int64_t adc_first = 0;    // precession: first ADC sample served, in ADC order
     int64_t adc_count = 0;    //             number of ADC samples served (= evaluated points of the signal kernel)
     int64_t table_off = 0;    // byte offset of this block's records in the table buffer
+    int64_t lin_pts = 0;      // precession: leading samples (a multiple of 16) that signal_lin_kernel may serve, see plan.cpp
     int64_t n_tiles = 0;      // RF: tiles in the block's table (see RfTileHdr)
     // precession block end record: k' = -gamma_bar * K(T) [turns/m] and tau = T [s] (Eq 12-13)
     double kend[3] = {0, 0, 0};

@@ -374,6 +374,24 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
         Block &b = blocks[bi];
         b.table_off = (int64_t)off;
+        // Cartesian readouts: does k' (and tau) advance by a constant step inside EVERY aligned group of 16 samples?
+        // Checked on the fp64 records (turns / m): every sample within 1e-13 relative + 1e-8 turns / m (1e-13 s) of the
+        // line through the group's first and last sample, the level at which the ADC times themselves are equally
+        // spaced.  Such blocks go to signal_lin_kernel (signal.cuh), the n % 16 tail to signal_kernel.
+        if (b.type == kBlockPrecession && !motion && b.adc_count >= 2048) {
+            const double *src = krec.data() + 4 * krec_first[bi];
+            const int64_t n_g = b.adc_count / 16;
+            bool ok = true;
+            for (int64_t g = 0; g < n_g && ok; ++g) {
+                const double *q = src + 4 * 16 * g;
+                for (int c = 0; c < 4 && ok; ++c) {
+                    const double a0 = q[c], a1 = q[4 * 15 + c], step = (a1 - a0) / 15.0;
+                    const double tol = 1e-13 * std::max(std::fabs(a0), std::fabs(a1)) + (c == 3 ? 1e-13 : 1e-8);
+                    for (int j = 1; j < 15 && ok; ++j) ok = std::fabs(q[4 * j + c] - (a0 + j * step)) <= tol;
+                }
+            }
+            if (ok) b.lin_pts = n_g * 16;
+        }
         const size_t bytes = b.type == kBlockRF ? rf_img[bi].size() : size_t(b.adc_count) * rec_bytes;
         off = align_up(off + bytes, kAlign);
     }
@@ -429,6 +447,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             if (b.type == kBlockRF) { ++launches; pending = false; continue; }
             if (pending) ++launches;
             if (b.adc_count > 0) launches += (params->output_mode == BLOCH_OUT_SUM_ALL) ? 2 : 1;
+            if (params->output_mode == BLOCH_OUT_SUM_ALL && b.lin_pts > 0 && b.lin_pts < b.adc_count) ++launches;  // tail
             pending = true;
         }
         if (pending) ++launches;

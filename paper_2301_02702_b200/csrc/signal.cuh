@@ -272,6 +272,133 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
     }
 }
 
+// Cartesian readouts: the rotation recurrence alone (see signal_kernel, mode 3), launched instead of signal_kernel for
+// precession blocks whose table the PLANNER found to advance by a constant step inside every aligned group of kLinP
+// samples (Block::lin_pts of them; fp64 check on the untruncated table, plan.cpp).  A thread keeps only its group's first
+// record and the step, so the fp64-phase variant needs ~1/2 of signal_kernel<8, true>'s registers and two or three CTAs
+// fit on an SM; 5 MUFU and ~136 issue slots per 16 evaluations.  The block's remaining n_pts % kLinP samples go
+// through signal_kernel with the same chunking (one more launch, same partial rows).
+constexpr int kLinP = 16;
+
+template <bool PH64>
+__global__ void __launch_bounds__(kSigThreads, 2)
+signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__restrict__ A_,
+                  const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
+                  const float *__restrict__ scal /* [0] = max 1/T2 */, float2 *__restrict__ partial, int row_stride,
+                  int p_off) {
+    constexpr int P = kLinP;
+    using RecT = typename std::conditional<PH64, double4, float4>::type;
+    using PosT = typename std::conditional<PH64, double4, float4>::type;
+    using real = typename std::conditional<PH64, double, float>::type;
+    __shared__ __align__(128) PosT shA[2][kSigTile];
+    __shared__ __align__(128) float4 shS[2][kSigTile];
+    __shared__ __align__(8) uint64_t bar[2];
+    const RecT *recs = reinterpret_cast<const RecT *>(recs_);
+    const PosT *A = reinterpret_cast<const PosT *>(A_);
+    const int tid = threadIdx.x;
+    const int s0 = blockIdx.y * spins_per_chunk;
+    const int s1 = min(n_spins, s0 + spins_per_chunk);
+    const int n_tiles = (s1 - s0 + kSigTile - 1) / kSigTile;
+    auto issue = [&](int t) {
+        const int b = t & 1;
+        const int base = s0 + t * kSigTile;
+        const uint32_t cnt = (uint32_t)min(kSigTile, s1 - base);
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + sizeof(float4)));
+        bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
+        bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
+    };
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init_fence();
+        if (n_tiles > 0) issue(0);
+        if (n_tiles > 1) issue(1);
+    }
+    const int g = blockIdx.x * (int)blockDim.x + tid;
+    const bool live = g < n_groups;
+    RecT r0, r1;
+    r0.x = 0; r0.y = 0; r0.z = 0; r0.w = 0;
+    r1 = r0;
+    if (live) {
+        r0 = recs[(size_t)g * P];
+        r1 = recs[(size_t)g * P + P - 1];
+    }
+    constexpr real inv = (real)1 / (real)(P - 1);
+    const real dkx = (r1.x - r0.x) * inv, dky = (r1.y - r0.y) * inv, dkz = (r1.z - r0.z) * inv, dta = (r1.w - r0.w) * inv;
+    const float tf0 = (float)r0.w;
+    const float cd = (float)dta * 0.6931471805599453f;  // dwell ln 2; times e2 = -log2(e)/T2 gives -dwell/T2
+    // q = exp(-dwell/T2) by the cubic series when dwell/T2 <= 0.02 for every spin (as in signal_kernel), else MUFU.EX2
+    const bool series = __all_sync(0xffffffffu, fabsf(cd) * (scal[0] * kLog2e) <= 0.02f);
+    float ar[P], ai[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) { ar[j] = 0.f; ai[j] = 0.f; }
+    auto phase_sincos = [&](real qx, real qy, real qz, real qt, const PosT &a, float &sn, float &cs) {
+        if (PH64) {
+            double th = fma((double)qx, (double)a.x, fma((double)qy, (double)a.y,
+                            fma((double)qz, (double)a.z, (double)qt * (double)a.w)));  // turns
+            th += 1572864.0;  // 1.5 * 2^20: low word = frac(theta) in 0.32 fixed point (see the file header)
+            const unsigned lo = (unsigned)__double2loint(th);
+            const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;
+            const float ang = fr * 6.283185307179586f;
+            sn = __sinf(ang);
+            cs = __cosf(ang);
+        } else {
+            const float th = fmaf((float)qx, (float)a.x, fmaf((float)qy, (float)a.y,
+                                  fmaf((float)qz, (float)a.z, (float)qt * (float)a.w)));  // radians
+            sn = __sinf(th);
+            cs = __cosf(th);
+        }
+    };
+    __syncthreads();
+    for (int t = 0; t < n_tiles; ++t) {
+        const int b = t & 1;
+        mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
+        const int cnt = min(kSigTile, s1 - (s0 + t * kSigTile));
+#pragma unroll 2
+        for (int s = 0; s < cnt; ++s) {
+            const PosT a = shA[b][s];
+            const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            float sn, cs, sd, cdl;
+            phase_sincos(r0.x, r0.y, r0.z, r0.w, a, sn, cs);
+            phase_sincos(dkx, dky, dkz, dta, a, sd, cdl);
+            const float e = ex2_approx(tf0 * st.w);
+            const float y = cd * st.w;  // -dwell/T2
+            float qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+            if (!series) qd = ex2_approx((float)dta * st.w);
+            float pr = qd * cdl, pi = qd * sd;  // zeta^(2^m)
+            const float er = st.x * e, ei = st.y * e;
+            float wr[P], wi[P];
+            wr[0] = fmaf(er, cs, -ei * sn);
+            wi[0] = fmaf(er, sn, ei * cs);
+#pragma unroll
+            for (int h = 1; h < P; h *= 2) {
+#pragma unroll
+                for (int j = 0; j < h; ++j) {
+                    wr[h + j] = fmaf(wr[j], pr, -wi[j] * pi);
+                    wi[h + j] = fmaf(wr[j], pi, wi[j] * pr);
+                }
+                if (2 * h < P) {
+                    const float t2 = fmaf(pr, pr, -pi * pi);
+                    pi = 2.0f * pr * pi;
+                    pr = t2;
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                ar[j] += wr[j];
+                ai[j] += wi[j];
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && t + 2 < n_tiles) issue(t + 2);
+    }
+    if (live) {
+        float2 *dst = partial + (size_t)blockIdx.y * row_stride + p_off + (size_t)g * P;
+#pragma unroll
+        for (int j = 0; j < P; ++j) dst[j] = make_float2(ar[j], ai[j]);
+    }
+}
+
 // Second pass of a7: fixed-order sum over the spin chunks.  blockDim = (32, 8): x = point, y = chunk lane.
 __global__ void __launch_bounds__(256)
 reduce_kernel(const float2 *__restrict__ partial, int n_chunks, int n_pts, float2 *__restrict__ out) {

@@ -240,3 +240,35 @@ def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode
     emax, nrmse = errors(out["1"], out["0"])
     print(f"recurrence on/off {phase_mode}: max {emax:.3e} nrmse {nrmse:.3e}")
     assert 0 < emax <= 2e-5 and nrmse <= 5e-6      # different arithmetic (not bitwise), same answer
+
+
+@pytest.mark.parametrize("phase_mode,n_adc", [("fp32", 2048), ("fp32", 4103), ("fp64", 2061), ("fp64", 8192)])
+def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_adc, monkeypatch):
+    """A block of >= 2048 equally spaced samples on a plateau: the planner hands its first n - n % 16 samples to
+    signal_lin_kernel (16 samples per thread, recurrence only) and the tail to signal_kernel<1>.  Against the oracle
+    and against the per-sample kernel (BLOCH_SIGNAL_LIN=0); short T2 (dwell / T2 up to 0.04) also drives the
+    MUFU.EX2 form of q in the fp64 cases."""
+    import torch
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    dwell = 4e-6 if phase_mode == "fp32" else 2e-4
+    t1 = 4e-4 + n_adc * dwell
+    g = {0: ([2e-4, 3e-4, t1], [0, 1e-3, 1e-3] if phase_mode == "fp32" else [0, 1e-4, 1e-4]),
+         1: ([2e-4, 3e-4, t1], [0, -5e-4, -5e-4] if phase_mode == "fp32" else [0, -5e-5, -5e-5])}
+    adc = 3.5e-4 + (np.arange(n_adc) + 0.5) * dwell
+    s = seq(g=g, rf=rf, adc=adc, t_end=t1 + 1e-4, dt_rf_max=1.0)
+    ph = rand_phantom(777, 23, t2=(0.03, 0.3) if phase_mode == "fp32" else (0.005, 0.3))
+    launches = check(B, oracle_mod, ph, s, f"lin kernel {phase_mode} n_adc={n_adc}", phase_mode=phase_mode)
+    pl = B.Plan(s, path="per_block", phase_mode=phase_mode)
+    assert launches == B.bloch_plan_get_info(pl.handle)["n_launches"]      # the tail launch is counted by the planner
+    pl.close()
+    dev = B.phantom_to_device(ph)
+    out = {}
+    for lin in ("1", "0"):
+        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
+        plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+        out[lin] = plan.simulate(*dev).cpu().numpy()
+        torch.cuda.synchronize()
+        plan.close()
+    emax, nrmse = errors(out["1"], out["0"])
+    print(f"lin kernel on/off {phase_mode} n_adc={n_adc}: max {emax:.3e} nrmse {nrmse:.3e}")
+    assert 0 < emax <= 3e-5 and nrmse <= 8e-6     # fp32: both sit on the fp32 phase floor (no echo in this sequence)
