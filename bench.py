@@ -36,6 +36,7 @@ FP32_PER_EVAL = 15         # FP32-pipe instructions per (spin, evaluated point) 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full captures
 NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v3_signal_kernel_cfg4_ncu.txt"),
                ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v3_rf_kernel_cfg4_ncu.txt"),
+               ("config3_brain_epi128", "signal"): (6.57e6, "profiles/r01_v4_signal_lin_kernel_cfg3_ncu.txt"),
                ("config5_mrf_fisp", "fused"): (1229.9e6, "profiles/r01_v3_seq_kernel_cfg5_ncu.txt")}
 
 
