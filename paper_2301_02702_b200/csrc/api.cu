@@ -83,6 +83,13 @@ int sig_max_P(const bloch_plan *plan) {
     return (plan->info.phase_mode == BLOCH_PHASE_FP64 && plan->info.motion_mode == BLOCH_MOTION_LINEAR) ? 4 : 8;
 }
 
+// Launch shape of a precession block: blocks that go to signal_lin_kernel (Block::lin_pts) are chunked as P = 8 blocks
+// whatever the plan (their kernel holds 2 CTAs per SM also with fp64 phase and motion).
+SigShape block_shape(const bloch_plan *plan, const Block &b, int64_t n_spins, int sm_count) {
+    const bool lin = b.lin_pts > 0 && env_int("BLOCH_SIGNAL_LIN", 1);
+    return sig_shape(b.adc_count, n_spins, sm_count, lin ? 8 : sig_max_P(plan));
+}
+
 // Partial-sum buffer (a7): consecutive ADC-bearing precession blocks with the same launch shape share one
 // buffer P[chunk][points of the batch] and ONE second-pass launch, up to kPartialCapBytes; at least the
 // largest single block always fits.
@@ -92,7 +99,7 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
     size_t worst = 1, total = 0;
     for (const Block &b : plan->blocks) {
         if (b.type != kBlockPrecession || b.adc_count == 0) continue;
-        const SigShape s = sig_shape(b.adc_count, n_spins, sm_count, sig_max_P(plan));
+        const SigShape s = block_shape(plan, b, n_spins, sm_count);
         const size_t e = size_t(s.chunks) * size_t(b.adc_count);
         worst = std::max(worst, e);
         total += e;
@@ -717,7 +724,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     launches += 2;
                 }
             } else {
-                const SigShape s = sig_shape(n_pts, n, sms, sig_max_P(plan));
+                const SigShape s = block_shape(plan, b, n, sms);
                 if (!batch_open) {  // look ahead: how many of the following blocks share this batch
                     batch_shape = s;
                     batch_adc_first = b.adc_first;
@@ -727,7 +734,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     for (size_t bj = bi; bj < plan->blocks.size(); ++bj) {
                         const Block &c = plan->blocks[bj];
                         if (c.type != kBlockPrecession || c.adc_count == 0) continue;
-                        const SigShape sc = sig_shape(c.adc_count, n, sms, sig_max_P(plan));
+                        const SigShape sc = block_shape(plan, c, n, sms);
                         if (sc.P != s.P || sc.chunks != s.chunks || sc.spins_per_chunk != s.spins_per_chunk ||
                             sc.threads != s.threads) break;
                         if (batch_pts + c.adc_count > cap_pts || batch_pts + c.adc_count > INT32_MAX) break;
@@ -748,33 +755,30 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else if (mo) BLOCH_LAUNCH_SIG3(PP, false, true, w.A, w.V);                                             \
         else BLOCH_LAUNCH_SIG3(PP, false, false, w.A, nullptr);                                                \
     } while (0)
-                if (b.lin_pts > 0 && allow_lin && !mo) {
-                    // Cartesian readout (planner: constant k' step inside every aligned group of kLinP samples): the
-                    // recurrence kernel on the first lin_pts samples, the n % kLinP tail through signal_kernel<1>;
-                    // both with this block's chunking, so the partial rows and the second pass are unchanged
+                if (b.lin_pts > 0 && allow_lin) {
+                    // Cartesian readout (planner: constant k' step, quadratic mu', inside every aligned group of kLinP
+                    // samples): the recurrence kernel on the first lin_pts samples, the n % kLinP tail through
+                    // signal_kernel<1>; both with this block's chunking, so the partial rows and the second pass are unchanged
                     const int n_groups = (int)(b.lin_pts / kLinP);
                     const dim3 lgrid((unsigned)((n_groups + kSigThreads - 1) / kSigThreads), s.chunks);
-                    if (ph64)
-                        signal_lin_kernel<true><<<lgrid, kSigThreads, 0, stream>>>(
-                            recs, n_groups, w.Ad, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);
-                    else
-                        signal_lin_kernel<false><<<lgrid, kSigThreads, 0, stream>>>(
-                            recs, n_groups, w.A, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial, row, poff);
                     const int n_tail = n_pts - (int)b.lin_pts;
-                    if (n_tail > 0) {
-                        const void *trecs = (const unsigned char *)recs + (size_t)b.lin_pts * (ph64 ? 32 : 16);
-                        const dim3 tgrid(1, s.chunks);
-                        const int toff = poff + (int)b.lin_pts;
-                        if (ph64)
-                            signal_kernel<1, true, false><<<tgrid, 32, 0, stream>>>(
-                                trecs, n_tail, w.Ad, nullptr, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial,
-                                row, toff, 0);
-                        else
-                            signal_kernel<1, false, false><<<tgrid, 32, 0, stream>>>(
-                                trecs, n_tail, w.A, nullptr, w.S, n, s.spins_per_chunk, (const float *)w.scal, w.partial,
-                                row, toff, 0);
-                        ++launches;
-                    }
+                    const void *trecs = (const unsigned char *)recs + (size_t)b.lin_pts * (ph64 ? 32 : 16) * (mo ? 2 : 1);
+                    const dim3 tgrid(1, s.chunks);
+                    const int toff = poff + (int)b.lin_pts;
+#define BLOCH_LAUNCH_LIN(H, M, AP, VP)                                                                              \
+    do {                                                                                                            \
+        signal_lin_kernel<H, M><<<lgrid, kSigThreads, 0, stream>>>(recs, n_groups, AP, VP, w.S, n, s.spins_per_chunk, \
+                                                                   (const float *)w.scal, w.partial, row, poff);    \
+        if (n_tail > 0)                                                                                             \
+            signal_kernel<1, H, M><<<tgrid, 32, 0, stream>>>(trecs, n_tail, AP, VP, w.S, n, s.spins_per_chunk,      \
+                                                             (const float *)w.scal, w.partial, row, toff, 0);       \
+    } while (0)
+                    if (ph64 && mo) BLOCH_LAUNCH_LIN(true, true, w.Ad, w.Vd);
+                    else if (ph64) BLOCH_LAUNCH_LIN(true, false, w.Ad, nullptr);
+                    else if (mo) BLOCH_LAUNCH_LIN(false, true, w.A, w.V);
+                    else BLOCH_LAUNCH_LIN(false, false, w.A, nullptr);
+#undef BLOCH_LAUNCH_LIN
+                    if (n_tail > 0) ++launches;
                 }
                 else if (s.P == 8) BLOCH_LAUNCH_SIG(8);
                 else if (s.P == 4) BLOCH_LAUNCH_SIG(4);

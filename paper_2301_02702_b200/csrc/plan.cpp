@@ -378,7 +378,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         // Checked on the fp64 records (turns / m): every sample within 1e-13 relative + 1e-8 turns / m (1e-13 s) of the
         // line through the group's first and last sample, the level at which the ADC times themselves are equally
         // spaced.  Such blocks go to signal_lin_kernel (signal.cuh), the n % 16 tail to signal_kernel.
-        if (b.type == kBlockPrecession && !motion && b.adc_count >= 2048) {
+        if (b.type == kBlockPrecession && b.adc_count >= 2048) {
             const double *src = krec.data() + 4 * krec_first[bi];
             const int64_t n_g = b.adc_count / 16;
             bool ok = true;
@@ -388,6 +388,20 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                     const double a0 = q[c], a1 = q[4 * 15 + c], step = (a1 - a0) / 15.0;
                     const double tol = 1e-13 * std::max(std::fabs(a0), std::fabs(a1)) + (c == 3 ? 1e-13 : 1e-8);
                     for (int j = 1; j < 15 && ok; ++j) ok = std::fabs(q[4 * j + c] - (a0 + j * step)) <= tol;
+                }
+            }
+            // motion: the first moment mu' must be a quadratic in the sample index (exact on a plateau): residual against
+            // the parabola through samples 0, 8, 15 within 1e-13 relative + 1e-9 turns s / m
+            if (motion) {
+                const double *msrc = mrec.data() + 4 * krec_first[bi];
+                for (int64_t g = 0; g < n_g && ok; ++g) {
+                    const double *q = msrc + 4 * 16 * g;
+                    for (int c = 0; c < 3 && ok; ++c) {
+                        const double m0 = q[c], m8 = q[4 * 8 + c], m15 = q[4 * 15 + c];
+                        const double qb = ((m15 - m0) / 15.0 - (m8 - m0) / 8.0) / 7.0, qa = (m8 - m0) / 8.0 - 8.0 * qb;
+                        const double tol = 1e-13 * std::max(std::fabs(m0), std::fabs(m15)) + 1e-9;
+                        for (int j = 1; j < 15 && ok; ++j) ok = std::fabs(q[4 * j + c] - (m0 + j * (qa + j * qb))) <= tol;
+                    }
                 }
             }
             if (ok) b.lin_pts = n_g * 16;

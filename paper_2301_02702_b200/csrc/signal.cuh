@@ -279,22 +279,31 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
 // fit on an SM; 5 MUFU and ~136 issue slots per 16 evaluations.  The block's remaining n_pts % kLinP samples go
 // through signal_kernel with the same chunking (one more launch, same partial rows).
 constexpr int kLinP = 16;
+constexpr int kLinMid = 8;  // motion: the third record that fixes the quadratic of mu'
 
-template <bool PH64>
+// MO (motion plans, x(t) = x + v t): on a plateau the first moment mu' is a quadratic in the sample index, so
+// theta_j = theta_0 + j alpha + j^2 beta with alpha = dk' . x + a . v + f' dwell, beta = b . v (a, b from the group's
+// records 0, kLinMid, kLinP - 1), and w_{j+1} = w_j zeta_j, zeta_{j+1} = zeta_j rho with zeta_0 = q exp(i (alpha + beta)),
+// rho = exp(2 i beta): three sincos per spin and two complex multiplies per sample.  2 beta is tiny (1e-5 rad at
+// 0.1 m/s), so rho comes from its series and adds no MUFU error to the j^2 term.
+template <bool PH64, bool MO>
 __global__ void __launch_bounds__(kSigThreads, 2)
-signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__restrict__ A_,
+signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__restrict__ A_, const void *__restrict__ V_,
                   const float4 *__restrict__ S, int n_spins, int spins_per_chunk,
                   const float *__restrict__ scal /* [0] = max 1/T2 */, float2 *__restrict__ partial, int row_stride,
                   int p_off) {
     constexpr int P = kLinP;
+    constexpr int RS = MO ? 2 : 1;
     using RecT = typename std::conditional<PH64, double4, float4>::type;
     using PosT = typename std::conditional<PH64, double4, float4>::type;
     using real = typename std::conditional<PH64, double, float>::type;
     __shared__ __align__(128) PosT shA[2][kSigTile];
     __shared__ __align__(128) float4 shS[2][kSigTile];
+    __shared__ __align__(128) PosT shV[MO ? 2 : 1][MO ? kSigTile : 1];
     __shared__ __align__(8) uint64_t bar[2];
     const RecT *recs = reinterpret_cast<const RecT *>(recs_);
     const PosT *A = reinterpret_cast<const PosT *>(A_);
+    const PosT *V = reinterpret_cast<const PosT *>(V_);
     const int tid = threadIdx.x;
     const int s0 = blockIdx.y * spins_per_chunk;
     const int s1 = min(n_spins, s0 + spins_per_chunk);
@@ -303,9 +312,10 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
         const int b = t & 1;
         const int base = s0 + t * kSigTile;
         const uint32_t cnt = (uint32_t)min(kSigTile, s1 - base);
-        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + sizeof(float4)));
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)((MO ? 2 : 1) * sizeof(PosT) + sizeof(float4)));
         bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
         bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
+        if (MO) bulk_g2s(shV[b], V + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
     };
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -316,15 +326,29 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
     }
     const int g = blockIdx.x * (int)blockDim.x + tid;
     const bool live = g < n_groups;
-    RecT r0, r1;
+    RecT r0, r1, m0, m8, m15;
     r0.x = 0; r0.y = 0; r0.z = 0; r0.w = 0;
-    r1 = r0;
+    r1 = r0; m0 = r0; m8 = r0; m15 = r0;
     if (live) {
-        r0 = recs[(size_t)g * P];
-        r1 = recs[(size_t)g * P + P - 1];
+        r0 = recs[(size_t)RS * g * P];
+        r1 = recs[(size_t)RS * (g * P + P - 1)];
+        if (MO) {
+            m0 = recs[(size_t)RS * g * P + 1];
+            m8 = recs[(size_t)RS * (g * P + kLinMid) + 1];
+            m15 = recs[(size_t)RS * (g * P + P - 1) + 1];
+        }
     }
     constexpr real inv = (real)1 / (real)(P - 1);
     const real dkx = (r1.x - r0.x) * inv, dky = (r1.y - r0.y) * inv, dkz = (r1.z - r0.z) * inv, dta = (r1.w - r0.w) * inv;
+    // mu'(j) = m0 + a j + b j^2 through j = 0, kLinMid, P - 1
+    constexpr real i8 = (real)1 / (real)kLinMid, i7 = (real)1 / (real)(P - 1 - kLinMid);
+    const real bx = MO ? ((m15.x - m0.x) * inv - (m8.x - m0.x) * i8) * i7 : (real)0;
+    const real by = MO ? ((m15.y - m0.y) * inv - (m8.y - m0.y) * i8) * i7 : (real)0;
+    const real bz = MO ? ((m15.z - m0.z) * inv - (m8.z - m0.z) * i8) * i7 : (real)0;
+    // a + b (the first step's moment increment)
+    const real abx = MO ? (m8.x - m0.x) * i8 - (real)(kLinMid - 1) * bx : (real)0;
+    const real aby = MO ? (m8.y - m0.y) * i8 - (real)(kLinMid - 1) * by : (real)0;
+    const real abz = MO ? (m8.z - m0.z) * i8 - (real)(kLinMid - 1) * bz : (real)0;
     const float tf0 = (float)r0.w;
     const float cd = (float)dta * 0.6931471805599453f;  // dwell ln 2; times e2 = -log2(e)/T2 gives -dwell/T2
     // q = exp(-dwell/T2) by the cubic series when dwell/T2 <= 0.02 for every spin (as in signal_kernel), else MUFU.EX2
@@ -332,19 +356,23 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
     float ar[P], ai[P];
 #pragma unroll
     for (int j = 0; j < P; ++j) { ar[j] = 0.f; ai[j] = 0.f; }
-    auto phase_sincos = [&](real qx, real qy, real qz, real qt, const PosT &a, float &sn, float &cs) {
+    // sin and cos of k . x + w tau (+ u . v); fp32: radians, fp64: turns reduced as described in the file header
+    auto phase_sincos = [&](real qx, real qy, real qz, real qt, real ux, real uy, real uz, const PosT &a, const PosT &vv,
+                            float &sn, float &cs) {
         if (PH64) {
             double th = fma((double)qx, (double)a.x, fma((double)qy, (double)a.y,
                             fma((double)qz, (double)a.z, (double)qt * (double)a.w)));  // turns
-            th += 1572864.0;  // 1.5 * 2^20: low word = frac(theta) in 0.32 fixed point (see the file header)
+            if (MO) th = fma((double)ux, (double)vv.x, fma((double)uy, (double)vv.y, fma((double)uz, (double)vv.z, th)));
+            th += 1572864.0;  // 1.5 * 2^20: low word = frac(theta) in 0.32 fixed point
             const unsigned lo = (unsigned)__double2loint(th);
             const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;
             const float ang = fr * 6.283185307179586f;
             sn = __sinf(ang);
             cs = __cosf(ang);
         } else {
-            const float th = fmaf((float)qx, (float)a.x, fmaf((float)qy, (float)a.y,
-                                  fmaf((float)qz, (float)a.z, (float)qt * (float)a.w)));  // radians
+            float th = fmaf((float)qx, (float)a.x, fmaf((float)qy, (float)a.y,
+                            fmaf((float)qz, (float)a.z, (float)qt * (float)a.w)));  // radians
+            if (MO) th = fmaf((float)ux, (float)vv.x, fmaf((float)uy, (float)vv.y, fmaf((float)uz, (float)vv.z, th)));
             sn = __sinf(th);
             cs = __cosf(th);
         }
@@ -358,29 +386,51 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
         for (int s = 0; s < cnt; ++s) {
             const PosT a = shA[b][s];
             const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            PosT vv;
+            vv.x = 0; vv.y = 0; vv.z = 0; vv.w = 0;
+            if (MO) vv = shV[b][s];
             float sn, cs, sd, cdl;
-            phase_sincos(r0.x, r0.y, r0.z, r0.w, a, sn, cs);
-            phase_sincos(dkx, dky, dkz, dta, a, sd, cdl);
+            phase_sincos(r0.x, r0.y, r0.z, r0.w, m0.x, m0.y, m0.z, a, vv, sn, cs);
+            phase_sincos(dkx, dky, dkz, dta, abx, aby, abz, a, vv, sd, cdl);
             const float e = ex2_approx(tf0 * st.w);
             const float y = cd * st.w;  // -dwell/T2
             float qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
             if (!series) qd = ex2_approx((float)dta * st.w);
-            float pr = qd * cdl, pi = qd * sd;  // zeta^(2^m)
+            float pr = qd * cdl, pi = qd * sd;  // zeta (MO: zeta_0), then zeta^(2^m) (static) or zeta_j (MO)
             const float er = st.x * e, ei = st.y * e;
             float wr[P], wi[P];
             wr[0] = fmaf(er, cs, -ei * sn);
             wi[0] = fmaf(er, sn, ei * cs);
+            if (MO) {
+                // rho = exp(2 i beta): beta = b . v in turns (fp64) or radians (fp32)
+                float ang = 2.0f * (float)(bx * vv.x + by * vv.y + bz * vv.z);
+                if (PH64) ang *= 6.283185307179586f;
+                const float a2 = ang * ang;
+                float rr = fmaf(a2, fmaf(a2, 1.0f / 24.0f, -0.5f), 1.0f);
+                float ri = ang * fmaf(a2, fmaf(a2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+                if (fabsf(ang) > 0.05f) { rr = __cosf(ang); ri = __sinf(ang); }  // series truncation 2e-11 below that
 #pragma unroll
-            for (int h = 1; h < P; h *= 2) {
-#pragma unroll
-                for (int j = 0; j < h; ++j) {
-                    wr[h + j] = fmaf(wr[j], pr, -wi[j] * pi);
-                    wi[h + j] = fmaf(wr[j], pi, wi[j] * pr);
-                }
-                if (2 * h < P) {
-                    const float t2 = fmaf(pr, pr, -pi * pi);
-                    pi = 2.0f * pr * pi;
+                for (int j = 1; j < P; ++j) {
+                    wr[j] = fmaf(wr[j - 1], pr, -wi[j - 1] * pi);
+                    wi[j] = fmaf(wr[j - 1], pi, wi[j - 1] * pr);
+                    const float t2 = fmaf(pr, rr, -pi * ri);
+                    pi = fmaf(pr, ri, pi * rr);
                     pr = t2;
+                }
+            } else {
+                // w_j = w_0 zeta^j through zeta^2, zeta^4, zeta^8: dependency depth log2(P)
+#pragma unroll
+                for (int h = 1; h < P; h *= 2) {
+#pragma unroll
+                    for (int j = 0; j < h; ++j) {
+                        wr[h + j] = fmaf(wr[j], pr, -wi[j] * pi);
+                        wi[h + j] = fmaf(wr[j], pi, wi[j] * pr);
+                    }
+                    if (2 * h < P) {
+                        const float t2 = fmaf(pr, pr, -pi * pi);
+                        pi = 2.0f * pr * pi;
+                        pr = t2;
+                    }
                 }
             }
 #pragma unroll

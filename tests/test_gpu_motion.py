@@ -130,3 +130,25 @@ def test_zero_velocity_equals_the_static_plan_and_velocities_need_a_motion_plan(
         plan.simulate(*dev, velocity=vel)
     assert e.value.code == -1
     plan.close()
+
+
+@pytest.mark.parametrize("phase_mode,n_adc", [("fp32", 2051), ("fp64", 4096)])
+def test_moving_spins_on_cartesian_plateau_take_the_quadratic_recurrence(B, oracle_mod, phase_mode, n_adc, monkeypatch):
+    """>= 2048 equally spaced samples on a plateau with moving spins: k' is linear and the first moment mu' quadratic in
+    the sample index, so the planner hands the block to signal_lin_kernel<., motion> (w_{j+1} = w_j zeta_j,
+    zeta_{j+1} = zeta_j rho).  Against the oracle and against the per-sample kernel (BLOCH_SIGNAL_LIN=0)."""
+    import torch
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    dwell = 4e-6
+    t1 = 4e-4 + n_adc * dwell
+    g = {0: ([2e-4, 3e-4, t1], [0, 1e-3, 1e-3]), 1: ([2e-4, 3e-4, t1], [0, -5e-4, -5e-4])}
+    adc = 3.5e-4 + (np.arange(n_adc) + 0.5) * dwell
+    s = seq(g=g, rf=rf, adc=adc, t_end=t1 + 1e-4, dt_rf_max=1.0)
+    ph, v = moving_phantom(700, 31)
+    out = {}
+    for lin in ("1", "0"):
+        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
+        out[lin], _ = run_both(B, oracle_mod, ph, s, v, 1e-5, f"motion recurrence {phase_mode} lin={lin}", phase_mode=phase_mode)
+    emax, nrmse = errors(out["1"], out["0"])
+    print(f"motion recurrence on/off {phase_mode}: max {emax:.3e} nrmse {nrmse:.3e}")
+    assert 0 < emax <= 3e-5 and nrmse <= 8e-6
