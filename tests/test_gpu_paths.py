@@ -272,3 +272,44 @@ def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_
     emax, nrmse = errors(out["1"], out["0"])
     print(f"lin kernel on/off {phase_mode} n_adc={n_adc}: max {emax:.3e} nrmse {nrmse:.3e}")
     assert 0 < emax <= 3e-5 and nrmse <= 8e-6     # fp32: both sit on the fp32 phase floor (no echo in this sequence)
+
+
+@pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
+def test_signal_lin_kernel_on_an_epi_train_of_short_lines(B, oracle_mod, phase_mode, monkeypatch):
+    """50 EPI lines of 48 samples on the plateaus only (ramps and blips between lines are not sampled): every aligned
+    group of 16 lies inside one line, so the whole 2400-sample block goes to signal_lin_kernel although k' and tau
+    jump between groups.  A second sequence shifts the first line by 5 samples: groups then straddle the line ends,
+    the planner must NOT flag the block, and the per-warp choice inside signal_kernel takes over."""
+    import torch
+    rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
+    dwell, n_line, n_lines, ramp, G = 5e-6, 48, 50, 1e-4, 6e-3
+    ph = rand_phantom(900, 29)
+    dev = B.phantom_to_device(ph)
+    for extra in (0, 5):
+        t, v, ty, vy, adc = [2e-4], [0.0], [2e-4], [0.0], []
+        for ln in range(n_lines):
+            sgn = 1.0 if ln % 2 == 0 else -1.0
+            t0 = t[-1]
+            n_here = n_line + (extra if ln == 0 else 0)
+            flat = n_here * dwell
+            t += [t0 + ramp, t0 + ramp + flat, t0 + 2 * ramp + flat]
+            v += [sgn * G, sgn * G, 0.0]
+            adc.append(t0 + ramp + (np.arange(n_here) + 0.5) * dwell)
+            ty += [t0 + 2 * ramp + flat - 5e-5, t0 + 2 * ramp + flat - 2.5e-5, t0 + 2 * ramp + flat]
+            vy += [0.0, 1.5e-3, 0.0]
+        adc = np.concatenate(adc)
+        s = seq(g={0: (t, v), 1: (ty, vy)}, rf=rf, adc=adc, t_end=t[-1] + 1e-4, dt_rf_max=1.0)
+        check(B, oracle_mod, ph, s, f"EPI short lines {phase_mode} shift={extra}", phase_mode=phase_mode)
+        out = {}
+        for lin in ("1", "0"):
+            monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
+            plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+            out[lin] = plan.simulate(*dev).cpu().numpy()
+            torch.cuda.synchronize()
+            plan.close()
+        monkeypatch.delenv("BLOCH_SIGNAL_LIN")
+        emax, nrmse = errors(out["1"], out["0"])
+        print(f"EPI short lines on/off {phase_mode} shift={extra}: max {emax:.3e} nrmse {nrmse:.3e}")
+        assert emax <= 3e-5 and nrmse <= 8e-6
+        if extra == 0:
+            assert emax > 0      # the recurrence kernel did run
