@@ -358,23 +358,35 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
     for (int j = 0; j < P; ++j) { ar[j] = 0.f; ai[j] = 0.f; }
     // sin and cos of k . x + w tau (+ u . v); fp32: radians, fp64: turns reduced as described in the file header
     auto phase_sincos = [&](real qx, real qy, real qz, real qt, real ux, real uy, real uz, const PosT &a, const PosT &vv,
-                            float &sn, float &cs) {
+                            float &sn, float &cs, bool accurate) {
         if (PH64) {
             double th = fma((double)qx, (double)a.x, fma((double)qy, (double)a.y,
                             fma((double)qz, (double)a.z, (double)qt * (double)a.w)));  // turns
             if (MO) th = fma((double)ux, (double)vv.x, fma((double)uy, (double)vv.y, fma((double)uz, (double)vv.z, th)));
             th += 1572864.0;  // 1.5 * 2^20: low word = frac(theta) in 0.32 fixed point
             const unsigned lo = (unsigned)__double2loint(th);
-            const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;
-            const float ang = fr * 6.283185307179586f;
-            sn = __sinf(ang);
-            cs = __cosf(ang);
+            if (accurate) {
+                // the step's rotation is applied up to P - 1 times: full-precision sincos of the signed fraction
+                const float fs = (float)(int)lo * 2.3283064365386963e-10f;  // [-0.5, 0.5) turns
+                sincospif(2.0f * fs, &sn, &cs);
+            } else {
+                const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;
+                const float ang = fr * 6.283185307179586f;
+                sn = __sinf(ang);
+                cs = __cosf(ang);
+            }
         } else {
             float th = fmaf((float)qx, (float)a.x, fmaf((float)qy, (float)a.y,
                             fmaf((float)qz, (float)a.z, (float)qt * (float)a.w)));  // radians
             if (MO) th = fmaf((float)ux, (float)vv.x, fmaf((float)uy, (float)vv.y, fmaf((float)uz, (float)vv.z, th)));
-            sn = __sinf(th);
-            cs = __cosf(th);
+            if (accurate) {
+                float r = th * 0.15915494309189535f;  // turns; the step's phase is a few radians at most
+                r -= rintf(r);
+                sincospif(2.0f * r, &sn, &cs);
+            } else {
+                sn = __sinf(th);
+                cs = __cosf(th);
+            }
         }
     };
     __syncthreads();
@@ -390,8 +402,8 @@ signal_lin_kernel(const void *__restrict__ recs_, int n_groups, const void *__re
             vv.x = 0; vv.y = 0; vv.z = 0; vv.w = 0;
             if (MO) vv = shV[b][s];
             float sn, cs, sd, cdl;
-            phase_sincos(r0.x, r0.y, r0.z, r0.w, m0.x, m0.y, m0.z, a, vv, sn, cs);
-            phase_sincos(dkx, dky, dkz, dta, abx, aby, abz, a, vv, sd, cdl);
+            phase_sincos(r0.x, r0.y, r0.z, r0.w, m0.x, m0.y, m0.z, a, vv, sn, cs, false);
+            phase_sincos(dkx, dky, dkz, dta, abx, aby, abz, a, vv, sd, cdl, true);
             const float e = ex2_approx(tf0 * st.w);
             const float y = cd * st.w;  // -dwell/T2
             float qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
