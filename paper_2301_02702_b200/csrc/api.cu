@@ -87,7 +87,20 @@ int sig_max_P(const bloch_plan *plan) {
 // whatever the plan (their kernel holds 2 CTAs per SM also with fp64 phase and motion).
 SigShape block_shape(const bloch_plan *plan, const Block &b, int64_t n_spins, int sm_count) {
     const bool lin = b.lin_pts > 0 && env_int("BLOCH_SIGNAL_LIN", 1);
-    return sig_shape(b.adc_count, n_spins, sm_count, lin ? 8 : sig_max_P(plan));
+    if (!lin) return sig_shape(b.adc_count, n_spins, sm_count, sig_max_P(plan));
+    // signal_lin_kernel: one thread per group of kLinP samples, 2 CTAs of 256 threads per SM (or proportionally more
+    // CTAs of fewer warps for short blocks), the spins split over enough chunks to fill the machine
+    SigShape s;
+    s.P = kLinP;
+    const int64_t n_groups = b.lin_pts / kLinP;
+    s.threads = (int)std::min<int64_t>(kSigThreads, (n_groups + 31) / 32 * 32);
+    s.ptiles = (int)((n_groups + s.threads - 1) / s.threads);
+    const int per_sm = std::min(2 * (kSigThreads / s.threads), 8);
+    int64_t chunks = ((int64_t)sm_count * per_sm + s.ptiles - 1) / s.ptiles;
+    chunks = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(chunks, (n_spins + 31) / 32), 65535));
+    s.spins_per_chunk = (int)std::max<int64_t>(1, (n_spins + chunks - 1) / chunks);
+    s.chunks = (int)std::max<int64_t>(1, (n_spins + s.spins_per_chunk - 1) / s.spins_per_chunk);
+    return s;
 }
 
 // Partial-sum buffer (a7): consecutive ADC-bearing precession blocks with the same launch shape share one
@@ -760,14 +773,14 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     // samples): the recurrence kernel on the first lin_pts samples, the n % kLinP tail through
                     // signal_kernel<1>; both with this block's chunking, so the partial rows and the second pass are unchanged
                     const int n_groups = (int)(b.lin_pts / kLinP);
-                    const dim3 lgrid((unsigned)((n_groups + kSigThreads - 1) / kSigThreads), s.chunks);
+                    const dim3 lgrid(s.ptiles, s.chunks);
                     const int n_tail = n_pts - (int)b.lin_pts;
                     const void *trecs = (const unsigned char *)recs + (size_t)b.lin_pts * (ph64 ? 32 : 16) * (mo ? 2 : 1);
                     const dim3 tgrid(1, s.chunks);
                     const int toff = poff + (int)b.lin_pts;
 #define BLOCH_LAUNCH_LIN(H, M, AP, VP)                                                                              \
     do {                                                                                                            \
-        signal_lin_kernel<H, M><<<lgrid, kSigThreads, 0, stream>>>(recs, n_groups, AP, VP, w.S, n, s.spins_per_chunk, \
+        signal_lin_kernel<H, M><<<lgrid, s.threads, 0, stream>>>(recs, n_groups, AP, VP, w.S, n, s.spins_per_chunk, \
                                                                    (const float *)w.scal, w.partial, row, poff);    \
         if (n_tail > 0)                                                                                             \
             signal_kernel<1, H, M><<<tgrid, 32, 0, stream>>>(trecs, n_tail, AP, VP, w.S, n, s.spins_per_chunk,      \

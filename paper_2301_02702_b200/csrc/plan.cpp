@@ -378,7 +378,10 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         // Checked on the fp64 records (turns / m): every sample within 1e-13 relative + 1e-8 turns / m (1e-13 s) of the
         // line through the group's first and last sample, the level at which the ADC times themselves are equally
         // spaced.  Such blocks go to signal_lin_kernel (signal.cuh), the n % 16 tail to signal_kernel.
-        if (b.type == kBlockPrecession && b.adc_count >= 2048) {
+        // (blocks of >= 20 groups that fill >= 60 % of the lanes of their warps: below that the per-sample kernel,
+        // which gives every lane a sample, is the faster one)
+        const int64_t lin_groups = b.adc_count / 16;
+        if (b.type == kBlockPrecession && lin_groups >= 20 && 10 * lin_groups >= 6 * ((lin_groups + 31) / 32 * 32)) {
             const double *src = krec.data() + 4 * krec_first[bi];
             const int64_t n_g = b.adc_count / 16;
             bool ok = true;
