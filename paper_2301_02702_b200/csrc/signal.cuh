@@ -117,14 +117,14 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
     // zeta = q exp(i delta), delta = dk' . x + f' dwell: one sincos for theta_0 and one for delta per spin, then one
     // complex multiply per sample on the FMA pipe -- (5 MUFU + ~74 issue slots) / P instead of 2 + 1/P MUFU per
     // evaluation.  dk' is the slope through the thread's first and last sample; the mode is taken when every
-    // sample in between lies on that line to within the rounding of the table itself (1.25e-7 relative to the larger
-    // end in fp32, i.e. 1-2 ulp; 1e-13 in fp64), so the phase it reconstructs differs from the tabulated one by no more
+    // sample in between lies on that line to within the rounding of the table itself (2.5e-7 relative to the larger
+    // end in fp32, i.e. 2-4 ulp; 1e-13 in fp64), so the phase it reconstructs differs from the tabulated one by no more
     // than the table's own rounding.  Not for motion plans (the first-moment term is quadratic in time).
     real dkx = 0, dky = 0, dkz = 0, dta = 0;
     bool lin = false;
     if (!MO && P > 2 && allow_lin) {
         constexpr real inv = (real)1 / (real)(P - 1);
-        constexpr real rel = PH64 ? (real)1e-13 : (real)1.25e-7;
+        constexpr real rel = PH64 ? (real)1e-13 : (real)2.5e-7;  // fp32: 1 ulp of table rounding + 1 ulp of this check's own arithmetic
         dkx = (kx[P - 1] - kx[0]) * inv;
         dky = (ky[P - 1] - ky[0]) * inv;
         dkz = (kz[P - 1] - kz[0]) * inv;
