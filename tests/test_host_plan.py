@@ -159,3 +159,28 @@ def test_scanner_limits_are_checked_when_given(B):
     for name in ("1", "2", "3"):
         h = B.bloch_plan_create(W.small(name).seq, G_max=60e-3)
         B.bloch_plan_destroy(h)
+
+
+def test_planner_flags_all_cartesian_blocks_for_the_recurrence_kernel(B):
+    """Block::lin_pts is visible through n_launches: a flagged block whose length is not a multiple of 16 costs one more
+    launch (its tail).  Flagged: equally spaced samples on a plateau (also with motion, where mu' is a parabola).
+    Not flagged: samples running through the ramp (k' quadratic), unequal spacing, fewer than 20 groups."""
+    def launches(adc, g, **kw):
+        s = seq(g=g, adc=adc, t_end=3.1e-2)
+        h = B.bloch_plan_create(s, **kw)
+        info = B.bloch_plan_get_info(h)
+        B.bloch_plan_destroy(h)
+        return info["n_launches"]
+
+    plateau = {0: ([1e-4, 2e-4, 3e-2], [0, 5e-3, 5e-3])}
+    t0, dw = 2.5e-4, 5e-6
+    base = launches(t0 + np.arange(2048) * dw, plateau)
+    assert launches(t0 + np.arange(2053) * dw, plateau) == base + 1                      # tail of 5 samples
+    assert launches(t0 + np.arange(2053) * dw, plateau, motion="linear", dt_max=1e-5) == \
+        launches(t0 + np.arange(2048) * dw, plateau, motion="linear", dt_max=1e-5) + 1
+    assert launches(1.5e-4 + np.arange(2053) * dw, plateau) == base                      # first samples on the ramp
+    jit = t0 + np.arange(2053) * dw
+    jit[1000] += 1e-9
+    assert launches(jit, plateau) == base                                                # one sample 1 ns late
+    assert launches(t0 + np.arange(317) * dw, plateau) == base                           # 19 groups: too short
+    assert launches(t0 + np.arange(325) * dw, plateau) == base + 1                       # 20 groups + tail of 5
