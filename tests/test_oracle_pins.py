@@ -387,6 +387,28 @@ def test_grid_contents_and_rf_refinement(oracle_mod):
     assert adc.tolist() == [-1] * 7 + [0, -1, 1, -1, -1]
 
 
+@pytest.mark.parametrize("t0", [0.0, 0.7300001, 12.000123, 14.9876543])
+def test_rf_train_late_in_a_long_sequence_keeps_its_nominal_step_count(oracle_mod, t0):
+    """Reading G18, pinned by counting: an RF train of 1000 samples of nominal 1 us with
+    dt_rf_max = 1 us is 1000 RF intervals wherever it sits on the time axis.  At t ~ 12 s the spacing of doubles is
+    1.8e-15 s, so rf_t[i+1] - rf_t[i] exceeds 1e-6 by rounding for about a third of the samples; a refinement rule
+    without the 1e-12 s time tolerance (reading G13) cuts those in two (it did: 362 of config 5's 1000 TRs).  A piece
+    that really is longer than dt_rf_max -- by more than the tolerance -- is still cut."""
+    n, dt = 1000, 1e-6
+    rf_t = t0 + np.arange(n) * dt
+    s = seq(rf=(rf_t, np.full(n, dt), np.full(n, 1e-6), np.zeros(n)), t_end=t0 + n * dt + 1e-3, dt_rf_max=dt)
+    t, _, rf, _ = oracle_mod.grid(s)
+    assert int(rf.sum()) == n                                   # the nominal count, not n + (rounding splits)
+    steps = np.diff(t)[rf.astype(bool)]
+    assert steps.min() > 0.99 * dt and steps.max() < 1.01 * dt  # and no half steps hide in it
+    # the physics agrees: the train's flip angle on resonance is gamma * B1 * n * dt whatever the grid (P3), so the
+    # count is the only thing this reading can change -- and the count is what the benchmark's spin*steps are made of
+    # genuinely longer pieces are cut: 2.5 us -> 3 sub-steps, 1 us + 5e-12 s -> 2
+    for dur, parts in ((2.5e-6, 3), (1e-6 + 5e-12, 2), (1e-6 + 5e-13, 1)):
+        s2 = seq(rf=([t0 + 1e-4], [dur], [1e-6], [0.0]), t_end=t0 + 1e-3, dt_rf_max=dt)
+        assert int(oracle_mod.grid(s2)[2].sum()) == parts
+
+
 # ---------------------------------------------------------------------------------------------- f2
 def test_grouped_output_is_a_fisp_ensemble_dictionary(oracle_mod):
     """three (T1, T2) entries, each an ensemble of 128 isochromats whose spoiler phase covers
