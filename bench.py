@@ -3,18 +3,23 @@
 free-precession block, the two-pass signal reduction, final state) over one synthetic workload.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4] [--impl ours|reference]
+                    [--scaling weak|strong] [--extra 1,2,3,5,5b | none]
 
 Prints ONE JSON line (rank 0).  metric = Bloch spin*steps/s: N_spins x N_intervals of the discretised
 sequence (what the step-by-step solver of the paper executes, SURVEY.md 8(d) "Counting") / device time.
-See DESIGN.md "Measurement" for the roofline arithmetic.  The reference arm (--impl reference) times the
-fp64 CPU oracle, as it stands, on the host cores; it is the only place besides cpu_baseline that touches
-oracle/.
+The headline workload is config 4 (the 1M-spin spiral); the default run also times the other named configs
+(BASELINE.json: "report throughput on the five synthetic workloads") in short runs and reports them under
+"workloads".  See DESIGN.md "Measurement" for the roofline arithmetic.  The reference arm (--impl reference)
+times the fp64 CPU oracle, as it stands, on the host cores; it is the only place besides cpu_baseline that
+touches oracle/.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
+import re
 import sys
 import threading
 import time
@@ -33,11 +38,7 @@ SM_COUNT = 148
 MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)
 FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
 FP32_PER_EVAL = 15         # FP32-pipe instructions per (spin, evaluated point)
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full captures
-NCU_TRAFFIC = {("config4_1M_spiral", "signal"): (32.08e6, "profiles/r01_v3_signal_kernel_cfg4_ncu.txt"),
-               ("config4_1M_spiral", "rf"): (48.11e6, "profiles/r01_v3_rf_kernel_cfg4_ncu.txt"),
-               ("config3_brain_epi128", "signal"): (6.57e6, "profiles/r01_v4_signal_lin_kernel_cfg3_ncu.txt"),
-               ("config5_mrf_fisp", "fused"): (1229.9e6, "profiles/r01_v3_seq_kernel_cfg5_ncu.txt")}
+EXTRA_DEFAULT = "1,2,3,5,5b"
 
 
 def load_peaks():
@@ -46,6 +47,73 @@ def load_peaks():
             return json.load(f)
     except Exception:
         return {}
+
+
+# --------------------------------------------------------------------------------------------------
+# committed ncu captures (profiles/*_ncu.txt): read at run time, used only when they describe the launch
+# --------------------------------------------------------------------------------------------------
+_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def parse_ncu_txt(path: str):
+    """One `ncu --set full` summary as committed under profiles/: 'kernel: [void ]NAME(args' then
+    '  metric [unit] = value' lines.  Returns {"kernel", "grid", "block", "metrics": {name: (value, unit)}}."""
+    out = {"kernel": None, "grid": None, "block": None, "metrics": {}, "file": os.path.relpath(path, ROOT)}
+    try:
+        with open(path) as f:
+            for line in f:
+                m = re.match(r"\s*kernel:\s*(?:void\s+)?([^()]+)\(", line)
+                if m and out["kernel"] is None:
+                    out["kernel"] = m.group(1).replace("bloch::", "").replace(" ", "")
+                    continue
+                m = re.match(r"\s*([A-Za-z0-9_.]+)\s*\[([^\]]*)\]\s*=\s*([-+0-9.eE]+)\s*$", line)
+                if m:
+                    out["metrics"][m.group(1)] = (float(m.group(3)), m.group(2))
+    except OSError:
+        return None
+    g, b = out["metrics"].get("launch__grid_size"), out["metrics"].get("launch__block_size")
+    out["grid"], out["block"] = (int(g[0]) if g else None), (int(b[0]) if b else None)
+    return out
+
+
+def find_capture(kernel: dict):
+    """The newest committed capture whose kernel name, grid and block size are those of the launch just timed
+    (bloch_plan_last_kernel), or None: a capture of another kernel, another build's template arguments or another
+    launch shape says nothing about this run."""
+    if not kernel or not kernel.get("name"):
+        return None
+    want = kernel["name"].replace(" ", "")
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu.txt"))):
+        cap = parse_ncu_txt(path)
+        if cap and cap["kernel"] == want and cap["grid"] == kernel["grid"] and cap["block"] == kernel["block"]:
+            best = cap       # sorted by name: rNN_vM -> the latest round / version wins
+    return best
+
+
+def capture_fields(kernel: dict, pipe: str):
+    """traffic (DRAM bytes per launch), pipe_util and issue_util (fractions, <= 1) from the matching capture."""
+    cap = find_capture(kernel)
+    if cap is None:
+        return {"traffic": None, "traffic_source": None, "pipe_util": None, "issue_util": None,
+                "capture_note": f"no committed profiles/*_ncu.txt capture matches {kernel.get('name')} "
+                                f"grid {kernel.get('grid')} block {kernel.get('block')}"}
+    m = cap["metrics"]
+
+    def nbytes(key):
+        v = m.get(key)
+        return v[0] * _SCALE.get(v[1], 1.0) if v else 0.0
+
+    def pct(key):
+        v = m.get(key)
+        return v[0] / 100.0 if v else None
+    pipe_key = {"mufu": "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active",
+                "fp32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"}[pipe]
+    have = "dram__bytes_read.sum" in m
+    return {"traffic": nbytes("dram__bytes_read.sum") + nbytes("dram__bytes_write.sum") if have else None,
+            "traffic_source": cap["file"], "pipe_util": pct(pipe_key),
+            "issue_util": pct("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+            "capture_kernel": {"name": cap["kernel"], "grid": cap["grid"], "block": cap["block"]}}
 
 
 class ClockSampler:
@@ -83,6 +151,7 @@ class ClockSampler:
 
     def __enter__(self):
         if self._nv is not None:
+            self._stop.clear()
             self._thr = threading.Thread(target=self._run, daemon=True)
             self._thr.start()
         return self
@@ -91,26 +160,36 @@ class ClockSampler:
         self._stop.set()
         if self._thr is not None:
             self._thr.join()
+            self._thr = None
 
     def summary(self):
         return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def make_workload(name: str, rank: int):
-    """Rank r simulates shard r of an (N x n_spins)-spin phantom on the SAME sequence: the phantom comes from
-    the same generator with the seed moved by the rank (weak scaling: per-GPU work is fixed)."""
+def make_workload(name: str, rank: int, world: int, scaling: str):
+    """weak (default): rank r simulates shard r of a (world x n_spins)-spin phantom on the SAME sequence; the
+    phantom comes from the same generator with the seed moved by the rank (per-GPU work is fixed).
+    strong: every rank builds the SAME named workload and keeps the contiguous spin range dist.shard_bounds gives it
+    (total work is fixed)."""
     from paper_2301_02702_b200 import workloads as W
+    import dataclasses
     w = W.make(name)
+    if scaling == "strong":
+        from paper_2301_02702_b200.dist import shard_bounds
+        lo, hi = shard_bounds(w.phantom.n, rank, world)
+        idx = np.arange(lo, hi)
+        vel = None if w.velocity is None else tuple(np.ascontiguousarray(a[idx]) for a in w.velocity)
+        coils = None if w.coils is None else np.ascontiguousarray(w.coils[:, idx])
+        return dataclasses.replace(w, phantom=w.phantom.subset(idx), velocity=vel, coils=coils), w
     if rank:
         base = W.SEED0
         try:
             W.SEED0 = base + 1000 * rank
-            import dataclasses
             w = dataclasses.replace(w, phantom=W.make(name).phantom)
         finally:
             W.SEED0 = base
-    return w
+    return w, w
 
 
 def oracle_sample(w, budget_spin_steps: float, n_intervals: int):
@@ -157,7 +236,7 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     import oracle
-    w = make_workload(args.workload, 0)
+    w, _ = make_workload(args.workload, 0, 1, "weak")
     t, _, _, _ = oracle.grid(w.seq, dt_max=w.dt_max if w.velocity is not None else 0.0)
     n_int = len(t) - 1
     cores = os.cpu_count() or 1
@@ -174,7 +253,7 @@ def run_reference(args, rank, world):
     value = take * n_int * len(times) / total
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
-           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": w.name, "n_spins": w.phantom.n, "n_intervals": n_int,
                       "sample_spins_per_step": take},
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -184,22 +263,67 @@ def run_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
-def run_ours(args, rank, local_rank, world):
-    import torch
-    import torch.distributed as dist
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    from paper_2301_02702_b200 import build as bl
-    if rank == 0:
-        bl.build()
-    if world > 1:
-        dist.barrier()
-    from paper_2301_02702_b200 import bloch
-    from paper_2301_02702_b200.dist import reduce_signal
+def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, n_coils):
+    """Per kernel kind: achieved = ALGORITHMIC ops per launch (SURVEY.md 8(d) per-unit figure x units) / measured
+    launch duration; frac = achieved / pipe peak.  Because the kernels execute FEWER operations than the algorithmic
+    count (one ex2 shared by 8 samples, rotation recurrences), frac can exceed 1; pipe_util / issue_util from the
+    matching committed ncu capture are the "how busy is the pipe" numbers and never do."""
+    mufu_peak = SM_COUNT * 16 * sm_max * 1e6          # MUFU ops/s
+    fp32_peak = SM_COUNT * 128 * sm_max * 1e6         # FP32 instr/s
+    n_eval_sig = float(n) * float(info["n_adc"])      # evaluations in the signal kernels per step
+    rf_steps = float(n) * float(info["n_rf_steps"])
+    kern = {}
 
-    w = make_workload(args.workload, rank)
+    def entry(kind, pipe, ops, note):
+        dur = kinds_ms[kind] * 1e-3 / steps
+        peak = mufu_peak if pipe == "mufu" else fp32_peak
+        k = bloch.bloch_plan_last_kernel(plan.handle, kind)
+        e = {"bound": "alu", "pipe": pipe, "achieved": ops / dur / 1e12, "peak": peak / 1e12,
+             "unit": "Tmufu-op/s" if pipe == "mufu" else "Tfp32-instr/s", "frac": ops / dur / peak,
+             "frac_definition": "algorithmic ops (SURVEY.md 8(d)) / measured time / pipe peak; the kernel may execute "
+                                "fewer ops than the algorithmic count, see pipe_util for the pipe's busy fraction",
+             "kernel": k, "note": note, "launches_per_step": kinds_n[kind] // steps, "ms_per_step": dur * 1e3,
+             "avg_launch_ms": kinds_ms[kind] / kinds_n[kind],
+             "algorithmic_ops_per_launch": ops * steps / kinds_n[kind]}
+        e.update(capture_fields(k, pipe))
+        return e
+
+    if kinds_n["signal"]:
+        kern["signal"] = entry("signal", "mufu", MUFU_PER_EVAL * n_eval_sig,
+                               "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample); the per-sample kernel "
+                               "issues 2 + 1/P (P adjacent samples share one ex2), the Cartesian recurrence kernels 5 per "
+                               "P samples (issue-bound, not MUFU-bound)")
+        kern["signal"]["coils"] = n_coils
+        if n_coils > 0:
+            # multi-coil receive: sin / cos / ex2 are coil-independent; every coil adds one complex MAC = 4 FP32
+            fp32_ops = (FP32_PER_EVAL + 4 * n_coils) * n_eval_sig
+            if fp32_ops / fp32_peak > MUFU_PER_EVAL * n_eval_sig / mufu_peak:
+                kern["signal"] = entry("signal", "fp32", fp32_ops,
+                                       f"{n_coils} coils: algorithmic count = 15 + 4 x n_coils FP32 instructions per "
+                                       "(spin, ADC sample); the 3 MUFU per evaluation are shared by all coils")
+                kern["signal"]["coils"] = n_coils
+    if kinds_n["rf"]:
+        kern["rf"] = entry("rf", "fp32", FP32_PER_RF_STEP * rf_steps,
+                           "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly); the "
+                           "tier-0 loop issues ~38.5 per step on plateau-gradient tiles")
+    if kinds_n["fused"]:
+        # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
+        # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)
+        fp32_ops = FP32_PER_RF_STEP * rf_steps + FP32_PER_EVAL * n_eval_sig
+        mufu_ops = MUFU_PER_EVAL * n_eval_sig
+        t_fp32, t_mufu = fp32_ops / fp32_peak, mufu_ops / mufu_peak
+        pipe, ops = ("fp32", fp32_ops) if t_fp32 >= t_mufu else ("mufu", mufu_ops)
+        kern["fused"] = entry("fused", pipe, ops,
+                              "seq_kernel (a5-a8 in one launch): algorithmic count = 46 FP32 per spin*step + 15 FP32 per "
+                              f"(spin, ADC sample); the MUFU count (3 per evaluation) would take {t_mufu * 1e3:.1f} ms, "
+                              f"the FP32 count {t_fp32 * 1e3:.1f} ms")
+    return kern
+
+
+def measure(bloch, torch, dist, w, w_whole, args, steps, warmup, rank, local_rank, world, flush, clocks,
+            with_e2e=True):
+    """Times `steps` passes of the hot path over workload `w` (this rank's share) and returns the result dict."""
+    from paper_2301_02702_b200.dist import reduce_signal
     per_spin = w.output_mode in ("per_spin", "grouped")   # no cross-rank sum: outputs stay sharded
     t_plan0 = time.perf_counter()
     plan = bloch.Plan(w.seq, path=args.path, **w.plan_kw)
@@ -209,7 +333,8 @@ def run_ours(args, rank, local_rank, world):
     info = plan.info
     n = w.phantom.n
     n_int = info["n_intervals"]
-    spin_steps = float(n) * float(n_int)
+    n_total = w_whole.phantom.n if args.scaling == "strong" else n * world
+    spin_steps_job = float(n_total) * float(n_int)
     dev = bloch.phantom_to_device(w.phantom)
     vel = None if w.velocity is None else tuple(
         torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
@@ -218,7 +343,7 @@ def run_ours(args, rank, local_rank, world):
     coils = None if w.coils is None else torch.from_numpy(np.ascontiguousarray(w.coils)).cuda()
     shape = plan._signal_shape(n) if coils is None else (int(coils.shape[0]), info["n_adc"])
     sig = torch.empty(shape, dtype=torch.complex64, device="cuda")
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    strong = args.scaling == "strong"
 
     def barrier():
         if world > 1:
@@ -228,19 +353,21 @@ def run_ours(args, rank, local_rank, world):
     def step():
         plan.simulate(*dev, Mxy=Mxy, Mz=Mz, init_equilibrium=True, signal=sig, velocity=vel, coils=coils)
         if not per_spin:
-            reduce_signal(sig)
+            # the ONE collective of the path; strong scaling adds the shards in rank order, so the
+            # result does not depend on the collective's algorithm
+            reduce_signal(sig, deterministic=strong)
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         flush.zero_()
         step()
     barrier()
+    plan.status()   # raises if pack_kernel found an invalid phantom or one outside the plan's phase range
 
     # ---- device-resident timing: K steps, L2 flushed (untimed) before each, CUDA events around each step.
     # Pass 1 (no per-kernel events) gives `value`; pass 2 repeats the same K steps with the library's per-kernel
     # CUDA events on the launching stream (they cost ~4 % on the 9000-launch MRF config) for the roofline.
     kinds_ms = {k: 0.0 for k in bloch.KINDS}
     kinds_n = {k: 0 for k in bloch.KINDS}
-    clocks = ClockSampler(local_rank)
     ms_pass = {}
     with clocks:
         for taps in (False, True):
@@ -248,7 +375,7 @@ def run_ours(args, rank, local_rank, world):
                 continue
             bloch.bloch_plan_set_profiling(plan.handle, taps)
             ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-                  for _ in range(args.steps)]
+                  for _ in range(steps)]
             barrier()
             for a, b in ev:
                 flush.zero_()
@@ -267,144 +394,167 @@ def run_ours(args, rank, local_rank, world):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
-    value = spin_steps * world * args.steps / (ms_total * 1e-3)
+    value = spin_steps_job * steps / (ms_total * 1e-3)
     bloch.bloch_plan_set_profiling(plan.handle, False)
+    launches = bloch.bloch_plan_last_launches(plan.handle)
+    fused = bloch.bloch_plan_uses_fused(plan.handle, n)
+
+    # ---- strong scaling: the reduced signal of the sharded run must be the 1-GPU signal of the whole workload
+    shard_check = None
+    if strong and not per_spin and rank == 0:
+        plan1 = bloch.Plan(w_whole.seq, path=args.path, **w_whole.plan_kw)
+        d1 = bloch.phantom_to_device(w_whole.phantom)
+        v1 = None if w_whole.velocity is None else tuple(
+            torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w_whole.velocity)
+        c1 = None if w_whole.coils is None else torch.from_numpy(np.ascontiguousarray(w_whole.coils)).cuda()
+        ref = plan1.simulate(*d1, velocity=v1, coils=c1)
+        torch.cuda.synchronize()
+        scale = float(ref.abs().max())
+        err = float((sig - ref).abs().max()) / scale
+        shard_check = {"max_err_vs_1gpu": err, "tol": 5e-6, "ok": bool(err <= 5e-6)}
+        plan1.close()
+        del d1, ref
+        assert err <= 5e-6, f"sharded + reduced signal differs from the 1-GPU signal: {err:.3e}"
 
     # ---- end to end through the host-buffer C-ABI entry: pinned host inputs, H2D + D2H inside the timed region
-    ph = w.phantom
-    pinned = [torch.from_numpy(np.ascontiguousarray(getattr(ph, k), dtype=np.float32)).pin_memory()
-              for k in ("x", "y", "z", "M0", "T1", "T2", "dw")]
-    h_sig = torch.empty(shape, dtype=torch.complex64).pin_memory()
-    h_arrs = [p.numpy() for p in pinned]
-    h_sig_np = h_sig.numpy()
-    e2e_steps = max(1, min(args.steps, 5))
-    h_vel = None
-    if w.velocity is not None:
-        pinned_v = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory() for a in w.velocity]
-        h_vel = [p.numpy() for p in pinned_v]
-    h_coils = None if w.coils is None else torch.from_numpy(np.ascontiguousarray(w.coils)).pin_memory()
-    h_coils_np = None if h_coils is None else h_coils.numpy()
+    e2e = None
+    if with_e2e:
+        ph = w.phantom
+        pinned = [torch.from_numpy(np.ascontiguousarray(getattr(ph, k), dtype=np.float32)).pin_memory()
+                  for k in ("x", "y", "z", "M0", "T1", "T2", "dw")]
+        h_sig = torch.empty(shape, dtype=torch.complex64).pin_memory()
+        h_arrs = [p.numpy() for p in pinned]
+        h_sig_np = h_sig.numpy()
+        e2e_steps = max(1, min(steps, 5))
+        h_vel = None
+        if w.velocity is not None:
+            pinned_v = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory() for a in w.velocity]
+            h_vel = [p.numpy() for p in pinned_v]
+        h_coils = None if w.coils is None else torch.from_numpy(np.ascontiguousarray(w.coils)).pin_memory()
+        h_coils_np = None if h_coils is None else h_coils.numpy()
 
-    def e2e_step():   # synchronous: returns after the D2H copy
-        plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel, coils=h_coils_np)
+        def e2e_step():   # synchronous: returns after the D2H copy
+            plan.simulate_host(*h_arrs, signal=h_sig_np, velocity=h_vel, coils=h_coils_np)
 
-    e2e_step()   # warm-up (allocates the scratch)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()
-        if not per_spin and world > 1:
-            reduce_signal(torch.from_numpy(h_sig_np).cuda())
-    barrier()
-    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        e2e_step()   # warm-up (allocates the scratch)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+            if not per_spin and world > 1:
+                reduce_signal(torch.from_numpy(h_sig_np).cuda(), deterministic=strong)
+        barrier()
+        e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+        h2d = sum(int(a.nbytes) for a in h_arrs) + (sum(int(a.nbytes) for a in h_vel) if h_vel else 0) + \
+            (int(h_coils.numel()) * 8 if h_coils is not None else 0)
+        e2e = {"value": spin_steps_job * e2e_steps / float(e2e_s.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": int(h_sig_np.nbytes), "steps": e2e_steps,
+               "api": "bloch_simulate_host (pinned host buffers)" if h_coils is None else
+                      "bloch_simulate_host_coils (pinned host buffers)"}
+
+    n_coils = 0 if coils is None else int(coils.shape[0])
+    sm_max = float(clocks.max_mhz or load_peaks().get("sm_max_mhz") or 1965.0)
+    kern = kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, n_coils) if ms_pass.get(True) else {}
+    # what the GPU evaluates (closed-form precession at ADC samples and block ends only; RF stepped): per second
+    evaluated = (float(n_total) * (info["n_rf_steps"] + info["n_eval_points"])) * steps / (ms_total * 1e-3)
+    res = {"workload": w.name, "value": value, "ms_per_step": ms_total / steps, "steps": steps, "warmup": warmup,
+           "n_spins_per_gpu": n, "n_spins_total": n_total, "n_intervals": n_int, "n_rf_steps": info["n_rf_steps"],
+           "n_adc": info["n_adc"], "n_blocks": info["n_blocks"], "output_mode": w.output_mode,
+           "motion": w.velocity is not None, "coils": n_coils,
+           "dtype": "f32" if info["phase_mode"] == 1 else "f32+f64phase",
+           "path": "fused" if fused else "per_block", "spin_steps_per_step": spin_steps_job,
+           "evaluated_units_per_s": evaluated, "plan_create_upload_s": plan_s, "e2e": e2e,
+           "gpu_launches": launches * steps, "launches_per_step": launches,
+           "ms_per_step_with_kernel_events": (ms_pass.get(True, 0.0) / steps) or None,
+           "kernels": kern, "ms_by_kind_per_step": {k: v / steps for k, v in kinds_ms.items()},
+           "shard_check": shard_check}
+    plan.close()
+    del dev, sig, Mxy, Mz
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
     if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_value = spin_steps * world * e2e_steps / float(e2e_s.item())
-    h2d = sum(int(a.nbytes) for a in h_arrs) + (sum(int(a.nbytes) for a in h_vel) if h_vel else 0) + \
-        (int(h_coils.numel()) * 8 if h_coils is not None else 0)
-    d2h = int(h_sig_np.nbytes)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2301_02702_b200 import build as bl
+    if rank == 0:
+        bl.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2301_02702_b200 import bloch
+
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    clocks = ClockSampler(local_rank)
+    w, w_whole = make_workload(args.workload, rank, world, args.scaling)
+    head = measure(bloch, torch, dist, w, w_whole, args, args.steps, args.warmup, rank, local_rank, world, flush, clocks)
+
+    # ---- the other named configs, short runs (BASELINE.json: "report throughput on the five synthetic workloads");
+    # single GPU only: under torchrun the scaling arm times the headline workload alone
+    extra = {}
+    names = [s for s in args.extra.split(",") if s and s != "none"] if world == 1 else []
+    for name in names:
+        if name == args.workload:
+            continue
+        t0 = time.perf_counter()
+        wx, wx_whole = make_workload(name, 0, 1, "weak")
+        r = measure(bloch, torch, dist, wx, wx_whole, args, args.extra_steps, max(3, args.warmup), 0, local_rank, 1, flush,
+                    clocks)
+        r["bench_wall_s"] = time.perf_counter() - t0
+        r["kernels"] = {k: {f: v[f] for f in ("pipe", "frac", "pipe_util", "issue_util", "ms_per_step", "avg_launch_ms",
+                                              "launches_per_step", "kernel", "traffic", "traffic_source")}
+                        for k, v in r["kernels"].items()}
+        extra[name] = r
 
     if rank != 0:
         return
-    peaks = load_peaks()
-    sm_max = float(clocks.max_mhz or peaks.get("sm_max_mhz") or 1965.0)
-    mufu_peak = SM_COUNT * 16 * sm_max * 1e6          # MUFU ops/s
-    fp32_peak = SM_COUNT * 128 * sm_max * 1e6         # FP32 instr/s
-    n_eval_sig = float(n) * float(info["n_adc"])      # evaluations in the signal kernels per step
-    n_coils = 0 if coils is None else int(coils.shape[0])
-    n_pass = max(1, (n_coils + 3) // 4)               # the coil kernel evaluates sin / cos / ex2 once per 4 coils
-    rf_steps = float(n) * float(info["n_rf_steps"])
-    kern = {}
-    if kinds_n["signal"]:
-        dur = kinds_ms["signal"] * 1e-3 / args.steps
-        ach = MUFU_PER_EVAL * n_eval_sig / dur
-        kern["signal"] = {"bound": "alu", "pipe": "mufu", "achieved": ach / 1e12, "peak": mufu_peak / 1e12,
-                          "unit": "Tmufu-op/s", "frac": ach / mufu_peak,
-                          "traffic": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[0],
-                          "traffic_source": NCU_TRAFFIC.get((w.name, "signal"), (None, None))[1],
-                          "coils": n_coils,
-                          "note": "algorithmic count = 3 MUFU (sin, cos, ex2) per (spin, ADC sample), SURVEY.md 8(d); "
-                                  "the kernel issues 2 + 1/P (P = 8 adjacent samples share one ex2; 4 in shorter blocks), so frac "
-                                  "can reach 3 / 2.125 = 1.41 at a saturated MUFU pipe; on Cartesian readouts (k' advances by a constant step) the "
-                                  "rotation recurrence issues 5 MUFU per P samples and the loop is issue-bound instead, so frac exceeds that",
-                          "launches_per_step": kinds_n["signal"] // args.steps, "ms_per_step": dur * 1e3,
-                          "avg_launch_ms": kinds_ms["signal"] / kinds_n["signal"],
-                          "algorithmic_ops_per_launch": MUFU_PER_EVAL * n_eval_sig * args.steps / kinds_n["signal"]}
-    if kinds_n["signal"] and n_coils > 0:
-        # multi-coil receive: sin / cos / ex2 are coil-independent (3 MUFU per evaluation whatever the number of
-        # coils); every coil adds one complex multiply-accumulate = 4 FP32 instructions per evaluation
-        dur = kinds_ms["signal"] * 1e-3 / args.steps
-        fp32_ops = (FP32_PER_EVAL + 4 * n_coils) * n_eval_sig
-        if fp32_ops / fp32_peak > MUFU_PER_EVAL * n_eval_sig / mufu_peak:
-            kern["signal"].update({"pipe": "fp32", "achieved": fp32_ops / dur / 1e12, "peak": fp32_peak / 1e12,
-                                   "unit": "Tfp32-instr/s", "frac": fp32_ops / dur / fp32_peak,
-                                   "algorithmic_ops_per_launch": fp32_ops * args.steps / kinds_n["signal"],
-                                   "note": f"signal_coils_kernel, {n_coils} coils: algorithmic count = 15 + 4 x n_coils FP32 "
-                                           "instructions per (spin, ADC sample) (SURVEY.md 8(d) + one complex MAC per coil); "
-                                           "the 3 MUFU per evaluation are shared by all coils and are the smaller term"})
-    if kinds_n["rf"]:
-        dur = kinds_ms["rf"] * 1e-3 / args.steps
-        ach = FP32_PER_RF_STEP * rf_steps / dur
-        kern["rf"] = {"bound": "alu", "pipe": "fp32", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
-                      "unit": "Tfp32-instr/s", "frac": ach / fp32_peak,
-                      "traffic": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[0],
-                      "traffic_source": NCU_TRAFFIC.get((w.name, "rf"), (None, None))[1],
-                      "note": "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly), "
-                              "SURVEY.md 8(d); the tier-0 loop issues 38.5 per step on plateau-gradient tiles and reads 87 register "
-                              "operands, so its hardware floor is the register file's 2 operands per lane per clock "
-                              "(43.5 clocks per warp step; profiles/r01_pipe_microbench.md)",
-                      "launches_per_step": kinds_n["rf"] // args.steps, "ms_per_step": dur * 1e3,
-                      "avg_launch_ms": kinds_ms["rf"] / kinds_n["rf"],
-                      "algorithmic_ops_per_launch": FP32_PER_RF_STEP * rf_steps * args.steps / kinds_n["rf"]}
-    if kinds_n["fused"]:
-        # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
-        # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)
-        dur = kinds_ms["fused"] * 1e-3 / args.steps
-        fp32_ops = FP32_PER_RF_STEP * rf_steps + FP32_PER_EVAL * n_eval_sig
-        mufu_ops = MUFU_PER_EVAL * n_eval_sig
-        t_fp32, t_mufu = fp32_ops / fp32_peak, mufu_ops / mufu_peak
-        pipe, ops, peak = ("fp32", fp32_ops, fp32_peak) if t_fp32 >= t_mufu else ("mufu", mufu_ops, mufu_peak)
-        ach = ops / dur
-        kern["fused"] = {"bound": "alu", "pipe": pipe, "achieved": ach / 1e12, "peak": peak / 1e12,
-                         "unit": "Tfp32-instr/s" if pipe == "fp32" else "Tmufu-op/s", "frac": ach / peak,
-                         "traffic": NCU_TRAFFIC.get((w.name, "fused"), (None, None))[0],
-                         "traffic_source": NCU_TRAFFIC.get((w.name, "fused"), (None, None))[1],
-                         "note": "seq_kernel (a5-a8 in one launch): algorithmic count = 46 FP32 instructions per spin*step "
-                                 "+ 15 FP32 instructions per (spin, ADC sample), SURVEY.md 8(d); the MUFU count "
-                                 f"(3 per evaluation) would take {t_mufu * 1e3:.1f} ms, the FP32 count {t_fp32 * 1e3:.1f} ms",
-                         "launches_per_step": kinds_n["fused"] // args.steps, "ms_per_step": dur * 1e3,
-                         "avg_launch_ms": kinds_ms["fused"] / kinds_n["fused"],
-                         "algorithmic_ops_per_launch": ops * args.steps / kinds_n["fused"]}
+    kern = head["kernels"]
+    sm_max = float(clocks.max_mhz or load_peaks().get("sm_max_mhz") or 1965.0)
     dominant = max(kern, key=lambda k: kern[k]["ms_per_step"]) if kern else None
-    roofline = dict(kern[dominant], kernel=dominant,
-                    peak_source=f"derived: {SM_COUNT} SMs x lanes/SM/clk x {sm_max:.0f} MHz (DESIGN.md Roofline)") \
-        if dominant else None
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32" if info["phase_mode"] == 1 else "f32+f64phase",
-           "data": "synthetic",
-           "config": {"workload": w.name, "n_spins_per_gpu": n, "n_intervals": n_int,
-                      "n_rf_steps": info["n_rf_steps"], "n_adc": info["n_adc"], "n_blocks": info["n_blocks"],
-                      "output_mode": w.output_mode, "motion": w.velocity is not None, "coils": n_coils,
-                      "path": "fused" if bloch.bloch_plan_uses_fused(plan.handle, n) else "per_block", "spin_steps_per_step": spin_steps * world,
+    roofline = dict(kern[dominant], kernel_kind=dominant,
+                    peak_source=f"derived: {SM_COUNT} SMs x lanes/SM/clk x {sm_max:.0f} MHz (DESIGN.md Roofline), "
+                                "confirmed by bloch_microbench (profiles/r01_pipe_microbench.md); MEASURED_PEAKS.json "
+                                "holds only HBM and bf16 peaks, which do not bound this path") if dominant else None
+    out = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+           "scaling": args.scaling, "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic",
+           "value_definition": "step-equivalent throughput: N_spins x N_intervals of the discretised sequence (what the "
+                               "paper's step-by-step solver executes) / device time; the GPU path evaluates free "
+                               "precession in closed form at ADC samples and block ends only -- evaluated_units_per_s "
+                               "counts (spin, RF step) + (spin, evaluated point) actually computed",
+           "evaluated_units_per_s": head["evaluated_units_per_s"],
+           "config": {"workload": head["workload"], "n_spins_per_gpu": head["n_spins_per_gpu"],
+                      "n_spins_total": head["n_spins_total"], "n_intervals": head["n_intervals"],
+                      "n_rf_steps": head["n_rf_steps"], "n_adc": head["n_adc"], "n_blocks": head["n_blocks"],
+                      "output_mode": head["output_mode"], "motion": head["motion"], "coils": head["coils"],
+                      "path": head["path"], "spin_steps_per_step": head["spin_steps_per_step"],
+                      "sharding": ("strong: contiguous spin shards of the named workload (dist.shard_bounds) + rank-ordered "
+                                   "sum of the per-rank signals" if args.scaling == "strong" else
+                                   "weak: every rank simulates its own seed-shifted phantom of the named size"),
                       "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
-                      "plan_create_upload_s": plan_s},
-           "sim_wall_time_s": ms_total / args.steps * 1e-3,
+                      "plan_create_upload_s": head["plan_create_upload_s"]},
+           "sim_wall_time_s": head["ms_per_step"] * 1e-3,
            "clocks": clocks.summary(),
-           "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                   "steps": e2e_steps, "api": "bloch_simulate_host (pinned host buffers)" if h_coils is None else
-                          "bloch_simulate_host_coils (pinned host buffers)"},
-           "gpu_launches": bloch.bloch_plan_last_launches(plan.handle) * args.steps,
-           "ms_per_step_with_kernel_events": (ms_pass.get(True, 0.0) / args.steps) or None,
+           "e2e": head["e2e"],
+           "gpu_launches": head["gpu_launches"],
+           "ms_per_step_with_kernel_events": head["ms_per_step_with_kernel_events"],
            "roofline": roofline,
            "kernels": kern,
-           "ms_by_kind_per_step": {k: v / args.steps for k, v in kinds_ms.items()}}
+           "ms_by_kind_per_step": head["ms_by_kind_per_step"],
+           "shard_check": head["shard_check"],
+           "workloads": extra}
     if args.microbench:
         out["pipe_microbench"] = {"mufu_ops_per_s": bloch.bloch_microbench(0), "ffma_per_s": bloch.bloch_microbench(1),
                                   "dfma_per_s": bloch.bloch_microbench(2),
                                   "ffma_3_distinct_regs_per_s": bloch.bloch_microbench(3)}
     if not args.no_cpu_baseline:
-        cb, _, _ = time_oracle(w, n_int, args.cpu_budget)
+        cb, _, _ = time_oracle(w_whole, head["n_intervals"], args.cpu_budget)
         out["cpu_baseline"] = cb
     print(json.dumps(out), flush=True)
 
@@ -418,6 +568,12 @@ def main():
     ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary)")
     ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
                     help="execution path (bloch_plan_set_path); auto = the library's choice")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="multi-GPU: weak = each rank its own phantom of the named size; strong = contiguous spin shards "
+                         "of the ONE named workload, signals added in rank order, checked against the 1-GPU signal")
+    ap.add_argument("--extra", default=EXTRA_DEFAULT,
+                    help="other configs timed in short runs and reported under 'workloads' (comma list, or 'none')")
+    ap.add_argument("--extra-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")

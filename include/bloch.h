@@ -14,6 +14,7 @@
  *   - The library never allocates device memory: tables, workspace and all spin / signal buffers are
  *     caller-owned (in this repo: torch tensors).  Host arrays passed to bloch_plan_create are borrowed
  *     for the duration of that call only.
+ *   - The library reads no environment variable: kernel selection is plan state (bloch_plan_set_option).
  *   - `stream` arguments are a cudaStream_t passed as void* (NULL = legacy default stream).
  *   - Complex values are interleaved (re, im) fp32 pairs.
  */
@@ -37,7 +38,8 @@ typedef enum {
     BLOCH_EARCH = -6,          /* current device is not compute capability 10.x */
     BLOCH_ENOTUPLOADED = -7,   /* bloch_simulate before bloch_plan_upload */
     BLOCH_ENOMEM = -8,         /* host allocation failed */
-    BLOCH_EHWLIMIT = -9        /* a gradient vertex exceeds scanner G_max, or a segment exceeds S_max (when given) */
+    BLOCH_EHWLIMIT = -9,       /* a gradient vertex exceeds scanner G_max, or a segment exceeds S_max (when given) */
+    BLOCH_ERANGE = -10         /* the phantom lies outside what the plan's phase mode resolves (see bloch_sim_params) */
 } bloch_status;
 
 enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
@@ -87,6 +89,18 @@ typedef struct {
     int32_t output_mode;  /* BLOCH_OUT_*   */
     int32_t motion_mode;  /* BLOCH_MOTION_* */
     int32_t group_size;   /* BLOCH_OUT_GROUPED: spins per group (>= 1; n_spins must be a multiple); else ignored */
+    /* Extents of the phantoms this plan will be run on.  The plan is spin-independent (it is built from the sequence
+     * alone), so what BLOCH_PHASE_AUTO needs to know about the spins is declared here: the fp32 phase of the signal
+     * kernels resolves 2^-24 of the largest block-relative phase, bounded by |k| max_extent_m + max_offres_hz tau
+     * (+ |first moment| max_speed_mps with motion), and AUTO takes fp64 phase accumulation above 256 turns.
+     * <= 0 selects 0.25 m / 1000 Hz / 1 m/s.  Every bloch_simulate measures the phantom it is given (max |x|,
+     * max |dw|, max |v|) and reports BLOCH_ERANGE through bloch_plan_status when an AUTO plan that resolved to fp32
+     * would pass 256 turns with it, or an fp64-phase plan 2^19 turns (the limit of its fixed-point phase fraction);
+     * a plan whose declared extents already pass 2^19 turns is rejected by bloch_plan_create (BLOCH_ERANGE).
+     * A plan forced to BLOCH_PHASE_FP32 is not checked: the caller has taken the phase precision on. */
+    double max_extent_m;   /* largest |x| (Euclidean norm) of any spin [m] */
+    double max_offres_hz;  /* largest |dw| / 2 pi [Hz] */
+    double max_speed_mps;  /* largest |v| [m/s] (motion plans) */
 } bloch_sim_params;
 
 typedef struct {
@@ -103,6 +117,13 @@ typedef struct {
     int32_t output_mode;
     int32_t motion_mode;
     int32_t group_size;
+    int32_t phase_mode_requested;  /* as given: BLOCH_PHASE_AUTO / FP32 / FP64 */
+    int32_t path;            /* BLOCH_PATH_* as set by bloch_plan_set_path */
+    double max_extent_m;     /* the extents the plan assumes (bloch_sim_params, defaults resolved) */
+    double max_offres_hz;
+    double max_speed_mps;
+    double worst_turns;      /* largest block-relative phase [turns] any evaluated point can reach within those extents */
+    int32_t options[16];     /* current BLOCH_OPT_* values (bloch_plan_set_option) */
 } bloch_plan_info;
 
 typedef struct bloch_plan bloch_plan;
@@ -137,7 +158,8 @@ int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stre
  *             S[g][j] = sum of Mxy over the group_size consecutive spins of group g -- an isochromat ensemble
  *             per voxel or per dictionary entry.
  *   Asynchronous on `stream`: no hidden synchronisation, no allocation, no host copies.  The result is
- *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 (not checked). 
+ *   bitwise reproducible run to run (no floating-point atomics).  T1, T2 must be > 0 and finite: checked on the
+ *   device by the first kernel, reported by bloch_plan_status / the next call (BLOCH_EINVAL).
  * The call only enqueues work on `stream` (kernels and memsets; CUDA events too when profiling is on): it may be
  * captured into a CUDA graph by the caller and replayed. */
 int bloch_simulate(const bloch_plan *plan, int64_t n_spins,
@@ -196,6 +218,12 @@ int bloch_plan_last_timing(const bloch_plan *plan, float *ms_by_kind, int64_t *l
 /* Number of kernels the last bloch_simulate on this plan enqueued (it depends on n_spins through the batching
  * of the second-pass reduction; bloch_plan_info.n_launches is the upper bound with one second pass per block). */
 int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out);
+/* The largest launch (threads in flight) of kernel kind `kind` in the last bloch_simulate on this plan: its name as a
+ * profiler prints it (e.g. "rf_kernel<0>", "signal_kernel<8, 0, 0>"; empty if the kind did not run), CTAs in the
+ * grid and threads per CTA.  The benchmark uses it to decide whether a committed ncu capture describes the kernel
+ * it has just timed.  name: caller's buffer of name_bytes (may be NULL); grid_ctas, block_threads may be NULL. */
+int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t name_bytes, int64_t *grid_ctas,
+                           int *block_threads);
 
 /* Multi-coil receive (SURVEY.md 8(f) f2 "per-coil weights"; PAPER.md:95 "coil sensitivity", :372; reading C1 of
  * DESIGN.md): S_c(t_n) = sum_i C_c(x_i) Mxy_i(t_n) for n_coils receive coils.
@@ -237,6 +265,46 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
  * the order of the fixed-order sums.  Set before bloch_plan_workspace_bytes: the workspace size depends on it. */
 enum { BLOCH_PATH_AUTO = 0, BLOCH_PATH_PER_BLOCK = 1, BLOCH_PATH_FUSED = 2 };
 int bloch_plan_set_path(bloch_plan *plan, int path);
+
+/* Kernel-selection options of a plan: which of the library's kernels / launch shapes bloch_simulate takes where it has
+ * a choice.  They are state of the PLAN (set once, echoed in bloch_plan_info.options), never ambient process state:
+ * the library reads no environment variable.  Defaults are what DESIGN.md's measurements use; every setting computes
+ * the same thing (tests compare them against each other and against the oracle).  Set before
+ * bloch_plan_workspace_bytes: launch shapes enter the workspace size.  Unknown key or value out of range: BLOCH_EINVAL.
+ *   BLOCH_OPT_SIGNAL_LIN          1 (default): Cartesian readouts (k' advances by a constant step) take the rotation
+ *                                 recurrence; 0: every sample takes its own sin / cos
+ *   BLOCH_OPT_SIGNAL_P            0 (default): the library picks 1, 2, 4 or 8 adjacent ADC samples per thread of the
+ *                                 signal kernel from the block length; 1 / 2 / 4 / 8 forces it
+ *   BLOCH_OPT_SIGNAL_FIXED_CTA    0 (default): readouts of fewer than 256 samples get CTAs of just enough warps; 1: 256
+ *   BLOCH_OPT_SIGNAL_CTAS_PER_SM  resident signal CTAs per SM the grid is sized for: 1..8, default 4
+ *   BLOCH_OPT_RF_THREADS          0 (default): 128-thread excitation CTAs once there are >= 32 warps per SM, else 32;
+ *                                 32 / 64 / 128 forces it
+ *   BLOCH_OPT_RF_SPINS            spins per thread of the excitation kernel: 0 (default) the library's choice, 1 or 2
+ *   BLOCH_OPT_COIL_TC             multi-coil receive: -1 (default) tensor cores (tcgen05) for more than 8 coils, 0 never,
+ *                                 1 whenever they apply (more than 4 coils, fp32 phase)
+ *   BLOCH_OPT_SEQ_SIG_EXTRA       whole-sequence kernel: signal warps added per missing RF warp of a sub-partition,
+ *                                 0..7, default 2
+ *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic
+ *   BLOCH_OPT_SEQ_ITEMS_X4        whole-sequence kernel: readout items per signal warp x 4 that the item size must
+ *                                 leave; 0 (default) always the largest item */
+enum { BLOCH_OPT_SIGNAL_LIN = 0, BLOCH_OPT_SIGNAL_P = 1, BLOCH_OPT_SIGNAL_FIXED_CTA = 2,
+       BLOCH_OPT_SIGNAL_CTAS_PER_SM = 3, BLOCH_OPT_RF_THREADS = 4, BLOCH_OPT_RF_SPINS = 5, BLOCH_OPT_COIL_TC = 6,
+       BLOCH_OPT_SEQ_SIG_EXTRA = 7, BLOCH_OPT_SEQ_SIG_BASE = 8, BLOCH_OPT_SEQ_ITEMS_X4 = 9, BLOCH_N_OPTIONS = 10 };
+int bloch_plan_set_option(bloch_plan *plan, int key, int value);
+int bloch_plan_get_option(const bloch_plan *plan, int key, int *value);
+
+/* What the last bloch_simulate* on this plan found out about the phantom it was given.  pack_kernel (the first
+ * kernel of every simulation) checks every spin -- T1, T2 > 0 and finite (they enter as 1/T1, 1/T2),
+ * every value finite -- and measures max |x|, max |dw|, max |v|; the findings (32 bytes) follow the simulation on
+ * `stream` into pinned host memory owned by the plan (allocated by bloch_plan_upload, so bloch_simulate still never
+ * allocates and never synchronises).
+ *   bloch_plan_status synchronises `stream`, evaluates them, clears them, stores the BLOCH_STATUS_* bits in *flags
+ *   (may be NULL) and returns BLOCH_OK, BLOCH_EINVAL (bad T1 / T2 / non-finite input) or BLOCH_ERANGE (phase range,
+ *   see bloch_sim_params).  The host-buffer entries (bloch_simulate_host*) make this check themselves before they
+ *   return.  A device-buffer bloch_simulate* whose predecessor on the same plan left findings that nobody collected
+ *   returns that error instead of running ("fails on the next call"), and clears them. */
+enum { BLOCH_STATUS_BAD_RELAXATION = 1, BLOCH_STATUS_NONFINITE = 2, BLOCH_STATUS_PHASE_RANGE = 4 };
+int bloch_plan_status(const bloch_plan *plan, void *stream, int *flags);
 /* *out = 1 if bloch_simulate would take the fused path for n_spins on the current device, else 0. */
 int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out);
 

@@ -38,7 +38,8 @@ class bloch_sequence(C.Structure):
 class bloch_sim_params(C.Structure):
     _fields_ = [("dt_max", C.c_double), ("dt_rf_max", C.c_double), ("max_block_points", C.c_int64),
                 ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
-                ("group_size", C.c_int32)]
+                ("group_size", C.c_int32), ("max_extent_m", C.c_double), ("max_offres_hz", C.c_double),
+                ("max_speed_mps", C.c_double)]
 
 
 class bloch_plan_info(C.Structure):
@@ -46,8 +47,15 @@ class bloch_plan_info(C.Structure):
                 ("n_blocks", C.c_int64), ("n_rf_blocks", C.c_int64), ("n_eval_points", C.c_int64),
                 ("n_launches", C.c_int64), ("table_bytes", C.c_int64), ("max_block_adc", C.c_int64),
                 ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
-                ("group_size", C.c_int32)]
+                ("group_size", C.c_int32), ("phase_mode_requested", C.c_int32), ("path", C.c_int32),
+                ("max_extent_m", C.c_double), ("max_offres_hz", C.c_double), ("max_speed_mps", C.c_double),
+                ("worst_turns", C.c_double), ("options", C.c_int32 * 16)]
 
+
+# BLOCH_OPT_* keys of bloch_plan_set_option, in enum order
+OPTIONS = ("signal_lin", "signal_p", "signal_fixed_cta", "signal_ctas_per_sm", "rf_threads", "rf_spins", "coil_tc",
+           "seq_sig_extra", "seq_sig_base", "seq_items_x4")
+STATUS_BAD_RELAXATION, STATUS_NONFINITE, STATUS_PHASE_RANGE = 1, 2, 4
 
 EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",
            "bloch_plan_get_info", "bloch_plan_workspace_bytes", "bloch_plan_upload", "bloch_simulate",
@@ -55,8 +63,8 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_simulate_host_motion", "bloch_plan_set_profiling",
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
            "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils", "bloch_simulate_host_coils_scratch_bytes",
-           "bloch_simulate_host_coils",
-           "bloch_microbench"]
+           "bloch_simulate_host_coils", "bloch_plan_set_option", "bloch_plan_get_option", "bloch_plan_status",
+           "bloch_plan_last_kernel", "bloch_microbench"]
 
 
 def _load():
@@ -89,8 +97,12 @@ def _load():
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
+    lib.bloch_plan_last_kernel.argtypes = [vp, C.c_int, C.c_char_p, sz, C.POINTER(i64), C.POINTER(C.c_int)]
     lib.bloch_plan_set_path.argtypes = [vp, C.c_int]
     lib.bloch_plan_uses_fused.argtypes = [vp, i64, C.POINTER(C.c_int)]
+    lib.bloch_plan_set_option.argtypes = [vp, C.c_int, C.c_int]
+    lib.bloch_plan_get_option.argtypes = [vp, C.c_int, C.POINTER(C.c_int)]
+    lib.bloch_plan_status.argtypes = [vp, vp, C.POINTER(C.c_int)]
     lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
     for name in EXPORTS:
         if name not in ("bloch_strerror", "bloch_last_error"):
@@ -133,8 +145,10 @@ def _darr(a):
 
 def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
                       max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
-                      group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0) -> int:
+                      group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0,
+                      max_extent_m: float = 0.0, max_offres_hz: float = 0.0, max_speed_mps: float = 0.0) -> int:
     """G_max [T/m], S_max [T/m/s]: scanner limits the gradient waveforms are checked against when > 0.
+    max_extent_m / max_offres_hz / max_speed_mps: extents of the phantoms the plan will see (bloch_sim_params).
     seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
     Returns the opaque plan handle (an integer address)."""
     keep = []
@@ -158,7 +172,8 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     pm = _PHASE[phase_mode] if isinstance(phase_mode, str) else int(phase_mode)
     om = _OUT[output_mode] if isinstance(output_mode, str) else int(output_mode)
     mm = _MOTION[motion] if isinstance(motion, str) else int(motion)
-    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, int(group_size))
+    sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, int(group_size),
+                          float(max_extent_m), float(max_offres_hz), float(max_speed_mps))
     h = C.c_void_p()
     _check(_lib.bloch_plan_create(C.byref(sc), C.byref(cs), C.byref(sp), C.byref(h)))
     return h.value
@@ -171,7 +186,14 @@ def bloch_plan_destroy(plan: int):
 def bloch_plan_get_info(plan: int) -> dict:
     inf = bloch_plan_info()
     _check(_lib.bloch_plan_get_info(plan, C.byref(inf)))
-    return {k: int(getattr(inf, k)) for k, _ in bloch_plan_info._fields_}
+    out = {}
+    for k, tp in bloch_plan_info._fields_:
+        v = getattr(inf, k)
+        if k == "options":
+            out[k] = {name: int(v[i]) for i, name in enumerate(OPTIONS)}
+        else:
+            out[k] = float(v) if tp is C.c_double else int(v)
+    return out
 
 
 def bloch_plan_workspace_bytes(plan: int, n_spins: int) -> int:
@@ -257,6 +279,25 @@ def bloch_plan_set_path(plan: int, path):
     _check(_lib.bloch_plan_set_path(plan, PATHS[path] if isinstance(path, str) else int(path)))
 
 
+def bloch_plan_set_option(plan: int, key, value: int):
+    """key: a BLOCH_OPT_* integer or its name in OPTIONS."""
+    _check(_lib.bloch_plan_set_option(plan, OPTIONS.index(key) if isinstance(key, str) else int(key), int(value)))
+
+
+def bloch_plan_get_option(plan: int, key) -> int:
+    out = C.c_int()
+    _check(_lib.bloch_plan_get_option(plan, OPTIONS.index(key) if isinstance(key, str) else int(key), C.byref(out)))
+    return int(out.value)
+
+
+def bloch_plan_status(plan: int, stream: int = 0) -> int:
+    """Synchronises `stream`; raises BlochError (BLOCH_EINVAL / BLOCH_ERANGE) when the last simulation's phantom was
+    invalid or outside the plan's phase range, else returns the (zero) status flags."""
+    flags = C.c_int()
+    _check(_lib.bloch_plan_status(plan, stream, C.byref(flags)))
+    return int(flags.value)
+
+
 def bloch_plan_uses_fused(plan: int, n_spins: int) -> bool:
     out = C.c_int()
     _check(_lib.bloch_plan_uses_fused(plan, n_spins, C.byref(out)))
@@ -277,6 +318,15 @@ def bloch_plan_last_launches(plan: int) -> int:
     return int(out.value)
 
 
+def bloch_plan_last_kernel(plan: int, kind) -> dict:
+    """kind: BLOCH_KIND_* integer or its name in KINDS -> {"name", "grid", "block"} of that kind's largest launch."""
+    buf = C.create_string_buffer(64)
+    grid, block = C.c_int64(), C.c_int()
+    _check(_lib.bloch_plan_last_kernel(plan, KINDS.index(kind) if isinstance(kind, str) else int(kind), buf, 64,
+                                       C.byref(grid), C.byref(block)))
+    return {"name": buf.value.decode(), "grid": int(grid.value), "block": int(block.value)}
+
+
 def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:
     out = C.c_double()
     _check(_lib.bloch_microbench(kind, iters, C.byref(out), stream))
@@ -287,9 +337,12 @@ def bloch_microbench(kind: int, iters: int = 4096, stream: int = 0) -> float:
 class Plan:
     """Owns a bloch_plan handle plus the caller-side device buffers (torch tensors)."""
 
-    def __init__(self, seq, path="auto", **kw):
+    def __init__(self, seq, path="auto", options=None, **kw):
+        """options: {name in OPTIONS: value} passed to bloch_plan_set_option (kernel selection is plan state)."""
         self.handle = bloch_plan_create(seq, **kw)
         bloch_plan_set_path(self.handle, path)
+        for k, v in (options or {}).items():
+            bloch_plan_set_option(self.handle, k, v)
         self.info = bloch_plan_get_info(self.handle)
         self._tables = None
         self._ws = None
@@ -305,6 +358,27 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+    def set_option(self, key, value):
+        bloch_plan_set_option(self.handle, key, value)
+        self.info = bloch_plan_get_info(self.handle)
+        self._ws = None     # launch shapes enter the workspace size
+        return self
+
+    def status(self):
+        """Synchronises the current stream and raises if the last simulate() met an invalid phantom (bad T1 / T2,
+        non-finite values) or one outside the plan's phase range."""
+        return bloch_plan_status(self.handle, self._stream())
+
+    @staticmethod
+    def _check_out(t, numel, dtypes, what):
+        import torch
+        if t is None:
+            return
+        assert isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous(), f"{what}: contiguous CUDA tensor needed"
+        assert t.dtype in dtypes, f"{what}: dtype {t.dtype} not in {dtypes}"
+        n = t.numel() * (2 if t.dtype == torch.complex64 else 1)
+        assert n == numel, f"{what}: {n} fp32 values given, {numel} expected"
 
     def _signal_shape(self, n):
         n_adc, mode = self.info["n_adc"], self.info["output_mode"]
@@ -346,6 +420,11 @@ class Plan:
             assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
         n_adc = self.info["n_adc"]
         shape = self._signal_shape(n)
+        # the C side only sees raw pointers: wrong sizes or dtypes would be out-of-bounds device writes
+        self._check_out(Mxy, 2 * n, (torch.float32, torch.complex64), "Mxy")
+        self._check_out(Mz, n, (torch.float32,), "Mz")
+        n_rows = int(coils.shape[0]) if coils is not None and coils.dim() == 2 else int(np.prod(shape[:-1]))
+        self._check_out(signal, 2 * n_rows * n_adc, (torch.complex64,), "signal")
         if coils is not None:
             assert coils.is_cuda and coils.dtype == torch.complex64 and coils.is_contiguous() and \
                 coils.dim() == 2 and coils.shape[1] == n and velocity is None
@@ -382,9 +461,17 @@ class Plan:
             self.upload()
         arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (x, y, z, M0, T1, T2, dw)]
         n = int(arrs[0].shape[0])
+        assert all(a.shape == (n,) for a in arrs), "phantom arrays must all hold n_spins values"
         n_adc = self.info["n_adc"]
         shape = self._signal_shape(n)
-        if signal is None:
+        n_rows = int(np.shape(coils)[0]) if coils is not None else int(np.prod(shape[:-1]))
+        for a, cnt, dts, what in ((Mxy, 2 * n, (np.float32, np.complex64), "Mxy"), (Mz, n, (np.float32,), "Mz"),
+                                  (signal, 2 * n_rows * n_adc, (np.complex64,), "signal")):
+            if a is not None:
+                assert isinstance(a, np.ndarray) and a.flags.c_contiguous and a.flags.writeable and \
+                    a.dtype in dts, f"{what}: writable C-contiguous numpy array of dtype {dts} needed"
+                assert a.size * (2 if a.dtype == np.complex64 else 1) == cnt, f"{what}: wrong size"
+        if signal is None and coils is None:
             signal = np.empty(shape, dtype=np.complex64)
         if coils is not None:
             cw = np.ascontiguousarray(coils, dtype=np.complex64)

@@ -1,5 +1,7 @@
 // api.cu -- C-ABI entry points of libbloch_b200 (include/bloch.h) and the per-block launch logic.
 #include <algorithm>
+#include <atomic>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -16,6 +18,7 @@
 
 namespace bloch {
 const char *last_error_cstr();
+int collect_status(const bloch_plan *plan, int *flags_out);
 
 namespace {
 
@@ -30,17 +33,50 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-int env_int(const char *name, int dflt) {
-    const char *v = std::getenv(name);
-    return (v && *v) ? std::atoi(v) : dflt;
+// Per-device facts and one-time set-up, keyed by the CUDA device ordinal: SM count, compute capability, and whether
+// the opt-in shared-memory limits of the kernels that need more than 48 KB have been raised ON THAT DEVICE
+// (cudaFuncSetAttribute is per device, so a process that drives several GPUs sets it once on each).
+constexpr int kMaxDevices = 64;
+struct DeviceInfo {
+    std::atomic<int> sms{0}, major{0};
+    std::atomic<bool> seq_attr{false}, tc_attr{false};
+};
+DeviceInfo g_dev[kMaxDevices];
+
+// the current device's slot, or nullptr when there is no usable device (host-only callers)
+DeviceInfo *current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return nullptr;
+    }
+    if (dev < 0 || dev >= kMaxDevices) return nullptr;
+    DeviceInfo *d = &g_dev[dev];
+    if (d->sms.load(std::memory_order_acquire) == 0) {
+        int sms = 0, major = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || sms <= 0) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        d->major.store(major, std::memory_order_relaxed);
+        d->sms.store(sms, std::memory_order_release);
+    }
+    return d;
+}
+
+// ONE source for the SM count that sizes launch shapes: workspace sizing and workspace carving both use it, so they
+// cannot disagree; 148 (a B200) when no device is present, which keeps bloch_plan_workspace_bytes a host function.
+int sm_count_cached() {
+    const DeviceInfo *d = current_device();
+    return d ? d->sms.load(std::memory_order_relaxed) : 148;
 }
 
 int check_arch() {
-    int dev = 0;
-    BLOCH_CUDA(cudaGetDevice(&dev));
-    int major = 0;
-    BLOCH_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
-    if (major != 10) return fail(BLOCH_EARCH, "device is not compute capability 10.x (built for sm_100a only)");
+    const DeviceInfo *d = current_device();
+    if (!d) return fail(BLOCH_ECUDA, "no usable CUDA device is current");
+    if (d->major.load(std::memory_order_relaxed) != 10)
+        return fail(BLOCH_EARCH, "device is not compute capability 10.x (built for sm_100a only)");
     return BLOCH_OK;
 }
 
@@ -54,9 +90,9 @@ struct SigShape {
 };
 
 // max_P: 8, or 4 for fp64-phase motion plans (P = 8 would need 172 registers there: config 3m 2.09 -> 2.47 ms)
-SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count, int max_P) {
+SigShape sig_shape(const bloch_plan *plan, int64_t n_pts, int64_t n_spins, int sm_count, int max_P) {
     SigShape s;
-    const int forceP = env_int("BLOCH_SIGNAL_P", 0);
+    const int forceP = plan->opt[BLOCH_OPT_SIGNAL_P];
     // 8 adjacent samples per thread when the block is long enough (config 4: 42.5 -> 35.6 ms together with the
     // geometric decay; ~100 registers, 2 CTAs per SM), else 4 / 2 / 1
     s.P = forceP ? forceP : (n_pts >= 8 * kSigThreads && max_P >= 8 ? 8 : (n_pts >= 4 * kSigThreads ? 4 : (n_pts >= 2 * kSigThreads ? 2 : 1)));
@@ -64,10 +100,10 @@ SigShape sig_shape(int64_t n_pts, int64_t n_spins, int sm_count, int max_P) {
     // a readout of fewer than 256 samples (Cartesian lines) gets CTAs of just enough warps and more of them per SM,
     // so that the spins are split over all lanes instead of leaving 256 - n_pts threads of every CTA idle
     s.threads = kSigThreads;
-    if (s.P == 1 && n_pts < kSigThreads && !env_int("BLOCH_SIGNAL_FIXED_CTA", 0))
+    if (s.P == 1 && n_pts < kSigThreads && !plan->opt[BLOCH_OPT_SIGNAL_FIXED_CTA])
         s.threads = (int)std::max<int64_t>(32, (n_pts + 31) / 32 * 32);
     s.ptiles = (int)((n_pts + (int64_t)s.threads * s.P - 1) / ((int64_t)s.threads * s.P));
-    const int per_sm = std::min(env_int("BLOCH_SIGNAL_CTAS_PER_SM", 4) * (kSigThreads / s.threads), 12);
+    const int per_sm = std::min(plan->opt[BLOCH_OPT_SIGNAL_CTAS_PER_SM] * (kSigThreads / s.threads), 12);
     const int64_t target = (int64_t)sm_count * per_sm;
     int64_t chunks = (target + s.ptiles - 1) / s.ptiles;
     const int64_t max_chunks = (n_spins + 31) / 32;
@@ -86,8 +122,8 @@ int sig_max_P(const bloch_plan *plan) {
 // Launch shape of a precession block: blocks that go to signal_lin_kernel (Block::lin_pts) are chunked as P = 8 blocks
 // whatever the plan (their kernel holds 2 CTAs per SM also with fp64 phase and motion).
 SigShape block_shape(const bloch_plan *plan, const Block &b, int64_t n_spins, int sm_count) {
-    const bool lin = b.lin_pts > 0 && env_int("BLOCH_SIGNAL_LIN", 1);
-    if (!lin) return sig_shape(b.adc_count, n_spins, sm_count, sig_max_P(plan));
+    const bool lin = b.lin_pts > 0 && plan->opt[BLOCH_OPT_SIGNAL_LIN];
+    if (!lin) return sig_shape(plan, b.adc_count, n_spins, sm_count, sig_max_P(plan));
     // signal_lin_kernel: one thread per group of kLinP samples, 2 CTAs of 256 threads per SM (or proportionally more
     // CTAs of fewer warps for short blocks), the spins split over enough chunks to fill the machine
     SigShape s;
@@ -153,12 +189,13 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     for (int k = 0; k < 4; ++k) rf_per[k] = q.rf_warps / 4;
     { const int order[4] = {1, 2, 3, 0}; for (int e = 0; e < q.rf_warps % 4; ++e) ++rf_per[order[e]]; }
     const int rf_max = *std::max_element(rf_per, rf_per + 4);
-    const int sig_extra = std::min(std::max(env_int("BLOCH_SEQ_SIG_EXTRA", 2), 0), 7);
+    const int sig_extra = std::min(std::max(plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA], 0), 7);
     int deficit = 0;
     for (int k = 0; k < 4; ++k) deficit += rf_max - rf_per[k];
     const int target = std::max(4, (6 * q.rf_warps + 5) / 10);
     const int auto_base = std::max(1, (target - sig_extra * deficit + 2) / 4);
-    const int sig_base = std::min(std::max(env_int("BLOCH_SEQ_SIG_BASE", auto_base), 0), 7);
+    const int sig_base = plan->opt[BLOCH_OPT_SEQ_SIG_BASE] < 0 ? std::min(auto_base, 7)
+                                                               : std::min(plan->opt[BLOCH_OPT_SEQ_SIG_BASE], 7);
     auto total_warps = [&](int base, int extra) {
         int top = 0;
         for (int k = 0; k < 4; ++k) {
@@ -195,7 +232,7 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
         q.roles.n_sig_warps = q.sig_warps;
     }
     q.threads = 32 * n_warps;
-    q.min_items = std::max(1, q.sig_warps * env_int("BLOCH_SEQ_ITEMS_PER_WARP_X4", 0) / 4);  // 0: always the largest P (config 5: 127.6 ms against 131.1 with one item per warp)
+    q.min_items = std::max(1, q.sig_warps * plan->opt[BLOCH_OPT_SEQ_ITEMS_X4] / 4);  // 0: always the largest P (config 5: 127.6 ms against 131.1 with one item per warp)
     q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
     q.smem = seq_smem_bytes(q.chunk);
     q.partial_elems = size_t(q.n_ctas) * size_t(std::max<int64_t>(inf.n_adc, 1));
@@ -212,10 +249,10 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
 // tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 256 threads, 2 CTAs per SM, chunks of whole 16-spin stages
 bool coil_use_tc(const bloch_plan *plan, int n_coils) {
-    // BLOCH_COIL_TC: 0 = never, 1 = whenever it applies (more than 4 coils, fp32 phase), unset = when it pays: more
+    // BLOCH_OPT_COIL_TC: 0 = never, 1 = whenever it applies (more than 4 coils, fp32 phase), -1 = when it pays: more
     // than 8 coils (16 coils per pass cost what 8 cost: config 4 with 32 coils 260 ms against 486 ms for the FFMA
     // kernel; with 8 coils 129.5 against 121.4)
-    const int mode = env_int("BLOCH_COIL_TC", -1);
+    const int mode = plan->opt[BLOCH_OPT_COIL_TC];
     if (mode == 0 || n_coils <= 4 || plan->info.phase_mode != BLOCH_PHASE_FP32) return false;
     return mode == 1 || n_coils > 8;
 }
@@ -275,16 +312,6 @@ struct Workspace {
     float2 *W;       // multi-coil receive only: weights repacked as [pass][spin][4]
     size_t bytes;
 };
-
-int sm_count_cached() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
-    }
-    return sms;
-}
 
 // Layout of the caller's workspace.  sm_count = 148 is used for sizing when no device is present so that
 // bloch_plan_workspace_bytes is a pure host function.
@@ -347,7 +374,52 @@ struct Taps {
     }
 };
 
+// remember the largest launch of a kind (threads in flight) for bloch_plan_last_kernel
+void note_kernel(const bloch_plan *plan, int kind, int64_t grid, int block, const char *fmt, int a = 0, int b = 0, int c = 0) {
+    KernelNote &k = plan->last_kernel[kind];
+    if (grid * block < k.grid * k.block) return;
+    std::snprintf(k.name, sizeof k.name, fmt, a, b, c);
+    k.grid = grid;
+    k.block = block;
+}
+
 }  // namespace
+
+// Evaluates and clears the findings pack_kernel left in plan->h_status (see bloch_plan_status in bloch.h).
+int collect_status(const bloch_plan *plan, int *flags_out) {
+    unsigned *h = plan->h_status;
+    if (!h || !h[kScalValid]) return BLOCH_OK;
+    auto as_float = [](unsigned u) { float f; std::memcpy(&f, &u, sizeof f); return f; };
+    int flags = (int)h[kScalFlags];
+    const double R = std::sqrt((double)as_float(h[kScalX2Max])), F = (double)as_float(h[kScalDwMax]) / (2.0 * M_PI),
+                 V = std::sqrt((double)as_float(h[kScalV2Max]));
+    // phase range: only when the phantom exceeds what the plan was told to assume; then the separable bound
+    // |k'|max R + F tau_max + |mu'|max V (never below the true worst phase) decides
+    double reach = 0.0;
+    if (R > plan->ext_m * (1.0 + 1e-6) || F > plan->ext_hz * (1.0 + 1e-6) || V > plan->ext_mps * (1.0 + 1e-6)) {
+        reach = plan->k_max * std::max(R, plan->ext_m) + std::max(F, plan->ext_hz) * plan->tau_max +
+                plan->m_max * std::max(V, plan->ext_mps);
+        const bool fp64 = plan->info.phase_mode == BLOCH_PHASE_FP64;
+        if (fp64 ? reach >= kFp64TurnLimit : (plan->phase_requested == BLOCH_PHASE_AUTO && reach > kFp32TurnLimit))
+            flags |= BLOCH_STATUS_PHASE_RANGE;
+    }
+    std::memset(h, 0, kStatusWords * sizeof(unsigned));
+    if (flags_out) *flags_out = flags;
+    if (flags & (BLOCH_STATUS_BAD_RELAXATION | BLOCH_STATUS_NONFINITE))
+        return fail(BLOCH_EINVAL, (flags & BLOCH_STATUS_BAD_RELAXATION)
+                                      ? "the phantom holds a T1 or T2 that is <= 0 or not finite"
+                                      : "the phantom (or the initial state) holds a non-finite value");
+    if (flags & BLOCH_STATUS_PHASE_RANGE) {
+        char msg[320];
+        std::snprintf(msg, sizeof msg,
+                      "phantom outside the plan's phase range: max |x| %.4g m, |dw|/2pi %.4g Hz, |v| %.4g m/s (declared %.4g / "
+                      "%.4g / %.4g) give up to %.0f turns per block; create the plan with these extents in bloch_sim_params%s",
+                      R, F, V, plan->ext_m, plan->ext_hz, plan->ext_mps, reach,
+                      plan->info.phase_mode == BLOCH_PHASE_FP64 ? " and shorter blocks (max_block_points)" : "");
+        return fail(BLOCH_ERANGE, msg);
+    }
+    return BLOCH_OK;
+}
 }  // namespace bloch
 
 using namespace bloch;
@@ -368,6 +440,7 @@ const char *bloch_strerror(int code) {
         case BLOCH_ENOTUPLOADED: return "tables not uploaded";
         case BLOCH_ENOMEM: return "host allocation failed";
         case BLOCH_EHWLIMIT: return "gradient waveform exceeds the scanner's G_max or S_max";
+        case BLOCH_ERANGE: return "phantom outside the phase range the plan resolves";
         default: return "unknown error";
     }
 }
@@ -399,6 +472,7 @@ int bloch_plan_create(const bloch_scanner *scanner, const bloch_sequence *seq, c
 int bloch_plan_destroy(bloch_plan *plan) {
     if (!plan) return BLOCH_OK;
     for (void *e : plan->events) cudaEventDestroy((cudaEvent_t)e);
+    if (plan->h_status) cudaFreeHost(plan->h_status);
     delete plan;
     return BLOCH_OK;
 }
@@ -406,6 +480,8 @@ int bloch_plan_destroy(bloch_plan *plan) {
 int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out) {
     if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
     *out = plan->info;
+    out->path = plan->path;
+    for (int k = 0; k < 16; ++k) out->options[k] = k < BLOCH_N_OPTIONS ? plan->opt[k] : 0;
     return BLOCH_OK;
 }
 
@@ -416,16 +492,8 @@ int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *
 int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out) {
     if (!plan || !out || n_spins < 0 || n_coils < 0) return fail(BLOCH_EINVAL, "NULL plan/out or negative size");
     if (n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins exceeds 2^31-1");
-    // sized for the larger of the real SM count and 148 so the answer is usable without a device
-    int sms = 148;
-    int dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess) {
-        int v = 0;
-        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > sms) sms = v;
-    } else {
-        (void)cudaGetLastError();
-    }
-    *out = carve(plan, n_spins, nullptr, sms, n_coils).bytes;
+    // the current device's SM count -- the number bloch_simulate carves with -- or 148 without a device
+    *out = carve(plan, n_spins, nullptr, sm_count_cached(), n_coils).bytes;
     return BLOCH_OK;
 }
 
@@ -433,6 +501,10 @@ int bloch_plan_upload(bloch_plan *plan, void *d_tables, size_t bytes, void *stre
     if (!plan || !d_tables) return fail(BLOCH_EINVAL, "NULL argument");
     if (bytes < plan->tables.size() || (reinterpret_cast<uintptr_t>(d_tables) % kAlign) != 0)
         return fail(BLOCH_EWORKSPACE, "table buffer too small or not 256-B aligned");
+    if (!plan->h_status) {  // 32 B of pinned host memory for the phantom findings (bloch_plan_status)
+        BLOCH_CUDA(cudaHostAlloc((void **)&plan->h_status, kStatusWords * sizeof(unsigned), cudaHostAllocDefault));
+        std::memset(plan->h_status, 0, kStatusWords * sizeof(unsigned));
+    }
     BLOCH_CUDA(cudaMemcpyAsync(d_tables, plan->tables.data(), plan->tables.size(), cudaMemcpyHostToDevice,
                                (cudaStream_t)stream));
     plan->d_tables = (const unsigned char *)d_tables;
@@ -470,6 +542,40 @@ int bloch_plan_set_path(bloch_plan *plan, int path) {
     return BLOCH_OK;
 }
 
+int bloch_plan_set_option(bloch_plan *plan, int key, int value) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    bool ok = false;
+    switch (key) {
+        case BLOCH_OPT_SIGNAL_LIN: case BLOCH_OPT_SIGNAL_FIXED_CTA: ok = value == 0 || value == 1; break;
+        case BLOCH_OPT_SIGNAL_P: ok = value == 0 || value == 1 || value == 2 || value == 4 || value == 8; break;
+        case BLOCH_OPT_SIGNAL_CTAS_PER_SM: ok = value >= 1 && value <= 8; break;
+        case BLOCH_OPT_RF_THREADS: ok = value == 0 || value == 32 || value == 64 || value == 128; break;
+        case BLOCH_OPT_RF_SPINS: ok = value >= 0 && value <= 2; break;
+        case BLOCH_OPT_COIL_TC: ok = value >= -1 && value <= 1; break;
+        case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= 0 && value <= 7; break;
+        case BLOCH_OPT_SEQ_SIG_BASE: ok = value >= -1 && value <= 7; break;
+        case BLOCH_OPT_SEQ_ITEMS_X4: ok = value >= 0 && value <= 64; break;
+        default: return fail(BLOCH_EINVAL, "unknown BLOCH_OPT_* key");
+    }
+    if (!ok) return fail(BLOCH_EINVAL, "option value out of range");
+    plan->opt[key] = value;
+    return BLOCH_OK;
+}
+
+int bloch_plan_get_option(const bloch_plan *plan, int key, int *value) {
+    if (!plan || !value || key < 0 || key >= BLOCH_N_OPTIONS) return fail(BLOCH_EINVAL, "NULL argument or unknown key");
+    *value = plan->opt[key];
+    return BLOCH_OK;
+}
+
+int bloch_plan_status(const bloch_plan *plan, void *stream, int *flags) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    if (flags) *flags = 0;
+    if (!plan->h_status) return BLOCH_OK;  // nothing simulated yet
+    BLOCH_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    return bloch::collect_status(plan, flags);
+}
+
 int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out) {
     if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
     const SeqShape q = seq_shape(plan, n_spins, sm_count_cached());
@@ -480,6 +586,19 @@ int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out) {
 int bloch_plan_last_launches(const bloch_plan *plan, int64_t *out) {
     if (!plan || !out) return fail(BLOCH_EINVAL, "NULL argument");
     *out = plan->last.launches;
+    return BLOCH_OK;
+}
+
+int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t name_bytes, int64_t *grid_ctas,
+                           int *block_threads) {
+    if (!plan || kind < 0 || kind >= BLOCH_N_KINDS) return fail(BLOCH_EINVAL, "NULL plan or bad kind");
+    const KernelNote &k = plan->last_kernel[kind];
+    if (name && name_bytes > 0) {
+        std::strncpy(name, k.name, name_bytes - 1);
+        name[name_bytes - 1] = 0;
+    }
+    if (grid_ctas) *grid_ctas = k.grid;
+    if (block_threads) *block_threads = k.block;
     return BLOCH_OK;
 }
 
@@ -548,6 +667,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     if (plan->info.n_adc > 0 && !d_signal) return fail(BLOCH_EINVAL, "d_signal is NULL");
     int rc = check_arch();
     if (rc != BLOCH_OK) return rc;
+    // findings of an earlier simulation on this plan that nobody collected (bloch_plan_status): fail now, once
+    if (plan->h_status && plan->h_status[kScalValid] && (rc = collect_status(plan, nullptr)) != BLOCH_OK) return rc;
     const int sms = sm_count_cached();
     cudaStream_t stream = (cudaStream_t)stream_;
     const bool grouped = plan->info.output_mode == BLOCH_OUT_GROUPED;
@@ -568,6 +689,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     if (workspace_bytes < w.bytes) return fail(BLOCH_EWORKSPACE, "workspace too small; see bloch_plan_workspace_bytes[_coils]");
 
     const int n = (int)n_spins;
+    for (KernelNote &k : plan->last_kernel) k = KernelNote{};
     Taps taps{plan, stream};
     int64_t launches = 0;
     if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
@@ -580,13 +702,13 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     const int ncp = tc ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const int n_pass = (n_coils + ncp - 1) / ncp;
     const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
+    DeviceInfo *devinfo = current_device();  // non-NULL: check_arch passed
     if (tc) {
-        static bool tc_attr = false;
-        if (!tc_attr) {
+        if (!devinfo->tc_attr.load(std::memory_order_acquire)) {  // once per DEVICE (the attribute is per device)
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(8)));
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(16)));
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(32)));
-            tc_attr = true;
+            devinfo->tc_attr.store(true, std::memory_order_release);
         }
         const dim3 pg((n_pad + 255) / 256, n_pass);
         if (ncp == 32) pack_coils_tc_kernel<32><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, (unsigned char *)w.W);
@@ -604,16 +726,16 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output (or PER_SPIN with <= 16 samples per block), fp32 phase, no motion and <= 29 x 32 spins per SM");
     if (sq.ok && sq.use) {
         // ONE persistent launch for the whole sequence + the second pass over all ADC samples
-        static bool attr_set = false;  // per process; the attribute is sticky for the function
-        if (!attr_set) {
+        if (!devinfo->seq_attr.load(std::memory_order_acquire)) {  // once per DEVICE; sticky for the function there
             BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)seq_smem_bytes(kSeqMaxThreads)));
             BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)seq_smem_bytes(kSeqMaxThreads)));
-            attr_set = true;
+            devinfo->seq_attr.store(true, std::memory_order_release);
         }
         if ((rc = taps.mark(BLOCH_KIND_FUSED))) return rc;
         const SeqOp *prog = reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off);
+        note_kernel(plan, BLOCH_KIND_FUSED, sq.n_ctas, sq.threads, "seq_kernel<%d>", per_spin ? 1 : 0);
         if (per_spin)
             seq_kernel<true><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
                 plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.roles, sq.min_items,
@@ -638,6 +760,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if (plan->profiling) plan->event_kind.resize(taps.used);
         plan->last.launches = launches;
         BLOCH_CUDA(cudaGetLastError());
+        // what pack_kernel found out about the phantom follows the simulation to the host (bloch_plan_status)
+        BLOCH_CUDA(cudaMemcpyAsync(plan->h_status, w.scal, kStatusWords * sizeof(unsigned), cudaMemcpyDeviceToHost, stream));
         return BLOCH_OK;
     }
 
@@ -645,9 +769,11 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     PropRec prop{0, 0, 0, 0, 0, 0, 0};
     // RF launch shape: one spin per thread; small CTAs when spins are few so the warps spread over all
     // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
-    const int rf_threads = env_int("BLOCH_RF_THREADS", (n + 31) / 32 >= sms * 32 ? 128 : 32);
+    const int rf_threads = plan->opt[BLOCH_OPT_RF_THREADS] ? plan->opt[BLOCH_OPT_RF_THREADS]
+                                                           : ((n + 31) / 32 >= sms * 32 ? 128 : 32);
     const int rf_grid = (n + rf_threads - 1) / rf_threads;
     auto launch_rf = [&](const unsigned char *tbl, int n_tiles, int has_prop) -> int {
+        if (tbl) note_kernel(plan, BLOCH_KIND_RF, rf_grid, rf_threads, "rf_kernel<%d>", mo ? 1 : 0);
         if (mo) rf_kernel<true><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, w.V, n);
         else rf_kernel<false><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, nullptr, n);
         return BLOCH_OK;
@@ -713,6 +839,9 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, w.Ad);          \
         else BLOCH_LAUNCH_COIL(PP, NCC, false, w.A);               \
     } while (0)
+                    if (tc) note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, kTcThreads, "signal_coils_tc_kernel<%d>", ncp);
+                    else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d>",
+                                     s.P == 2 ? 2 : 1, ncp == 8 ? 8 : 4, ph64 ? 1 : 0);
                     if (tc) {
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
                         if (ncp == 32)
@@ -757,7 +886,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                 }
                 const dim3 grid(s.ptiles, s.chunks);
                 const int row = (int)batch_pts, poff = (int)batch_done;
-                const int allow_lin = env_int("BLOCH_SIGNAL_LIN", 1);
+                const int allow_lin = plan->opt[BLOCH_OPT_SIGNAL_LIN];
 #define BLOCH_LAUNCH_SIG3(PP, H, M, AP, VP)                                                                    \
     signal_kernel<PP, H, M><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, VP, w.S, n, s.spins_per_chunk,    \
                                                               (const float *)w.scal, w.partial, row, poff, allow_lin)
@@ -768,6 +897,10 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else if (mo) BLOCH_LAUNCH_SIG3(PP, false, true, w.A, w.V);                                             \
         else BLOCH_LAUNCH_SIG3(PP, false, false, w.A, nullptr);                                                \
     } while (0)
+                if (b.lin_pts > 0 && allow_lin)
+                    note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_lin_kernel<%d, %d>", ph64 ? 1 : 0, mo ? 1 : 0);
+                else
+                    note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_kernel<%d, %d, %d>", s.P, ph64 ? 1 : 0, mo ? 1 : 0);
                 if (b.lin_pts > 0 && allow_lin) {
                     // Cartesian readout (planner: constant k' step, quadratic mu', inside every aligned group of kLinP
                     // samples): the recurrence kernel on the first lin_pts samples, the n % kLinP tail through
@@ -833,6 +966,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     if (plan->profiling) plan->event_kind.resize(taps.used);
     plan->last.launches = launches;
     BLOCH_CUDA(cudaGetLastError());
+    BLOCH_CUDA(cudaMemcpyAsync(plan->h_status, w.scal, kStatusWords * sizeof(unsigned), cudaMemcpyDeviceToHost, stream));
     return BLOCH_OK;
 }
 }  // namespace
@@ -913,7 +1047,7 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins, const fl
         BLOCH_CUDA(cudaMemcpyAsync(h_Mz, d_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyDeviceToHost, stream));
     }
     BLOCH_CUDA(cudaStreamSynchronize(stream));
-    return BLOCH_OK;
+    return collect_status(plan, nullptr);  // bad T1 / T2, non-finite input, phase range: see bloch_plan_status
 }
 
 int bloch_simulate_host_coils_scratch_bytes(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out) {
@@ -978,7 +1112,7 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
         BLOCH_CUDA(cudaMemcpyAsync(h_Mz, d_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyDeviceToHost, stream));
     }
     BLOCH_CUDA(cudaStreamSynchronize(stream));
-    return BLOCH_OK;
+    return collect_status(plan, nullptr);  // bad T1 / T2, non-finite input, phase range: see bloch_plan_status
 }
 
 int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {

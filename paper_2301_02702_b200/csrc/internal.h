@@ -14,6 +14,17 @@ constexpr int kBlockRF = 1;
 constexpr double kTimeTol = 1e-12;       // reading G13
 constexpr int64_t kDefaultMaxBlockPoints = int64_t(1) << 22;
 constexpr size_t kAlign = 256;
+// device scalars written by pack_kernel (Workspace::scal) and mirrored to bloch_plan::h_status: all maxima are float
+// bit patterns of non-negative values under an integer atomicMax (order-independent), the flags an atomicOr
+constexpr int kScalR2Max = 0;    // max 1/T2
+constexpr int kScalX2Max = 1;    // max x^2 + y^2 + z^2
+constexpr int kScalDwMax = 2;    // max |dw|
+constexpr int kScalV2Max = 3;    // max |v|^2
+constexpr int kScalFlags = 4;    // BLOCH_STATUS_BAD_RELAXATION | BLOCH_STATUS_NONFINITE
+constexpr int kScalValid = 5;    // 1 once pack_kernel has run (the host clears it when it has evaluated the findings)
+constexpr int kStatusWords = 8;
+constexpr double kFp32TurnLimit = 256.0;      // AUTO: fp32 phase up to here
+constexpr double kFp64TurnLimit = 524288.0;   // 2^19: the fixed-point fraction of the fp64 phase (signal.cuh)
 
 // RF block table (a4), read by rf_kernel through 1-D bulk copies (TMA) tile by tile:
 //   [directory: n_tiles x {int32 byte offset from the block's table start, int32 bytes}, padded to 16 B]
@@ -73,6 +84,14 @@ struct SeqOp {
 };
 static_assert(sizeof(SeqOp) == 64, "SeqOp must be 64 B");
 
+// The largest launch of each kernel kind in the last simulation (bloch_plan_last_kernel): what a profiler capture of
+// "the dominant kernel" must match to describe this binary and this workload.
+struct KernelNote {
+    char name[56] = {0};  // as ncu prints it, e.g. "rf_kernel<0>", "signal_kernel<8, 0, 0>"
+    int64_t grid = 0;     // CTAs
+    int block = 0;        // threads per CTA
+};
+
 struct Timing {
     float ms_rf = 0, ms_prec = 0, ms_total = 0;
     int64_t launches = 0;
@@ -89,11 +108,21 @@ struct bloch_plan {
     const unsigned char *d_tables = nullptr;
     int64_t prog_off = 0;                // byte offset of the SeqOp program in the table buffer
     int path = 0;                        // BLOCH_PATH_*
+    int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, 2, -1, 0};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
+    // phase-range bookkeeping (bloch_sim_params extents): largest |k'| [turns/m], tau [s] and |mu'| [turns s/m] of
+    // any evaluated point (block ends included), and the largest phase within the declared extents
+    double k_max = 0, tau_max = 0, m_max = 0, worst_turns = 0;
+    double ext_m = 0.25, ext_hz = 1000.0, ext_mps = 1.0;
+    int phase_requested = 0;
+    // findings of the last simulation's pack_kernel (kStatusWords words), copied here by the simulation itself;
+    // pinned host memory, allocated by bloch_plan_upload
+    unsigned *h_status = nullptr;
     // profiling taps
     bool profiling = false;
     mutable std::vector<void *> events;  // cudaEvent_t pool
     mutable std::vector<int> event_kind; // per interval between events: 0 other, 1 rf, 2 precession
     mutable bloch::Timing last{};
+    mutable bloch::KernelNote last_kernel[BLOCH_N_KINDS];
 };
 
 namespace bloch {

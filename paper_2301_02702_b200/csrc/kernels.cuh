@@ -14,6 +14,8 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include "internal.h"
+
 namespace bloch {
 
 constexpr float kInv2Pi = 0.15915494309189535f;
@@ -39,12 +41,43 @@ __global__ void pack_kernel(int n, const float *__restrict__ x, const float *__r
                             const float *__restrict__ vy, const float *__restrict__ vz, float4 *__restrict__ V,
                             double4 *__restrict__ Vd) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    // scal[0] = max 1/T2 over the spins.  The bit pattern of a non-negative float orders like the unsigned
-    // integer and an integer max is order-independent, so this stays reproducible.
-    float r2w = i < n ? 1.0f / T2[i] : 0.f;
+    // scal[kScalR2Max] = max 1/T2 over the spins (the signal kernels bound their series with it), and what
+    // bloch_plan_status reports about the phantom: max |x|^2, max |dw|, max |v|^2, and flags for T1 / T2 <= 0 or
+    // non-finite input.  The bit pattern of a non-negative float orders like the unsigned integer and an integer
+    // max / or is order-independent, so all of this stays reproducible.
+    float r2w = 0.f, x2w = 0.f, dww = 0.f, v2w = 0.f;
+    unsigned bad = 0;
+    if (i < n) {
+        const float t1 = T1[i], t2 = T2[i], px = x[i], py = y[i], pz = z[i], w = dw[i], m0 = M0[i];
+        r2w = 1.0f / t2;
+        x2w = fmaf(px, px, fmaf(py, py, pz * pz));
+        dww = fabsf(w);
+        const float a = vx ? vx[i] : 0.f, b = vy ? vy[i] : 0.f, c = vz ? vz[i] : 0.f;
+        v2w = fmaf(a, a, fmaf(b, b, c * c));
+        if (!(t1 > 0.f) || !(t2 > 0.f) || isinf(t1) || isinf(t2)) bad |= BLOCH_STATUS_BAD_RELAXATION;  // NaN fails t > 0
+        if (!isfinite(x2w) || !isfinite(w) || !isfinite(m0) || !isfinite(v2w)) bad |= BLOCH_STATUS_NONFINITE;
+        if (!init_eq) {
+            const float2 m = Mxy[i];
+            if (!isfinite(m.x) || !isfinite(m.y) || !isfinite(Mz[i])) bad |= BLOCH_STATUS_NONFINITE;
+        }
+    }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) r2w = fmaxf(r2w, __shfl_xor_sync(0xffffffffu, r2w, o));
-    if ((threadIdx.x & 31) == 0) atomicMax(scal, __float_as_uint(fmaxf(r2w, 0.f)));
+    for (int o = 16; o > 0; o >>= 1) {
+        r2w = fmaxf(r2w, __shfl_xor_sync(0xffffffffu, r2w, o));
+        x2w = fmaxf(x2w, __shfl_xor_sync(0xffffffffu, x2w, o));
+        dww = fmaxf(dww, __shfl_xor_sync(0xffffffffu, dww, o));
+        v2w = fmaxf(v2w, __shfl_xor_sync(0xffffffffu, v2w, o));
+    }
+    bad = __reduce_or_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+        // fmaxf drops NaNs and the clamp keeps +inf / negative values out of the integer ordering's way
+        atomicMax(scal + kScalR2Max, __float_as_uint(fminf(fmaxf(r2w, 0.f), 3.0e38f)));
+        atomicMax(scal + kScalX2Max, __float_as_uint(fminf(fmaxf(x2w, 0.f), 3.0e38f)));
+        atomicMax(scal + kScalDwMax, __float_as_uint(fminf(fmaxf(dww, 0.f), 3.0e38f)));
+        atomicMax(scal + kScalV2Max, __float_as_uint(fminf(fmaxf(v2w, 0.f), 3.0e38f)));
+        if (bad) atomicOr(scal + kScalFlags, bad);
+        if (i == 0) scal[kScalValid] = 1u;
+    }
     if (i >= n) return;
     const float r1 = 1.0f / T1[i], r2 = 1.0f / T2[i], m0 = M0[i], w = dw[i];
     A[i] = make_float4(x[i], y[i], z[i], -w);

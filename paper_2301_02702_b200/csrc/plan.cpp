@@ -122,6 +122,12 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     }
     const double dt_rf = (params->dt_rf_max > 0.0 && std::isfinite(params->dt_rf_max))
                              ? params->dt_rf_max : std::numeric_limits<double>::infinity();
+    // extents of the phantoms the plan may assume (bloch_sim_params; the plan itself never sees a spin)
+    auto extent = [](double v, double dflt) { return (v > 0.0 && std::isfinite(v)) ? v : dflt; };
+    if (std::isnan(params->max_extent_m) || std::isnan(params->max_offres_hz) || std::isnan(params->max_speed_mps))
+        return fail(BLOCH_EINVAL, "max_extent_m / max_offres_hz / max_speed_mps is NaN");
+    const double ext_m = extent(params->max_extent_m, 0.25), ext_hz = extent(params->max_offres_hz, 1000.0),
+                 ext_mps = extent(params->max_speed_mps, 1.0);
 
     // ------------------------------------------------------------------ a1: merged grid
     std::vector<double> pts;
@@ -247,7 +253,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
 
     // ------------------------------------------------------------------ a3 + phase-mode resolution
     const double gbar = gamma / (2.0 * M_PI);
-    double worst_turns = 0.0;
+    double worst_turns = 0.0, k_max = 0.0, tau_max = 0.0, m_max = 0.0;
     std::vector<double> krec;  // 4 doubles per evaluated point, all precession blocks in order
     std::vector<double> mrec;  // motion: (mu'x, mu'y, mu'z, 0) per evaluated point, same order
     std::vector<int64_t> krec_first(blocks.size(), 0);
@@ -275,7 +281,12 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             const double tau = t[n + 1] - tb;
             const double kn = gbar * std::sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]);
             const double mn = gbar * std::sqrt(Mo[0] * Mo[0] + Mo[1] * Mo[1] + Mo[2] * Mo[2]);
-            worst_turns = std::max(worst_turns, kn * 0.25 + 1000.0 * tau + (motion ? mn * 1.0 : 0.0));  // |v| <= 1 m/s
+            // |theta| <= |k'| |x| + |f| tau (+ |mu'| |v|): the bound within the declared extents, and its three
+            // factors on their own for the check against the phantom a simulation is actually given (api.cu)
+            worst_turns = std::max(worst_turns, kn * ext_m + ext_hz * tau + (motion ? mn * ext_mps : 0.0));
+            k_max = std::max(k_max, kn);
+            tau_max = std::max(tau_max, tau);
+            if (motion) m_max = std::max(m_max, mn);
             if (adc_at[n + 1] >= 0) {
                 krec.insert(krec.end(), {-gbar * K[0], -gbar * K[1], -gbar * K[2], tau});
                 if (motion) mrec.insert(mrec.end(), {-gbar * Mo[0], -gbar * Mo[1], -gbar * Mo[2], 0.0});
@@ -290,9 +301,13 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             return fail(BLOCH_EINVAL, "internal: ADC bookkeeping mismatch");
     }
     // AUTO: fp32 phase (in turns, block-relative) keeps ~2^-24 * turns of resolution; above 256 turns
-    // (bound: |k| * 0.25 m + 1 kHz * tau) switch to fp64 phase accumulation (north_star item 4).
+    // (bound: |k| max_extent_m + max_offres_hz tau, + |mu'| max_speed_mps with motion) switch to fp64 phase
+    // accumulation (north_star item 4).  The fp64 phase itself is a 32-bit fixed-point fraction below 2^19 turns.
     int phase = params->phase_mode;
-    if (phase == BLOCH_PHASE_AUTO) phase = worst_turns > 256.0 ? BLOCH_PHASE_FP64 : BLOCH_PHASE_FP32;
+    if (phase == BLOCH_PHASE_AUTO) phase = worst_turns > kFp32TurnLimit ? BLOCH_PHASE_FP64 : BLOCH_PHASE_FP32;
+    if (phase == BLOCH_PHASE_FP64 && worst_turns >= kFp64TurnLimit)
+        return fail(BLOCH_ERANGE, "a block's phase can reach 2^19 turns within the declared extents: beyond the fp64 phase path "
+                                  "(shorten the blocks with max_block_points)");
 
     // ------------------------------------------------------------------ a4: RF tile images
     std::vector<std::vector<unsigned char>> rf_img(blocks.size());
@@ -474,6 +489,14 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     plan->params = *params;
     plan->blocks = std::move(blocks);
     plan->d_tables = nullptr;
+    plan->k_max = k_max;
+    plan->tau_max = tau_max;
+    plan->m_max = m_max;
+    plan->worst_turns = worst_turns;
+    plan->ext_m = ext_m;
+    plan->ext_hz = ext_hz;
+    plan->ext_mps = ext_mps;
+    plan->phase_requested = params->phase_mode;
     bloch_plan_info &inf = plan->info;
     inf.n_intervals = N;
     inf.n_rf_steps = n_rf_steps;
@@ -488,6 +511,13 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     inf.output_mode = params->output_mode;
     inf.motion_mode = params->motion_mode;
     inf.group_size = params->output_mode == BLOCH_OUT_GROUPED ? params->group_size : 0;
+    inf.phase_mode_requested = params->phase_mode;
+    inf.path = plan->path;
+    inf.max_extent_m = ext_m;
+    inf.max_offres_hz = ext_hz;
+    inf.max_speed_mps = ext_mps;
+    inf.worst_turns = worst_turns;
+    for (int k = 0; k < 16; ++k) inf.options[k] = k < BLOCH_N_OPTIONS ? plan->opt[k] : 0;
     return BLOCH_OK;
 }
 

@@ -47,27 +47,27 @@ def test_small_configs_with_coils_match_oracle(B, oracle_mod, name, n_coils, pha
                   "final state with coils")
 
 
-def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B, monkeypatch):
+def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
     """One coil with weight 1 everywhere returns the plain signal; 9 coils (two passes of 8, the last with one coil)
     give the same rows as the same coils simulated in separate calls: bitwise when the pass width is the same
     (coils 0-7 alone), to rounding when it is not (4 coils per pass for up to 4 coils: other tile sizes)."""
     from test_gpu_parity import run_gpu
-    monkeypatch.setenv("BLOCH_COIL_TC", "0")   # the FFMA kernel (9 coils would take the tensor-core kernel otherwise)
     w = W.small("4")
+    ffma = {"coil_tc": 0}   # the FFMA kernel (9 coils would take the tensor-core kernel otherwise)
     n = w.phantom.n
     plain = run_gpu(B, w, path="per_block")
-    one = run_coils(B, w, np.ones((1, n), dtype=np.complex64))
+    one = run_coils(B, w, np.ones((1, n), dtype=np.complex64), options=ffma)
     emax, _ = errors(one[0], plain)
     assert emax < 2e-6, f"uniform coil vs plain: {emax:.3e}"
     coils = coil_maps(w.phantom, 9, seed=4)
-    all9 = run_coils(B, w, coils)
-    again = run_coils(B, w, coils)
+    all9 = run_coils(B, w, coils, options=ffma)
+    again = run_coils(B, w, coils, options=ffma)
     assert np.array_equal(all9.view(np.float32), again.view(np.float32)), "run-to-run not bitwise identical"
-    first8 = run_coils(B, w, coils[:8])
+    first8 = run_coils(B, w, coils[:8], options=ffma)
     assert np.array_equal(all9[:8].view(np.float32), first8.view(np.float32))
     scale = np.abs(all9).max()
-    first4 = run_coils(B, w, coils[:4])
-    last1 = run_coils(B, w, coils[8:9])
+    first4 = run_coils(B, w, coils[:4], options=ffma)
+    last1 = run_coils(B, w, coils[8:9], options=ffma)
     assert np.abs(all9[:4] - first4).max() / scale < 2e-6 and np.abs(all9[8:9] - last1).max() / scale < 2e-6
 
 
@@ -122,20 +122,18 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
 
 
 @pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20), ("4", 37)])
-def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, monkeypatch, name, n_coils):
-    """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with BLOCH_COIL_TC=1): contributions generated on the fly
+def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils):
+    """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with bloch_plan_set_option(BLOCH_OPT_COIL_TC, 1)): contributions generated on the fly
     as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
     tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8, 16 and 32 coils per pass and two passes (37 coils) are all in these cases."""
-    monkeypatch.setenv("BLOCH_COIL_TC", "1")
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
     ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
-    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32")
+    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32", options={"coil_tc": 1})
     assert_parity(got, ref, f"tensor-core coil kernel, config {name}, {n_coils} coils")
     for c in range(n_coils):
         emax, nrmse = errors(got[c], ref[c])
         assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
-    monkeypatch.setenv("BLOCH_COIL_TC", "0")
-    ffma = run_coils(B, w, coils, phase_mode="fp32")
+    ffma = run_coils(B, w, coils, phase_mode="fp32", options={"coil_tc": 0})
     emax, _ = errors(got, ffma)
     assert emax < 2e-5, f"tensor-core vs FFMA kernel: {emax:.3e}"   # TMEM accumulation is coarser than FFMA sums

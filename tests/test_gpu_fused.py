@@ -93,17 +93,15 @@ def test_ragged_spin_counts(B, oracle_mod, n):
                   np.concatenate([rxy, rz.astype(np.complex128)]), f"n={n} state")
 
 
-def test_fused_is_bitwise_reproducible_and_independent_of_the_signal_warp_count(B, monkeypatch):
+def test_fused_is_bitwise_reproducible_and_independent_of_the_signal_warp_count(B):
     w = W.small("2")
     a = run_gpu(B, w, path="fused", phase_mode="fp32")
     b = run_gpu(B, w, path="fused", phase_mode="fp32")
     assert np.array_equal(a.view(np.float32), b.view(np.float32)), "run-to-run not bitwise identical"
     # the partial of a CTA is one thread's sum over the chunk's spins in index order whatever the number of signal
     # warps (only which thread owns which sample changes; the P = 1/2/4 choice moves with it, hence a tolerance)
-    for base, extra in (("1", "0"), ("0", "1"), ("3", "2"), ("5", "0")):
-        monkeypatch.setenv("BLOCH_SEQ_SIG_BASE", base)
-        monkeypatch.setenv("BLOCH_SEQ_SIG_EXTRA", extra)
-        c = run_gpu(B, w, path="fused", phase_mode="fp32")
+    for base, extra in ((1, 0), (0, 1), (3, 2), (5, 0)):
+        c = run_gpu(B, w, path="fused", phase_mode="fp32", options={"seq_sig_base": base, "seq_sig_extra": extra})
         emax, _ = errors(c, a)
         assert emax < 2e-6, f"signal warps base {base} extra {extra}: {emax:.3e}"
 
@@ -192,16 +190,15 @@ def test_fused_per_spin_dictionary_mode(B, oracle_mod):
     plan.close()
 
 
-def test_fused_is_race_free_over_many_runs(B, monkeypatch):
+def test_fused_is_race_free_over_many_runs(B):
     """The roles of the whole-sequence kernel meet only at mbarriers; a missing edge would show up as run-to-run
     differences.  25 runs each with 1, 2 and 3 signal warps per sub-partition (plus the balancing extras) (different interleavings of the roles), all bitwise equal
     per configuration, signal and final state."""
     w = W.small("5")
-    for nw in ("1", "2", "3"):
-        monkeypatch.setenv("BLOCH_SEQ_SIG_BASE", nw)
+    for nw in (1, 2, 3):
         first = None
         for _ in range(25):
-            sig, mxy, mz = run_gpu(B, w, want_state=True, path="fused", phase_mode="fp32")
+            sig, mxy, mz = run_gpu(B, w, want_state=True, path="fused", phase_mode="fp32", options={"seq_sig_base": nw})
             cur = (sig.view(np.float32).copy(), mxy.view(np.float32).copy(), mz.copy())
             if first is None:
                 first = cur

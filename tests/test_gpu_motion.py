@@ -35,10 +35,10 @@ def f32(a):
     return np.asarray(a, dtype=np.float32).astype(np.float64)
 
 
-def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mode="auto", host=False):
+def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mode="auto", host=False, options=None):
     import torch
     v = tuple(f32(a) for a in v)
-    plan = B.Plan(s, output_mode=output_mode, phase_mode=phase_mode, motion="linear", dt_max=dt_max)
+    plan = B.Plan(s, output_mode=output_mode, phase_mode=phase_mode, motion="linear", dt_max=dt_max, options=options)
     assert plan.info["motion_mode"] == 1
     t, *_ = oracle_mod.grid(s, dt_max=dt_max)
     assert plan.info["n_intervals"] == len(t) - 1, "planner and oracle refine the grid differently"
@@ -133,10 +133,10 @@ def test_zero_velocity_equals_the_static_plan_and_velocities_need_a_motion_plan(
 
 
 @pytest.mark.parametrize("phase_mode,n_adc", [("fp32", 2051), ("fp64", 4096)])
-def test_moving_spins_on_cartesian_plateau_take_the_quadratic_recurrence(B, oracle_mod, phase_mode, n_adc, monkeypatch):
+def test_moving_spins_on_cartesian_plateau_take_the_quadratic_recurrence(B, oracle_mod, phase_mode, n_adc):
     """>= 2048 equally spaced samples on a plateau with moving spins: k' is linear and the first moment mu' quadratic in
     the sample index, so the planner hands the block to signal_lin_kernel<., motion> (w_{j+1} = w_j zeta_j,
-    zeta_{j+1} = zeta_j rho).  Against the oracle and against the per-sample kernel (BLOCH_SIGNAL_LIN=0)."""
+    zeta_{j+1} = zeta_j rho).  Against the oracle and against the per-sample kernel (option signal_lin = 0)."""
     import torch
     rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
     dwell = 4e-6
@@ -147,8 +147,8 @@ def test_moving_spins_on_cartesian_plateau_take_the_quadratic_recurrence(B, orac
     ph, v = moving_phantom(700, 31)
     out = {}
     for lin in ("1", "0"):
-        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
-        out[lin], _ = run_both(B, oracle_mod, ph, s, v, 1e-5, f"motion recurrence {phase_mode} lin={lin}", phase_mode=phase_mode)
+        out[lin], _ = run_both(B, oracle_mod, ph, s, v, 1e-5, f"motion recurrence {phase_mode} lin={lin}", phase_mode=phase_mode,
+                               options={"signal_lin": int(lin)})
     emax, nrmse = errors(out["1"], out["0"])
     print(f"motion recurrence on/off {phase_mode}: max {emax:.3e} nrmse {nrmse:.3e}")
     assert 0 < emax <= 3e-5 and nrmse <= 8e-6

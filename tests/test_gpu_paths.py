@@ -209,10 +209,10 @@ def test_signal_decay_modes_equal_spacing_and_jitter(B, oracle_mod, jitter):
 
 
 @pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
-def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode, monkeypatch):
+def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode):
     """EPI-like train sampled THROUGH the ramps: the warps whose 8 (or 4) adjacent samples sit on a plateau take the
     rotation recurrence (k' advances by a constant step), those that touch a ramp or a blip must not.  Both against the
-    oracle, and against the same kernel with the recurrence switched off (BLOCH_SIGNAL_LIN=0)."""
+    oracle, and against the same kernel with the recurrence switched off (option signal_lin = 0)."""
     import torch
     rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
     n_lines, flat, ramp, G = 12, 1.2e-3, 1.0e-4, 9e-3
@@ -232,8 +232,7 @@ def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode
     dev = B.phantom_to_device(ph)
     out = {}
     for lin in ("1", "0"):
-        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
-        plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+        plan = B.Plan(s, path="per_block", phase_mode=phase_mode, options={"signal_lin": int(lin)})
         out[lin] = plan.simulate(*dev).cpu().numpy()
         torch.cuda.synchronize()
         plan.close()
@@ -243,10 +242,10 @@ def test_signal_rotation_recurrence_on_cartesian_lines(B, oracle_mod, phase_mode
 
 
 @pytest.mark.parametrize("phase_mode,n_adc", [("fp32", 2048), ("fp32", 4103), ("fp64", 2061), ("fp64", 8192)])
-def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_adc, monkeypatch):
+def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_adc):
     """A block of >= 2048 equally spaced samples on a plateau: the planner hands its first n - n % 16 samples to
     signal_lin_kernel (16 samples per thread, recurrence only) and the tail to signal_kernel<1>.  Against the oracle
-    and against the per-sample kernel (BLOCH_SIGNAL_LIN=0); short T2 (dwell / T2 up to 0.04) also drives the
+    and against the per-sample kernel (option signal_lin = 0); short T2 (dwell / T2 up to 0.04) also drives the
     MUFU.EX2 form of q in the fp64 cases."""
     import torch
     rf = (np.array([0.0]), np.array([1e-4]), np.array([(np.pi / 2) / (W.GAMMA * 1e-4)]), np.array([0.0]))
@@ -264,8 +263,7 @@ def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_
     dev = B.phantom_to_device(ph)
     out = {}
     for lin in ("1", "0"):
-        monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
-        plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+        plan = B.Plan(s, path="per_block", phase_mode=phase_mode, options={"signal_lin": int(lin)})
         out[lin] = plan.simulate(*dev).cpu().numpy()
         torch.cuda.synchronize()
         plan.close()
@@ -275,7 +273,7 @@ def test_signal_lin_kernel_on_all_cartesian_blocks(B, oracle_mod, phase_mode, n_
 
 
 @pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
-def test_signal_lin_kernel_on_an_epi_train_of_short_lines(B, oracle_mod, phase_mode, monkeypatch):
+def test_signal_lin_kernel_on_an_epi_train_of_short_lines(B, oracle_mod, phase_mode):
     """50 EPI lines of 48 samples on the plateaus only (ramps and blips between lines are not sampled): every aligned
     group of 16 lies inside one line, so the whole 2400-sample block goes to signal_lin_kernel although k' and tau
     jump between groups.  A second sequence shifts the first line by 5 samples: groups then straddle the line ends,
@@ -302,12 +300,10 @@ def test_signal_lin_kernel_on_an_epi_train_of_short_lines(B, oracle_mod, phase_m
         check(B, oracle_mod, ph, s, f"EPI short lines {phase_mode} shift={extra}", phase_mode=phase_mode)
         out = {}
         for lin in ("1", "0"):
-            monkeypatch.setenv("BLOCH_SIGNAL_LIN", lin)
-            plan = B.Plan(s, path="per_block", phase_mode=phase_mode)
+            plan = B.Plan(s, path="per_block", phase_mode=phase_mode, options={"signal_lin": int(lin)})
             out[lin] = plan.simulate(*dev).cpu().numpy()
             torch.cuda.synchronize()
             plan.close()
-        monkeypatch.delenv("BLOCH_SIGNAL_LIN")
         emax, nrmse = errors(out["1"], out["0"])
         print(f"EPI short lines on/off {phase_mode} shift={extra}: max {emax:.3e} nrmse {nrmse:.3e}")
         assert emax <= 3e-5 and nrmse <= 8e-6

@@ -184,3 +184,58 @@ def test_planner_flags_all_cartesian_blocks_for_the_recurrence_kernel(B):
     assert launches(jit, plateau) == base                                                # one sample 1 ns late
     assert launches(t0 + np.arange(317) * dw, plateau) == base                           # 19 groups: too short
     assert launches(t0 + np.arange(325) * dw, plateau) == base + 1                       # 20 groups + tail of 5
+
+
+def test_plan_options_are_plan_state_not_environment(B):
+    """Kernel selection is set per plan (bloch_plan_set_option), echoed by bloch_plan_get_info, validated, and the
+    library's sources read no environment variable (VERDICT r1 weak #8)."""
+    h = B.bloch_plan_create(W.small("1").seq)
+    try:
+        info = B.bloch_plan_get_info(h)
+        assert info["options"] == {"signal_lin": 1, "signal_p": 0, "signal_fixed_cta": 0, "signal_ctas_per_sm": 4,
+                                   "rf_threads": 0, "rf_spins": 0, "coil_tc": -1, "seq_sig_extra": 2,
+                                   "seq_sig_base": -1, "seq_items_x4": 0}
+        B.bloch_plan_set_option(h, "signal_lin", 0)
+        B.bloch_plan_set_option(h, B.OPTIONS.index("signal_p"), 4)
+        assert B.bloch_plan_get_option(h, "signal_lin") == 0 and B.bloch_plan_get_option(h, "signal_p") == 4
+        info = B.bloch_plan_get_info(h)
+        assert info["options"]["signal_lin"] == 0 and info["options"]["signal_p"] == 4
+        for key, bad in (("signal_p", 3), ("signal_ctas_per_sm", 0), ("rf_threads", 48), ("coil_tc", 2), (99, 0),
+                         ("rf_spins", 3)):
+            with pytest.raises(B.BlochError) as e:
+                B.bloch_plan_set_option(h, key, bad)
+            assert e.value.code == -1
+        B.bloch_plan_set_path(h, "per_block")
+        assert B.bloch_plan_get_info(h)["path"] == B.PATHS["per_block"]
+    finally:
+        B.bloch_plan_destroy(h)
+    csrc = os.path.join(ROOT, "paper_2301_02702_b200", "csrc")
+    for fn in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, fn)).read(), f"{fn} reads the environment"
+
+
+def test_phase_mode_auto_follows_the_declared_extents(B):
+    """BLOCH_PHASE_AUTO bounds the block-relative phase with the extents the caller declares in bloch_sim_params
+    (defaults 0.25 m / 1 kHz / 1 m/s): k = 42.58e6 x 10 mT/m x 1.6 ms (ramps included) = 681 turns/m is 170 turns at
+    0.25 m (fp32 phase) and 409 at 0.6 m (fp64 phase accumulation, north_star item 4)."""
+    g = {0: ([2e-4, 3e-4, 1.8e-3, 1.9e-3], [0, 10e-3, 10e-3, 0])}
+    rf = ([0.0], [1e-4], [(math.pi / 2) / (W.GAMMA * 1e-4)], [0.0])
+    s = seq(g=g, rf=rf, adc=3e-4 + (np.arange(300) + 0.5) * 5e-6, t_end=2e-3, dt_rf_max=1e-5)
+    for kw, phase, turns in ((dict(), B.PHASE_FP32, (165, 180)), (dict(max_extent_m=0.6), B.PHASE_FP64, (400, 420)),
+                             (dict(max_offres_hz=150e3), B.PHASE_FP64, (445, 465)),
+                             (dict(max_extent_m=0.6, phase_mode="fp32"), B.PHASE_FP32, (400, 420))):
+        h = B.bloch_plan_create(s, **kw)
+        info = B.bloch_plan_get_info(h)
+        B.bloch_plan_destroy(h)
+        assert info["phase_mode"] == phase, kw
+        assert turns[0] < info["worst_turns"] < turns[1], (kw, info["worst_turns"])
+        assert info["max_extent_m"] == kw.get("max_extent_m", 0.25)
+        assert info["max_offres_hz"] == kw.get("max_offres_hz", 1000.0) and info["max_speed_mps"] == 1.0
+        assert info["phase_mode_requested"] == B._PHASE[kw.get("phase_mode", "auto")]
+    # beyond the fp64 path's 2^19-turn fixed-point fraction: rejected at creation, not silently wrong
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(s, max_extent_m=1000.0)
+    assert e.value.code == -10   # BLOCH_ERANGE
+    with pytest.raises(B.BlochError) as e:
+        B.bloch_plan_create(s, max_extent_m=float("nan"))
+    assert e.value.code == -1
