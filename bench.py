@@ -326,7 +326,7 @@ def measure(bloch, torch, dist, w, w_whole, args, steps, warmup, rank, local_ran
     from paper_2301_02702_b200.dist import reduce_signal
     per_spin = w.output_mode in ("per_spin", "grouped")   # no cross-rank sum: outputs stay sharded
     t_plan0 = time.perf_counter()
-    plan = bloch.Plan(w.seq, path=args.path, **w.plan_kw)
+    plan = bloch.Plan(w.seq, path=args.path, options=args.options, **w.plan_kw)
     plan.upload()
     torch.cuda.synchronize()
     plan_s = time.perf_counter() - t_plan0
@@ -402,7 +402,7 @@ def measure(bloch, torch, dist, w, w_whole, args, steps, warmup, rank, local_ran
     # ---- strong scaling: the reduced signal of the sharded run must be the 1-GPU signal of the whole workload
     shard_check = None
     if strong and not per_spin and rank == 0:
-        plan1 = bloch.Plan(w_whole.seq, path=args.path, **w_whole.plan_kw)
+        plan1 = bloch.Plan(w_whole.seq, path=args.path, options=args.options, **w_whole.plan_kw)
         d1 = bloch.phantom_to_device(w_whole.phantom)
         v1 = None if w_whole.velocity is None else tuple(
             torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w_whole.velocity)
@@ -538,7 +538,7 @@ def run_ours(args, rank, local_rank, world):
                                    "sum of the per-rank signals" if args.scaling == "strong" else
                                    "weak: every rank simulates its own seed-shifted phantom of the named size"),
                       "l2": "512 MiB buffer written before every timed step (untimed); per-step CUDA events",
-                      "plan_create_upload_s": head["plan_create_upload_s"]},
+                      "plan_options": args.options, "plan_create_upload_s": head["plan_create_upload_s"]},
            "sim_wall_time_s": head["ms_per_step"] * 1e-3,
            "clocks": clocks.summary(),
            "e2e": head["e2e"],
@@ -574,11 +574,14 @@ def main():
     ap.add_argument("--extra", default=EXTRA_DEFAULT,
                     help="other configs timed in short runs and reported under 'workloads' (comma list, or 'none')")
     ap.add_argument("--extra-steps", type=int, default=3)
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="diagnostic: a kernel-selection option of the plan (bloch_plan_set_option), e.g. rf_spins=2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-taps", action="store_true", help="diagnostic: no per-kernel CUDA events inside the timed steps")
     ap.add_argument("--cpu-budget", type=float, default=0.0, help="spin*steps for the cpu_baseline sample (0 = auto)")
     ap.add_argument("--microbench", action="store_true", help="also run the MUFU/FFMA/DFMA pipe micro-benchmarks")
     args = ap.parse_args()
+    args.options = {k: int(v) for k, v in (o.split("=", 1) for o in args.option)}
     from paper_2301_02702_b200.dist import env_world
     rank, local_rank, world = env_world()
     if args.cpu_budget <= 0:

@@ -769,12 +769,16 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     PropRec prop{0, 0, 0, 0, 0, 0, 0};
     // RF launch shape: one spin per thread; small CTAs when spins are few so the warps spread over all
     // 592 sub-partitions, 128-thread CTAs once there are >= 32 warps per SM
+    // two spins per thread (rf_pair_kernel; static plans) on request: measured in DESIGN.md section 12
+    const bool rf_pair = !mo && plan->opt[BLOCH_OPT_RF_SPINS] == 2;
+    const int rf_items = rf_pair ? (n + 1) / 2 : n;
     const int rf_threads = plan->opt[BLOCH_OPT_RF_THREADS] ? plan->opt[BLOCH_OPT_RF_THREADS]
-                                                           : ((n + 31) / 32 >= sms * 32 ? 128 : 32);
-    const int rf_grid = (n + rf_threads - 1) / rf_threads;
+                                                           : ((rf_items + 31) / 32 >= sms * 32 ? 128 : 32);
+    const int rf_grid = (rf_items + rf_threads - 1) / rf_threads;
     auto launch_rf = [&](const unsigned char *tbl, int n_tiles, int has_prop) -> int {
-        if (tbl) note_kernel(plan, BLOCH_KIND_RF, rf_grid, rf_threads, "rf_kernel<%d>", mo ? 1 : 0);
-        if (mo) rf_kernel<true><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, w.V, n);
+        if (tbl) note_kernel(plan, BLOCH_KIND_RF, rf_grid, rf_threads, rf_pair ? "rf_pair_kernel" : "rf_kernel<%d>", mo ? 1 : 0);
+        if (rf_pair) rf_pair_kernel<<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, n);
+        else if (mo) rf_kernel<true><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, w.V, n);
         else rf_kernel<false><<<rf_grid, rf_threads, 0, stream>>>(tbl, n_tiles, prop, has_prop, w.A, w.C, w.S, nullptr, n);
         return BLOCH_OK;
     };

@@ -155,6 +155,53 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
 #undef BLOCH_RF_LOAD
 }
 
+// Tier-0 tile for TWO spins per thread (static plans).  The step record (wx, wy, wx^2 + wy^2 and, on general tiles, g)
+// is warp-uniform and the same for both spins, so it is loaded once, and the two spins' cross products sit next to
+// each other in the instruction stream with wx, wy in the same operand slot (the operand-reuse cache can then serve
+// the second read: the RF step is bound by register-file operand bandwidth).  Each spin's own
+// arithmetic is rf_increment<0> exactly as in rf_tile<0, MODE>, so the result is bitwise that of one spin per thread.
+template <int MODE>
+__device__ __forceinline__ void rf_tile0_pair(const unsigned char *tile, const RfTileHdr &hd, const RfSpin &sa,
+                                              const RfSpin &sb, const RfRelax &ra, const RfRelax &rb, float (&h)[6],
+                                              float (&l)[6]) {
+    const float4 *rec = reinterpret_cast<const float4 *>(tile + kRfHdrBytes);
+    const int n = hd.n_steps;
+    const float dtdw_a = hd.dt * sa.dw, dtdw_b = hd.dt * sb.dw;
+    const float wz_ua = fmaf(hd.gx, sa.x, fmaf(hd.gy, sa.y, fmaf(hd.gz, sa.z, dtdw_a)));
+    const float wz_ub = fmaf(hd.gx, sb.x, fmaf(hd.gy, sb.y, fmaf(hd.gz, sb.z, dtdw_b)));
+    const float wz2_ua = __fmul_rn(wz_ua, wz_ua), wz2_ub = __fmul_rn(wz_ub, wz_ub);
+#define BLOCH_RF_PAIR_STEP(k)                                                                          \
+    {                                                                                                  \
+        float wx, wy, wza, wzb, qa, qb;                                                                \
+        if (MODE == 0) {                                                                               \
+            const float4 a = rec[k];                                                                   \
+            wx = a.x; wy = a.y; wza = wz_ua; wzb = wz_ub;                                              \
+            qa = __fadd_rn(a.z, wz2_ua); qb = __fadd_rn(a.z, wz2_ub);                                  \
+        } else {                                                                                       \
+            const float4 a = rec[2 * (k)], g = rec[2 * (k) + 1];                                       \
+            wx = a.x; wy = a.y;                                                                        \
+            wza = fmaf(g.x, sa.x, fmaf(g.y, sa.y, fmaf(g.z, sa.z, dtdw_a)));                           \
+            wzb = fmaf(g.x, sb.x, fmaf(g.y, sb.y, fmaf(g.z, sb.z, dtdw_b)));                           \
+            qa = fmaf(wza, wza, a.z); qb = fmaf(wzb, wzb, a.z);                                        \
+        }                                                                                              \
+        float ta0, ta1, ta2, tb0, tb1, tb2;                                                            \
+        rf_increment<0>(wx, wy, wza, qa, h[0] + l[0], h[1] + l[1], h[2] + l[2], ra, ta0, ta1, ta2);    \
+        rf_increment<0>(wx, wy, wzb, qb, h[3] + l[3], h[4] + l[4], h[5] + l[5], rb, tb0, tb1, tb2);    \
+        l[0] += ta0; l[1] += ta1; l[2] += ta2; l[3] += tb0; l[4] += tb1; l[5] += tb2;                  \
+    }
+    int k = 0;
+    for (; k + 8 <= n; k += 8) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) BLOCH_RF_PAIR_STEP(k + j)
+#pragma unroll
+        for (int c = 0; c < 6; ++c) fold(h[c], l[c]);
+    }
+    for (; k < n; ++k) BLOCH_RF_PAIR_STEP(k)
+#pragma unroll
+    for (int c = 0; c < 6; ++c) fold(h[c], l[c]);
+#undef BLOCH_RF_PAIR_STEP
+}
+
 constexpr int kRfMaxThreads = 128;
 
 // MO: motion plans (48-B step records, velocities); the static instantiation keeps its registers and shared
@@ -234,6 +281,84 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         }
     }
     if (active) S[i] = make_float4(hx + lx, hy + ly, hz + lz, s.w);
+}
+
+// Two spins per thread (static plans; BLOCH_OPT_RF_SPINS): thread t owns spins t and t + ceil(n / 2).  Tiles whose
+// bound on q leaves tier 0 (never with the configs' pulses) fall back to rf_tile one spin after the other.
+__global__ void __launch_bounds__(kRfMaxThreads)
+rf_pair_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int has_prop,
+               const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
+    __shared__ __align__(128) unsigned char buf[2][kRfHdrBytes + kRfTileSteps * 32];
+    __shared__ __align__(8) uint64_t bar[2];
+    const int tid = threadIdx.x;
+    const int2 *dir = reinterpret_cast<const int2 *>(tbl);
+    if (tid == 0 && n_tiles > 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init_fence();
+        for (int b = 0; b < 2 && b < n_tiles; ++b) {
+            const int2 d = dir[b];
+            mbar_expect_tx(&bar[b], (uint32_t)d.y);
+            bulk_g2s(buf[b], tbl + d.x, (uint32_t)d.y, &bar[b]);
+        }
+    }
+    const int half = (n + 1) / 2;
+    const int ia = blockIdx.x * blockDim.x + tid, ib = ia + half;
+    const bool act_a = ia < half, act_b = act_a && ib < n;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 0.f, 0.f);
+    float4 aa = zero, ca = one, st_a = zero, ab = zero, cb = one, st_b = zero;
+    if (act_a) { aa = A[ia]; ca = Cc[ia]; st_a = S[ia]; }
+    if (act_b) { ab = A[ib]; cb = Cc[ib]; st_b = S[ib]; }
+    float h[6] = {st_a.x, st_a.y, st_a.z, st_b.x, st_b.y, st_b.z};
+    float l[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (has_prop) {
+        propagate(prop, aa, ca, zero, h[0], h[1], h[2]);
+        propagate(prop, ab, cb, zero, h[3], h[4], h[5]);
+    }
+    const RfSpin sa{aa.x, aa.y, aa.z, ca.w, ca.x, ca.y, ca.z, 0.f, 0.f, 0.f};
+    const RfSpin sb{ab.x, ab.y, ab.z, cb.w, cb.x, cb.y, cb.z, 0.f, 0.f, 0.f};
+    const float ax = fmaxf(fabsf(sa.x), fabsf(sb.x)), ay = fmaxf(fabsf(sa.y), fabsf(sb.y)),
+                az = fmaxf(fabsf(sa.z), fabsf(sb.z)), adw = fmaxf(fabsf(sa.dw), fabsf(sb.dw));
+    __syncthreads();  // barrier initialisation visible to every waiter
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int b = t & 1;
+        mbar_wait(&bar[b], (uint32_t)((t >> 1) & 1));
+        const unsigned char *tile = buf[b];
+        const RfTileHdr hd = *reinterpret_cast<const RfTileHdr *>(tile);
+        RfRelax ra, rb;
+        ra.D1 = -expm1f(-hd.dt * sa.r1); ra.D2 = -expm1f(-hd.dt * sa.r2);
+        ra.E1 = 1.0f - ra.D1; ra.E2 = 1.0f - ra.D2; ra.D1m0 = ra.D1 * sa.m0;
+        rb.D1 = -expm1f(-hd.dt * sb.r1); rb.D2 = -expm1f(-hd.dt * sb.r2);
+        rb.E1 = 1.0f - rb.D1; rb.E2 = 1.0f - rb.D2; rb.D1m0 = rb.D1 * sb.m0;
+        const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
+        const float qb = fmaf(wzb, wzb, hd.wxy2_max);
+        const bool uni = (hd.flags & kRfFlagUniformG) != 0;
+        if (__all_sync(0xffffffffu, qb <= 0.00390625f)) {
+            if (uni) rf_tile0_pair<0>(tile, hd, sa, sb, ra, rb, h, l);
+            else rf_tile0_pair<1>(tile, hd, sa, sb, ra, rb, h, l);
+        } else {
+            const int tier = __all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2;
+#define BLOCH_RF_ONE(T, M, SP, RX, O) rf_tile<T, M>(tile, hd, SP, RX, h[O], h[O + 1], h[O + 2], l[O], l[O + 1], l[O + 2])
+#define BLOCH_RF_BOTH(T)                                                              \
+    do {                                                                              \
+        if (uni) { BLOCH_RF_ONE(T, 0, sa, ra, 0); BLOCH_RF_ONE(T, 0, sb, rb, 3); }    \
+        else { BLOCH_RF_ONE(T, 1, sa, ra, 0); BLOCH_RF_ONE(T, 1, sb, rb, 3); }        \
+    } while (0)
+            if (tier == 1) BLOCH_RF_BOTH(1);
+            else BLOCH_RF_BOTH(2);
+#undef BLOCH_RF_BOTH
+#undef BLOCH_RF_ONE
+        }
+        __syncthreads();  // every thread is done reading buf[b]
+        if (tid == 0 && t + 2 < n_tiles) {
+            const int2 d = dir[t + 2];
+            mbar_expect_tx(&bar[b], (uint32_t)d.y);
+            bulk_g2s(buf[b], tbl + d.x, (uint32_t)d.y, &bar[b]);
+        }
+    }
+    if (act_a) S[ia] = make_float4(h[0] + l[0], h[1] + l[1], h[2] + l[2], st_a.w);
+    if (act_b) S[ib] = make_float4(h[3] + l[3], h[4] + l[4], h[5] + l[5], st_b.w);
 }
 
 }  // namespace bloch

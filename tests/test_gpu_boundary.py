@@ -134,8 +134,8 @@ def test_off_resonance_and_speed_extents_are_measured_too(B):
     with pytest.raises(B.BlochError) as e:
         plan.status()
     assert e.value.code == ERANGE
-    v = tuple(torch.full((ph.n,), val, dtype=torch.float32, device="cuda") for val in (40.0, 0.0, 0.0))
-    plan.simulate(*dev, velocity=v)                     # 40 m/s x first moment
+    v = tuple(torch.full((ph.n,), val, dtype=torch.float32, device="cuda") for val in (400.0, 0.0, 0.0))
+    plan.simulate(*dev, velocity=v)                     # 400 m/s x first moment (~0.7 turn s/m) on top of 172 turns
     with pytest.raises(B.BlochError) as e:
         plan.status()
     assert e.value.code == ERANGE

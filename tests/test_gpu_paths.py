@@ -309,3 +309,28 @@ def test_signal_lin_kernel_on_an_epi_train_of_short_lines(B, oracle_mod, phase_m
         assert emax <= 3e-5 and nrmse <= 8e-6
         if extra == 0:
             assert emax > 0      # the recurrence kernel did run
+
+
+@pytest.mark.parametrize("name", ["1", "2", "4", "5"])
+def test_two_spins_per_thread_rf_kernel_is_bitwise_the_one_spin_kernel(B, oracle_mod, name):
+    """rf_pair_kernel (BLOCH_OPT_RF_SPINS = 2): thread t owns spins t and t + ceil(n / 2) and shares the step record
+    between them; every spin's own arithmetic is unchanged, so signal and final magnetisation are bitwise those of
+    rf_kernel (odd spin counts, compact and general tiles, propagate at block starts), and match the oracle."""
+    from test_gpu_parity import run_gpu
+    w = W.small(name)
+    out = {}
+    for spins in (1, 2):
+        out[spins] = run_gpu(B, w, want_state=True, path="per_block", options={"rf_spins": spins})
+    for a, b in zip(out[1], out[2]):
+        assert np.array_equal(np.asarray(a).view(np.float32), np.asarray(b).view(np.float32))
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, output_mode=w.output_mode, return_state=True)
+    emax, nrmse = errors(out[2][0], ref)
+    assert emax <= 1e-4 and nrmse <= 1e-5
+    # an odd number of spins: the last thread's second spin does not exist
+    ph = w.phantom.subset(np.arange(w.phantom.n - (1 - w.phantom.n % 2)))
+    assert ph.n % 2 == 1
+    w2 = W.Workload(w.name, ph, w.seq, phase_mode=w.phase_mode, output_mode=w.output_mode)
+    a = run_gpu(B, w2, want_state=True, path="per_block", options={"rf_spins": 1})
+    b = run_gpu(B, w2, want_state=True, path="per_block", options={"rf_spins": 2})
+    for u, v in zip(a, b):
+        assert np.array_equal(np.asarray(u).view(np.float32), np.asarray(v).view(np.float32))
