@@ -161,10 +161,15 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
 struct SeqShape {
     bool ok, use;
     int n_ctas, chunk, rf_warps, sig_warps, threads, min_items;
+    int ring_slots, slot_stride;  // partial-row ring: [ring_slots][n_ctas][slot_stride] float2
     SeqRoles roles;
-    size_t smem, partial_elems;
+    size_t smem, partial_elems, ticket_off;  // float2 elements of the partial area; where the tickets start in it
 };
-constexpr size_t kSeqPartialCapBytes = size_t(8) << 30;
+// The ring holds the partial rows of the kSeqRingSlots blocks between "written" and "summed over CTAs" (seq.cuh), so
+// its size is set by the LARGEST block, not by the sequence (config 5: 8 x 147 x 1024 x 8 B = 9.6 MB, where one row per
+// CTA over the whole sequence was 1.2 GB); the path is unavailable only if that passes kSeqRingCapBytes (a single block
+// of > 900k samples on 148 SMs; max_block_points cuts such blocks).
+constexpr size_t kSeqRingCapBytes = size_t(8) << 30;
 
 SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     SeqShape q{};
@@ -235,8 +240,14 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     q.min_items = std::max(1, q.sig_warps * plan->opt[BLOCH_OPT_SEQ_ITEMS_X4] / 4);  // 0: always the largest P (config 5: 127.6 ms against 131.1 with one item per warp)
     q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
     q.smem = seq_smem_bytes(q.chunk);
-    q.partial_elems = size_t(q.n_ctas) * size_t(std::max<int64_t>(inf.n_adc, 1));
-    if (q.partial_elems * sizeof(float2) > kSeqPartialCapBytes || inf.max_block_adc > INT32_MAX) return q;
+    if (inf.max_block_adc > INT32_MAX / 2) return q;
+    q.slot_stride = (int)std::max<int64_t>(32, (inf.max_block_adc + 31) / 32 * 32);
+    q.ring_slots = kSeqRingSlots;
+    if (ps) { q.ring_slots = 1; q.slot_stride = 32; }  // PER_SPIN: no partial rows at all
+    const size_t ring_elems = ps ? 0 : size_t(q.ring_slots) * size_t(q.n_ctas) * size_t(q.slot_stride);
+    if (ring_elems * sizeof(float2) > kSeqRingCapBytes) return q;
+    q.ticket_off = (ring_elems + 31) / 32 * 32;
+    q.partial_elems = q.ticket_off + (size_t(2) * size_t(std::max<int64_t>(plan->n_adc_blocks, 1)) * sizeof(int) + 7) / 8;
     q.ok = true;
     // AUTO: the fused kernel pays when the excitation is a fair share of the work and the full set of signal warps
     // fits beside the RF warps (its readout runs on sig_warps warps per SM only).  Measured, fused / per-block ms:
@@ -736,21 +747,32 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         if ((rc = taps.mark(BLOCH_KIND_FUSED))) return rc;
         const SeqOp *prog = reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off);
         note_kernel(plan, BLOCH_KIND_FUSED, sq.n_ctas, sq.threads, "seq_kernel<%d>", per_spin ? 1 : 0);
-        if (per_spin)
-            seq_kernel<true><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
-                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.roles, sq.min_items,
-                (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, (float2 *)d_signal);
-        else
-            seq_kernel<false><<<sq.n_ctas, sq.threads, sq.smem, stream>>>(
-                plan->d_tables, prog, (int)plan->blocks.size(), w.A, w.C, w.S, n, sq.chunk, sq.rf_warps, sq.roles, sq.min_items,
-                (const float *)w.scal, w.partial, (long long)plan->info.n_adc, d_Mxy ? 1 : 0, nullptr);
-        ++launches;
-        if (plan->info.n_adc > 0 && !per_spin) {
-            if ((rc = taps.mark(BLOCH_KIND_REDUCE))) return rc;
-            reduce_kernel<<<(unsigned)((plan->info.n_adc + 31) / 32), dim3(32, 8), 0, stream>>>(
-                w.partial, sq.n_ctas, (int)plan->info.n_adc, (float2 *)d_signal);
-            ++launches;
+        // kernel arguments by address (cudaLaunchCooperativeKernel)
+        const unsigned char *a_tables = plan->d_tables;
+        int a_nops = (int)plan->blocks.size(), a_n = n, a_chunk = sq.chunk, a_rfw = sq.rf_warps, a_min = sq.min_items;
+        const float4 *a_A = w.A, *a_C = w.C;
+        float4 *a_S = w.S;
+        SeqRoles a_roles = sq.roles;
+        const float *a_scal = (const float *)w.scal;
+        float2 *a_ring = w.partial;
+        int a_slots = sq.ring_slots, a_stride = sq.slot_stride, a_nblk = (int)plan->n_adc_blocks;
+        int *a_tickets = reinterpret_cast<int *>(w.partial + sq.ticket_off);
+        const SeqAdcBlock *a_blk = reinterpret_cast<const SeqAdcBlock *>(plan->d_tables + plan->adcblk_off);
+        float2 *a_sig = per_spin ? nullptr : (float2 *)d_signal, *a_ps = per_spin ? (float2 *)d_signal : nullptr;
+        long long a_nadc = (long long)plan->info.n_adc;
+        int a_final = d_Mxy ? 1 : 0;
+        void *args[] = {&a_tables, &prog, &a_nops, &a_A, &a_C, &a_S, &a_n, &a_chunk, &a_rfw, &a_roles, &a_min, &a_scal,
+                        &a_ring, &a_slots, &a_stride, &a_tickets, &a_nblk, &a_blk, &a_sig, &a_nadc, &a_final, &a_ps};
+        if (per_spin) {
+            BLOCH_CUDA(cudaLaunchKernel((const void *)seq_kernel<true>, dim3(sq.n_ctas), dim3(sq.threads), args, sq.smem, stream));
+        } else {
+            // the CTAs wait for one another's tickets (integer counters) when they sum the partial rows, so all of them
+            // must be resident: a cooperative launch guarantees it (n_ctas <= SMs, one CTA per SM)
+            BLOCH_CUDA(cudaMemsetAsync(a_tickets, 0, size_t(2) * size_t(std::max(a_nblk, 1)) * sizeof(int), stream));
+            BLOCH_CUDA(cudaLaunchCooperativeKernel((const void *)seq_kernel<false>, dim3(sq.n_ctas), dim3(sq.threads), args,
+                                                   sq.smem, stream));
         }
+        ++launches;
         if (d_Mxy) {
             if ((rc = taps.mark(BLOCH_KIND_OTHER))) return rc;
             unpack_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, w.S, (float2 *)d_Mxy, d_Mz);

@@ -92,6 +92,15 @@ struct KernelNote {
     int block = 0;        // threads per CTA
 };
 
+// The ADC-bearing precession blocks in order (appended to the table buffer at bloch_plan::adcblk_off): what the fused
+// kernel's lagging sum over CTAs needs to know about a block it finished a few blocks ago.
+struct SeqAdcBlock {
+    int64_t adc_first;
+    int32_t n;
+    int32_t pad;
+};
+static_assert(sizeof(SeqAdcBlock) == 16, "SeqAdcBlock must be 16 B");
+
 struct Timing {
     float ms_rf = 0, ms_prec = 0, ms_total = 0;
     int64_t launches = 0;
@@ -107,6 +116,8 @@ struct bloch_plan {
     std::vector<unsigned char> tables;   // host staging copy of the device tables
     const unsigned char *d_tables = nullptr;
     int64_t prog_off = 0;                // byte offset of the SeqOp program in the table buffer
+    int64_t n_adc_blocks = 0;            // precession blocks that serve ADC samples
+    int64_t adcblk_off = 0;              // byte offset of the SeqAdcBlock array in the table buffer
     int path = 0;                        // BLOCH_PATH_*
     int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, 2, -1, 0};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
     // phase-range bookkeeping (bloch_sim_params extents): largest |k'| [turns/m], tau [s] and |mu'| [turns s/m] of

@@ -430,9 +430,20 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     // whole-sequence program for the fused kernel: one SeqOp per block
     const size_t prog_off = off;
     off = align_up(off + blocks.size() * sizeof(SeqOp), kAlign);
-    if (off == 0) off = kAlign;
+    const size_t adcblk_off = off;
+    {
+        size_t n_adc_blocks = 0;
+        for (const Block &b : blocks) n_adc_blocks += (b.type == kBlockPrecession && b.adc_count > 0) ? 1 : 0;
+        off = align_up(off + std::max<size_t>(n_adc_blocks, 1) * sizeof(SeqAdcBlock), kAlign);
+    }
     plan->tables.assign(off, 0);
     plan->prog_off = (int64_t)prog_off;
+    plan->adcblk_off = (int64_t)adcblk_off;
+    {
+        SeqAdcBlock *ab = reinterpret_cast<SeqAdcBlock *>(plan->tables.data() + adcblk_off);
+        for (const Block &b : blocks)
+            if (b.type == kBlockPrecession && b.adc_count > 0) *ab++ = SeqAdcBlock{b.adc_first, (int32_t)b.adc_count, 0};
+    }
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
         const Block &b = blocks[bi];
         SeqOp op;
@@ -488,6 +499,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     plan->gamma = gamma;
     plan->params = *params;
     plan->blocks = std::move(blocks);
+    plan->n_adc_blocks = 0;
+    for (const Block &b : plan->blocks) plan->n_adc_blocks += (b.type == kBlockPrecession && b.adc_count > 0) ? 1 : 0;
     plan->d_tables = nullptr;
     plan->k_max = k_max;
     plan->tau_max = tau_max;

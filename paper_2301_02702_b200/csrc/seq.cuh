@@ -14,8 +14,14 @@
 //                       shared array and carry straight on with the next pulse
 //   warps R+1 .. R+G    signal warps: for every published state evaluate the block's ADC samples (a6: a thread
 //                       owns P adjacent samples and walks the chunk's spins in shared memory, arithmetic as
-//                       signal_kernel) and write the CTA's partial sums P[cta][adc] (a7; reduce_kernel adds
-//                       the CTAs in index order -- still no float atomics, still bitwise reproducible).  The
+//                       signal_kernel) and write the CTA's partial sums of that block into a RING of partial rows
+//                       ring[block % R][cta][sample] (a7).  The sum over the CTAs is made inside the same launch,
+//                       a few blocks later: CTA c adds, in CTA order, rows 0 .. n_ctas-1 of ITS slice of
+//                       the block's samples and writes the signal -- no float atomics, a fixed order whatever the
+//                       timing, so still bitwise reproducible; integer tickets (arrive / reduced, one pair per block)
+//                       say when a block's rows are complete and when its ring slot may be written again.  The
+//                       signal warp that finishes a block last in its CTA raises the CTA's ticket and makes the
+//                       CTA's sum of the block kSeqReduceLag blocks back.  The
 //                       block's samples are cut into items of 32 x P samples which the warps take from a
 //                       shared counter, so a sub-partition that holds fewer RF warps serves more items; a
 //                       sample's sum is one thread's walk over the chunk in spin order whichever warp takes it
@@ -39,6 +45,17 @@ constexpr int kSeqTileStride = 4224;  // >= kRfHdrBytes + kRfTileSteps * 32 (sta
 constexpr int kSeqMaxThreads = 1024;
 constexpr int kSeqStateBufs = 4;
 constexpr int kSeqBarBytes = 256;
+// Partial-row ring: kSeqRingSlots blocks may lie between "partial row written" and "summed over the CTAs", and a CTA
+// sums its slice of block g - kSeqReduceLag when it has finished block g, so the CTAs may drift kSeqRingSlots -
+// kSeqReduceLag blocks apart before anyone waits for a ticket.  Measured alternatives (config 5 / config 2, against
+// 124.2 / 2.237 ms with one partial row per CTA over the whole sequence, summed by a second kernel): this layout 125.2 /
+// 2.217; tickets looked at every fourth block (2 blocks of drift) 127.0 / 2.254; 26 to 64 slots with a lag of a quarter
+// of them 127.0 / 2.334 (the last `lag` blocks are summed after the sequence's end: a tail short sequences feel); a
+// dedicated reducer warp polling every 200 ns 126.1 / 2.42, every 2 us 125.3 / 2.33, asleep on an mbarrier 128.5 /
+// 2.34; the roles as separate non-inlined functions 133.8 / 3.06 (spills under the 64-register cap).
+constexpr int kSeqReduceLag = 3;
+constexpr int kSeqRingSlots = 8;
+static_assert(kSeqRingSlots > kSeqReduceLag + 1, "ring too short");
 
 // Role of each warp of the CTA, chosen on the host (api.cu seq_shape) so that every SM sub-partition (warp id mod 4)
 // carries about the same load: >= 0: RF warp with that index (spins 32 i .. 32 i + 31 of the chunk), -1: producer,
@@ -55,7 +72,46 @@ static_assert(kSeqTileStride >= kRfHdrBytes + kRfTileSteps * 32 && kSeqTileStrid
 __host__ __device__ inline size_t seq_smem_bytes(int chunk) {
     return size_t(kSeqStages) * kSeqTileStride + kSeqBarBytes + size_t(1 + kSeqStateBufs) * chunk * sizeof(float4);
 }
-static_assert((2 * kSeqStages + 2 * kSeqStateBufs) * 8 + kSeqStateBufs * 4 <= kSeqBarBytes, "barrier area");
+static_assert((2 * kSeqStages + 2 * kSeqStateBufs) * 8 + 2 * kSeqStateBufs * 4 <= kSeqBarBytes, "barrier area");
+
+// cross-CTA tickets of the partial-row ring (integers only)
+__device__ __forceinline__ int ld_acquire_gpu(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void wait_ticket(const int *ctr, int target, int lane) {
+    if (lane == 0)
+        while (ld_acquire_gpu(ctr) < target) __nanosleep(200);
+    __syncwarp();
+}
+
+// One CTA's share of the sum over CTAs for one block: samples [cta n_pts / n_ctas, (cta + 1) n_pts / n_ctas) of the
+// block, rows added in CTA order (lane r takes rows r, r + 32, ...; fixed butterfly across lanes).
+__device__ __forceinline__ void seq_reduce_slice(const float2 *slot, int slot_stride, int n_ctas, int cta, int n_pts,
+                                                 float2 *__restrict__ sig, int lane, const int *arrive, int *reduced) {
+    wait_ticket(arrive, n_ctas, lane);  // every CTA's row of this block is written and visible
+    const int p_lo = (int)((long long)cta * n_pts / n_ctas), p_hi = (int)((long long)(cta + 1) * n_pts / n_ctas);
+    for (int p = p_lo; p < p_hi; ++p) {
+        float re = 0.f, im = 0.f;
+        for (int r = lane; r < n_ctas; r += 32) {
+            const float2 v = __ldcg(slot + (size_t)r * slot_stride + p);  // L2: the slot is rewritten by other SMs
+            re += v.x;
+            im += v.y;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            re += __shfl_xor_sync(0xffffffffu, re, o);
+            im += __shfl_xor_sync(0xffffffffu, im, o);
+        }
+        if (lane == 0) sig[p] = make_float2(re, im);
+    }
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence();  // this CTA's reads of the slot are done before the slot is declared free
+        atomicAdd(reduced, 1);
+    }
+}
 
 // One item (32 x P adjacent ADC samples starting at `base`) of a precession block for the chunk's spins.
 template <int P>
@@ -148,7 +204,11 @@ template <bool PS>
 __global__ void __launch_bounds__(kSeqMaxThreads, 1)
 seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ ops, int n_ops,
            const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n, int chunk,
-           int rf_warps, SeqRoles roles, int min_items, const float *__restrict__ scal, float2 *__restrict__ partial,
+           int rf_warps, SeqRoles roles, int min_items, const float *__restrict__ scal,
+           float2 *__restrict__ prow /* [ring_slots][n_ctas][slot_stride] partial rows */, int ring_slots, int slot_stride,
+           int *__restrict__ tickets /* [2][n_adc_blocks]: arrive, reduced; zeroed before the launch */, int n_adc_blocks,
+           const SeqAdcBlock *__restrict__ adc_blocks /* [n_adc_blocks] */,
+           float2 *__restrict__ sig /* SUM_ALL: signal[n_adc] */,
            long long n_adc, int final_state, float2 *__restrict__ out_ps /* PER_SPIN plans: out[spin][adc], else NULL */) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *ring = smem;
@@ -156,6 +216,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
     uint64_t *tile_full = bars, *tile_empty = bars + kSeqStages, *st_full = bars + 2 * kSeqStages,
              *st_empty = bars + 2 * kSeqStages + kSeqStateBufs;
     int *item_ctr = reinterpret_cast<int *>(bars + 2 * kSeqStages + 2 * kSeqStateBufs);  // [kSeqStateBufs]
+    int *fin_ctr = item_ctr + kSeqStateBufs;  // [kSeqStateBufs]: signal warps that have finished the block
     float4 *shA = reinterpret_cast<float4 *>(smem + kSeqStages * kSeqTileStride + kSeqBarBytes);
     float4 *shS = shA + chunk;  // [kSeqStateBufs][chunk]
     const int tid = threadIdx.x, warp = tid >> 5;
@@ -173,6 +234,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             mbar_init(&st_full[k], n_rf_thr);
             mbar_init(&st_empty[k], max(nsig, 1));
             item_ctr[k] = 0;
+            fin_ctr[k] = 0;
         }
         mbar_init_fence();
     }
@@ -277,7 +339,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                     const int b = pub % kSeqStateBufs, use = pub / kSeqStateBufs;
                     if (use > 0) mbar_wait(&st_empty[b], (uint32_t)((use - 1) & 1));
                     if (active) shS[b * chunk + r] = make_float4(hx, hy, hz, s.w);
-                    if (r == 0) item_ctr[b] = 0;  // every signal warp is past its last atomicAdd of the previous use
+                    if (r == 0) { item_ctr[b] = 0; fin_ctr[b] = 0; }  // every signal warp is past its last atomicAdd of the previous use
                     mbar_arrive(&st_full[b]);
                     ++pub;
                 }
@@ -297,13 +359,17 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
     {
         const int lane = tid & 31;
         const float r2max_log2e = scal[0] * kLog2e;
-        float2 *row = partial + (size_t)blockIdx.x * (size_t)n_adc;
-        int pub = 0;
+        const int n_ctas = gridDim.x, cta = blockIdx.x;
+        int *arrive = tickets, *reduced = tickets + n_adc_blocks;
+        const size_t slot_elems = (size_t)n_ctas * slot_stride;
+        int pub = 0;  // = index of the block among the ADC-bearing precession blocks (adc_blocks[pub])
         for (int oi = 0; oi < n_ops; ++oi) {
             const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
             if (tn.x != kBlockPrecession || tn.y == 0) continue;
             const float4 *recs = reinterpret_cast<const float4 *>(tables + ops[oi].table_off);
-            float2 *out = row + ops[oi].adc_first;
+            // the ring slot is free once every CTA has summed its slice of the block that used it before
+            if (pub >= ring_slots) wait_ticket(&reduced[pub - ring_slots], n_ctas, lane);
+            float2 *out = prow + (size_t)(pub % ring_slots) * slot_elems + (size_t)cta * slot_stride;
             const int b = pub % kSeqStateBufs;
             mbar_wait(&st_full[b], (uint32_t)((pub / kSeqStateBufs) & 1));
             const float4 *stS = shS + b * chunk;
@@ -311,7 +377,28 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else if (tn.y >= 64 * min_items) seq_signal_block<2>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else seq_signal_block<1>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            // the warp that finishes the block last in this CTA announces the CTA's row and takes the CTA's reduce duty
+            __syncwarp();
+            int last = 0;
+            if (lane == 0) {
+                __threadfence();  // this warp's partial sums are visible before it counts itself done
+                last = atomicAdd(&fin_ctr[b], 1) == roles.n_sig_warps - 1;
+            }
+            last = __shfl_sync(0xffffffffu, last, 0);
             mbar_arrive(&st_empty[b]);
+            if (last) {
+                if (lane == 0) {
+                    __threadfence();
+                    atomicAdd(&arrive[pub], 1);
+                }
+                // this CTA's slice of the block finished kSeqReduceLag blocks ago; after the last block, of the rest too
+                const int h_hi = pub == n_adc_blocks - 1 ? pub : pub - kSeqReduceLag;
+                for (int h = max(pub - kSeqReduceLag, 0); h <= h_hi; ++h) {
+                    const SeqAdcBlock ab = adc_blocks[h];
+                    seq_reduce_slice(prow + (size_t)(h % ring_slots) * slot_elems, slot_stride, n_ctas, cta, ab.n,
+                                     sig + ab.adc_first, lane, &arrive[h], &reduced[h]);
+                }
+            }
             ++pub;
         }
     }
