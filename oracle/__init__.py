@@ -41,10 +41,14 @@ def _load():
                                             [dp, dp, C.c_int, dp, C.c_int, C.c_int, C.c_int])
         _lib.bloch_ref_simulate_motion.restype = C.c_int
         _lib.bloch_ref_simulate_motion.argtypes = (_lib.bloch_ref_simulate.argtypes + [C.c_double, dp, dp, dp])
+        _lib.bloch_ref_simulate_waveform.restype = C.c_int
+        _lib.bloch_ref_simulate_waveform.argtypes = (_lib.bloch_ref_simulate_motion.argtypes + [dp, dp, i64])
         _lib.bloch_ref_grid.restype = i64
         _lib.bloch_ref_grid.argtypes = seq_args + [dp, dp, C.POINTER(C.c_uint8), C.POINTER(i64)]
         _lib.bloch_ref_grid_motion.restype = i64
         _lib.bloch_ref_grid_motion.argtypes = _lib.bloch_ref_grid.argtypes + [C.c_double]
+        _lib.bloch_ref_grid_waveform.restype = i64
+        _lib.bloch_ref_grid_waveform.argtypes = _lib.bloch_ref_grid_motion.argtypes + [dp, dp, i64, dp]
     return _lib
 
 
@@ -69,13 +73,16 @@ def _seq_args(seq, keep):
 
 def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state: bool = False,
              n_threads: int | None = None, gamma: float = GAMMA, force_excitation: bool = False,
-             velocity=None, dt_max: float = 0.0, group_size: int = 0, coils=None):
+             velocity=None, dt_max: float = 0.0, group_size: int = 0, coils=None, waveform=None):
     """Step-by-step fp64 Bloch integration (SURVEY.md 8(c) listing).
 
     phantom: object with fp64 arrays x, y, z, M0, T1, T2, dw.   seq: object with g_t, g_v (3 arrays each),
     rf_t, rf_dt, rf_re, rf_im, adc_t, t_end, dt_rf_max.
     velocity: optional (vx, vy, vz) fp64 arrays [m/s]: every spin moves as x(t) = x + v t (PAPER.md:96, :236);
     dt_max then refines every interval to at most dt_max (:180).
+    waveform: optional (t, u) vertex arrays of a shared piecewise-linear motion waveform: every spin then moves as
+    x(t) = x + velocity * u(t) (velocity = per-spin amplitude vectors; u held at its end values outside the vertices,
+    which join the time grid); without it u(t) = t (reading M2; "motion field u(x, t)").
     Returns complex128 signal [n_adc] ("sum") or [n_spins, n_adc] ("per_spin"); with return_state also
     (Mxy complex128 [n_spins], Mz float64 [n_spins]).
     coils: optional complex [n_coils, n_spins] receive sensitivities at the spins (output_mode "sum" only):
@@ -93,7 +100,7 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
             raise ValueError("coils must be [n_coils, n_spins]")
         res = simulate(phantom, seq, output_mode="per_spin", state=state, return_state=return_state,
                        n_threads=n_threads, gamma=gamma, force_excitation=force_excitation, velocity=velocity,
-                       dt_max=dt_max)
+                       dt_max=dt_max, waveform=waveform)
         per = res[0] if return_state else res
         out = Wc @ per
         return (out,) + tuple(res[1:]) if return_state else out
@@ -106,7 +113,7 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
             raise ValueError("group_size must be positive and divide the number of spins")
         res = simulate(phantom, seq, output_mode="per_spin", state=state, return_state=return_state,
                        n_threads=n_threads, gamma=gamma, force_excitation=force_excitation, velocity=velocity,
-                       dt_max=dt_max)
+                       dt_max=dt_max, waveform=waveform)
         per = res[0] if return_state else res
         grouped = per.reshape(n_all // group_size, group_size, per.shape[1]).sum(axis=1)
         return (grouped,) + tuple(res[1:]) if return_state else grouped
@@ -135,6 +142,8 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     common = [C.c_double(gamma), *sargs, C.c_int64(n), *pa, mxy.ctypes.data_as(dp), mz.ctypes.data_as(dp),
               C.c_int(use_state), sig.ctypes.data_as(dp), C.c_int(mode), C.c_int(int(n_threads)),
               C.c_int(1 if force_excitation else 0)]
+    if waveform is not None and velocity is None:
+        raise ValueError("a motion waveform needs per-spin amplitudes (velocity=)")
     if velocity is None and not dt_max:
         rc = lib.bloch_ref_simulate(*common)
     else:
@@ -144,7 +153,15 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
                 a, pk = _d(np.broadcast_to(np.asarray(velocity[k], dtype=np.float64), (n,)))
                 keep.append(a)
                 va[k] = pk
-        rc = lib.bloch_ref_simulate_motion(*common, C.c_double(float(dt_max)), *va)
+        if waveform is None:
+            rc = lib.bloch_ref_simulate_motion(*common, C.c_double(float(dt_max)), *va)
+        else:
+            wt, wtp = _d(waveform[0]); wu, wup = _d(waveform[1])
+            if wt.shape != wu.shape or wt.ndim != 1 or wt.shape[0] < 1:
+                raise ValueError("waveform must be two equally long 1-D arrays (t, u)")
+            keep += [wt, wu]
+            rc = lib.bloch_ref_simulate_waveform(*common, C.c_double(float(dt_max)), *va, wtp, wup,
+                                                 C.c_int64(wt.shape[0]))
     if rc != 0:
         raise ValueError(f"bloch_ref_simulate failed with code {rc}")
     if return_state:
@@ -152,20 +169,26 @@ def simulate(phantom, seq, *, output_mode: str = "sum", state=None, return_state
     return sig
 
 
-def grid(seq, dt_max: float = 0.0):
-    """The oracle's own discretisation: (t[n+1], G[n+1,3], rf[n] uint8, adc[n+1] int64)."""
+def grid(seq, dt_max: float = 0.0, waveform=None):
+    """The oracle's own discretisation: (t[n+1], G[n+1,3], rf[n] uint8, adc[n+1] int64); with a motion waveform
+    (t, u) its vertices are points of the grid."""
     lib = _load()
     keep = []
     sargs, _ = _seq_args(seq, keep)
     null_d = C.POINTER(C.c_double)()
-    n = lib.bloch_ref_grid_motion(*sargs, null_d, null_d, C.POINTER(C.c_uint8)(), C.POINTER(C.c_int64)(),
-                                  C.c_double(float(dt_max)))
+    wargs = [null_d, null_d, C.c_int64(0), null_d]
+    if waveform is not None:
+        wt, wtp = _d(waveform[0]); wu, wup = _d(waveform[1])
+        keep += [wt, wu]
+        wargs = [wtp, wup, C.c_int64(wt.shape[0]), null_d]
+    n = lib.bloch_ref_grid_waveform(*sargs, null_d, null_d, C.POINTER(C.c_uint8)(), C.POINTER(C.c_int64)(),
+                                    C.c_double(float(dt_max)), *wargs)
     if n < 0:
         raise ValueError(f"bloch_ref_grid failed with code {n}")
     t = np.zeros(n + 1); G = np.zeros((n + 1, 3)); rf = np.zeros(max(n, 1), dtype=np.uint8)
     adc = np.zeros(n + 1, dtype=np.int64)
     dp = C.POINTER(C.c_double)
-    lib.bloch_ref_grid_motion(*sargs, t.ctypes.data_as(dp), G.ctypes.data_as(dp),
-                              rf.ctypes.data_as(C.POINTER(C.c_uint8)), adc.ctypes.data_as(C.POINTER(C.c_int64)),
-                              C.c_double(float(dt_max)))
+    lib.bloch_ref_grid_waveform(*sargs, t.ctypes.data_as(dp), G.ctypes.data_as(dp),
+                                rf.ctypes.data_as(C.POINTER(C.c_uint8)), adc.ctypes.data_as(C.POINTER(C.c_int64)),
+                                C.c_double(float(dt_max)), *wargs)
     return t, G, rf[:n], adc

@@ -21,6 +21,11 @@
  * and takes the trapezoid of Eq (12)-(13) on Bz(t_n) = G(t_n) . x(t_n); dt_max adds the intermediate points.  Pins M1-M5:
  * tests/test_oracle_motion_pins.py (closed-form phase under constant G, bipolar velocity encoding, O(dt^2)
  * convergence on a ramp, regime consistency).
+ * General motion ("motion field u(x, t)"; reading M2): bloch_ref_simulate_waveform moves every spin
+ * as x(t) = x + a u(t), a per-spin amplitude vector, u(t) a shared piecewise-linear waveform given by vertices (held at
+ * its end values outside them; the vertices join the time grid).  u(t) = t is the constant-velocity case.  Pins W1-W5
+ * in the same test file (closed forms under constant G for sinusoidal and stop-and-go u, reduction to x + v t,
+ * displacement-only phase, O(dt^2) convergence under a ramp).
  *
  * Pins (tests/test_oracle_pins.py): closed forms P1-P10 of SURVEY.md 8(c); no value printed by the paper
  * exists for this path, so "against the paper's own numbers" the parity is unpinned (stated in DESIGN.md).
@@ -46,6 +51,7 @@ typedef struct {
     double *b1im;     /* n */
     uint8_t *rf;      /* n : 1 if the interval is covered by an RF sample (reading G18) */
     int64_t *adc;     /* n+1 : ADC sample index recorded at point n, or -1 */
+    double *u;        /* n+1 : motion waveform u(t_n) (x(t) = x + a u(t)); u(t) = t without a waveform */
 } ref_grid;
 
 static int cmp_double(const void *a, const void *b) {
@@ -83,8 +89,22 @@ static int64_t rf_cover(const double *rf_t, const double *rf_dt, int64_t rf_n, d
     return -1;
 }
 
+/* motion waveform u at time t: linear interpolation of the vertices, held at the end values outside them */
+static double interp_waveform(const double *mt, const double *mu, int64_t n, double t) {
+    if (n <= 0) return t;
+    if (t <= mt[0]) return mu[0];
+    if (t >= mt[n - 1]) return mu[n - 1];
+    int64_t lo = 0, hi = n - 1;
+    while (hi - lo > 1) {
+        int64_t mid = (lo + hi) / 2;
+        if (mt[mid] <= t) lo = mid; else hi = mid;
+    }
+    double w = (t - mt[lo]) / (mt[hi] - mt[lo]);
+    return mu[lo] + w * (mu[hi] - mu[lo]);
+}
+
 static void grid_free(ref_grid *g) {
-    free(g->t); free(g->G); free(g->b1re); free(g->b1im); free(g->rf); free(g->adc);
+    free(g->t); free(g->G); free(g->b1re); free(g->b1im); free(g->rf); free(g->adc); free(g->u);
     memset(g, 0, sizeof(*g));
 }
 
@@ -110,10 +130,11 @@ static int grid_build(ref_grid *g,
                       const double *const gt[3], const double *const gv[3], const int64_t gn[3],
                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
                       int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
-                      double dt_max) {
+                      double dt_max, const double *mo_t, const double *mo_u, int64_t mo_n) {
     memset(g, 0, sizeof(*g));
     if (!(t_end > 0.0)) return -1;
-    int64_t cap = 2 + gn[0] + gn[1] + gn[2] + 2 * rf_n + adc_n;
+    for (int64_t i = 1; i < mo_n; ++i) if (!(mo_t[i] > mo_t[i - 1])) return -6;
+    int64_t cap = 2 + gn[0] + gn[1] + gn[2] + 2 * rf_n + adc_n + (mo_n > 0 ? mo_n : 0);
     double *raw = (double *)malloc(sizeof(double) * (size_t)cap);
     if (!raw) return -2;
     int64_t m = 0;
@@ -123,6 +144,8 @@ static int grid_build(ref_grid *g,
         for (int64_t i = 0; i < gn[a]; ++i) raw[m++] = gt[a][i];
     for (int64_t i = 0; i < rf_n; ++i) { raw[m++] = rf_t[i]; raw[m++] = rf_t[i] + rf_dt[i]; }
     for (int64_t i = 0; i < adc_n; ++i) raw[m++] = adc_t[i];
+    /* the vertices of the motion waveform are points of the grid (those inside the sequence) */
+    for (int64_t i = 0; i < mo_n; ++i) if (mo_t[i] >= 0.0 && mo_t[i] <= t_end) raw[m++] = mo_t[i];
     qsort(raw, (size_t)m, sizeof(double), cmp_double);
     /* unique with tolerance, clipped to [0, t_end] */
     int64_t u = 0;
@@ -145,7 +168,8 @@ static int grid_build(ref_grid *g,
     g->b1im = (double *)calloc((size_t)total, sizeof(double));
     g->rf = (uint8_t *)calloc((size_t)total, 1);
     g->adc = (int64_t *)malloc(sizeof(int64_t) * (size_t)total);
-    if (!g->t || !g->G || !g->b1re || !g->b1im || !g->rf || !g->adc) { free(raw); grid_free(g); return -2; }
+    g->u = (double *)malloc(sizeof(double) * (size_t)total);
+    if (!g->t || !g->G || !g->b1re || !g->b1im || !g->rf || !g->adc || !g->u) { free(raw); grid_free(g); return -2; }
     int64_t k = 0;
     g->t[k++] = raw[0];
     for (int64_t i = 0; i + 1 < u; ++i) {
@@ -157,6 +181,7 @@ static int grid_build(ref_grid *g,
     free(raw);
     for (int64_t n = 0; n <= g->n; ++n) {
         for (int a = 0; a < 3; ++a) g->G[3 * n + a] = interp_axis(gt[a], gv[a], gn[a], g->t[n]);
+        g->u[n] = interp_waveform(mo_t, mo_u, mo_n, g->t[n]);
         g->adc[n] = -1;
     }
     for (int64_t n = 0; n < g->n; ++n) {
@@ -193,9 +218,10 @@ static void integrate_spin(const ref_grid *g, double gamma, double x, double y, 
         double Gz = 0.5 * (g->G[3 * n + 2] + g->G[3 * n + 5]);
         double Bz = Gx * x + Gy * y + Gz * z + dw / gamma;                 /* Eq (2) */
         if (vel) {
-            /* motion x(t) = x + v t: the trapezoid of Eq (12)-(13) is taken on the
-             * effective field itself, Bz(t_n) = G(t_n) . x(t_n), at the two ends of the interval (:180, :336) */
-            double t0 = g->t[n], t1 = g->t[n + 1];
+            /* motion x(t) = x + v u(t), u(t) = t for a constant velocity: the trapezoid of
+             * Eq (12)-(13) is taken on the effective field itself, Bz(t_n) = G(t_n) . x(t_n), at the two ends of the
+             * interval (:180, :336) */
+            double t0 = g->u[n], t1 = g->u[n + 1];
             double b0 = g->G[3 * n + 0] * (x + vel[0] * t0) + g->G[3 * n + 1] * (y + vel[1] * t0)
                         + g->G[3 * n + 2] * (z + vel[2] * t0);
             double b1 = g->G[3 * n + 3] * (x + vel[0] * t1) + g->G[3 * n + 4] * (y + vel[1] * t1)
@@ -249,7 +275,7 @@ static void integrate_spin(const ref_grid *g, double gamma, double x, double y, 
  *   flags        bit 0: force every interval through the excitation branch (invariant I5 only)
  *   returns 0, or <0 on invalid input.
  */
-int bloch_ref_simulate_motion(double gamma,
+int bloch_ref_simulate_waveform(double gamma,
                        const double *gx_t, const double *gx_v, int64_t gx_n,
                        const double *gy_t, const double *gy_v, int64_t gy_n,
                        const double *gz_t, const double *gz_v, int64_t gz_n,
@@ -259,12 +285,14 @@ int bloch_ref_simulate_motion(double gamma,
                        const double *M0, const double *T1, const double *T2, const double *dw,
                        double *Mxy, double *Mz, int use_state,
                        double *signal, int output_mode, int n_threads, int flags,
-                       double dt_max, const double *vx, const double *vy, const double *vz) {
+                       double dt_max, const double *vx, const double *vy, const double *vz,
+                       const double *mo_t, const double *mo_u, int64_t mo_n) {
     const double *const gt[3] = {gx_t, gy_t, gz_t};
     const double *const gv[3] = {gx_v, gy_v, gz_v};
     const int64_t gn[3] = {gx_n, gy_n, gz_n};
     ref_grid g;
-    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max);
+    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max,
+                        mo_t, mo_u, mo_n);
     if (rc) return rc;
     const int moving = vx && vy && vz;
     int nth = n_threads > 0 ? n_threads : 1;
@@ -321,6 +349,24 @@ int bloch_ref_simulate_motion(double gamma,
     return 0;
 }
 
+/* Constant velocities: x(t) = x + v t, i.e. the waveform entry with u(t) = t. */
+int bloch_ref_simulate_motion(double gamma,
+                       const double *gx_t, const double *gx_v, int64_t gx_n,
+                       const double *gy_t, const double *gy_v, int64_t gy_n,
+                       const double *gz_t, const double *gz_v, int64_t gz_n,
+                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
+                       int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
+                       int64_t n_spins, const double *x, const double *y, const double *z,
+                       const double *M0, const double *T1, const double *T2, const double *dw,
+                       double *Mxy, double *Mz, int use_state,
+                       double *signal, int output_mode, int n_threads, int flags,
+                       double dt_max, const double *vx, const double *vy, const double *vz) {
+    return bloch_ref_simulate_waveform(gamma, gx_t, gx_v, gx_n, gy_t, gy_v, gy_n, gz_t, gz_v, gz_n, rf_t, rf_dt, rf_re,
+                                       rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, n_spins, x, y, z, M0, T1, T2, dw,
+                                       Mxy, Mz, use_state, signal, output_mode, n_threads, flags, dt_max, vx, vy, vz,
+                                       NULL, NULL, 0);
+}
+
 /* The static-phantom entry: no motion, no dt_max refinement. */
 int bloch_ref_simulate(double gamma,
                        const double *gx_t, const double *gx_v, int64_t gx_n,
@@ -342,17 +388,19 @@ int bloch_ref_simulate(double gamma,
  * Call with t_out == NULL to get the number of intervals; otherwise fills t_out[n+1], G_out[3(n+1)],
  * rf_out[n], adc_out[n+1] (caller-allocated).  Returns n (>= 0) or <0 on error.
  */
-int64_t bloch_ref_grid_motion(const double *gx_t, const double *gx_v, int64_t gx_n,
+int64_t bloch_ref_grid_waveform(const double *gx_t, const double *gx_v, int64_t gx_n,
                        const double *gy_t, const double *gy_v, int64_t gy_n,
                        const double *gz_t, const double *gz_v, int64_t gz_n,
                        const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
                        int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
-                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out, double dt_max) {
+                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out, double dt_max,
+                       const double *mo_t, const double *mo_u, int64_t mo_n, double *u_out) {
     const double *const gt[3] = {gx_t, gy_t, gz_t};
     const double *const gv[3] = {gx_v, gy_v, gz_v};
     const int64_t gn[3] = {gx_n, gy_n, gz_n};
     ref_grid g;
-    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max);
+    int rc = grid_build(&g, gt, gv, gn, rf_t, rf_dt, rf_re, rf_im, rf_n, adc_t, adc_n, t_end, dt_rf_max, dt_max,
+                        mo_t, mo_u, mo_n);
     if (rc) return rc;
     int64_t n = g.n;
     if (t_out) {
@@ -360,9 +408,20 @@ int64_t bloch_ref_grid_motion(const double *gx_t, const double *gx_v, int64_t gx
         if (G_out) memcpy(G_out, g.G, sizeof(double) * 3 * (size_t)(n + 1));
         if (rf_out) memcpy(rf_out, g.rf, (size_t)n);
         if (adc_out) memcpy(adc_out, g.adc, sizeof(int64_t) * (size_t)(n + 1));
+        if (u_out) memcpy(u_out, g.u, sizeof(double) * (size_t)(n + 1));
     }
     grid_free(&g);
     return n;
+}
+
+int64_t bloch_ref_grid_motion(const double *gx_t, const double *gx_v, int64_t gx_n,
+                       const double *gy_t, const double *gy_v, int64_t gy_n,
+                       const double *gz_t, const double *gz_v, int64_t gz_n,
+                       const double *rf_t, const double *rf_dt, const double *rf_re, const double *rf_im,
+                       int64_t rf_n, const double *adc_t, int64_t adc_n, double t_end, double dt_rf_max,
+                       double *t_out, double *G_out, uint8_t *rf_out, int64_t *adc_out, double dt_max) {
+    return bloch_ref_grid_waveform(gx_t, gx_v, gx_n, gy_t, gy_v, gy_n, gz_t, gz_v, gz_n, rf_t, rf_dt, rf_re, rf_im, rf_n,
+                                   adc_t, adc_n, t_end, dt_rf_max, t_out, G_out, rf_out, adc_out, dt_max, NULL, NULL, 0, NULL);
 }
 
 int64_t bloch_ref_grid(const double *gx_t, const double *gx_v, int64_t gx_n,
