@@ -216,7 +216,7 @@ def time_oracle(w, n_intervals: int, budget_spin_steps: float):
     t0 = time.perf_counter()
     if coils is None:
         oracle.simulate(ph, w.seq, output_mode=w.output_mode, n_threads=cores, velocity=vel, dt_max=w.dt_max,
-                        group_size=w.group_size)
+                        group_size=w.group_size, waveform=w.waveform)
     else:
         # the oracle's coil path holds the per-spin signals [spins, n_adc] in memory: feed it batches of spins
         # (spins are independent, the coil signals add) so that the batch stays below ~1 GB
@@ -237,7 +237,7 @@ def run_reference(args, rank, world):
         return
     import oracle
     w, _ = make_workload(args.workload, 0, 1, "weak")
-    t, _, _, _ = oracle.grid(w.seq, dt_max=w.dt_max if w.velocity is not None else 0.0)
+    t, _, _, _ = oracle.grid(w.seq, dt_max=w.dt_max if w.velocity is not None else 0.0, waveform=w.waveform)
     n_int = len(t) - 1
     cores = os.cpu_count() or 1
     # size a step at ~3 s of CPU work from a short probe
@@ -565,7 +565,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary)")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 3w (3 with periodic non-rigid motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary)")
     ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
                     help="execution path (bloch_plan_set_path); auto = the library's choice")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],

@@ -44,7 +44,7 @@ typedef enum {
 
 enum { BLOCH_PHASE_AUTO = 0, BLOCH_PHASE_FP32 = 1, BLOCH_PHASE_FP64 = 2 };
 enum { BLOCH_OUT_SUM_ALL = 0, BLOCH_OUT_PER_SPIN = 1, BLOCH_OUT_GROUPED = 2 };
-enum { BLOCH_MOTION_NONE = 0, BLOCH_MOTION_LINEAR = 1 };
+enum { BLOCH_MOTION_NONE = 0, BLOCH_MOTION_LINEAR = 1, BLOCH_MOTION_WAVEFORM = 2 };
 
 /* Scanner.  Only gamma enters the arithmetic (Eq 1-2, :105-114); B0, G_max, S_max are
  * limits: when G_max [T/m] or S_max [T/m/s] is > 0, bloch_plan_create checks every gradient vertex and every
@@ -79,7 +79,15 @@ typedef struct {
  * equal sub-steps (the paper's "intermediate points in the case of motion", :180); ignored without motion
  * or when <= 0 / inf.  motion_mode: BLOCH_MOTION_LINEAR builds the first-moment tables that let every spin
  * move as x(t) = x + v t (PAPER.md:96 motion field, :236 experiment (d)); velocities are given to
- * bloch_simulate_motion.  max_block_points: precession blocks hold at most
+ * bloch_simulate_motion.  BLOCH_MOTION_WAVEFORM is the general form x(t) = x + a u(t) ("motion field
+ * u(x, t)"; reading M2): u is ONE piecewise-linear waveform shared by all spins, given here by its vertices
+ * (motion_t strictly ascending [s], motion_u [any unit], motion_n >= 1; HOST arrays borrowed for the duration of
+ * bloch_plan_create; u keeps its end values outside the vertices, and the vertices inside [0, t_end] join the time
+ * grid), and a is the per-spin amplitude vector [m per unit of u] passed to bloch_simulate_motion in place of the
+ * velocities -- periodic (cardiac, respiratory) displacement, stop-and-go, pulsatile flow; u(t) = t is MOTION_LINEAR.
+ * The effective field is sampled at the interval ends and integrated by the paper's trapezoid on the dt_max-refined
+ * grid either way, so one more spin-independent table (the moment of G u) serves every spin.
+ * max_block_points: precession blocks hold at most
  * this many evaluated points (the paper's Nblocks memory bound, :171); <= 0 selects the default. */
 typedef struct {
     double dt_max;
@@ -100,7 +108,10 @@ typedef struct {
      * A plan forced to BLOCH_PHASE_FP32 is not checked: the caller has taken the phase precision on. */
     double max_extent_m;   /* largest |x| (Euclidean norm) of any spin [m] */
     double max_offres_hz;  /* largest |dw| / 2 pi [Hz] */
-    double max_speed_mps;  /* largest |v| [m/s] (motion plans) */
+    double max_speed_mps;  /* largest |v| [m/s] (MOTION_LINEAR) or amplitude |a| [m per unit of u] (MOTION_WAVEFORM) */
+    const double *motion_t;  /* BLOCH_MOTION_WAVEFORM: vertex times of u(t), strictly ascending; else ignored */
+    const double *motion_u;  /*                        vertex values */
+    int64_t motion_n;
 } bloch_sim_params;
 
 typedef struct {
@@ -170,7 +181,8 @@ int bloch_simulate(const bloch_plan *plan, int64_t n_spins,
 
 /* bloch_simulate for a moving phantom: spin i is at x_i + v_i t at sequence time t.
  * d_vx, d_vy, d_vz: fp32 device arrays [m/s] of n_spins each; the plan must have been created with
- * motion_mode = BLOCH_MOTION_LINEAR (else BLOCH_EINVAL).  All three NULL = bloch_simulate.  The effective
+ * motion_mode = BLOCH_MOTION_LINEAR or BLOCH_MOTION_WAVEFORM (else BLOCH_EINVAL); with a waveform plan they hold the
+ * amplitude vectors a_i of x_i(t) = x_i + a_i u(t) [m per unit of u].  All three NULL = bloch_simulate.  The effective
  * field is sampled at the ends of every interval of the dt_max-refined grid and integrated by the trapezoidal
  * rule exactly as the paper prescribes (:180, :336); because x(t) is linear in t this needs only one more
  * spin-independent table, the first moment sum of (G_n t_n + G_{n+1} t_{n+1}) dt_n / 2. */

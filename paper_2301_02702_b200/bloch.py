@@ -18,8 +18,8 @@ PHASE_AUTO, PHASE_FP32, PHASE_FP64 = 0, 1, 2
 OUT_SUM_ALL, OUT_PER_SPIN, OUT_GROUPED = 0, 1, 2
 _PHASE = {"auto": PHASE_AUTO, "fp32": PHASE_FP32, "fp64": PHASE_FP64}
 _OUT = {"sum": OUT_SUM_ALL, "per_spin": OUT_PER_SPIN, "grouped": OUT_GROUPED}
-MOTION_NONE, MOTION_LINEAR = 0, 1
-_MOTION = {"none": MOTION_NONE, "linear": MOTION_LINEAR}
+MOTION_NONE, MOTION_LINEAR, MOTION_WAVEFORM = 0, 1, 2
+_MOTION = {"none": MOTION_NONE, "linear": MOTION_LINEAR, "waveform": MOTION_WAVEFORM}
 
 _dp = C.POINTER(C.c_double)
 _fp = C.c_void_p  # float* (host or device) passed as an address
@@ -39,7 +39,7 @@ class bloch_sim_params(C.Structure):
     _fields_ = [("dt_max", C.c_double), ("dt_rf_max", C.c_double), ("max_block_points", C.c_int64),
                 ("phase_mode", C.c_int32), ("output_mode", C.c_int32), ("motion_mode", C.c_int32),
                 ("group_size", C.c_int32), ("max_extent_m", C.c_double), ("max_offres_hz", C.c_double),
-                ("max_speed_mps", C.c_double)]
+                ("max_speed_mps", C.c_double), ("motion_t", _dp), ("motion_u", _dp), ("motion_n", C.c_int64)]
 
 
 class bloch_plan_info(C.Structure):
@@ -146,9 +146,11 @@ def _darr(a):
 def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
                       max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
                       group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0,
-                      max_extent_m: float = 0.0, max_offres_hz: float = 0.0, max_speed_mps: float = 0.0) -> int:
+                      max_extent_m: float = 0.0, max_offres_hz: float = 0.0, max_speed_mps: float = 0.0,
+                      waveform=None) -> int:
     """G_max [T/m], S_max [T/m/s]: scanner limits the gradient waveforms are checked against when > 0.
     max_extent_m / max_offres_hz / max_speed_mps: extents of the phantoms the plan will see (bloch_sim_params).
+    waveform: (t, u) vertex arrays of the shared motion waveform for motion="waveform" (x(t) = x + a u(t)).
     seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
     Returns the opaque plan handle (an integer address)."""
     keep = []
@@ -174,6 +176,12 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     mm = _MOTION[motion] if isinstance(motion, str) else int(motion)
     sp = bloch_sim_params(float(dt_max), float(dt_rf_max), int(max_block_points), pm, om, mm, int(group_size),
                           float(max_extent_m), float(max_offres_hz), float(max_speed_mps))
+    if waveform is not None:
+        wt, sp.motion_t = _darr(waveform[0]); wu, sp.motion_u = _darr(waveform[1])
+        if wt.shape != wu.shape or wt.ndim != 1:
+            raise ValueError("waveform must be two equally long 1-D arrays (t, u)")
+        keep += [wt, wu]
+        sp.motion_n = wt.shape[0]
     h = C.c_void_p()
     _check(_lib.bloch_plan_create(C.byref(sc), C.byref(cs), C.byref(sp), C.byref(h)))
     return h.value

@@ -116,7 +116,7 @@ SigShape sig_shape(const bloch_plan *plan, int64_t n_pts, int64_t n_spins, int s
 }
 
 int sig_max_P(const bloch_plan *plan) {
-    return (plan->info.phase_mode == BLOCH_PHASE_FP64 && plan->info.motion_mode == BLOCH_MOTION_LINEAR) ? 4 : 8;
+    return (plan->info.phase_mode == BLOCH_PHASE_FP64 && plan->info.motion_mode != BLOCH_MOTION_NONE) ? 4 : 8;
 }
 
 // Launch shape of a precession block: blocks that go to signal_lin_kernel (Block::lin_pts) are chunked as P = 8 blocks
@@ -339,7 +339,7 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.C = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.S = (float4 *)take(size_t(n_spins) * sizeof(float4));
     w.Ad = plan->info.phase_mode == BLOCH_PHASE_FP64 ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
-    const bool mo = plan->info.motion_mode == BLOCH_MOTION_LINEAR;
+    const bool mo = plan->info.motion_mode != BLOCH_MOTION_NONE;
     w.V = mo ? (float4 *)take(size_t(n_spins) * sizeof(float4)) : nullptr;
     w.Vd = (mo && plan->info.phase_mode == BLOCH_PHASE_FP64) ? (double4 *)take(size_t(n_spins) * sizeof(double4)) : nullptr;
     w.scal = (unsigned *)take(kAlign);
@@ -666,9 +666,9 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
     const bool has_v = d_vx || d_vy || d_vz;
     if (has_v && !(d_vx && d_vy && d_vz)) return fail(BLOCH_EINVAL, "give all of d_vx, d_vy, d_vz or none");
-    if (has_v && plan->info.motion_mode != BLOCH_MOTION_LINEAR)
-        return fail(BLOCH_EINVAL, "velocities given but the plan was not created with BLOCH_MOTION_LINEAR");
-    const bool mo = plan->info.motion_mode == BLOCH_MOTION_LINEAR;
+    if (has_v && plan->info.motion_mode == BLOCH_MOTION_NONE)
+        return fail(BLOCH_EINVAL, "velocities given but the plan was created without motion (BLOCH_MOTION_LINEAR / _WAVEFORM)");
+    const bool mo = plan->info.motion_mode != BLOCH_MOTION_NONE;
     if (n_spins < 0 || n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins out of range");
     if (!plan->d_tables) return fail(BLOCH_ENOTUPLOADED, "call bloch_plan_upload first");
     if (n_spins > 0 && (!d_x || !d_y || !d_z || !d_M0 || !d_T1 || !d_T2 || !d_dw))

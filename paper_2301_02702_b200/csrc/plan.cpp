@@ -73,9 +73,19 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         return fail(BLOCH_EINVAL, "bad output_mode");
     if (params->output_mode == BLOCH_OUT_GROUPED && params->group_size < 1)
         return fail(BLOCH_EINVAL, "group_size must be >= 1 with BLOCH_OUT_GROUPED");
-    if (params->motion_mode != BLOCH_MOTION_NONE && params->motion_mode != BLOCH_MOTION_LINEAR)
+    if (params->motion_mode != BLOCH_MOTION_NONE && params->motion_mode != BLOCH_MOTION_LINEAR &&
+        params->motion_mode != BLOCH_MOTION_WAVEFORM)
         return fail(BLOCH_EINVAL, "bad motion_mode");
-    const bool motion = params->motion_mode == BLOCH_MOTION_LINEAR;
+    const bool motion = params->motion_mode != BLOCH_MOTION_NONE;
+    const bool waveform = params->motion_mode == BLOCH_MOTION_WAVEFORM;
+    if (waveform) {
+        if (params->motion_n < 1 || !params->motion_t || !params->motion_u)
+            return fail(BLOCH_EINVAL, "BLOCH_MOTION_WAVEFORM needs motion_t, motion_u and motion_n >= 1");
+        if (!ascending(params->motion_t, params->motion_n, true))
+            return fail(BLOCH_ENONMONOTONIC, "motion waveform vertex times must be strictly ascending and finite");
+        for (int64_t i = 0; i < params->motion_n; ++i)
+            if (!std::isfinite(params->motion_u[i])) return fail(BLOCH_EINVAL, "motion waveform value not finite");
+    }
     const double dt_mo = (motion && params->dt_max > 0.0 && std::isfinite(params->dt_max))
                              ? params->dt_max : std::numeric_limits<double>::infinity();
     for (int a = 0; a < 3; ++a) {
@@ -160,6 +170,12 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         pts.insert(pts.end(), seq->adc_t, seq->adc_t + seq->adc_n);
         merge_run(first);
     }
+    if (waveform) {  // the vertices of the motion waveform that lie inside the sequence are points of the grid
+        const size_t first = pts.size();
+        for (int64_t i = 0; i < params->motion_n; ++i)
+            if (params->motion_t[i] >= 0.0 && params->motion_t[i] <= seq->t_end) pts.push_back(params->motion_t[i]);
+        merge_run(first);
+    }
     std::vector<double> coarse;
     coarse.reserve(pts.size());
     for (double t : pts) {
@@ -190,6 +206,24 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         }
     }
     const int64_t N = (int64_t)rf_of.size();
+    // motion waveform at the grid points: x(t_n) = x + a u_n; u(t) = t for constant velocities (MOTION_LINEAR), else
+    // the piecewise-linear interpolant of the vertices, held at its end values outside them (forward sweep)
+    std::vector<double> u(motion ? t.size() : 0);
+    if (motion && !waveform) u = t;
+    if (waveform) {
+        const double *mt = params->motion_t, *mu = params->motion_u;
+        const int64_t mn = params->motion_n;
+        int64_t seg = 0;
+        for (size_t n = 0; n < t.size(); ++n) {
+            const double tn = t[n];
+            if (tn <= mt[0]) u[n] = mu[0];
+            else if (tn >= mt[mn - 1]) u[n] = mu[mn - 1];
+            else {
+                while (seg + 2 < mn && mt[seg + 1] <= tn) ++seg;
+                u[n] = mu[seg] + (tn - mt[seg]) / (mt[seg + 1] - mt[seg]) * (mu[seg + 1] - mu[seg]);
+            }
+        }
+    }
     std::vector<double> G(3 * t.size(), 0.0);
     for (int a = 0; a < 3; ++a) sample_axis(seq->g_t[a], seq->g_v[a], seq->g_n[a], t, G, a);
     // ADC index per point (both ascending)
@@ -277,7 +311,8 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             const double dt = t[n + 1] - t[n];
             for (int a = 0; a < 3; ++a) K[a] += 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]) * dt;  // Eq 12-13
             // motion: the same trapezoid on G(t) t, so that sum of Bz(t_n) = G_n . (x + v t_n) splits into K . x + Mo . v
-            for (int a = 0; a < 3; ++a) Mo[a] += 0.5 * (G[3 * n + a] * t[n] + G[3 * (n + 1) + a] * t[n + 1]) * dt;
+            if (motion)
+                for (int a = 0; a < 3; ++a) Mo[a] += 0.5 * (G[3 * n + a] * u[n] + G[3 * (n + 1) + a] * u[n + 1]) * dt;
             const double tau = t[n + 1] - tb;
             const double kn = gbar * std::sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]);
             const double mn = gbar * std::sqrt(Mo[0] * Mo[0] + Mo[1] * Mo[1] + Mo[2] * Mo[2]);
@@ -326,7 +361,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             s.wy = (float)(gamma * dt * seq->rf_im[j]);
             for (int a = 0; a < 3; ++a) s.g[a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] + G[3 * (n + 1) + a]));
             for (int a = 0; a < 3; ++a)
-                s.h[a] = (float)(gamma * dt * 0.5 * (G[3 * n + a] * t[n] + G[3 * (n + 1) + a] * t[n + 1]));
+                s.h[a] = motion ? (float)(gamma * dt * 0.5 * (G[3 * n + a] * u[n] + G[3 * (n + 1) + a] * u[n + 1])) : 0.f;
             s.dt = (float)dt;
         }
         // cut into tiles: at most kRfTileSteps steps, one dt per tile

@@ -75,12 +75,15 @@ class Workload:
     dt_max: float = 0.0            # spacing of the intermediate points needed with motion
     group_size: int = 0            # output_mode "grouped": spins per group
     coils: np.ndarray | None = None  # complex64 [n_coils, n_spins] receive sensitivities (reading C1)
+    waveform: tuple | None = None    # (t, u) vertices of a shared motion waveform: x(t) = x + velocity * u(t) (reading M2)
 
     @property
     def plan_kw(self) -> dict:
         kw = dict(phase_mode=self.phase_mode, output_mode=self.output_mode)
         if self.velocity is not None:
             kw.update(motion="linear", dt_max=self.dt_max)
+        if self.waveform is not None:
+            kw.update(motion="waveform", waveform=self.waveform)
         if self.output_mode == "grouped":
             kw.update(group_size=self.group_size)
         return kw
@@ -474,6 +477,23 @@ def config3m(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, vy: float = 
     return Workload("config3m_brain_epi128_motion", ph, w.seq, phase_mode="fp64", velocity=vel, dt_max=dt_max)
 
 
+def config3w(n_grid: int = 256, n_epi: int = 128, n_rf: int = 1000, dt_max: float = 1e-5) -> Workload:
+    """Config 3 (off-resonance included) under NON-RIGID periodic motion, the general motion field u(x, t) of
+    PAPER.md:96 in its separable form x(t) = x + a(x) u(t): u(t) = sin(2 pi t / 50 ms) given by 101 vertices per period
+    (a breathing-like displacement, sped up so that the 73 ms EPI sees one and a half periods), amplitude growing
+    from 0.5 mm to 2.5 mm along y (in-plane stretch) plus a 0.3 mm through-slice part; intermediate points every dt_max."""
+    w = config3(n_grid, n_epi, n_rf)
+    ph = w.phantom
+    period = 50e-3
+    n_v = int(math.ceil(w.seq.t_end / period * 100)) + 1
+    wt = np.arange(n_v) * (period / 100)
+    wu = np.sin(2 * math.pi * wt / period)
+    ay = 1.5e-3 + 1e-3 * (ph.y / 0.1)
+    amp = (np.zeros(ph.n), _f32(ay), _f32(np.full(ph.n, 0.3e-3)))
+    return Workload("config3w_brain_epi128_periodic_motion", ph, w.seq, phase_mode="fp64", velocity=amp, dt_max=dt_max,
+                    waveform=(wt, wu))
+
+
 def coil_maps(ph: Phantom, n_coils: int, radius: float = 0.15, seed: int = 0) -> np.ndarray:
     """Smooth synthetic receive sensitivities, complex64 [n_coils, n_spins]: coils on a ring of `radius` around the
     z axis, magnitude r0^2 / (d^2 + r0^2) with d the in-plane distance to the coil and r0 = 0.1 m, phase = the angle
@@ -492,7 +512,7 @@ def config4c(n_coils: int = 8, **kw) -> Workload:
     return dataclasses.replace(w, name=f"config4c_1M_spiral_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
 
 
-CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "4": config4, "5": config5, "5b": config5b,
+CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "3w": config3w, "4": config4, "5": config5, "5b": config5b,
            "5c": config5c, "4c": config4c,
            "4c32": lambda **kw: config4c(n_coils=32, **kw)}
 
@@ -514,6 +534,8 @@ def small(name: str) -> Workload:
         return config3(n_grid=48, n_epi=32, n_rf=250)
     if name == "3m":
         return config3m(n_grid=24, n_epi=16, n_rf=100)
+    if name == "3w":
+        return config3w(n_grid=24, n_epi=16, n_rf=100)
     if name == "4":
         return config4(n_spins=5003, n_shots=3, n_samp=700, n_rf=300, turns=8.0 * 700 / 4096)
     if name == "5":

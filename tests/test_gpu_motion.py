@@ -35,12 +35,14 @@ def f32(a):
     return np.asarray(a, dtype=np.float32).astype(np.float64)
 
 
-def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mode="auto", host=False, options=None):
+def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mode="auto", host=False, options=None,
+             waveform=None, **plan_kw):
     import torch
     v = tuple(f32(a) for a in v)
-    plan = B.Plan(s, output_mode=output_mode, phase_mode=phase_mode, motion="linear", dt_max=dt_max, options=options)
-    assert plan.info["motion_mode"] == 1
-    t, *_ = oracle_mod.grid(s, dt_max=dt_max)
+    mo = dict(motion="linear") if waveform is None else dict(motion="waveform", waveform=waveform)
+    plan = B.Plan(s, output_mode=output_mode, phase_mode=phase_mode, dt_max=dt_max, options=options, **mo, **plan_kw)
+    assert plan.info["motion_mode"] == (1 if waveform is None else 2)
+    t, *_ = oracle_mod.grid(s, dt_max=dt_max, waveform=waveform)
     assert plan.info["n_intervals"] == len(t) - 1, "planner and oracle refine the grid differently"
     if host:
         Mxy = np.zeros((ph.n, 2), dtype=np.float32)
@@ -56,7 +58,8 @@ def run_both(B, oracle_mod, ph, s, v, dt_max, what, output_mode="sum", phase_mod
         torch.cuda.synchronize()
         sig, m, z = sig.cpu().numpy(), Mxy.cpu().numpy(), Mz.cpu().numpy()
     plan.close()
-    ref, rxy, rz = oracle_mod.simulate(ph, s, velocity=v, dt_max=dt_max, output_mode=output_mode, return_state=True)
+    ref, rxy, rz = oracle_mod.simulate(ph, s, velocity=v, dt_max=dt_max, output_mode=output_mode, return_state=True,
+                                       waveform=waveform)
     got_state = np.concatenate([m[:, 0] + 1j * m[:, 1], z.astype(np.complex128)])
     ref_state = np.concatenate([rxy, rz.astype(np.complex128)])
     for name, g, r in (("signal", sig, ref), ("state", got_state, ref_state)):
@@ -152,3 +155,108 @@ def test_moving_spins_on_cartesian_plateau_take_the_quadratic_recurrence(B, orac
     emax, nrmse = errors(out["1"], out["0"])
     print(f"motion recurrence on/off {phase_mode}: max {emax:.3e} nrmse {nrmse:.3e}")
     assert 0 < emax <= 3e-5 and nrmse <= 8e-6
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# General motion x(t) = x + a u(t) (BLOCH_MOTION_WAVEFORM; "motion field u(x, t)", reading M2)
+# ------------------------------------------------------------------------------------------------------------------
+def amplitudes(n, seed, scale=3e-3):
+    rng = np.random.default_rng(seed)
+    return tuple(rng.uniform(-scale, scale, n) for _ in range(3))
+
+
+@pytest.mark.parametrize("phase_mode", ["fp32", "fp64"])
+def test_epi_under_sinusoidal_nonrigid_displacement(B, oracle_mod, phase_mode):
+    """Config-1-like EPI while every spin oscillates with its own amplitude vector (up to 3 mm) on a shared 200 Hz
+    sinusoid given by 20 vertices per period: RF block, ramps, blips and plateaus all see the moving spins; the
+    Cartesian-recurrence kernel must only take the groups on which the waveform is linear (the planner's parabola
+    check), the rest goes through the per-sample kernel."""
+    w = W.small("1")
+    n = w.phantom.n
+    wt = np.arange(int(w.seq.t_end / 2.5e-4) + 2) * 2.5e-4
+    wf = (wt, np.sin(2 * np.pi * 200.0 * wt))
+    a = amplitudes(n, 41)
+    sig, ref = run_both(B, oracle_mod, w.phantom, w.seq, a, 2e-5, f"EPI sinusoidal motion {phase_mode}", phase_mode=phase_mode,
+                        waveform=wf, max_speed_mps=6e-3)
+    static = oracle_mod.simulate(w.phantom, w.seq)
+    assert errors(ref, static)[0] > 1e-2, "the motion must change the signal for the test to mean anything"
+    run_both(B, oracle_mod, w.phantom, w.seq, a, 2e-5, f"same through the host entry {phase_mode}", phase_mode=phase_mode,
+             waveform=wf, host=True, max_speed_mps=6e-3)
+
+
+def test_waveform_u_equal_t_is_bitwise_the_linear_motion_plan(B, oracle_mod):
+    """u(t) = t as a two-vertex waveform builds the same tables as BLOCH_MOTION_LINEAR: signal and final state bitwise."""
+    import torch
+    w = W.small("3m")
+    dev = B.phantom_to_device(w.phantom)
+    vel = tuple(torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
+    out = []
+    for kw in (dict(motion="linear"), dict(motion="waveform", waveform=([0.0, w.seq.t_end], [0.0, w.seq.t_end]))):
+        plan = B.Plan(w.seq, phase_mode="fp64", dt_max=w.dt_max, **kw)
+        Mxy = torch.zeros(w.phantom.n, 2, dtype=torch.float32, device="cuda")
+        Mz = torch.zeros(w.phantom.n, dtype=torch.float32, device="cuda")
+        sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, velocity=vel)
+        assert plan.status() == 0
+        out.append((sig.cpu().numpy(), Mxy.cpu().numpy(), Mz.cpu().numpy()))
+        plan.close()
+    for a, b in zip(*out):
+        assert np.array_equal(a.view(np.float32), b.view(np.float32))
+
+
+def test_stop_and_go_motion_slice_selective_rf_and_per_spin_output(B, oracle_mod):
+    """A displacement that ramps up during the slice-selective pulse, holds through the readout prephaser and returns
+    during the readout (stop-and-go): motion RF tiles with a non-linear u, and per-spin output."""
+    n_rf = 300
+    dt = 1e-6
+    tm = (np.arange(n_rf) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - n_rf * dt / 2) / (n_rf * dt))
+    b1 = env * np.deg2rad(70) / (W.GAMMA * dt * env.sum())
+    rf = (2e-4 + np.arange(n_rf) * dt, np.full(n_rf, dt), b1, np.zeros(n_rf))
+    g = {2: ([1e-4, 2e-4, 5e-4, 6e-4, 8e-4, 9e-4], [0, 15e-3, 15e-3, 0, -11e-3, 0]),
+         0: ([1.0e-3, 1.1e-3, 2.6e-3, 2.7e-3], [0, 7e-3, 7e-3, 0])}
+    adc = 1.1e-3 + (np.arange(300) + 0.5) * 5e-6
+    s = seq(g=g, rf=rf, adc=adc, t_end=3e-3, dt_rf_max=dt)
+    wf = ([1.5e-4, 4.5e-4, 1.6e-3, 2.2e-3], [0.0, 1.0, 1.0, 0.0])
+    ph, _ = moving_phantom(900, 43)
+    a = amplitudes(ph.n, 44, scale=2e-3)
+    run_both(B, oracle_mod, ph, s, a, 1e-5, "stop-and-go, slice-select", waveform=wf, max_speed_mps=4e-3)
+    sub = ph.subset(np.arange(31))
+    run_both(B, oracle_mod, sub, s, tuple(x[:31] for x in a), 1e-5, "stop-and-go, per spin", waveform=wf,
+             output_mode="per_spin", max_speed_mps=4e-3)
+
+
+def test_waveform_plan_argument_errors(B):
+    s = W.small("1").seq
+    for kw, code in ((dict(motion="waveform"), -1), (dict(motion="waveform", waveform=([1e-3, 5e-4], [0.0, 1.0])), -2),
+                     (dict(motion="waveform", waveform=([0.0, 1e-3], [0.0, float("nan")])), -1)):
+        with pytest.raises(B.BlochError) as e:
+            B.Plan(s, **kw)
+        assert e.value.code == code
+
+
+def test_full_config3_under_periodic_nonrigid_motion(B, oracle_mod):
+    """Workload 3w at full size (131,072 spins, EPI 128 x 128, fp64 phase, off-resonance, breathing-like non-rigid
+    displacement), whole oracle."""
+    import torch
+    w = W.make("3w")
+    plan = B.Plan(w.seq, **w.plan_kw)
+    dev = B.phantom_to_device(w.phantom)
+    amp = tuple(torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in w.velocity)
+    Mxy = torch.zeros(w.phantom.n, 2, dtype=torch.float32, device="cuda")
+    Mz = torch.zeros(w.phantom.n, dtype=torch.float32, device="cuda")
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, velocity=amp)
+    assert plan.status() == 0
+    plan.close()
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, velocity=w.velocity, dt_max=w.dt_max, waveform=w.waveform,
+                                       return_state=True)
+    m = Mxy.cpu().numpy()
+    for name, got, want in (("signal", sig.cpu().numpy(), ref),
+                            ("state", np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)]),
+                             np.concatenate([rxy, rz.astype(np.complex128)]))):
+        emax, nrmse = errors(got, want)
+        print(f"config 3w full-size {name}: max {emax:.3e} nrmse {nrmse:.3e}")
+        assert emax <= TOL_MAX and nrmse <= TOL_NRMSE
+    static = oracle_mod.simulate(w.phantom.subset(np.arange(0, w.phantom.n, 64)), w.seq)
+    moving = oracle_mod.simulate(w.phantom.subset(np.arange(0, w.phantom.n, 64)), w.seq,
+                                 velocity=tuple(a[::64] for a in w.velocity), dt_max=w.dt_max, waveform=w.waveform)
+    assert errors(moving, static)[0] > 1e-2

@@ -239,3 +239,19 @@ def test_phase_mode_auto_follows_the_declared_extents(B):
     with pytest.raises(B.BlochError) as e:
         B.bloch_plan_create(s, max_extent_m=float("nan"))
     assert e.value.code == -1
+
+
+def test_waveform_motion_plan_merges_the_vertices_like_the_oracle(B, oracle_mod):
+    """BLOCH_MOTION_WAVEFORM: the vertices of u(t) inside the sequence are points of the planner's grid exactly as they
+    are of the oracle's, on top of the dt_max refinement; vertices outside [0, t_end] only shape u."""
+    w = W.small("1")
+    wf = (np.array([-1e-3, 1.234e-4, 3.3e-4, 9.871e-4, w.seq.t_end + 1e-3]), np.array([0.0, 0.5, 1.0, -1.0, 0.0]))
+    for dt_max in (0.0, 3e-5):
+        h = B.bloch_plan_create(w.seq, motion="waveform", waveform=wf, dt_max=dt_max)
+        info = B.bloch_plan_get_info(h)
+        B.bloch_plan_destroy(h)
+        t, _, rf, _ = oracle_mod.grid(w.seq, dt_max=dt_max, waveform=wf)
+        assert info["n_intervals"] == len(t) - 1 and info["n_rf_steps"] == int(rf.sum()) and info["motion_mode"] == 2
+    h = B.bloch_plan_create(w.seq, motion="linear", dt_max=3e-5)
+    assert B.bloch_plan_get_info(h)["n_intervals"] < info["n_intervals"]     # the inner vertices added points
+    B.bloch_plan_destroy(h)
