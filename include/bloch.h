@@ -243,15 +243,22 @@ int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t 
  *   d_signal  DEVICE, float2 [n_coils][n_adc] row-major, written
  *   workspace as bloch_simulate, sized by bloch_plan_workspace_bytes_coils(plan, n_spins, n_coils)
  * Everything else as bloch_simulate (same integration, same final magnetisation).  The plan must be BLOCH_OUT_SUM_ALL
- * without motion (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  The coil-independent part of every evaluation (phase,
- * sin / cos / exp) is computed once per 4 or 8 coils; with more than 8 coils (fp32 phase) the sum over spins runs on the
- * tensor cores (tcgen05, 3xTF32, 16 or 32 coils per pass).  Asynchronous on `stream`; never allocates. */
+ * (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  Moving spins: bloch_simulate_coils_motion (motion plans; velocities /
+ * amplitudes as bloch_simulate_motion, all three NULL = none).  The coil-independent part of every evaluation (phase,
+ * sin / cos / exp) is computed once per 4 or 8 coils; with more than 4 coils (fp32 phase) the sum over spins runs on the
+ * tensor cores (tcgen05 with the generated operand in tensor memory, 3xTF32, 8, 16 or 32 coils per pass).  Asynchronous on `stream`; never allocates. */
 int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out);
 int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
                          const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
                          const float *d_dw, int n_coils, const float *d_coil, float *d_Mxy, float *d_Mz,
                          int init_equilibrium, float *d_signal, void *d_workspace, size_t workspace_bytes,
                          void *stream);
+
+int bloch_simulate_coils_motion(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                                const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                                const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz, int n_coils,
+                                const float *d_coil, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                                void *d_workspace, size_t workspace_bytes, void *stream);
 
 /* Host-buffer variant of bloch_simulate_coils: phantom, coil weights (float2 [n_coils][n_spins]), state and signal
  * (float2 [n_coils][n_adc]) are HOST arrays (pinned memory makes the copies asynchronous); H2D and D2H copies are
@@ -263,6 +270,11 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
                               const float *h_dw, int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz,
                               int init_equilibrium, float *h_signal, void *d_scratch, size_t scratch_bytes,
                               void *stream);
+int bloch_simulate_host_coils_motion(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                                     const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                                     const float *h_dw, const float *h_vx, const float *h_vy, const float *h_vz,
+                                     int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz, int init_equilibrium,
+                                     float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
 
 /* Execution path of bloch_simulate for this plan.
  *   BLOCH_PATH_PER_BLOCK: one excitation launch per RF block and one signal launch per precession block.
@@ -292,8 +304,8 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *   BLOCH_OPT_RF_THREADS          0 (default): 128-thread excitation CTAs once there are >= 32 warps per SM, else 32;
  *                                 32 / 64 / 128 forces it
  *   BLOCH_OPT_RF_SPINS            spins per thread of the excitation kernel: 0 (default) the library's choice, 1 or 2
- *   BLOCH_OPT_COIL_TC             multi-coil receive: -1 (default) tensor cores (tcgen05) for more than 8 coils, 0 never,
- *                                 1 whenever they apply (more than 4 coils, fp32 phase)
+ *   BLOCH_OPT_COIL_TC             multi-coil receive: -1 (default) and 1: tensor cores (tcgen05, A operand in tensor
+ *                                 memory) whenever they apply (more than 4 coils, fp32 phase); 0: never
  *   BLOCH_OPT_SEQ_SIG_EXTRA       whole-sequence kernel: signal warps added per missing RF warp of a sub-partition,
  *                                 0..7, default 2
  *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic

@@ -64,7 +64,7 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
            "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils", "bloch_simulate_host_coils_scratch_bytes",
            "bloch_simulate_host_coils", "bloch_plan_set_option", "bloch_plan_get_option", "bloch_plan_status",
-           "bloch_plan_last_kernel", "bloch_microbench"]
+           "bloch_plan_last_kernel", "bloch_simulate_coils_motion", "bloch_simulate_host_coils_motion", "bloch_microbench"]
 
 
 def _load():
@@ -94,6 +94,8 @@ def _load():
     lib.bloch_simulate_coils.argtypes = [vp, i64] + [_fp] * 7 + [C.c_int, _fp, _fp, _fp, C.c_int, _fp, vp, sz, vp]
     lib.bloch_simulate_host_coils_scratch_bytes.argtypes = [vp, i64, C.c_int, C.POINTER(sz)]
     lib.bloch_simulate_host_coils.argtypes = lib.bloch_simulate_coils.argtypes
+    lib.bloch_simulate_coils_motion.argtypes = [vp, i64] + [_fp] * 10 + [C.c_int, _fp, _fp, _fp, C.c_int, _fp, vp, sz, vp]
+    lib.bloch_simulate_host_coils_motion.argtypes = lib.bloch_simulate_coils_motion.argtypes
     lib.bloch_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.bloch_plan_last_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i64)]
     lib.bloch_plan_last_launches.argtypes = [vp, C.POINTER(i64)]
@@ -240,6 +242,20 @@ def bloch_simulate_coils(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, n_coi
     DEVICE address of float2 [n_coils][n_adc]."""
     _check(_lib.bloch_simulate_coils(plan, n_spins, x, y, z, M0, T1, T2, dw, n_coils, coil, Mxy, Mz,
                                      int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_coils_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, n_coils: int, coil, Mxy, Mz,
+                                init_equilibrium: bool, signal, workspace, workspace_bytes: int, stream: int = 0):
+    """bloch_simulate_coils for moving spins (motion plans); vx, vy, vz raw DEVICE addresses or None for all three."""
+    _check(_lib.bloch_simulate_coils_motion(plan, n_spins, x, y, z, M0, T1, T2, dw, vx, vy, vz, n_coils, coil, Mxy, Mz,
+                                            int(bool(init_equilibrium)), signal, workspace, workspace_bytes, stream))
+
+
+def bloch_simulate_host_coils_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, n_coils: int, coil, Mxy,
+                                     Mz, init_equilibrium: bool, signal, scratch, scratch_bytes: int, stream: int = 0):
+    """bloch_simulate_coils_motion with HOST phantom / velocity / coil / state / signal addresses."""
+    _check(_lib.bloch_simulate_host_coils_motion(plan, n_spins, x, y, z, M0, T1, T2, dw, vx, vy, vz, n_coils, coil, Mxy,
+                                                 Mz, int(bool(init_equilibrium)), signal, scratch, scratch_bytes, stream))
 
 
 def bloch_simulate_host_coils_scratch_bytes(plan: int, n_spins: int, n_coils: int) -> int:
@@ -435,16 +451,21 @@ class Plan:
         self._check_out(signal, 2 * n_rows * n_adc, (torch.complex64,), "signal")
         if coils is not None:
             assert coils.is_cuda and coils.dtype == torch.complex64 and coils.is_contiguous() and \
-                coils.dim() == 2 and coils.shape[1] == n and velocity is None
+                coils.dim() == 2 and coils.shape[1] == n
             n_coils = int(coils.shape[0])
             if signal is None:
                 signal = torch.empty((n_coils, n_adc), dtype=torch.complex64, device="cuda")
             ws = self._workspace(n, n_coils)
-            bloch_simulate_coils(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(),
-                                 T1.data_ptr(), T2.data_ptr(), dw.data_ptr(), n_coils, coils.data_ptr(),
-                                 None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
-                                 init_equilibrium, signal.data_ptr() if signal.numel() else None,
-                                 ws.data_ptr(), ws.numel(), self._stream())
+            vp = [None, None, None]
+            if velocity is not None:
+                for t in velocity:
+                    assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
+                vp = [t.data_ptr() for t in velocity]
+            bloch_simulate_coils_motion(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(),
+                                        T1.data_ptr(), T2.data_ptr(), dw.data_ptr(), *vp, n_coils, coils.data_ptr(),
+                                        None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
+                                        init_equilibrium, signal.data_ptr() if signal.numel() else None,
+                                        ws.data_ptr(), ws.numel(), self._stream())
             return signal
         if signal is None:
             signal = torch.empty(shape, dtype=torch.complex64, device="cuda")
@@ -483,17 +504,20 @@ class Plan:
             signal = np.empty(shape, dtype=np.complex64)
         if coils is not None:
             cw = np.ascontiguousarray(coils, dtype=np.complex64)
-            assert cw.ndim == 2 and cw.shape[1] == n and velocity is None
+            assert cw.ndim == 2 and cw.shape[1] == n
             n_coils = int(cw.shape[0])
+            hv = [None, None, None] if velocity is None else \
+                [np.ascontiguousarray(a, dtype=np.float32) for a in velocity]
             if signal is None or signal.shape != (n_coils, n_adc):
                 signal = np.empty((n_coils, n_adc), dtype=np.complex64)
             need = max(bloch_simulate_host_coils_scratch_bytes(self.handle, n, n_coils), 256)
             if self._scratch is None or self._scratch.numel() < need:
                 self._scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
-            bloch_simulate_host_coils(self.handle, n, *[a.ctypes.data for a in arrs], n_coils, cw.ctypes.data,
-                                      None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
-                                      init_equilibrium, signal.ctypes.data if signal.size else None,
-                                      self._scratch.data_ptr(), self._scratch.numel(), self._stream())
+            bloch_simulate_host_coils_motion(self.handle, n, *[a.ctypes.data for a in arrs],
+                                             *[None if a is None else a.ctypes.data for a in hv], n_coils, cw.ctypes.data,
+                                             None if Mxy is None else Mxy.ctypes.data, None if Mz is None else Mz.ctypes.data,
+                                             init_equilibrium, signal.ctypes.data if signal.size else None,
+                                             self._scratch.data_ptr(), self._scratch.numel(), self._stream())
             return signal
         need = max(bloch_simulate_host_scratch_bytes(self.handle, n), 256)
         if self._scratch is None or self._scratch.numel() < need:

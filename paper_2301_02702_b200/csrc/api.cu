@@ -258,14 +258,14 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
 }
 
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
-// tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 256 threads, 2 CTAs per SM, chunks of whole 16-spin stages
+// tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 288 threads, 2 CTAs per SM, chunks of whole 16-spin stages
 bool coil_use_tc(const bloch_plan *plan, int n_coils) {
-    // BLOCH_OPT_COIL_TC: 0 = never, 1 = whenever it applies (more than 4 coils, fp32 phase), -1 = when it pays: more
-    // than 8 coils (16 coils per pass cost what 8 cost: config 4 with 32 coils 260 ms against 486 ms for the FFMA
-    // kernel; with 8 coils 129.5 against 121.4)
+    // BLOCH_OPT_COIL_TC: 0 = never, -1 / 1 = whenever it applies: more than 4 coils and fp32 phase.  With the A operand
+    // in tensor memory one pass of the tcgen05 kernel costs the same for 8, 16 and 32 coils (config 4: 106-107 ms)
+    // and beats the FFMA kernel from its first pass of 8 (121 ms); up to 4 coils the 4-wide FFMA kernel (~90 ms) stays.
     const int mode = plan->opt[BLOCH_OPT_COIL_TC];
-    if (mode == 0 || n_coils <= 4 || plan->info.phase_mode != BLOCH_PHASE_FP32) return false;
-    return mode == 1 || n_coils > 8;
+    return mode != 0 && n_coils > 4 && plan->info.phase_mode == BLOCH_PHASE_FP32 &&
+           plan->info.motion_mode == BLOCH_MOTION_NONE;  // moving spins: the FFMA kernel
 }
 
 SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp, bool tc) {
@@ -646,12 +646,22 @@ int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d
                          const float *d_dw, int n_coils, const float *d_coil, float *d_Mxy, float *d_Mz,
                          int init_equilibrium, float *d_signal, void *d_workspace, size_t workspace_bytes,
                          void *stream_) {
+    return bloch_simulate_coils_motion(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, nullptr, nullptr, nullptr,
+                                       n_coils, d_coil, d_Mxy, d_Mz, init_equilibrium, d_signal, d_workspace,
+                                       workspace_bytes, stream_);
+}
+
+int bloch_simulate_coils_motion(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                                const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                                const float *d_dw, const float *d_vx, const float *d_vy, const float *d_vz, int n_coils,
+                                const float *d_coil, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                                void *d_workspace, size_t workspace_bytes, void *stream_) {
     if (!plan) return bloch::fail(BLOCH_EINVAL, "NULL plan");
     if (n_coils < 1 || n_coils > 4096) return bloch::fail(BLOCH_EINVAL, "n_coils must be in [1, 4096]");
     if (n_spins > 0 && !d_coil) return bloch::fail(BLOCH_EINVAL, "d_coil is NULL");
-    if (plan->info.output_mode != BLOCH_OUT_SUM_ALL || plan->info.motion_mode != BLOCH_MOTION_NONE)
-        return bloch::fail(BLOCH_EINVAL, "multi-coil receive needs a BLOCH_OUT_SUM_ALL plan without motion");
-    return bloch::simulate_impl(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, nullptr, nullptr, nullptr, n_coils,
+    if (plan->info.output_mode != BLOCH_OUT_SUM_ALL)
+        return bloch::fail(BLOCH_EINVAL, "multi-coil receive needs a BLOCH_OUT_SUM_ALL plan");
+    return bloch::simulate_impl(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, d_vx, d_vy, d_vz, n_coils,
                                 d_coil, d_Mxy, d_Mz, init_equilibrium, d_signal, d_workspace, workspace_bytes, stream_);
 }
 
@@ -857,13 +867,15 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     const float4 *Wp = reinterpret_cast<const float4 *>(w.W + (size_t)pass * n * ncp);
                     const int in_pass = std::min(ncp, n_coils - pass * ncp);
                     if (pass > 0 && (rc = taps.mark(BLOCH_KIND_SIGNAL))) return rc;
-#define BLOCH_LAUNCH_COIL(PP, NCC, H, AP)                                                                           \
-    signal_coils_kernel<PP, NCC, H><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, w.S, Wp, n, s.spins_per_chunk,   \
-                                                                      (const float *)w.scal, w.partial)
-#define BLOCH_LAUNCH_COIL2(PP, NCC)                                \
-    do {                                                           \
-        if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, w.Ad);          \
-        else BLOCH_LAUNCH_COIL(PP, NCC, false, w.A);               \
+#define BLOCH_LAUNCH_COIL(PP, NCC, H, M, AP, VP)                                                                       \
+    signal_coils_kernel<PP, NCC, H, M><<<grid, s.threads, 0, stream>>>(recs, n_pts, AP, VP, w.S, Wp, n, s.spins_per_chunk, \
+                                                                         (const float *)w.scal, w.partial)
+#define BLOCH_LAUNCH_COIL2(PP, NCC)                                        \
+    do {                                                                   \
+        if (ph64 && mo) BLOCH_LAUNCH_COIL(PP, NCC, true, true, w.Ad, w.Vd);    \
+        else if (ph64) BLOCH_LAUNCH_COIL(PP, NCC, true, false, w.Ad, nullptr); \
+        else if (mo) BLOCH_LAUNCH_COIL(PP, NCC, false, true, w.A, w.V);        \
+        else BLOCH_LAUNCH_COIL(PP, NCC, false, false, w.A, nullptr);           \
     } while (0)
                     if (tc) note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, kTcThreads, "signal_coils_tc_kernel<%d>", ncp);
                     else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d>",
@@ -1084,7 +1096,7 @@ int bloch_simulate_host_coils_scratch_bytes(const bloch_plan *plan, int64_t n_sp
     const size_t arr = align_up(size_t(n_spins) * sizeof(float), kAlign);
     const size_t coil = align_up(size_t(n_coils) * size_t(n_spins) * sizeof(float2), kAlign);
     const size_t sig = align_up(size_t(n_coils) * size_t(plan->info.n_adc) * sizeof(float2), kAlign);
-    *out = 10 * arr + coil + sig + ws + kAlign;
+    *out = 13 * arr + coil + sig + ws + kAlign;
     return BLOCH_OK;
 }
 
@@ -1093,7 +1105,19 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
                               const float *h_dw, int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz,
                               int init_equilibrium, float *h_signal, void *d_scratch, size_t scratch_bytes,
                               void *stream_) {
+    return bloch_simulate_host_coils_motion(plan, n_spins, h_x, h_y, h_z, h_M0, h_T1, h_T2, h_dw, nullptr, nullptr, nullptr,
+                                            n_coils, h_coil, h_Mxy, h_Mz, init_equilibrium, h_signal, d_scratch,
+                                            scratch_bytes, stream_);
+}
+
+int bloch_simulate_host_coils_motion(const bloch_plan *plan, int64_t n_spins, const float *h_x, const float *h_y,
+                                     const float *h_z, const float *h_M0, const float *h_T1, const float *h_T2,
+                                     const float *h_dw, const float *h_vx, const float *h_vy, const float *h_vz,
+                                     int n_coils, const float *h_coil, float *h_Mxy, float *h_Mz, int init_equilibrium,
+                                     float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream_) {
     if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    const bool has_v = h_vx || h_vy || h_vz;
+    if (has_v && !(h_vx && h_vy && h_vz)) return fail(BLOCH_EINVAL, "give all of h_vx, h_vy, h_vz or none");
     size_t need = 0;
     int rc = bloch_simulate_host_coils_scratch_bytes(plan, n_spins, n_coils, &need);
     if (rc) return rc;
@@ -1122,15 +1146,24 @@ int bloch_simulate_host_coils(const bloch_plan *plan, int64_t n_spins, const flo
         BLOCH_CUDA(cudaMemcpyAsync(d_Mxy, h_Mxy, size_t(n_spins) * 2 * sizeof(float), cudaMemcpyHostToDevice, stream));
         BLOCH_CUDA(cudaMemcpyAsync(d_Mz, h_Mz, size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
     }
-    float *d_coil = (float *)(base + 10 * arr);
+    float *d_v[3] = {nullptr, nullptr, nullptr};
+    if (has_v) {
+        const float *hv[3] = {h_vx, h_vy, h_vz};
+        for (int k = 0; k < 3; ++k) {
+            d_v[k] = (float *)(base + (10 + k) * arr);
+            if (n_spins > 0)
+                BLOCH_CUDA(cudaMemcpyAsync(d_v[k], hv[k], size_t(n_spins) * sizeof(float), cudaMemcpyHostToDevice, stream));
+        }
+    }
+    float *d_coil = (float *)(base + 13 * arr);
     if (n_spins > 0)
         BLOCH_CUDA(cudaMemcpyAsync(d_coil, h_coil, size_t(n_coils) * size_t(n_spins) * sizeof(float2),
                                    cudaMemcpyHostToDevice, stream));
-    float *d_sig = (float *)(base + 10 * arr + coil);
-    unsigned char *d_ws = base + 10 * arr + coil + align_up(sig, kAlign);
+    float *d_sig = (float *)(base + 13 * arr + coil);
+    unsigned char *d_ws = base + 13 * arr + coil + align_up(sig, kAlign);
     const size_t ws_bytes = scratch_bytes - (size_t)(d_ws - base);
-    rc = bloch_simulate_coils(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], n_coils, d_coil, d_Mxy, d_Mz,
-                              init_equilibrium, d_sig, d_ws, ws_bytes, stream_);
+    rc = bloch_simulate_coils_motion(plan, n_spins, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d_v[0], d_v[1], d_v[2],
+                                     n_coils, d_coil, d_Mxy, d_Mz, init_equilibrium, d_sig, d_ws, ws_bytes, stream_);
     if (rc) return rc;
     if (sig > 0) BLOCH_CUDA(cudaMemcpyAsync(h_signal, d_sig, sig, cudaMemcpyDeviceToHost, stream));
     if (h_Mxy && n_spins > 0) {

@@ -38,23 +38,28 @@ pack_coils_kernel(int n, int n_coils, int ncp, const float2 *__restrict__ coil, 
     }
 }
 
-template <int P, int NC, bool PH64>
-__global__ void __launch_bounds__(kSigThreads, NC == 8 ? 2 : 4)
-signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_,
+// MO (motion plans, x(t) = x + v u(t)): every record (k', tau) is followed by (mu', 0), the spins' velocities /
+// amplitudes are one more staged tile, and the phase gains mu' . v, exactly as in signal_kernel.
+template <int P, int NC, bool PH64, bool MO>
+__global__ void __launch_bounds__(kSigThreads, (NC == 8 || MO) ? 2 : 4)
+signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict__ A_, const void *__restrict__ V_,
                     const float4 *__restrict__ S, const float4 *__restrict__ W /* this pass: NC / 2 float4 per spin */,
                     int n_spins, int spins_per_chunk, const float *__restrict__ scal,
                     float2 *__restrict__ partial /* [NC][chunks][n_pts] */) {
     using RecT = typename std::conditional<PH64, double4, float4>::type;
     using PosT = typename std::conditional<PH64, double4, float4>::type;
     using real = typename std::conditional<PH64, double, float>::type;
-    constexpr int TILE = NC == 8 ? 128 : kSigTile;  // spins per staged tile (static shared memory stays < 48 KB)
+    constexpr int TILE = (NC == 8 || MO) ? 128 : kSigTile;  // spins per staged tile (static shared memory stays < 48 KB)
     __shared__ __align__(128) PosT shA[2][TILE];
     __shared__ __align__(128) float4 shS[2][TILE];
     constexpr int WQ = NC / 2;  // float4 per spin
     __shared__ __align__(128) float4 shW[2][WQ * TILE];
+    __shared__ __align__(128) PosT shV[MO ? 2 : 1][MO ? TILE : 1];
     __shared__ __align__(8) uint64_t bar[2];
     const RecT *recs = reinterpret_cast<const RecT *>(recs_);
     const PosT *A = reinterpret_cast<const PosT *>(A_);
+    const PosT *V = reinterpret_cast<const PosT *>(V_);
+    constexpr int RS = MO ? 2 : 1;
     const int tid = threadIdx.x;
     const int s0 = blockIdx.y * spins_per_chunk;
     const int s1 = min(n_spins, s0 + spins_per_chunk);
@@ -63,10 +68,11 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         const int b = t & 1;
         const int base = s0 + t * TILE;
         const uint32_t cnt = (uint32_t)min(TILE, s1 - base);
-        mbar_expect_tx(&bar[b], cnt * (uint32_t)(sizeof(PosT) + (1 + WQ) * sizeof(float4)));
+        mbar_expect_tx(&bar[b], cnt * (uint32_t)((MO ? 2 : 1) * sizeof(PosT) + (1 + WQ) * sizeof(float4)));
         bulk_g2s(shA[b], A + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
         bulk_g2s(shS[b], S + base, cnt * (uint32_t)sizeof(float4), &bar[b]);
         bulk_g2s(shW[b], W + WQ * (size_t)base, cnt * (uint32_t)(WQ * sizeof(float4)), &bar[b]);
+        if (MO) bulk_g2s(shV[b], V + base, cnt * (uint32_t)sizeof(PosT), &bar[b]);
     };
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -76,7 +82,7 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         if (n_tiles > 1) issue(1);
     }
     const int p0 = (blockIdx.x * (int)blockDim.x + tid) * P;  // blockDim.x < kSigThreads for blocks of few samples
-    real kx[P], ky[P], kz[P], tau[P];
+    real kx[P], ky[P], kz[P], tau[P], ux[MO ? P : 1], uy[MO ? P : 1], uz[MO ? P : 1];
     float tf[P], cj[P], ar[NC][P], ai[NC][P];
     float cmax = 0.f;
 #pragma unroll
@@ -84,8 +90,14 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         const int p = p0 + j;
         RecT r;
         r.x = 0; r.y = 0; r.z = 0; r.w = j ? tau[0] : (real)0;
-        if (p < n_pts) r = recs[p];
+        if (p < n_pts) r = recs[RS * p];
         kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
+        if (MO) {
+            RecT m;
+            m.x = 0; m.y = 0; m.z = 0; m.w = 0;
+            if (p < n_pts) m = recs[RS * p + 1];
+            ux[j] = m.x; uy[j] = m.y; uz[j] = m.z;
+        }
         tf[j] = (float)r.w;
         cj[j] = (float)(r.w - tau[0]) * 0.6931471805599453f;
         cmax = fmaxf(cmax, fabsf(cj[j]));
@@ -102,6 +114,9 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
         for (int s = 0; s < cnt; ++s) {
             const PosT a = shA[b][s];
             const float4 st = shS[b][s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
+            PosT vv;
+            vv.x = 0; vv.y = 0; vv.z = 0; vv.w = 0;
+            if (MO) vv = shV[b][s];
             float wr[NC], wi[NC];
 #pragma unroll
             for (int q = 0; q < WQ; ++q) {
@@ -115,6 +130,8 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
                 if (PH64) {
                     double th = fma((double)kx[j], (double)a.x, fma((double)ky[j], (double)a.y,
                                     fma((double)kz[j], (double)a.z, (double)tau[j] * (double)a.w)));  // turns
+                    if (MO) th = fma((double)ux[j], (double)vv.x, fma((double)uy[j], (double)vv.y,
+                                     fma((double)uz[j], (double)vv.z, th)));
                     th += 1572864.0;  // 1.5 * 2^20: the low word is frac(theta) in 0.32 fixed point (signal.cuh)
                     const unsigned lo = (unsigned)__double2loint(th);
                     const float fr = __uint_as_float(0x3f800000u | (lo >> 9)) - 1.0f;
@@ -122,8 +139,10 @@ signal_coils_kernel(const void *__restrict__ recs_, int n_pts, const void *__res
                     sn = __sinf(ang);
                     cs = __cosf(ang);
                 } else {
-                    const float th = fmaf((float)kx[j], (float)a.x, fmaf((float)ky[j], (float)a.y,
-                                          fmaf((float)kz[j], (float)a.z, (float)tau[j] * (float)a.w)));  // radians
+                    float th = fmaf((float)kx[j], (float)a.x, fmaf((float)ky[j], (float)a.y,
+                                    fmaf((float)kz[j], (float)a.z, (float)tau[j] * (float)a.w)));  // radians
+                    if (MO) th = fmaf((float)ux[j], (float)vv.x, fmaf((float)uy[j], (float)vv.y,
+                                      fmaf((float)uz[j], (float)vv.z, th)));
                     sn = __sinf(th);
                     cs = __cosf(th);
                 }

@@ -77,7 +77,7 @@ def test_coil_argument_errors_and_edge_cases(B):
     n = w.phantom.n
     dev = B.phantom_to_device(w.phantom)
     coils = torch.ones(2, n, dtype=torch.complex64, device="cuda")
-    for kw in (dict(output_mode="per_spin"), dict(motion="linear", dt_max=1e-4)):
+    for kw in (dict(output_mode="per_spin"),):
         plan = B.Plan(w.seq, **kw)
         ws = torch.empty(1 << 24, dtype=torch.uint8, device="cuda")
         sig = torch.empty(2, plan.info["n_adc"], dtype=torch.complex64, device="cuda")
@@ -137,3 +137,47 @@ def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils):
     ffma = run_coils(B, w, coils, phase_mode="fp32", options={"coil_tc": 0})
     emax, _ = errors(got, ffma)
     assert emax < 2e-5, f"tensor-core vs FFMA kernel: {emax:.3e}"   # TMEM accumulation is coarser than FFMA sums
+
+
+@pytest.mark.parametrize("phase_mode,n_coils,wave", [("fp32", 3, False), ("fp64", 8, False), ("fp32", 6, True), ("fp64", 11, True)])
+def test_coils_with_moving_spins(B, oracle_mod, phase_mode, n_coils, wave):
+    """Coils x motion (PAPER.md:95 coil sensitivity, :96 motion field): S_c(t) = sum_i C_c(x_i) Mxy_i(t) with every spin
+    moving, constant velocities or amplitudes on a shared waveform; the weights stay those of the spin's home position
+    (they are per-spin inputs, reading C1).  Device and host entries; 11 coils = two passes of the 8-wide kernel."""
+    import torch
+    w = W.small("1")
+    n = w.phantom.n
+    rng = np.random.default_rng(50 + n_coils)
+    coils = coil_maps(w.phantom, n_coils, seed=20 + n_coils)
+    if wave:
+        wt = np.arange(int(w.seq.t_end / 2.5e-4) + 2) * 2.5e-4
+        wf = (wt, np.sin(2 * np.pi * 300.0 * wt))
+        v = tuple(rng.uniform(-2e-3, 2e-3, n).astype(np.float32).astype(np.float64) for _ in range(3))
+        kw = dict(motion="waveform", waveform=wf, dt_max=2e-5, max_speed_mps=4e-3)
+    else:
+        wf = None
+        v = tuple(rng.uniform(-0.2, 0.2, n).astype(np.float32).astype(np.float64) for _ in range(3))
+        kw = dict(motion="linear", dt_max=2e-5)
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), velocity=v, dt_max=2e-5,
+                                       waveform=wf, return_state=True)
+    plan = B.Plan(w.seq, phase_mode=phase_mode, **kw)
+    dev = B.phantom_to_device(w.phantom)
+    vel = tuple(torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda() for a in v)
+    Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda")
+    Mz = torch.zeros(n, dtype=torch.float32, device="cuda")
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, velocity=vel, coils=torch.from_numpy(coils).cuda())
+    assert plan.status() == 0
+    got = sig.cpu().numpy()
+    assert_parity(got, ref, f"coils x motion {phase_mode} {n_coils} coils wave={wave}")
+    for c in range(n_coils):
+        emax, nrmse = errors(got[c], ref[c])
+        assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
+    m = Mxy.cpu().numpy()
+    assert_parity(np.concatenate([m[:, 0] + 1j * m[:, 1], Mz.cpu().numpy().astype(np.complex128)]),
+                  np.concatenate([rxy, rz.astype(np.complex128)]), "final state, coils x motion")
+    ph = w.phantom
+    host = plan.simulate_host(ph.x, ph.y, ph.z, ph.M0, ph.T1, ph.T2, ph.dw, velocity=v, coils=coils)
+    assert np.array_equal(host.view(np.float32), got.view(np.float32)), "host entry differs from the device entry"
+    static = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128))
+    assert errors(ref, static)[0] > 1e-2, "the motion must change the signal for the test to mean anything"
+    plan.close()
