@@ -27,8 +27,11 @@
  * in the same test file (closed forms under constant G for sinusoidal and stop-and-go u, reduction to x + v t,
  * displacement-only phase, O(dt^2) convergence under a ramp).
  *
- * Pins (tests/test_oracle_pins.py): closed forms P1-P10 of SURVEY.md 8(c); no value printed by the paper
- * exists for this path, so "against the paper's own numbers" the parity is unpinned (stated in DESIGN.md).
+ * Pins (tests/test_oracle_pins.py): closed forms and invariants P1-P12 (the adiabatic
+ * hyperbolic-secant profile P11, the frequency-offset slice shift P12), the count pin of reading G18 (an RF train late
+ * in a long sequence keeps its nominal step count) and the grouped FISP pin; motion M1-M5 and W1-W5, coils C1 in their
+ * own test files.  No value printed by the paper exists for this path, so "against the paper's own numbers" the parity
+ * is unpinned (stated in DESIGN.md).
  *
  * Build: gcc -O2 -std=c11 -fopenmp -fPIC -shared bloch_ref.c -o libbloch_ref.so -lm   (no fast-math)
  */
