@@ -108,7 +108,8 @@ def capture_fields(kernel: dict, pipe: str):
         v = m.get(key)
         return v[0] / 100.0 if v else None
     pipe_key = {"mufu": "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active",
-                "fp32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"}[pipe]
+                "fp32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active",
+                "tf32": "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active"}[pipe]
     have = "dram__bytes_read.sum" in m
     return {"traffic": nbytes("dram__bytes_read.sum") + nbytes("dram__bytes_write.sum") if have else None,
             "traffic_source": cap["file"], "pipe_util": pct(pipe_key),
@@ -294,7 +295,26 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
                                "issues 2 + 1/P (P adjacent samples share one ex2), the Cartesian recurrence kernels 5 per "
                                "P samples (issue-bound, not MUFU-bound)")
         kern["signal"]["coils"] = n_coils
-        if n_coils > 0:
+        k_sig = bloch.bloch_plan_last_kernel(plan.handle, "signal")
+        if n_coils > 0 and k_sig["name"].startswith("signal_coils_tc_kernel"):
+            # tcgen05 kernel: the receive sum is a dense contraction [samples x spins] x [spins x coils], complex:
+            # algorithmic 8 real flops per (spin, ADC sample, coil); the kernel executes 3x that (3xTF32).  Peak for
+            # TF32 = the measured dense bf16 peak x the nominal 1/2 ratio (B200_PROFILING.md).
+            dur = kinds_ms["signal"] * 1e-3 / steps
+            flops = 8.0 * n_coils * n_eval_sig
+            peaks = load_peaks()
+            tf32_peak = 0.5 * float(peaks.get("bf16_tflops") or 2250.0 * 0.75) * 1e12
+            e = kern["signal"]
+            e.update({"bound": "tensor", "pipe": "tf32", "achieved": flops / dur / 1e12, "peak": tf32_peak / 1e12,
+                      "unit": "TFLOP/s", "frac": flops / dur / tf32_peak,
+                      "algorithmic_ops_per_launch": flops * steps / kinds_n["signal"],
+                      "peak_source": "MEASURED_PEAKS.json bf16_tflops x 0.5 (nominal TF32 : BF16 ratio)" if peaks.get("bf16_tflops")
+                                     else "fallback: 0.75 x 2250 nominal bf16 TFLOP/s x 0.5",
+                      "note": f"{n_coils} coils on tcgen05 (kind::tf32, A operand generated into tensor memory): algorithmic "
+                              "8 flops per (spin, ADC sample, coil); the instruction count (6 MMAs of M128 x N x K8 per 8 spins, "
+                              "~74 clocks each whatever N) bounds the kernel, not the tensor pipe's flop rate"})
+            e.update(capture_fields(k_sig, "tf32"))
+        elif n_coils > 0:
             # multi-coil receive: sin / cos / ex2 are coil-independent; every coil adds one complex MAC = 4 FP32
             fp32_ops = (FP32_PER_EVAL + 4 * n_coils) * n_eval_sig
             if fp32_ops / fp32_peak > MUFU_PER_EVAL * n_eval_sig / mufu_peak:
