@@ -14,6 +14,8 @@
 //
 // The work per step is chosen per tile and per warp from a bound on q (tile header maxima x the spin's own
 // |x|, |y|, |z|, |dw|), so the hot loops are branch-free:
+//   tier -1 q <= 2^-14: series through q only (the q^2 terms are below q^2.5 / 120 = 2.4e-13 |M| per step: 2.4e-7 over the
+//                       1e6 steps of an MRF schedule), otherwise as tier 0 -- every pulse of the five configs
 //   tier 0  q <= 2^-8 : series through q^2 (truncation < 1.2e-11), state carried as hi + lo with the
 //                       increments summed in lo and folded into hi every 8 steps (error-free Fast2Sum)
 //   tier 1  q <= 1/4  : series through q^3 (truncation < 1.1e-8), Kahan-compensated state
@@ -36,7 +38,10 @@ struct RfRelax {
 
 template <int TIER>
 __device__ __forceinline__ void rf_series(float q, float &ca, float &cb) {
-    if (TIER == 0) {
+    if (TIER == -1) {
+        ca = fmaf(q, 1.0f / 6.0f, -1.0f);
+        cb = fmaf(q, -1.0f / 24.0f, 0.5f);
+    } else if (TIER == 0) {
         ca = fmaf(q, fmaf(q, -1.0f / 120.0f, 1.0f / 6.0f), -1.0f);
         cb = fmaf(q, fmaf(q, 1.0f / 720.0f, -1.0f / 24.0f), 0.5f);
     } else if (TIER == 1) {
@@ -74,6 +79,27 @@ __device__ __forceinline__ void rf_increment(float wx, float wy, float wz, float
     tx = fmaf(r.E2, dx, -r.D2 * mx);
     ty = fmaf(r.E2, dy, -r.D2 * my);
     tz = fmaf(r.E1, dz, fmaf(-r.D1, mz, r.D1m0));
+}
+
+// The same step for the hi + lo tiers (TIER <= 0), added straight into the low part: l <- l + E d - D m (+ D1 M0 z),
+// the sum folded into the FMAs that form the increment (two instructions per component instead of three).
+template <int TIER>
+__device__ __forceinline__ void rf_accumulate(float wx, float wy, float wz, float q, float mx, float my, float mz,
+                                              const RfRelax &r, float &lx, float &ly, float &lz) {
+    float ca, cb;
+    rf_series<TIER>(q, ca, cb);
+    const float ux = fmaf(wy, mz, -wz * my);  // u = w x M
+    const float uy = fmaf(wz, mx, -wx * mz);
+    const float uz = fmaf(wx, my, -wy * mx);
+    const float vx = fmaf(wy, uz, -wz * uy);  // v = w x u
+    const float vy = fmaf(wz, ux, -wx * uz);
+    const float vz = fmaf(wx, uy, -wy * ux);
+    const float dx = fmaf(ca, ux, cb * vx);
+    const float dy = fmaf(ca, uy, cb * vy);
+    const float dz = fmaf(ca, uz, cb * vz);
+    lx = fmaf(r.E2, dx, fmaf(-r.D2, mx, lx));
+    ly = fmaf(r.E2, dy, fmaf(-r.D2, my, ly));
+    lz = fmaf(r.E1, dz, fmaf(-r.D1, mz, lz + r.D1m0));
 }
 
 __device__ __forceinline__ void kahan_add(float &m, float &c, float d) {
@@ -120,23 +146,19 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
         wz = fmaf(h.x, sp.vx, fmaf(h.y, sp.vy, fmaf(h.z, sp.vz, wz)));                \
         q = fmaf(wz, wz, a.z);                                                        \
     }
-    if (TIER == 0) {
+    if (TIER <= 0) {
         int k = 0;
         for (; k + 8 <= n; k += 8) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 BLOCH_RF_LOAD(k + j)
-                float tx, ty, tz;
-                rf_increment<0>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, tx, ty, tz);
-                lx += tx; ly += ty; lz += tz;
+                rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
             }
             fold(hx, lx); fold(hy, ly); fold(hz, lz);
         }
         for (; k < n; ++k) {
             BLOCH_RF_LOAD(k)
-            float tx, ty, tz;
-            rf_increment<0>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, tx, ty, tz);
-            lx += tx; ly += ty; lz += tz;
+            rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
         }
         fold(hx, lx); fold(hy, ly); fold(hz, lz);
     } else {
@@ -159,8 +181,8 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
 // is warp-uniform and the same for both spins, so it is loaded once, and the two spins' cross products sit next to
 // each other in the instruction stream with wx, wy in the same operand slot (the operand-reuse cache can then serve
 // the second read: the RF step is bound by register-file operand bandwidth).  Each spin's own
-// arithmetic is rf_increment<0> exactly as in rf_tile<0, MODE>, so the result is bitwise that of one spin per thread.
-template <int MODE>
+// arithmetic is rf_accumulate<TIER> exactly as in rf_tile<TIER, MODE>, so the result is bitwise that of one spin per thread.
+template <int TIER, int MODE>
 __device__ __forceinline__ void rf_tile0_pair(const unsigned char *tile, const RfTileHdr &hd, const RfSpin &sa,
                                               const RfSpin &sb, const RfRelax &ra, const RfRelax &rb, float (&h)[6],
                                               float (&l)[6]) {
@@ -184,10 +206,8 @@ __device__ __forceinline__ void rf_tile0_pair(const unsigned char *tile, const R
             wzb = fmaf(g.x, sb.x, fmaf(g.y, sb.y, fmaf(g.z, sb.z, dtdw_b)));                           \
             qa = fmaf(wza, wza, a.z); qb = fmaf(wzb, wzb, a.z);                                        \
         }                                                                                              \
-        float ta0, ta1, ta2, tb0, tb1, tb2;                                                            \
-        rf_increment<0>(wx, wy, wza, qa, h[0] + l[0], h[1] + l[1], h[2] + l[2], ra, ta0, ta1, ta2);    \
-        rf_increment<0>(wx, wy, wzb, qb, h[3] + l[3], h[4] + l[4], h[5] + l[5], rb, tb0, tb1, tb2);    \
-        l[0] += ta0; l[1] += ta1; l[2] += ta2; l[3] += tb0; l[4] += tb1; l[5] += tb2;                  \
+        rf_accumulate<TIER>(wx, wy, wza, qa, h[0] + l[0], h[1] + l[1], h[2] + l[2], ra, l[0], l[1], l[2]);    \
+        rf_accumulate<TIER>(wx, wy, wzb, qb, h[3] + l[3], h[4] + l[4], h[5] + l[5], rb, l[3], l[4], l[5]);    \
     }
     int k = 0;
     for (; k + 8 <= n; k += 8) {
@@ -203,6 +223,7 @@ __device__ __forceinline__ void rf_tile0_pair(const unsigned char *tile, const R
 }
 
 constexpr int kRfMaxThreads = 128;
+constexpr float kRfQLin = 6.103515625e-05f;  // 2^-14: below it the series of a, b stop at the term linear in q (tier -1)
 
 // MO: motion plans (48-B step records, velocities); the static instantiation keeps its registers and shared
 // memory (48 registers, 8.3 KB) so that 10 CTAs of 128 threads fit an SM.
@@ -260,7 +281,8 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         if (MO) wzb = fmaf(hd.hx_max, avx, fmaf(hd.hy_max, avy, fmaf(hd.hz_max, avz, wzb)));
         const float qb = fmaf(wzb, wzb, hd.wxy2_max);
         const int mode = MO ? 2 : ((hd.flags & kRfFlagUniformG) ? 0 : 1);  // motion plans hold motion tiles only
-        const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
+        const int tier = __all_sync(0xffffffffu, qb <= kRfQLin) ? -1
+                         : (__all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2));
 #define BLOCH_RF_TILE(T, M) rf_tile<T, M>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz)
 #define BLOCH_RF_MODES(T)                       \
     do {                                        \
@@ -268,7 +290,8 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
         else if (mode == 0) BLOCH_RF_TILE(T, 0);\
         else BLOCH_RF_TILE(T, 1);               \
     } while (0)
-        if (tier == 0) BLOCH_RF_MODES(0);
+        if (tier == -1) BLOCH_RF_MODES(-1);
+        else if (tier == 0) BLOCH_RF_MODES(0);
         else if (tier == 1) BLOCH_RF_MODES(1);
         else BLOCH_RF_MODES(2);
 #undef BLOCH_RF_MODES
@@ -334,9 +357,12 @@ rf_pair_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop,
         const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
         const float qb = fmaf(wzb, wzb, hd.wxy2_max);
         const bool uni = (hd.flags & kRfFlagUniformG) != 0;
-        if (__all_sync(0xffffffffu, qb <= 0.00390625f)) {
-            if (uni) rf_tile0_pair<0>(tile, hd, sa, sb, ra, rb, h, l);
-            else rf_tile0_pair<1>(tile, hd, sa, sb, ra, rb, h, l);
+        if (__all_sync(0xffffffffu, qb <= kRfQLin)) {
+            if (uni) rf_tile0_pair<-1, 0>(tile, hd, sa, sb, ra, rb, h, l);
+            else rf_tile0_pair<-1, 1>(tile, hd, sa, sb, ra, rb, h, l);
+        } else if (__all_sync(0xffffffffu, qb <= 0.00390625f)) {
+            if (uni) rf_tile0_pair<0, 0>(tile, hd, sa, sb, ra, rb, h, l);
+            else rf_tile0_pair<0, 1>(tile, hd, sa, sb, ra, rb, h, l);
         } else {
             const int tier = __all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2;
 #define BLOCH_RF_ONE(T, M, SP, RX, O) rf_tile<T, M>(tile, hd, SP, RX, h[O], h[O + 1], h[O + 2], l[O], l[O + 1], l[O + 2])

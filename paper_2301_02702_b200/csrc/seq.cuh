@@ -302,14 +302,16 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                     const float wzb = fmaf(hd.gx_max, ax, fmaf(hd.gy_max, ay, fmaf(hd.gz_max, az, hd.dt * adw)));
                     const float qb = fmaf(wzb, wzb, hd.wxy2_max);
                     const bool uni = (hd.flags & kRfFlagUniformG) != 0;
-                    const int tier = __all_sync(0xffffffffu, qb <= 0.00390625f) ? 0
-                                     : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2);
+                    const int tier = __all_sync(0xffffffffu, qb <= kRfQLin) ? -1
+                                     : (__all_sync(0xffffffffu, qb <= 0.00390625f) ? 0
+                                        : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2));
 #define BLOCH_SEQ_TILE(T)                                                          \
     do {                                                                           \
         if (uni) rf_tile<T, 0>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);          \
         else rf_tile<T, 1>(tile, hd, sp, rx, hx, hy, hz, lx, ly, lz);              \
     } while (0)
-                    if (tier == 0) BLOCH_SEQ_TILE(0);
+                    if (tier == -1) BLOCH_SEQ_TILE(-1);
+                    else if (tier == 0) BLOCH_SEQ_TILE(0);
                     else if (tier == 1) BLOCH_SEQ_TILE(1);
                     else BLOCH_SEQ_TILE(2);
 #undef BLOCH_SEQ_TILE
