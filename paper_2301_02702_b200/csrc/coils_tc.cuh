@@ -145,14 +145,14 @@ signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 
     constexpr int kTcBTile = tc_btile(NC), kTcBGroup = tc_bgroup(NC), kTcSlotBytes = tc_slot(NC), kTcSlots = tc_slots(NC);
     constexpr uint32_t kIdesc = tc_idesc(2 * NC);
     static_assert(2 * NC <= kTcDCols, "accumulator columns");
-    // Consecutive MMAs into ONE accumulator serialise on it (~30 clocks each: measured, 8 coils 120 ms); chains into
-    // different accumulators overlap.  As many accumulators as the 64 reserved columns hold -- 4 for 8 coils (hi.hi and
-    // the two lo terms of the Cr and of the Ci products each on their own), 2 for 16 coils (Cr | Ci products), 1 for 32 --
-    // added up in the epilogue: 8 coils 120 -> 107 ms with two, see DESIGN.md for four.
+    // Accumulator columns, in groups of 2 NC that the epilogue adds up.  Up to 16 coils per pass the wide scheme is used
+    // (kWide, see the MMA issue loop): 8 coils: [Cr: hh + lh | Cr: hl | Ci: hh + lh | Ci: hl], 16 coils: [hh + lh | hl];
+    // 32 coils: one group.  (Separate accumulator chains by themselves change nothing: 8 coils on four chains 106.8 ms,
+    // 32 coils on one 107.7 ms.)
+    constexpr bool kWide = 4 * NC <= kTcDCols;
     constexpr int kAcc = kTcDCols / (2 * NC) >= 4 ? 4 : (kTcDCols / (2 * NC) >= 2 ? 2 : 1);
-    constexpr uint32_t kA1 = kAcc == 4 ? 2 * NC : 0;                           // Cr lo terms
-    constexpr uint32_t kA2 = kAcc == 4 ? 4 * NC : (kAcc == 2 ? 2 * NC : 0);    // Ci hi.hi
-    constexpr uint32_t kA3 = kAcc == 4 ? 6 * NC : kA2;                         // Ci lo terms
+    constexpr uint32_t kCi = kAcc == 4 ? 4 * NC : 0;        // the Ci products' own accumulator when there is room
+    constexpr uint32_t kIdescW = tc_idesc(4 * NC);          // N = 4 NC: [B hi | B lo]
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *slots = smem;                                    // [kTcSlots][spin A (256 B) | spin S (256 B) | B tiles]
     uint64_t *full = reinterpret_cast<uint64_t *>(slots + kTcSlots * kTcSlotBytes);  // [kTcSlots] TMA landed
@@ -214,12 +214,23 @@ signal_coils_tc_kernel(const float4 *__restrict__ recs, int n_pts, const float4 
                 for (int gq = 0; gq < kTcGroups; ++gq) {
                     const uint32_t ag = a0 + gq * 32, bg = b0 + gq * kTcBGroup;  // A parts: columns +0 cr hi, +8 cr lo, +16 ci hi, +24 ci lo
                     const uint32_t first = (st == 0 && gq == 0) ? 0u : 1u;  // 0: the accumulator's first MMA overwrites
-                    tc_mma_ts(tmem, ag + 0, tc_desc(bg + 0 * kTcBTile), kIdesc, first);                       // cr hi x B hi
-                    tc_mma_ts(tmem + kA2, ag + 16, tc_desc(bg + 2 * kTcBTile), kIdesc, kAcc >= 2 ? first : 1u); // ci hi x B' hi
-                    tc_mma_ts(tmem + kA1, ag + 8, tc_desc(bg + 0 * kTcBTile), kIdesc, kAcc == 4 ? first : 1u);  // cr lo x B hi
-                    tc_mma_ts(tmem + kA3, ag + 24, tc_desc(bg + 2 * kTcBTile), kIdesc, kAcc == 4 ? first : 1u); // ci lo x B' hi
-                    tc_mma_ts(tmem + kA1, ag + 0, tc_desc(bg + 1 * kTcBTile), kIdesc, 1u);                    // cr hi x B lo
-                    tc_mma_ts(tmem + kA3, ag + 16, tc_desc(bg + 3 * kTcBTile), kIdesc, 1u);                   // ci hi x B' lo
+                    if (kWide) {
+                        // An instruction costs the same for any N (~74 clocks), and the B tiles [B hi | B lo] lie side by
+                        // side along N: ONE instruction of N = 4 NC gives hi x B hi in the accumulator's first 2 NC
+                        // columns and hi x B lo in the next 2 NC; the lo x B hi product adds into the first 2 NC.
+                        // 4 instructions per 8 spins instead of 6; the column groups are added in the epilogue.
+                        tc_mma_ts(tmem, ag + 0, tc_desc(bg + 0 * kTcBTile), kIdescW, first);                      // cr hi x [B hi | B lo]
+                        tc_mma_ts(tmem + kCi, ag + 16, tc_desc(bg + 2 * kTcBTile), kIdescW, kCi ? first : 1u);    // ci hi x [B' hi | B' lo]
+                        tc_mma_ts(tmem, ag + 8, tc_desc(bg + 0 * kTcBTile), kIdesc, 1u);                          // cr lo x B hi
+                        tc_mma_ts(tmem + kCi, ag + 24, tc_desc(bg + 2 * kTcBTile), kIdesc, 1u);                   // ci lo x B' hi
+                    } else {
+                        tc_mma_ts(tmem, ag + 0, tc_desc(bg + 0 * kTcBTile), kIdesc, first);    // cr hi x B hi
+                        tc_mma_ts(tmem, ag + 16, tc_desc(bg + 2 * kTcBTile), kIdesc, 1u);      // ci hi x B' hi
+                        tc_mma_ts(tmem, ag + 8, tc_desc(bg + 0 * kTcBTile), kIdesc, 1u);       // cr lo x B hi
+                        tc_mma_ts(tmem, ag + 24, tc_desc(bg + 2 * kTcBTile), kIdesc, 1u);      // ci lo x B' hi
+                        tc_mma_ts(tmem, ag + 0, tc_desc(bg + 1 * kTcBTile), kIdesc, 1u);       // cr hi x B lo
+                        tc_mma_ts(tmem, ag + 16, tc_desc(bg + 3 * kTcBTile), kIdesc, 1u);      // ci hi x B' lo
+                    }
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mma_done[ab])) : "memory");
                 // refill the ring: the slot of stage st + kTcSlots - 1 held stage st - 1, whose MMAs must be complete
