@@ -32,7 +32,7 @@ typedef enum {
     BLOCH_OK = 0,
     BLOCH_EINVAL = -1,         /* NULL pointer, negative size, non-finite value, bad enum */
     BLOCH_ENONMONOTONIC = -2,  /* gradient vertex / RF sample / ADC times not ascending, or RF samples overlap */
-    BLOCH_EADC_IN_RF = -3,     /* an ADC time lies strictly inside an RF-active run (reading G7) */
+    BLOCH_EADC_IN_RF = -3,     /* (not returned any more: ADC samples inside an RF run are served, reading G7) */
     BLOCH_EWORKSPACE = -4,     /* workspace / table buffer too small or misaligned (256 B) */
     BLOCH_ECUDA = -5,          /* a CUDA runtime call failed; text in bloch_last_error() */
     BLOCH_EARCH = -6,          /* current device is not compute capability 10.x */

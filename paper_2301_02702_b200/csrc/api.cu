@@ -988,7 +988,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         prop.mx = b.mend[0];
         prop.my = b.mend[1];
         prop.mz = b.mend[2];
-        pending = true;
+        pending = b.count > 0;  // an empty block (an ADC sample inside an RF run) has nothing to propagate
     }
     if (d_Mxy) {
         if (pending) {

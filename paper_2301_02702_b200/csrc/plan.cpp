@@ -242,7 +242,19 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     const int64_t max_pts = params->max_block_points > 0 ? params->max_block_points : kDefaultMaxBlockPoints;
     std::vector<Block> blocks;
     {
+        // An ADC sample with RF on both sides of it (strictly inside an RF run, or at t = 0 / t_end of a sequence that
+        // starts / ends with RF) is served by an EMPTY precession block (no interval, tau = 0: the sample is Mxy as it
+        // stands, which is what the step-by-step integrator records, reading G7) that cuts the RF run in two.
+        auto empty_block = [&blocks](int64_t at) {
+            Block e;
+            e.type = kBlockPrecession;
+            e.first = at;
+            e.count = 0;
+            blocks.push_back(e);
+        };
+        auto inside_rf = [&](int64_t n) { return n > 0 && n < N && rf_of[n - 1] >= 0 && rf_of[n] >= 0 && adc_at[n] >= 0; };
         int64_t n = 0;
+        if (N > 0 && rf_of[0] >= 0 && adc_at[0] >= 0) empty_block(0);
         while (n < N) {
             Block b;
             b.type = rf_of[n] >= 0 ? kBlockRF : kBlockPrecession;
@@ -254,23 +266,22 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                     ++pts_in;
                 }
                 ++n;
+                if (b.type == kBlockRF && inside_rf(n)) break;
             }
             if (n == b.first) ++n;  // max_pts == 0 guard: always advance
             b.count = n - b.first;
             blocks.push_back(b);
+            if (b.type == kBlockRF && inside_rf(n)) empty_block(n);
         }
+        if (N > 0 && rf_of[N - 1] >= 0 && adc_at[N] >= 0) empty_block(N);
     }
-    // ADC assignment (reading G7): strictly inside an RF run -> error; on an RF/precession boundary ->
-    // served by the precession block (tau = 0 or tau = T); on a precession/precession cut -> the earlier.
+    // ADC assignment (reading G7): on an RF/precession boundary -> served by the precession block (tau = 0 or
+    // tau = T); on a precession/precession cut -> the earlier; with RF on both sides -> the empty block made above.
     for (size_t bi = 0; bi < blocks.size(); ++bi) {
         Block &b = blocks[bi];
         if (b.type == kBlockRF) {
             for (int64_t n = b.first + 1; n < b.first + b.count; ++n)
-                if (adc_at[n] >= 0) return fail(BLOCH_EADC_IN_RF, "ADC sample strictly inside an RF-active run");
-            if (bi == 0 && adc_at[0] >= 0)
-                return fail(BLOCH_EADC_IN_RF, "ADC sample at t = 0 with RF starting at t = 0");
-            if (bi + 1 == blocks.size() && adc_at[N] >= 0)
-                return fail(BLOCH_EADC_IN_RF, "ADC sample at t_end with RF ending at t_end");
+                if (adc_at[n] >= 0) return fail(BLOCH_EADC_IN_RF, "internal: ADC sample left inside an RF block");
             continue;
         }
         const bool serve_start = (bi == 0) || (blocks[bi - 1].type == kBlockRF);
@@ -526,7 +537,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             if (pending) ++launches;
             if (b.adc_count > 0) launches += (params->output_mode == BLOCH_OUT_SUM_ALL) ? 2 : 1;
             if (params->output_mode == BLOCH_OUT_SUM_ALL && b.lin_pts > 0 && b.lin_pts < b.adc_count) ++launches;  // tail
-            pending = true;
+            pending = b.count > 0;
         }
         if (pending) ++launches;
     }

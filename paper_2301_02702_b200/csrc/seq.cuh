@@ -347,7 +347,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                 }
                 const double4 k4 = *reinterpret_cast<const double4 *>(&ops[oi].kend[0]);
                 prop.kx = k4.x; prop.ky = k4.y; prop.kz = k4.z; prop.tau = k4.w;
-                pending = true;
+                pending = k4.w != 0.0;  // an empty block (an ADC sample inside an RF run) has nothing to propagate
             }
         }
         if (final_state) {

@@ -334,3 +334,35 @@ def test_two_spins_per_thread_rf_kernel_is_bitwise_the_one_spin_kernel(B, oracle
     b = run_gpu(B, w2, want_state=True, path="per_block", options={"rf_spins": 2})
     for u, v in zip(a, b):
         assert np.array_equal(np.asarray(u).view(np.float32), np.asarray(v).view(np.float32))
+
+
+@pytest.mark.parametrize("path", ["per_block", "fused"])
+def test_adc_samples_during_an_rf_pulse(B, oracle_mod, path):
+    """ADC samples strictly inside an RF run, at its first and at its last instant (reading G7: Mxy after the step that
+    ends at the sample's time): served through empty precession blocks that cut the run; signal and final state against
+    the oracle, which integrates straight through."""
+    from test_gpu_parity import run_gpu
+    n_rf, dt = 600, 2e-6
+    tm = (np.arange(n_rf) + 0.5) * dt
+    env = np.sinc(4.0 * (tm - n_rf * dt / 2) / (n_rf * dt))
+    b1 = env * np.deg2rad(80) / (W.GAMMA * dt * env.sum())
+    rf = (np.arange(n_rf) * dt, np.full(n_rf, dt), b1 * np.cos(0.3), b1 * np.sin(0.3))
+    t_rf = n_rf * dt
+    g = {2: ([0.0, t_rf, t_rf + 1e-4, t_rf + 3e-4, t_rf + 4e-4], [8e-3, 8e-3, 0.0, -6e-3, 0.0]),
+         0: ([t_rf + 4e-4, t_rf + 5e-4, t_rf + 1.5e-3], [0.0, 5e-3, 5e-3])}
+    adc = np.concatenate([[0.0], np.arange(1, 30) * 20 * dt, [t_rf - 3e-6 + 1e-6], [t_rf],
+                          t_rf + 5e-4 + np.arange(100) * 1e-5])
+    s = seq(g=g, rf=rf, adc=adc, t_end=t_rf + 1.5e-3, dt_rf_max=dt)
+    rng = np.random.default_rng(61)
+    n = 1111
+    ph = W._phantom(rng.uniform(-.08, .08, n), rng.uniform(-.08, .08, n), rng.uniform(-.004, .004, n),
+                    rng.uniform(.5, 1, n), rng.uniform(.3, 2, n), rng.uniform(.03, .3, n), rng.uniform(-200, 200, n))
+    w = W.Workload("adc_in_rf", ph, s, phase_mode="fp32")
+    got, gxy, gz = run_gpu(B, w, want_state=True, path=path)
+    ref, rxy, rz = oracle_mod.simulate(ph, s, return_state=True)
+    assert np.abs(ref[1:31]).max() > 0.05 * np.abs(ref).max()      # the in-pulse samples carry signal
+    emax, nrmse = errors(got, ref)
+    print(f"ADC inside RF, {path}: max {emax:.3e} nrmse {nrmse:.3e}")
+    assert emax <= 1e-4 and nrmse <= 1e-5
+    emax, nrmse = errors(np.concatenate([gxy, gz.astype(np.complex128)]), np.concatenate([rxy, rz.astype(np.complex128)]))
+    assert emax <= 1e-4 and nrmse <= 1e-5

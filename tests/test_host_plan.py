@@ -59,10 +59,6 @@ def test_plan_error_paths(B):
     with pytest.raises(B.BlochError) as e:
         B.bloch_plan_create(seq(**bad))
     assert e.value.code == -2
-    bad = dict(ok); bad["adc"] = [5e-5]                 # strictly inside the RF run
-    with pytest.raises(B.BlochError) as e:
-        B.bloch_plan_create(seq(**bad, dt_rf_max=1e-5))
-    assert e.value.code == -3
     bad = dict(ok); bad["rf"] = ([0.0, 5e-5], [1e-4, 1e-4], [1e-6, 1e-6], [0.0, 0.0])   # overlap
     with pytest.raises(B.BlochError) as e:
         B.bloch_plan_create(seq(**bad))
@@ -255,3 +251,20 @@ def test_waveform_motion_plan_merges_the_vertices_like_the_oracle(B, oracle_mod)
     h = B.bloch_plan_create(w.seq, motion="linear", dt_max=3e-5)
     assert B.bloch_plan_get_info(h)["n_intervals"] < info["n_intervals"]     # the inner vertices added points
     B.bloch_plan_destroy(h)
+
+
+def test_adc_samples_inside_an_rf_run_cut_it_with_empty_precession_blocks(B, oracle_mod):
+    """Reading G7: an ADC sample with RF on both sides is Mxy as it stands at that step boundary (what the oracle records).
+    The planner serves it with an EMPTY precession block that cuts the RF run; also at t = 0 and at t_end."""
+    n = 40
+    rf = (np.arange(n) * 1e-5, np.full(n, 1e-5), np.full(n, 2e-6), np.zeros(n))
+    s = seq(rf=rf, adc=[0.0, 5e-5, 1.3e-4, 1.35e-4, 4e-4], t_end=4e-4, dt_rf_max=1e-5)   # the RF run is the whole sequence
+    h = B.bloch_plan_create(s)
+    info = B.bloch_plan_get_info(h)
+    B.bloch_plan_destroy(h)
+    t, _, rfm, adc = oracle_mod.grid(s)
+    assert info["n_intervals"] == len(t) - 1 and info["n_rf_steps"] == int(rfm.sum())
+    # 1.35e-4 is not an RF sample edge: it becomes a grid point that splits one RF sample into two steps
+    assert info["n_rf_steps"] == n + 1
+    assert info["n_adc"] == 5 and info["n_rf_blocks"] == 4 and info["n_blocks"] == 9 and info["max_block_adc"] == 1
+    assert info["n_eval_points"] == info["n_adc"] + (info["n_blocks"] - info["n_rf_blocks"])
