@@ -17,6 +17,7 @@ from __future__ import annotations
 
 import argparse
 import glob
+import hashlib
 import json
 import os
 import re
@@ -55,13 +56,30 @@ def load_peaks():
 _SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 
 
+def csrc_sha256() -> str:
+    """Hash of the device code (every .cuh and internal.h under csrc/): a committed capture names the hash of the sources
+    it was taken from, and describes this binary only if that is still the hash of the sources."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2301_02702_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith(".cuh") or name == "internal.h":
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()
+
+
 def parse_ncu_txt(path: str):
     """One `ncu --set full` summary as committed under profiles/: 'kernel: [void ]NAME(args' then
     '  metric [unit] = value' lines.  Returns {"kernel", "grid", "block", "metrics": {name: (value, unit)}}."""
-    out = {"kernel": None, "grid": None, "block": None, "metrics": {}, "file": os.path.relpath(path, ROOT)}
+    out = {"kernel": None, "grid": None, "block": None, "metrics": {}, "file": os.path.relpath(path, ROOT), "csrc": None}
     try:
         with open(path) as f:
             for line in f:
+                m = re.match(r"#\s*csrc_sha256:\s*([0-9a-f]{64})", line)
+                if m:
+                    out["csrc"] = m.group(1)
+                    continue
                 m = re.match(r"\s*kernel:\s*(?:void\s+)?([^()]+)\(", line)
                 if m and out["kernel"] is None:
                     out["kernel"] = m.group(1).replace("bloch::", "").replace(" ", "")
@@ -77,16 +95,19 @@ def parse_ncu_txt(path: str):
 
 
 def find_capture(kernel: dict):
-    """The newest committed capture whose kernel name, grid and block size are those of the launch just timed
-    (bloch_plan_last_kernel), or None: a capture of another kernel, another build's template arguments or another
-    launch shape says nothing about this run."""
+    """The newest committed capture that describes the launch just timed: same kernel name, grid and block size
+    (bloch_plan_last_kernel) AND taken from the device sources as they stand (the `# csrc_sha256:` line of the capture
+    equals the hash of csrc/*.cuh now).  Anything else -- another kernel, other template arguments, another launch
+    shape, sources edited since the capture, a capture without a hash -- says nothing about this binary: None."""
     if not kernel or not kernel.get("name"):
         return None
     want = kernel["name"].replace(" ", "")
+    now = csrc_sha256()
     best = None
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu.txt"))):
         cap = parse_ncu_txt(path)
-        if cap and cap["kernel"] == want and cap["grid"] == kernel["grid"] and cap["block"] == kernel["block"]:
+        if cap and cap["kernel"] == want and cap["grid"] == kernel["grid"] and cap["block"] == kernel["block"] \
+                and cap["csrc"] == now:
             best = cap       # sorted by name: rNN_vM -> the latest round / version wins
     return best
 
@@ -96,8 +117,9 @@ def capture_fields(kernel: dict, pipe: str):
     cap = find_capture(kernel)
     if cap is None:
         return {"traffic": None, "traffic_source": None, "pipe_util": None, "issue_util": None,
-                "capture_note": f"no committed profiles/*_ncu.txt capture matches {kernel.get('name')} "
-                                f"grid {kernel.get('grid')} block {kernel.get('block')}"}
+                "capture_note": f"no committed profiles/*_ncu.txt capture of {kernel.get('name')} grid {kernel.get('grid')} "
+                                f"block {kernel.get('block')} was taken from the device sources as they stand "
+                                f"(csrc_sha256 {csrc_sha256()[:12]}...)"}
     m = cap["metrics"]
 
     def nbytes(key):
