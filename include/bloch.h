@@ -152,6 +152,11 @@ int bloch_plan_create(const bloch_scanner *scanner, const bloch_sequence *seq,
 int bloch_plan_destroy(bloch_plan *plan);
 int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out);
 
+/* The plan's table image in HOST memory: *h_tables points at table_bytes bytes owned by the plan (borrowed until it is
+ * destroyed) -- what bloch_plan_upload copies to the device.  For callers that upload by other means, and for tests
+ * that compare plans. */
+int bloch_plan_host_tables(const bloch_plan *plan, const void **h_tables, size_t *bytes);
+
 /* Bytes of caller-allocated device workspace bloch_simulate needs for n_spins (256-B aligned buffer). */
 int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out);
 
@@ -331,6 +336,30 @@ enum { BLOCH_STATUS_BAD_RELAXATION = 1, BLOCH_STATUS_NONFINITE = 2, BLOCH_STATUS
 int bloch_plan_status(const bloch_plan *plan, void *stream, int *flags);
 /* *out = 1 if bloch_simulate would take the fused path for n_spins on the current device, else 0. */
 int bloch_plan_uses_fused(const bloch_plan *plan, int64_t n_spins, int *out);
+
+/* Files (PAPER.md:93 Fig 1 "each arrow represents a file", :99-101).  The paper reads Pulseq sequence files and writes
+ * ISMRM Raw Data but fixes nothing of either format, and neither can be checked against anything here; these calls read
+ * and write THIS LIBRARY'S OWN line-oriented text container for exactly the arrays of bloch_scanner / bloch_sequence and
+ * for the raw samples (layout: csrc/io.cpp) -- not Pulseq, not ISMRMRD.  Numbers are C99 hexadecimal floating-point
+ * literals, so a round trip is bit-exact: a plan built from a file has bitwise the tables of a plan built from the
+ * arrays.  Host only; all pointers are HOST memory.
+ *   bloch_sequence_write      scanner may be NULL (zeros are written).
+ *   bloch_sequence_read       *out is owned by the library until bloch_sequence_file_free.
+ *   bloch_sequence_file_get   fills *scanner (may be NULL) and *seq with pointers INTO the file object (borrowed; valid
+ *                             until it is freed), ready for bloch_plan_create.
+ *   bloch_signal_write        h_signal: n_rows x n_adc interleaved (re, im) fp32 (rows = 1, coils, spins or groups);
+ *                             h_adc_t (n_adc sample times) may be NULL.
+ *   bloch_signal_read         with h_signal == NULL only *n_rows and *n_adc are returned; else capacity_complex >=
+ *                             n_rows x n_adc (BLOCH_EWORKSPACE otherwise); h_adc_t may be NULL.
+ * Errors: BLOCH_EINVAL (cannot open, malformed, wrong magic), BLOCH_ENOMEM. */
+typedef struct bloch_sequence_file bloch_sequence_file;
+int bloch_sequence_write(const char *path, const bloch_scanner *scanner, const bloch_sequence *seq);
+int bloch_sequence_read(const char *path, bloch_sequence_file **out);
+int bloch_sequence_file_get(const bloch_sequence_file *file, bloch_scanner *scanner, bloch_sequence *seq);
+int bloch_sequence_file_free(bloch_sequence_file *file);
+int bloch_signal_write(const char *path, const float *h_signal, int64_t n_rows, int64_t n_adc, const double *h_adc_t);
+int bloch_signal_read(const char *path, float *h_signal, int64_t capacity_complex, int64_t *n_rows, int64_t *n_adc,
+                      double *h_adc_t);
 
 /* Pipe micro-benchmarks used for the roofline denominators (MEASURED_PEAKS.json has only HBM and bf16):
  * kind 0 = MUFU (sin/cos/ex2 mix), 1 = FFMA (two operands reused), 2 = DFMA, 3 = FFMA with three different changing

@@ -64,7 +64,9 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_plan_last_timing", "bloch_plan_last_launches", "bloch_plan_set_path", "bloch_plan_uses_fused",
            "bloch_plan_workspace_bytes_coils", "bloch_simulate_coils", "bloch_simulate_host_coils_scratch_bytes",
            "bloch_simulate_host_coils", "bloch_plan_set_option", "bloch_plan_get_option", "bloch_plan_status",
-           "bloch_plan_last_kernel", "bloch_simulate_coils_motion", "bloch_simulate_host_coils_motion", "bloch_microbench"]
+           "bloch_plan_last_kernel", "bloch_simulate_coils_motion", "bloch_simulate_host_coils_motion", "bloch_sequence_write",
+           "bloch_sequence_read", "bloch_sequence_file_get", "bloch_sequence_file_free", "bloch_signal_write",
+           "bloch_signal_read", "bloch_plan_host_tables", "bloch_microbench"]
 
 
 def _load():
@@ -106,6 +108,13 @@ def _load():
     lib.bloch_plan_get_option.argtypes = [vp, C.c_int, C.POINTER(C.c_int)]
     lib.bloch_plan_status.argtypes = [vp, vp, C.POINTER(C.c_int)]
     lib.bloch_microbench.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), vp]
+    lib.bloch_plan_host_tables.argtypes = [vp, C.POINTER(vp), C.POINTER(sz)]
+    lib.bloch_sequence_write.argtypes = [C.c_char_p, C.POINTER(bloch_scanner), C.POINTER(bloch_sequence)]
+    lib.bloch_sequence_read.argtypes = [C.c_char_p, C.POINTER(vp)]
+    lib.bloch_sequence_file_get.argtypes = [vp, C.POINTER(bloch_scanner), C.POINTER(bloch_sequence)]
+    lib.bloch_sequence_file_free.argtypes = [vp]
+    lib.bloch_signal_write.argtypes = [C.c_char_p, _fp, i64, i64, _dp]
+    lib.bloch_signal_read.argtypes = [C.c_char_p, _fp, i64, C.POINTER(i64), C.POINTER(i64), _dp]
     for name in EXPORTS:
         if name not in ("bloch_strerror", "bloch_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -145,17 +154,7 @@ def _darr(a):
     return a, a.ctypes.data_as(_dp)
 
 
-def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
-                      max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
-                      group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0,
-                      max_extent_m: float = 0.0, max_offres_hz: float = 0.0, max_speed_mps: float = 0.0,
-                      waveform=None) -> int:
-    """G_max [T/m], S_max [T/m/s]: scanner limits the gradient waveforms are checked against when > 0.
-    max_extent_m / max_offres_hz / max_speed_mps: extents of the phantoms the plan will see (bloch_sim_params).
-    waveform: (t, u) vertex arrays of the shared motion waveform for motion="waveform" (x(t) = x + a u(t)).
-    seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
-    Returns the opaque plan handle (an integer address)."""
-    keep = []
+def _c_sequence(seq, keep):
     cs = bloch_sequence()
     for a in range(3):
         t, tp = _darr(seq.g_t[a]); v, vp_ = _darr(seq.g_v[a])
@@ -170,6 +169,72 @@ def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None
     ad, cs.adc_t = _darr(seq.adc_t)
     keep += [rt, rd, rr, ri, ad]
     cs.rf_n, cs.adc_n, cs.t_end = rt.shape[0], ad.shape[0], float(seq.t_end)
+    return cs
+
+
+def bloch_sequence_write(path: str, seq, *, gamma: float = 0.0, B0: float = 0.0, G_max: float = 0.0, S_max: float = 0.0):
+    """Writes scanner + sequence to the library's own text container (bit-exact; NOT Pulseq)."""
+    keep = []
+    cs = _c_sequence(seq, keep)
+    sc = bloch_scanner(float(gamma), float(B0), float(G_max), float(S_max))
+    _check(_lib.bloch_sequence_write(os.fsencode(path), C.byref(sc), C.byref(cs)))
+
+
+def bloch_sequence_read(path: str):
+    """-> (scanner dict, sequence object with numpy copies of g_t, g_v, rf_t, rf_dt, rf_re, rf_im, adc_t, t_end)."""
+    from types import SimpleNamespace
+    h = C.c_void_p()
+    _check(_lib.bloch_sequence_read(os.fsencode(path), C.byref(h)))
+    try:
+        sc, cs = bloch_scanner(), bloch_sequence()
+        _check(_lib.bloch_sequence_file_get(h, C.byref(sc), C.byref(cs)))
+
+        def arr(p, n):
+            return np.ctypeslib.as_array(p, shape=(n,)).copy() if n else np.zeros(0)
+        seq = SimpleNamespace(g_t=[arr(cs.g_t[a], cs.g_n[a]) for a in range(3)],
+                              g_v=[arr(cs.g_v[a], cs.g_n[a]) for a in range(3)],
+                              rf_t=arr(cs.rf_t, cs.rf_n), rf_dt=arr(cs.rf_dt, cs.rf_n), rf_re=arr(cs.rf_re, cs.rf_n),
+                              rf_im=arr(cs.rf_im, cs.rf_n), adc_t=arr(cs.adc_t, cs.adc_n), t_end=float(cs.t_end))
+        scanner = dict(gamma=sc.gamma, B0=sc.B0, G_max=sc.G_max, S_max=sc.S_max)
+    finally:
+        _lib.bloch_sequence_file_free(h)
+    return scanner, seq
+
+
+def bloch_signal_write(path: str, signal, adc_t=None):
+    """signal: complex64 numpy array [n_adc] or [rows, n_adc]; adc_t optional float64 [n_adc]."""
+    sig = np.ascontiguousarray(signal, dtype=np.complex64)
+    rows, n_adc = (1, sig.shape[0]) if sig.ndim == 1 else (sig.shape[0], sig.shape[1])
+    t = None if adc_t is None else np.ascontiguousarray(adc_t, dtype=np.float64)
+    if t is not None and t.shape != (n_adc,):
+        raise ValueError("adc_t must hold n_adc times")
+    _check(_lib.bloch_signal_write(os.fsencode(path), sig.ctypes.data, rows, n_adc,
+                                   None if t is None else t.ctypes.data_as(_dp)))
+
+
+def bloch_signal_read(path: str):
+    """-> (complex64 [rows, n_adc], adc_t float64 [n_adc])."""
+    rows, n_adc = C.c_int64(), C.c_int64()
+    _check(_lib.bloch_signal_read(os.fsencode(path), None, 0, C.byref(rows), C.byref(n_adc), None))
+    sig = np.zeros((rows.value, n_adc.value), dtype=np.complex64)
+    t = np.zeros(n_adc.value, dtype=np.float64)
+    _check(_lib.bloch_signal_read(os.fsencode(path), sig.ctypes.data, sig.size, C.byref(rows), C.byref(n_adc),
+                                  t.ctypes.data_as(_dp)))
+    return sig, t
+
+
+def bloch_plan_create(seq, *, gamma: float = 0.0, dt_rf_max: float | None = None, dt_max: float = 0.0,
+                      max_block_points: int = 0, phase_mode="auto", output_mode="sum", motion="none",
+                      group_size: int = 0, G_max: float = 0.0, S_max: float = 0.0, B0: float = 0.0,
+                      max_extent_m: float = 0.0, max_offres_hz: float = 0.0, max_speed_mps: float = 0.0,
+                      waveform=None) -> int:
+    """G_max [T/m], S_max [T/m/s]: scanner limits the gradient waveforms are checked against when > 0.
+    max_extent_m / max_offres_hz / max_speed_mps: extents of the phantoms the plan will see (bloch_sim_params).
+    waveform: (t, u) vertex arrays of the shared motion waveform for motion="waveform" (x(t) = x + a u(t)).
+    seq: object with g_t, g_v (3 arrays each), rf_t, rf_dt, rf_re, rf_im, adc_t, t_end[, dt_rf_max].
+    Returns the opaque plan handle (an integer address)."""
+    keep = []
+    cs = _c_sequence(seq, keep)
     if dt_rf_max is None:
         dt_rf_max = float(getattr(seq, "dt_rf_max", 0.0))
     sc = bloch_scanner(float(gamma), float(B0), float(G_max), float(S_max))
@@ -204,6 +269,13 @@ def bloch_plan_get_info(plan: int) -> dict:
         else:
             out[k] = float(v) if tp is C.c_double else int(v)
     return out
+
+
+def bloch_plan_host_tables(plan: int) -> bytes:
+    """A copy of the plan's table image (what bloch_plan_upload sends to the device)."""
+    ptr, n = C.c_void_p(), C.c_size_t()
+    _check(_lib.bloch_plan_host_tables(plan, C.byref(ptr), C.byref(n)))
+    return C.string_at(ptr.value, n.value)
 
 
 def bloch_plan_workspace_bytes(plan: int, n_spins: int) -> int:

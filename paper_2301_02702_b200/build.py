@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libbloch_b200.so")
-SOURCES = ["api.cu", "plan.cpp"]
+SOURCES = ["api.cu", "plan.cpp", "io.cpp"]
 DEPS = SOURCES + ["coils.cuh", "coils_tc.cuh", "kernels.cuh", "rf.cuh", "seq.cuh", "signal.cuh", "tma.cuh", "internal.h", os.path.join("..", "..", "include", "bloch.h")]
 
 

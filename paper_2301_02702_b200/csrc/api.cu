@@ -496,6 +496,13 @@ int bloch_plan_get_info(const bloch_plan *plan, bloch_plan_info *out) {
     return BLOCH_OK;
 }
 
+int bloch_plan_host_tables(const bloch_plan *plan, const void **h_tables, size_t *bytes) {
+    if (!plan || !h_tables || !bytes) return fail(BLOCH_EINVAL, "NULL argument");
+    *h_tables = plan->tables.data();
+    *bytes = plan->tables.size();
+    return BLOCH_OK;
+}
+
 int bloch_plan_workspace_bytes(const bloch_plan *plan, int64_t n_spins, size_t *out) {
     return bloch_plan_workspace_bytes_coils(plan, n_spins, 0, out);
 }
