@@ -135,6 +135,50 @@ __device__ __forceinline__ void propagate(const PropRec &p, const float4 &a, con
     mz = __fmaf_rn(__fsub_rn(mz, c.z), e1, c.z);  // Eq 11
 }
 
+// One evaluated point of a precession block for the accurate (per-spin / grouped) readouts: its record as doubles in
+// turns/m and seconds, whatever the table's format (fp64-phase tables hold turns/m, fp32-phase tables rad/m), and the
+// first-moment record that follows it in motion plans.
+struct PointRec {
+    double kx, ky, kz, tau, ux, uy, uz;
+};
+template <bool PH64>
+__device__ __forceinline__ PointRec load_point(const void *__restrict__ recs_, int p, bool motion) {
+    PointRec r;
+    r.ux = 0.; r.uy = 0.; r.uz = 0.;
+    const int rs = motion ? 2 : 1;  // motion plans: (k', tau) is followed by (mu', 0)
+    if (PH64) {
+        const double4 q = reinterpret_cast<const double4 *>(recs_)[rs * p];
+        r.kx = q.x; r.ky = q.y; r.kz = q.z; r.tau = q.w;
+        if (motion) {
+            const double4 m = reinterpret_cast<const double4 *>(recs_)[rs * p + 1];
+            r.ux = m.x; r.uy = m.y; r.uz = m.z;
+        }
+    } else {
+        const float4 q = reinterpret_cast<const float4 *>(recs_)[rs * p];
+        r.kx = (double)q.x * 0.15915494309189535; r.ky = (double)q.y * 0.15915494309189535;
+        r.kz = (double)q.z * 0.15915494309189535; r.tau = q.w;
+        if (motion) {
+            const float4 m = reinterpret_cast<const float4 *>(recs_)[rs * p + 1];
+            r.ux = (double)m.x * 0.15915494309189535; r.uy = (double)m.y * 0.15915494309189535;
+            r.uz = (double)m.z * 0.15915494309189535;
+        }
+    }
+    return r;
+}
+
+// c_in = Mxy(0) exp(-tau/T2) exp(i theta) of one spin at one point, accurate functions, phase in fp64 turns
+__device__ __forceinline__ float2 accurate_contribution(const PointRec &r, const float4 &a, const float4 &c, const float4 &s,
+                                                        const float4 *v) {
+    double th = r.kx * (double)a.x + r.ky * (double)a.y + r.kz * (double)a.z - (double)c.w * 0.15915494309189535 * r.tau;
+    if (v) th += r.ux * (double)v->x + r.uy * (double)v->y + r.uz * (double)v->z;
+    th -= rint(th);
+    float sn, cs;
+    sincospif(2.0f * (float)th, &sn, &cs);
+    const float e = expf(-(float)r.tau * c.y);
+    const float er = s.x * e, ei = s.y * e;
+    return make_float2(er * cs - ei * sn, er * sn + ei * cs);
+}
+
 // PER_SPIN output (dictionary mode): one thread per (spin, point); accurate functions because nothing
 // averages the per-evaluation error; phase in fp64 turns.  recs are float4 or double4 by PH64.
 template <bool PH64>
@@ -145,37 +189,11 @@ perspin_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restri
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)n_spins * n_pts) return;
     const int sp = (int)(gid / n_pts), p = (int)(gid % n_pts);
-    double kx, ky, kz, tau, ux = 0., uy = 0., uz = 0.;
-    const int rs = V ? 2 : 1;  // motion plans: (k', tau) is followed by (mu', 0)
-    if (PH64) {
-        const double4 r = reinterpret_cast<const double4 *>(recs_)[rs * p];
-        kx = r.x; ky = r.y; kz = r.z; tau = r.w;
-        if (V) {
-            const double4 m = reinterpret_cast<const double4 *>(recs_)[rs * p + 1];
-            ux = m.x; uy = m.y; uz = m.z;
-        }
-    } else {
-        const float4 r = reinterpret_cast<const float4 *>(recs_)[rs * p];  // fp32-phase tables hold k' in rad/m
-        kx = (double)r.x * 0.15915494309189535; ky = (double)r.y * 0.15915494309189535;
-        kz = (double)r.z * 0.15915494309189535; tau = r.w;
-        if (V) {
-            const float4 m = reinterpret_cast<const float4 *>(recs_)[rs * p + 1];
-            ux = (double)m.x * 0.15915494309189535; uy = (double)m.y * 0.15915494309189535;
-            uz = (double)m.z * 0.15915494309189535;
-        }
-    }
+    const PointRec r = load_point<PH64>(recs_, p, V != nullptr);
     const float4 a = A[sp], c = Cc[sp], s = S[sp];
-    double th = kx * (double)a.x + ky * (double)a.y + kz * (double)a.z - (double)c.w * 0.15915494309189535 * tau;
-    if (V) {
-        const float4 v = V[sp];
-        th += ux * (double)v.x + uy * (double)v.y + uz * (double)v.z;
-    }
-    th -= rint(th);
-    float sn, cs;
-    sincospif(2.0f * (float)th, &sn, &cs);
-    const float e = expf(-(float)tau * c.y);
-    const float er = s.x * e, ei = s.y * e;
-    out[(size_t)sp * n_adc_total + adc_first + p] = make_float2(er * cs - ei * sn, er * sn + ei * cs);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (V) v = V[sp];
+    out[(size_t)sp * n_adc_total + adc_first + p] = accurate_contribution(r, a, c, s, V ? &v : nullptr);
 }
 
 // GROUPED output: one warp per group of `gs` consecutive spins (an isochromat ensemble);
@@ -189,43 +207,17 @@ grouped_kernel(const void *__restrict__ recs_, int n_pts, const float4 *__restri
                int n_groups, int gs, long long n_adc_total, long long adc_first, float2 *__restrict__ out) {
     const int warp = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (warp >= n_groups) return;
-    const int rs = V ? 2 : 1;
     const long long s0 = (long long)warp * gs;
     for (int p = 0; p < n_pts; ++p) {
-        double kx, ky, kz, tau, ux = 0., uy = 0., uz = 0.;
-        if (PH64) {
-            const double4 r = reinterpret_cast<const double4 *>(recs_)[rs * p];
-            kx = r.x; ky = r.y; kz = r.z; tau = r.w;
-            if (V) {
-                const double4 m = reinterpret_cast<const double4 *>(recs_)[rs * p + 1];
-                ux = m.x; uy = m.y; uz = m.z;
-            }
-        } else {
-            const float4 r = reinterpret_cast<const float4 *>(recs_)[rs * p];
-            kx = (double)r.x * 0.15915494309189535; ky = (double)r.y * 0.15915494309189535;
-            kz = (double)r.z * 0.15915494309189535; tau = r.w;
-            if (V) {
-                const float4 m = reinterpret_cast<const float4 *>(recs_)[rs * p + 1];
-                ux = (double)m.x * 0.15915494309189535; uy = (double)m.y * 0.15915494309189535;
-                uz = (double)m.z * 0.15915494309189535;
-            }
-        }
+        const PointRec r = load_point<PH64>(recs_, p, V != nullptr);
         float re = 0.f, im = 0.f;
         for (int k = lane; k < gs; k += 32) {
             const float4 a = A[s0 + k], c = Cc[s0 + k], s = S[s0 + k];
-            double th = kx * (double)a.x + ky * (double)a.y + kz * (double)a.z -
-                        (double)c.w * 0.15915494309189535 * tau;
-            if (V) {
-                const float4 v = V[s0 + k];
-                th += ux * (double)v.x + uy * (double)v.y + uz * (double)v.z;
-            }
-            th -= rint(th);
-            float sn, cs;
-            sincospif(2.0f * (float)th, &sn, &cs);
-            const float e = expf(-(float)tau * c.y);
-            const float er = s.x * e, ei = s.y * e;
-            re += er * cs - ei * sn;
-            im += er * sn + ei * cs;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (V) v = V[s0 + k];
+            const float2 w = accurate_contribution(r, a, c, s, V ? &v : nullptr);
+            re += w.x;
+            im += w.y;
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

@@ -324,18 +324,12 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                 if (PS && tn.y > 0) {
                     // PER_SPIN output (dictionary mode; blocks of a few samples): the spin's own thread evaluates
                     // them with the accurate functions and fp64 phase of perspin_kernel -- no signal warps
-                    const float4 *recs = reinterpret_cast<const float4 *>(tables + ops[oi].table_off);
+                    const void *recs = tables + ops[oi].table_off;
                     float2 *row = out_ps + (size_t)i * (size_t)n_adc + ops[oi].adc_first;
+                    const float4 now = make_float4(hx, hy, hz, s.w);
                     for (int p = 0; p < tn.y; ++p) {
-                        const float4 rc = recs[p];  // k' in rad/m, tau
-                        double th = ((double)rc.x * (double)a.x + (double)rc.y * (double)a.y + (double)rc.z * (double)a.z) *
-                                        0.15915494309189535 - (double)c.w * 0.15915494309189535 * (double)rc.w;
-                        th -= rint(th);
-                        float sn, cs;
-                        sincospif(2.0f * (float)th, &sn, &cs);
-                        const float e = expf(-rc.w * c.y);
-                        const float er = hx * e, ei = hy * e;
-                        if (active) row[p] = make_float2(er * cs - ei * sn, er * sn + ei * cs);
+                        const float2 w = accurate_contribution(load_point<false>(recs, p, false), a, c, now, nullptr);
+                        if (active) row[p] = w;
                     }
                 } else if (tn.y > 0) {  // publish the block-start state for the signal warps
                     const int b = pub % kSeqStateBufs, use = pub / kSeqStateBufs;
