@@ -36,6 +36,7 @@
 #include "internal.h"
 #include "kernels.cuh"
 #include "rf.cuh"
+#include "signal.cuh"
 #include "tma.cuh"
 
 namespace bloch {
@@ -140,41 +141,8 @@ __device__ __forceinline__ void seq_signal_item(const float4 *__restrict__ recs,
     const bool geom = P > 2 && series && __all_sync(0xffffffffu, dev * r2max_log2e <= 1e-6f);
     auto run = [&](auto mode_tag) {
         constexpr int MODE = decltype(mode_tag)::value;  // 0: MUFU.EX2 per sample, 1: series per sample, 2: geometric
-        constexpr bool SERIES = MODE != 0;
 #pragma unroll 2
-        for (int s = 0; s < cnt; ++s) {
-            const float4 a = shA[s];
-            const float4 st = shS[s];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
-            float er0 = 0.f, ei0 = 0.f, qd = 1.f;
-            if (MODE == 2) {
-                const float y = cj[1] * st.w;  // -dwell/T2
-                qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
-            }
-#pragma unroll
-            for (int j = 0; j < P; ++j) {
-                const float th = fmaf(kx[j], a.x, fmaf(ky[j], a.y, fmaf(kz[j], a.z, tau[j] * a.w)));  // radians
-                const float sn = __sinf(th), cs = __cosf(th);
-                float er, ei;
-                if (j == 0 || !SERIES) {
-                    const float e = ex2_approx(tau[j] * st.w);
-                    er = st.x * e;
-                    ei = st.y * e;
-                    if (j == 0) { er0 = er; ei0 = ei; }
-                } else if (MODE == 2) {
-                    er0 *= qd;
-                    ei0 *= qd;
-                    er = er0;
-                    ei = ei0;
-                } else {
-                    const float y = cj[j] * st.w;
-                    const float pe = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
-                    er = er0 * pe;
-                    ei = ei0 * pe;
-                }
-                ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
-                ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
-            }
-        }
+        for (int s = 0; s < cnt; ++s) signal_spin_fp32<P, MODE>(kx, ky, kz, tau, cj, shA[s], shS[s], ar, ai);
     };
     if (geom) run(std::integral_constant<int, 2>{});
     else if (series) run(std::integral_constant<int, 1>{});

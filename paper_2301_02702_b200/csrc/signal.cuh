@@ -36,6 +36,45 @@ namespace bloch {
 constexpr int kSigThreads = 256;
 constexpr int kSigTile = 256;  // spins per staged tile
 
+// fp32 phase, static spins: the contributions of ONE spin to a thread's P adjacent samples, added into (ar, ai).  The one
+// copy of this arithmetic: signal_kernel and the signal warps of the whole-sequence kernel (seq.cuh) both call it.
+// MODE 0: one MUFU.EX2 per sample, 1: decay of sample j from sample 0 by the cubic series, 2: geometric decay.
+// a = (x, y, z, f'), st = (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2); k' in rad/m, cj[j] = (tau_j - tau_0) ln 2.
+template <int P, int MODE>
+__device__ __forceinline__ void signal_spin_fp32(const float (&kx)[P], const float (&ky)[P], const float (&kz)[P],
+                                                 const float (&tau)[P], const float (&cj)[P], const float4 &a,
+                                                 const float4 &st, float (&ar)[P], float (&ai)[P]) {
+    float er0 = 0.f, ei0 = 0.f, qd = 1.f;
+    if (MODE == 2) {
+        const float y = cj[1] * st.w;  // -dwell/T2
+        qd = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        const float th = fmaf(kx[j], a.x, fmaf(ky[j], a.y, fmaf(kz[j], a.z, tau[j] * a.w)));  // radians
+        const float sn = __sinf(th), cs = __cosf(th);  // FMUL by 1/(2 pi) + MUFU.SIN / MUFU.COS
+        float er, ei;
+        if (j == 0 || MODE == 0) {
+            const float e = ex2_approx(tau[j] * st.w);  // MUFU.EX2: exp(-tau/T2)
+            er = st.x * e;
+            ei = st.y * e;
+            if (j == 0) { er0 = er; ei0 = ei; }
+        } else if (MODE == 2) {
+            er0 *= qd;  // running product: exp(-(tau_0 + j dwell)/T2)
+            ei0 *= qd;
+            er = er0;
+            ei = ei0;
+        } else {
+            const float y = cj[j] * st.w;  // -(tau_j - tau_0)/T2
+            const float pe = fmaf(y, fmaf(y, fmaf(y, 1.0f / 6.0f, 0.5f), 1.0f), 1.0f);
+            er = er0 * pe;
+            ei = ei0 * pe;
+        }
+        ar[j] = fmaf(er, cs, fmaf(-ei, sn, ar[j]));
+        ai[j] = fmaf(er, sn, fmaf(ei, cs, ai[j]));
+    }
+}
+
 // MO (motion plans): every record (k', tau) is followed by (mu', 0), the spins' velocities are a third staged
 // tile, and the phase gains mu' . v (x(t) = x + v t).
 // fp32 phase, static plans: held to 64 registers (P <= 4: 4 CTAs per SM) or 85 (P = 8: 3 CTAs per SM); ptxas otherwise
@@ -213,6 +252,12 @@ signal_kernel(const void *__restrict__ recs_, int n_pts, const void *__restrict_
                     ai[j] += wi[j];
                 }
                 continue;
+            }
+            if constexpr (!PH64 && !MO) {
+                if (MODE < 3) {
+                    signal_spin_fp32<P, MODE < 3 ? MODE : 0>(kx, ky, kz, tau, cj, a, st, ar, ai);
+                    continue;
+                }
             }
 #pragma unroll
             for (int j = 0; j < P; ++j) {
