@@ -524,6 +524,9 @@ def run_ours(args, rank, local_rank, world):
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
     torch.cuda.set_device(local_rank)
     if world > 1:
+        # communicator lines ("NCCL INFO ...") are the evidence that NCCL carried the one collective of the path; the
+        # JSON result stays ONE line of its own on rank 0's stdout
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2301_02702_b200 import build as bl
     if rank == 0:
