@@ -333,7 +333,7 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
                       "peak_source": "MEASURED_PEAKS.json bf16_tflops x 0.5 (nominal TF32 : BF16 ratio)" if peaks.get("bf16_tflops")
                                      else "fallback: 0.75 x 2250 nominal bf16 TFLOP/s x 0.5",
                       "note": f"{n_coils} coils on tcgen05 (kind::tf32, A operand generated into tensor memory): algorithmic "
-                              "8 flops per (spin, ADC sample, coil); the instruction count (6 MMAs of M128 x N x K8 per 8 spins, "
+                              "8 flops per (spin, ADC sample, coil); the instruction count (4 MMAs of M128 x N x K8 per 8 spins, "
                               "~74 clocks each whatever N) bounds the kernel, not the tensor pipe's flop rate"})
             e.update(capture_fields(k_sig, "tf32"))
         elif n_coils > 0:
@@ -347,7 +347,7 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
     if kinds_n["rf"]:
         kern["rf"] = entry("rf", "fp32", FP32_PER_RF_STEP * rf_steps,
                            "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly); the "
-                           "tier-0 loop issues ~38.5 per step on plateau-gradient tiles")
+                           "small-angle loop (q <= 2^-14: every pulse of the configs) issues 31 FP + ~4 other per step, so frac can pass 1")
     if kinds_n["fused"]:
         # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
         # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)

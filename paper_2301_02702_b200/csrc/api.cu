@@ -188,8 +188,11 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     // (the producer's sub-partition 0 takes an extra one last) and every sub-partition gets sig_base signal warps plus
     // sig_extra for every RF warp it holds fewer than the fullest one, so that all four carry about the same load.
     // Measured on config 5 (14 RF warps: 3,4,4,3): signal warps 3,1,1,3 124.1 ms; 3,2,2,3 125.9; 2,1,1,2 128.4;
-    // 1,1,1,1 144.8; 2,2,2,2 133.6; 5,1,1,5 127.0.  Default: two extra per missing RF warp, and a base that brings the
-    // total to about 0.6 signal warps per RF warp.
+    // 1,1,1,1 144.8; 2,2,2,2 133.6; 5,1,1,5 127.0.  With the 31-instruction RF step (rf.cuh, tier -1) the RF warps
+    // got faster and the balance moved: 3,1,1,3 124.2 ms, 4,2,2,4 119.3, 3,2,2,3 119.8, 4,1,1,4 122.7, 3,3,3,3 121.6;
+    // config 2 (4 RF warps, 16 RF steps per ADC sample) is indifferent (1,1,1,1 2.108 ms, 2,2,2,2 2.128).  Default: two
+    // extra per missing RF warp, and a base that brings the total to about 0.85 signal warps per RF warp at one ADC
+    // sample per RF step, scaled by the sequence's samples per RF step within [0.5, 1.25].
     int rf_per[4], sig_per[4], cnt_per[4];
     for (int k = 0; k < 4; ++k) rf_per[k] = q.rf_warps / 4;
     { const int order[4] = {1, 2, 3, 0}; for (int e = 0; e < q.rf_warps % 4; ++e) ++rf_per[order[e]]; }
@@ -197,7 +200,8 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     const int sig_extra = std::min(std::max(plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA], 0), 7);
     int deficit = 0;
     for (int k = 0; k < 4; ++k) deficit += rf_max - rf_per[k];
-    const int target = std::max(4, (6 * q.rf_warps + 5) / 10);
+    const double adc_per_rf = inf.n_rf_steps > 0 ? double(inf.n_adc) / double(inf.n_rf_steps) : 1.0;
+    const int target = std::max(4, (int)std::lround(0.85 * q.rf_warps * std::min(std::max(adc_per_rf, 0.5), 1.25)));
     const int auto_base = std::max(1, (target - sig_extra * deficit + 2) / 4);
     const int sig_base = plan->opt[BLOCH_OPT_SEQ_SIG_BASE] < 0 ? std::min(auto_base, 7)
                                                                : std::min(plan->opt[BLOCH_OPT_SEQ_SIG_BASE], 7);
