@@ -858,6 +858,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     grouped_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n_groups, gs,
                                                                     (long long)plan->info.n_adc, (long long)b.adc_first,
                                                                     (float2 *)d_signal);
+                note_kernel(plan, BLOCH_KIND_SIGNAL, grid, 256, "grouped_kernel<%d>", ph64 ? 1 : 0);
                 ++launches;
             } else if (per_spin) {
                 const long long total = (long long)n * n_pts;
@@ -870,6 +871,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     perspin_kernel<false><<<grid, 256, 0, stream>>>(recs, n_pts, w.A, w.C, w.S, w.V, n,
                                                                     (long long)plan->info.n_adc, (long long)b.adc_first,
                                                                     (float2 *)d_signal);
+                note_kernel(plan, BLOCH_KIND_SIGNAL, grid, 256, "perspin_kernel<%d>", ph64 ? 1 : 0);
                 ++launches;
             } else if (n_coils > 0) {
                 const SigShape s = coil_shape(n_pts, n, sms, ncp, tc);

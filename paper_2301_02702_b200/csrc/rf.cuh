@@ -117,6 +117,17 @@ __device__ __forceinline__ void fold(float &hi, float &lo) {
     hi = s;
 }
 
+// Hi + lo tiers (TIER <= 0): the step loop is unrolled rf_fold(TIER) deep and the low part is folded into the high part
+// once per trip.  The loop is instruction-bound, so the loop overhead (9 instructions per trip) and the folds (9 per fold)
+// both show.  Measured with tier -1 (every pulse of the configs), rf ms per step of config 4 / whole-sequence ms of
+// config 5 / 5b: 4 steps per fold: 43.2; 8: 39.1 / 119.3 / 136.3; 16: 37.9 / 118.7 / 132.0; 24: 37.9 / 116.9 / 133.7;
+// 32: 37.6 / 115.0 / 131.6 (unrolled 32 deep but folded every 16: 37.9 / 119.0 / 134.5; every 8: 38.4 / 118.1 / 134.7).
+// |l| stays below fold |w| |M|: tier -1 (|w| <= 2^-7) takes 32, so that |l| <= |M| / 4 and the sums into l round at
+// 2^-26 |M| or finer (2^-28 |M| with 8: the final magnetisation of config 5, 1e6 steps, moved from NRMSE 3.3e-7 to
+// 5.2e-7 against the whole oracle, tolerance 1e-5; every signal unchanged to the digits printed); tier 0
+// (|w| <= 2^-4) keeps 8, |l| <= |M| / 2.
+__host__ __device__ constexpr int rf_fold(int tier) { return tier < 0 ? 32 : 8; }
+
 // One tile of steps.  State in and out as (h, l) with h + l the magnetisation.
 // MODE 0: compact records (uniform gradient part), 1: general records, 2: general + motion records.
 template <int TIER, int MODE>
@@ -148,9 +159,10 @@ __device__ __forceinline__ void rf_tile(const unsigned char *tile, const RfTileH
     }
     if (TIER <= 0) {
         int k = 0;
-        for (; k + 8 <= n; k += 8) {
+        constexpr int kFold = rf_fold(TIER);
+        for (; k + kFold <= n; k += kFold) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            for (int j = 0; j < kFold; ++j) {
                 BLOCH_RF_LOAD(k + j)
                 rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
             }
@@ -210,9 +222,10 @@ __device__ __forceinline__ void rf_tile0_pair(const unsigned char *tile, const R
         rf_accumulate<TIER>(wx, wy, wzb, qb, h[3] + l[3], h[4] + l[4], h[5] + l[5], rb, l[3], l[4], l[5]);    \
     }
     int k = 0;
-    for (; k + 8 <= n; k += 8) {
+    constexpr int kFold = rf_fold(TIER);  // as rf_tile: bitwise the one-spin kernel
+    for (; k + kFold <= n; k += kFold) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) BLOCH_RF_PAIR_STEP(k + j)
+        for (int j = 0; j < kFold; ++j) BLOCH_RF_PAIR_STEP(k + j)
 #pragma unroll
         for (int c = 0; c < 6; ++c) fold(h[c], l[c]);
     }
