@@ -218,6 +218,29 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins,
                                float *h_Mxy, float *h_Mz, int init_equilibrium,
                                float *h_signal, void *d_scratch, size_t scratch_bytes, void *stream);
 
+/* bloch_simulate for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same computation for a static plan (BLOCH_MOTION_NONE; any output mode, phase
+ * mode and path), but the workspace -- the packed spin records and the per-chunk partial signal rows of the two-pass
+ * reduction -- is a device array of BLOCH_STATIC_WORKSPACE_BYTES inside
+ * the library, which every GPU context that loads the library holds until it exits.  The caller passes only inputs
+ * and outputs (device pointers, as bloch_simulate); the tables must have been uploaded into caller memory.
+ *   - Allocates nothing: no cudaMalloc / cudaFree / cudaHostAlloc / event or stream creation, on any path.  Plans with
+ *     profiling switched on are refused (BLOCH_EINVAL: the taps create CUDA events), motion plans too.
+ *   - BLOCH_EWORKSPACE (text in bloch_last_error) when bloch_plan_workspace_bytes(plan, n_spins) exceeds
+ *     BLOCH_STATIC_WORKSPACE_BYTES: nothing is enqueued; use bloch_simulate with a caller workspace.  Sizes that fit:
+ *     e.g. 131,072 spins of config 3 (fp64 phase, 21.0 MB), config 2 and config 5 whole (1.1 / 16 MB), ~600,000 spins
+ *     of an fp32-phase plan with short blocks.
+ *   - Every call on a device shares the ONE array, which keeps the previous call's contents; the call clears what must
+ *     start at zero on `stream` itself.  Two calls whose GPU work overlaps (different streams, or one stream per
+ *     thread) RACE on the array: serialise them (one stream, or an event between them).  Results are bitwise those of
+ *     bloch_simulate.  Asynchronous on `stream`, no synchronisation. */
+#define BLOCH_STATIC_WORKSPACE_BYTES (32u << 20)
+int bloch_simulate_static(const bloch_plan *plan, int64_t n_spins,
+                          const float *d_x, const float *d_y, const float *d_z, const float *d_M0,
+                          const float *d_T1, const float *d_T2, const float *d_dw,
+                          float *d_Mxy, float *d_Mz, int init_equilibrium,
+                          float *d_signal, void *stream);
+
 /* Timing taps for the benchmark.  With bloch_plan_set_profiling(plan, 1) bloch_simulate records one CUDA
  * event on `stream` before every kernel it launches (and one after the last); off by default.  After the
  * caller has synchronised `stream`, bloch_plan_last_timing fills, per kernel kind, the summed device time

@@ -66,7 +66,7 @@ EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_cr
            "bloch_simulate_host_coils", "bloch_plan_set_option", "bloch_plan_get_option", "bloch_plan_status",
            "bloch_plan_last_kernel", "bloch_simulate_coils_motion", "bloch_simulate_host_coils_motion", "bloch_sequence_write",
            "bloch_sequence_read", "bloch_sequence_file_get", "bloch_sequence_file_free", "bloch_signal_write",
-           "bloch_signal_read", "bloch_plan_host_tables", "bloch_microbench"]
+           "bloch_signal_read", "bloch_plan_host_tables", "bloch_simulate_static", "bloch_microbench"]
 
 
 def _load():
@@ -87,6 +87,7 @@ def _load():
     lib.bloch_plan_upload.argtypes = [vp, vp, sz, vp]
     sim_args = [vp, i64] + [_fp] * 7 + [_fp, _fp, C.c_int, _fp, vp, sz, vp]
     lib.bloch_simulate.argtypes = sim_args
+    lib.bloch_simulate_static.argtypes = [vp, i64] + [_fp] * 7 + [_fp, _fp, C.c_int, _fp, vp]
     lib.bloch_simulate_host_scratch_bytes.argtypes = [vp, i64, C.POINTER(sz)]
     lib.bloch_simulate_host.argtypes = sim_args
     mo_args = [vp, i64] + [_fp] * 10 + [_fp, _fp, C.c_int, _fp, vp, sz, vp]
@@ -293,6 +294,17 @@ def bloch_simulate(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, Mxy, Mz, in
     """All array arguments are raw DEVICE addresses (ints) or None."""
     _check(_lib.bloch_simulate(plan, n_spins, x, y, z, M0, T1, T2, dw, Mxy, Mz, int(bool(init_equilibrium)),
                                signal, workspace, workspace_bytes, stream))
+
+
+STATIC_WORKSPACE_BYTES = 32 << 20  # BLOCH_STATIC_WORKSPACE_BYTES of include/bloch.h
+
+
+def bloch_simulate_static(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, Mxy, Mz, init_equilibrium: bool,
+                          signal, stream: int = 0):
+    """bloch_simulate on the library's own static device workspace (allocates nothing; static plans whose workspace
+    is at most STATIC_WORKSPACE_BYTES).  All array arguments are raw DEVICE addresses (ints) or None."""
+    _check(_lib.bloch_simulate_static(plan, n_spins, x, y, z, M0, T1, T2, dw, Mxy, Mz, int(bool(init_equilibrium)),
+                                      signal, stream))
 
 
 def bloch_simulate_motion(plan: int, n_spins: int, x, y, z, M0, T1, T2, dw, vx, vy, vz, Mxy, Mz,
@@ -552,6 +564,27 @@ class Plan:
                               None if Mxy is None else Mxy.data_ptr(), None if Mz is None else Mz.data_ptr(),
                               init_equilibrium, signal.data_ptr() if signal.numel() else None,
                               ws.data_ptr(), ws.numel(), self._stream())
+        return signal
+
+    def simulate_static(self, x, y, z, M0, T1, T2, dw, signal, Mxy=None, Mz=None, init_equilibrium=True):
+        """bloch_simulate_static: as simulate(), but the workspace is the library's static device array and NOTHING is
+        allocated here either -- `signal` (complex64 CUDA tensor of the plan's output shape) must be passed in.  Calls
+        whose GPU work overlaps race on the shared array: keep them on one stream."""
+        import torch
+        if self._tables is None:
+            raise RuntimeError("upload() the plan's tables first (simulate_static allocates nothing)")
+        n = int(x.numel())
+        for t in (x, y, z, M0, T1, T2, dw):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n
+        n_rows = int(np.prod(self._signal_shape(n)[:-1]))
+        assert signal is not None, "simulate_static writes into a caller tensor"
+        self._check_out(Mxy, 2 * n, (torch.float32, torch.complex64), "Mxy")
+        self._check_out(Mz, n, (torch.float32,), "Mz")
+        self._check_out(signal, 2 * n_rows * self.info["n_adc"], (torch.complex64,), "signal")
+        bloch_simulate_static(self.handle, n, x.data_ptr(), y.data_ptr(), z.data_ptr(), M0.data_ptr(), T1.data_ptr(),
+                              T2.data_ptr(), dw.data_ptr(), None if Mxy is None else Mxy.data_ptr(),
+                              None if Mz is None else Mz.data_ptr(), init_equilibrium,
+                              signal.data_ptr() if signal.numel() else None, self._stream())
         return signal
 
     def simulate_host(self, x, y, z, M0, T1, T2, dw, Mxy=None, Mz=None, init_equilibrium=True, signal=None,

@@ -1187,6 +1187,65 @@ int bloch_simulate_host_coils_motion(const bloch_plan *plan, int64_t n_spins, co
     return collect_status(plan, nullptr);  // bad T1 / T2, non-finite input, phase range: see bloch_plan_status
 }
 
+// ---- bloch_simulate_static: the simulation with the library's OWN scratch memory, no allocation anywhere ----
+// The workspace of bloch_simulate (packed spin records, the per-chunk partial signal rows signal_kernel / seq_kernel
+// write and reduce_kernel sums, tickets) lives in this file-scope device array instead of a caller buffer.  Every
+// context that loads the library holds these BLOCH_STATIC_WORKSPACE_BYTES until exit.  In host code the array's name
+// is only a stand-in: the device address comes from cudaGetSymbolAddress, once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_workspace[BLOCH_STATIC_WORKSPACE_BYTES];
+
+namespace bloch {
+namespace {
+std::atomic<void *> g_static_workspace_ptr[kMaxDevices];  // per device: the array's address in that device's context
+
+// the current device's address of g_static_workspace (no allocation: the array is part of the loaded module)
+int static_workspace(void **out) {
+    int dev = 0;
+    BLOCH_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(BLOCH_ECUDA, "device ordinal beyond the library's per-device table");
+    void *p = g_static_workspace_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        BLOCH_CUDA(cudaGetSymbolAddress(&p, g_static_workspace));
+        if (!p || (reinterpret_cast<uintptr_t>(p) % kAlign) != 0)
+            return fail(BLOCH_ECUDA, "cudaGetSymbolAddress returned a NULL or misaligned static workspace");
+        g_static_workspace_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return BLOCH_OK;
+}
+}  // namespace
+}  // namespace bloch
+
+int bloch_simulate_static(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
+                          const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,
+                          const float *d_dw, float *d_Mxy, float *d_Mz, int init_equilibrium, float *d_signal,
+                          void *stream_) {
+    if (!plan) return fail(BLOCH_EINVAL, "NULL plan");
+    if (n_spins < 0 || n_spins > INT32_MAX) return fail(BLOCH_EINVAL, "n_spins out of range");
+    if (plan->info.motion_mode != BLOCH_MOTION_NONE)
+        return fail(BLOCH_EINVAL, "bloch_simulate_static: static plans only (no motion); use bloch_simulate_motion");
+    // the timing taps create CUDA events on first use: an allocation this entry point promises not to make
+    if (plan->profiling)
+        return fail(BLOCH_EINVAL, "bloch_simulate_static: switch bloch_plan_set_profiling off (its taps create CUDA events)");
+    size_t need = 0;
+    int rc = bloch_plan_workspace_bytes(plan, n_spins, &need);
+    if (rc != BLOCH_OK) return rc;
+    if (need > size_t(BLOCH_STATIC_WORKSPACE_BYTES)) {
+        char msg[200];
+        std::snprintf(msg, sizeof msg,
+                      "bloch_simulate_static: %lld spins of this plan need %zu B of workspace, the static array holds %zu B; "
+                      "use bloch_simulate with a caller workspace", (long long)n_spins, need, size_t(BLOCH_STATIC_WORKSPACE_BYTES));
+        return fail(BLOCH_EWORKSPACE, msg);
+    }
+    void *ws = nullptr;
+    if (n_spins > 0 && (rc = bloch::static_workspace(&ws)) != BLOCH_OK) return rc;
+    // simulate_impl treats its workspace as uninitialised memory: it clears the findings word and the tickets of the
+    // whole-sequence kernel on `stream` before the kernels that use them and overwrites everything else before
+    // reading it, so the contents the previous call left in the array do not matter.
+    return bloch::simulate_impl(plan, n_spins, d_x, d_y, d_z, d_M0, d_T1, d_T2, d_dw, nullptr, nullptr, nullptr, 0, nullptr,
+                                d_Mxy, d_Mz, init_equilibrium, d_signal, ws, size_t(BLOCH_STATIC_WORKSPACE_BYTES), stream_);
+}
+
 int bloch_microbench(int kind, int iters, double *ops_per_s, void *stream_) {
     if (!ops_per_s || iters <= 0 || kind < 0 || kind > 3) return fail(BLOCH_EINVAL, "bad microbench argument");
     int rc = check_arch();
