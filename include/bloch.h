@@ -228,8 +228,8 @@ int bloch_simulate_host_motion(const bloch_plan *plan, int64_t n_spins,
  *     profiling switched on are refused (BLOCH_EINVAL: the taps create CUDA events), motion plans too.
  *   - BLOCH_EWORKSPACE (text in bloch_last_error) when bloch_plan_workspace_bytes(plan, n_spins) exceeds
  *     BLOCH_STATIC_WORKSPACE_BYTES: nothing is enqueued; use bloch_simulate with a caller workspace.  Sizes that fit:
- *     e.g. 131,072 spins of config 3 (fp64 phase, 21.0 MB), config 2 and config 5 whole (1.1 / 16 MB), ~600,000 spins
- *     of an fp32-phase plan with short blocks.
+ *     e.g. the whole of config 3 (131,072 spins, fp64 phase: 20.2 MB), config 2 (1.3 MB), config 5 (12.8 MB) and
+ *     config 5b (4.8 MB); ~595,000 spins of an fp32-phase plan with short blocks (config 4's 1,000,000 need 203 MB).
  *   - Every call on a device shares the ONE array, which keeps the previous call's contents; the call clears what must
  *     start at zero on `stream` itself.  Two calls whose GPU work overlaps (different streams, or one stream per
  *     thread) RACE on the array: serialise them (one stream, or an event between them).  Results are bitwise those of
