@@ -161,7 +161,8 @@ size_t partial_elems_for(const bloch_plan *plan, int64_t n_spins, int sm_count) 
 struct SeqShape {
     bool ok, use;
     int n_ctas, chunk, rf_warps, sig_warps, threads, min_items;
-    int ring_slots, slot_stride;  // partial-row ring: [ring_slots][n_ctas][slot_stride] float2
+    int ring_slots, slot_stride;  // partial-row ring: [ring_slots][n_ctas][slot_stride] float2 ([..][n_ctas][nc][slot_stride] with coils)
+    int nc;                       // weights per spin record with receive coils (4 or 8), else 0
     SeqRoles roles;
     size_t smem, partial_elems, ticket_off;  // float2 elements of the partial area; where the tickets start in it
 };
@@ -171,9 +172,15 @@ struct SeqShape {
 // of > 900k samples on 148 SMs; max_block_points cuts such blocks).
 constexpr size_t kSeqRingCapBytes = size_t(8) << 30;
 
-SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
+// L2-resident partial rows: with coils a slot is nc times larger, so fewer slots are kept once the ring passes this
+constexpr size_t kSeqRingL2Bytes = size_t(48) << 20;
+
+SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_coils = 0) {
     SeqShape q{};
     const bloch_plan_info &inf = plan->info;
+    // receive coils: up to 8 in the one launch, SUM_ALL plans; more take the per-block kernels
+    if (n_coils < 0 || n_coils > 8 || (n_coils > 0 && inf.output_mode != BLOCH_OUT_SUM_ALL)) return q;
+    q.nc = n_coils == 0 ? 0 : (n_coils <= 4 ? 4 : 8);
     // PER_SPIN plans qualify when every block holds only a few samples (dictionary mode: the RF thread that owns
     // the spin evaluates them itself, no signal warps)
     const bool ps = inf.output_mode == BLOCH_OUT_PER_SPIN;
@@ -200,8 +207,12 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     const int sig_extra = std::min(std::max(plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA], 0), 7);
     int deficit = 0;
     for (int k = 0; k < 4; ++k) deficit += rf_max - rf_per[k];
-    const double adc_per_rf = inf.n_rf_steps > 0 ? double(inf.n_adc) / double(inf.n_rf_steps) : 1.0;
-    const int target = std::max(4, (int)std::lround(0.85 * q.rf_warps * std::min(std::max(adc_per_rf, 0.5), 1.25)));
+    // with coils an evaluation costs (15 + 4 nc) / 15 of a plain one and has no P > 1 savings: ask for as many signal
+    // warps as fit (the loop below gives warps back until the CTA holds 1024 threads)
+    const double adc_per_rf = (inf.n_rf_steps > 0 ? double(inf.n_adc) / double(inf.n_rf_steps) : 1.0) *
+                              (q.nc > 0 ? (19.0 + 4.0 * q.nc) / 15.0 : 1.0);
+    const double adc_cap = q.nc > 0 ? 4.0 : 1.25;
+    const int target = std::max(4, (int)std::lround(0.85 * q.rf_warps * std::min(std::max(adc_per_rf, 0.5), adc_cap)));
     const int auto_base = std::max(1, (target - sig_extra * deficit + 2) / 4);
     const int sig_base = plan->opt[BLOCH_OPT_SEQ_SIG_BASE] < 0 ? std::min(auto_base, 7)
                                                                : std::min(plan->opt[BLOCH_OPT_SEQ_SIG_BASE], 7);
@@ -243,12 +254,17 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count) {
     q.threads = 32 * n_warps;
     q.min_items = std::max(1, q.sig_warps * plan->opt[BLOCH_OPT_SEQ_ITEMS_X4] / 4);  // 0: always the largest P (config 5: 127.6 ms against 131.1 with one item per warp)
     q.n_ctas = (int)((n_spins + q.chunk - 1) / q.chunk);
-    q.smem = seq_smem_bytes(q.chunk);
+    q.smem = seq_smem_bytes(q.chunk, q.nc);
+    if (q.smem > size_t(227) * 1024) return q;
     if (inf.max_block_adc > INT32_MAX / 2) return q;
     q.slot_stride = (int)std::max<int64_t>(32, (inf.max_block_adc + 31) / 32 * 32);
     q.ring_slots = kSeqRingSlots;
     if (ps) { q.ring_slots = 1; q.slot_stride = 32; }  // PER_SPIN: no partial rows at all
-    const size_t ring_elems = ps ? 0 : size_t(q.ring_slots) * size_t(q.n_ctas) * size_t(q.slot_stride);
+    const size_t slot_elems = size_t(q.n_ctas) * size_t(std::max(q.nc, 1)) * size_t(q.slot_stride);
+    // coils: keep the ring in L2 if that leaves at least lag + 2 slots (the CTAs may then drift 2 blocks apart)
+    while (q.nc > 0 && q.ring_slots > kSeqReduceLag + 2 && size_t(q.ring_slots) * slot_elems * sizeof(float2) > kSeqRingL2Bytes)
+        --q.ring_slots;
+    const size_t ring_elems = ps ? 0 : size_t(q.ring_slots) * slot_elems;
     if (ring_elems * sizeof(float2) > kSeqRingCapBytes) return q;
     q.ticket_off = (ring_elems + 31) / 32 * 32;
     q.partial_elems = q.ticket_off + (size_t(2) * size_t(std::max<int64_t>(plan->n_adc_blocks, 1)) * sizeof(int) + 7) / 8;
@@ -270,6 +286,14 @@ bool coil_use_tc(const bloch_plan *plan, int n_coils) {
     const int mode = plan->opt[BLOCH_OPT_COIL_TC];
     return mode != 0 && n_coils > 4 && plan->info.phase_mode == BLOCH_PHASE_FP32 &&
            plan->info.motion_mode == BLOCH_MOTION_NONE;  // moving spins: the FFMA kernel
+}
+
+// Multi-coil receive inside the whole-sequence kernel (seq_kernel<false, NC>): when the plan takes that path for
+// n_spins and there are at most 8 coils.  Everything that sizes or carves the workspace asks this ONE function.
+bool coil_use_fused(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_coils) {
+    if (n_coils <= 0) return false;
+    const SeqShape q = seq_shape(plan, n_spins, sm_count, n_coils);
+    return q.ok && q.use;
 }
 
 SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp, bool tc) {
@@ -349,8 +373,8 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     w.scal = (unsigned *)take(kAlign);
     size_t pbytes = kAlign;
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
-        const SeqShape q = seq_shape(plan, n_spins, sm_count);
-        if (n_coils > 0) {
+        const SeqShape q = seq_shape(plan, n_spins, sm_count, n_coils);
+        if (n_coils > 0 && !(q.ok && q.use)) {
             const bool tc_ = coil_use_tc(plan, n_coils);
             w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, tc_ ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils), tc_);
         }
@@ -358,7 +382,7 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
-    const bool tc_ws = n_coils > 0 && coil_use_tc(plan, n_coils);
+    const bool tc_ws = n_coils > 0 && coil_use_tc(plan, n_coils) && !coil_use_fused(plan, n_spins, sm_count, n_coils);
     const int ncp = tc_ws ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const size_t n_pass = size_t((n_coils + ncp - 1) / ncp);
     // the tcgen05 kernel takes its weights as ready-made B tiles: 2048 B per 8 spins (spins padded to whole stages)
@@ -730,7 +754,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                      (const float2 *)d_Mxy, d_Mz, init_equilibrium ? 1 : 0,
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
-    const bool tc = n_coils > 0 && coil_use_tc(plan, n_coils);
+    const bool coil_fused = coil_use_fused(plan, n_spins, sms, n_coils);
+    const bool tc = n_coils > 0 && !coil_fused && coil_use_tc(plan, n_coils);
     const int ncp = tc ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const int n_pass = (n_coils + ncp - 1) / ncp;
     const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
@@ -752,22 +777,25 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         ++launches;
     }
 
-    SeqShape sq = seq_shape(plan, n_spins, sms);
-    if (n_coils > 0) sq.use = false;  // multi-coil receive runs on the per-block path
+    const SeqShape sq = seq_shape(plan, n_spins, sms, n_coils);  // coils: up to 8 inside the launch, else per-block
     if (plan->path == BLOCH_PATH_FUSED && !sq.ok)
-        return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output (or PER_SPIN with <= 16 samples per block), fp32 phase, no motion and <= 29 x 32 spins per SM");
+        return fail(BLOCH_EINVAL, "BLOCH_PATH_FUSED needs SUM_ALL output (or PER_SPIN with <= 16 samples per block), fp32 phase, no motion, <= 29 x 32 spins per SM and <= 8 receive coils");
     if (sq.ok && sq.use) {
         // ONE persistent launch for the whole sequence + the second pass over all ADC samples
         if (!devinfo->seq_attr.load(std::memory_order_acquire)) {  // once per DEVICE; sticky for the function there
-            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)seq_smem_bytes(kSeqMaxThreads)));
-            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)seq_smem_bytes(kSeqMaxThreads)));
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)seq_smem_bytes(kSeqMaxThreads, 4)));
+            BLOCH_CUDA(cudaFuncSetAttribute(seq_kernel<false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)seq_smem_bytes(kSeqMaxThreads, 8)));
             devinfo->seq_attr.store(true, std::memory_order_release);
         }
         if ((rc = taps.mark(BLOCH_KIND_FUSED))) return rc;
         const SeqOp *prog = reinterpret_cast<const SeqOp *>(plan->d_tables + plan->prog_off);
-        note_kernel(plan, BLOCH_KIND_FUSED, sq.n_ctas, sq.threads, "seq_kernel<%d>", per_spin ? 1 : 0);
+        note_kernel(plan, BLOCH_KIND_FUSED, sq.n_ctas, sq.threads, "seq_kernel<%d, %d>", per_spin ? 1 : 0, sq.nc);
         // kernel arguments by address (cudaLaunchCooperativeKernel)
         const unsigned char *a_tables = plan->d_tables;
         int a_nops = (int)plan->blocks.size(), a_n = n, a_chunk = sq.chunk, a_rfw = sq.rf_warps, a_min = sq.min_items;
@@ -782,16 +810,20 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         float2 *a_sig = per_spin ? nullptr : (float2 *)d_signal, *a_ps = per_spin ? (float2 *)d_signal : nullptr;
         long long a_nadc = (long long)plan->info.n_adc;
         int a_final = d_Mxy ? 1 : 0;
+        const float4 *a_W = reinterpret_cast<const float4 *>(w.W);  // coils: nc float2 per spin (pack_coils_kernel, one pass)
+        int a_ncoils = n_coils;
         void *args[] = {&a_tables, &prog, &a_nops, &a_A, &a_C, &a_S, &a_n, &a_chunk, &a_rfw, &a_roles, &a_min, &a_scal,
-                        &a_ring, &a_slots, &a_stride, &a_tickets, &a_nblk, &a_blk, &a_sig, &a_nadc, &a_final, &a_ps};
+                        &a_ring, &a_slots, &a_stride, &a_tickets, &a_nblk, &a_blk, &a_sig, &a_nadc, &a_final, &a_ps,
+                        &a_W, &a_ncoils};
         if (per_spin) {
-            BLOCH_CUDA(cudaLaunchKernel((const void *)seq_kernel<true>, dim3(sq.n_ctas), dim3(sq.threads), args, sq.smem, stream));
+            BLOCH_CUDA(cudaLaunchKernel((const void *)seq_kernel<true, 0>, dim3(sq.n_ctas), dim3(sq.threads), args, sq.smem, stream));
         } else {
             // the CTAs wait for one another's tickets (integer counters) when they sum the partial rows, so all of them
             // must be resident: a cooperative launch guarantees it (n_ctas <= SMs, one CTA per SM)
             BLOCH_CUDA(cudaMemsetAsync(a_tickets, 0, size_t(2) * size_t(std::max(a_nblk, 1)) * sizeof(int), stream));
-            BLOCH_CUDA(cudaLaunchCooperativeKernel((const void *)seq_kernel<false>, dim3(sq.n_ctas), dim3(sq.threads), args,
-                                                   sq.smem, stream));
+            const void *fn = sq.nc == 8 ? (const void *)seq_kernel<false, 8>
+                                        : (sq.nc == 4 ? (const void *)seq_kernel<false, 4> : (const void *)seq_kernel<false, 0>);
+            BLOCH_CUDA(cudaLaunchCooperativeKernel(fn, dim3(sq.n_ctas), dim3(sq.threads), args, sq.smem, stream));
         }
         ++launches;
         if (d_Mxy) {

@@ -70,8 +70,10 @@ static_assert(kSeqTileStride >= kRfHdrBytes + kRfTileSteps * 32 && kSeqTileStrid
 
 // dynamic shared memory: [ring: kSeqStages x kSeqTileStride][barriers + item counters: 256 B][shA: chunk float4]
 // [shS: kSeqStateBufs x chunk float4]
-__host__ __device__ inline size_t seq_smem_bytes(int chunk) {
-    return size_t(kSeqStages) * kSeqTileStride + kSeqBarBytes + size_t(1 + kSeqStateBufs) * chunk * sizeof(float4);
+// [shW: chunk x NC float2] with NC receive coils
+__host__ __device__ inline size_t seq_smem_bytes(int chunk, int nc = 0) {
+    return size_t(kSeqStages) * kSeqTileStride + kSeqBarBytes + size_t(1 + kSeqStateBufs) * chunk * sizeof(float4) +
+           size_t(chunk) * nc * sizeof(float2);
 }
 static_assert((2 * kSeqStages + 2 * kSeqStateBufs) * 8 + 2 * kSeqStateBufs * 4 <= kSeqBarBytes, "barrier area");
 
@@ -167,8 +169,86 @@ __device__ __forceinline__ void seq_signal_block(const float4 *__restrict__ recs
     }
 }
 
+// The same for n_coils receive coils: a CTA's row of a block is [NC][slot_stride] (coil-major), the signal [n_coils][n_adc].
+__device__ __forceinline__ void seq_reduce_slice_coils(const float2 *slot, int slot_stride, int nc, int n_ctas, int cta,
+                                                       int n_pts, float2 *__restrict__ sig, long long n_adc, int n_coils,
+                                                       int lane, const int *arrive, int *reduced) {
+    wait_ticket(arrive, n_ctas, lane);
+    const int p_lo = (int)((long long)cta * n_pts / n_ctas), p_hi = (int)((long long)(cta + 1) * n_pts / n_ctas);
+    const size_t row = (size_t)nc * slot_stride;
+    for (int c = 0; c < n_coils; ++c) {
+        for (int p = p_lo; p < p_hi; ++p) {
+            float re = 0.f, im = 0.f;
+            for (int r = lane; r < n_ctas; r += 32) {
+                const float2 v = __ldcg(slot + (size_t)r * row + (size_t)c * slot_stride + p);
+                re += v.x;
+                im += v.y;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                re += __shfl_xor_sync(0xffffffffu, re, o);
+                im += __shfl_xor_sync(0xffffffffu, im, o);
+            }
+            if (lane == 0) sig[(size_t)c * (size_t)n_adc + p] = make_float2(re, im);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence();
+        atomicAdd(reduced, 1);
+    }
+}
+
+// Multi-coil item (reading C1): 32 adjacent samples, one per lane, NC coil sums per sample.  A spin's
+// contribution (phase, sin / cos, decay: signal_spin_fp32) does not depend on the coil; every coil adds one complex
+// multiply-add with the spin's weight (shW: NC float2 per spin, read as warp-wide broadcasts).
+template <int NC>
+__device__ __forceinline__ void seq_signal_item_coils(const float4 *__restrict__ recs, int n_pts, int base,
+                                                      const float4 *shA, const float4 *shS, const float4 *shW, int cnt,
+                                                      int lane, int slot_stride, float2 *__restrict__ out) {
+    const int p = base + lane;
+    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (p < n_pts) r = recs[p];
+    const float kx[1] = {r.x}, ky[1] = {r.y}, kz[1] = {r.z}, tau[1] = {r.w}, cj[1] = {0.f};
+    float ar[NC], ai[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) { ar[c] = 0.f; ai[c] = 0.f; }
+#pragma unroll 2
+    for (int s = 0; s < cnt; ++s) {
+        float cr[1] = {0.f}, ci[1] = {0.f};
+        signal_spin_fp32<1, 0>(kx, ky, kz, tau, cj, shA[s], shS[s], cr, ci);
+#pragma unroll
+        for (int k = 0; k < NC / 2; ++k) {
+            const float4 w = shW[s * (NC / 2) + k];  // two coils' weights
+            ar[2 * k] = fmaf(cr[0], w.x, fmaf(-ci[0], w.y, ar[2 * k]));
+            ai[2 * k] = fmaf(cr[0], w.y, fmaf(ci[0], w.x, ai[2 * k]));
+            ar[2 * k + 1] = fmaf(cr[0], w.z, fmaf(-ci[0], w.w, ar[2 * k + 1]));
+            ai[2 * k + 1] = fmaf(cr[0], w.w, fmaf(ci[0], w.z, ai[2 * k + 1]));
+        }
+    }
+    if (p < n_pts) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) out[(size_t)c * slot_stride + p] = make_float2(ar[c], ai[c]);
+    }
+}
+
+template <int NC>
+__device__ __forceinline__ void seq_signal_block_coils(const float4 *__restrict__ recs, int n_pts, const float4 *shA,
+                                                       const float4 *shS, const float4 *shW, int cnt, int lane,
+                                                       int *item_ctr, int slot_stride, float2 *__restrict__ out) {
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = atomicAdd(item_ctr, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        const int base = item * 32;
+        if (base >= n_pts) break;
+        seq_signal_item_coils<NC>(recs, n_pts, base, shA, shS, shW, cnt, lane, slot_stride, out);
+    }
+}
+
 // PS: PER_SPIN plans (a separate instantiation so that the SUM_ALL kernel keeps its 64 registers without spills)
-template <bool PS>
+// NC: receive coils per spin record (0: none; 4 or 8: SUM_ALL plans with up to NC coils, sums per coil in the same launch)
+template <bool PS, int NC>
 __global__ void __launch_bounds__(kSeqMaxThreads, 1)
 seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ ops, int n_ops,
            const float4 *__restrict__ A, const float4 *__restrict__ Cc, float4 *__restrict__ S, int n, int chunk,
@@ -177,7 +257,10 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
            int *__restrict__ tickets /* [2][n_adc_blocks]: arrive, reduced; zeroed before the launch */, int n_adc_blocks,
            const SeqAdcBlock *__restrict__ adc_blocks /* [n_adc_blocks] */,
            float2 *__restrict__ sig /* SUM_ALL: signal[n_adc] */,
-           long long n_adc, int final_state, float2 *__restrict__ out_ps /* PER_SPIN plans: out[spin][adc], else NULL */) {
+           long long n_adc, int final_state, float2 *__restrict__ out_ps /* PER_SPIN plans: out[spin][adc], else NULL */,
+           const float4 *__restrict__ Wc /* NC > 0: NC / 2 float4 of coil weights per spin (pack_coils_kernel) */,
+           int n_coils /* NC > 0: rows of sig, [n_coils][n_adc] */) {
+    static_assert(NC == 0 || ((NC == 4 || NC == 8) && !PS), "coils: SUM_ALL plans, 4 or 8 weights per spin record");
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *ring = smem;
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kSeqStages * kSeqTileStride);
@@ -187,6 +270,7 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
     int *fin_ctr = item_ctr + kSeqStateBufs;  // [kSeqStateBufs]: signal warps that have finished the block
     float4 *shA = reinterpret_cast<float4 *>(smem + kSeqStages * kSeqTileStride + kSeqBarBytes);
     float4 *shS = shA + chunk;  // [kSeqStateBufs][chunk]
+    float4 *shW = shS + kSeqStateBufs * chunk;  // NC > 0: [chunk][NC / 2]
     const int tid = threadIdx.x, warp = tid >> 5;
     const int n_rf_thr = rf_warps * 32;
     const int nsig = roles.n_sig_warps * 32;
@@ -242,6 +326,10 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             c = Cc[i];
             s = S[i];
             shA[r] = a;
+            if constexpr (NC > 0) {  // visible to the signal warps with the first published state (st_full)
+#pragma unroll
+                for (int k = 0; k < NC / 2; ++k) shW[r * (NC / 2) + k] = Wc[(size_t)i * (NC / 2) + k];
+            }
         }
         float hx = s.x, hy = s.y, hz = s.z, lx = 0.f, ly = 0.f, lz = 0.f;
         const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z, 0.f, 0.f, 0.f};
@@ -325,7 +413,8 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
         const float r2max_log2e = scal[0] * kLog2e;
         const int n_ctas = gridDim.x, cta = blockIdx.x;
         int *arrive = tickets, *reduced = tickets + n_adc_blocks;
-        const size_t slot_elems = (size_t)n_ctas * slot_stride;
+        const size_t row_elems = (size_t)(NC > 0 ? NC : 1) * slot_stride;  // one CTA's row(s) of a block
+        const size_t slot_elems = (size_t)n_ctas * row_elems;
         int pub = 0;  // = index of the block among the ADC-bearing precession blocks (adc_blocks[pub])
         for (int oi = 0; oi < n_ops; ++oi) {
             const int2 tn = *reinterpret_cast<const int2 *>(&ops[oi]);
@@ -333,12 +422,13 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             const float4 *recs = reinterpret_cast<const float4 *>(tables + ops[oi].table_off);
             // the ring slot is free once every CTA has summed its slice of the block that used it before
             if (pub >= ring_slots) wait_ticket(&reduced[pub - ring_slots], n_ctas, lane);
-            float2 *out = prow + (size_t)(pub % ring_slots) * slot_elems + (size_t)cta * slot_stride;
+            float2 *out = prow + (size_t)(pub % ring_slots) * slot_elems + (size_t)cta * row_elems;
             const int b = pub % kSeqStateBufs;
             mbar_wait(&st_full[b], (uint32_t)((pub / kSeqStateBufs) & 1));
             const float4 *stS = shS + b * chunk;
             // item size: the largest P that still leaves min_items items (about one per signal warp)
-            if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            if constexpr (NC > 0) seq_signal_block_coils<NC>(recs, tn.y, shA, stS, shW, cnt, lane, &item_ctr[b], slot_stride, out);
+            else if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else if (tn.y >= 64 * min_items) seq_signal_block<2>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else seq_signal_block<1>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             // the warp that finishes the block last in this CTA announces the CTA's row and takes the CTA's reduce duty
@@ -359,8 +449,12 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
                 const int h_hi = pub == n_adc_blocks - 1 ? pub : pub - kSeqReduceLag;
                 for (int h = max(pub - kSeqReduceLag, 0); h <= h_hi; ++h) {
                     const SeqAdcBlock ab = adc_blocks[h];
-                    seq_reduce_slice(prow + (size_t)(h % ring_slots) * slot_elems, slot_stride, n_ctas, cta, ab.n,
-                                     sig + ab.adc_first, lane, &arrive[h], &reduced[h]);
+                    if constexpr (NC > 0)
+                        seq_reduce_slice_coils(prow + (size_t)(h % ring_slots) * slot_elems, slot_stride, NC, n_ctas, cta,
+                                               ab.n, sig + ab.adc_first, n_adc, n_coils, lane, &arrive[h], &reduced[h]);
+                    else
+                        seq_reduce_slice(prow + (size_t)(h % ring_slots) * slot_elems, slot_stride, n_ctas, cta, ab.n,
+                                         sig + ab.adc_first, lane, &arrive[h], &reduced[h]);
                 }
             }
             ++pub;

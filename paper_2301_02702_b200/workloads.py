@@ -512,9 +512,15 @@ def config4c(n_coils: int = 8, **kw) -> Workload:
     return dataclasses.replace(w, name=f"config4c_1M_spiral_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
 
 
+def config5x(n_coils: int = 8, **kw) -> Workload:
+    """Config 5 (MRF FISP) received by 8 coils: the multi-coil sums inside the whole-sequence kernel (f2 x a5-a8)."""
+    w = config5(**kw)
+    return dataclasses.replace(w, name=f"config5x_mrf_fisp_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
+
+
 CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "3w": config3w, "4": config4, "5": config5, "5b": config5b,
            "5c": config5c, "4c": config4c,
-           "4c32": lambda **kw: config4c(n_coils=32, **kw)}
+           "4c32": lambda **kw: config4c(n_coils=32, **kw), "5x8": config5x}
 
 
 def make(name: str, **kw) -> Workload:

@@ -53,21 +53,21 @@ def test_uniform_coil_is_the_plain_signal_and_passes_are_independent(B):
     (coils 0-7 alone), to rounding when it is not (4 coils per pass for up to 4 coils: other tile sizes)."""
     from test_gpu_parity import run_gpu
     w = W.small("4")
-    ffma = {"coil_tc": 0}   # the FFMA kernel (9 coils would take the tensor-core kernel otherwise)
+    ffma = {"coil_tc": 0}   # the per-block FFMA kernel (the tensor-core kernel / the whole-sequence kernel otherwise)
     n = w.phantom.n
     plain = run_gpu(B, w, path="per_block")
-    one = run_coils(B, w, np.ones((1, n), dtype=np.complex64), options=ffma)
+    one = run_coils(B, w, np.ones((1, n), dtype=np.complex64), options=ffma, path="per_block")
     emax, _ = errors(one[0], plain)
     assert emax < 2e-6, f"uniform coil vs plain: {emax:.3e}"
     coils = coil_maps(w.phantom, 9, seed=4)
-    all9 = run_coils(B, w, coils, options=ffma)
-    again = run_coils(B, w, coils, options=ffma)
+    all9 = run_coils(B, w, coils, options=ffma, path="per_block")
+    again = run_coils(B, w, coils, options=ffma, path="per_block")
     assert np.array_equal(all9.view(np.float32), again.view(np.float32)), "run-to-run not bitwise identical"
-    first8 = run_coils(B, w, coils[:8], options=ffma)
+    first8 = run_coils(B, w, coils[:8], options=ffma, path="per_block")
     assert np.array_equal(all9[:8].view(np.float32), first8.view(np.float32))
     scale = np.abs(all9).max()
-    first4 = run_coils(B, w, coils[:4], options=ffma)
-    last1 = run_coils(B, w, coils[8:9], options=ffma)
+    first4 = run_coils(B, w, coils[:4], options=ffma, path="per_block")
+    last1 = run_coils(B, w, coils[8:9], options=ffma, path="per_block")
     assert np.abs(all9[:4] - first4).max() / scale < 2e-6 and np.abs(all9[8:9] - last1).max() / scale < 2e-6
 
 
@@ -129,12 +129,12 @@ def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils):
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
     ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
-    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32", options={"coil_tc": 1})
+    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32", options={"coil_tc": 1}, path="per_block")
     assert_parity(got, ref, f"tensor-core coil kernel, config {name}, {n_coils} coils")
     for c in range(n_coils):
         emax, nrmse = errors(got[c], ref[c])
         assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
-    ffma = run_coils(B, w, coils, phase_mode="fp32", options={"coil_tc": 0})
+    ffma = run_coils(B, w, coils, phase_mode="fp32", options={"coil_tc": 0}, path="per_block")
     emax, _ = errors(got, ffma)
     assert emax < 2e-5, f"tensor-core vs FFMA kernel: {emax:.3e}"   # TMEM accumulation is coarser than FFMA sums
 
@@ -181,3 +181,79 @@ def test_coils_with_moving_spins(B, oracle_mod, phase_mode, n_coils, wave):
     static = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128))
     assert errors(ref, static)[0] > 1e-2, "the motion must change the signal for the test to mean anything"
     plan.close()
+
+
+def run_coils_path(B, w, coils, path, want_state=True, **kw):
+    """Signal, final state and what the plan reports about the launch, on a given path."""
+    import torch
+    plan = B.Plan(w.seq, path=path, phase_mode="fp32", output_mode="sum", **kw)
+    dev = B.phantom_to_device(w.phantom)
+    n = w.phantom.n
+    Mxy = torch.zeros(n, 2, dtype=torch.float32, device="cuda") if want_state else None
+    Mz = torch.zeros(n, dtype=torch.float32, device="cuda") if want_state else None
+    sig = plan.simulate(*dev, Mxy=Mxy, Mz=Mz, coils=torch.from_numpy(np.ascontiguousarray(coils)).cuda())
+    torch.cuda.synchronize()
+    out = dict(sig=sig.cpu().numpy(), launches=B.bloch_plan_last_launches(plan.handle),
+               fused=B.bloch_plan_last_kernel(plan.handle, "fused")["name"])
+    if want_state:
+        m = Mxy.cpu().numpy()
+        out.update(mxy=m[:, 0] + 1j * m[:, 1], mz=Mz.cpu().numpy())
+    plan.close()
+    return out
+
+
+@pytest.mark.parametrize("name,n_coils", [("2", 1), ("2", 4), ("2", 7), ("5", 3), ("5", 8), ("1", 5), ("4", 6)])
+def test_coils_inside_the_whole_sequence_kernel(B, oracle_mod, name, n_coils):
+    """f2 x (a5-a8 in one launch): up to 8 receive coils are summed per coil inside seq_kernel<0, NC> (ring of partial
+    rows per coil, sum over the CTAs in the launch).  Against the oracle per coil, and against the per-block kernels."""
+    w = W.small(name)
+    coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
+    ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
+    f = run_coils_path(B, w, coils, "fused")
+    nc = 4 if n_coils <= 4 else 8
+    assert f["fused"] == f"seq_kernel<0, {nc}>", f["fused"]
+    assert f["launches"] == 4, f["launches"]          # pack, pack_coils, seq_kernel, unpack
+    assert f["sig"].shape == ref.shape == (n_coils, w.seq.adc_t.size)
+    emax, nrmse = assert_parity(f["sig"], ref, f"config {name}, {n_coils} coils, whole-sequence kernel")
+    print(f"config {name} fused with {n_coils} coils: max {emax:.3e} nrmse {nrmse:.3e}")
+    for c in range(n_coils):
+        e, r = errors(f["sig"][c], ref[c])
+        assert e <= 1e-4 and r <= 1e-5, f"coil {c}: max {e:.3e} nrmse {r:.3e}"
+    assert_parity(np.concatenate([f["mxy"], f["mz"].astype(np.complex128)]),
+                  np.concatenate([rxy, rz.astype(np.complex128)]), "final state")
+    p = run_coils_path(B, w, coils, "per_block")
+    assert p["fused"] == ""
+    assert np.array_equal(f["mxy"], p["mxy"]) and np.array_equal(f["mz"], p["mz"]), "final state differs bitwise between paths"
+    e, _ = errors(f["sig"], p["sig"])
+    assert e < 2e-5, f"fused vs per-block coil signals: {e:.3e}"
+    for _ in range(4):   # integer tickets, fixed summation order: bitwise reproducible
+        g = run_coils_path(B, w, coils, "fused", want_state=False)
+        assert np.array_equal(g["sig"].view(np.float32), f["sig"].view(np.float32))
+
+
+def test_fused_coils_limits_and_auto_choice(B):
+    w = W.small("5")
+    # more than 8 coils: AUTO runs the per-block kernels, a forced FUSED plan is refused
+    c9 = coil_maps(w.phantom, 9, seed=3)
+    a = run_coils_path(B, w, c9, "auto", want_state=False)
+    assert a["fused"] == "" and a["sig"].shape[0] == 9
+    with pytest.raises(B.BlochError) as e:
+        run_coils_path(B, w, c9, "fused", want_state=False)
+    assert e.value.code == -1
+    # up to 8: AUTO takes the whole-sequence kernel where it would without coils, and both agree
+    c8 = c9[:8]
+    a8 = run_coils_path(B, w, c8, "auto", want_state=False)
+    assert a8["fused"] == "seq_kernel<0, 8>"
+    e, _ = errors(a8["sig"], a["sig"][:8])
+    assert e < 2e-5
+    # a uniform coil is the plain signal of the same path (same summation order per sample: close, not bitwise --
+    # the plain kernel shares one ex2 between adjacent samples)
+    import torch
+    one = np.ones((1, w.phantom.n), dtype=np.complex64)
+    u = run_coils_path(B, w, one, "fused", want_state=False)
+    plan = B.Plan(w.seq, path="fused", phase_mode="fp32")
+    plain = plan.simulate(*B.phantom_to_device(w.phantom))
+    torch.cuda.synchronize()
+    e, _ = errors(u["sig"][0], plain.cpu().numpy())
+    plan.close()
+    assert e < 2e-6, f"{e:.3e}"

@@ -126,3 +126,52 @@ def test_full_size_dictionary_every_row_against_the_whole_oracle(B):
     print(f"config 5b worst row on its own scale: {row_err.max():.3e} (entry {int(row_err.argmax())})")
     assert row_err.max() <= TOL_MAX
     assert_parity(state_vec(mxy, mz), state_vec(z["Mxy"], z["Mz"]), "config 5b final magnetisation, every entry")
+
+
+def test_full_size_config5_with_8_coils_inside_the_whole_sequence_kernel(B, oracle_mod):
+    """Workload 5x8 (config 5 received by 8 coils, f2 x whole-sequence kernel) at full size: 65,536 spins, 1,024,000
+    samples x 8 coils in ONE launch.  (1) The coil maps are normalised to add up to one at every spin, so the sum of
+    the 8 coil signals is the plain signal (reading C1 is linear in the weights) -- compared with the WHOLE oracle of
+    config 5, every sample.  (2) A 96-spin subset against the oracle with coils, every coil on its own scale.
+    (3) Superposition per coil S_c(full) = S_c(subset) + S_c(complement), which ties the full-size launch to (2)."""
+    import torch
+    w = W.make("5x8")
+    z = load_golden("5", W.make("5"))       # same phantom and sequence: the oracle of config 5, all 65,536 spins
+    n = w.phantom.n
+    # complex maps that add up to 1 + 0i at every spin: magnitudes normalised, imaginary parts made zero-sum over coils
+    m = np.abs(w.coils).astype(np.float64)
+    m /= m.sum(axis=0, keepdims=True)
+    q = m * np.sin(np.angle(w.coils))
+    q -= q.mean(axis=0, keepdims=True)
+    coils = (m + 1j * q).astype(np.complex64)
+    plan = B.Plan(w.seq, phase_mode="fp32")
+
+    def run(idx):
+        ph = w.phantom if idx is None else w.phantom.subset(idx)
+        c = coils if idx is None else np.ascontiguousarray(coils[:, idx])
+        sig = plan.simulate(*B.phantom_to_device(ph), coils=torch.from_numpy(c).cuda())
+        torch.cuda.synchronize()
+        return sig.cpu().numpy(), B.bloch_plan_last_kernel(plan.handle, "fused")["name"], \
+            B.bloch_plan_last_launches(plan.handle)
+
+    full, kernel, launches = run(None)
+    assert kernel == "seq_kernel<0, 8>" and launches == 3, (kernel, launches)
+    assert full.shape == (8, 1_024_000)
+    assert np.array_equal(full.view(np.float32), run(None)[0].view(np.float32)), "not bitwise reproducible"
+    total = full.astype(np.complex128).sum(axis=0)
+    resid = np.abs(coils.astype(np.complex128).sum(axis=0) - 1.0).max()   # complex64 rounding of the normalised maps
+    assert resid < 1e-6
+    assert_parity(total, z["signal"], "config 5x8: sum of the 8 coil signals vs whole oracle of config 5 (65536 spins)")
+    sub = np.linspace(0, n - 1, 96).astype(np.int64)
+    s_sub = run(sub)[0]
+    ref = oracle_mod.simulate(w.phantom.subset(sub), w.seq, coils=coils[:, sub].astype(np.complex128))
+    assert_parity(s_sub, ref, "config 5x8 subset, all coils")
+    for c in range(8):
+        assert_parity(s_sub[c], ref[c], f"config 5x8 subset, coil {c}")
+    mask = np.ones(n, dtype=bool)
+    mask[sub] = False
+    s_rest = run(np.flatnonzero(mask))[0]
+    plan.close()
+    for c in range(8):
+        emax, nrmse = errors(s_sub[c].astype(np.complex128) + s_rest[c], full[c])
+        assert emax < 5e-6 and nrmse < 1e-6, f"coil {c} superposition: max {emax:.3e} nrmse {nrmse:.3e}"
