@@ -351,13 +351,13 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
     if kinds_n["fused"]:
         # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
         # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)
-        fp32_ops = FP32_PER_RF_STEP * rf_steps + FP32_PER_EVAL * n_eval_sig
+        fp32_ops = FP32_PER_RF_STEP * rf_steps + (FP32_PER_EVAL + 4 * n_coils) * n_eval_sig   # + one complex MAC per coil
         mufu_ops = MUFU_PER_EVAL * n_eval_sig
         t_fp32, t_mufu = fp32_ops / fp32_peak, mufu_ops / mufu_peak
         pipe, ops = ("fp32", fp32_ops) if t_fp32 >= t_mufu else ("mufu", mufu_ops)
         kern["fused"] = entry("fused", pipe, ops,
                               "seq_kernel (a5-a8 in one launch): algorithmic count = 46 FP32 per spin*step + 15 FP32 per "
-                              f"(spin, ADC sample); the MUFU count (3 per evaluation) would take {t_mufu * 1e3:.1f} ms, "
+                              f"(spin, ADC sample){' + 4 per coil (' + str(n_coils) + ' coils)' if n_coils else ''}; the MUFU count (3 per evaluation) would take {t_mufu * 1e3:.1f} ms, "
                               f"the FP32 count {t_fp32 * 1e3:.1f} ms")
     return kern
 
@@ -610,7 +610,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 3w (3 with periodic non-rigid motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary)")
+    ap.add_argument("--workload", default="4", help="config name: 1, 2, 3, 3m (3 with motion), 3w (3 with periodic non-rigid motion), 4 (default, 1M-spin spiral), 4c (4 with 8 receive coils), 4c32 (32 coils), 5, 5b, 5c (ensemble dictionary), 5x8 (5 with 8 receive coils)")
     ap.add_argument("--path", default="auto", choices=["auto", "per_block", "fused"],
                     help="execution path (bloch_plan_set_path); auto = the library's choice")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],

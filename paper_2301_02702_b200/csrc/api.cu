@@ -274,6 +274,13 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
     // N_rf/N_adc = 0.98: 13.1 / 15.5 at 65,536 spins, 42.1 / 29.4 at 131,044 (3 signal warps left);
     // 0.49: 5.97 / 6.17 at 65,536, 22.2 / 11.3 at 131,072;  0.06: 1.05 / 0.84 at 65,522.
     q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || full_layout));
+    // Coils under AUTO: the 8-wide sums cost ~50 issue slots per evaluation on the FMA pipe, so once a block holds
+    // enough (spin, sample) pairs to fill the tcgen05 kernel the per-block launches win.  Measured, fused / per-block
+    // ms: config 5 x 8 coils (6.7e7 pairs per block) 212-221 / 198.7; config 2 x 8 coils (1.0e6) 2.25 / 3.36; up to 4
+    // coils the launch wins on both (config 5 x 4: 178.5 / 206.8; config 2 x 4: 2.15 / 3.19).
+    if (q.nc == 8 && plan->path != BLOCH_PATH_FUSED && plan->opt[BLOCH_OPT_COIL_TC] != 0 &&
+        n_spins * inf.max_block_adc >= (int64_t(1) << 24))
+        q.use = false;
     return q;
 }
 

@@ -199,50 +199,76 @@ __device__ __forceinline__ void seq_reduce_slice_coils(const float2 *slot, int s
     }
 }
 
-// Multi-coil item (reading C1): 32 adjacent samples, one per lane, NC coil sums per sample.  A spin's
+// Multi-coil item (reading C1): 32 x P adjacent samples, P per lane, NC coil sums per sample.  A spin's
 // contribution (phase, sin / cos, decay: signal_spin_fp32) does not depend on the coil; every coil adds one complex
-// multiply-add with the spin's weight (shW: NC float2 per spin, read as warp-wide broadcasts).
-template <int NC>
+// multiply-add with the spin's weight (shW: NC float2 per spin, read as warp-wide broadcasts, shared by the P samples).
+// P = 2 for up to 4 coils (16 accumulators); 8 coils keep P = 1 under the kernel's 64-register cap.
+template <int NC, int P>
 __device__ __forceinline__ void seq_signal_item_coils(const float4 *__restrict__ recs, int n_pts, int base,
                                                       const float4 *shA, const float4 *shS, const float4 *shW, int cnt,
-                                                      int lane, int slot_stride, float2 *__restrict__ out) {
-    const int p = base + lane;
-    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (p < n_pts) r = recs[p];
-    const float kx[1] = {r.x}, ky[1] = {r.y}, kz[1] = {r.z}, tau[1] = {r.w}, cj[1] = {0.f};
-    float ar[NC], ai[NC];
+                                                      int lane, float r2max_log2e, int slot_stride,
+                                                      float2 *__restrict__ out) {
+    const int p0 = base + lane * P;
+    float kx[P], ky[P], kz[P], tau[P], cj[P];
+    float cmax = 0.f;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) { ar[c] = 0.f; ai[c] = 0.f; }
+    for (int j = 0; j < P; ++j) {
+        const int p = p0 + j;
+        float4 r = make_float4(0.f, 0.f, 0.f, j ? tau[0] : 0.f);
+        if (p < n_pts) r = recs[p];
+        kx[j] = r.x; ky[j] = r.y; kz[j] = r.z; tau[j] = r.w;
+        cj[j] = (r.w - tau[0]) * 0.6931471805599453f;
+        cmax = fmaxf(cmax, fabsf(cj[j]));
+    }
+    const bool series = P > 1 && __all_sync(0xffffffffu, cmax * r2max_log2e <= 0.02f);  // as seq_signal_item
+    float ar[P][NC], ai[P][NC];
+#pragma unroll
+    for (int j = 0; j < P; ++j)
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { ar[j][c] = 0.f; ai[j][c] = 0.f; }
+    auto run = [&](auto mode_tag) {
+        constexpr int MODE = decltype(mode_tag)::value;  // 0: MUFU.EX2 per sample, 1: series from sample 0
 #pragma unroll 2
-    for (int s = 0; s < cnt; ++s) {
-        float cr[1] = {0.f}, ci[1] = {0.f};
-        signal_spin_fp32<1, 0>(kx, ky, kz, tau, cj, shA[s], shS[s], cr, ci);
+        for (int s = 0; s < cnt; ++s) {
+            float cr[P], ci[P];
 #pragma unroll
-        for (int k = 0; k < NC / 2; ++k) {
-            const float4 w = shW[s * (NC / 2) + k];  // two coils' weights
-            ar[2 * k] = fmaf(cr[0], w.x, fmaf(-ci[0], w.y, ar[2 * k]));
-            ai[2 * k] = fmaf(cr[0], w.y, fmaf(ci[0], w.x, ai[2 * k]));
-            ar[2 * k + 1] = fmaf(cr[0], w.z, fmaf(-ci[0], w.w, ar[2 * k + 1]));
-            ai[2 * k + 1] = fmaf(cr[0], w.w, fmaf(ci[0], w.z, ai[2 * k + 1]));
+            for (int j = 0; j < P; ++j) { cr[j] = 0.f; ci[j] = 0.f; }
+            signal_spin_fp32<P, MODE>(kx, ky, kz, tau, cj, shA[s], shS[s], cr, ci);
+#pragma unroll
+            for (int k = 0; k < NC / 2; ++k) {
+                const float4 w = shW[s * (NC / 2) + k];  // two coils' weights
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    ar[j][2 * k] = fmaf(cr[j], w.x, fmaf(-ci[j], w.y, ar[j][2 * k]));
+                    ai[j][2 * k] = fmaf(cr[j], w.y, fmaf(ci[j], w.x, ai[j][2 * k]));
+                    ar[j][2 * k + 1] = fmaf(cr[j], w.z, fmaf(-ci[j], w.w, ar[j][2 * k + 1]));
+                    ai[j][2 * k + 1] = fmaf(cr[j], w.w, fmaf(ci[j], w.z, ai[j][2 * k + 1]));
+                }
+            }
         }
-    }
-    if (p < n_pts) {
+    };
+    if (series) run(std::integral_constant<int, 1>{});
+    else run(std::integral_constant<int, 0>{});
 #pragma unroll
-        for (int c = 0; c < NC; ++c) out[(size_t)c * slot_stride + p] = make_float2(ar[c], ai[c]);
-    }
+    for (int j = 0; j < P; ++j)
+        if (p0 + j < n_pts) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) out[(size_t)c * slot_stride + p0 + j] = make_float2(ar[j][c], ai[j][c]);
+        }
 }
 
-template <int NC>
+template <int NC, int P>
 __device__ __forceinline__ void seq_signal_block_coils(const float4 *__restrict__ recs, int n_pts, const float4 *shA,
                                                        const float4 *shS, const float4 *shW, int cnt, int lane,
-                                                       int *item_ctr, int slot_stride, float2 *__restrict__ out) {
+                                                       int *item_ctr, float r2max_log2e, int slot_stride,
+                                                       float2 *__restrict__ out) {
     for (;;) {
         int item = 0;
         if (lane == 0) item = atomicAdd(item_ctr, 1);
         item = __shfl_sync(0xffffffffu, item, 0);
-        const int base = item * 32;
+        const int base = item * (32 * P);
         if (base >= n_pts) break;
-        seq_signal_item_coils<NC>(recs, n_pts, base, shA, shS, shW, cnt, lane, slot_stride, out);
+        seq_signal_item_coils<NC, P>(recs, n_pts, base, shA, shS, shW, cnt, lane, r2max_log2e, slot_stride, out);
     }
 }
 
@@ -427,8 +453,13 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             mbar_wait(&st_full[b], (uint32_t)((pub / kSeqStateBufs) & 1));
             const float4 *stS = shS + b * chunk;
             // item size: the largest P that still leaves min_items items (about one per signal warp)
-            if constexpr (NC > 0) seq_signal_block_coils<NC>(recs, tn.y, shA, stS, shW, cnt, lane, &item_ctr[b], slot_stride, out);
-            else if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
+            if constexpr (NC > 0) {
+                // two samples per lane with up to 4 coils when that still leaves an item for every signal warp
+                if (NC == 4 && tn.y >= 64 * roles.n_sig_warps)
+                    seq_signal_block_coils<NC, NC == 4 ? 2 : 1>(recs, tn.y, shA, stS, shW, cnt, lane, &item_ctr[b], r2max_log2e, slot_stride, out);
+                else
+                    seq_signal_block_coils<NC, 1>(recs, tn.y, shA, stS, shW, cnt, lane, &item_ctr[b], r2max_log2e, slot_stride, out);
+            } else if (tn.y >= 128 * min_items) seq_signal_block<4>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else if (tn.y >= 64 * min_items) seq_signal_block<2>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             else seq_signal_block<1>(recs, tn.y, shA, stS, cnt, lane, &item_ctr[b], r2max_log2e, out);
             // the warp that finishes the block last in this CTA announces the CTA's row and takes the CTA's reduce duty

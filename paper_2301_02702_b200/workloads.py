@@ -512,19 +512,24 @@ def config4c(n_coils: int = 8, **kw) -> Workload:
     return dataclasses.replace(w, name=f"config4c_1M_spiral_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
 
 
-def config5x(n_coils: int = 8, **kw) -> Workload:
-    """Config 5 (MRF FISP) received by 8 coils: the multi-coil sums inside the whole-sequence kernel (f2 x a5-a8)."""
-    w = config5(**kw)
-    return dataclasses.replace(w, name=f"config5x_mrf_fisp_{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
+def with_coils(base: str, n_coils: int, **kw) -> Workload:
+    """Config `base` received by n_coils synthetic coils ("5x8": config 5 with 8 coils -- the multi-coil sums inside
+    the whole-sequence kernel, f2 x a5-a8)."""
+    w = CONFIGS[base](**kw)
+    return dataclasses.replace(w, name=f"{w.name}_x{n_coils}coils", coils=coil_maps(w.phantom, n_coils))
 
 
 CONFIGS = {"1": config1, "2": config2, "3": config3, "3m": config3m, "3w": config3w, "4": config4, "5": config5, "5b": config5b,
            "5c": config5c, "4c": config4c,
-           "4c32": lambda **kw: config4c(n_coils=32, **kw), "5x8": config5x}
+           "4c32": lambda **kw: config4c(n_coils=32, **kw)}
 
 
 def make(name: str, **kw) -> Workload:
-    return CONFIGS[str(name)](**kw)
+    name = str(name)
+    if name not in CONFIGS and "x" in name:   # "<config>x<n_coils>", e.g. "5x8", "2x4"
+        base, n_coils = name.split("x")
+        return with_coils(base, int(n_coils), **kw)
+    return CONFIGS[name](**kw)
 
 
 def small(name: str) -> Workload:

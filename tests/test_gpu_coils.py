@@ -240,7 +240,8 @@ def test_fused_coils_limits_and_auto_choice(B):
     with pytest.raises(B.BlochError) as e:
         run_coils_path(B, w, c9, "fused", want_state=False)
     assert e.value.code == -1
-    # up to 8: AUTO takes the whole-sequence kernel where it would without coils, and both agree
+    # up to 8: AUTO takes the whole-sequence kernel where it would without coils (unless 8 coils meet blocks large
+    # enough for the tcgen05 kernel: 2^24 (spin, sample) pairs), and both agree
     c8 = c9[:8]
     a8 = run_coils_path(B, w, c8, "auto", want_state=False)
     assert a8["fused"] == "seq_kernel<0, 8>"

@@ -144,7 +144,8 @@ def test_full_size_config5_with_8_coils_inside_the_whole_sequence_kernel(B, orac
     q = m * np.sin(np.angle(w.coils))
     q -= q.mean(axis=0, keepdims=True)
     coils = (m + 1j * q).astype(np.complex64)
-    plan = B.Plan(w.seq, phase_mode="fp32")
+    # forced: with 8 coils and 6.7e7 (spin, sample) pairs per block AUTO prefers the per-block tcgen05 kernel
+    plan = B.Plan(w.seq, phase_mode="fp32", path="fused")
 
     def run(idx):
         ph = w.phantom if idx is None else w.phantom.subset(idx)
