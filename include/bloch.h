@@ -274,7 +274,10 @@ int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t 
  * (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  Moving spins: bloch_simulate_coils_motion (motion plans; velocities /
  * amplitudes as bloch_simulate_motion, all three NULL = none).  The coil-independent part of every evaluation (phase,
  * sin / cos / exp) is computed once per 4 or 8 coils; with more than 4 coils (fp32 phase) the sum over spins runs on the
- * tensor cores (tcgen05 with the generated operand in tensor memory, 3xTF32, 8, 16 or 32 coils per pass).  Asynchronous on `stream`; never allocates. */
+ * tensor cores (tcgen05 with the generated operand in tensor memory, 3xTF32, 8, 16 or 32 coils per pass).  Plans that
+ * take the whole-sequence kernel (BLOCH_PATH_FUSED, or AUTO where it qualifies: static spins, fp32 phase) sum up to 8
+ * coils inside that one launch; more coils, or 8 coils on blocks large enough for the tensor-core kernel, run block by
+ * block (BLOCH_PATH_FUSED with more than 8 coils: BLOCH_EINVAL).  Asynchronous on `stream`; never allocates. */
 int bloch_plan_workspace_bytes_coils(const bloch_plan *plan, int64_t n_spins, int n_coils, size_t *out);
 int bloch_simulate_coils(const bloch_plan *plan, int64_t n_spins, const float *d_x, const float *d_y,
                          const float *d_z, const float *d_M0, const float *d_T1, const float *d_T2,

@@ -12,9 +12,12 @@
 // FFMA kernel at 8 coils.
 // The complex product is made real by stacking K:  A = [Cr | Ci],  B = [[Wr, Wi], [-Wi, Wr]]  ->  D = [Dr | Di],
 // and every product runs as hi*hi + lo*hi + hi*lo ("3xTF32", ~2^-21 relative), because plain TF32 (2^-11) breaks
-// the 1e-5 NRMSE bound on small phantoms: 6 MMA instructions per 8 spins and 128 samples.  B tiles (weights, negated /
-// swapped / split as above) are prepared once per simulation by pack_coils_tc_kernel in exactly the shared-memory
-// operand layout and arrive by bulk copies (TMA).
+// the 1e-5 NRMSE bound on small phantoms: 6 MMA instructions per 8 spins and 128 samples -- 4 for up to 16 coils per
+// pass, where the B tiles of a group lie [B hi | B lo] side by side along N and the hi part of A meets both in ONE
+// instruction of N = 4 NC (its halves land in two accumulator column groups, added in the epilogue): an instruction of
+// this shape costs ~74 clocks whatever N, so the count is what matters (8 coils: 105.9 -> 93.3 ms on config 4).  B
+// tiles (weights, negated / swapped / split as above) are prepared once per simulation by pack_coils_tc_kernel in
+// exactly the shared-memory operand layout and arrive by bulk copies (TMA).
 //
 // B operand layout (no swizzle, K-major): 8-row x 16-byte core matrices (4 TF32 per row), contiguous 128 B each;
 //     byte offset of element (row r, k) = (r / 8) * 256 + (k / 4) * 128 + (r % 8) * 16 + (k % 4) * 4
@@ -25,8 +28,9 @@
 // own the TMEM lanes 32 (w % 4) .. + 31 (a warp reaches only its lane quarter): warps 0-3 generate the even stages,
 // warps 4-7 the odd ones, each thread its sample's
 // row of the stage, then tcgen05.wait::st, fence, arrive on the stage's mbarrier; lane 0 of the control warp waits for it,
-// issues the stage's 12 MMAs and commits them to the mbarrier that frees the A stage.  No CTA-wide barrier in the loop.
-// Spin records and B tiles ride a 4-slot TMA ring refilled by the control thread.  Epilogue: tcgen05.ld 32 lanes x 16
+// issues the stage's 8 (32 coils per pass: 12) MMAs and commits them to the mbarrier that frees the A stage.  No
+// CTA-wide barrier in the loop.  Spin records and B tiles ride an 8-slot (32 coils: 6-slot) TMA ring refilled by the
+// control thread.  Epilogue: tcgen05.ld 32 lanes x 16
 // columns per warp -> P[coil][chunk][sample].
 #pragma once
 #include "coils.cuh"
