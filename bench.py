@@ -3,13 +3,14 @@
 free-precession block, the two-pass signal reduction, final state) over one synthetic workload.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4] [--impl ours|reference]
-                    [--scaling weak|strong] [--extra 1,2,3,5,5b | none]
+                    [--scaling weak|strong] [--extra 1,2,3,5,5b,3m,4c,5x4 | none]
 
 Prints ONE JSON line (rank 0).  metric = Bloch spin*steps/s: N_spins x N_intervals of the discretised
 sequence (what the step-by-step solver of the paper executes, SURVEY.md 8(d) "Counting") / device time.
 The headline workload is config 4 (the 1M-spin spiral); the default run also times the other named configs
-(BASELINE.json: "report throughput on the five synthetic workloads") in short runs and reports them under
-"workloads".  See DESIGN.md "Measurement" for the roofline arithmetic.  The reference arm (--impl reference)
+(BASELINE.json: "report throughput on the five synthetic workloads") and one workload per widening row (3m: motion,
+4c: 8 coils block by block on tcgen05, 5x4: 4 coils inside the whole-sequence kernel) in short runs and reports them
+under "workloads".  See DESIGN.md "Measurement" for the roofline arithmetic.  The reference arm (--impl reference)
 times the fp64 CPU oracle, as it stands, on the host cores; it is the only place besides cpu_baseline that
 touches oracle/.
 """
@@ -39,7 +40,7 @@ SM_COUNT = 148
 MUFU_PER_EVAL = 3          # sin, cos, ex2 per (spin, evaluated point)
 FP32_PER_RF_STEP = 46      # Eq 6-9 + 11 written directly, per spin*step
 FP32_PER_EVAL = 15         # FP32-pipe instructions per (spin, evaluated point)
-EXTRA_DEFAULT = "1,2,3,5,5b"
+EXTRA_DEFAULT = "1,2,3,5,5b,3m,4c,5x4"   # the five named configs + motion (f1) + coils per block / in the one launch (f2)
 
 
 def load_peaks():

@@ -9,7 +9,9 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <atomic>
 #include <limits>
+#include <thread>
 #include <utility>
 
 #include "internal.h"
@@ -34,28 +36,52 @@ bool ascending(const double *a, int64_t n, bool strict) {
     return true;
 }
 
-// Piecewise-linear gradient of one axis sampled on the (ascending) grid by a forward sweep.
-void sample_axis(const double *gt, const double *gv, int64_t gn, const std::vector<double> &t,
-                 std::vector<double> &out, int axis) {
-    const size_t np = t.size();
-    int64_t seg = 0;
-    for (size_t n = 0; n < np; ++n) {
-        double v = 0.0;
-        const double tn = t[n];
-        if (gn == 1) {
-            v = (std::fabs(tn - gt[0]) <= kTimeTol) ? gv[0] : 0.0;
-        } else if (gn >= 2 && tn >= gt[0] - kTimeTol && tn <= gt[gn - 1] + kTimeTol) {
-            while (seg + 2 < gn && gt[seg + 1] <= tn) ++seg;
-            const double t0 = gt[seg], t1 = gt[seg + 1];
-            double w = (t1 > t0) ? (tn - t0) / (t1 - t0) : 1.0;
-            w = std::min(1.0, std::max(0.0, w));
-            v = gv[seg] + w * (gv[seg + 1] - gv[seg]);
+// Piecewise-linear gradients of the three axes sampled on the points [n0, n1) of the (ascending) grid by a forward
+// sweep: out[3 n + axis].
+void sample_axes(const bloch_sequence *seq, const std::vector<double> &t, size_t n0, size_t n1, double *out) {
+    for (int axis = 0; axis < 3; ++axis) {
+        const double *gt = seq->g_t[axis], *gv = seq->g_v[axis];
+        const int64_t gn = seq->g_n[axis];
+        int64_t seg = 0;
+        if (gn >= 2 && n0 < n1)  // start the sweep at the segment that holds t[n0]
+            seg = std::max<int64_t>(0, std::min<int64_t>(gn - 2, (std::upper_bound(gt, gt + gn, t[n0]) - gt) - 1));
+        for (size_t n = n0; n < n1; ++n) {
+            double v = 0.0;
+            const double tn = t[n];
+            if (gn == 1) {
+                v = (std::fabs(tn - gt[0]) <= kTimeTol) ? gv[0] : 0.0;
+            } else if (gn >= 2 && tn >= gt[0] - kTimeTol && tn <= gt[gn - 1] + kTimeTol) {
+                while (seg + 2 < gn && gt[seg + 1] <= tn) ++seg;
+                const double t0 = gt[seg], t1 = gt[seg + 1];
+                double w = (t1 > t0) ? (tn - t0) / (t1 - t0) : 1.0;
+                w = std::min(1.0, std::max(0.0, w));
+                v = gv[seg] + w * (gv[seg + 1] - gv[seg]);
+            }
+            out[3 * n + axis] = v;
         }
-        out[3 * n + axis] = v;
     }
 }
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// fn(i) for i in [0, n) on up to `threads` host threads (items handed out in order from a shared counter).  The plan's
+// blocks are independent of one another once the grid is fixed (a3, a4, table fill), and every result is written to
+// the block's own slot, so the tables are the same bytes whatever the thread count.
+template <class F>
+void parallel_for(size_t n, unsigned threads, F fn) {
+    if (threads <= 1 || n <= 1) {
+        for (size_t i = 0; i < n; ++i) fn(i);
+        return;
+    }
+    std::atomic<size_t> next{0};
+    auto work = [&]() {
+        for (size_t i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+    };
+    std::vector<std::thread> pool;
+    for (unsigned k = 1; k < threads; ++k) pool.emplace_back(work);
+    work();
+    for (std::thread &th : pool) th.join();
+}
 
 }  // namespace
 
@@ -224,8 +250,13 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             }
         }
     }
+    // long sequences (config 5: 3.1e6 intervals, 2001 blocks) are planned on several host threads
+    const unsigned n_thr = N < 200000 ? 1u : std::min(16u, std::max(1u, std::thread::hardware_concurrency()));
     std::vector<double> G(3 * t.size(), 0.0);
-    for (int a = 0; a < 3; ++a) sample_axis(seq->g_t[a], seq->g_v[a], seq->g_n[a], t, G, a);
+    {   // contiguous slices of the grid, one sweep per slice (the segment a slice starts in is found by bisection)
+        const size_t n_sl = n_thr > 1 ? 4 * n_thr : 1, np = t.size();
+        parallel_for(n_sl, n_thr, [&](size_t k) { sample_axes(seq, t, np * k / n_sl, np * (k + 1) / n_sl, G.data()); });
+    }
     // ADC index per point (both ascending)
     std::vector<int64_t> adc_at(t.size(), -1);
     {
@@ -303,20 +334,40 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     std::vector<double> mrec;  // motion: (mu'x, mu'y, mu'z, 0) per evaluated point, same order
     std::vector<int64_t> krec_first(blocks.size(), 0);
     int64_t n_rf_steps = 0, n_rf_blocks = 0, n_eval = 0, max_block_adc = 0;
-    for (size_t bi = 0; bi < blocks.size(); ++bi) {
-        Block &b = blocks[bi];
-        if (b.type == kBlockRF) {
-            n_rf_steps += b.count;
-            ++n_rf_blocks;
-            continue;
+    {
+        int64_t n_rec = 0;  // a block's records start where the blocks before it end: one per ADC sample it serves
+        for (size_t bi = 0; bi < blocks.size(); ++bi) {
+            const Block &b = blocks[bi];
+            if (b.type == kBlockRF) {
+                n_rf_steps += b.count;
+                ++n_rf_blocks;
+                continue;
+            }
+            krec_first[bi] = n_rec;
+            n_rec += b.adc_count;
+            n_eval += b.adc_count + 1;
+            max_block_adc = std::max(max_block_adc, b.adc_count);
         }
-        krec_first[bi] = (int64_t)krec.size() / 4;
+        krec.resize(4 * (size_t)n_rec);
+        if (motion) mrec.resize(4 * (size_t)n_rec);
+    }
+    struct A3Max { double worst = 0.0, k = 0.0, tau = 0.0, m = 0.0; };
+    std::vector<A3Max> a3max(blocks.size());
+    std::atomic<int> a3_bad{0};
+    parallel_for(blocks.size(), n_thr, [&](size_t bi) {
+        Block &b = blocks[bi];
+        if (b.type == kBlockRF) return;
+        A3Max &mx = a3max[bi];
+        double *kr = krec.data() + 4 * krec_first[bi];
+        double *mr = motion ? mrec.data() + 4 * krec_first[bi] : nullptr;
+        int64_t w = 0;  // records written
         const bool serve_start = (bi == 0) || (blocks[bi - 1].type == kBlockRF);
         double K[3] = {0, 0, 0}, Mo[3] = {0, 0, 0};
         const double tb = t[b.first];
-        if (serve_start && adc_at[b.first] >= 0) {
-            krec.insert(krec.end(), {0.0, 0.0, 0.0, 0.0});
-            if (motion) mrec.insert(mrec.end(), {0.0, 0.0, 0.0, 0.0});
+        if (serve_start && adc_at[b.first] >= 0 && w < b.adc_count) {
+            for (int c = 0; c < 4; ++c) kr[c] = 0.0;
+            if (motion) for (int c = 0; c < 4; ++c) mr[c] = 0.0;
+            ++w;
         }
         for (int64_t n = b.first; n < b.first + b.count; ++n) {
             const double dt = t[n + 1] - t[n];
@@ -326,25 +377,35 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                 for (int a = 0; a < 3; ++a) Mo[a] += 0.5 * (G[3 * n + a] * u[n] + G[3 * (n + 1) + a] * u[n + 1]) * dt;
             const double tau = t[n + 1] - tb;
             const double kn = gbar * std::sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]);
-            const double mn = gbar * std::sqrt(Mo[0] * Mo[0] + Mo[1] * Mo[1] + Mo[2] * Mo[2]);
+            const double mn = motion ? gbar * std::sqrt(Mo[0] * Mo[0] + Mo[1] * Mo[1] + Mo[2] * Mo[2]) : 0.0;
             // |theta| <= |k'| |x| + |f| tau (+ |mu'| |v|): the bound within the declared extents, and its three
             // factors on their own for the check against the phantom a simulation is actually given (api.cu)
-            worst_turns = std::max(worst_turns, kn * ext_m + ext_hz * tau + (motion ? mn * ext_mps : 0.0));
-            k_max = std::max(k_max, kn);
-            tau_max = std::max(tau_max, tau);
-            if (motion) m_max = std::max(m_max, mn);
+            mx.worst = std::max(mx.worst, kn * ext_m + ext_hz * tau + (motion ? mn * ext_mps : 0.0));
+            mx.k = std::max(mx.k, kn);
+            mx.tau = std::max(mx.tau, tau);
+            if (motion) mx.m = std::max(mx.m, mn);
             if (adc_at[n + 1] >= 0) {
-                krec.insert(krec.end(), {-gbar * K[0], -gbar * K[1], -gbar * K[2], tau});
-                if (motion) mrec.insert(mrec.end(), {-gbar * Mo[0], -gbar * Mo[1], -gbar * Mo[2], 0.0});
+                if (w >= b.adc_count) { a3_bad.store(1); break; }
+                double *q = kr + 4 * w;
+                q[0] = -gbar * K[0]; q[1] = -gbar * K[1]; q[2] = -gbar * K[2]; q[3] = tau;
+                if (motion) {
+                    double *qm = mr + 4 * w;
+                    qm[0] = -gbar * Mo[0]; qm[1] = -gbar * Mo[1]; qm[2] = -gbar * Mo[2]; qm[3] = 0.0;
+                }
+                ++w;
             }
         }
         for (int a = 0; a < 3; ++a) b.kend[a] = -gbar * K[a];
         for (int a = 0; a < 3; ++a) b.mend[a] = -gbar * Mo[a];
         b.tau_end = t[b.first + b.count] - tb;
-        n_eval += b.adc_count + 1;
-        max_block_adc = std::max(max_block_adc, b.adc_count);
-        if ((int64_t)krec.size() / 4 - krec_first[bi] != b.adc_count)
-            return fail(BLOCH_EINVAL, "internal: ADC bookkeeping mismatch");
+        if (w != b.adc_count) a3_bad.store(1);
+    });
+    if (a3_bad.load()) return fail(BLOCH_EINVAL, "internal: ADC bookkeeping mismatch");
+    for (const A3Max &mx : a3max) {
+        worst_turns = std::max(worst_turns, mx.worst);
+        k_max = std::max(k_max, mx.k);
+        tau_max = std::max(tau_max, mx.tau);
+        m_max = std::max(m_max, mx.m);
     }
     // AUTO: fp32 phase (in turns, block-relative) keeps ~2^-24 * turns of resolution; above 256 turns
     // (bound: |k| max_extent_m + max_offres_hz tau, + |mu'| max_speed_mps with motion) switch to fp64 phase
@@ -357,9 +418,10 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
 
     // ------------------------------------------------------------------ a4: RF tile images
     std::vector<std::vector<unsigned char>> rf_img(blocks.size());
-    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+    std::atomic<int> a4_bad{0};
+    parallel_for(blocks.size(), n_thr, [&](size_t bi) {
         Block &b = blocks[bi];
-        if (b.type != kBlockRF) continue;
+        if (b.type != kBlockRF) return;
         // per step, in fp32 as the kernel sees them: rotation vector w = gamma * B * dt (Eq 8); the gradient
         // part is per metre, mean of the two vertex values (reading G5)
         struct StepF { float wx, wy, g[3], dt, h[3]; };
@@ -425,16 +487,16 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             dir[2 * ti] = (int32_t)off0;
             dir[2 * ti + 1] = (int32_t)(img.size() - off0);
         }
-        if (img.size() > (size_t)INT32_MAX) return fail(BLOCH_EINVAL, "RF block table exceeds 2 GiB");
-    }
+        if (img.size() > (size_t)INT32_MAX) a4_bad.store(1);
+    });
+    if (a4_bad.load()) return fail(BLOCH_EINVAL, "RF block table exceeds 2 GiB");
 
     // ------------------------------------------------------------------ tables: layout + fill
     size_t off = 0;
     // precession records: (k', tau) per ADC sample, followed by (mu', 0) with motion
     const size_t rec_bytes = (phase == BLOCH_PHASE_FP64 ? 32 : 16) * (motion ? 2 : 1);
-    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+    parallel_for(blocks.size(), n_thr, [&](size_t bi) {
         Block &b = blocks[bi];
-        b.table_off = (int64_t)off;
         // Cartesian readouts: does k' (and tau) advance by a constant step inside EVERY aligned group of 16 samples?
         // Checked on the fp64 records (turns / m): every sample within 1e-13 relative + 1e-8 turns / m (1e-13 s) of the
         // line through the group's first and last sample, the level at which the ADC times themselves are equally
@@ -470,6 +532,10 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
             }
             if (ok) b.lin_pts = n_g * 16;
         }
+    });
+    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+        Block &b = blocks[bi];
+        b.table_off = (int64_t)off;
         const size_t bytes = b.type == kBlockRF ? rf_img[bi].size() : size_t(b.adc_count) * rec_bytes;
         off = align_up(off + bytes, kAlign);
     }
@@ -502,7 +568,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         op.tau_end = b.tau_end;
         std::memcpy(plan->tables.data() + prog_off + bi * sizeof(SeqOp), &op, sizeof(op));
     }
-    for (size_t bi = 0; bi < blocks.size(); ++bi) {
+    parallel_for(blocks.size(), n_thr, [&](size_t bi) {
         const Block &b = blocks[bi];
         unsigned char *dst = plan->tables.data() + b.table_off;
         if (b.type == kBlockRF) {
@@ -526,7 +592,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                 }
             }
         }
-    }
+    });
 
     // ------------------------------------------------------------------ launch count (SUM_ALL, final state)
     int64_t launches = 2;  // pack + unpack
