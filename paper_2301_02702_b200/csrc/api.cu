@@ -421,10 +421,11 @@ struct Taps {
 };
 
 // remember the largest launch of a kind (threads in flight) for bloch_plan_last_kernel
-void note_kernel(const bloch_plan *plan, int kind, int64_t grid, int block, const char *fmt, int a = 0, int b = 0, int c = 0) {
+void note_kernel(const bloch_plan *plan, int kind, int64_t grid, int block, const char *fmt, int a = 0, int b = 0, int c = 0,
+                 int d = 0) {
     KernelNote &k = plan->last_kernel[kind];
     if (grid * block < k.grid * k.block) return;
-    std::snprintf(k.name, sizeof k.name, fmt, a, b, c);
+    std::snprintf(k.name, sizeof k.name, fmt, a, b, c, d);
     k.grid = grid;
     k.block = block;
 }
@@ -930,8 +931,8 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else BLOCH_LAUNCH_COIL(PP, NCC, false, false, w.A, nullptr);           \
     } while (0)
                     if (tc) note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, kTcThreads, "signal_coils_tc_kernel<%d>", ncp);
-                    else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d>",
-                                     s.P == 2 ? 2 : 1, ncp == 8 ? 8 : 4, ph64 ? 1 : 0);
+                    else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d, %d>",
+                                     s.P == 2 ? 2 : 1, ncp == 8 ? 8 : 4, ph64 ? 1 : 0, mo ? 1 : 0);
                     if (tc) {
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
                         if (ncp == 32)
