@@ -338,7 +338,7 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *   BLOCH_OPT_COIL_TC             multi-coil receive: -1 (default) and 1: tensor cores (tcgen05, A operand in tensor
  *                                 memory) whenever they apply (more than 4 coils, fp32 phase); 0: never
  *   BLOCH_OPT_SEQ_SIG_EXTRA       whole-sequence kernel: signal warps added per missing RF warp of a sub-partition,
- *                                 0..7, default 2
+ *                                 0..7; -1 (default): 2, or 0 with receive coils
  *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic
  *   BLOCH_OPT_SEQ_ITEMS_X4        whole-sequence kernel: readout items per signal warp x 4 that the item size must
  *                                 leave; 0 (default) always the largest item */

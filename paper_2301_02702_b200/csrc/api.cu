@@ -204,7 +204,11 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
     for (int k = 0; k < 4; ++k) rf_per[k] = q.rf_warps / 4;
     { const int order[4] = {1, 2, 3, 0}; for (int e = 0; e < q.rf_warps % 4; ++e) ++rf_per[order[e]]; }
     const int rf_max = *std::max_element(rf_per, rf_per + 4);
-    const int sig_extra = std::min(std::max(plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA], 0), 7);
+    // -1: two per missing RF warp; none with coils, where the signal warps are the heavier load and an equal number per
+    // sub-partition is the better balance (config 5 x 4 coils: 4,4,4,4 162.6 ms against 168.8 for 5,3,3,5; x 8 coils
+    // 205.2 against 213.0)
+    const int sig_extra = plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA] < 0 ? (q.nc > 0 ? 0 : 2)
+                                                                 : std::min(plan->opt[BLOCH_OPT_SEQ_SIG_EXTRA], 7);
     int deficit = 0;
     for (int k = 0; k < 4; ++k) deficit += rf_max - rf_per[k];
     // with coils an evaluation costs (15 + 4 nc) / 15 of a plain one and has no P > 1 savings: ask for as many signal
@@ -276,8 +280,8 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
     q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || full_layout));
     // Coils under AUTO: the 8-wide sums cost ~50 issue slots per evaluation on the FMA pipe, so once a block holds
     // enough (spin, sample) pairs to fill the tcgen05 kernel the per-block launches win.  Measured, fused / per-block
-    // ms: config 5 x 8 coils (6.7e7 pairs per block) 212-221 / 198.7; config 2 x 8 coils (1.0e6) 2.25 / 3.36; up to 4
-    // coils the launch wins on both (config 5 x 4: 178.5 / 206.8; config 2 x 4: 2.15 / 3.19).
+    // ms: config 5 x 8 coils (6.7e7 pairs per block) 205.2 / 198.7; config 2 x 8 coils (1.0e6) 2.22 / 3.36; up to 4
+    // coils the launch wins on both (config 5 x 4: 162.6 / 206.8; config 2 x 4: 2.13 / 3.19).
     if (q.nc == 8 && plan->path != BLOCH_PATH_FUSED && plan->opt[BLOCH_OPT_COIL_TC] != 0 &&
         n_spins * inf.max_block_adc >= (int64_t(1) << 24))
         q.use = false;
@@ -606,7 +610,7 @@ int bloch_plan_set_option(bloch_plan *plan, int key, int value) {
         case BLOCH_OPT_RF_THREADS: ok = value == 0 || value == 32 || value == 64 || value == 128; break;
         case BLOCH_OPT_RF_SPINS: ok = value >= 0 && value <= 2; break;
         case BLOCH_OPT_COIL_TC: ok = value >= -1 && value <= 1; break;
-        case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= 0 && value <= 7; break;
+        case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_SIG_BASE: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_ITEMS_X4: ok = value >= 0 && value <= 64; break;
         default: return fail(BLOCH_EINVAL, "unknown BLOCH_OPT_* key");

@@ -119,7 +119,7 @@ struct bloch_plan {
     int64_t n_adc_blocks = 0;            // precession blocks that serve ADC samples
     int64_t adcblk_off = 0;              // byte offset of the SeqAdcBlock array in the table buffer
     int path = 0;                        // BLOCH_PATH_*
-    int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, 2, -1, 0};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
+    int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, -1, -1, 0};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
     // phase-range bookkeeping (bloch_sim_params extents): largest |k'| [turns/m], tau [s] and |mu'| [turns s/m] of
     // any evaluated point (block ends included), and the largest phase within the declared extents
     double k_max = 0, tau_max = 0, m_max = 0, worst_turns = 0;

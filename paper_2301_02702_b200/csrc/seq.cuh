@@ -221,11 +221,13 @@ __device__ __forceinline__ void seq_signal_item_coils(const float4 *__restrict__
         cmax = fmaxf(cmax, fabsf(cj[j]));
     }
     const bool series = P > 1 && __all_sync(0xffffffffu, cmax * r2max_log2e <= 0.02f);  // as seq_signal_item
-    float ar[P][NC], ai[P][NC];
+    // coil sums in pairs (coils 2k, 2k + 1): the complex multiply-adds run as packed FP32 (fma.rn.f32x2: one issue slot
+    // for two coils; each lane rounds as fmaf does)
+    float2 ar[P][NC / 2], ai[P][NC / 2];
 #pragma unroll
     for (int j = 0; j < P; ++j)
 #pragma unroll
-        for (int c = 0; c < NC; ++c) { ar[j][c] = 0.f; ai[j][c] = 0.f; }
+        for (int k = 0; k < NC / 2; ++k) { ar[j][k] = make_float2(0.f, 0.f); ai[j][k] = make_float2(0.f, 0.f); }
     auto run = [&](auto mode_tag) {
         constexpr int MODE = decltype(mode_tag)::value;  // 0: MUFU.EX2 per sample, 1: series from sample 0
 #pragma unroll 2
@@ -236,13 +238,14 @@ __device__ __forceinline__ void seq_signal_item_coils(const float4 *__restrict__
             signal_spin_fp32<P, MODE>(kx, ky, kz, tau, cj, shA[s], shS[s], cr, ci);
 #pragma unroll
             for (int k = 0; k < NC / 2; ++k) {
-                const float4 w = shW[s * (NC / 2) + k];  // two coils' weights
+                const float4 w = shW[s * (NC / 2) + k];  // two coils' weights as (re, re', im, im')
+                const float2 wr = make_float2(w.x, w.y), wi = make_float2(w.z, w.w);
 #pragma unroll
                 for (int j = 0; j < P; ++j) {
-                    ar[j][2 * k] = fmaf(cr[j], w.x, fmaf(-ci[j], w.y, ar[j][2 * k]));
-                    ai[j][2 * k] = fmaf(cr[j], w.y, fmaf(ci[j], w.x, ai[j][2 * k]));
-                    ar[j][2 * k + 1] = fmaf(cr[j], w.z, fmaf(-ci[j], w.w, ar[j][2 * k + 1]));
-                    ai[j][2 * k + 1] = fmaf(cr[j], w.w, fmaf(ci[j], w.z, ai[j][2 * k + 1]));
+                    const float2 c2 = make_float2(cr[j], cr[j]), d2 = make_float2(ci[j], ci[j]),
+                                 n2 = make_float2(-ci[j], -ci[j]);
+                    ar[j][k] = __ffma2_rn(c2, wr, __ffma2_rn(n2, wi, ar[j][k]));
+                    ai[j][k] = __ffma2_rn(c2, wi, __ffma2_rn(d2, wr, ai[j][k]));
                 }
             }
         }
@@ -253,7 +256,10 @@ __device__ __forceinline__ void seq_signal_item_coils(const float4 *__restrict__
     for (int j = 0; j < P; ++j)
         if (p0 + j < n_pts) {
 #pragma unroll
-            for (int c = 0; c < NC; ++c) out[(size_t)c * slot_stride + p0 + j] = make_float2(ar[j][c], ai[j][c]);
+            for (int k = 0; k < NC / 2; ++k) {
+                out[(size_t)(2 * k) * slot_stride + p0 + j] = make_float2(ar[j][k].x, ai[j][k].x);
+                out[(size_t)(2 * k + 1) * slot_stride + p0 + j] = make_float2(ar[j][k].y, ai[j][k].y);
+            }
         }
 }
 
@@ -354,7 +360,10 @@ seq_kernel(const unsigned char *__restrict__ tables, const SeqOp *__restrict__ o
             shA[r] = a;
             if constexpr (NC > 0) {  // visible to the signal warps with the first published state (st_full)
 #pragma unroll
-                for (int k = 0; k < NC / 2; ++k) shW[r * (NC / 2) + k] = Wc[(size_t)i * (NC / 2) + k];
+                for (int k = 0; k < NC / 2; ++k) {  // (re, im, re', im') of coils 2k, 2k + 1 -> (re, re', im, im')
+                    const float4 w = Wc[(size_t)i * (NC / 2) + k];
+                    shW[r * (NC / 2) + k] = make_float4(w.x, w.z, w.y, w.w);
+                }
             }
         }
         float hx = s.x, hy = s.y, hz = s.z, lx = 0.f, ly = 0.f, lz = 0.f;
