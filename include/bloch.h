@@ -274,7 +274,8 @@ int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t 
  * (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  Moving spins: bloch_simulate_coils_motion (motion plans; velocities /
  * amplitudes as bloch_simulate_motion, all three NULL = none).  The coil-independent part of every evaluation (phase,
  * sin / cos / exp) is computed once per 4 or 8 coils; with more than 4 coils (fp32 phase) the sum over spins runs on the
- * tensor cores (tcgen05 with the generated operand in tensor memory, 3xTF32, 8, 16 or 32 coils per pass).  Plans that
+ * tensor cores (tcgen05 with the generated operand in tensor memory, two FP16 pieces per value with FP32 accumulation
+ * -- 22 significant bits, as 3xTF32 --, 8, 16 or 32 coils per pass).  Plans that
  * take the whole-sequence kernel (BLOCH_PATH_FUSED, or AUTO where it qualifies: static spins, fp32 phase) sum up to 8
  * coils inside that one launch; more coils, or 8 coils on blocks large enough for the tensor-core kernel, run block by
  * block (BLOCH_PATH_FUSED with more than 8 coils: BLOCH_EINVAL).  Asynchronous on `stream`; never allocates. */
@@ -335,8 +336,10 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *   BLOCH_OPT_RF_THREADS          0 (default): 128-thread excitation CTAs once there are >= 32 warps per SM, else 32;
  *                                 32 / 64 / 128 forces it
  *   BLOCH_OPT_RF_SPINS            spins per thread of the excitation kernel: 0 (default) the library's choice, 1 or 2
- *   BLOCH_OPT_COIL_TC             multi-coil receive: -1 (default) and 1: tensor cores (tcgen05, A operand in tensor
- *                                 memory) whenever they apply (more than 4 coils, fp32 phase); 0: never
+ *   BLOCH_OPT_COIL_TC             multi-coil receive: tensor cores (tcgen05, A operand in tensor memory) whenever
+ *                                 they apply (more than 4 coils, fp32 phase, static spins): -1 (default) and 2 with
+ *                                 FP16 operand pieces scaled from measured maxima (2 instructions per 8 spins), 1 with
+ *                                 3xTF32 (4 instructions); 0: never (the FFMA kernel)
  *   BLOCH_OPT_SEQ_SIG_EXTRA       whole-sequence kernel: signal warps added per missing RF warp of a sub-partition,
  *                                 0..7; -1 (default): 2, or 0 with receive coils
  *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic

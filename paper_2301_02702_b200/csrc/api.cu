@@ -12,6 +12,7 @@
 #include "kernels.cuh"
 #include "coils.cuh"
 #include "coils_tc.cuh"
+#include "coils_h.cuh"
 #include "rf.cuh"
 #include "seq.cuh"
 #include "signal.cuh"
@@ -39,7 +40,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 constexpr int kMaxDevices = 64;
 struct DeviceInfo {
     std::atomic<int> sms{0}, major{0};
-    std::atomic<bool> seq_attr{false}, tc_attr{false};
+    std::atomic<bool> seq_attr{false}, tc_attr{false}, h_attr{false};
 };
 DeviceInfo g_dev[kMaxDevices];
 
@@ -291,7 +292,7 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
 // tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 288 threads, 2 CTAs per SM, chunks of whole 16-spin stages
 bool coil_use_tc(const bloch_plan *plan, int n_coils) {
-    // BLOCH_OPT_COIL_TC: 0 = never, -1 / 1 = whenever it applies: more than 4 coils and fp32 phase.  With the A operand
+    // BLOCH_OPT_COIL_TC: 0 = never, -1 / 1 / 2 = whenever it applies: more than 4 coils and fp32 phase.  With the A operand
     // in tensor memory one pass of the tcgen05 kernel costs the same for 8, 16 and 32 coils (config 4: 106-107 ms)
     // and beats the FFMA kernel from its first pass of 8 (121 ms); up to 4 coils the 4-wide FFMA kernel (~90 ms) stays.
     const int mode = plan->opt[BLOCH_OPT_COIL_TC];
@@ -306,6 +307,12 @@ bool coil_use_fused(const bloch_plan *plan, int64_t n_spins, int sm_count, int n
     const SeqShape q = seq_shape(plan, n_spins, sm_count, n_coils);
     return q.ok && q.use;
 }
+
+// which tensor-core kernel: FP16 operands (coils_h.cuh, 2 instructions per 8 spins) or 3xTF32 (coils_tc.cuh, 4)
+// Measured on config 4 (signal kernels, per simulation): 8 coils 93.2 -> 85.3 ms, 16 coils 94.2 -> 86.3, 32 coils
+// 106.4 -> 87.6; rounded (not truncated) operand pieces: errors against the oracle 2-3x smaller.  -1 (default) and 2:
+// FP16; 1: 3xTF32.
+bool coil_tc_fp16(const bloch_plan *plan) { return plan->opt[BLOCH_OPT_COIL_TC] != 1; }
 
 SigShape coil_shape(int64_t n_pts, int64_t n_spins, int sm_count, int ncp, bool tc) {
     if (tc) {
@@ -609,7 +616,7 @@ int bloch_plan_set_option(bloch_plan *plan, int key, int value) {
         case BLOCH_OPT_SIGNAL_CTAS_PER_SM: ok = value >= 1 && value <= 8; break;
         case BLOCH_OPT_RF_THREADS: ok = value == 0 || value == 32 || value == 64 || value == 128; break;
         case BLOCH_OPT_RF_SPINS: ok = value >= 0 && value <= 2; break;
-        case BLOCH_OPT_COIL_TC: ok = value >= -1 && value <= 1; break;
+        case BLOCH_OPT_COIL_TC: ok = value >= -1 && value <= 2; break;
         case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_SIG_BASE: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_ITEMS_X4: ok = value >= 0 && value <= 64; break;
@@ -772,7 +779,23 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
     const int n_pass = (n_coils + ncp - 1) / ncp;
     const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;
     DeviceInfo *devinfo = current_device();  // non-NULL: check_arch passed
-    if (tc) {
+    const bool tc_h = tc && coil_tc_fp16(plan);
+    if (tc_h) {
+        if (!devinfo->h_attr.load(std::memory_order_acquire)) {  // once per DEVICE (the attribute is per device)
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_h_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem(8)));
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_h_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem(16)));
+            BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_h_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem(32)));
+            devinfo->h_attr.store(true, std::memory_order_release);
+        }
+        // operand scales from measured maxima (scal[6], scal[7]; cleared with the findings word above), then the B tiles
+        coil_scales_kernel<<<std::min(4 * sms, (n + 255) / 256 * std::max(n_coils, 1)), 256, 0, stream>>>(
+            n, w.C, w.S, (const float2 *)d_coil, (long long)n_coils * n, w.scal);
+        const dim3 pg((n_pad + 255) / 256, n_pass);
+        if (ncp == 32) pack_coils_h_kernel<32><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, w.scal, (unsigned char *)w.W);
+        else if (ncp == 16) pack_coils_h_kernel<16><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, w.scal, (unsigned char *)w.W);
+        else pack_coils_h_kernel<8><<<pg, 256, 0, stream>>>(n, n_pad, n_coils, (const float2 *)d_coil, w.scal, (unsigned char *)w.W);
+        launches += 2;
+    } else if (tc) {
         if (!devinfo->tc_attr.load(std::memory_order_acquire)) {  // once per DEVICE (the attribute is per device)
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(8)));
             BLOCH_CUDA(cudaFuncSetAttribute(signal_coils_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem(16)));
@@ -934,10 +957,22 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         else if (mo) BLOCH_LAUNCH_COIL(PP, NCC, false, true, w.A, w.V);        \
         else BLOCH_LAUNCH_COIL(PP, NCC, false, false, w.A, nullptr);           \
     } while (0)
-                    if (tc) note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, kTcThreads, "signal_coils_tc_kernel<%d>", ncp);
+                    if (tc) note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, kTcThreads,
+                                        tc_h ? "signal_coils_h_kernel<%d>" : "signal_coils_tc_kernel<%d>", ncp);
                     else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d, %d>",
                                      s.P == 2 ? 2 : 1, ncp == 8 ? 8 : 4, ph64 ? 1 : 0, mo ? 1 : 0);
-                    if (tc) {
+                    if (tc_h) {
+                        const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * h_btile(ncp);
+                        if (ncp == 32)
+                            signal_coils_h_kernel<32><<<grid, kTcThreads, h_smem(32), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                        else if (ncp == 16)
+                            signal_coils_h_kernel<16><<<grid, kTcThreads, h_smem(16), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                        else
+                            signal_coils_h_kernel<8><<<grid, kTcThreads, h_smem(8), stream>>>(
+                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                    } else if (tc) {
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
                         if (ncp == 32)
                             signal_coils_tc_kernel<32><<<grid, kTcThreads, tc_smem(32), stream>>>(

@@ -121,16 +121,18 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
     assert np.abs(mz).max() > 0.1
 
 
+@pytest.mark.parametrize("tc", [1, 2])
 @pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20), ("4", 37)])
-def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils):
+def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils, tc):
     """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with bloch_plan_set_option(BLOCH_OPT_COIL_TC, 1)): contributions generated on the fly
     as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
     tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8, 16 and 32 coils per pass and two passes (37 coils) are all in these cases."""
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
     ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
-    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32", options={"coil_tc": 1}, path="per_block")
-    assert_parity(got, ref, f"tensor-core coil kernel, config {name}, {n_coils} coils")
+    got, gxy, gz, launches = run_coils(B, w, coils, want_state=True, phase_mode="fp32", options={"coil_tc": tc}, path="per_block")
+    emax, nrmse = assert_parity(got, ref, f"tensor-core coil kernel, config {name}, {n_coils} coils")
+    print(f"coil_tc={tc} config {name} {n_coils} coils: max {emax:.3e} nrmse {nrmse:.3e}")
     for c in range(n_coils):
         emax, nrmse = errors(got[c], ref[c])
         assert emax <= 1e-4 and nrmse <= 1e-5, f"coil {c}: max {emax:.3e} nrmse {nrmse:.3e}"
@@ -258,3 +260,36 @@ def test_fused_coils_limits_and_auto_choice(B):
     e, _ = errors(u["sig"][0], plain.cpu().numpy())
     plan.close()
     assert e < 2e-6, f"{e:.3e}"
+
+
+@pytest.mark.parametrize("m_scale,w_scale,init", [(1.0, 1.0, "big"), (2.0 ** -14, 2.0 ** 17, "eq"), (3.0e4, 7.0e-6, "eq"),
+                                                 (1.0, 0.0, "eq")])
+def test_fp16_tensor_core_coil_kernel_scales_its_operands(B, oracle_mod, m_scale, w_scale, init):
+    """The FP16 tensor-core coil kernel (csrc/coils_h.cuh) scales both MMA operands by powers of two taken from measured
+    maxima (FP16 has 5 exponent bits): magnetisations and coil weights far from 1, an initial state larger than M0, and
+    all-zero weights must come out as the oracle has them, on the scale of the result."""
+    import dataclasses
+    w = W.small("4")
+    ph = dataclasses.replace(w.phantom, M0=(w.phantom.M0 * m_scale).astype(np.float32).astype(np.float64))
+    w = dataclasses.replace(w, phantom=ph)
+    coils = (coil_maps(ph, 8, seed=5) * w_scale).astype(np.complex64)
+    state = None
+    if init == "big":   # |M(0)| = 3 M0, tipped: the bound on |M| is max(M0, |M(0)|)
+        state = ((2.0 * ph.M0 * np.exp(0.3j * np.arange(ph.n))).astype(np.complex64), (2.2 * ph.M0).astype(np.float32))
+    ref = oracle_mod.simulate(ph, w.seq, coils=coils.astype(np.complex128),
+                              state=None if state is None else (state[0].astype(np.complex128), state[1].astype(np.float64)))
+    import torch
+    plan = B.Plan(w.seq, path="per_block", phase_mode="fp32", options={"coil_tc": 2})
+    dev = B.phantom_to_device(ph)
+    kw = {}
+    if state is not None:
+        kw = dict(Mxy=torch.view_as_real(torch.from_numpy(state[0]).cuda()).contiguous(), Mz=torch.from_numpy(state[1]).cuda(),
+                  init_equilibrium=False)
+    got = plan.simulate(*dev, coils=torch.from_numpy(coils).cuda(), **kw).cpu().numpy()
+    assert B.bloch_plan_last_kernel(plan.handle, "signal")["name"] == "signal_coils_h_kernel<8>"
+    plan.close()
+    if w_scale == 0.0:
+        assert not got.any() and not np.asarray(ref).any()
+        return
+    emax, nrmse = assert_parity(got, ref, f"fp16 coil kernel, M0 x {m_scale:g}, weights x {w_scale:g}, init {init}")
+    print(f"fp16 coil kernel, M0 x {m_scale:g}, weights x {w_scale:g}, init {init}: max {emax:.3e} nrmse {nrmse:.3e}")

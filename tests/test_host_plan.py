@@ -196,7 +196,7 @@ def test_plan_options_are_plan_state_not_environment(B):
         assert B.bloch_plan_get_option(h, "signal_lin") == 0 and B.bloch_plan_get_option(h, "signal_p") == 4
         info = B.bloch_plan_get_info(h)
         assert info["options"]["signal_lin"] == 0 and info["options"]["signal_p"] == 4
-        for key, bad in (("signal_p", 3), ("signal_ctas_per_sm", 0), ("rf_threads", 48), ("coil_tc", 2), (99, 0),
+        for key, bad in (("signal_p", 3), ("signal_ctas_per_sm", 0), ("rf_threads", 48), ("coil_tc", 3), (99, 0),
                          ("rf_spins", 3)):
             with pytest.raises(B.BlochError) as e:
                 B.bloch_plan_set_option(h, key, bad)
