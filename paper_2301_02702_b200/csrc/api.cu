@@ -291,13 +291,18 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
 
 // Multi-coil signal kernel (coils.cuh): P = 2 adjacent samples per thread (8 x P accumulators), grid as sig_shape.
 // tc: the tcgen05 kernel (coils_tc.cuh): 128 samples per CTA of 288 threads, 2 CTAs per SM, chunks of whole 16-spin stages
-bool coil_use_tc(const bloch_plan *plan, int n_coils) {
-    // BLOCH_OPT_COIL_TC: 0 = never, -1 / 1 / 2 = whenever it applies: more than 4 coils and fp32 phase.  With the A operand
-    // in tensor memory one pass of the tcgen05 kernel costs the same for 8, 16 and 32 coils (config 4: 106-107 ms)
-    // and beats the FFMA kernel from its first pass of 8 (121 ms); up to 4 coils the 4-wide FFMA kernel (~90 ms) stays.
+bool coil_use_tc(const bloch_plan *plan, int64_t n_spins, int n_coils) {
+    // BLOCH_OPT_COIL_TC: 0 = never; otherwise whenever it applies: fp32 phase, static spins (moving spins and fp64 phase:
+    // the FFMA kernel) and
+    //   1 (3xTF32 kernel, coils_tc.cuh): more than 4 coils -- one pass costs the same for 8, 16 and 32 coils (config 4:
+    //     93-107 ms) and beats the FFMA kernel from its first pass of 8 (121 ms); up to 4 coils the 4-wide FFMA kernel
+    //     (93 ms) stays;
+    //   -1 (default) / 2 (FP16 kernel, coils_h.cuh): any number of coils once there are 4096 spins -- a pass of up to 8
+    //     coils takes 80.9 ms on config 4, less than the 4-wide FFMA kernel's 93.2 for 1 to 4 coils.
     const int mode = plan->opt[BLOCH_OPT_COIL_TC];
-    return mode != 0 && n_coils > 4 && plan->info.phase_mode == BLOCH_PHASE_FP32 &&
-           plan->info.motion_mode == BLOCH_MOTION_NONE;  // moving spins: the FFMA kernel
+    if (mode == 0 || n_coils < 1 || plan->info.phase_mode != BLOCH_PHASE_FP32 || plan->info.motion_mode != BLOCH_MOTION_NONE)
+        return false;
+    return n_coils > 4 || (mode != 1 && n_spins >= 4096);
 }
 
 // Multi-coil receive inside the whole-sequence kernel (seq_kernel<false, NC>): when the plan takes that path for
@@ -393,14 +398,14 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     if (plan->info.output_mode == BLOCH_OUT_SUM_ALL) {
         const SeqShape q = seq_shape(plan, n_spins, sm_count, n_coils);
         if (n_coils > 0 && !(q.ok && q.use)) {
-            const bool tc_ = coil_use_tc(plan, n_coils);
+            const bool tc_ = coil_use_tc(plan, n_spins, n_coils);
             w.partial_elems = coil_partial_elems_for(plan, n_spins, sm_count, tc_ ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils), tc_);
         }
         else w.partial_elems = (q.ok && q.use) ? q.partial_elems : partial_elems_for(plan, n_spins, sm_count);
         pbytes = w.partial_elems * sizeof(float2);
     }
     w.partial = (float2 *)take(pbytes);
-    const bool tc_ws = n_coils > 0 && coil_use_tc(plan, n_coils) && !coil_use_fused(plan, n_spins, sm_count, n_coils);
+    const bool tc_ws = n_coils > 0 && coil_use_tc(plan, n_spins, n_coils) && !coil_use_fused(plan, n_spins, sm_count, n_coils);
     const int ncp = tc_ws ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const size_t n_pass = size_t((n_coils + ncp - 1) / ncp);
     // the tcgen05 kernel takes its weights as ready-made B tiles: 2048 B per 8 spins (spins padded to whole stages)
@@ -774,7 +779,7 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                                                      w.A, w.C, w.S, w.Ad, w.scal, d_vx, d_vy, d_vz, w.V, w.Vd);
     ++launches;
     const bool coil_fused = coil_use_fused(plan, n_spins, sms, n_coils);
-    const bool tc = n_coils > 0 && !coil_fused && coil_use_tc(plan, n_coils);
+    const bool tc = n_coils > 0 && !coil_fused && coil_use_tc(plan, n_spins, n_coils);
     const int ncp = tc ? tc_coils_per_pass(n_coils) : coils_per_pass(n_coils);
     const int n_pass = (n_coils + ncp - 1) / ncp;
     const int n_pad = (n + kTcStageSpins - 1) / kTcStageSpins * kTcStageSpins;

@@ -7,19 +7,21 @@
 // shape costs ~74 clocks whatever N and K, so the instruction count decides:
 //   * K = 16 halves per instruction: the complex product is stacked along K, A = [Cr(8 spins) | Ci(8 spins)],
 //     B = [[Wr, Wi], [-Wi, Wr]], so ONE instruction covers 8 spins completely (two with TF32: K = 8).
-//   * Every value is split into two FP16 pieces x s = hi + lo / 2^11 (hi = fp16(x s), lo = fp16((x s - hi) 2^11): 22
-//     significant bits, what hi + lo TF32 pieces carry), and hi x [B hi | B lo] is one instruction of N = 4 NC with the
-//     two B tiles side by side along N; lo x B hi is the second.  2 instructions per 8 spins and 128 samples (TF32: 4).
+//   * Every value is split into two FP16 pieces x s = hi + lo (hi = fp16(x s), lo = fp16(x s - hi): 22 significant
+//     bits, what hi + lo TF32 pieces carry), and hi x [B hi | B lo] is one instruction of N = 4 NC with the two B tiles
+//     side by side along N; lo x B hi is the second.  2 instructions per 8 spins and 128 samples (TF32: 4).
 //   * FP16 has 5 exponent bits: both operands are scaled by powers of two taken from measured maxima (coil_scales_kernel:
-//     the largest |M| a spin can reach, max(M0, |M(0)|), and the largest weight component), so that the largest piece
-//     sits at 2^13..2^14; pieces below 6e-8 of that underflow, which is 2^-37 of the largest contribution.  The hi x hi
-//     products land in accumulator columns [0, 2 NC), the two cross products (scaled by 2^11) in [2 NC, 4 NC); the
-//     epilogue returns (hh + 2^-11 mix) / (s_A s_B).  lo x lo (2^-22 relative) is dropped, as in 3xTF32.
+//     the largest |M| a spin can reach, max(M0, |M(0)|), and the largest weight component), so that the largest value
+//     sits in [2^13, 2^14).  A piece is then exact to max(2^-11 of itself, 3e-8) -- the FP16 subnormal spacing, 2^-38 of
+//     the largest value --, so lo needs no scale of its own: it goes subnormal only for values below 2^-17 of the
+//     largest, where the absolute error stays at 3e-8.  hi x hi lands in accumulator columns [0, 2 NC), the cross
+//     products in [2 NC, 4 NC); the epilogue returns (hh + mix) / (s_A s_B).  lo x lo (2^-22 relative) is dropped, as
+//     in 3xTF32.
 // B operand layout (no swizzle, K-major): 8-row x 16-byte core matrices (8 halves per row), contiguous 128 B each;
 //     byte offset of element (row n, k) = (n / 8) * 256 + (k / 8) * 128 + (n % 8) * 16 + (k % 8) * 2,  rows [B hi | B lo]
 // A operand in TMEM: row m = lane m, K = 16 halves = 8 consecutive 32-bit columns (k = 2 j in the low half of column j);
-// a stage (16 spins) = 2 groups x [hi (8 columns) | lo (8 columns)] = 32 columns, four stages deep, after the 128
-// accumulator columns (4 NC <= 128: up to 32 coils per pass take the wide instruction).
+// a stage (16 spins) = 2 groups x [hi (8 columns) | lo (8 columns)] = 32 columns, after the 4 NC accumulator columns
+// (up to 32 coils per pass take the wide instruction), as many stages as the CTA's 256 columns hold (at most 7).
 #pragma once
 #include <cuda_fp16.h>
 
@@ -29,10 +31,10 @@ namespace bloch {
 
 constexpr int kScalMMax = 6;          // scal[]: bound on |M| of any spin (float bits), coil_scales_kernel
 constexpr int kScalWMax = 7;          // scal[]: largest |re|, |im| of a coil weight
-constexpr int kHAStages = 4;
 constexpr int kHAStageCols = kTcGroups * 16;   // per 8-spin group: hi (8 columns) | lo (8 columns)
-constexpr int kHDCols = 128;
-static_assert(kHDCols + kHAStages * kHAStageCols <= kTcCols, "TMEM columns");
+// TMEM (256 columns per CTA, two CTAs per SM): 4 NC accumulator columns, the rest A stages: 7 / 6 / 4 for 8 / 16 / 32 coils
+__host__ __device__ constexpr int h_dcols(int nc) { return 4 * nc; }
+__host__ __device__ constexpr int h_astages(int nc) { return (kTcCols - 4 * nc) / kHAStageCols < 7 ? (kTcCols - 4 * nc) / kHAStageCols : 7; }
 constexpr int kHSlots = 8;
 __host__ __device__ constexpr int h_btile(int nc) { return 4 * nc * 32; }   // per 8-spin group: 4 NC rows x 16 halves
 __host__ __device__ constexpr int h_slot(int nc) { return kTcStageSpins * 32 + kTcGroups * h_btile(nc); }
@@ -74,7 +76,7 @@ coil_scales_kernel(int n, const float4 *__restrict__ Cc, const float4 *__restric
 
 __device__ __forceinline__ void h_split(float x, __half &hi, __half &lo) {
     hi = __float2half_rn(x);
-    lo = __float2half_rn((x - __half2float(hi)) * 2048.0f);
+    lo = __float2half_rn(x - __half2float(hi));
 }
 
 // Weights -> B tiles.  Bt[pass][group][4 NC rows x 16 halves], group = spin / 8 over the spins padded to a multiple of 16.
@@ -130,7 +132,8 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
                       float2 *__restrict__ partial /* [NC][chunks][n_pts] */) {
     constexpr int kBTile = h_btile(NC), kSlotBytes = h_slot(NC);
     constexpr uint32_t kIdescW = h_idesc(4 * NC), kIdescN = h_idesc(2 * NC);
-    static_assert(4 * NC <= kHDCols, "accumulator columns");
+    constexpr int kHDCols = h_dcols(NC), kHAStages = h_astages(NC);
+    static_assert(kHDCols + kHAStages * kHAStageCols <= kTcCols && kHAStages >= 2, "TMEM columns");
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *slots = smem;                                    // [kHSlots][spin A (256 B) | spin S (256 B) | B tiles]
     uint64_t *full = reinterpret_cast<uint64_t *>(slots + kHSlots * kSlotBytes);    // [kHSlots] TMA landed
@@ -191,8 +194,8 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
                 for (int gq = 0; gq < kTcGroups; ++gq) {
                     const uint32_t ag = a0 + gq * 16, bg = b0 + gq * kBTile;  // A parts: columns +0 hi, +8 lo
                     const uint32_t first = (st == 0 && gq == 0) ? 0u : 1u;
-                    h_mma_ts(tmem, ag + 0, tc_desc(bg), kIdescW, first);          // hi x [B hi | B lo] -> [hh | hl 2^11]
-                    h_mma_ts(tmem + 2 * NC, ag + 8, tc_desc(bg), kIdescN, 1u);    // lo x B hi          ->      [lh 2^11]
+                    h_mma_ts(tmem, ag + 0, tc_desc(bg), kIdescW, first);          // hi x [B hi | B lo] -> [hh | hl]
+                    h_mma_ts(tmem + 2 * NC, ag + 8, tc_desc(bg), kIdescN, 1u);    // lo x B hi          ->      [lh]
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mma_done[ab])) : "memory");
                 if (st + kHSlots - 1 < n_stages) {  // the slot of stage st + kHSlots - 1 held stage st - 1
@@ -214,6 +217,7 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
         }
         const float kx = r.x, ky = r.y, kz = r.z, tau = r.w;
         const float sA = h_scale(scal[kScalMMax]);
+        const float lsA = (float)((int)((__float_as_uint(sA) >> 23) & 0xffu) - 127);  // log2 s_A, folded into the decay's exponent
         for (int st = set; st < n_stages; st += kTcGenWarps / 4) {
             const int ab = st % kHAStages, sl = st % kHSlots;
             if (st >= kHAStages) {  // the MMAs that read this A stage kHAStages stages ago are complete
@@ -237,15 +241,15 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
                         const float4 sv = spS[sp];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
                         const float th = fmaf(kx, a.x, fmaf(ky, a.y, fmaf(kz, a.z, tau * a.w)));  // radians
                         const float sn = __sinf(th), cs = __cosf(th);
-                        const float e = ex2_approx(tau * sv.w) * sA;
+                        const float e = ex2_approx(fmaf(tau, sv.w, lsA));  // s_A exp(-tau / T2)
                         const float er = sv.x * e, ei = sv.y * e;
                         cr[h] = fmaf(er, cs, -ei * sn);
                         ci[h] = fmaf(er, sn, ei * cs);
                     }
                     const __half2 hr = __floats2half2_rn(cr[0], cr[1]), hi_ = __floats2half2_rn(ci[0], ci[1]);
                     const float2 fr = __half22float2(hr), fi = __half22float2(hi_);
-                    const __half2 lr = __floats2half2_rn((cr[0] - fr.x) * 2048.0f, (cr[1] - fr.y) * 2048.0f);
-                    const __half2 li = __floats2half2_rn((ci[0] - fi.x) * 2048.0f, (ci[1] - fi.y) * 2048.0f);
+                    const __half2 lr = __floats2half2_rn(cr[0] - fr.x, cr[1] - fr.y);
+                    const __half2 li = __floats2half2_rn(ci[0] - fi.x, ci[1] - fi.y);
                     v[16 * gq + m] = *reinterpret_cast<const uint32_t *>(&hr);
                     v[16 * gq + 4 + m] = *reinterpret_cast<const uint32_t *>(&hi_);
                     v[16 * gq + 8 + m] = *reinterpret_cast<const uint32_t *>(&lr);
@@ -280,7 +284,7 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                     for (int c = 0; c < 16; ++c)
-                        acc[c0 + c] = fmaf(__uint_as_float(mx[c]), 1.0f / 2048.0f, __uint_as_float(hh[c])) * inv;
+                        acc[c0 + c] = (__uint_as_float(hh[c]) + __uint_as_float(mx[c])) * inv;
                 }
             }
             const int pp = blockIdx.x * kTcM + row;
