@@ -319,7 +319,27 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
                                "P samples (issue-bound, not MUFU-bound)")
         kern["signal"]["coils"] = n_coils
         k_sig = bloch.bloch_plan_last_kernel(plan.handle, "signal")
-        if n_coils > 0 and k_sig["name"].startswith("signal_coils_tc_kernel"):
+        if n_coils > 0 and k_sig["name"].startswith("signal_coils_h_kernel"):
+            # tcgen05 kernel with FP16 operands (two pieces per value, FP32 accumulation): the receive sum is a dense
+            # contraction [samples x spins] x [spins x coils], complex: algorithmic 8 real flops per (spin, ADC sample,
+            # coil); the kernel executes 3x that.  Peak for FP16 = the measured dense bf16 peak (same rate).
+            dur = kinds_ms["signal"] * 1e-3 / steps
+            flops = 8.0 * n_coils * n_eval_sig
+            peaks = load_peaks()
+            h_peak = float(peaks.get("bf16_tflops") or 2250.0 * 0.75) * 1e12
+            e = kern["signal"]
+            e.update({"bound": "tensor", "pipe": "f16", "achieved": flops / dur / 1e12, "peak": h_peak / 1e12,
+                      "unit": "TFLOP/s", "frac": flops / dur / h_peak,
+                      "algorithmic_ops_per_launch": flops * steps / kinds_n["signal"],
+                      "peak_source": "MEASURED_PEAKS.json bf16_tflops (FP16 runs at the bf16 rate)" if peaks.get("bf16_tflops")
+                                     else "fallback: 0.75 x 2250 nominal bf16 TFLOP/s",
+                      "note": f"{n_coils} coils on tcgen05 (kind::f16, A operand generated into tensor memory, operands split "
+                              "into two FP16 pieces scaled from measured maxima): algorithmic 8 flops per (spin, ADC sample, "
+                              "coil); 2 MMAs of M128 x N x K16 per 8 spins.  The kernel is bound by GENERATING the A operand "
+                              "(sin / cos / ex2 + the split: ~27 instructions per (spin, sample), issue slots 70 %), not by the "
+                              "tensor pipe: see issue_util"})
+            e.update(capture_fields(k_sig, "tf32"))
+        elif n_coils > 0 and k_sig["name"].startswith("signal_coils_tc_kernel"):
             # tcgen05 kernel: the receive sum is a dense contraction [samples x spins] x [spins x coils], complex:
             # algorithmic 8 real flops per (spin, ADC sample, coil); the kernel executes 3x that (3xTF32).  Peak for
             # TF32 = the measured dense bf16 peak x the nominal 1/2 ratio (B200_PROFILING.md).

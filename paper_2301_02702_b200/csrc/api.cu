@@ -281,7 +281,7 @@ SeqShape seq_shape(const bloch_plan *plan, int64_t n_spins, int sm_count, int n_
     q.use = plan->path == BLOCH_PATH_FUSED || (4 * inf.n_rf_steps >= inf.n_adc && (ps || full_layout));
     // Coils under AUTO: the 8-wide sums cost ~50 issue slots per evaluation on the FMA pipe, so once a block holds
     // enough (spin, sample) pairs to fill the tcgen05 kernel the per-block launches win.  Measured, fused / per-block
-    // ms: config 5 x 8 coils (6.7e7 pairs per block) 205.2 / 198.7; config 2 x 8 coils (1.0e6) 2.22 / 3.36; up to 4
+    // ms: config 5 x 8 coils (6.7e7 pairs per block) 205.2 / 186.6; config 2 x 8 coils (1.0e6) 2.22 / 3.36; up to 4
     // coils the launch wins on both (config 5 x 4: 162.6 / 206.8; config 2 x 4: 2.13 / 3.19).
     if (q.nc == 8 && plan->path != BLOCH_PATH_FUSED && plan->opt[BLOCH_OPT_COIL_TC] != 0 &&
         n_spins * inf.max_block_adc >= (int64_t(1) << 24))
