@@ -273,7 +273,7 @@ int bloch_plan_last_kernel(const bloch_plan *plan, int kind, char *name, size_t 
  * Everything else as bloch_simulate (same integration, same final magnetisation).  The plan must be BLOCH_OUT_SUM_ALL
  * (else BLOCH_EINVAL); 1 <= n_coils <= 4096.  Moving spins: bloch_simulate_coils_motion (motion plans; velocities /
  * amplitudes as bloch_simulate_motion, all three NULL = none).  The coil-independent part of every evaluation (phase,
- * sin / cos / exp) is computed once per 4 or 8 coils; with more than 4 coils (fp32 phase) the sum over spins runs on the
+ * sin / cos / exp) is computed once per pass of coils; with fp32 phase and static spins the sum over spins runs on the
  * tensor cores (tcgen05 with the generated operand in tensor memory, two FP16 pieces per value with FP32 accumulation
  * -- 22 significant bits, as 3xTF32 --, 8, 16 or 32 coils per pass).  Plans that
  * take the whole-sequence kernel (BLOCH_PATH_FUSED, or AUTO where it qualifies: static spins, fp32 phase) sum up to 8
@@ -337,9 +337,10 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *                                 32 / 64 / 128 forces it
  *   BLOCH_OPT_RF_SPINS            spins per thread of the excitation kernel: 0 (default) the library's choice, 1 or 2
  *   BLOCH_OPT_COIL_TC             multi-coil receive: tensor cores (tcgen05, A operand in tensor memory) whenever
- *                                 they apply (more than 4 coils, fp32 phase, static spins): -1 (default) and 2 with
- *                                 FP16 operand pieces scaled from measured maxima (2 instructions per 8 spins), 1 with
- *                                 3xTF32 (4 instructions); 0: never (the FFMA kernel)
+ *                                 they apply (fp32 phase, static spins): -1 (default) and 2 with FP16 operand
+ *                                 pieces scaled from measured maxima (2 instructions per 8 spins; any number of coils
+ *                                 from 4096 spins on), 1 with 3xTF32 (4 instructions; more than 4 coils); 0: never
+ *                                 (the FFMA kernel)
  *   BLOCH_OPT_SEQ_SIG_EXTRA       whole-sequence kernel: signal warps added per missing RF warp of a sub-partition,
  *                                 0..7; -1 (default): 2, or 0 with receive coils
  *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic

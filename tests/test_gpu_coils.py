@@ -124,9 +124,10 @@ def test_host_buffer_coil_entry_is_identical_to_the_device_entry(B):
 @pytest.mark.parametrize("tc", [1, 2])
 @pytest.mark.parametrize("name,n_coils", [("1", 5), ("4", 8), ("5", 11), ("2", 20), ("4", 37)])
 def test_tensor_core_coil_kernel_matches_oracle(B, oracle_mod, name, n_coils, tc):
-    """The tcgen05 / TMEM kernel (csrc/coils_tc.cuh; opt-in with bloch_plan_set_option(BLOCH_OPT_COIL_TC, 1)): contributions generated on the fly
-    as the A operand, 3xTF32 products, accumulators in TMEM.  Same acceptance as every other path; ragged sample
-    tiles (n_adc not a multiple of 128), ragged 16-spin stages, 8, 16 and 32 coils per pass and two passes (37 coils) are all in these cases."""
+    """The tcgen05 / TMEM kernels (option coil_tc: 1 = csrc/coils_tc.cuh with 3xTF32 products, 2 = csrc/coils_h.cuh with FP16
+    operand pieces, the default): contributions generated on the fly as the A operand in tensor memory, accumulators in
+    TMEM.  Same acceptance as every other path; ragged sample tiles (n_adc not a multiple of 128), ragged 16-spin
+    stages, 8, 16 and 32 coils per pass and two passes (37 coils) are all in these cases."""
     w = W.small(name)
     coils = coil_maps(w.phantom, n_coils, seed=10 + n_coils)
     ref, rxy, rz = oracle_mod.simulate(w.phantom, w.seq, coils=coils.astype(np.complex128), return_state=True)
