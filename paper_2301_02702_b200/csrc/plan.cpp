@@ -166,47 +166,52 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                  ext_mps = extent(params->max_speed_mps, 1.0);
 
     // ------------------------------------------------------------------ a1: merged grid
-    std::vector<double> pts;
-    pts.reserve(size_t(2 + seq->g_n[0] + seq->g_n[1] + seq->g_n[2] + 2 * seq->rf_n + seq->adc_n));
-    // every source is ascending on its own (validated above), so the union is a merge of sorted runs, not a sort
-    // (config 5: 5.1e6 points; std::sort took half of the planning time)
-    pts.push_back(0.0);
-    pts.push_back(seq->t_end);
-    auto merge_run = [&pts](size_t run_first) {
-        std::inplace_merge(pts.begin(), pts.begin() + (std::ptrdiff_t)run_first, pts.end());
+    // Every source is ascending on its own (validated above), so the union is a merge of sorted runs, not a sort
+    // (config 5: 5.1e6 points; std::sort took half of the planning time), and the merge writes the clamped, de-duplicated
+    // grid directly: small runs (end points, gradient vertices, waveform vertices) are merged into one first, then ONE
+    // three-way pass over (small runs, RF sample edges, ADC times).
+    std::vector<double> small_pts;
+    small_pts.reserve(size_t(2 + seq->g_n[0] + seq->g_n[1] + seq->g_n[2]) + (waveform ? size_t(params->motion_n) : 0));
+    small_pts.push_back(0.0);
+    small_pts.push_back(seq->t_end);
+    auto merge_small = [&small_pts](size_t run_first) {
+        std::inplace_merge(small_pts.begin(), small_pts.begin() + (std::ptrdiff_t)run_first, small_pts.end());
     };
     for (int a = 0; a < 3; ++a) {
-        const size_t first = pts.size();
-        pts.insert(pts.end(), seq->g_t[a], seq->g_t[a] + seq->g_n[a]);
-        merge_run(first);
-    }
-    {
-        const size_t first = pts.size();
-        for (int64_t i = 0; i < seq->rf_n; ++i) {
-            pts.push_back(seq->rf_t[i]);
-            pts.push_back(seq->rf_t[i] + seq->rf_dt[i]);
-        }
-        // rf_t[i] + rf_dt[i] may exceed rf_t[i + 1] by rounding when samples abut: insertion pass over the run
-        for (size_t k = first + 1; k < pts.size(); ++k)
-            for (size_t m = k; m > first && pts[m] < pts[m - 1]; --m) std::swap(pts[m], pts[m - 1]);
-        merge_run(first);
-    }
-    {
-        const size_t first = pts.size();
-        pts.insert(pts.end(), seq->adc_t, seq->adc_t + seq->adc_n);
-        merge_run(first);
+        const size_t first = small_pts.size();
+        small_pts.insert(small_pts.end(), seq->g_t[a], seq->g_t[a] + seq->g_n[a]);
+        merge_small(first);
     }
     if (waveform) {  // the vertices of the motion waveform that lie inside the sequence are points of the grid
-        const size_t first = pts.size();
+        const size_t first = small_pts.size();
         for (int64_t i = 0; i < params->motion_n; ++i)
-            if (params->motion_t[i] >= 0.0 && params->motion_t[i] <= seq->t_end) pts.push_back(params->motion_t[i]);
-        merge_run(first);
+            if (params->motion_t[i] >= 0.0 && params->motion_t[i] <= seq->t_end) small_pts.push_back(params->motion_t[i]);
+        merge_small(first);
     }
+    std::vector<double> rf_pts(size_t(2 * seq->rf_n));
+    for (int64_t i = 0; i < seq->rf_n; ++i) {
+        rf_pts[2 * i] = seq->rf_t[i];
+        rf_pts[2 * i + 1] = seq->rf_t[i] + seq->rf_dt[i];
+    }
+    // rf_t[i] + rf_dt[i] may exceed rf_t[i + 1] by rounding when samples abut: insertion pass over the run
+    for (size_t k = 1; k < rf_pts.size(); ++k)
+        for (size_t m = k; m > 0 && rf_pts[m] < rf_pts[m - 1]; --m) std::swap(rf_pts[m], rf_pts[m - 1]);
     std::vector<double> coarse;
-    coarse.reserve(pts.size());
-    for (double t : pts) {
-        t = std::min(std::max(t, 0.0), seq->t_end);
-        if (coarse.empty() || t - coarse.back() > kTimeTol) coarse.push_back(t);
+    coarse.reserve(small_pts.size() + rf_pts.size() + size_t(seq->adc_n));
+    {
+        const double *pa = small_pts.data(), *ea = pa + small_pts.size();
+        const double *pb = rf_pts.data(), *eb = pb + rf_pts.size();
+        const double *pc = seq->adc_t, *ec = pc + seq->adc_n;
+        const double inf = std::numeric_limits<double>::infinity();
+        while (pa < ea || pb < eb || pc < ec) {
+            const double va = pa < ea ? *pa : inf, vb = pb < eb ? *pb : inf, vc = pc < ec ? *pc : inf;
+            double t;
+            if (va <= vb && va <= vc) { t = va; ++pa; }
+            else if (vb <= vc) { t = vb; ++pb; }
+            else { t = vc; ++pc; }
+            t = std::min(std::max(t, 0.0), seq->t_end);
+            if (coarse.empty() || t - coarse.back() > kTimeTol) coarse.push_back(t);
+        }
     }
     // RF coverage of the coarse intervals (sweep), then refinement of RF-active ones
     std::vector<double> t;          // refined points
