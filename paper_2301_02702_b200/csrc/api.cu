@@ -372,6 +372,7 @@ struct Workspace {
     float2 *partial;
     size_t partial_elems;
     float2 *W;       // multi-coil receive only: weights repacked as [pass][spin][4]
+    float4 *Sp;      // FP16 tensor-core coil kernel only: block-start states in polar form
     size_t bytes;
 };
 
@@ -413,6 +414,7 @@ Workspace carve(const bloch_plan *plan, int64_t n_spins, void *base, int sm_coun
     const size_t w_bytes = tc_ws ? n_pass * (n_pad / 8) * tc_bgroup(ncp)
                                                                        : n_pass * size_t(n_spins) * ncp * sizeof(float2);
     w.W = n_coils > 0 ? (float2 *)take(w_bytes) : nullptr;
+    w.Sp = (tc_ws && coil_tc_fp16(plan)) ? (float4 *)take(size_t(n_spins) * sizeof(float4)) : nullptr;
     w.bytes = off;
     return w;
 }
@@ -967,16 +969,20 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
                     else note_kernel(plan, BLOCH_KIND_SIGNAL, (int64_t)grid.x * grid.y, s.threads, "signal_coils_kernel<%d, %d, %d, %d>",
                                      s.P == 2 ? 2 : 1, ncp == 8 ? 8 : 4, ph64 ? 1 : 0, mo ? 1 : 0);
                     if (tc_h) {
+                        if (pass == 0) {  // this block's start states in polar form, once for all passes
+                            coil_polar_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, w.S, w.Sp);
+                            ++launches;
+                        }
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * h_btile(ncp);
                         if (ncp == 32)
                             signal_coils_h_kernel<32><<<grid, kTcThreads, h_smem(32), stream>>>(
-                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                                (const float4 *)recs, n_pts, w.A, w.Sp, Bp, n, s.spins_per_chunk, w.scal, w.partial);
                         else if (ncp == 16)
                             signal_coils_h_kernel<16><<<grid, kTcThreads, h_smem(16), stream>>>(
-                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                                (const float4 *)recs, n_pts, w.A, w.Sp, Bp, n, s.spins_per_chunk, w.scal, w.partial);
                         else
                             signal_coils_h_kernel<8><<<grid, kTcThreads, h_smem(8), stream>>>(
-                                (const float4 *)recs, n_pts, w.A, w.S, Bp, n, s.spins_per_chunk, w.scal, w.partial);
+                                (const float4 *)recs, n_pts, w.A, w.Sp, Bp, n, s.spins_per_chunk, w.scal, w.partial);
                     } else if (tc) {
                         const unsigned char *Bp = (const unsigned char *)w.W + (size_t)pass * (n_pad / 8) * tc_bgroup(ncp);
                         if (ncp == 32)

@@ -74,6 +74,17 @@ coil_scales_kernel(int n, const float4 *__restrict__ Cc, const float4 *__restric
     }
 }
 
+// Block-start state in polar form for the generators: (|Mxy|, arg Mxy, Mz, e2).  A contribution is then
+// |Mxy| e^{-tau/T2} (cos, sin)(theta + arg Mxy): the argument rides in the phase's FMA chain for free and the complex
+// rotation (6 instructions per (spin, sample)) becomes 3 multiplies.  One small launch per block.
+__global__ void __launch_bounds__(256)
+coil_polar_kernel(int n, const float4 *__restrict__ S, float4 *__restrict__ Sp) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 s = S[i];
+    Sp[i] = make_float4(hypotf(s.x, s.y), atan2f(s.y, s.x), s.z, s.w);
+}
+
 __device__ __forceinline__ void h_split(float x, __half &hi, __half &lo) {
     hi = __float2half_rn(x);
     lo = __float2half_rn(x - __half2float(hi));
@@ -127,7 +138,8 @@ __device__ __forceinline__ void h_mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint6
 template <int NC>
 __global__ void __launch_bounds__(kTcThreads, 2)
 signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *__restrict__ A,
-                      const float4 *__restrict__ S, const unsigned char *__restrict__ Bt /* this pass */,
+                      const float4 *__restrict__ S /* polar states, coil_polar_kernel */,
+                      const unsigned char *__restrict__ Bt /* this pass */,
                       int n_spins, int spins_per_chunk /* multiple of 16 */, const unsigned *__restrict__ scal,
                       float2 *__restrict__ partial /* [NC][chunks][n_pts] */) {
     constexpr int kBTile = h_btile(NC), kSlotBytes = h_slot(NC);
@@ -238,13 +250,12 @@ signal_coils_h_kernel(const float4 *__restrict__ recs, int n_pts, const float4 *
                     for (int h = 0; h < 2; ++h) {
                         const int sp = 8 * gq + 2 * m + h;
                         const float4 a = spA[sp];
-                        const float4 sv = spS[sp];  // (Mxy.re, Mxy.im, Mz, e2 = -log2(e)/T2)
-                        const float th = fmaf(kx, a.x, fmaf(ky, a.y, fmaf(kz, a.z, tau * a.w)));  // radians
+                        const float4 sv = spS[sp];  // polar: (|Mxy|, arg Mxy, Mz, e2 = -log2(e)/T2)
+                        const float th = fmaf(kx, a.x, fmaf(ky, a.y, fmaf(kz, a.z, fmaf(tau, a.w, sv.y))));  // radians
                         const float sn = __sinf(th), cs = __cosf(th);
-                        const float e = ex2_approx(fmaf(tau, sv.w, lsA));  // s_A exp(-tau / T2)
-                        const float er = sv.x * e, ei = sv.y * e;
-                        cr[h] = fmaf(er, cs, -ei * sn);
-                        ci[h] = fmaf(er, sn, ei * cs);
+                        const float me = sv.x * ex2_approx(fmaf(tau, sv.w, lsA));  // s_A |Mxy| exp(-tau / T2)
+                        cr[h] = me * cs;
+                        ci[h] = me * sn;
                     }
                     const __half2 hr = __floats2half2_rn(cr[0], cr[1]), hi_ = __floats2half2_rn(ci[0], ci[1]);
                     const float2 fr = __half22float2(hr), fi = __half22float2(hi_);
