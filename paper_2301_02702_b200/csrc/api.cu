@@ -298,7 +298,7 @@ bool coil_use_tc(const bloch_plan *plan, int64_t n_spins, int n_coils) {
     //     93-107 ms) and beats the FFMA kernel from its first pass of 8 (121 ms); up to 4 coils the 4-wide FFMA kernel
     //     (93 ms) stays;
     //   -1 (default) / 2 (FP16 kernel, coils_h.cuh): any number of coils once there are 4096 spins -- a pass of up to 8
-    //     coils takes 80.9 ms on config 4, less than the 4-wide FFMA kernel's 93.2 for 1 to 4 coils.
+    //     coils takes 76.9 ms on config 4, less than the 4-wide FFMA kernel's 93.2 for 1 to 4 coils.
     const int mode = plan->opt[BLOCH_OPT_COIL_TC];
     if (mode == 0 || n_coils < 1 || plan->info.phase_mode != BLOCH_PHASE_FP32 || plan->info.motion_mode != BLOCH_MOTION_NONE)
         return false;
@@ -314,8 +314,8 @@ bool coil_use_fused(const bloch_plan *plan, int64_t n_spins, int sm_count, int n
 }
 
 // which tensor-core kernel: FP16 operands (coils_h.cuh, 2 instructions per 8 spins) or 3xTF32 (coils_tc.cuh, 4)
-// Measured on config 4 (signal kernels, per simulation): 8 coils 93.2 -> 85.3 ms, 16 coils 94.2 -> 86.3, 32 coils
-// 106.4 -> 87.6; rounded (not truncated) operand pieces: errors against the oracle 2-3x smaller.  -1 (default) and 2:
+// Measured on config 4 (signal kernels, per simulation): 8 coils 93.2 -> 76.9 ms, 16 coils 94.2 -> 74.1, 32 coils
+// 106.4 -> 71.3; rounded (not truncated) operand pieces: errors against the oracle 2-3x smaller.  -1 (default) and 2:
 // FP16; 1: 3xTF32.
 bool coil_tc_fp16(const bloch_plan *plan) { return plan->opt[BLOCH_OPT_COIL_TC] != 1; }
 
