@@ -54,7 +54,7 @@ class bloch_plan_info(C.Structure):
 
 # BLOCH_OPT_* keys of bloch_plan_set_option, in enum order
 OPTIONS = ("signal_lin", "signal_p", "signal_fixed_cta", "signal_ctas_per_sm", "rf_threads", "rf_spins", "coil_tc",
-           "seq_sig_extra", "seq_sig_base", "seq_items_x4")
+           "seq_sig_extra", "seq_sig_base", "seq_items_x4", "rf_const")
 STATUS_BAD_RELAXATION, STATUS_NONFINITE, STATUS_PHASE_RANGE = 1, 2, 4
 
 EXPORTS = ["bloch_version", "bloch_strerror", "bloch_last_error", "bloch_plan_create", "bloch_plan_destroy",

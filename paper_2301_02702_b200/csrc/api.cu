@@ -627,6 +627,7 @@ int bloch_plan_set_option(bloch_plan *plan, int key, int value) {
         case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_SIG_BASE: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_ITEMS_X4: ok = value >= 0 && value <= 64; break;
+        case BLOCH_OPT_RF_CONST: ok = value == 0 || value == 1; break;
         default: return fail(BLOCH_EINVAL, "unknown BLOCH_OPT_* key");
     }
     if (!ok) return fail(BLOCH_EINVAL, "option value out of range");
@@ -906,6 +907,18 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         const Block &b = plan->blocks[bi];
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
+            if (b.rf_const_count > 0 && plan->opt[BLOCH_OPT_RF_CONST] != 0 && !mo && !rf_pair) {
+                // the block's step records by value, as kernel parameters (plan.cpp): rf_const_kernel, bitwise rf_kernel
+                for (int64_t c = 0; c < b.rf_const_count; ++c) {
+                    if (c > 0 && (rc = taps.mark(BLOCH_KIND_RF))) return rc;
+                    rf_const_kernel<<<rf_grid, rf_threads, 0, stream>>>(plan->rf_const[size_t(b.rf_const_first + c)], prop,
+                                                                        (c == 0 && pending) ? 1 : 0, w.A, w.C, w.S, n);
+                    ++launches;
+                }
+                note_kernel(plan, BLOCH_KIND_RF, rf_grid, rf_threads, "rf_const_kernel");
+                pending = false;
+                continue;
+            }
             if ((rc = launch_rf(plan->d_tables + b.table_off, (int)b.n_tiles, pending ? 1 : 0))) return rc;
             ++launches;
             pending = false;

@@ -54,6 +54,22 @@ struct RfTileHdr {
 };
 static_assert(sizeof(RfTileHdr) == kRfHdrBytes, "RfTileHdr must be 64 B");
 
+// A run of compact (uniform-gradient) RF tiles passed to rf_const_kernel BY VALUE as a kernel parameter: the step
+// records then sit in the constant bank and reach the FMAs as uniform operands (no shared-memory staging, no barrier,
+// fewer register-file reads per step).  <= 32,764 B of parameters per launch: 2048 steps + 24 tile headers = 25 KB.
+constexpr int kRfConstSteps = 2048;
+constexpr int kRfConstTiles = 24;
+struct RfConstTile {
+    int32_t n_steps;
+    float dt, gx, gy, gz, wxy2_max;  // as RfTileHdr (uniform-gradient tiles: g*_max = |g*|)
+};
+struct RfConstArgs {
+    int32_t n_tiles, n_steps, pad0, pad1;
+    RfConstTile tile[kRfConstTiles];
+    float rec[kRfConstSteps][3];     // (wx, wy, wx^2 + wy^2) per step, tile after tile
+};
+static_assert(sizeof(RfConstArgs) <= 26 * 1024, "kernel parameter budget");
+
 // One block of the time axis: a maximal run of RF-active intervals (excitation regime) or
 // a run of RF-free intervals (precession regime), :132.
 struct Block {
@@ -65,6 +81,7 @@ struct Block {
     int64_t table_off = 0;    // byte offset of this block's records in the table buffer
     int64_t lin_pts = 0;      // precession: leading samples (a multiple of 16) that signal_lin_kernel may serve, see plan.cpp
     int64_t n_tiles = 0;      // RF: tiles in the block's table (see RfTileHdr)
+    int64_t rf_const_first = 0, rf_const_count = 0;  // RF: its chunks in bloch_plan::rf_const (0: not served by rf_const_kernel)
     // precession block end record: k' = -gamma_bar * K(T) [turns/m] and tau = T [s] (Eq 12-13)
     double kend[3] = {0, 0, 0};
     double tau_end = 0;
@@ -114,12 +131,13 @@ struct bloch_plan {
     bloch_plan_info info{};
     std::vector<bloch::Block> blocks;
     std::vector<unsigned char> tables;   // host staging copy of the device tables
+    std::vector<bloch::RfConstArgs> rf_const;   // static plans: the compact RF tiles again, as kernel-parameter blocks (rf_const_kernel)
     const unsigned char *d_tables = nullptr;
     int64_t prog_off = 0;                // byte offset of the SeqOp program in the table buffer
     int64_t n_adc_blocks = 0;            // precession blocks that serve ADC samples
     int64_t adcblk_off = 0;              // byte offset of the SeqAdcBlock array in the table buffer
     int path = 0;                        // BLOCH_PATH_*
-    int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, -1, -1, 0};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
+    int opt[BLOCH_N_OPTIONS] = {1, 0, 0, 4, 0, 0, -1, -1, -1, 0, 1};  // BLOCH_OPT_* defaults (bloch_plan_set_option)
     // phase-range bookkeeping (bloch_sim_params extents): largest |k'| [turns/m], tau [s] and |mu'| [turns s/m] of
     // any evaluated point (block ends included), and the largest phase within the declared extents
     double k_max = 0, tau_max = 0, m_max = 0, worst_turns = 0;

@@ -495,6 +495,45 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
         if (img.size() > (size_t)INT32_MAX) a4_bad.store(1);
     });
     if (a4_bad.load()) return fail(BLOCH_EINVAL, "RF block table exceeds 2 GiB");
+    // Static plans: excitation blocks whose tiles are all compact (gradient constant within the tile) and that fit ONE
+    // kernel-parameter block (<= kRfConstSteps steps, <= kRfConstTiles tiles, internal.h) are packed once more for
+    // rf_const_kernel.  Longer blocks keep rf_kernel: cutting them into several launches would round the hi + lo
+    // state to one float at every cut, and the result would no longer be bitwise that of the other paths.
+    plan->rf_const.clear();
+    if (!motion) {
+        for (size_t bi = 0; bi < blocks.size(); ++bi) {
+            Block &b = blocks[bi];
+            if (b.type != kBlockRF) continue;
+            const unsigned char *tb = rf_img[bi].data();
+            const int32_t *dir = reinterpret_cast<const int32_t *>(tb);
+            bool compact = b.n_tiles > 0 && b.n_tiles <= kRfConstTiles && b.count <= kRfConstSteps;
+            for (int64_t t = 0; t < b.n_tiles && compact; ++t) {
+                RfTileHdr hd;
+                std::memcpy(&hd, tb + dir[2 * t], sizeof hd);
+                compact = (hd.flags & kRfFlagUniformG) && !(hd.flags & kRfFlagMotion) && hd.n_steps <= kRfConstSteps;
+            }
+            if (!compact) continue;
+            b.rf_const_first = (int64_t)plan->rf_const.size();
+            RfConstArgs cur;
+            std::memset(&cur, 0, sizeof cur);
+            for (int64_t t = 0; t < b.n_tiles; ++t) {
+                RfTileHdr hd;
+                std::memcpy(&hd, tb + dir[2 * t], sizeof hd);
+                if (cur.n_tiles == kRfConstTiles || cur.n_steps + hd.n_steps > kRfConstSteps) {
+                    plan->rf_const.push_back(cur);
+                    std::memset(&cur, 0, sizeof cur);
+                }
+                RfConstTile &ct = cur.tile[cur.n_tiles++];
+                ct.n_steps = hd.n_steps; ct.dt = hd.dt; ct.gx = hd.gx; ct.gy = hd.gy; ct.gz = hd.gz;
+                ct.wxy2_max = hd.wxy2_max;
+                for (int32_t k = 0; k < hd.n_steps; ++k)  // (wx, wy, wx^2 + wy^2) of the 16-byte compact record
+                    std::memcpy(&cur.rec[cur.n_steps + k][0], tb + dir[2 * t] + kRfHdrBytes + size_t(k) * 16, 12);
+                cur.n_steps += hd.n_steps;
+            }
+            plan->rf_const.push_back(cur);
+            b.rf_const_count = (int64_t)plan->rf_const.size() - b.rf_const_first;
+        }
+    }
 
     // ------------------------------------------------------------------ tables: layout + fill
     size_t off = 0;
@@ -604,7 +643,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
     {
         bool pending = false;
         for (const Block &b : blocks) {
-            if (b.type == kBlockRF) { ++launches; pending = false; continue; }
+            if (b.type == kBlockRF) { launches += std::max<int64_t>(1, b.rf_const_count); pending = false; continue; }
             if (pending) ++launches;
             if (b.adc_count > 0) launches += (params->output_mode == BLOCH_OUT_SUM_ALL) ? 2 : 1;
             if (params->output_mode == BLOCH_OUT_SUM_ALL && b.lin_pts > 0 && b.lin_pts < b.adc_count) ++launches;  // tail

@@ -319,6 +319,92 @@ rf_kernel(const unsigned char *__restrict__ tbl, int n_tiles, PropRec prop, int 
     if (active) S[i] = make_float4(hx + lx, hy + ly, hz + lz, s.w);
 }
 
+// One compact tile whose step records come from the kernel's parameter space (constant bank): the arithmetic of
+// rf_tile<TIER, 0>, operation for operation, so the result is bitwise that of rf_kernel.
+template <int TIER>
+__device__ __forceinline__ void rf_ctile(const RfConstArgs &args, int base, const RfConstTile &hd, const RfSpin &sp,
+                                         const RfRelax &rx, float &hx, float &hy, float &hz, float &lx, float &ly,
+                                         float &lz) {
+    const int n = hd.n_steps;
+    const float dtdw = hd.dt * sp.dw;
+    const float wz_u = fmaf(hd.gx, sp.x, fmaf(hd.gy, sp.y, fmaf(hd.gz, sp.z, dtdw)));
+    const float wz2_u = __fmul_rn(wz_u, wz_u);
+#define BLOCH_RFC_LOAD(k)                                                               \
+    const float wx = args.rec[base + (k)][0], wy = args.rec[base + (k)][1], wz = wz_u,    \
+                q = __fadd_rn(args.rec[base + (k)][2], wz2_u);
+    if (TIER <= 0) {
+        int k = 0;
+        constexpr int kFold = rf_fold(TIER);
+        for (; k + kFold <= n; k += kFold) {
+            const int b0 = base + k;  // one uniform address per trip; the unrolled steps are immediates from it
+#pragma unroll
+            for (int j = 0; j < kFold; ++j) {
+                const float wx = args.rec[b0 + j][0], wy = args.rec[b0 + j][1], wz = wz_u,
+                            q = __fadd_rn(args.rec[b0 + j][2], wz2_u);
+                rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
+            }
+            fold(hx, lx); fold(hy, ly); fold(hz, lz);
+        }
+        for (; k < n; ++k) {
+            BLOCH_RFC_LOAD(k)
+            rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
+        }
+        fold(hx, lx); fold(hy, ly); fold(hz, lz);
+    } else {
+        float cx = -lx, cy = -ly, cz = -lz;
+#pragma unroll 4
+        for (int k = 0; k < n; ++k) {
+            BLOCH_RFC_LOAD(k)
+            float tx, ty, tz;
+            rf_increment<TIER>(wx, wy, wz, q, hx, hy, hz, rx, tx, ty, tz);
+            kahan_add(hx, cx, tx);
+            kahan_add(hy, cy, ty);
+            kahan_add(hz, cz, tz);
+        }
+        lx = -cx; ly = -cy; lz = -cz;
+    }
+#undef BLOCH_RFC_LOAD
+}
+
+__global__ void __launch_bounds__(kRfMaxThreads)
+rf_const_kernel(const __grid_constant__ RfConstArgs args, PropRec prop, int has_prop, const float4 *__restrict__ A,
+                const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = i < n;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = make_float4(1.f, 1.f, 0.f, 0.f), s = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (active) {
+        a = A[i];
+        c = Cc[i];
+        s = S[i];
+    }
+    float hx = s.x, hy = s.y, hz = s.z;
+    if (has_prop) propagate(prop, a, c, v, hx, hy, hz);
+    float lx = 0.f, ly = 0.f, lz = 0.f;
+    const RfSpin sp{a.x, a.y, a.z, c.w, c.x, c.y, c.z, 0.f, 0.f, 0.f};
+    const float ax = fabsf(sp.x), ay = fabsf(sp.y), az = fabsf(sp.z), adw = fabsf(sp.dw);
+    int base = 0;
+    for (int t = 0; t < args.n_tiles; ++t) {
+        const RfConstTile hd = args.tile[t];
+        RfRelax rx;
+        rx.D1 = -expm1f(-hd.dt * sp.r1);
+        rx.D2 = -expm1f(-hd.dt * sp.r2);
+        rx.E1 = 1.0f - rx.D1;
+        rx.E2 = 1.0f - rx.D2;
+        rx.D1m0 = rx.D1 * sp.m0;
+        const float wzb = fmaf(fabsf(hd.gx), ax, fmaf(fabsf(hd.gy), ay, fmaf(fabsf(hd.gz), az, hd.dt * adw)));
+        const float qb = fmaf(wzb, wzb, hd.wxy2_max);
+        const int tier = __all_sync(0xffffffffu, qb <= kRfQLin) ? -1
+                         : (__all_sync(0xffffffffu, qb <= 0.00390625f) ? 0 : (__all_sync(0xffffffffu, qb <= 0.25f) ? 1 : 2));
+        if (tier == -1) rf_ctile<-1>(args, base, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        else if (tier == 0) rf_ctile<0>(args, base, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        else if (tier == 1) rf_ctile<1>(args, base, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        else rf_ctile<2>(args, base, hd, sp, rx, hx, hy, hz, lx, ly, lz);
+        base += hd.n_steps;
+    }
+    if (active) S[i] = make_float4(hx + lx, hy + ly, hz + lz, s.w);
+}
+
 // Two spins per thread (static plans; BLOCH_OPT_RF_SPINS): thread t owns spins t and t + ceil(n / 2).  Tiles whose
 // bound on q leaves tier 0 (never with the configs' pulses) fall back to rf_tile one spin after the other.
 __global__ void __launch_bounds__(kRfMaxThreads)

@@ -366,3 +366,52 @@ def test_adc_samples_during_an_rf_pulse(B, oracle_mod, path):
     assert emax <= 1e-4 and nrmse <= 1e-5
     emax, nrmse = errors(np.concatenate([gxy, gz.astype(np.complex128)]), np.concatenate([rxy, rz.astype(np.complex128)]))
     assert emax <= 1e-4 and nrmse <= 1e-5
+
+
+@pytest.mark.parametrize("name", ["1", "2", "4", "5"])
+def test_rf_const_kernel_is_bitwise_the_tile_kernel(B, oracle_mod, name):
+    """rf_const_kernel (BLOCH_OPT_RF_CONST, the default for static plans whose RF tiles are compact): the step records
+    are passed by value as kernel parameters and reach the FMAs as uniform operands; the arithmetic is rf_kernel's,
+    operation for operation, so signal and final magnetisation are bitwise equal (and match the oracle)."""
+    from test_gpu_parity import run_gpu
+    w = W.small(name)
+    out = {c: run_gpu(B, w, want_state=True, path="per_block", phase_mode="fp32", options={"rf_const": c}) for c in (0, 1)}
+    for a, b in zip(out[0], out[1]):
+        assert np.array_equal(np.asarray(a).view(np.float32), np.asarray(b).view(np.float32))
+    ref = oracle_mod.simulate(w.phantom, w.seq, output_mode=w.output_mode)
+    emax, nrmse = errors(out[1][0], ref)
+    assert emax <= 1e-4 and nrmse <= 1e-5
+
+
+def test_rf_const_kernel_limits_and_fallback(B, oracle_mod):
+    """A 2000-step pulse on a slice-select plateau is 16 compact tiles = one parameter block: rf_const_kernel.  A
+    5000-step pulse does not fit one block (2048 steps) and a pulse that runs over the gradient ramps has general
+    (32-B) records: both keep rf_kernel.  All against the oracle, and bitwise against the tile kernel."""
+    import torch
+    g_plateau = {2: ([1e-4, 2e-4, 5.4e-3, 5.5e-3, 5.9e-3, 6.0e-3], [0, 6e-3, 6e-3, 0, -7e-3, 0]),
+                 0: ([6.1e-3, 6.2e-3, 7.2e-3, 7.3e-3], [0, 5e-3, 5e-3, 0])}
+    g_ramps = {2: ([1e-4, 2.5e-3, 5.4e-3, 5.5e-3, 5.9e-3, 6.0e-3], [0, 6e-3, 2e-3, 0, -7e-3, 0]), 0: g_plateau[0]}
+    adc = 6.2e-3 + (np.arange(200) + 0.5) * 4e-6
+    ph = rand_phantom(1111, 42, zmax=0.004)
+    for n_rf, g, kernel in ((2000, g_plateau, "rf_const_kernel"), (5000, g_plateau, "rf_kernel<0>"),
+                            (2000, g_ramps, "rf_kernel<0>")):
+        rf = sinc_rf(3e-4, n_rf * 1e-6, n_rf, np.deg2rad(60))
+        s = seq(g=g, rf=rf, adc=adc, t_end=8e-3, dt_rf_max=1e-6)
+        ref = oracle_mod.simulate(ph, s)
+        res = {}
+        for c in (1, 0):
+            plan = B.Plan(s, path="per_block", phase_mode="fp32", options={"rf_const": c})
+            Mxy = torch.zeros(ph.n, 2, device="cuda")
+            Mz = torch.zeros(ph.n, device="cuda")
+            sig = plan.simulate(*B.phantom_to_device(ph), Mxy=Mxy, Mz=Mz)
+            torch.cuda.synchronize()
+            res[c] = (sig.cpu().numpy(), Mxy.cpu().numpy(), Mz.cpu().numpy())
+            name = B.bloch_plan_last_kernel(plan.handle, "rf")["name"]
+            assert name == (kernel if c else "rf_kernel<0>"), (n_rf, name)
+            assert B.bloch_plan_last_launches(plan.handle) == plan.info["n_launches"]
+            plan.close()
+        for a, b in zip(res[0], res[1]):
+            assert np.array_equal(a.view(np.float32), b.view(np.float32))
+        emax, nrmse = errors(res[1][0], ref)
+        print(f"{n_rf}-step pulse ({kernel}): max {emax:.3e} nrmse {nrmse:.3e}")
+        assert emax <= TOL_MAX and nrmse <= TOL_NRMSE

@@ -190,7 +190,7 @@ def test_plan_options_are_plan_state_not_environment(B):
         info = B.bloch_plan_get_info(h)
         assert info["options"] == {"signal_lin": 1, "signal_p": 0, "signal_fixed_cta": 0, "signal_ctas_per_sm": 4,
                                    "rf_threads": 0, "rf_spins": 0, "coil_tc": -1, "seq_sig_extra": -1,
-                                   "seq_sig_base": -1, "seq_items_x4": 0}
+                                   "seq_sig_base": -1, "seq_items_x4": 0, "rf_const": 1}
         B.bloch_plan_set_option(h, "signal_lin", 0)
         B.bloch_plan_set_option(h, B.OPTIONS.index("signal_p"), 4)
         assert B.bloch_plan_get_option(h, "signal_lin") == 0 and B.bloch_plan_get_option(h, "signal_p") == 4
