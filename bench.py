@@ -368,7 +368,8 @@ def kernel_rooflines(bloch, plan, w, n, info, kinds_ms, kinds_n, steps, sm_max, 
     if kinds_n["rf"]:
         kern["rf"] = entry("rf", "fp32", FP32_PER_RF_STEP * rf_steps,
                            "algorithmic count = 46 FP32 instructions per spin*step (Eq 6-9 + 11 written directly); the "
-                           "small-angle loop (q <= 2^-14: every pulse of the configs) issues 31 FP + ~4 other per step, so frac can pass 1")
+                           "small-angle loop (q <= 2^-14: every pulse of the configs) issues 31 FP + ~4-6 other per step (rf_const_kernel: "
+                           "step records as kernel parameters, uniform operands), so frac can pass 1")
     if kinds_n["fused"]:
         # whole-sequence kernel: excitation and readout share the SM, so both algorithmic counts land on one launch;
         # the binding pipe is the one whose count / peak is larger (FP32 on every config that takes this path)
