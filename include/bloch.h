@@ -346,11 +346,11 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *   BLOCH_OPT_SEQ_SIG_BASE        whole-sequence kernel: signal warps per sub-partition, 0..7; -1 (default) automatic
  *   BLOCH_OPT_SEQ_ITEMS_X4        whole-sequence kernel: readout items per signal warp x 4 that the item size must
  *                                 leave; 0 (default) always the largest item
- *   BLOCH_OPT_RF_CONST            1 (default): excitation blocks of static plans whose gradient is constant within
- *                                 every tile take rf_const_kernel -- the step records passed by value as kernel
- *                                 parameters (constant bank, uniform operands; blocks of up to 2048 steps in up to
- *                                 24 tiles, longer ones keep the tile kernel); 0: always the shared-memory tile
- *                                 kernel.  Bitwise the same result either way. */
+ *   BLOCH_OPT_RF_CONST            1 (default): from 16,384 spins on, excitation blocks of static plans whose gradient
+ *                                 is constant within every tile take rf_const_kernel -- the step records passed by
+ *                                 value as kernel parameters (constant bank, uniform operands; blocks of up to 2048
+ *                                 steps in up to 24 tiles, longer ones keep the tile kernel); 2: for any number of
+ *                                 spins; 0: always the shared-memory tile kernel.  Bitwise the same result. */
 enum { BLOCH_OPT_SIGNAL_LIN = 0, BLOCH_OPT_SIGNAL_P = 1, BLOCH_OPT_SIGNAL_FIXED_CTA = 2,
        BLOCH_OPT_SIGNAL_CTAS_PER_SM = 3, BLOCH_OPT_RF_THREADS = 4, BLOCH_OPT_RF_SPINS = 5, BLOCH_OPT_COIL_TC = 6,
        BLOCH_OPT_SEQ_SIG_EXTRA = 7, BLOCH_OPT_SEQ_SIG_BASE = 8, BLOCH_OPT_SEQ_ITEMS_X4 = 9, BLOCH_OPT_RF_CONST = 10,

@@ -627,7 +627,7 @@ int bloch_plan_set_option(bloch_plan *plan, int key, int value) {
         case BLOCH_OPT_SEQ_SIG_EXTRA: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_SIG_BASE: ok = value >= -1 && value <= 7; break;
         case BLOCH_OPT_SEQ_ITEMS_X4: ok = value >= 0 && value <= 64; break;
-        case BLOCH_OPT_RF_CONST: ok = value == 0 || value == 1; break;
+        case BLOCH_OPT_RF_CONST: ok = value >= 0 && value <= 2; break;
         default: return fail(BLOCH_EINVAL, "unknown BLOCH_OPT_* key");
     }
     if (!ok) return fail(BLOCH_EINVAL, "option value out of range");
@@ -907,7 +907,9 @@ int simulate_impl(const bloch_plan *plan, int64_t n_spins, const float *d_x, con
         const Block &b = plan->blocks[bi];
         if (b.type == kBlockRF) {
             if ((rc = taps.mark(BLOCH_KIND_RF))) return rc;
-            if (b.rf_const_count > 0 && plan->opt[BLOCH_OPT_RF_CONST] != 0 && !mo && !rf_pair) {
+            // (from 16,384 spins on: below that the launch is latency-bound and the 25 KB of parameters cost 2-3 us)
+            if (b.rf_const_count > 0 && !mo && !rf_pair &&
+                (plan->opt[BLOCH_OPT_RF_CONST] == 2 || (plan->opt[BLOCH_OPT_RF_CONST] == 1 && n >= 16384))) {
                 // the block's step records by value, as kernel parameters (plan.cpp): rf_const_kernel, bitwise rf_kernel
                 for (int64_t c = 0; c < b.rf_const_count; ++c) {
                     if (c > 0 && (rc = taps.mark(BLOCH_KIND_RF))) return rc;

@@ -375,11 +375,11 @@ def test_rf_const_kernel_is_bitwise_the_tile_kernel(B, oracle_mod, name):
     operation for operation, so signal and final magnetisation are bitwise equal (and match the oracle)."""
     from test_gpu_parity import run_gpu
     w = W.small(name)
-    out = {c: run_gpu(B, w, want_state=True, path="per_block", phase_mode="fp32", options={"rf_const": c}) for c in (0, 1)}
-    for a, b in zip(out[0], out[1]):
+    out = {c: run_gpu(B, w, want_state=True, path="per_block", phase_mode="fp32", options={"rf_const": c}) for c in (0, 2)}
+    for a, b in zip(out[0], out[2]):
         assert np.array_equal(np.asarray(a).view(np.float32), np.asarray(b).view(np.float32))
     ref = oracle_mod.simulate(w.phantom, w.seq, output_mode=w.output_mode)
-    emax, nrmse = errors(out[1][0], ref)
+    emax, nrmse = errors(out[2][0], ref)
     assert emax <= 1e-4 and nrmse <= 1e-5
 
 
@@ -399,7 +399,7 @@ def test_rf_const_kernel_limits_and_fallback(B, oracle_mod):
         s = seq(g=g, rf=rf, adc=adc, t_end=8e-3, dt_rf_max=1e-6)
         ref = oracle_mod.simulate(ph, s)
         res = {}
-        for c in (1, 0):
+        for c in (2, 0):   # 2: rf_const_kernel where it applies whatever the number of spins (1: from 16,384 spins on)
             plan = B.Plan(s, path="per_block", phase_mode="fp32", options={"rf_const": c})
             Mxy = torch.zeros(ph.n, 2, device="cuda")
             Mz = torch.zeros(ph.n, device="cuda")
@@ -410,8 +410,13 @@ def test_rf_const_kernel_limits_and_fallback(B, oracle_mod):
             assert name == (kernel if c else "rf_kernel<0>"), (n_rf, name)
             assert B.bloch_plan_last_launches(plan.handle) == plan.info["n_launches"]
             plan.close()
-        for a, b in zip(res[0], res[1]):
+        for a, b in zip(res[0], res[2]):
             assert np.array_equal(a.view(np.float32), b.view(np.float32))
-        emax, nrmse = errors(res[1][0], ref)
+        emax, nrmse = errors(res[2][0], ref)
         print(f"{n_rf}-step pulse ({kernel}): max {emax:.3e} nrmse {nrmse:.3e}")
         assert emax <= TOL_MAX and nrmse <= TOL_NRMSE
+    plan = B.Plan(s, path="per_block", phase_mode="fp32")          # default (1): 1111 spins are below the threshold
+    plan.simulate(*B.phantom_to_device(ph))
+    torch.cuda.synchronize()
+    assert B.bloch_plan_last_kernel(plan.handle, "rf")["name"] == "rf_kernel<0>"
+    plan.close()
