@@ -348,7 +348,7 @@ int bloch_plan_set_path(bloch_plan *plan, int path);
  *                                 leave; 0 (default) always the largest item
  *   BLOCH_OPT_RF_CONST            1 (default): from 16,384 spins on, excitation blocks of static plans whose gradient
  *                                 is constant within every tile take rf_const_kernel -- the step records passed by
- *                                 value as kernel parameters (constant bank, uniform operands; blocks of up to 2048
+ *                                 value as kernel parameters (constant bank, uniform operands; blocks of up to 2000
  *                                 steps in up to 24 tiles, longer ones keep the tile kernel); 2: for any number of
  *                                 spins; 0: always the shared-memory tile kernel.  Bitwise the same result. */
 enum { BLOCH_OPT_SIGNAL_LIN = 0, BLOCH_OPT_SIGNAL_P = 1, BLOCH_OPT_SIGNAL_FIXED_CTA = 2,

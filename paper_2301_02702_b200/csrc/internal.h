@@ -56,8 +56,8 @@ static_assert(sizeof(RfTileHdr) == kRfHdrBytes, "RfTileHdr must be 64 B");
 
 // A run of compact (uniform-gradient) RF tiles passed to rf_const_kernel BY VALUE as a kernel parameter: the step
 // records then sit in the constant bank and reach the FMAs as uniform operands (no shared-memory staging, no barrier,
-// fewer register-file reads per step).  <= 32,764 B of parameters per launch: 2048 steps + 24 tile headers = 25 KB.
-constexpr int kRfConstSteps = 2048;
+// fewer register-file reads per step).  <= 32,764 B of parameters per launch: 2000 steps of 16 B + 24 tile headers = 32,592 B.
+constexpr int kRfConstSteps = 2000;
 constexpr int kRfConstTiles = 24;
 struct RfConstTile {
     int32_t n_steps;
@@ -66,9 +66,9 @@ struct RfConstTile {
 struct RfConstArgs {
     int32_t n_tiles, n_steps, pad0, pad1;
     RfConstTile tile[kRfConstTiles];
-    float rec[kRfConstSteps][3];     // (wx, wy, wx^2 + wy^2) per step, tile after tile
+    float rec[kRfConstSteps * 4];    // (wx, wy, wx^2 + wy^2, 0) per step, tile after tile: the 16-byte compact records
 };
-static_assert(sizeof(RfConstArgs) <= 26 * 1024, "kernel parameter budget");
+static_assert(sizeof(RfConstArgs) <= 32764 - 160, "kernel parameter budget: 32,764 B with the other arguments");
 
 // One block of the time axis: a maximal run of RF-active intervals (excitation regime) or
 // a run of RF-free intervals (precession regime), :132.

@@ -526,8 +526,7 @@ int build_plan(const bloch_scanner *scanner, const bloch_sequence *seq, const bl
                 RfConstTile &ct = cur.tile[cur.n_tiles++];
                 ct.n_steps = hd.n_steps; ct.dt = hd.dt; ct.gx = hd.gx; ct.gy = hd.gy; ct.gz = hd.gz;
                 ct.wxy2_max = hd.wxy2_max;
-                for (int32_t k = 0; k < hd.n_steps; ++k)  // (wx, wy, wx^2 + wy^2) of the 16-byte compact record
-                    std::memcpy(&cur.rec[cur.n_steps + k][0], tb + dir[2 * t] + kRfHdrBytes + size_t(k) * 16, 12);
+                std::memcpy(&cur.rec[4 * cur.n_steps], tb + dir[2 * t] + kRfHdrBytes, size_t(hd.n_steps) * 16);  // compact records
                 cur.n_steps += hd.n_steps;
             }
             plan->rf_const.push_back(cur);

@@ -329,18 +329,18 @@ __device__ __forceinline__ void rf_ctile(const RfConstArgs &args, int base, cons
     const float dtdw = hd.dt * sp.dw;
     const float wz_u = fmaf(hd.gx, sp.x, fmaf(hd.gy, sp.y, fmaf(hd.gz, sp.z, dtdw)));
     const float wz2_u = __fmul_rn(wz_u, wz_u);
-#define BLOCH_RFC_LOAD(k)                                                               \
-    const float wx = args.rec[base + (k)][0], wy = args.rec[base + (k)][1], wz = wz_u,    \
-                q = __fadd_rn(args.rec[base + (k)][2], wz2_u);
+#define BLOCH_RFC_LOAD(k)                                                                         \
+    const float wx = args.rec[4 * (base + (k))], wy = args.rec[4 * (base + (k)) + 1], wz = wz_u,    \
+                q = __fadd_rn(args.rec[4 * (base + (k)) + 2], wz2_u);
     if (TIER <= 0) {
         int k = 0;
         constexpr int kFold = rf_fold(TIER);
         for (; k + kFold <= n; k += kFold) {
-            const int b0 = base + k;  // one uniform address per trip; the unrolled steps are immediates from it
+            const int o = 4 * (base + k);  // one uniform offset per trip; the unrolled steps are immediates from it
 #pragma unroll
             for (int j = 0; j < kFold; ++j) {
-                const float wx = args.rec[b0 + j][0], wy = args.rec[b0 + j][1], wz = wz_u,
-                            q = __fadd_rn(args.rec[b0 + j][2], wz2_u);
+                const float wx = args.rec[o + 4 * j], wy = args.rec[o + 4 * j + 1], wz = wz_u,
+                            q = __fadd_rn(args.rec[o + 4 * j + 2], wz2_u);
                 rf_accumulate<TIER>(wx, wy, wz, q, hx + lx, hy + ly, hz + lz, rx, lx, ly, lz);
             }
             fold(hx, lx); fold(hy, ly); fold(hz, lz);

@@ -385,7 +385,7 @@ def test_rf_const_kernel_is_bitwise_the_tile_kernel(B, oracle_mod, name):
 
 def test_rf_const_kernel_limits_and_fallback(B, oracle_mod):
     """A 2000-step pulse on a slice-select plateau is 16 compact tiles = one parameter block: rf_const_kernel.  A
-    5000-step pulse does not fit one block (2048 steps) and a pulse that runs over the gradient ramps has general
+    5000-step pulse does not fit one block (2000 steps) and a pulse that runs over the gradient ramps has general
     (32-B) records: both keep rf_kernel.  All against the oracle, and bitwise against the tile kernel."""
     import torch
     g_plateau = {2: ([1e-4, 2e-4, 5.4e-3, 5.5e-3, 5.9e-3, 6.0e-3], [0, 6e-3, 6e-3, 0, -7e-3, 0]),
