@@ -10,11 +10,13 @@ from test_gpu_parity import B  # noqa: F401  (fixture)
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("name,path", [("1", "per_block"), ("2", "per_block"), ("5", "per_block"), ("5", "fused")])
-def test_simulate_is_graph_capturable_and_replays_bitwise(B, name, path):
+@pytest.mark.parametrize("name,path,options", [("1", "per_block", None), ("2", "per_block", None), ("5", "per_block", None),
+                                               ("5", "fused", None), ("4", "per_block", {"rf_const": 2})])
+def test_simulate_is_graph_capturable_and_replays_bitwise(B, name, path, options):
+    """(rf_const = 2: the excitation kernel whose step records are a 32 KB kernel parameter, captured by value)"""
     import torch
     w = W.small(name)
-    plan = B.Plan(w.seq, path=path, phase_mode="fp32")
+    plan = B.Plan(w.seq, path=path, phase_mode="fp32", options=options)
     dev = B.phantom_to_device(w.phantom)
     n = w.phantom.n
     sig = torch.zeros(plan.info["n_adc"], dtype=torch.complex64, device="cuda")
