@@ -366,7 +366,10 @@ __device__ __forceinline__ void rf_ctile(const RfConstArgs &args, int base, cons
 #undef BLOCH_RFC_LOAD
 }
 
-__global__ void __launch_bounds__(kRfMaxThreads)
+// (a minimum of 4 ... 8 CTAs per SM in the launch bounds: still 40 registers, but ptxas schedules the unrolled steps
+// differently and config 4's excitation goes 36.3 -> 34.8 ms; 10: 35.1; 14 or 16: 37.6.  The same hint makes rf_kernel
+// slower, 37.5 -> 38.3 ms.)
+__global__ void __launch_bounds__(kRfMaxThreads, 8)
 rf_const_kernel(const __grid_constant__ RfConstArgs args, PropRec prop, int has_prop, const float4 *__restrict__ A,
                 const float4 *__restrict__ Cc, float4 *__restrict__ S, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
