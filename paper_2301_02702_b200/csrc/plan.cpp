@@ -78,7 +78,10 @@ void parallel_for(size_t n, unsigned threads, F fn) {
         for (size_t i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
     };
     std::vector<std::thread> pool;
-    for (unsigned k = 1; k < threads; ++k) pool.emplace_back(work);
+    try {
+        for (unsigned k = 1; k < threads; ++k) pool.emplace_back(work);
+    } catch (...) {  // no more threads to be had: the ones that started, and this one, share the items
+    }
     work();
     for (std::thread &th : pool) th.join();
 }
